@@ -1,0 +1,171 @@
+/*
+ * routebalance.h -- C ABI of the B200-native RouteBalance per-batch scheduling decision.
+ *
+ * What the library computes (citations: P:Lnnn = line nnn of the paper text PAPER.md,
+ * "RouteBalance: Fused Model Routing and Load Balancing for Heterogeneous LLM Serving"):
+ *
+ *   estimate  (§4.2 "Model estimator"):  k-nearest labelled prompts of every query embedding in a
+ *             reference bank; distance-weighted per-model predicted quality Q^[r,m] and expected output
+ *             length L^[r,m].
+ *   latency   (§4.2 "Latency heads"):    T^[r,i] = T^tpot_i * (d_i/b_i + L^[r,m(i)]); the wait term
+ *             d_i/b_i is dropped when instance i has a free decode slot.
+ *   cost      (Eq. 2):                 C^[r,i] = l_r * c_in[m(i)] + L^[r,m(i)] * c_out[m(i)].
+ *   score     (Eq. 1):                 S[r,i] = w_qual*Q^ + w_cost*(1 - C^/max_j C^) + w_lat*(1 - T^/max_j T^).
+ *   dispatch  (§4.1, "Dead reckoning"): requests in LPT order (key max_m L^[r,m], longest
+ *             first); each takes argmax_i S[r,i]; the chosen instance's local decode state grows by L^
+ *             before the next request is scored.
+ *
+ * Every step runs in hand-written sm_100a CUDA kernels; there is no CPU fallback.  The exact operation
+ * order (one IEEE binary32 round-to-nearest operation per line, never fused) is stated in DESIGN.md
+ * "Canonical arithmetic"; readings of the paper where it is silent are listed in DESIGN.md "Readings".
+ *
+ * Conventions for every call
+ *   - Pointers marked [host|device] may be either; they are classified with cudaPointerGetAttributes.
+ *     Pointers marked [host] must be host memory.
+ *   - Input buffers are consumed before the call returns (host pointers) or in stream order on the
+ *     context's stream (device pointers).  The library never keeps a caller pointer.
+ *   - Outputs to host pointers are complete when the call returns; outputs to device pointers are complete
+ *     in stream order on the context's stream.
+ *   - All matrices are dense row-major.  Optional outputs may be NULL.
+ *   - On any non-RB_OK return nothing the caller can observe has changed, except rb_last_error().
+ *   - One context = one CUDA stream = one caller thread at a time.  Several contexts may coexist.
+ */
+#ifndef ROUTEBALANCE_H_
+#define ROUTEBALANCE_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct rb_ctx rb_ctx; /* opaque; owns all device memory it uses */
+
+typedef enum {
+  RB_OK = 0,
+  RB_EINVAL = 1,       /* bad argument (size, range, NULL, non-finite coefficient) */
+  RB_ECUDA = 2,        /* a CUDA runtime/driver call failed; see rb_last_error */
+  RB_ENOMEM = 3,       /* host or device allocation failed */
+  RB_ESTATE = 4,       /* call order violated (e.g. rb_decide before rb_set_instances) */
+  RB_EUNSUPPORTED = 5  /* valid request this build cannot serve (e.g. no sm_100 device) */
+} rb_status;
+
+typedef enum { RB_F32 = 0, RB_BF16 = 1 } rb_dtype;
+
+/* Per-tier latency head.  The paper's head is a gradient-boosted TPOT regressor per (model, GPU) tier
+ * (P:L119); its trained trees are not available, so the head is the linear stand-in of BASELINE.json:
+ *   tpot_i = decode_ms_per_tok * (1 + batch_slope * b_i)      [ms per output token]
+ *   T^[r,i] = prefill_ms_per_tok * l_r + tpot_i * (wait_i + L^[r,tier(i)])
+ * prefill_ms_per_tok = 0 recovers the paper's formula exactly. */
+typedef struct {
+  float prefill_ms_per_tok;
+  float decode_ms_per_tok;
+  float batch_slope;
+} rb_lat_head;
+
+typedef struct {
+  int32_t bank_dtype;     /* rb_dtype of bank_emb as passed to rb_create.                 default RB_F32  */
+  int32_t store_dtype;    /* rb_dtype the bank is stored and searched in.                 default RB_BF16 */
+                          /* RB_BF16: bank and queries are rounded to bf16 (RNE) once; similarity is the   */
+                          /* dot product of the rounded values (tcgen05 tensor-core scan).                 */
+                          /* RB_F32: fp32 bank, exact fp64-accumulated scan; meant for small banks.        */
+  int32_t weight_mode;    /* 0: inverse distance 1/(dist+eps) ("distance-weighted"); 1: uniform     */
+  float dist_eps;         /* eps above.                                                   default 1e-6    */
+  int32_t rerank_slack;   /* RB_BF16 only: the scan keeps k+slack candidates per query, their similarities */
+                          /* are recomputed exactly (fp64 accumulate) and the best k kept. default 6       */
+  int32_t lpt_enabled;    /* 1: dispatch in LPT order; 0: in input order.         default 1       */
+  int32_t update_enabled; /* 1: dead-reckoning update after each dispatch; 0: none. default 1    */
+  int32_t max_batch;      /* largest B any later call may pass (scratch sizing).          default 4096    */
+  int32_t use_graph;      /* 1: replay the decision as a captured CUDA graph.             default 1       */
+  void* stream;           /* cudaStream_t all work is ordered on; NULL = legacy default stream            */
+} rb_options;
+
+/* Fills *opt with the defaults listed above.  opt [host]. */
+void rb_options_default(rb_options* opt);
+
+/* Creates a context holding the reference bank (N labelled prompts, d-dim embeddings, per-model
+ * quality label in [0,1] and output length for each of M models).
+ *   bank_emb      [host|device] N x d, dtype opt->bank_dtype (fp32, or bf16 as raw uint16)
+ *   bank_quality  [host|device] N x M fp32
+ *   bank_outlen   [host|device] N x M fp32
+ *   k             neighbours per query, 1 <= k <= 64, k + rerank_slack <= 64, k <= N
+ *   d             must be a multiple of 8; M in [1,16]; N < 2^31
+ * The bank is copied (and converted to store_dtype); the caller may free its buffers on return.
+ * Errors: RB_EINVAL on bad sizes/NULL, RB_EUNSUPPORTED without an sm_100 device, RB_ENOMEM, RB_ECUDA. */
+rb_status rb_create(rb_ctx** out, const void* bank_emb, const float* bank_quality,
+                    const float* bank_outlen, int64_t N, int32_t d, int32_t M, int32_t k,
+                    const rb_options* opt /* NULL = defaults */);
+
+/* Defines the instance set I (fixed at runtime; Table 1) and resets the dead-reckoned
+ * state to (queued_tokens = 0, running = 0).
+ *   tier      [host] I entries in [0,M): model/tier served by instance i, m(i)
+ *   cap       [host] I entries >= 1: decode slots of instance i ("free decode slot" <=> running < cap)
+ *   price_in  [host] M entries >= 0: price per input token of tier m (any unit; only ratios matter)
+ *   price_out [host] M entries >= 0
+ *   heads     [host] M latency heads, coefficients finite and >= 0
+ *   1 <= I <= 1024.  May be called again at any time between decisions (tier loss). */
+rb_status rb_set_instances(rb_ctx* ctx, int32_t I, const int32_t* tier, const int32_t* cap,
+                           const float* price_in, const float* price_out, const rb_lat_head* heads);
+
+/* Seeds the dead-reckoned state from telemetry: queued_tokens[i] = pending decode tokens
+ * d_i >= 0 (finite), running[i] = decode batch size b_i >= 0.  Both [host|device], I entries. */
+rb_status rb_set_state(rb_ctx* ctx, const float* queued_tokens, const int32_t* running);
+
+/* Reads the current dead-reckoned state back.  Both [host|device], I entries; either may be NULL. */
+rb_status rb_get_state(rb_ctx* ctx, float* queued_tokens, int32_t* running);
+
+/* Dead reckoning between batches (BASELINE.json; the drain rule is this library's, reading 22):
+ * every instance with b_i > 0 drains d_i <- max(0, d_i - b_i * elapsed_ms / tpot_i); b_i <- 0 when d_i
+ * reaches 0.  elapsed_ms must be finite and >= 0. */
+rb_status rb_advance_state(rb_ctx* ctx, float elapsed_ms);
+
+/* One per-batch decision: estimate -> score -> LPT greedy dispatch, committing the dead-reckoned updates.
+ *   query_emb    [host|device] B x d fp32 prompt embeddings (unit norm expected, not enforced)
+ *   prompt_len   [host|device] B int32 input token counts l_r >= 0
+ *   w            [host] (w_qual, w_lat, w_cost), each >= 0, |sum - 1| <= 1e-5
+ *   assignment   [host|device] B int32: chosen instance per request (indexed like the input batch)
+ *   scores       [host|device] B x I fp32 or NULL: row r = S[r,:] as seen when r was dispatched
+ *   pred_quality [host|device] B x M or NULL; pred_outlen likewise
+ *   nn_idx       [host|device] B x k int32 or NULL: neighbours, best first (similarity desc, index asc)
+ *   nn_sim       [host|device] B x k fp32 or NULL
+ * 1 <= B <= max_batch.  RB_ESTATE before rb_set_instances. */
+rb_status rb_decide(rb_ctx* ctx, const float* query_emb, const int32_t* prompt_len, int32_t B,
+                    const float w[3], int32_t* assignment, float* scores, float* pred_quality,
+                    float* pred_outlen, int32_t* nn_idx, float* nn_sim);
+
+/* The score + dispatch stages alone, from caller-supplied predictions (quality, outlen: B x M fp32,
+ * [host|device]).  commit = 0 leaves the dead-reckoned state untouched (weight sweeps from one state).
+ *   scores0 [host|device] B x I or NULL: S[r,:] of every request evaluated from the batch-start state
+ *   order   [host|device] B int32 or NULL: dispatch order (order[j] = request dispatched j-th) */
+rb_status rb_decide_from_predictions(rb_ctx* ctx, const float* quality, const float* outlen,
+                                     const int32_t* prompt_len, int32_t B, const float w[3],
+                                     int32_t commit, int32_t* assignment, float* scores,
+                                     float* scores0, int32_t* order);
+
+/* The estimate stage alone (KNN scan + merge + aggregate); outputs as in rb_decide, any may be NULL. */
+rb_status rb_estimate(rb_ctx* ctx, const float* query_emb, int32_t B, float* pred_quality,
+                      float* pred_outlen, int32_t* nn_idx, float* nn_sim);
+
+/* Device time of the stages of the most recent rb_decide / rb_estimate on this context, measured with
+ * CUDA events on the context's stream (only when the call ran with stage timing enabled through
+ * rb_set_stage_timing(ctx, 1), which also disables graph replay for that context).
+ *   us [host] 6 floats: stage (query staging), scan, merge, aggregate, score, dispatch. */
+rb_status rb_set_stage_timing(rb_ctx* ctx, int32_t enabled);
+rb_status rb_last_stage_us(rb_ctx* ctx, float us[6]);
+
+/* Number of kernel launches (graph nodes count individually) issued by this context so far. */
+int64_t rb_launch_count(const rb_ctx* ctx);
+
+/* Blocks until all work issued on the context's stream has finished. */
+rb_status rb_sync(rb_ctx* ctx);
+
+/* Human-readable description of the last failure on ctx ("" if none).  Valid until the next call. */
+const char* rb_last_error(const rb_ctx* ctx);
+
+/* Frees everything the context owns.  NULL is allowed. */
+void rb_destroy(rb_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ROUTEBALANCE_H_ */

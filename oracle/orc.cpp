@@ -1,0 +1,289 @@
+// orc.cpp -- ORACLE.  Test infrastructure, not product code.
+//
+// A plain, slow, obviously-correct CPU statement of RouteBalance's per-batch scheduling decision, written
+// from the paper text alone (P:Lnnn = line nnn of PAPER.md).  Only tests/, __graft_entry__.smoke() and
+// bench.py's cpu_baseline / --impl reference legs may load this file.  It shares no code, header, table or
+// helper with the CUDA library under paper_2606_17949_b200/, and neither includes the other.
+//
+// The method is a heuristic pipeline (approximate predictor + greedy assignment), so apart from the
+// neighbour search -- which is the brute-force definition of "k nearest" -- the oracle follows the
+// algorithm step by step, in the paper's order.  Every fp32 line below is ONE IEEE-754 binary32
+// round-to-nearest-even operation (build with -ffp-contract=off, no -ffast-math), because the LPT
+// assignment must be reproducible bit for bit.  Readings of points where the paper is silent are numbered
+// as in DESIGN.md "Readings".
+//
+// Pins (tests/test_oracle_*.py, all "-m 'not gpu'"): hand-worked examples W0/W1/W2 (tests/golden/),
+// the 6x-cheaper closed form of P:L90, simplex corners, k=N -> bank mean, k=1 -> nearest row's labels,
+// scikit-learn KNeighborsRegressor(weights='distance', algorithm='brute'), single-instance cluster,
+// LPT ordering invariant, exhaustive assignment on tiny inputs, price/latency scale invariance,
+// tier-loss == masking, advance closed form.  Parity unpinned: none of the functions below; the paper's
+// end-to-end outcomes (tier shares, DeepEval quality) need its dataset and cluster and are not computed here.
+//
+// C ABI, host pointers only, stateless: every function maps input arrays to output arrays.
+
+#include <algorithm>
+#include <cmath>
+#include <cstdint>
+#include <cstring>
+#include <numeric>
+#include <vector>
+
+namespace {
+
+// bfloat16 = upper 16 bits of binary32.  Round-to-nearest-even from binary32 (reading 4: the storage
+// precision of bank and queries is part of the definition).
+inline uint16_t f32_to_bf16_rne(float f) {
+  uint32_t u;
+  std::memcpy(&u, &f, 4);
+  if ((u & 0x7fffffffu) > 0x7f800000u) return (uint16_t)((u >> 16) | 0x0040u);  // NaN stays NaN
+  uint32_t lsb = (u >> 16) & 1u;
+  u += 0x7fffu + lsb;
+  return (uint16_t)(u >> 16);
+}
+inline float bf16_to_f32(uint16_t h) {
+  uint32_t u = (uint32_t)h << 16;
+  float f;
+  std::memcpy(&f, &u, 4);
+  return f;
+}
+
+// Value of element (row n, column c) of a matrix held as fp32 (dtype 0) or raw bf16 (dtype 1), after
+// rounding to the storage dtype `store` (0 = keep fp32, 1 = bf16).
+inline double stored_value(const void* base, int dtype, int store, int64_t off) {
+  if (dtype == 1) return (double)bf16_to_f32(((const uint16_t*)base)[off]);
+  float f = ((const float*)base)[off];
+  if (store == 1) f = bf16_to_f32(f32_to_bf16_rne(f));
+  return (double)f;
+}
+
+}  // namespace
+
+extern "C" {
+
+// Rounds n fp32 values to bf16 (RNE); out receives the raw 16-bit patterns.
+int orc_round_bf16(const float* in, uint16_t* out, int64_t n) {
+  for (int64_t i = 0; i < n; ++i) out[i] = f32_to_bf16_rne(in[i]);
+  return 0;
+}
+
+// Step 1-3 ("queries a distance-weighted FAISS KNN index (k=10)"; reading 1: exact inner-product
+// search over the stored vectors; reading 3: equal similarities -> smaller bank index first).
+//   s[r,n] = fl32( sum_{c=0}^{d-1} (double)x~[r,c] * (double)e~[n,c] ), summed in index order in fp64.
+//   nn[r][0..k-1] = the k rows with the largest s, ordered by (s descending, n ascending).
+// bank: N x d in bank_dtype (0 fp32 / 1 raw bf16); query: B x d fp32; both rounded to store_dtype first.
+int orc_knn(const void* bank, int bank_dtype, int store_dtype, const float* query, int64_t N, int d,
+            int B, int k, int32_t* nn_idx, float* nn_sim) {
+  if (k < 1 || k > N) return 1;
+  std::vector<double> x(d);
+  std::vector<float> s(N);
+  std::vector<int32_t> ord(N);
+  for (int r = 0; r < B; ++r) {
+    for (int c = 0; c < d; ++c) x[c] = stored_value(query, 0, store_dtype, (int64_t)r * d + c);
+#pragma omp parallel for schedule(static)
+    for (int64_t n = 0; n < N; ++n) {
+      double acc = 0.0;
+      for (int c = 0; c < d; ++c) acc += x[c] * stored_value(bank, bank_dtype, store_dtype, n * d + c);
+      s[n] = (float)acc;
+    }
+    std::iota(ord.begin(), ord.end(), 0);
+    std::partial_sort(ord.begin(), ord.begin() + k, ord.end(), [&](int32_t a, int32_t b) {
+      if (s[a] != s[b]) return s[a] > s[b];
+      return a < b;
+    });
+    for (int j = 0; j < k; ++j) {
+      nn_idx[(int64_t)r * k + j] = ord[j];
+      nn_sim[(int64_t)r * k + j] = s[ord[j]];
+    }
+  }
+  return 0;
+}
+
+// Step 4-5 ("distance-weighted"; "one lookup returns a predicted quality and expected length for
+// every candidate").  Reading 2: dist = sqrt(max(0, 2 - 2 s)) (Euclidean distance of unit vectors),
+// w = 1/(dist + eps); weight_mode 1 = uniform.  Reading 8: L^ uses the same weights as Q^.
+int orc_aggregate(const int32_t* nn_idx, const float* nn_sim, const float* bank_quality,
+                  const float* bank_outlen, int B, int k, int M, int weight_mode, float eps,
+                  float* pred_quality, float* pred_outlen) {
+  std::vector<float> w(k);
+  for (int r = 0; r < B; ++r) {
+    for (int j = 0; j < k; ++j) {
+      if (weight_mode == 1) {
+        w[j] = 1.0f;
+      } else {
+        float t = 2.0f * nn_sim[(int64_t)r * k + j];
+        float u = 2.0f - t;
+        u = std::max(u, 0.0f);
+        float dist = std::sqrt(u);
+        float den = dist + eps;
+        w[j] = 1.0f / den;
+      }
+    }
+    for (int m = 0; m < M; ++m) {
+      float numq = 0.0f, numl = 0.0f, den = 0.0f;
+      for (int j = 0; j < k; ++j) {
+        int64_t n = nn_idx[(int64_t)r * k + j];
+        float pq = w[j] * bank_quality[n * M + m];
+        numq = numq + pq;
+        float pl = w[j] * bank_outlen[n * M + m];
+        numl = numl + pl;
+        den = den + w[j];
+      }
+      pred_quality[(int64_t)r * M + m] = numq / den;
+      pred_outlen[(int64_t)r * M + m] = numl / den;
+    }
+  }
+  return 0;
+}
+
+// One row of Eq. 1 for request r against the state (dq, bq).
+//   P:L92-95 Eq. 2   C[r,m] = l_r * c_in[m] + L^[r,m] * c_out[m]
+//   P:L119           T[r,i] = tpot_i * (d_i/b_i + L^[r,m(i)]); "if the instance has a free decode slot only
+//                    the second term applies" (reading 11: free <=> b_i < cap_i); reading 9: linear head
+//                    tpot_i = dec*(1+slope*b_i); reading 10: plus a prefill term pre*l_r (pre = 0 -> paper).
+//   P:L82-90 Eq. 1   S = w_qual*Q^ + w_cost*(1 - C/max_j C) + w_lat*(1 - T/max_j T), maxima over the
+//                    request's candidates j (reading 13), a zero maximum makes the term 0 (reading 14);
+//                    summed in Eq. 1's order (reading 15): (w_q*Q + w_c*cost) + w_l*lat.
+static void score_row(int I, int M, const int32_t* tier, const int32_t* cap, const float* price_in,
+                      const float* price_out, const float* pre, const float* dec, const float* slope,
+                      const float* dq, const int32_t* bq, const float* Q, const float* L, int32_t ell,
+                      const float* w /*qual,lat,cost*/, float* S) {
+  (void)M;
+  std::vector<float> C(I), T(I);
+  float Cmax = 0.0f, Tmax = 0.0f;
+  bool first = true;
+  for (int i = 0; i < I; ++i) {
+    int t = tier[i];
+    float c1 = (float)ell * price_in[t];
+    float c2 = L[t] * price_out[t];
+    C[i] = c1 + c2;
+    float a = slope[t] * (float)bq[i];
+    a = 1.0f + a;
+    float tpot = dec[t] * a;
+    float wait = (bq[i] < cap[i]) ? 0.0f : dq[i] / (float)bq[i];
+    float u = wait + L[t];
+    float v = tpot * u;
+    float p = pre[t] * (float)ell;
+    T[i] = p + v;
+    if (first || C[i] > Cmax) Cmax = C[i];
+    if (first || T[i] > Tmax) Tmax = T[i];
+    first = false;
+  }
+  for (int i = 0; i < I; ++i) {
+    int t = tier[i];
+    float ct = (Cmax > 0.0f) ? 1.0f - (C[i] / Cmax) : 0.0f;
+    float lt = (Tmax > 0.0f) ? 1.0f - (T[i] / Tmax) : 0.0f;
+    float t1 = w[0] * Q[t];
+    float t2 = w[2] * ct;
+    float A = t1 + t2;
+    float t3 = w[1] * lt;
+    S[i] = A + t3;
+  }
+}
+
+// Steps 6-9: Algorithm 1 (caption P:L109, prose P:L111).
+//   key_r = max_m L^[r,m] over tiers that have an instance (reading 16/23), requests dispatched by
+//   (key descending, r ascending) when lpt_enabled, else in input order.
+//   Each dispatch: S[r,:] from the CURRENT local state; i* = first in the order (S descending, d ascending,
+//   i ascending) (reading 17); then, if update_enabled, d[i*] += L^[r,m(i*)] and the decode batch
+//   grows by one while a slot is free (reading 18).
+//   scores0 = S[r,:] of every request from the batch-start state (reading 19).
+// dq/bq in: batch-start state; dq_out/bq_out: state after the batch (equal to the input when !update).
+int orc_decide_from_predictions(int I, int M, const int32_t* tier, const int32_t* cap,
+                                const float* price_in, const float* price_out, const float* pre,
+                                const float* dec, const float* slope, const float* dq_in,
+                                const int32_t* bq_in, const float* quality, const float* outlen,
+                                const int32_t* prompt_len, int B, const float* w, int lpt_enabled,
+                                int update_enabled, int32_t* assignment, float* scores, float* scores0,
+                                int32_t* order, float* dq_out, int32_t* bq_out) {
+  std::vector<float> dq(dq_in, dq_in + I);
+  std::vector<int32_t> bq(bq_in, bq_in + I);
+  std::vector<char> present(M, 0);
+  for (int i = 0; i < I; ++i) present[tier[i]] = 1;
+
+  std::vector<float> key(B);
+  for (int r = 0; r < B; ++r) {
+    bool first = true;
+    float kmax = 0.0f;
+    for (int m = 0; m < M; ++m) {
+      if (!present[m]) continue;
+      float l = outlen[(int64_t)r * M + m];
+      if (first || l > kmax) kmax = l;
+      first = false;
+    }
+    key[r] = kmax;
+  }
+  std::vector<int32_t> ord(B);
+  std::iota(ord.begin(), ord.end(), 0);
+  if (lpt_enabled) {
+    std::stable_sort(ord.begin(), ord.end(), [&](int32_t a, int32_t b) { return key[a] > key[b]; });
+  }
+
+  std::vector<float> S(I);
+  for (int r = 0; r < B; ++r) {
+    score_row(I, M, tier, cap, price_in, price_out, pre, dec, slope, dq_in, bq_in,
+              quality + (int64_t)r * M, outlen + (int64_t)r * M, prompt_len[r], w, S.data());
+    if (scores0) std::copy(S.begin(), S.end(), scores0 + (int64_t)r * I);
+  }
+
+  for (int j = 0; j < B; ++j) {
+    int r = ord[j];
+    const float* Q = quality + (int64_t)r * M;
+    const float* L = outlen + (int64_t)r * M;
+    score_row(I, M, tier, cap, price_in, price_out, pre, dec, slope, dq.data(), bq.data(), Q, L,
+              prompt_len[r], w, S.data());
+    int best = 0;
+    for (int i = 1; i < I; ++i) {
+      if (S[i] > S[best] || (S[i] == S[best] && dq[i] < dq[best])) best = i;
+    }
+    assignment[r] = best;
+    if (scores) std::copy(S.begin(), S.end(), scores + (int64_t)r * I);
+    if (order) order[j] = r;
+    if (update_enabled) {
+      dq[best] = dq[best] + L[tier[best]];
+      if (bq[best] < cap[best]) bq[best] += 1;
+    }
+  }
+  if (dq_out) std::copy(dq.begin(), dq.end(), dq_out);
+  if (bq_out) std::copy(bq.begin(), bq.end(), bq_out);
+  return 0;
+}
+
+// Step 10 (BASELINE.json rb_advance_state; reading 22: the drain rule is ours, the paper re-reads telemetry):
+// each instance with b_i > 0 completes b_i tokens every tpot_i ms.
+int orc_advance_state(int I, const int32_t* tier, const float* dec, const float* slope, float elapsed_ms,
+                      float* dq, int32_t* bq) {
+  for (int i = 0; i < I; ++i) {
+    if (bq[i] <= 0) continue;
+    int t = tier[i];
+    float a = slope[t] * (float)bq[i];
+    a = 1.0f + a;
+    float tpot = dec[t] * a;
+    float q = elapsed_ms / tpot;
+    float done = (float)bq[i] * q;
+    float d = dq[i] - done;
+    d = std::max(d, 0.0f);
+    dq[i] = d;
+    if (d == 0.0f) bq[i] = 0;
+  }
+  return 0;
+}
+
+// A second, separately labelled CPU figure for bench.py only (never used for parity): the same brute-force
+// scan with an fp32 accumulator the compiler may vectorise.  Returns the index of the best row per query.
+int orc_scan_fast_f32(const float* bank, const float* query, int64_t N, int d, int B, int32_t* best) {
+  for (int r = 0; r < B; ++r) {
+    float bs = -INFINITY;
+    int32_t bi = 0;
+    const float* x = query + (int64_t)r * d;
+    for (int64_t n = 0; n < N; ++n) {
+      const float* e = bank + n * d;
+      float acc = 0.0f;
+      for (int c = 0; c < d; ++c) acc += x[c] * e[c];
+      if (acc > bs) { bs = acc; bi = (int32_t)n; }
+    }
+    best[r] = bi;
+  }
+  return 0;
+}
+
+}  // extern "C"
