@@ -1,0 +1,195 @@
+"""Thin ctypes binding over the C ABI of include/routebalance.h (argument marshalling only -- every step of the
+path runs in the CUDA kernels of librouteb.so).  The function names are the C names.  Array arguments may be
+torch tensors (CPU or CUDA) or numpy arrays; they must be contiguous and of the stated dtype.
+
+There is no fallback: importing this module fails if the library has not been built
+(`python paper_2606_17949_b200/build.py`), and every call raises RbError on a non-RB_OK status.
+"""
+import ctypes
+import os
+
+import numpy as np
+
+try:
+    import torch
+except ImportError:  # pragma: no cover
+    torch = None
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "librouteb.so")
+if not os.path.exists(LIB_PATH):
+    raise ImportError("librouteb.so is not built (run `python paper_2606_17949_b200/build.py`); "
+                      "there is no CPU fallback for the RouteBalance decision path")
+_lib = ctypes.CDLL(LIB_PATH)
+
+RB_OK, RB_EINVAL, RB_ECUDA, RB_ENOMEM, RB_ESTATE, RB_EUNSUPPORTED = range(6)
+RB_F32, RB_BF16 = 0, 1
+_STATUS = {0: "RB_OK", 1: "RB_EINVAL", 2: "RB_ECUDA", 3: "RB_ENOMEM", 4: "RB_ESTATE", 5: "RB_EUNSUPPORTED"}
+EXPORTS = ["rb_options_default", "rb_create", "rb_set_instances", "rb_set_state", "rb_get_state", "rb_advance_state",
+           "rb_decide", "rb_decide_from_predictions", "rb_estimate", "rb_set_stage_timing", "rb_last_stage_us",
+           "rb_launch_count", "rb_sync", "rb_last_error", "rb_destroy"]
+
+
+class rb_options(ctypes.Structure):
+    _fields_ = [("bank_dtype", ctypes.c_int32), ("store_dtype", ctypes.c_int32), ("weight_mode", ctypes.c_int32),
+                ("dist_eps", ctypes.c_float), ("rerank_slack", ctypes.c_int32), ("lpt_enabled", ctypes.c_int32),
+                ("update_enabled", ctypes.c_int32), ("max_batch", ctypes.c_int32), ("use_graph", ctypes.c_int32),
+                ("stream", ctypes.c_void_p)]
+
+
+class rb_lat_head(ctypes.Structure):
+    _fields_ = [("prefill_ms_per_tok", ctypes.c_float), ("decode_ms_per_tok", ctypes.c_float),
+                ("batch_slope", ctypes.c_float)]
+
+
+class RbError(RuntimeError):
+    def __init__(self, status, msg):
+        super().__init__("%s: %s" % (_STATUS.get(status, status), msg))
+        self.status = status
+
+
+_vp, _i32, _i64, _f = ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64, ctypes.c_float
+_lib.rb_options_default.argtypes = [ctypes.POINTER(rb_options)]
+_lib.rb_options_default.restype = None
+_lib.rb_create.argtypes = [ctypes.POINTER(_vp), _vp, _vp, _vp, _i64, _i32, _i32, _i32, ctypes.POINTER(rb_options)]
+_lib.rb_set_instances.argtypes = [_vp, _i32, _vp, _vp, _vp, _vp, ctypes.POINTER(rb_lat_head)]
+_lib.rb_set_state.argtypes = [_vp, _vp, _vp]
+_lib.rb_get_state.argtypes = [_vp, _vp, _vp]
+_lib.rb_advance_state.argtypes = [_vp, _f]
+_lib.rb_decide.argtypes = [_vp, _vp, _vp, _i32, ctypes.POINTER(_f * 3), _vp, _vp, _vp, _vp, _vp, _vp]
+_lib.rb_decide_from_predictions.argtypes = [_vp, _vp, _vp, _vp, _i32, ctypes.POINTER(_f * 3), _i32, _vp, _vp, _vp, _vp]
+_lib.rb_estimate.argtypes = [_vp, _vp, _i32, _vp, _vp, _vp, _vp]
+_lib.rb_set_stage_timing.argtypes = [_vp, _i32]
+_lib.rb_last_stage_us.argtypes = [_vp, ctypes.POINTER(_f * 6)]
+_lib.rb_launch_count.argtypes = [_vp]
+_lib.rb_launch_count.restype = _i64
+_lib.rb_sync.argtypes = [_vp]
+_lib.rb_last_error.argtypes = [_vp]
+_lib.rb_last_error.restype = ctypes.c_char_p
+_lib.rb_destroy.argtypes = [_vp]
+_lib.rb_destroy.restype = None
+
+
+def _ptr(a, dtype=None):
+    """Raw address of a contiguous torch tensor / numpy array (None -> NULL)."""
+    if a is None:
+        return None
+    if torch is not None and isinstance(a, torch.Tensor):
+        if not a.is_contiguous():
+            raise ValueError("tensor must be contiguous")
+        if dtype is not None and a.dtype != dtype:
+            raise ValueError("expected %s, got %s" % (dtype, a.dtype))
+        return a.data_ptr()
+    a_np = np.asarray(a)
+    if not a_np.flags["C_CONTIGUOUS"]:
+        raise ValueError("array must be contiguous")
+    if dtype is not None:
+        want = {torch.float32: np.float32, torch.int32: np.int32, torch.bfloat16: np.uint16}[dtype] if torch else dtype
+        if a_np.dtype != want:
+            raise ValueError("expected %s, got %s" % (want, a_np.dtype))
+    return a_np.ctypes.data
+
+
+def _check(ctx, st):
+    if st != RB_OK:
+        msg = _lib.rb_last_error(ctx).decode() if ctx else ""
+        raise RbError(st, msg)
+
+
+def rb_options_default():
+    o = rb_options()
+    _lib.rb_options_default(ctypes.byref(o))
+    return o
+
+
+def rb_create(bank_emb, bank_quality, bank_outlen, N, d, M, k, opt=None):
+    """Returns the opaque context handle.  bank_emb: float32 [N,d], or bfloat16 (torch) / uint16 (numpy)."""
+    ctx = _vp()
+    if opt is None:
+        opt = rb_options_default()
+    f32 = torch.float32 if torch else np.float32
+    st = _lib.rb_create(ctypes.byref(ctx), _ptr(bank_emb), _ptr(bank_quality, f32), _ptr(bank_outlen, f32), N, d, M, k,
+                        ctypes.byref(opt))
+    if st != RB_OK:
+        msg = _lib.rb_last_error(ctx).decode() if ctx else ""
+        if ctx:
+            _lib.rb_destroy(ctx)
+        raise RbError(st, msg)
+    return ctx
+
+
+def rb_set_instances(ctx, tier, cap, price_in, price_out, heads):
+    """tier, cap: int sequences [I]; price_in/out: float sequences [M]; heads: M (prefill, decode, slope) triples."""
+    tier = np.ascontiguousarray(tier, dtype=np.int32)
+    cap = np.ascontiguousarray(cap, dtype=np.int32)
+    pin = np.ascontiguousarray(price_in, dtype=np.float32)
+    pout = np.ascontiguousarray(price_out, dtype=np.float32)
+    h = (rb_lat_head * len(heads))(*[rb_lat_head(*map(float, x)) for x in heads])
+    _check(ctx, _lib.rb_set_instances(ctx, len(tier), tier.ctypes.data, cap.ctypes.data, pin.ctypes.data,
+                                      pout.ctypes.data, h))
+
+
+def rb_set_state(ctx, queued_tokens, running):
+    f32, i32 = (torch.float32, torch.int32) if torch else (np.float32, np.int32)
+    _check(ctx, _lib.rb_set_state(ctx, _ptr(queued_tokens, f32), _ptr(running, i32)))
+
+
+def rb_get_state(ctx, queued_tokens, running):
+    f32, i32 = (torch.float32, torch.int32) if torch else (np.float32, np.int32)
+    _check(ctx, _lib.rb_get_state(ctx, _ptr(queued_tokens, f32), _ptr(running, i32)))
+
+
+def rb_advance_state(ctx, elapsed_ms):
+    _check(ctx, _lib.rb_advance_state(ctx, float(elapsed_ms)))
+
+
+def _w3(w):
+    return ctypes.byref((_f * 3)(*[float(x) for x in w]))
+
+
+def rb_decide(ctx, query_emb, prompt_len, B, w, assignment, scores=None, pred_quality=None, pred_outlen=None,
+              nn_idx=None, nn_sim=None):
+    f32, i32 = (torch.float32, torch.int32) if torch else (np.float32, np.int32)
+    _check(ctx, _lib.rb_decide(ctx, _ptr(query_emb, f32), _ptr(prompt_len, i32), B, _w3(w), _ptr(assignment, i32),
+                               _ptr(scores, f32), _ptr(pred_quality, f32), _ptr(pred_outlen, f32), _ptr(nn_idx, i32),
+                               _ptr(nn_sim, f32)))
+
+
+def rb_decide_from_predictions(ctx, quality, outlen, prompt_len, B, w, commit, assignment, scores=None, scores0=None,
+                               order=None):
+    f32, i32 = (torch.float32, torch.int32) if torch else (np.float32, np.int32)
+    _check(ctx, _lib.rb_decide_from_predictions(ctx, _ptr(quality, f32), _ptr(outlen, f32), _ptr(prompt_len, i32), B,
+                                                _w3(w), int(commit), _ptr(assignment, i32), _ptr(scores, f32),
+                                                _ptr(scores0, f32), _ptr(order, i32)))
+
+
+def rb_estimate(ctx, query_emb, B, pred_quality=None, pred_outlen=None, nn_idx=None, nn_sim=None):
+    f32, i32 = (torch.float32, torch.int32) if torch else (np.float32, np.int32)
+    _check(ctx, _lib.rb_estimate(ctx, _ptr(query_emb, f32), B, _ptr(pred_quality, f32), _ptr(pred_outlen, f32),
+                                 _ptr(nn_idx, i32), _ptr(nn_sim, f32)))
+
+
+def rb_set_stage_timing(ctx, enabled):
+    _check(ctx, _lib.rb_set_stage_timing(ctx, int(enabled)))
+
+
+def rb_last_stage_us(ctx):
+    us = (_f * 6)()
+    _check(ctx, _lib.rb_last_stage_us(ctx, ctypes.byref(us)))
+    return dict(zip(["stage", "scan", "merge", "aggregate", "score", "dispatch"], list(us)))
+
+
+def rb_launch_count(ctx):
+    return int(_lib.rb_launch_count(ctx))
+
+
+def rb_sync(ctx):
+    _check(ctx, _lib.rb_sync(ctx))
+
+
+def rb_last_error(ctx):
+    return _lib.rb_last_error(ctx).decode()
+
+
+def rb_destroy(ctx):
+    _lib.rb_destroy(ctx)

@@ -1,0 +1,648 @@
+// rb_api.cu -- the C ABI of include/routebalance.h: context, argument checking, buffer staging, the launch
+// sequence of one decision (a0..a7) and its CUDA-graph replay (a9).  Every step of the path runs in the
+// kernels of scan_tc.cu / estimate.cu / score_dispatch.cu; nothing here computes on the host.
+#include "../../include/routebalance.h"
+
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <unordered_map>
+#include <vector>
+
+#include <cudaTypedefs.h>
+
+#include "rb_internal.cuh"
+
+using namespace rb;
+
+struct rb_ctx {
+  // problem
+  int64_t N = 0;
+  int d = 0, M = 0, k = 0, kc = 0, kcap = 0;
+  rb_options opt{};
+  cudaStream_t stream = nullptr;
+  bool own_stream = false;
+  int num_sms = 148;
+  // bank
+  void* bank = nullptr;          // bf16 [N x d] or fp32 [N x d]
+  float* bank_quality = nullptr; // [N x M]
+  float* bank_outlen = nullptr;
+  // instances
+  int I = 0;
+  int32_t *tier = nullptr, *cap = nullptr, *present = nullptr;
+  float *price_in = nullptr, *price_out = nullptr, *pre = nullptr, *dec = nullptr, *slope = nullptr;
+  float* dq = nullptr;
+  int32_t* bq = nullptr;
+  // per-call staging + scratch (sized by max_batch)
+  int Bpad_max = 0;
+  float* q32 = nullptr;             // [max_batch x d]
+  __nv_bfloat16* qs = nullptr;      // [Bpad_max x d]
+  int32_t* plen = nullptr;          // [max_batch]
+  CallParams* cp = nullptr;
+  CallParams* cp_ring = nullptr;    // pinned host ring feeding cp; slot reuse is guarded by cp_ev
+  cudaEvent_t cp_ev[64]{};
+  uint64_t cp_seq = 0;
+  float* part_sim = nullptr;        // [num_sms][kcap][Bpad_max]
+  int32_t* part_idx = nullptr;
+  float* sims = nullptr;            // fp32 storage only: [kF32Group x N]
+  float* cand_sim = nullptr;        // [max_batch x kc]
+  int32_t* cand_idx = nullptr;
+  int32_t* nn_idx = nullptr;        // [max_batch x k]
+  float* nn_sim = nullptr;
+  float *pred_q = nullptr, *pred_l = nullptr;   // [max_batch x M]
+  float *termA = nullptr, *termP = nullptr, *key = nullptr;
+  int32_t *order = nullptr, *assignment = nullptr;
+  float *scores = nullptr, *scores0 = nullptr;  // [max_batch x I], allocated by rb_set_instances
+  CUtensorMap tm_q{}, tm_bank{};
+  // graphs: key = B * 4 + kind (0 decide, 1 estimate, 2 from_predictions)
+  std::unordered_map<int64_t, cudaGraphExec_t> graphs;
+  std::unordered_map<int64_t, int> graph_nodes;
+  int64_t launches = 0;
+  bool stage_timing = false;
+  cudaEvent_t ev[8]{};
+  float stage_us[6]{};
+  std::string err;
+};
+
+namespace {
+
+constexpr int kF32Group = 64;   // queries per pass of the fp32-storage scan
+
+rb_status fail(rb_ctx* c, rb_status st, const char* what, cudaError_t e = cudaSuccess) {
+  if (c) {
+    char buf[512];
+    if (e != cudaSuccess)
+      snprintf(buf, sizeof buf, "%s: %s", what, cudaGetErrorString(e));
+    else
+      snprintf(buf, sizeof buf, "%s", what);
+    c->err = buf;
+  }
+  return st;
+}
+
+#define CK(call)                                              \
+  do {                                                        \
+    cudaError_t e_ = (call);                                  \
+    if (e_ != cudaSuccess) return fail(ctx, RB_ECUDA, #call, e_); \
+  } while (0)
+
+bool is_host_ptr(const void* p) {
+  cudaPointerAttributes a{};
+  if (cudaPointerGetAttributes(&a, p) != cudaSuccess) {
+    cudaGetLastError();
+    return true;
+  }
+  return !(a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged);
+}
+
+template <typename T>
+cudaError_t dev_alloc(T** p, size_t n) {
+  return cudaMalloc((void**)p, (n ? n : 1) * sizeof(T));
+}
+
+InstTable table_of(const rb_ctx* c) {
+  InstTable t;
+  t.I = c->I; t.M = c->M; t.tier = c->tier; t.cap = c->cap; t.price_in = c->price_in; t.price_out = c->price_out;
+  t.pre = c->pre; t.dec = c->dec; t.slope = c->slope; t.present = c->present;
+  return t;
+}
+
+rb_status encode_map(rb_ctx* ctx, CUtensorMap* map, void* base, uint64_t rows, uint64_t cols, uint32_t box_rows) {
+  static PFN_cuTensorMapEncodeTiled_v12000 fn = nullptr;
+  if (!fn) {
+    cudaDriverEntryPointQueryResult q;
+    void* p = nullptr;
+    CK(cudaGetDriverEntryPointByVersion("cuTensorMapEncodeTiled", &p, 12000, cudaEnableDefault, &q));
+    if (q != cudaDriverEntryPointSuccess || !p) return fail(ctx, RB_ECUDA, "cuTensorMapEncodeTiled entry point not found");
+    fn = (PFN_cuTensorMapEncodeTiled_v12000)p;
+  }
+  cuuint64_t dims[2] = {cols, rows};
+  cuuint64_t strides[1] = {cols * 2};
+  cuuint32_t box[2] = {(cuuint32_t)kTileK, box_rows};
+  cuuint32_t estr[2] = {1, 1};
+  CUresult r = fn(map, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, base, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                  CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) {
+    char buf[96];
+    snprintf(buf, sizeof buf, "cuTensorMapEncodeTiled failed (CUresult %d)", (int)r);
+    return fail(ctx, RB_ECUDA, buf);
+  }
+  return RB_OK;
+}
+
+bool finite_nonneg(float x) { return std::isfinite(x) && x >= 0.0f; }
+
+rb_status check_weights(rb_ctx* ctx, const float w[3]) {
+  if (!w) return fail(ctx, RB_EINVAL, "w is NULL");
+  float sum = 0.0f;
+  for (int j = 0; j < 3; ++j) {
+    if (!finite_nonneg(w[j])) return fail(ctx, RB_EINVAL, "weights must be finite and >= 0");
+    sum += w[j];
+  }
+  if (std::fabs(sum - 1.0f) > 1e-5f) return fail(ctx, RB_EINVAL, "weights must sum to 1 (3-simplex, P:L90)");
+  return RB_OK;
+}
+
+// ---- the launch sequence ------------------------------------------------------------------------------
+struct Timer {
+  rb_ctx* c;
+  int idx = 0;
+  explicit Timer(rb_ctx* c_) : c(c_) {}
+  void mark() {
+    if (c->stage_timing) cudaEventRecord(c->ev[idx++], c->stream);
+  }
+};
+
+rb_status enqueue_estimate(rb_ctx* ctx, int B, Timer& tm) {
+  cudaStream_t s = ctx->stream;
+  const int Bpad = (B + kTileM - 1) / kTileM * kTileM;
+  if (ctx->opt.store_dtype == RB_BF16) {
+    tm.mark();
+    CK(launch_stage_queries(ctx->q32, ctx->qs, B, Bpad, ctx->d, s));
+    tm.mark();
+    int grid = 0;
+    CK(launch_scan_tc(&ctx->tm_q, &ctx->tm_bank, ctx->N, ctx->d, B, Bpad, ctx->kcap, ctx->num_sms, ctx->part_sim,
+                      ctx->part_idx, &grid, s));
+    tm.mark();
+    CK(launch_merge(ctx->part_sim, ctx->part_idx, grid, ctx->kcap, Bpad, B, ctx->kc, ctx->N, ctx->cand_sim, ctx->cand_idx, s));
+    tm.mark();
+    CK(launch_aggregate((const __nv_bfloat16*)ctx->bank, ctx->qs, ctx->d, ctx->opt.rerank_slack > 0 ? 1 : 0, ctx->cand_sim,
+                        ctx->cand_idx, ctx->kc, ctx->k, ctx->bank_quality, ctx->bank_outlen, ctx->M, ctx->opt.weight_mode,
+                        ctx->opt.dist_eps, B, ctx->nn_idx, ctx->nn_sim, ctx->pred_q, ctx->pred_l, s));
+    ctx->launches += 4;
+  } else {
+    tm.mark();
+    tm.mark();
+    for (int r0 = 0; r0 < B; r0 += kF32Group) {
+      const int nq = (B - r0 < kF32Group) ? (B - r0) : kF32Group;
+      CK(launch_scan_f32((const float*)ctx->bank, ctx->q32 + (size_t)r0 * ctx->d, ctx->N, ctx->d, nq, ctx->sims, s));
+      CK(launch_select_f32(ctx->sims, ctx->N, nq, ctx->kc, ctx->cand_sim + (size_t)r0 * ctx->kc,
+                           ctx->cand_idx + (size_t)r0 * ctx->kc, s));
+      ctx->launches += 2;
+    }
+    tm.mark();
+    tm.mark();
+    CK(launch_aggregate(nullptr, nullptr, ctx->d, 0, ctx->cand_sim, ctx->cand_idx, ctx->kc, ctx->k, ctx->bank_quality,
+                        ctx->bank_outlen, ctx->M, ctx->opt.weight_mode, ctx->opt.dist_eps, B, ctx->nn_idx, ctx->nn_sim,
+                        ctx->pred_q, ctx->pred_l, s));
+    ctx->launches += 1;
+  }
+  tm.mark();
+  return RB_OK;
+}
+
+rb_status enqueue_dispatch(rb_ctx* ctx, int B, bool want_scores0, Timer& tm) {
+  cudaStream_t s = ctx->stream;
+  InstTable t = table_of(ctx);
+  CK(launch_score(t, ctx->dq, ctx->bq, ctx->pred_q, ctx->pred_l, ctx->plen, ctx->cp, B, ctx->termA, ctx->termP, ctx->key,
+                  want_scores0 ? ctx->scores0 : nullptr, s));
+  tm.mark();
+  CK(launch_dispatch(t, ctx->dq, ctx->bq, ctx->pred_l, ctx->termA, ctx->termP, ctx->key, ctx->cp, B, ctx->opt.lpt_enabled,
+                     ctx->opt.update_enabled, ctx->order, ctx->assignment, ctx->scores, s));
+  tm.mark();
+  ctx->launches += 3;
+  return RB_OK;
+}
+
+// kind: 0 = estimate + dispatch, 1 = estimate, 2 = dispatch (+scores0)
+rb_status run_path(rb_ctx* ctx, int B, int kind) {
+  const bool graph = ctx->opt.use_graph && !ctx->stage_timing;
+  Timer tm(ctx);
+  if (!graph) {
+    if (kind != 2) {
+      rb_status st = enqueue_estimate(ctx, B, tm);
+      if (st != RB_OK) return st;
+    }
+    if (kind != 1) return enqueue_dispatch(ctx, B, kind == 2, tm);
+    return RB_OK;
+  }
+  const int64_t gkey = (int64_t)B * 4 + kind;
+  auto it = ctx->graphs.find(gkey);
+  if (it == ctx->graphs.end()) {
+    const int64_t before = ctx->launches;
+    cudaGraph_t g = nullptr;
+    CK(cudaStreamBeginCapture(ctx->stream, cudaStreamCaptureModeThreadLocal));
+    rb_status st = RB_OK;
+    if (kind != 2) st = enqueue_estimate(ctx, B, tm);
+    if (st == RB_OK && kind != 1) st = enqueue_dispatch(ctx, B, kind == 2, tm);
+    cudaError_t e = cudaStreamEndCapture(ctx->stream, &g);
+    const int nodes = (int)(ctx->launches - before);
+    ctx->launches = before;
+    if (st != RB_OK) {
+      if (g) cudaGraphDestroy(g);
+      return st;
+    }
+    if (e != cudaSuccess) return fail(ctx, RB_ECUDA, "cudaStreamEndCapture", e);
+    cudaGraphExec_t ge = nullptr;
+    e = cudaGraphInstantiate(&ge, g, 0);
+    cudaGraphDestroy(g);
+    if (e != cudaSuccess) return fail(ctx, RB_ECUDA, "cudaGraphInstantiate", e);
+    it = ctx->graphs.emplace(gkey, ge).first;
+    ctx->graph_nodes[gkey] = nodes;
+  }
+  CK(cudaGraphLaunch(it->second, ctx->stream));
+  ctx->launches += ctx->graph_nodes[gkey];
+  return RB_OK;
+}
+
+void collect_stage_times(rb_ctx* ctx, int kind) {
+  if (!ctx->stage_timing) return;
+  cudaStreamSynchronize(ctx->stream);
+  for (float& v : ctx->stage_us) v = 0.0f;
+  // marks: estimate = 5 (4 intervals: stage, scan, merge, aggregate), dispatch = 2 more (score, dispatch)
+  const int first = (kind == 2) ? 4 : 0;
+  const int n_int = (kind == 0) ? 6 : (kind == 1 ? 4 : 2);
+  // kind 2 has no leading mark: its first interval start is unknown -> only the dispatch interval is reported
+  if (kind == 2) {
+    float ms = 0;
+    if (cudaEventElapsedTime(&ms, ctx->ev[0], ctx->ev[1]) == cudaSuccess) ctx->stage_us[5] = ms * 1000.0f;
+    return;
+  }
+  for (int j = 0; j < n_int; ++j) {
+    float ms = 0;
+    if (cudaEventElapsedTime(&ms, ctx->ev[j], ctx->ev[j + 1]) == cudaSuccess) ctx->stage_us[first + j] = ms * 1000.0f;
+  }
+}
+
+// Per-call parameters travel host -> device through a pinned ring so that the copy is truly asynchronous.
+rb_status push_params(rb_ctx* ctx, const CallParams& cp) {
+  const int slot = (int)(ctx->cp_seq % 64);
+  if (ctx->cp_seq >= 64) CK(cudaEventSynchronize(ctx->cp_ev[slot]));
+  ctx->cp_ring[slot] = cp;
+  CK(cudaMemcpyAsync(ctx->cp, &ctx->cp_ring[slot], sizeof cp, cudaMemcpyHostToDevice, ctx->stream));
+  CK(cudaEventRecord(ctx->cp_ev[slot], ctx->stream));
+  ctx->cp_seq++;
+  return RB_OK;
+}
+
+struct CopyBack {
+  rb_ctx* ctx;
+  bool any_host = false;
+  cudaError_t err = cudaSuccess;
+  void out(void* dst, const void* src, size_t bytes) {
+    if (!dst || err != cudaSuccess) return;
+    any_host |= is_host_ptr(dst);
+    err = cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDefault, ctx->stream);
+  }
+  void in(void* dst, const void* src, size_t bytes) {
+    if (err != cudaSuccess) return;
+    any_host |= is_host_ptr(src);
+    err = cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDefault, ctx->stream);
+  }
+};
+
+}  // namespace
+
+extern "C" {
+
+void rb_options_default(rb_options* opt) {
+  if (!opt) return;
+  std::memset(opt, 0, sizeof *opt);
+  opt->bank_dtype = RB_F32;
+  opt->store_dtype = RB_BF16;
+  opt->weight_mode = 0;
+  opt->dist_eps = 1e-6f;
+  opt->rerank_slack = 6;
+  opt->lpt_enabled = 1;
+  opt->update_enabled = 1;
+  opt->max_batch = 4096;
+  opt->use_graph = 1;
+  opt->stream = nullptr;
+}
+
+rb_status rb_create(rb_ctx** out, const void* bank_emb, const float* bank_quality, const float* bank_outlen, int64_t N,
+                    int32_t d, int32_t M, int32_t k, const rb_options* opt_in) {
+  if (!out) return RB_EINVAL;
+  *out = nullptr;
+  rb_options opt;
+  if (opt_in) opt = *opt_in; else rb_options_default(&opt);
+  if (!bank_emb || !bank_quality || !bank_outlen) return RB_EINVAL;
+  if (N < 1 || N >= (int64_t)1 << 31 || d < 8 || d % 8 != 0 || M < 1 || M > kMaxM || k < 1 || k > N) return RB_EINVAL;
+  if (opt.bank_dtype != RB_F32 && opt.bank_dtype != RB_BF16) return RB_EINVAL;
+  if (opt.store_dtype != RB_F32 && opt.store_dtype != RB_BF16) return RB_EINVAL;
+  if (opt.store_dtype == RB_F32 && opt.bank_dtype != RB_F32) return RB_EINVAL;
+  if (opt.store_dtype == RB_F32 || opt.rerank_slack < 0) opt.rerank_slack = 0;
+  if (k + opt.rerank_slack > kMaxK) return RB_EINVAL;
+  if (opt.max_batch < 1 || opt.max_batch > 4096) return RB_EINVAL;
+  if (!(opt.dist_eps >= 0.0f) || !std::isfinite(opt.dist_eps)) return RB_EINVAL;
+  if (opt.weight_mode != 0 && opt.weight_mode != 1) return RB_EINVAL;
+
+  int dev = 0;
+  cudaDeviceProp prop{};
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) {
+    cudaGetLastError();
+    return RB_EUNSUPPORTED;
+  }
+  if (prop.major != 10) return RB_EUNSUPPORTED;   // sm_100a kernels only; there is no fallback path
+
+  rb_ctx* ctx = new (std::nothrow) rb_ctx();
+  if (!ctx) return RB_ENOMEM;
+  ctx->N = N; ctx->d = d; ctx->M = M; ctx->k = k; ctx->opt = opt;
+  ctx->kc = k + opt.rerank_slack;
+  ctx->kcap = ctx->kc <= 16 ? 16 : (ctx->kc <= 32 ? 32 : 64);
+  ctx->num_sms = prop.multiProcessorCount;
+  ctx->Bpad_max = (opt.max_batch + kTileM - 1) / kTileM * kTileM;
+  *out = ctx;   // from here on errors keep the context so that rb_last_error works; caller destroys it
+
+  if (opt.stream) {
+    ctx->stream = (cudaStream_t)opt.stream;
+  } else {
+    CK(cudaStreamCreateWithFlags(&ctx->stream, cudaStreamNonBlocking));
+    ctx->own_stream = true;
+  }
+  for (auto& e : ctx->ev) CK(cudaEventCreate(&e));
+  for (auto& e : ctx->cp_ev) CK(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+  CK(cudaMallocHost((void**)&ctx->cp_ring, 64 * sizeof(CallParams)));
+  cudaStream_t s = ctx->stream;
+  const size_t nd = (size_t)N * d;
+#define ALLOC(ptr, n)                                                                 \
+  do {                                                                                \
+    cudaError_t e_ = dev_alloc(&(ptr), (n));                                          \
+    if (e_ != cudaSuccess) { cudaGetLastError(); return fail(ctx, RB_ENOMEM, "cudaMalloc " #ptr, e_); } \
+  } while (0)
+
+  if (opt.store_dtype == RB_BF16) {
+    __nv_bfloat16* b16 = nullptr;
+    ALLOC(b16, nd);
+    ctx->bank = b16;
+    if (opt.bank_dtype == RB_BF16) {
+      CK(cudaMemcpyAsync(b16, bank_emb, nd * 2, cudaMemcpyDefault, s));
+    } else {
+      // fp32 -> bf16 (RNE) once, in chunks through a bounded device buffer
+      const size_t chunk_rows = std::max<size_t>(1, ((size_t)64 << 20) / (size_t)d);
+      float* tmp = nullptr;
+      ALLOC(tmp, std::min<size_t>(chunk_rows, (size_t)N) * d);
+      for (size_t r0 = 0; r0 < (size_t)N; r0 += chunk_rows) {
+        const size_t rows = std::min(chunk_rows, (size_t)N - r0);
+        CK(cudaMemcpyAsync(tmp, (const float*)bank_emb + r0 * d, rows * d * 4, cudaMemcpyDefault, s));
+        // one "row" of rows*d elements: the staging kernel is a plain elementwise RNE conversion
+        CK(launch_stage_queries(tmp, b16 + r0 * d, 1, 1, (int)std::min<size_t>(rows * d, (size_t)INT32_MAX), s));
+        if (rows * d > (size_t)INT32_MAX) return fail(ctx, RB_EINVAL, "conversion chunk too large");
+      }
+      CK(cudaStreamSynchronize(s));
+      cudaFree(tmp);
+    }
+  } else {
+    float* b32 = nullptr;
+    ALLOC(b32, nd);
+    ctx->bank = b32;
+    CK(cudaMemcpyAsync(b32, bank_emb, nd * 4, cudaMemcpyDefault, s));
+    ALLOC(ctx->sims, (size_t)kF32Group * N);
+  }
+  ALLOC(ctx->bank_quality, (size_t)N * M);
+  ALLOC(ctx->bank_outlen, (size_t)N * M);
+  CK(cudaMemcpyAsync(ctx->bank_quality, bank_quality, (size_t)N * M * 4, cudaMemcpyDefault, s));
+  CK(cudaMemcpyAsync(ctx->bank_outlen, bank_outlen, (size_t)N * M * 4, cudaMemcpyDefault, s));
+
+  const size_t mb = opt.max_batch;
+  ALLOC(ctx->q32, mb * d);
+  ALLOC(ctx->plen, mb);
+  ALLOC(ctx->cp, 1);
+  ALLOC(ctx->cand_sim, mb * ctx->kc);
+  ALLOC(ctx->cand_idx, mb * ctx->kc);
+  ALLOC(ctx->nn_idx, mb * k);
+  ALLOC(ctx->nn_sim, mb * k);
+  ALLOC(ctx->pred_q, mb * M);
+  ALLOC(ctx->pred_l, mb * M);
+  ALLOC(ctx->termA, mb * M);
+  ALLOC(ctx->termP, mb * M);
+  ALLOC(ctx->key, mb);
+  ALLOC(ctx->order, mb);
+  ALLOC(ctx->assignment, mb);
+  ALLOC(ctx->tier, kMaxI);
+  ALLOC(ctx->cap, kMaxI);
+  ALLOC(ctx->dq, kMaxI);
+  ALLOC(ctx->bq, kMaxI);
+  ALLOC(ctx->present, kMaxM);
+  ALLOC(ctx->price_in, kMaxM);
+  ALLOC(ctx->price_out, kMaxM);
+  ALLOC(ctx->pre, kMaxM);
+  ALLOC(ctx->dec, kMaxM);
+  ALLOC(ctx->slope, kMaxM);
+  if (opt.store_dtype == RB_BF16) {
+    ALLOC(ctx->qs, (size_t)ctx->Bpad_max * d);
+    ALLOC(ctx->part_sim, (size_t)ctx->num_sms * ctx->kcap * ctx->Bpad_max);
+    ALLOC(ctx->part_idx, (size_t)ctx->num_sms * ctx->kcap * ctx->Bpad_max);
+    CK(cudaMemsetAsync(ctx->qs, 0, (size_t)ctx->Bpad_max * d * 2, s));
+    rb_status st = encode_map(ctx, &ctx->tm_bank, ctx->bank, (uint64_t)N, (uint64_t)d, kBoxN);
+    if (st != RB_OK) return st;
+    st = encode_map(ctx, &ctx->tm_q, ctx->qs, (uint64_t)ctx->Bpad_max, (uint64_t)d, kTileM);
+    if (st != RB_OK) return st;
+    CK(scan_tc_prepare());
+  }
+#undef ALLOC
+  CK(cudaStreamSynchronize(s));   // the caller may free its buffers on return
+  return RB_OK;
+}
+
+rb_status rb_set_instances(rb_ctx* ctx, int32_t I, const int32_t* tier, const int32_t* cap, const float* price_in,
+                           const float* price_out, const rb_lat_head* heads) {
+  if (!ctx) return RB_EINVAL;
+  if (!tier || !cap || !price_in || !price_out || !heads) return fail(ctx, RB_EINVAL, "NULL argument");
+  if (I < 1 || I > kMaxI) return fail(ctx, RB_EINVAL, "I out of range [1,1024]");
+  const int M = ctx->M;
+  int32_t present[kMaxM] = {0};
+  for (int i = 0; i < I; ++i) {
+    if (tier[i] < 0 || tier[i] >= M) return fail(ctx, RB_EINVAL, "tier out of range");
+    if (cap[i] < 1) return fail(ctx, RB_EINVAL, "cap must be >= 1");
+    present[tier[i]] = 1;
+  }
+  float pre[kMaxM], dec[kMaxM], slope[kMaxM];
+  for (int m = 0; m < M; ++m) {
+    if (!finite_nonneg(price_in[m]) || !finite_nonneg(price_out[m])) return fail(ctx, RB_EINVAL, "prices must be finite, >= 0");
+    if (!finite_nonneg(heads[m].prefill_ms_per_tok) || !finite_nonneg(heads[m].decode_ms_per_tok) ||
+        !finite_nonneg(heads[m].batch_slope))
+      return fail(ctx, RB_EINVAL, "latency head coefficients must be finite, >= 0");
+    pre[m] = heads[m].prefill_ms_per_tok; dec[m] = heads[m].decode_ms_per_tok; slope[m] = heads[m].batch_slope;
+  }
+  cudaStream_t s = ctx->stream;
+  // scores buffers depend on I
+  if (I != ctx->I) {
+    CK(cudaStreamSynchronize(s));
+    cudaFree(ctx->scores); cudaFree(ctx->scores0);
+    ctx->scores = ctx->scores0 = nullptr;
+    const size_t n = (size_t)ctx->opt.max_batch * I;
+    if (dev_alloc(&ctx->scores, n) != cudaSuccess || dev_alloc(&ctx->scores0, n) != cudaSuccess) {
+      cudaGetLastError();
+      ctx->I = 0;
+      return fail(ctx, RB_ENOMEM, "cudaMalloc scores");
+    }
+    for (auto& kv : ctx->graphs) cudaGraphExecDestroy(kv.second);   // grid shapes depend on I
+    ctx->graphs.clear();
+    ctx->graph_nodes.clear();
+  }
+  CK(cudaMemcpyAsync(ctx->tier, tier, I * 4, cudaMemcpyHostToDevice, s));
+  CK(cudaMemcpyAsync(ctx->cap, cap, I * 4, cudaMemcpyHostToDevice, s));
+  CK(cudaMemcpyAsync(ctx->present, present, M * 4, cudaMemcpyHostToDevice, s));
+  CK(cudaMemcpyAsync(ctx->price_in, price_in, M * 4, cudaMemcpyHostToDevice, s));
+  CK(cudaMemcpyAsync(ctx->price_out, price_out, M * 4, cudaMemcpyHostToDevice, s));
+  CK(cudaMemcpyAsync(ctx->pre, pre, M * 4, cudaMemcpyHostToDevice, s));
+  CK(cudaMemcpyAsync(ctx->dec, dec, M * 4, cudaMemcpyHostToDevice, s));
+  CK(cudaMemcpyAsync(ctx->slope, slope, M * 4, cudaMemcpyHostToDevice, s));
+  CK(cudaMemsetAsync(ctx->dq, 0, kMaxI * 4, s));
+  CK(cudaMemsetAsync(ctx->bq, 0, kMaxI * 4, s));
+  CK(cudaStreamSynchronize(s));   // stack arrays above are read by pageable copies
+  ctx->I = I;
+  return RB_OK;
+}
+
+rb_status rb_set_state(rb_ctx* ctx, const float* queued_tokens, const int32_t* running) {
+  if (!ctx) return RB_EINVAL;
+  if (ctx->I == 0) return fail(ctx, RB_ESTATE, "rb_set_state before rb_set_instances");
+  if (!queued_tokens || !running) return fail(ctx, RB_EINVAL, "NULL argument");
+  const bool host = is_host_ptr(queued_tokens) || is_host_ptr(running);
+  if (is_host_ptr(queued_tokens) && is_host_ptr(running)) {
+    for (int i = 0; i < ctx->I; ++i)
+      if (!finite_nonneg(queued_tokens[i]) || running[i] < 0) return fail(ctx, RB_EINVAL, "state must be finite, >= 0");
+  }
+  CK(cudaMemcpyAsync(ctx->dq, queued_tokens, ctx->I * 4, cudaMemcpyDefault, ctx->stream));
+  CK(cudaMemcpyAsync(ctx->bq, running, ctx->I * 4, cudaMemcpyDefault, ctx->stream));
+  if (host) CK(cudaStreamSynchronize(ctx->stream));
+  return RB_OK;
+}
+
+rb_status rb_get_state(rb_ctx* ctx, float* queued_tokens, int32_t* running) {
+  if (!ctx) return RB_EINVAL;
+  if (ctx->I == 0) return fail(ctx, RB_ESTATE, "rb_get_state before rb_set_instances");
+  CopyBack cb{ctx};
+  cb.out(queued_tokens, ctx->dq, ctx->I * 4);
+  cb.out(running, ctx->bq, ctx->I * 4);
+  if (cb.err != cudaSuccess) return fail(ctx, RB_ECUDA, "cudaMemcpyAsync", cb.err);
+  if (cb.any_host) CK(cudaStreamSynchronize(ctx->stream));
+  return RB_OK;
+}
+
+rb_status rb_advance_state(rb_ctx* ctx, float elapsed_ms) {
+  if (!ctx) return RB_EINVAL;
+  if (ctx->I == 0) return fail(ctx, RB_ESTATE, "rb_advance_state before rb_set_instances");
+  if (!finite_nonneg(elapsed_ms)) return fail(ctx, RB_EINVAL, "elapsed_ms must be finite and >= 0");
+  CK(launch_advance(table_of(ctx), ctx->dq, ctx->bq, elapsed_ms, ctx->stream));
+  ctx->launches += 1;
+  return RB_OK;
+}
+
+rb_status rb_decide(rb_ctx* ctx, const float* query_emb, const int32_t* prompt_len, int32_t B, const float w[3],
+                    int32_t* assignment, float* scores, float* pred_quality, float* pred_outlen, int32_t* nn_idx,
+                    float* nn_sim) {
+  if (!ctx) return RB_EINVAL;
+  if (ctx->I == 0) return fail(ctx, RB_ESTATE, "rb_decide before rb_set_instances");
+  if (!query_emb || !prompt_len || !assignment) return fail(ctx, RB_EINVAL, "NULL argument");
+  if (B < 1 || B > ctx->opt.max_batch) return fail(ctx, RB_EINVAL, "B out of range [1,max_batch]");
+  rb_status st = check_weights(ctx, w);
+  if (st != RB_OK) return st;
+  const CallParams cp{w[0], w[1], w[2], 1};
+  CopyBack cb{ctx};
+  cb.in(ctx->q32, query_emb, (size_t)B * ctx->d * 4);
+  cb.in(ctx->plen, prompt_len, (size_t)B * 4);
+  if (cb.err != cudaSuccess) return fail(ctx, RB_ECUDA, "cudaMemcpyAsync (inputs)", cb.err);
+  st = push_params(ctx, cp);
+  if (st != RB_OK) return st;
+  st = run_path(ctx, B, 0);
+  if (st != RB_OK) return st;
+  cb.out(assignment, ctx->assignment, (size_t)B * 4);
+  cb.out(scores, ctx->scores, (size_t)B * ctx->I * 4);
+  cb.out(pred_quality, ctx->pred_q, (size_t)B * ctx->M * 4);
+  cb.out(pred_outlen, ctx->pred_l, (size_t)B * ctx->M * 4);
+  cb.out(nn_idx, ctx->nn_idx, (size_t)B * ctx->k * 4);
+  cb.out(nn_sim, ctx->nn_sim, (size_t)B * ctx->k * 4);
+  if (cb.err != cudaSuccess) return fail(ctx, RB_ECUDA, "cudaMemcpyAsync (outputs)", cb.err);
+  collect_stage_times(ctx, 0);
+  // host-side inputs must be consumed and host-side outputs complete before returning
+  if (cb.any_host) CK(cudaStreamSynchronize(ctx->stream));
+  return RB_OK;
+}
+
+rb_status rb_estimate(rb_ctx* ctx, const float* query_emb, int32_t B, float* pred_quality, float* pred_outlen,
+                      int32_t* nn_idx, float* nn_sim) {
+  if (!ctx) return RB_EINVAL;
+  if (!query_emb) return fail(ctx, RB_EINVAL, "NULL argument");
+  if (B < 1 || B > ctx->opt.max_batch) return fail(ctx, RB_EINVAL, "B out of range [1,max_batch]");
+  CopyBack cb{ctx};
+  cb.in(ctx->q32, query_emb, (size_t)B * ctx->d * 4);
+  if (cb.err != cudaSuccess) return fail(ctx, RB_ECUDA, "cudaMemcpyAsync (inputs)", cb.err);
+  rb_status st = run_path(ctx, B, 1);
+  if (st != RB_OK) return st;
+  cb.out(pred_quality, ctx->pred_q, (size_t)B * ctx->M * 4);
+  cb.out(pred_outlen, ctx->pred_l, (size_t)B * ctx->M * 4);
+  cb.out(nn_idx, ctx->nn_idx, (size_t)B * ctx->k * 4);
+  cb.out(nn_sim, ctx->nn_sim, (size_t)B * ctx->k * 4);
+  if (cb.err != cudaSuccess) return fail(ctx, RB_ECUDA, "cudaMemcpyAsync (outputs)", cb.err);
+  collect_stage_times(ctx, 1);
+  if (cb.any_host) CK(cudaStreamSynchronize(ctx->stream));
+  return RB_OK;
+}
+
+rb_status rb_decide_from_predictions(rb_ctx* ctx, const float* quality, const float* outlen, const int32_t* prompt_len,
+                                     int32_t B, const float w[3], int32_t commit, int32_t* assignment, float* scores,
+                                     float* scores0, int32_t* order) {
+  if (!ctx) return RB_EINVAL;
+  if (ctx->I == 0) return fail(ctx, RB_ESTATE, "rb_decide_from_predictions before rb_set_instances");
+  if (!quality || !outlen || !prompt_len || !assignment) return fail(ctx, RB_EINVAL, "NULL argument");
+  if (B < 1 || B > ctx->opt.max_batch) return fail(ctx, RB_EINVAL, "B out of range [1,max_batch]");
+  rb_status st = check_weights(ctx, w);
+  if (st != RB_OK) return st;
+  const CallParams cp{w[0], w[1], w[2], commit ? 1 : 0};
+  CopyBack cb{ctx};
+  cb.in(ctx->pred_q, quality, (size_t)B * ctx->M * 4);
+  cb.in(ctx->pred_l, outlen, (size_t)B * ctx->M * 4);
+  cb.in(ctx->plen, prompt_len, (size_t)B * 4);
+  if (cb.err != cudaSuccess) return fail(ctx, RB_ECUDA, "cudaMemcpyAsync (inputs)", cb.err);
+  st = push_params(ctx, cp);
+  if (st != RB_OK) return st;
+  st = run_path(ctx, B, 2);
+  if (st != RB_OK) return st;
+  cb.out(assignment, ctx->assignment, (size_t)B * 4);
+  cb.out(scores, ctx->scores, (size_t)B * ctx->I * 4);
+  cb.out(scores0, ctx->scores0, (size_t)B * ctx->I * 4);
+  cb.out(order, ctx->order, (size_t)B * 4);
+  if (cb.err != cudaSuccess) return fail(ctx, RB_ECUDA, "cudaMemcpyAsync (outputs)", cb.err);
+  collect_stage_times(ctx, 2);
+  if (cb.any_host) CK(cudaStreamSynchronize(ctx->stream));
+  return RB_OK;
+}
+
+rb_status rb_set_stage_timing(rb_ctx* ctx, int32_t enabled) {
+  if (!ctx) return RB_EINVAL;
+  ctx->stage_timing = enabled != 0;
+  return RB_OK;
+}
+
+rb_status rb_last_stage_us(rb_ctx* ctx, float us[6]) {
+  if (!ctx || !us) return RB_EINVAL;
+  for (int j = 0; j < 6; ++j) us[j] = ctx->stage_us[j];
+  return RB_OK;
+}
+
+int64_t rb_launch_count(const rb_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+rb_status rb_sync(rb_ctx* ctx) {
+  if (!ctx) return RB_EINVAL;
+  CK(cudaStreamSynchronize(ctx->stream));
+  return RB_OK;
+}
+
+const char* rb_last_error(const rb_ctx* ctx) { return ctx ? ctx->err.c_str() : "null context"; }
+
+void rb_destroy(rb_ctx* ctx) {
+  if (!ctx) return;
+  if (ctx->stream) cudaStreamSynchronize(ctx->stream);
+  for (auto& kv : ctx->graphs) cudaGraphExecDestroy(kv.second);
+  void* ptrs[] = {ctx->bank, ctx->bank_quality, ctx->bank_outlen, ctx->tier, ctx->cap, ctx->present, ctx->price_in,
+                  ctx->price_out, ctx->pre, ctx->dec, ctx->slope, ctx->dq, ctx->bq, ctx->q32, ctx->qs, ctx->plen, ctx->cp,
+                  ctx->part_sim, ctx->part_idx, ctx->sims, ctx->cand_sim, ctx->cand_idx, ctx->nn_idx, ctx->nn_sim,
+                  ctx->pred_q, ctx->pred_l, ctx->termA, ctx->termP, ctx->key, ctx->order, ctx->assignment, ctx->scores,
+                  ctx->scores0};
+  for (void* p : ptrs) cudaFree(p);
+  for (auto& e : ctx->ev)
+    if (e) cudaEventDestroy(e);
+  for (auto& e : ctx->cp_ev)
+    if (e) cudaEventDestroy(e);
+  if (ctx->cp_ring) cudaFreeHost(ctx->cp_ring);
+  if (ctx->own_stream) cudaStreamDestroy(ctx->stream);
+  delete ctx;
+}
+
+}  // extern "C"

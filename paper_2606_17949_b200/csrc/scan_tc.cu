@@ -1,0 +1,354 @@
+// scan_tc.cu -- step a1 for bf16 storage: similarity scan of the reference bank on the 5th-gen tensor cores
+// with a fused per-query top-KCAP epilogue.  The B x N similarity matrix exists only in TMEM.
+//
+// Definition ("queries a ... KNN index (k=10) over the 14,919-prompt training split"; DESIGN.md
+// readings 1, 3, 4): s[r,n] = <q~_r, e~_n> over the bf16-rounded vectors; keep, per query, the best entries in
+// the order (s descending, n ascending).  Here each CTA keeps the best KCAP of its own slab of bank rows; the
+// cross-CTA merge is merge.cu and the exact re-rank is aggregate.cu.
+//
+// Shape of the kernel (one persistent CTA per SM, 6 warps):
+//   warp 0   TMA producer: cp.async.bulk.tensor tiles of the bank (64 rows x 64 bf16, 128B swizzle) and of the
+//            staged queries (128 x 64) into a 4-stage shared-memory ring, mbarrier complete_tx.
+//   warp 1   allocates TMEM (512 columns = two 128x256 fp32 accumulators) and issues tcgen05.mma
+//            (M=128 queries x N<=256 bank rows x K=16) from one lane; tcgen05.commit releases ring slots and
+//            publishes finished accumulators.
+//   warps 2-5  epilogue: thread t owns TMEM lane t = query t of the m-tile; tcgen05.ld 32 columns at a time,
+//            compare against the thread's current KCAP-th best similarity, append the rare survivors to a
+//            shared-memory buffer, then insert them into a sorted register list in warp lock-step.
+// Bank rows are split over CTAs in units of 64 rows; a CTA walks its slab in tiles of 256 rows and, for
+// B > 128, revisits each tile once per 128-query m-tile (bank tile then comes from L2), carrying the lists
+// through global memory between visits.
+#include "rb_internal.cuh"
+
+namespace rb {
+namespace {
+
+constexpr int kStages = 4;
+constexpr int kABytes = kTileM * kTileK * 2;       // 16 KB: 128 queries x 64 bf16
+constexpr int kBoxBytes = kBoxN * kTileK * 2;      //  8 KB: 64 bank rows x 64 bf16
+constexpr int kBBytes = kTileN * kTileK * 2;       // 32 KB
+constexpr int kStageBytes = kABytes + kBBytes;     // 48 KB
+constexpr int kCandSlots = 32;                     // one tcgen05.ld chunk can yield at most 32 survivors
+constexpr int kThreads = 192;
+constexpr int kSmemBytes = kStages * kStageBytes + kCandSlots * kTileM * 5 + 256 + 1024;
+
+// ---- PTX wrappers --------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+  const uint32_t addr = smem_u32(bar);
+  uint32_t ok;
+  do {
+    asm volatile(
+        "{\n\t.reg .pred P1;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%1], %2;\n\t"
+        "selp.b32 %0, 1, 0, P1;\n\t}"
+        : "=r"(ok)
+        : "r"(addr), "r"(parity)
+        : "memory");
+  } while (!ok);
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("{\n\t.reg .b64 st;\n\tmbarrier.arrive.expect_tx.shared::cta.b64 st, [%0], %1;\n\t}" ::"r"(smem_u32(bar)),
+               "r"(bytes)
+               : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+  asm volatile("{\n\t.reg .b64 st;\n\tmbarrier.arrive.shared::cta.b64 st, [%0];\n\t}" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void tma_load_2d(void* dst, const CUtensorMap* map, int c0, int c1, uint64_t* bar) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];" ::"r"(
+          smem_u32(dst)),
+      "l"(map), "r"(c0), "r"(c1), "r"(smem_u32(bar))
+      : "memory");
+}
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_commit(uint64_t* bar) {
+  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar))
+               : "memory");
+}
+// D[tmem] (+)= A[smem] * B[smem]^T, bf16 x bf16 -> fp32, one 128 x N x 16 step.
+__device__ __forceinline__ void tc_mma(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accum) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "setp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}" ::"r"(d_tmem),
+      "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accum)
+      : "memory");
+}
+// 32 lanes x 32 consecutive fp32 columns: thread t of the warp receives lane (base lane + t).
+__device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&r)[32]) {
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x32.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+      "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+      : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
+        "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]), "=r"(r[16]),
+        "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]), "=r"(r[24]),
+        "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
+      : "r"(taddr)
+      : "memory");
+}
+__device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+
+// Shared-memory matrix descriptor: K-major operand, 128-byte swizzle, rows of 128 bytes, 8-row groups 1024 B apart.
+__device__ __forceinline__ uint64_t make_smem_desc(uint32_t saddr) {
+  uint64_t desc = 0;
+  desc |= (uint64_t)((saddr & 0x3FFFF) >> 4);        // start address
+  desc |= (uint64_t)0 << 16;                          // leading-dimension byte offset: unused for swizzled K-major
+  desc |= (uint64_t)(1024 >> 4) << 32;                // stride-dimension byte offset
+  desc |= (uint64_t)1 << 46;                          // descriptor version (sm_100)
+  desc |= (uint64_t)2 << 61;                          // SWIZZLE_128B
+  return desc;
+}
+// Instruction descriptor, kind::f16: D fp32, A = B = bf16, both K-major, M x N.
+__device__ __forceinline__ uint32_t make_idesc(int m, int n) {
+  return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(n >> 3) << 17) | ((uint32_t)(m >> 4) << 24);
+}
+
+// Sorted insertion into a register-resident list (similarity descending; an equal similarity goes after the
+// entries already present, which have smaller bank indices because rows are scanned in ascending order).
+template <int K>
+__device__ __forceinline__ void list_insert(float (&v)[K], int32_t (&ix)[K], float s, int32_t id) {
+#pragma unroll
+  for (int j = K - 1; j >= 1; --j) {
+    const bool up = s > v[j - 1];
+    const bool here = (!up) && (s > v[j]);
+    const float nv = up ? v[j - 1] : (here ? s : v[j]);
+    const int32_t ni = up ? ix[j - 1] : (here ? id : ix[j]);
+    v[j] = nv;
+    ix[j] = ni;
+  }
+  const bool top = s > v[0];
+  v[0] = top ? s : v[0];
+  ix[0] = top ? id : ix[0];
+}
+
+template <int KCAP>
+__global__ void __launch_bounds__(kThreads, 1)
+scan_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_bank, int64_t N, int d,
+               int B, int Bpad, float* __restrict__ part_sim, int32_t* __restrict__ part_idx) {
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);   // 128B swizzle wants 1024 B alignment
+  float* cand_s = (float*)(smem + kStages * kStageBytes);
+  uint8_t* cand_c = (uint8_t*)(cand_s + kCandSlots * kTileM);
+  uint64_t* bars = (uint64_t*)(cand_c + kCandSlots * kTileM);
+  uint64_t* full = bars;                  // [kStages] TMA bytes landed
+  uint64_t* empty = bars + kStages;       // [kStages] MMAs that read the slot retired
+  uint64_t* tfull = bars + 2 * kStages;   // [2] accumulator complete
+  uint64_t* tempty = tfull + 2;           // [2] accumulator drained by the epilogue
+  uint32_t* tmem_slot = (uint32_t*)(tempty + 2);
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int n_mt = Bpad / kTileM;
+  const int nk = (d + kTileK - 1) / kTileK;
+  const int64_t units = (N + kBoxN - 1) / kBoxN;
+  const int64_t u0 = units * blockIdx.x / gridDim.x;
+  const int64_t u1 = units * (blockIdx.x + 1) / gridDim.x;
+  const int nunits = (int)(u1 - u0);
+  const int64_t row0 = u0 * kBoxN;
+  const int ntiles = (nunits + 3) / 4;
+
+  if (warp == 0 && lane == 0) {
+    asm volatile("prefetch.tensormap [%0];" ::"l"(&tm_q) : "memory");
+    asm volatile("prefetch.tensormap [%0];" ::"l"(&tm_bank) : "memory");
+    for (int s = 0; s < kStages; ++s) {
+      mbar_init(&full[s], 1);
+      mbar_init(&empty[s], 1);
+    }
+    for (int a = 0; a < 2; ++a) {
+      mbar_init(&tfull[a], 1);
+      mbar_init(&tempty[a], 4);
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  if (warp == 1) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)), "r"(512)
+                 : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+  }
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = *tmem_slot;
+
+  if (warp == 0) {
+    // ===== TMA producer =====
+    if (lane == 0) {
+      uint32_t kit = 0;
+      for (int tile = 0; tile < ntiles; ++tile) {
+        const int n0 = (int)(row0 + (int64_t)tile * kTileN);
+        const int nun = min(4, nunits - tile * 4);
+        for (int mt = 0; mt < n_mt; ++mt) {
+          for (int kc = 0; kc < nk; ++kc, ++kit) {
+            const int s = kit % kStages;
+            const uint32_t ph = (kit / kStages) & 1;
+            mbar_wait(&empty[s], ph ^ 1);
+            uint8_t* sa = smem + s * kStageBytes;
+            uint8_t* sb = sa + kABytes;
+            mbar_arrive_expect_tx(&full[s], kABytes + nun * kBoxBytes);
+            tma_load_2d(sa, &tm_q, kc * kTileK, mt * kTileM, &full[s]);
+            for (int u = 0; u < nun; ++u) tma_load_2d(sb + u * kBoxBytes, &tm_bank, kc * kTileK, n0 + u * kBoxN, &full[s]);
+          }
+        }
+      }
+    }
+    __syncwarp();
+  } else if (warp == 1) {
+    // ===== MMA issuer =====
+    if (lane == 0) {
+      uint32_t kit = 0, it = 0;
+      for (int tile = 0; tile < ntiles; ++tile) {
+        const int nun = min(4, nunits - tile * 4);
+        const uint32_t idesc = make_idesc(kTileM, nun * kBoxN);
+        for (int mt = 0; mt < n_mt; ++mt, ++it) {
+          const uint32_t acc = it & 1, aph = (it >> 1) & 1;
+          mbar_wait(&tempty[acc], aph ^ 1);
+          tc_fence_after();
+          const uint32_t d_tmem = tmem_base + acc * kTileN;
+          for (int kc = 0; kc < nk; ++kc, ++kit) {
+            const int s = kit % kStages;
+            const uint32_t ph = (kit / kStages) & 1;
+            mbar_wait(&full[s], ph);
+            tc_fence_after();
+            const uint32_t sa = smem_u32(smem + s * kStageBytes);
+            const uint64_t adesc = make_smem_desc(sa);
+            const uint64_t bdesc = make_smem_desc(sa + kABytes);
+#pragma unroll
+            for (int k4 = 0; k4 < kTileK / 16; ++k4) {
+              // +32 bytes along K inside the 128-byte swizzle row = +2 in the encoded start address
+              tc_mma(d_tmem, adesc + 2 * k4, bdesc + 2 * k4, idesc, (uint32_t)((kc | k4) != 0));
+            }
+            tc_commit(&empty[s]);
+          }
+          tc_commit(&tfull[acc]);
+        }
+      }
+    }
+    __syncwarp();
+  } else {
+    // ===== epilogue: fused per-query top-KCAP =====
+    const int quarter = warp & 3;              // TMEM lane quarter this warp may read
+    const int tl = quarter * 32 + lane;        // TMEM lane = query row inside the m-tile
+    float v[KCAP];
+    int32_t ix[KCAP];
+    uint32_t it = 0;
+    for (int tile = 0; tile < ntiles; ++tile) {
+      const int n0 = (int)(row0 + (int64_t)tile * kTileN);
+      const int nun = min(4, nunits - tile * 4);
+      const int ncols = nun * kBoxN;
+      const int nvalid = (int)min((int64_t)ncols, N - (int64_t)n0);   // rows >= N are TMA zero fill
+      for (int mt = 0; mt < n_mt; ++mt, ++it) {
+        const uint32_t acc = it & 1, aph = (it >> 1) & 1;
+        const int r = mt * kTileM + tl;
+        const bool warp_active = (mt * kTileM + quarter * 32) < B;   // warp-uniform
+        const size_t pbase = ((size_t)blockIdx.x * KCAP) * (size_t)Bpad + (size_t)r;
+        if (warp_active) {
+          if (tile == 0) {
+#pragma unroll
+            for (int j = 0; j < KCAP; ++j) { v[j] = -INFINITY; ix[j] = -1; }
+          } else if (n_mt > 1) {
+#pragma unroll
+            for (int j = 0; j < KCAP; ++j) {
+              v[j] = part_sim[pbase + (size_t)j * Bpad];
+              ix[j] = part_idx[pbase + (size_t)j * Bpad];
+            }
+          }
+        }
+        mbar_wait(&tfull[acc], aph);
+        tc_fence_after();
+        if (warp_active) {
+          float thr = (r < B) ? v[KCAP - 1] : INFINITY;   // padding lanes never collect
+          const uint32_t taddr = tmem_base + ((uint32_t)(quarter * 32) << 16) + acc * kTileN;
+          for (int c0 = 0; c0 < nvalid; c0 += 32) {
+            uint32_t regs[32];
+            tmem_ld32(taddr + c0, regs);
+            tmem_ld_wait();
+            int cnt = 0;
+            if (c0 + 32 <= nvalid) {
+#pragma unroll
+              for (int j = 0; j < 32; ++j) {
+                const float s = __uint_as_float(regs[j]);
+                if (s > thr) {
+                  cand_s[cnt * kTileM + tl] = s;
+                  cand_c[cnt * kTileM + tl] = (uint8_t)(c0 + j);
+                  ++cnt;
+                }
+              }
+            } else {
+#pragma unroll
+              for (int j = 0; j < 32; ++j) {
+                const float s = __uint_as_float(regs[j]);
+                if ((c0 + j < nvalid) && s > thr) {
+                  cand_s[cnt * kTileM + tl] = s;
+                  cand_c[cnt * kTileM + tl] = (uint8_t)(c0 + j);
+                  ++cnt;
+                }
+              }
+            }
+            // lock-step drain: every lane inserts its p-th survivor in the same iteration
+            for (int p = 0; __any_sync(0xffffffffu, p < cnt); ++p) {
+              if (p < cnt) {
+                const float s = cand_s[p * kTileM + tl];
+                if (s > thr) {
+                  list_insert<KCAP>(v, ix, s, n0 + (int)cand_c[p * kTileM + tl]);
+                  thr = v[KCAP - 1];
+                }
+              }
+            }
+          }
+        }
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&tempty[acc]);
+        if (warp_active && r < B && (n_mt > 1 || tile == ntiles - 1)) {
+#pragma unroll
+          for (int j = 0; j < KCAP; ++j) {
+            part_sim[pbase + (size_t)j * Bpad] = v[j];
+            part_idx[pbase + (size_t)j * Bpad] = ix[j];
+          }
+        }
+      }
+    }
+  }
+
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 1) {
+    tc_fence_after();
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(512) : "memory");
+  }
+}
+
+}  // namespace
+
+size_t scan_tc_smem_bytes() { return kSmemBytes; }
+
+cudaError_t scan_tc_prepare() {
+  cudaError_t e;
+  e = cudaFuncSetAttribute(scan_tc_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
+  if (e != cudaSuccess) return e;
+  e = cudaFuncSetAttribute(scan_tc_kernel<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
+  if (e != cudaSuccess) return e;
+  return cudaFuncSetAttribute(scan_tc_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
+}
+
+cudaError_t launch_scan_tc(const CUtensorMap* tm_q, const CUtensorMap* tm_bank, int64_t N, int d, int B, int Bpad,
+                           int kcap, int max_grid, float* part_sim, int32_t* part_idx, int* grid_out, cudaStream_t s) {
+  const int64_t units = (N + kBoxN - 1) / kBoxN;
+  const int grid = (int)(units < max_grid ? units : max_grid);
+  if (grid_out) *grid_out = grid;
+  if (kcap == 16)
+    scan_tc_kernel<16><<<grid, kThreads, kSmemBytes, s>>>(*tm_q, *tm_bank, N, d, B, Bpad, part_sim, part_idx);
+  else if (kcap == 32)
+    scan_tc_kernel<32><<<grid, kThreads, kSmemBytes, s>>>(*tm_q, *tm_bank, N, d, B, Bpad, part_sim, part_idx);
+  else
+    scan_tc_kernel<64><<<grid, kThreads, kSmemBytes, s>>>(*tm_q, *tm_bank, N, d, B, Bpad, part_sim, part_idx);
+  return cudaGetLastError();
+}
+
+}  // namespace rb

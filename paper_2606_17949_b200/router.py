@@ -1,0 +1,110 @@
+"""Convenience wrapper: owns an rb_ctx and torch output buffers; every method is one C-ABI call plus
+marshalling.  No arithmetic of the method lives here."""
+import torch
+
+from . import binding as rb
+
+
+class Router:
+    def __init__(self, bank_emb, bank_quality, bank_outlen, k, *, store="bf16", rerank_slack=None, weight_mode=0,
+                 dist_eps=1e-6, lpt_enabled=1, update_enabled=1, max_batch=4096, use_graph=1, device="cuda"):
+        N, d = bank_emb.shape
+        M = bank_quality.shape[1]
+        opt = rb.rb_options_default()
+        opt.bank_dtype = rb.RB_BF16 if bank_emb.dtype == torch.bfloat16 else rb.RB_F32
+        opt.store_dtype = rb.RB_BF16 if store == "bf16" else rb.RB_F32
+        if rerank_slack is not None:
+            opt.rerank_slack = rerank_slack
+        opt.weight_mode = weight_mode
+        opt.dist_eps = dist_eps
+        opt.lpt_enabled = lpt_enabled
+        opt.update_enabled = update_enabled
+        opt.max_batch = max_batch
+        opt.use_graph = use_graph
+        self.device = torch.device(device)
+        self.stream = torch.cuda.Stream(device=self.device)
+        opt.stream = self.stream.cuda_stream
+        self.N, self.d, self.M, self.k, self.max_batch = N, d, M, k, max_batch
+        self.I = 0
+        if torch.cuda.is_available():
+            torch.cuda.synchronize()   # the bank may have been produced on another stream
+        self.ctx = rb.rb_create(bank_emb.contiguous(), bank_quality.contiguous().float(),
+                                bank_outlen.contiguous().float(), N, d, M, k, opt)
+
+    def close(self):
+        if self.ctx is not None:
+            rb.rb_destroy(self.ctx)
+            self.ctx = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def set_instances(self, tier, cap, price_in, price_out, pre, dec, slope):
+        rb.rb_set_instances(self.ctx, tier, cap, price_in, price_out, list(zip(pre, dec, slope)))
+        self.I = len(tier)
+
+    def set_state(self, queued, running):
+        rb.rb_set_state(self.ctx, queued.contiguous().float(), running.contiguous().to(torch.int32))
+
+    def get_state(self):
+        q = torch.empty(self.I, dtype=torch.float32)
+        b = torch.empty(self.I, dtype=torch.int32)
+        rb.rb_get_state(self.ctx, q, b)
+        return q, b
+
+    def advance_state(self, elapsed_ms):
+        rb.rb_advance_state(self.ctx, elapsed_ms)
+
+    def _buf(self, shape, dtype, device):
+        return torch.empty(shape, dtype=dtype, device=device)
+
+    def decide(self, query, prompt_len, w, want=("scores", "pred", "nn"), out_device=None):
+        """query [B,d] float32, prompt_len [B] int32 (host or device).  Outputs land on out_device
+        (default: where the query lives).  Returns a dict of tensors."""
+        B = query.shape[0]
+        dev = out_device if out_device is not None else query.device
+        out = {"assignment": self._buf((B,), torch.int32, dev)}
+        if "scores" in want:
+            out["scores"] = self._buf((B, self.I), torch.float32, dev)
+        if "pred" in want:
+            out["pred_quality"] = self._buf((B, self.M), torch.float32, dev)
+            out["pred_outlen"] = self._buf((B, self.M), torch.float32, dev)
+        if "nn" in want:
+            out["nn_idx"] = self._buf((B, self.k), torch.int32, dev)
+            out["nn_sim"] = self._buf((B, self.k), torch.float32, dev)
+        rb.rb_decide(self.ctx, query, prompt_len, B, w, out["assignment"], out.get("scores"), out.get("pred_quality"),
+                     out.get("pred_outlen"), out.get("nn_idx"), out.get("nn_sim"))
+        return out
+
+    def estimate(self, query, out_device=None):
+        B = query.shape[0]
+        dev = out_device if out_device is not None else query.device
+        out = {"pred_quality": self._buf((B, self.M), torch.float32, dev),
+               "pred_outlen": self._buf((B, self.M), torch.float32, dev),
+               "nn_idx": self._buf((B, self.k), torch.int32, dev), "nn_sim": self._buf((B, self.k), torch.float32, dev)}
+        rb.rb_estimate(self.ctx, query, B, out["pred_quality"], out["pred_outlen"], out["nn_idx"], out["nn_sim"])
+        return out
+
+    def decide_from_predictions(self, quality, outlen, prompt_len, w, commit=0, out_device=None):
+        B = quality.shape[0]
+        dev = out_device if out_device is not None else quality.device
+        out = {"assignment": self._buf((B,), torch.int32, dev), "scores": self._buf((B, self.I), torch.float32, dev),
+               "scores0": self._buf((B, self.I), torch.float32, dev), "order": self._buf((B,), torch.int32, dev)}
+        rb.rb_decide_from_predictions(self.ctx, quality, outlen, prompt_len, B, w, commit, out["assignment"],
+                                      out["scores"], out["scores0"], out["order"])
+        return out
+
+    def sync(self):
+        rb.rb_sync(self.ctx)
+
+    def launch_count(self):
+        return rb.rb_launch_count(self.ctx)
+
+    def stage_us(self):
+        return rb.rb_last_stage_us(self.ctx)
+
+    def set_stage_timing(self, on):
+        rb.rb_set_stage_timing(self.ctx, on)

@@ -1,0 +1,246 @@
+"""Parity tests proper: the CUDA path (through the C ABI) against the oracle, element by element on the same
+seeded inputs.  Run with -m gpu on a B200."""
+import dataclasses
+
+import numpy as np
+import pytest
+import torch
+
+import parity
+from paper_2606_17949_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+
+def _router(bank, cfg, **kw):
+    from paper_2606_17949_b200.router import Router
+    return Router(bank["emb"], bank["quality"], bank["outlen"], cfg.k, store=cfg.store, **kw)
+
+
+def _setup(cfg, device="cuda", B=None, **kw):
+    bank = synth.make_bank(cfg, device=device)
+    it = synth.make_instances(cfg.I, cfg.M)
+    queued, running = synth.make_state(cfg.I, it["cap"], cfg.seed)
+    query = synth.make_queries(cfg, B=B, device=device)
+    plen = synth.make_prompt_len(cfg, B=B, device=device)
+    torch.cuda.synchronize()
+    rt = _router(bank, cfg, **kw)
+    rt.set_instances(**it)
+    rt.set_state(queued, running)
+    return bank, it, queued, running, query, plen, rt
+
+
+def _np(out):
+    torch.cuda.synchronize()
+    return {k: v.detach().cpu().numpy() for k, v in out.items()}
+
+
+def _full_parity(orc, cfg, w, B=None, sim_tol=0.0, **kw):
+    bank, it, queued, running, query, plen, rt = _setup(cfg, B=B, **kw)
+    out = rt.decide(query, plen, w)
+    rt.sync()
+    g = _np(out)
+    bank_np = parity.bank_to_numpy(bank["emb"])
+    qn, ln = bank["quality"].cpu().numpy(), bank["outlen"].cpu().numpy()
+    query_np, plen_np = query.cpu().numpy(), plen.cpu().numpy()
+    log = []
+    oi, os_, near = parity.check_topk(orc, bank_np, query_np, cfg.store, cfg.k, g["nn_idx"], g["nn_sim"], sim_tol, log)
+    parity.check_predictions(orc, g["pred_quality"], g["pred_outlen"], g["nn_idx"], g["nn_sim"], oi, os_, near, qn, ln,
+                             weight_mode=kw.get("weight_mode", 0))
+    inst = orc.Instances(**it)
+    state = rt.get_state()
+    parity.check_dispatch(orc, inst, queued.numpy(), running.numpy(), g["pred_quality"], g["pred_outlen"], plen_np, w, g,
+                          state_after=(state[0].numpy(), state[1].numpy()))
+    rt.close()
+    return g, near, log
+
+
+def test_c1_tiny_full_parity(orc):
+    """BASELINE.json configs[0]: N=4096, d=384 fp32 bank, B=16, I=13, k=10, w=(1/3,1/3,1/3), seed 0.
+    fp32 storage: similarities, neighbour order and predictions are bit-identical to the oracle."""
+    cfg = synth.CONFIGS["C1"]
+    g, near, _ = _full_parity(orc, cfg, synth.PRESETS["balanced"])
+    assert near == []
+
+
+@pytest.mark.parametrize("slack", [6, 0])
+@pytest.mark.parametrize("N,d,B", [(5000, 384, 16), (20011, 128, 300), (777, 64, 5), (64 * 148 * 2 + 3, 256, 128)])
+def test_bf16_scan_parity_ragged(orc, N, d, B, slack):
+    """tcgen05 scan + merge + aggregate on sizes spanning several tiles, a ragged tail (N not a multiple of
+    64), several m-tiles (B > 128) and fewer slabs than SMs (N = 777)."""
+    cfg = dataclasses.replace(synth.CONFIGS["C2"], N=N, d=d, B=B, Kc=16, seed=11)
+    tol = 0.0 if slack > 0 else 4e-6   # re-ranked similarities are exact; raw tensor-core sums are not
+    g, near, log = _full_parity(orc, cfg, synth.PRESETS["balanced"], sim_tol=tol, rerank_slack=slack, max_batch=512)
+    assert len(near) <= max(1, B // 20), log
+
+
+def test_bf16_k32_and_uniform_weights(orc):
+    cfg = dataclasses.replace(synth.CONFIGS["C2"], N=30000, d=384, B=40, k=32, Kc=16, seed=12)
+    _full_parity(orc, cfg, synth.PRESETS["quality"], rerank_slack=8, max_batch=64)
+    _full_parity(orc, cfg, synth.PRESETS["cost"], rerank_slack=0, sim_tol=4e-6, max_batch=64, weight_mode=1)
+
+
+def test_k_equals_one_and_batch_of_one(orc):
+    cfg = dataclasses.replace(synth.CONFIGS["C2"], N=4100, d=64, B=1, k=1, Kc=8, seed=13)
+    _full_parity(orc, cfg, synth.PRESETS["latency"], max_batch=1)
+
+
+def test_tiny_bank_k_equals_N(orc):
+    cfg = dataclasses.replace(synth.CONFIGS["C1"], N=12, d=16, B=3, k=12, Kc=2, seed=14)
+    _full_parity(orc, cfg, synth.PRESETS["balanced"], max_batch=4)
+    cfg = dataclasses.replace(cfg, store="bf16")
+    _full_parity(orc, cfg, synth.PRESETS["balanced"], max_batch=4, rerank_slack=0, sim_tol=4e-6)
+
+
+def test_host_buffers_equal_device_buffers(orc):
+    cfg = dataclasses.replace(synth.CONFIGS["C2"], N=9000, d=128, B=33, Kc=16, seed=15)
+    bank, it, queued, running, query, plen, rt = _setup(cfg, max_batch=64)
+    dev = _np(rt.decide(query, plen, synth.PRESETS["balanced"]))
+    rt.set_state(queued, running)
+    host = rt.decide(query.cpu(), plen.cpu(), synth.PRESETS["balanced"])   # host in, host out: complete on return
+    for key in dev:
+        assert np.array_equal(dev[key], host[key].numpy()), key
+    rt.close()
+
+
+@pytest.mark.parametrize("I,M,B", [(13, 4, 16), (64, 4, 200), (256, 8, 1024), (1, 1, 7), (33, 3, 50), (1024, 16, 64)])
+@pytest.mark.parametrize("lpt,upd", [(1, 1), (0, 1), (1, 0)])
+def test_dispatch_from_predictions_bit_exact(orc, I, M, B, lpt, upd):
+    """Score + LPT dispatch given identical predictions: scores bit-equal (bar: 1e-5 rel), assignment, order
+    and post-batch state bit-exact; single-warp (I <= 32) and multi-warp kernels; commit on/off."""
+    from paper_2606_17949_b200.router import Router
+    rng = np.random.default_rng(100 + I + B)
+    it = synth.make_instances(I, M, cap=int(rng.integers(1, 9)))
+    bank = dict(emb=torch.randn(64, 16), quality=torch.rand(64, M), outlen=torch.rand(64, M) * 100 + 1)
+    rt = Router(bank["emb"].cuda(), bank["quality"].cuda(), bank["outlen"].cuda(), 4, store="f32", max_batch=B,
+                lpt_enabled=lpt, update_enabled=upd)
+    rt.set_instances(**it)
+    queued = torch.from_numpy(rng.integers(0, 20001, I).astype(np.float32))
+    running = torch.from_numpy(np.minimum(rng.integers(0, 12, I), it["cap"]).astype(np.int32))
+    rt.set_state(queued, running)
+    Q = torch.from_numpy(rng.uniform(0, 1, (B, M)).astype(np.float32))
+    L = torch.from_numpy(rng.lognormal(5.5, 0.7, (B, M)).astype(np.float32))
+    if B > 8:
+        L[5] = L[2]                      # equal LPT keys -> request index decides
+    plen = torch.from_numpy(rng.integers(1, 4000, B).astype(np.int32))
+    inst = orc.Instances(**it)
+    for w in [synth.PRESETS["balanced"], (1.0, 0.0, 0.0), (0.0, 1.0, 0.0), (0.0, 0.0, 1.0), (0.2, 0.5, 0.3)]:
+        out = rt.decide_from_predictions(Q.cuda(), L.cuda(), plen.cuda(), w, commit=0)
+        g = _np(out)
+        ref = parity.check_dispatch(orc, inst, queued.numpy(), running.numpy(), Q.numpy(), L.numpy(), plen.numpy(), w, g,
+                                    lpt_enabled=lpt, update_enabled=upd)
+        assert np.array_equal(g["scores"], ref["scores"]) and np.array_equal(g["scores0"], ref["scores0"])
+        s = rt.get_state()
+        assert np.array_equal(s[0].numpy(), queued.numpy()) and np.array_equal(s[1].numpy(), running.numpy())
+    out = rt.decide_from_predictions(Q, L, plen, (0.2, 0.5, 0.3), commit=1)      # host buffers, committed
+    s = rt.get_state()
+    parity.check_dispatch(orc, inst, queued.numpy(), running.numpy(), Q.numpy(), L.numpy(), plen.numpy(), (0.2, 0.5, 0.3),
+                          {k: v.numpy() for k, v in out.items()}, lpt_enabled=lpt, update_enabled=upd,
+                          state_after=(s[0].numpy(), s[1].numpy()))
+    rt.close()
+
+
+def test_advance_state_and_stream_lockstep(orc):
+    """C2-shaped stream in miniature: Poisson windows, rb_advance_state between batches, all four presets;
+    the dead-reckoned state stays bit-identical to the oracle's over the whole stream."""
+    cfg = dataclasses.replace(synth.CONFIGS["C2"], N=6000, d=128, Kc=16, seed=16)
+    bank, it, queued, running, _, _, rt = _setup(cfg, max_batch=64)
+    inst = orc.Instances(**it)
+    sizes, elapsed = synth.poisson_windows(30.0, 60, seed=16)
+    allq = synth.make_queries(cfg, B=sum(sizes), device="cuda")
+    allp = synth.make_prompt_len(cfg, B=sum(sizes), device="cuda")
+    torch.cuda.synchronize()
+    dq, bq = queued.numpy(), running.numpy()
+    presets = list(synth.PRESETS.values())
+    off = 0
+    for j, (B, dt) in enumerate(zip(sizes, elapsed)):
+        rt.advance_state(dt)
+        dq, bq = orc.advance_state(inst, dq, bq, np.float32(dt))
+        w = presets[j % 4]
+        out = _np(rt.decide(allq[off:off + B], allp[off:off + B], w, want=("scores", "pred")))
+        s = rt.get_state()
+        ref = parity.check_dispatch(orc, inst, dq, bq, out["pred_quality"], out["pred_outlen"],
+                                    allp[off:off + B].cpu().numpy(), w, out, state_after=(s[0].numpy(), s[1].numpy()))
+        dq, bq = ref["queued"], ref["running"]
+        off += B
+    assert 4 <= min(sizes) and max(sizes) <= 64
+    rt.close()
+
+
+def test_graph_replay_equals_direct_launch(orc):
+    cfg = dataclasses.replace(synth.CONFIGS["C2"], N=8000, d=256, B=24, Kc=16, seed=17)
+    bank, it, queued, running, query, plen, rt = _setup(cfg, max_batch=32, use_graph=1)
+    a = _np(rt.decide(query, plen, synth.PRESETS["balanced"]))
+    rt.set_state(queued, running)
+    b = _np(rt.decide(query, plen, synth.PRESETS["balanced"]))    # replay of the captured graph
+    rt.close()
+    bank2, _, _, _, _, _, rt2 = _setup(cfg, max_batch=32, use_graph=0)
+    c = _np(rt2.decide(query, plen, synth.PRESETS["balanced"]))
+    rt2.close()
+    for key in a:
+        assert np.array_equal(a[key], b[key]) and np.array_equal(a[key], c[key]), key
+
+
+def test_error_codes_and_call_order():
+    from paper_2606_17949_b200 import binding as rb
+    from paper_2606_17949_b200.router import Router
+    emb = torch.randn(100, 16).cuda()
+    lab = torch.rand(100, 2).cuda()
+    with pytest.raises(rb.RbError) as e:
+        Router(emb, lab, lab, 101, store="f32")          # k > N
+    assert e.value.status == rb.RB_EINVAL
+    with pytest.raises(rb.RbError):
+        Router(torch.randn(100, 12).cuda(), lab, lab, 4)   # d % 8 != 0
+    rt = Router(emb, lab, lab, 4, store="f32", max_batch=8)
+    q = torch.randn(4, 16).cuda()
+    pl = torch.ones(4, dtype=torch.int32).cuda()
+    with pytest.raises(rb.RbError) as e:
+        rt.decide(q, pl, (1 / 3, 1 / 3, 1 / 3))
+    assert e.value.status == rb.RB_ESTATE
+    it = synth.make_instances(3, 2)
+    rt.set_instances(**it)
+    for bad_w in [(0.5, 0.5, 0.5), (-0.1, 0.6, 0.5), (float("nan"), 0.5, 0.5)]:
+        with pytest.raises(rb.RbError) as e:
+            rt.decide(q, pl, bad_w)
+        assert e.value.status == rb.RB_EINVAL
+    with pytest.raises(rb.RbError):
+        rt.decide(torch.randn(9, 16).cuda(), torch.ones(9, dtype=torch.int32).cuda(), (1, 0, 0))   # B > max_batch
+    with pytest.raises(rb.RbError):
+        rt.advance_state(-1.0)
+    bad = dict(it)
+    bad["tier"] = [0, 1, 2]
+    with pytest.raises(rb.RbError):
+        rt.set_instances(**bad)
+    out = rt.decide(q, pl, (1 / 3, 1 / 3, 1 / 3))
+    rt.sync()
+    assert rt.launch_count() > 0
+    assert int(out["assignment"].min()) >= 0 and int(out["assignment"].max()) < 3
+    rt.close()
+
+
+def test_c2_full_size_parity(orc):
+    """BASELINE.json configs[1] at full size (N=100k, d=768 bf16, B=64, I=13), in the launch configuration
+    bench.py times (graph replay, re-rank slack 6): every query checked against the oracle."""
+    cfg = synth.CONFIGS["C2"]
+    g, near, log = _full_parity(orc, cfg, synth.PRESETS["balanced"], max_batch=64)
+    assert len(near) <= 3, log
+
+
+def test_c4_bank_scan_sampled_parity(orc):
+    """BASELINE.json configs[3] (N=10M, d=384 bf16 = 7.68 GB): 8 queries checked against the oracle's
+    brute-force scan of the whole bank (one by one), B=64 launch shape."""
+    cfg = synth.CONFIGS["C4"]
+    bank, it, queued, running, query, plen, rt = _setup(cfg, max_batch=64)
+    out = _np(rt.estimate(query))
+    rt.close()
+    bank_np = parity.bank_to_numpy(bank["emb"])
+    qn, ln = bank["quality"].cpu().numpy(), bank["outlen"].cpu().numpy()
+    del bank
+    torch.cuda.empty_cache()
+    rows = [0, 7, 13, 21, 34, 47, 55, 63]
+    log = []
+    oi, os_, near = parity.check_topk(orc, bank_np, query.cpu().numpy()[rows], "bf16", cfg.k, out["nn_idx"][rows],
+                                      out["nn_sim"][rows], 0.0, log)
+    parity.check_predictions(orc, out["pred_quality"][rows], out["pred_outlen"][rows], out["nn_idx"][rows],
+                             out["nn_sim"][rows], oi, os_, near, qn, ln)
+    assert len(near) <= 2, log
