@@ -1,0 +1,471 @@
+#!/usr/bin/env python
+"""bench.py -- RouteBalance per-batch scheduling decision on B200: requests routed per second.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--l2 flush|warm] [--no-scan-c4]
+
+A *step* is one pass of the whole hot path over one batch of waiting requests: rb_advance_state(elapsed) +
+rb_decide(query_emb, prompt_len, w) = staging, tcgen05 bank scan with fused top-k, merge, re-rank + aggregate,
+score, LPT sort, greedy dispatch with dead-reckoned updates.  The workload is
+BASELINE.json configs[1], the paper-shaped stream (C2): N=100k x d=768 bf16 bank, M=4 tiers, I=13 instances,
+Poisson arrivals at 12 and 30 req/s batched into windows of 4..64 requests, the four weight presets in turn.
+All inputs are seeded synthetic stand-ins for the paper's dataset (paper_2606_17949_b200/synth.py).
+
+One JSON line is printed by rank 0:
+  value        requests routed per second, inputs resident in HBM, device time (CUDA events on the library's
+               stream, one pair per step, L2 flushed between steps by default), whole job over all ranks
+  e2e          the same through the C ABI with pinned HOST buffers: H2D of the step's queries and prompt
+               lengths and D2H of the assignment inside the timed region (wall clock per call; the call
+               returns when the host output is complete)
+  roofline     the bank-scan kernel (dominant): algorithmic bytes N*d*2 + B*d*2 per launch over its mean
+               launch duration, measured live with CUDA events around the kernel in a second pass over the
+               same steps (graph replay off, so the stage boundaries are visible), against the measured HBM
+               copy bandwidth in MEASURED_PEAKS.json
+  cpu_baseline the oracle (oracle/orc.cpp, as it stands) on the host cores over the first windows of the
+               same stream
+  scan_c4      BASELINE.json configs[3] (N=10M x d=384 bf16 = 7.68 GB, B=64): the scan kernel alone against
+               the HBM roofline -- the north-star's ">= 70 % of the HBM roofline" figure (bank >> L2)
+
+--impl reference times the oracle alone (this tier has no reference implementation; the oracle is the
+reference arm).  With --gpus N > 1 (torchrun) every rank runs an independent replica of the router on its
+own request stream ("replicas only"): no data-path collective.
+"""
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "requests routed/sec (per-batch rb_decide, C2 paper-shaped stream)"
+UNIT = "requests/s"
+L2_BYTES = 126 * 1024 * 1024
+
+
+def parse_args(argv=None):
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=1000)
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--l2", default="flush", choices=["flush", "warm"],
+                    help="flush: read a 3x-L2 buffer before every timed step; warm: back-to-back steps")
+    ap.add_argument("--no-scan-c4", action="store_true", help="skip the C4 (10M x 384) bank-scan roofline leg")
+    ap.add_argument("--cpu-seconds", type=float, default=15.0, help="budget of the cpu_baseline sample")
+    return ap.parse_args(argv)
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            j = json.load(f)
+        return float(j["hbm_gbs"]), float(j.get("bf16_tflops", 1590.0)), "measured (MEASURED_PEAKS.json)"
+    return 6650.0, 1590.0, "fallback (B200_PROFILING.md)"
+
+
+def recorded_traffic(name):
+    """dram bytes per launch of the scan kernel from the committed ncu --set full capture (profiles/), or None."""
+    p = os.path.join(ROOT, "profiles", "scan_traffic.json")
+    if not os.path.exists(p):
+        return None
+    with open(p) as f:
+        return json.load(f).get(name)
+
+
+def bank_to_numpy(emb):
+    """torch bank tensor (float32 or bfloat16) -> numpy float32 or raw-bf16 uint16 array (for the oracle)."""
+    import torch
+    e = emb.detach().cpu()
+    if e.dtype == torch.bfloat16:
+        return e.view(torch.int16).numpy().view(np.uint16)
+    return e.numpy()
+
+
+# ---- the C2 stream (pure input generation; no arithmetic of the method) -------------------------------------
+def c2_stream(cfg, n_steps, seed_shift=0):
+    """Window sizes / elapsed ms / weights for n_steps decisions: first half at 12 req/s, second at 30 req/s."""
+    from paper_2606_17949_b200 import synth
+    h = n_steps // 2
+    s1, e1 = synth.poisson_windows(12.0, h, seed=cfg.seed + seed_shift, stream=6) if h else ([], [])
+    s2, e2 = synth.poisson_windows(30.0, n_steps - h, seed=cfg.seed + seed_shift, stream=7)
+    sizes, elapsed = s1 + s2, e1 + e2
+    presets = list(synth.PRESETS.values())
+    weights = [presets[j % 4] for j in range(n_steps)]
+    return sizes, elapsed, weights
+
+
+# ---- clocks during the timed region ----------------------------------------------------------------------------
+class ClockSampler:
+    def __init__(self, index):
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._stop = threading.Event()
+        self._thr = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+        except Exception:
+            self.nv = None
+
+    def _run(self):
+        nv = self.nv
+        names = {nv.nvmlClocksEventReasonHwSlowdown: "hw_slowdown", nv.nvmlClocksEventReasonHwThermalSlowdown:
+                 "hw_thermal_slowdown", nv.nvmlClocksEventReasonSwThermalSlowdown: "sw_thermal_slowdown",
+                 nv.nvmlClocksEventReasonSwPowerCap: "sw_power_cap", nv.nvmlClocksEventReasonHwPowerBrakeSlowdown:
+                 "hw_power_brake"}
+        while not self._stop.is_set():
+            try:
+                self.samples.append(int(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                r = int(nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+                for bit, name in names.items():
+                    if r & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            self._stop.wait(0.01)
+
+    def __enter__(self):
+        if self.nv is not None:
+            self._thr = threading.Thread(target=self._run, daemon=True)
+            self._thr.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        if self._thr is not None:
+            self._thr.join()
+
+    def summary(self):
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": 0}
+        return {"sm_mhz": int(np.median(self.samples)), "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(self.samples)}
+
+
+# ---- rank plumbing (torch.distributed only when launched under torchrun) ---------------------------------------
+def dist_env():
+    return int(os.environ.get("RANK", 0)), int(os.environ.get("LOCAL_RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
+
+
+def reduce_over_ranks(dist, device, seconds, units, backend_is_gloo=False):
+    """Whole-job figure of N independent replicas: (max over ranks of the timed seconds, sum of units).
+    Separate from the timing code so that the world_size-2 gloo test can exercise it on CPU."""
+    import torch
+    t = torch.tensor([float(seconds)], dtype=torch.float64, device="cpu" if backend_is_gloo else device)
+    u = torch.tensor([float(units)], dtype=torch.float64, device="cpu" if backend_is_gloo else device)
+    if dist is not None and dist.is_initialized() and dist.get_world_size() > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(u.item())
+
+
+# ---- our arm ---------------------------------------------------------------------------------------------------
+def run_ours(args):
+    import torch
+    from paper_2606_17949_b200 import binding as rb       # raises if librouteb.so is missing: no fallback
+    from paper_2606_17949_b200 import synth
+    from paper_2606_17949_b200.router import Router
+
+    rank, local_rank, world = dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the decision path has no CPU fallback")
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        torch.cuda.set_device(local_rank)
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    dev = torch.device("cuda", local_rank if world > 1 else 0)
+    torch.cuda.set_device(dev)
+
+    cfg = synth.CONFIGS["C2"]
+    K, W = args.steps, max(args.warmup, 3)
+    sizes, elapsed, weights = c2_stream(cfg, W + K, seed_shift=rank)
+    n_req = sum(sizes)
+    bank = synth.make_bank(cfg, device=dev)
+    it = synth.make_instances(cfg.I, cfg.M)
+    queued, running = synth.make_state(cfg.I, it["cap"], cfg.seed)
+    allq = synth.make_queries(cfg, B=n_req, device=dev, stream=3 + 100 * rank)
+    allp = synth.make_prompt_len(cfg, B=n_req, device=dev, stream=4 + 100 * rank)
+    torch.cuda.synchronize()
+    rt = Router(bank["emb"], bank["quality"], bank["outlen"], cfg.k, store="bf16", max_batch=64, device=dev)
+    rt.set_instances(**it)
+    rt.set_state(queued, running)
+    offs = np.concatenate([[0], np.cumsum(sizes)]).astype(np.int64)
+    assign_dev = torch.empty(64, dtype=torch.int32, device=dev)
+    flush_buf = torch.ones(3 * L2_BYTES // 4, dtype=torch.float32, device=dev) if args.l2 == "flush" else None
+
+    def flush():
+        if flush_buf is not None:
+            with torch.cuda.stream(rt.stream):
+                flush_buf.sum()          # read-only sweep of 3x L2: evicts the bank without leaving dirty lines
+
+    def step_device(j):
+        B = sizes[j]
+        rb.rb_advance_state(rt.ctx, elapsed[j])
+        rb.rb_decide(rt.ctx, allq[offs[j]:offs[j + 1]], allp[offs[j]:offs[j + 1]], B, weights[j], assign_dev[:B])
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- leg 1: device-resident inputs, CUDA events per step on the library's stream ---------------------------
+    for j in range(W):
+        flush()
+        step_device(j)
+    barrier()
+    ev0 = [torch.cuda.Event(enable_timing=True) for _ in range(K)]
+    ev1 = [torch.cuda.Event(enable_timing=True) for _ in range(K)]
+    launches0 = rt.launch_count()
+    sampler = ClockSampler(dev.index or 0)
+    with sampler:
+        wall0 = time.perf_counter()
+        for j in range(K):
+            flush()
+            ev0[j].record(rt.stream)
+            step_device(W + j)
+            ev1[j].record(rt.stream)
+        barrier()
+        wall = time.perf_counter() - wall0
+        if wall < 0.5:   # keep the GPU under the same load a little longer so that the sampler sees it
+            t_end = time.perf_counter() + (0.5 - wall)
+            j = 0
+            while time.perf_counter() < t_end:
+                flush()
+                rb.rb_estimate(rt.ctx, allq[:sizes[0]], sizes[0])
+                j += 1
+            torch.cuda.synchronize()
+    launches = rt.launch_count() - launches0
+    step_ms = np.array([a.elapsed_time(b) for a, b in zip(ev0, ev1)])
+    dev_seconds = float(step_ms.sum()) / 1e3
+    timed_req = int(sum(sizes[W:W + K]))
+    t_max, units = reduce_over_ranks(dist, dev, dev_seconds, timed_req)
+    value = units / t_max
+
+    # ---- leg 2: end to end through the C ABI with pinned host buffers ------------------------------------------
+    q_host = allq[offs[W]:].cpu().pin_memory()
+    p_host = allp[offs[W]:].cpu().pin_memory()
+    a_host = torch.empty(64, dtype=torch.int32).pin_memory()
+    rt.set_state(queued, running)
+    hoff = offs[W:] - offs[W]
+    for j in range(3):
+        rb.rb_decide(rt.ctx, q_host[hoff[j]:hoff[j + 1]], p_host[hoff[j]:hoff[j + 1]], sizes[W + j], weights[W + j],
+                     a_host[:sizes[W + j]])
+    rt.set_state(queued, running)
+    barrier()
+    e2e_s = 0.0
+    for j in range(K):
+        flush()
+        rt.sync()
+        B = sizes[W + j]
+        t0 = time.perf_counter()
+        rb.rb_advance_state(rt.ctx, elapsed[W + j])
+        rb.rb_decide(rt.ctx, q_host[hoff[j]:hoff[j + 1]], p_host[hoff[j]:hoff[j + 1]], B, weights[W + j], a_host[:B])
+        e2e_s += time.perf_counter() - t0
+    barrier()
+    e2e_max, _ = reduce_over_ranks(dist, dev, e2e_s, timed_req)
+    h2d = float(np.mean([B * cfg.d * 4 + B * 4 + 16 for B in sizes[W:W + K]]))
+    d2h = float(np.mean([B * 4 for B in sizes[W:W + K]]))
+
+    # ---- leg 3: the dominant kernel alone (events around each stage; graph replay off) --------------------------
+    rt.set_state(queued, running)
+    rt.set_stage_timing(1)
+    scan_us, stage_sum = [], {}
+    nscan = min(K, 300)
+    for j in range(nscan):
+        flush()
+        step_device(W + j)
+        us = rt.stage_us()
+        scan_us.append(us["scan"])
+        for k_, v in us.items():
+            stage_sum[k_] = stage_sum.get(k_, 0.0) + v
+    rt.set_stage_timing(0)
+    hbm_peak, tf_peak, peak_src = measured_peaks()
+    mean_B = float(np.mean(sizes[W:W + nscan]))
+    scan_bytes = cfg.N * cfg.d * 2 + mean_B * cfg.d * 2
+    scan_mean_us = float(np.mean(scan_us))
+    achieved = scan_bytes / (scan_mean_us * 1e-6) / 1e9
+    roofline = {"bound": "hbm", "kernel": "scan_tc_kernel", "achieved": round(achieved, 1), "peak": hbm_peak,
+                "unit": "GB/s", "frac": round(achieved / hbm_peak, 4), "traffic": recorded_traffic("c2"),
+                "bytes_per_launch": int(scan_bytes), "launch_us": round(scan_mean_us, 2), "peak_source": peak_src,
+                "frac_of_nominal_8TBs": round(achieved / 8000.0, 4),
+                "stage_us_mean": {k_: round(v / nscan, 2) for k_, v in stage_sum.items()}}
+
+    out = {"metric": METRIC, "value": round(value, 1), "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+           "ms_per_step": round(t_max / K * 1e3, 5), "higher_is_better": True,
+           "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
+           "config": {"workload": "C2 paper-shaped stream (BASELINE.json configs[1])", "N": cfg.N, "d": cfg.d, "M": cfg.M,
+                      "I": cfg.I, "k": cfg.k, "B": "4..64 (mean %.1f)" % (timed_req / K), "bank": "bf16 153.6 MB",
+                      "arrivals": "Poisson 12 req/s (first half of the steps) and 30 req/s (second half)",
+                      "weights": "quality/latency/cost/balanced presets in turn", "rerank_slack": 6,
+                      "l2": "flushed before every step (read of a 3x-L2 buffer)" if args.l2 == "flush" else
+                      "warm (bank 153.6 MB vs 126 MB L2)", "graph": "CUDA graph replay per B",
+                      "parallelism": "replicas only" if world > 1 else "single GPU"},
+           "decision_us": {"mean": round(float(step_ms.mean()) * 1e3, 2), "p50": round(float(np.median(step_ms)) * 1e3, 2),
+                           "p99": round(float(np.percentile(step_ms, 99)) * 1e3, 2)},
+           "e2e": {"value": round(units / e2e_max, 1), "unit": UNIT, "h2d_bytes_per_step": round(h2d, 1),
+                   "d2h_bytes_per_step": round(d2h, 1), "us_per_decision": round(e2e_max / K * 1e6, 2)},
+           "gpu_launches": int(launches), "clocks": sampler.summary(), "roofline": roofline,
+           "paper_context": "paper: ~32 ms per decision at 12 req/s on its 96-core CPU host, encoder included (P:L7)"}
+
+    if rank == 0 and world == 1:
+        out["cpu_baseline"], out["parity"] = cpu_baseline_and_parity(args, cfg, bank, it, queued, running, rt, rb, synth)
+        rt.close()
+        del bank, rt, flush_buf
+        torch.cuda.empty_cache()
+        if not args.no_scan_c4:
+            out["scan_c4"] = scan_c4(synth, Router, dev, hbm_peak)
+    else:
+        rt.close()
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
+    if rank == 0:
+        print(json.dumps(out))
+    return out
+
+
+def cpu_baseline_and_parity(args, cfg, bank, it, queued, running, rt, rb, synth):
+    """The oracle on the host cores over the first windows of a C2 stream (about --cpu-seconds of work), and the
+    same windows through the CUDA path from the same start state; assignments compared decision by decision."""
+    import torch
+    from oracle import orc
+    sizes, elapsed, weights = c2_stream(cfg, 4096, seed_shift=50)
+    bank_np = bank_to_numpy(bank["emb"])
+    qn, ln = bank["quality"].cpu().numpy(), bank["outlen"].cpu().numpy()
+    inst = orc.Instances(**it)
+    dq, bq = queued.numpy().copy(), running.numpy().copy()
+    n_req = sum(sizes[:512])
+    allq = synth.make_queries(cfg, B=n_req, device="cpu", stream=93)
+    allp = synth.make_prompt_len(cfg, B=n_req, device="cpu", stream=94)
+    rt.set_state(queued, running)
+    a_dev = torch.empty(64, dtype=torch.int32)
+    off, done_req, same, t_cpu, n_dec = 0, 0, 0, 0.0, 0
+    while t_cpu < args.cpu_seconds and n_dec < 512:
+        B = sizes[n_dec]
+        q, p = allq[off:off + B].numpy(), allp[off:off + B].numpy()
+        t0 = time.perf_counter()
+        dq, bq = orc.advance_state(inst, dq, bq, np.float32(elapsed[n_dec]))
+        ref = orc.decide(bank_np, qn, ln, inst, dq, bq, q, p, weights[n_dec], cfg.k, store_dtype="bf16")
+        t_cpu += time.perf_counter() - t0
+        dq, bq = ref["queued"], ref["running"]
+        rb.rb_advance_state(rt.ctx, elapsed[n_dec])
+        rb.rb_decide(rt.ctx, allq[off:off + B].contiguous(), allp[off:off + B].contiguous(), B, weights[n_dec], a_dev[:B])
+        same += int(np.array_equal(a_dev[:B].numpy(), ref["assignment"]))
+        off += B
+        done_req += B
+        n_dec += 1
+    s = rt.get_state()
+    state_equal = bool(np.array_equal(s[0].numpy(), dq) and np.array_equal(s[1].numpy(), bq))
+    cpu = {"value": round(done_req / t_cpu, 2), "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle",
+           "sample": "first %d decisions (%d requests) of a C2 stream, full oracle (fp64-accumulated brute-force KNN "
+                     "+ aggregate + score + LPT), %.1f s" % (n_dec, done_req, t_cpu),
+           "ms_per_decision": round(t_cpu / n_dec * 1e3, 2)}
+    par = {"decisions": n_dec, "assignment_equal": same, "state_equal_after_stream": state_equal}
+    return cpu, par
+
+
+def scan_c4(synth, Router, dev, hbm_peak):
+    """BASELINE.json configs[3]: N=10M x d=384 bf16 bank (7.68 GB >> L2), B=64, k=10: the scan kernel alone."""
+    import torch
+    cfg = synth.CONFIGS["C4"]
+    bank = synth.make_bank(cfg, device=dev)
+    q = synth.make_queries(cfg, B=64, device=dev)
+    torch.cuda.synchronize()
+    rt = Router(bank["emb"], bank["quality"], bank["outlen"], cfg.k, store="bf16", max_batch=64, device=dev)
+    for _ in range(3):
+        rt.estimate(q)
+    rt.sync()
+    rt.set_stage_timing(1)
+    us = []
+    for _ in range(20):
+        rt.estimate(q)
+        us.append(rt.stage_us()["scan"])
+    rt.close()
+    t = float(np.mean(us))
+    nbytes = cfg.N * cfg.d * 2 + 64 * cfg.d * 2
+    ach = nbytes / (t * 1e-6) / 1e9
+    return {"workload": "C4 N=10M d=384 bf16 B=64 k=10", "kernel": "scan_tc_kernel", "launch_us": round(t, 1),
+            "bytes_per_launch": int(nbytes), "achieved": round(ach, 1), "unit": "GB/s", "peak": hbm_peak,
+            "frac": round(ach / hbm_peak, 4), "frac_of_nominal_8TBs": round(ach / 8000.0, 4),
+            "traffic": recorded_traffic("c4"), "l2": "bank 7.68 GB >> 126 MB L2"}
+
+
+# ---- reference arm = the oracle ---------------------------------------------------------------------------------
+def run_reference(args):
+    rank, _, world = dist_env()
+    if rank != 0:
+        return None
+    import torch
+    from oracle import orc
+    from paper_2606_17949_b200 import synth            # input generators only
+    cfg = synth.CONFIGS["C2"]
+    K, W = args.steps, max(args.warmup, 1)
+    bank = synth.make_bank(cfg, device="cpu")
+    bank_np = bank_to_numpy(bank["emb"])
+    qn, ln = bank["quality"].numpy(), bank["outlen"].numpy()
+    it = synth.make_instances(cfg.I, cfg.M)
+    inst = orc.Instances(**it)
+    queued, running = synth.make_state(cfg.I, it["cap"], cfg.seed)
+    dq, bq = queued.numpy().copy(), running.numpy().copy()
+    sizes, elapsed, weights = c2_stream(cfg, W + K)
+    # bounded sample: each step routes the first q requests of its window; q from a probe of one query
+    probe = synth.make_queries(cfg, B=1, device="cpu").numpy()
+    orc.knn(bank_np, probe, cfg.k)
+    t0 = time.perf_counter()
+    orc.knn(bank_np, probe, cfg.k)
+    t_query = time.perf_counter() - t0
+    budget = 150.0
+    q_per_step = int(max(1, min(64, budget / max(1e-9, t_query * (K + W)))))
+    sizes = [min(b, q_per_step) for b in sizes]
+    n_req = sum(sizes)
+    allq = synth.make_queries(cfg, B=n_req, device="cpu").numpy()
+    allp = synth.make_prompt_len(cfg, B=n_req, device="cpu").numpy()
+    offs = np.concatenate([[0], np.cumsum(sizes)]).astype(np.int64)
+
+    def step(j, dq, bq):
+        dq, bq = orc.advance_state(inst, dq, bq, np.float32(elapsed[j]))
+        ref = orc.decide(bank_np, qn, ln, inst, dq, bq, allq[offs[j]:offs[j + 1]], allp[offs[j]:offs[j + 1]],
+                         weights[j], cfg.k, store_dtype="bf16")
+        return ref["queued"], ref["running"]
+
+    for j in range(W):
+        dq, bq = step(j, dq, bq)
+    t0 = time.perf_counter()
+    for j in range(W, W + K):
+        dq, bq = step(j, dq, bq)
+    t = time.perf_counter() - t0
+    timed_req = int(sum(sizes[W:W + K]))
+    v = round(timed_req / t, 2)
+    sample = "each step = the first <=%d requests of its C2 window, full oracle on the host cores" % q_per_step
+    out = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+           "ms_per_step": round(t / K * 1e3, 3), "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+           "dtype": "f64 accumulate / f32", "data": "synthetic",
+           "config": {"workload": "C2 paper-shaped stream (BASELINE.json configs[1])", "N": cfg.N, "d": cfg.d, "M": cfg.M,
+                      "I": cfg.I, "k": cfg.k, "B": "<=%d per step (bounded sample)" % q_per_step},
+           "cpu_baseline": {"value": v, "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle", "sample": sample},
+           "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+           "gpu_launches": 0}
+    print(json.dumps(out))
+    return out
+
+
+def main(argv=None):
+    args = parse_args(argv)
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -28,6 +28,10 @@
 #include <numeric>
 #include <vector>
 
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
 namespace {
 
 // bfloat16 = upper 16 bits of binary32.  Round-to-nearest-even from binary32 (reading 4: the storage
@@ -59,6 +63,15 @@ inline double stored_value(const void* base, int dtype, int store, int64_t off) 
 }  // namespace
 
 extern "C" {
+
+// Threads the neighbour search uses (reported by bench.py's cpu_baseline as "cores"); no arithmetic.
+int orc_num_threads(void) {
+#ifdef _OPENMP
+  return omp_get_max_threads();
+#else
+  return 1;
+#endif
+}
 
 // Rounds n fp32 values to bf16 (RNE); out receives the raw 16-bit patterns.
 int orc_round_bf16(const float* in, uint16_t* out, int64_t n) {

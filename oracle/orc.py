@@ -47,6 +47,11 @@ def _i32(a):
     return np.ascontiguousarray(a, dtype=np.int32)
 
 
+def num_threads():
+    """Threads the oracle's neighbour search runs on (OpenMP default: all host cores)."""
+    return int(lib().orc_num_threads())
+
+
 def round_bf16(x):
     """fp32 array -> raw bf16 bit patterns (uint16), round-to-nearest-even."""
     x = _f32(x)
