@@ -56,6 +56,7 @@ def parse_args(argv=None):
     ap.add_argument("--l2", default="flush", choices=["flush", "warm"],
                     help="flush: read a 3x-L2 buffer before every timed step; warm: back-to-back steps")
     ap.add_argument("--no-scan-c4", action="store_true", help="skip the C4 (10M x 384) bank-scan roofline leg")
+    ap.add_argument("--skip-cpu", action="store_true", help="skip the cpu_baseline / parity leg (profiling runs)")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="budget of the cpu_baseline sample")
     return ap.parse_args(argv)
 
@@ -318,7 +319,9 @@ def run_ours(args):
            "paper_context": "paper: ~32 ms per decision at 12 req/s on its 96-core CPU host, encoder included (P:L7)"}
 
     if rank == 0 and world == 1:
-        out["cpu_baseline"], out["parity"] = cpu_baseline_and_parity(args, cfg, bank, it, queued, running, rt, rb, synth)
+        if not args.skip_cpu:
+            out["cpu_baseline"], out["parity"] = cpu_baseline_and_parity(args, cfg, bank, it, queued, running, rt, rb,
+                                                                         synth)
         rt.close()
         del bank, rt, flush_buf
         torch.cuda.empty_cache()
