@@ -1,5 +1,6 @@
 // estimate.cu -- the estimate stage around the tensor-core scan: query staging (a0), the exact fp32-storage
-// scan (a1, small banks), the cross-CTA top-k merge (a2) and the re-rank + aggregate kernel (a3).
+// scan (a1, small banks), and the per-query finishing kernel: cross-CTA top-k merge (a2), exact re-rank +
+// distance-weighted aggregate (a3) and the per-(request, tier) score terms (a4).
 // Citations: P:L115 (§4.2 "Model estimator"); readings 1-8 and "Canonical arithmetic".
 #include "rb_internal.cuh"
 
@@ -18,18 +19,20 @@ __device__ __forceinline__ float f32_unordered(uint32_t o) {
 __device__ __forceinline__ unsigned long long make_key(float sim, int32_t idx) {
   return ((unsigned long long)f32_ordered(sim) << 32) | (unsigned long long)(0xffffffffu - (uint32_t)idx);
 }
-__device__ __forceinline__ unsigned long long shfl64(unsigned long long x, int src) {
-  return __shfl_sync(0xffffffffu, x, src);
-}
-__device__ __forceinline__ unsigned long long shfl64_up1(unsigned long long x) { return __shfl_up_sync(0xffffffffu, x, 1); }
 
 // ---- a0 ---------------------------------------------------------------------------------------------
-__global__ void stage_queries_kernel(const float* __restrict__ q, __nv_bfloat16* __restrict__ qs, int B, int Bpad, int d) {
+__global__ void stage_queries_kernel(const CallParams* __restrict__ cp, __nv_bfloat16* __restrict__ qs, int B, int Bpad,
+                                     int d) {
+  const float* __restrict__ q = cp->query;
   const size_t n = (size_t)Bpad * d;
   for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
     const size_t r = i / d;
     qs[i] = (r < (size_t)B) ? __float2bfloat16_rn(q[i]) : __float2bfloat16_rn(0.0f);
   }
+}
+__global__ void convert_bf16_kernel(const float* __restrict__ in, __nv_bfloat16* __restrict__ out, size_t n) {
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x)
+    out[i] = __float2bfloat16_rn(in[i]);
 }
 
 // ---- a1, fp32 storage -----------------------------------------------------------------------------------
@@ -39,8 +42,10 @@ constexpr int kF32Rows = 128;   // bank rows per block, one per thread
 constexpr int kF32Q = 8;        // queries per register group
 constexpr int kF32Chunk = 64;   // columns staged per step
 __global__ void __launch_bounds__(kF32Rows)
-scan_f32_kernel(const float* __restrict__ bank, const float* __restrict__ q, int64_t N, int d, int nq, float* __restrict__ sims) {
+scan_f32_kernel(const float* __restrict__ bank, const CallParams* __restrict__ cp, int r0, int64_t N, int d, int nq,
+                float* __restrict__ sims) {
   __shared__ float xs[kF32Q][kF32Chunk];
+  const float* __restrict__ q = cp->query + (size_t)r0 * d;
   const int64_t n = (int64_t)blockIdx.x * kF32Rows + threadIdx.x;
   const float* row = bank + (n < N ? n : N - 1) * (int64_t)d;
   for (int q0 = 0; q0 < nq; q0 += kF32Q) {
@@ -115,88 +120,79 @@ select_f32_kernel(const float* __restrict__ sims, int64_t N, int kc, float* __re
   }
 }
 
-// ---- a2 ---------------------------------------------------------------------------------------------
-// One warp per query.  The running best-kc list lives across the warp (rank l in lane l, rank 32+l in the
-// second register); candidates stream in 32 at a time, survivors of the threshold are inserted one by one
-// with ballots and shuffles.  part_* layout: [grid][kcap][Bpad].
-__global__ void __launch_bounds__(128)
-merge_kernel(const float* __restrict__ part_sim, const int32_t* __restrict__ part_idx, int grid, int kcap, int Bpad, int B,
-             int kc, int64_t N, float* __restrict__ cand_sim, int32_t* __restrict__ cand_idx) {
-  const int r = blockIdx.x * 4 + (threadIdx.x >> 5);
-  const int lane = threadIdx.x & 31;
-  if (r >= B) return;
-  unsigned long long a = 0, b = 0;   // ranks lane and 32+lane, descending
-  unsigned long long thr = 0;        // key of rank kc-1
-  const int total = grid * kcap;
-  for (int base = 0; base < total; base += 32) {
-    const int e = base + lane;
-    unsigned long long key = 0;
-    if (e < total) {
-      const size_t off = (size_t)e * Bpad + r;
-      const int32_t id = part_idx[off];
-      if (id >= 0 && (int64_t)id < N) key = make_key(part_sim[off], id);
-    }
-    unsigned mask = __ballot_sync(0xffffffffu, key > thr);
-    while (mask) {
-      const int src = __ffs(mask) - 1;
-      mask &= mask - 1;
-      const unsigned long long x = shfl64(key, src);
-      if (x > thr) {
-        const int p = __popc(__ballot_sync(0xffffffffu, a > x)) + __popc(__ballot_sync(0xffffffffu, b > x));
-        const unsigned long long a_up = shfl64_up1(a), b_up = shfl64_up1(b), a_last = shfl64(a, 31);
-        const unsigned long long b_prev = (lane == 0) ? a_last : b_up;
-        a = (lane < p) ? a : ((lane == p) ? x : a_up);
-        b = (lane + 32 < p) ? b : ((lane + 32 == p) ? x : b_prev);
-        thr = (kc <= 32) ? shfl64(a, kc - 1) : shfl64(b, kc - 33);
-      }
-    }
-  }
-  for (int j = lane; j < kc; j += 32) {
-    const unsigned long long key = (j < 32) ? a : b;
-    const size_t o = (size_t)r * kc + j;
-    if (key == 0) {
-      cand_sim[o] = -INFINITY;
-      cand_idx[o] = -1;
-    } else {
-      cand_sim[o] = f32_unordered((uint32_t)(key >> 32));
-      cand_idx[o] = (int32_t)(0xffffffffu - (uint32_t)key);
-    }
-  }
-}
-
-// ---- a3 ---------------------------------------------------------------------------------------------
-// One block per query.  Optional exact re-rank (bf16 storage): the kc candidates' similarities are recomputed
-// from the stored bf16 rows with fp64 accumulation (products of bf16 values are exact), rounded once to fp32,
-// and re-ordered by (s desc, n asc); the best k are the neighbours.  Then:
-//   t = 2*s; u = 2 - t; u = max(u,0); dist = sqrt(u); w = 1/(dist + eps)      (uniform mode: w = 1)
-//   num_m = sum_j w_j*label[n_j,m] (j ascending, multiply then add); den = sum_j w_j; pred = num/den
-constexpr int kAggThreads = 256;
-__global__ void __launch_bounds__(kAggThreads)
-aggregate_kernel(const __nv_bfloat16* __restrict__ bank, const __nv_bfloat16* __restrict__ qs, int d, int rerank,
-                 const float* __restrict__ cand_sim, const int32_t* __restrict__ cand_idx, int kc, int k,
-                 const float* __restrict__ bank_quality, const float* __restrict__ bank_outlen, int M, int weight_mode,
-                 float eps, int32_t* __restrict__ nn_idx, float* __restrict__ nn_sim, float* __restrict__ pred_q,
-                 float* __restrict__ pred_l) {
+// ---- a2 + a3 + a4 ---------------------------------------------------------------------------------------
+// One CTA per query.
+//  merge   the nlists partial lists (each sorted by key, descending) are copied to shared memory as 64-bit
+//          keys; thread c owns list c and exposes its head; kc rounds of a block-wide maximum (REDUX on the
+//          high and low words, one barrier per round) pop the kc best in order.
+//  re-rank (bf16 storage): the kc candidates' similarities are recomputed from the stored bf16 rows with fp64
+//          accumulation (products of bf16 values are exact), rounded once to fp32, re-ordered by
+//          (s desc, n asc); the best k are the neighbours.
+//  aggregate:
+//          t = 2*s; u = 2 - t; u = max(u,0); dist = sqrt(u); w = 1/(dist + eps)      (uniform mode: w = 1)
+//          num_m = sum_j w_j*label[n_j,m] (j ascending, multiply then add); den = sum_j w_j; pred = num/den
+//  terms   (with_terms; Eq. 2, Eq. 1):
+//          c1 = (float)l*pin; c2 = L*pout; C = c1 + c2; Cmax over tiers that have an instance;
+//          ct = Cmax > 0 ? 1 - C/Cmax : 0; A = wq*Q + wc*ct; P = pre*(float)l; key = max_m L
+constexpr int kFinThreads = 512;
+__global__ void __launch_bounds__(kFinThreads)
+finish_kernel(FinishArgs a, InstTable t, const CallParams* __restrict__ cp) {
+  extern __shared__ unsigned long long s_keys[];   // [nlists][kcap]
+  __shared__ uint32_t s_red[2][kFinThreads / 32][2];
   __shared__ float s_sim[kMaxK];
   __shared__ int32_t s_idx[kMaxK];
   __shared__ float o_sim[kMaxK];
   __shared__ int32_t o_idx[kMaxK];
   __shared__ float s_w[kMaxK];
+  __shared__ float sQ[kMaxM], sL[kMaxM], sC[kMaxM];
   const int r = blockIdx.x;
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nwarps = kAggThreads / 32;
-  if (threadIdx.x < kc) {
-    s_sim[threadIdx.x] = cand_sim[(size_t)r * kc + threadIdx.x];
-    s_idx[threadIdx.x] = cand_idx[(size_t)r * kc + threadIdx.x];
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  constexpr int nwarps = kFinThreads / 32;
+  const int kc = a.kc, k = a.k, kcap = a.kcap, M = a.M;
+
+  // ---- merge ----
+  const int total = a.nlists * kcap;
+  for (int e = tid; e < total; e += kFinThreads) {
+    const int c = e / kcap, j = e - c * kcap;
+    const size_t off = ((size_t)c * a.Bpad + r) * kcap + j;
+    const int32_t id = a.part_idx[off];
+    s_keys[e] = (id >= 0 && (int64_t)id < a.N) ? make_key(a.part_sim[off], id) : 0ull;
   }
   __syncthreads();
-  if (rerank) {
-    const uint4* qrow = reinterpret_cast<const uint4*>(qs + (size_t)r * d);
-    const int nvec = d / 8;   // d % 8 == 0
+  int pos = 0;
+  unsigned long long hk = (tid < a.nlists) ? s_keys[(size_t)tid * kcap] : 0ull;
+  for (int j = 0; j < kc; ++j) {
+    const uint32_t hi = (uint32_t)(hk >> 32), lo = (uint32_t)hk;
+    const uint32_t whi = __reduce_max_sync(0xffffffffu, hi);
+    const uint32_t wlo = __reduce_max_sync(0xffffffffu, hi == whi ? lo : 0u);
+    if (lane == 0) { s_red[j & 1][warp][0] = whi; s_red[j & 1][warp][1] = wlo; }
+    __syncthreads();
+    const uint32_t xhi = lane < nwarps ? s_red[j & 1][lane][0] : 0u;
+    const uint32_t xlo = lane < nwarps ? s_red[j & 1][lane][1] : 0u;
+    const uint32_t ghi = __reduce_max_sync(0xffffffffu, xhi);
+    const uint32_t glo = __reduce_max_sync(0xffffffffu, xhi == ghi ? xlo : 0u);
+    const unsigned long long win = ((unsigned long long)ghi << 32) | glo;
+    if (win != 0ull && hk == win) {   // keys are distinct: exactly one owner
+      ++pos;
+      hk = pos < kcap ? s_keys[(size_t)tid * kcap + pos] : 0ull;
+    }
+    if (tid == 0) {
+      s_sim[j] = win ? f32_unordered(ghi) : -INFINITY;
+      s_idx[j] = win ? (int32_t)(0xffffffffu - glo) : -1;
+    }
+  }
+  __syncthreads();
+
+  // ---- exact re-rank ----
+  if (a.rerank) {
+    const uint4* qrow = reinterpret_cast<const uint4*>(a.qs + (size_t)r * a.d);
+    const int nvec = a.d / 8;   // d % 8 == 0
     for (int c = warp; c < kc; c += nwarps) {
       const int32_t id = s_idx[c];
       if (id < 0) continue;
-      const uint4* brow = reinterpret_cast<const uint4*>(bank + (size_t)id * d);
+      const uint4* brow = reinterpret_cast<const uint4*>(a.bank + (size_t)id * a.d);
       double acc = 0.0;
+#pragma unroll 4
       for (int vidx = lane; vidx < nvec; vidx += 32) {
         const uint4 xb = qrow[vidx], eb = brow[vidx];
         const __nv_bfloat162* xp = reinterpret_cast<const __nv_bfloat162*>(&xb);
@@ -214,39 +210,41 @@ aggregate_kernel(const __nv_bfloat16* __restrict__ bank, const __nv_bfloat16* __
     __syncthreads();
   }
   // rank by counting (keys are distinct because indices are)
-  if (threadIdx.x < kc) {
-    const int32_t id = s_idx[threadIdx.x];
-    const unsigned long long me = (id < 0) ? 0ull : make_key(s_sim[threadIdx.x], id);
+  if (tid < kc) {
+    const int32_t id = s_idx[tid];
+    const unsigned long long me = (id < 0) ? 0ull : make_key(s_sim[tid], id);
     int rank = 0;
     for (int j = 0; j < kc; ++j) {
       const int32_t oj = s_idx[j];
       const unsigned long long other = (oj < 0) ? 0ull : make_key(s_sim[j], oj);
-      rank += (other > me) || (other == me && j < (int)threadIdx.x);
+      rank += (other > me) || (other == me && j < tid);
     }
-    o_sim[rank] = s_sim[threadIdx.x];
+    o_sim[rank] = s_sim[tid];
     o_idx[rank] = id;
   }
   __syncthreads();
-  if (threadIdx.x < k) {
-    const float s = o_sim[threadIdx.x];
+  // ---- weights ----
+  if (tid < k) {
+    const float s = o_sim[tid];
     float w = 1.0f;
-    if (o_idx[threadIdx.x] < 0) {
+    if (o_idx[tid] < 0) {
       w = 0.0f;   // fewer than k rows reachable (cannot happen for k <= N); keeps the gather in bounds
-    } else if (weight_mode == 0) {
-      const float t = __fmul_rn(2.0f, s);
-      float u = __fsub_rn(2.0f, t);
+    } else if (a.weight_mode == 0) {
+      const float tt = __fmul_rn(2.0f, s);
+      float u = __fsub_rn(2.0f, tt);
       u = fmaxf(u, 0.0f);
       const float dist = __fsqrt_rn(u);
-      w = __fdiv_rn(1.0f, __fadd_rn(dist, eps));
+      w = __fdiv_rn(1.0f, __fadd_rn(dist, a.eps));
     }
-    s_w[threadIdx.x] = w;
-    if (nn_idx) nn_idx[(size_t)r * k + threadIdx.x] = o_idx[threadIdx.x];
-    if (nn_sim) nn_sim[(size_t)r * k + threadIdx.x] = s;
+    s_w[tid] = w;
+    if (cp->nn_idx) cp->nn_idx[(size_t)r * k + tid] = o_idx[tid];
+    if (cp->nn_sim) cp->nn_sim[(size_t)r * k + tid] = s;
   }
   __syncthreads();
-  if (threadIdx.x < 2 * M) {
-    const int m = threadIdx.x % M;
-    const float* lab = (threadIdx.x < M) ? bank_quality : bank_outlen;
+  // ---- aggregate: thread m < M -> quality, M <= thread < 2M -> output length ----
+  if (tid < 2 * M) {
+    const int m = tid % M;
+    const float* lab = (tid < M) ? a.bank_quality : a.bank_outlen;
     float num = 0.0f, den = 0.0f;
     for (int j = 0; j < k; ++j) {
       const float w = s_w[j];
@@ -256,24 +254,60 @@ aggregate_kernel(const __nv_bfloat16* __restrict__ bank, const __nv_bfloat16* __
       den = __fadd_rn(den, w);
     }
     const float pred = __fdiv_rn(num, den);
-    if (threadIdx.x < M) pred_q[(size_t)r * M + m] = pred;
-    else pred_l[(size_t)r * M + m] = pred;
+    if (tid < M) {
+      sQ[m] = pred;
+      a.pred_q[(size_t)r * M + m] = pred;
+      if (cp->pred_q) cp->pred_q[(size_t)r * M + m] = pred;
+    } else {
+      sL[m] = pred;
+      a.pred_l[(size_t)r * M + m] = pred;
+      if (cp->pred_l) cp->pred_l[(size_t)r * M + m] = pred;
+    }
+  }
+  if (!a.with_terms) return;
+  __syncthreads();
+  // ---- per-(request, tier) terms ----
+  const float ell = (float)cp->plen[r];
+  if (tid < M) sC[tid] = __fadd_rn(__fmul_rn(ell, t.price_in[tid]), __fmul_rn(sL[tid], t.price_out[tid]));
+  __syncthreads();
+  if (tid < M) {
+    const int m = tid;
+    float Cmax = 0.0f, kmax = 0.0f;
+    bool first = true;
+    for (int j = 0; j < M; ++j) {
+      if (!t.present[j]) continue;
+      if (first || sC[j] > Cmax) Cmax = sC[j];
+      if (first || sL[j] > kmax) kmax = sL[j];
+      first = false;
+    }
+    const float ct = (Cmax > 0.0f) ? __fsub_rn(1.0f, __fdiv_rn(sC[m], Cmax)) : 0.0f;
+    a.termA[(size_t)r * M + m] = __fadd_rn(__fmul_rn(cp->w_qual, sQ[m]), __fmul_rn(cp->w_cost, ct));
+    a.termP[(size_t)r * M + m] = __fmul_rn(t.pre[m], ell);
+    if (m == 0) a.key[r] = __fadd_rn(kmax, 0.0f);   // -0 -> +0 so that the sort key order equals float order
   }
 }
 
 }  // namespace
 
-cudaError_t launch_stage_queries(const float* q, __nv_bfloat16* qs, int B, int Bpad, int d, cudaStream_t s) {
-  const size_t n = (size_t)Bpad * d;
-  int blocks = (int)((n + 255) / 256);
-  if (blocks > 148 * 8) blocks = 148 * 8;
-  stage_queries_kernel<<<blocks, 256, 0, s>>>(q, qs, B, Bpad, d);
+cudaError_t launch_convert_bf16(const float* in, __nv_bfloat16* out, size_t n, cudaStream_t s) {
+  size_t blocks = (n + 255) / 256;
+  if (blocks > 148 * 16) blocks = 148 * 16;
+  convert_bf16_kernel<<<(int)blocks, 256, 0, s>>>(in, out, n);
   return cudaGetLastError();
 }
 
-cudaError_t launch_scan_f32(const float* bank, const float* q, int64_t N, int d, int nq, float* sims, cudaStream_t s) {
+cudaError_t launch_stage_queries(const CallParams* cp, __nv_bfloat16* qs, int B, int Bpad, int d, cudaStream_t s) {
+  const size_t n = (size_t)Bpad * d;
+  int blocks = (int)((n + 255) / 256);
+  if (blocks > 148 * 8) blocks = 148 * 8;
+  stage_queries_kernel<<<blocks, 256, 0, s>>>(cp, qs, B, Bpad, d);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_scan_f32(const float* bank, const CallParams* cp, int r0, int64_t N, int d, int nq, float* sims,
+                            cudaStream_t s) {
   const int blocks = (int)((N + kF32Rows - 1) / kF32Rows);
-  scan_f32_kernel<<<blocks, kF32Rows, 0, s>>>(bank, q, N, d, nq, sims);
+  scan_f32_kernel<<<blocks, kF32Rows, 0, s>>>(bank, cp, r0, N, d, nq, sims);
   return cudaGetLastError();
 }
 
@@ -283,18 +317,14 @@ cudaError_t launch_select_f32(const float* sims, int64_t N, int nq, int kc, floa
   return cudaGetLastError();
 }
 
-cudaError_t launch_merge(const float* part_sim, const int32_t* part_idx, int grid, int kcap, int Bpad, int B, int kc,
-                         int64_t N, float* cand_sim, int32_t* cand_idx, cudaStream_t s) {
-  merge_kernel<<<(B + 3) / 4, 128, 0, s>>>(part_sim, part_idx, grid, kcap, Bpad, B, kc, N, cand_sim, cand_idx);
-  return cudaGetLastError();
+size_t finish_smem_bytes(int nlists, int kcap) { return (size_t)nlists * kcap * sizeof(unsigned long long); }
+
+cudaError_t finish_prepare(size_t max_smem) {
+  return cudaFuncSetAttribute(finish_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)max_smem);
 }
 
-cudaError_t launch_aggregate(const __nv_bfloat16* bank, const __nv_bfloat16* qs, int d, int rerank, const float* cand_sim,
-                             const int32_t* cand_idx, int kc, int k, const float* bank_quality, const float* bank_outlen,
-                             int M, int weight_mode, float eps, int B, int32_t* nn_idx, float* nn_sim, float* pred_q,
-                             float* pred_l, cudaStream_t s) {
-  aggregate_kernel<<<B, kAggThreads, 0, s>>>(bank, qs, d, rerank, cand_sim, cand_idx, kc, k, bank_quality, bank_outlen, M,
-                                             weight_mode, eps, nn_idx, nn_sim, pred_q, pred_l);
+cudaError_t launch_finish(const FinishArgs& a, InstTable t, const CallParams* cp, int B, cudaStream_t s) {
+  finish_kernel<<<B, kFinThreads, finish_smem_bytes(a.nlists, a.kcap), s>>>(a, t, cp);
   return cudaGetLastError();
 }
 

@@ -50,9 +50,10 @@ struct rb_ctx {
   float* sims = nullptr;            // fp32 storage only: [kF32Group x N]
   float* cand_sim = nullptr;        // [max_batch x kc]
   int32_t* cand_idx = nullptr;
-  int32_t* nn_idx = nullptr;        // [max_batch x k]
-  float* nn_sim = nullptr;
-  float *pred_q = nullptr, *pred_l = nullptr;   // [max_batch x M]
+  int32_t* scratch_nn_idx = nullptr;   // [max_batch x k] staging for host callers
+  float* scratch_nn_sim = nullptr;
+  float *pred_q = nullptr, *pred_l = nullptr;   // [max_batch x M] the estimate, consumed by score/dispatch
+  float *stage_q = nullptr, *stage_l = nullptr; // [max_batch x M] staging of caller-supplied predictions (host)
   float *termA = nullptr, *termP = nullptr, *key = nullptr;
   int32_t *order = nullptr, *assignment = nullptr;
   float *scores = nullptr, *scores0 = nullptr;  // [max_batch x I], allocated by rb_set_instances
@@ -156,54 +157,59 @@ struct Timer {
   }
 };
 
-rb_status enqueue_estimate(rb_ctx* ctx, int B, Timer& tm) {
+// with_terms: the finishing kernel also derives the score terms (rb_decide); otherwise estimate only.
+rb_status enqueue_estimate(rb_ctx* ctx, int B, bool with_terms, Timer& tm) {
   cudaStream_t s = ctx->stream;
   const int Bpad = (B + kTileM - 1) / kTileM * kTileM;
+  FinishArgs fa{};
+  fa.kc = ctx->kc; fa.k = ctx->k; fa.N = ctx->N; fa.d = ctx->d;
+  fa.bank_quality = ctx->bank_quality; fa.bank_outlen = ctx->bank_outlen; fa.M = ctx->M;
+  fa.weight_mode = ctx->opt.weight_mode; fa.eps = ctx->opt.dist_eps; fa.with_terms = with_terms ? 1 : 0;
+  fa.pred_q = ctx->pred_q; fa.pred_l = ctx->pred_l; fa.termA = ctx->termA; fa.termP = ctx->termP; fa.key = ctx->key;
   if (ctx->opt.store_dtype == RB_BF16) {
     tm.mark();
-    CK(launch_stage_queries(ctx->q32, ctx->qs, B, Bpad, ctx->d, s));
+    CK(launch_stage_queries(ctx->cp, ctx->qs, B, Bpad, ctx->d, s));
     tm.mark();
     int grid = 0;
     CK(launch_scan_tc(&ctx->tm_q, &ctx->tm_bank, ctx->N, ctx->d, B, Bpad, ctx->kcap, ctx->num_sms, ctx->part_sim,
                       ctx->part_idx, &grid, s));
     tm.mark();
-    CK(launch_merge(ctx->part_sim, ctx->part_idx, grid, ctx->kcap, Bpad, B, ctx->kc, ctx->N, ctx->cand_sim, ctx->cand_idx, s));
-    tm.mark();
-    CK(launch_aggregate((const __nv_bfloat16*)ctx->bank, ctx->qs, ctx->d, ctx->opt.rerank_slack > 0 ? 1 : 0, ctx->cand_sim,
-                        ctx->cand_idx, ctx->kc, ctx->k, ctx->bank_quality, ctx->bank_outlen, ctx->M, ctx->opt.weight_mode,
-                        ctx->opt.dist_eps, B, ctx->nn_idx, ctx->nn_sim, ctx->pred_q, ctx->pred_l, s));
-    ctx->launches += 4;
+    fa.part_sim = ctx->part_sim; fa.part_idx = ctx->part_idx; fa.nlists = grid; fa.kcap = ctx->kcap; fa.Bpad = Bpad;
+    fa.bank = (const __nv_bfloat16*)ctx->bank; fa.qs = ctx->qs; fa.rerank = ctx->opt.rerank_slack > 0 ? 1 : 0;
+    ctx->launches += 2;
   } else {
     tm.mark();
     tm.mark();
     for (int r0 = 0; r0 < B; r0 += kF32Group) {
       const int nq = (B - r0 < kF32Group) ? (B - r0) : kF32Group;
-      CK(launch_scan_f32((const float*)ctx->bank, ctx->q32 + (size_t)r0 * ctx->d, ctx->N, ctx->d, nq, ctx->sims, s));
+      CK(launch_scan_f32((const float*)ctx->bank, ctx->cp, r0, ctx->N, ctx->d, nq, ctx->sims, s));
       CK(launch_select_f32(ctx->sims, ctx->N, nq, ctx->kc, ctx->cand_sim + (size_t)r0 * ctx->kc,
                            ctx->cand_idx + (size_t)r0 * ctx->kc, s));
       ctx->launches += 2;
     }
     tm.mark();
-    tm.mark();
-    CK(launch_aggregate(nullptr, nullptr, ctx->d, 0, ctx->cand_sim, ctx->cand_idx, ctx->kc, ctx->k, ctx->bank_quality,
-                        ctx->bank_outlen, ctx->M, ctx->opt.weight_mode, ctx->opt.dist_eps, B, ctx->nn_idx, ctx->nn_sim,
-                        ctx->pred_q, ctx->pred_l, s));
-    ctx->launches += 1;
+    // the selected candidates are one already-merged list per query: [1][B][kc]
+    fa.part_sim = ctx->cand_sim; fa.part_idx = ctx->cand_idx; fa.nlists = 1; fa.kcap = ctx->kc; fa.Bpad = B;
+    fa.bank = nullptr; fa.qs = nullptr; fa.rerank = 0;
   }
+  CK(launch_finish(fa, table_of(ctx), ctx->cp, B, s));
+  ctx->launches += 1;
   tm.mark();
   return RB_OK;
 }
 
-rb_status enqueue_dispatch(rb_ctx* ctx, int B, bool want_scores0, Timer& tm) {
+rb_status enqueue_dispatch(rb_ctx* ctx, int B, bool from_predictions, Timer& tm) {
   cudaStream_t s = ctx->stream;
   InstTable t = table_of(ctx);
-  CK(launch_score(t, ctx->dq, ctx->bq, ctx->pred_q, ctx->pred_l, ctx->plen, ctx->cp, B, ctx->termA, ctx->termP, ctx->key,
-                  want_scores0 ? ctx->scores0 : nullptr, s));
+  if (from_predictions) {
+    CK(launch_score(t, ctx->dq, ctx->bq, ctx->cp, B, ctx->termA, ctx->termP, ctx->key, s));
+    ctx->launches += 1;
+  }
   tm.mark();
-  CK(launch_dispatch(t, ctx->dq, ctx->bq, ctx->pred_l, ctx->termA, ctx->termP, ctx->key, ctx->cp, B, ctx->opt.lpt_enabled,
-                     ctx->opt.update_enabled, ctx->order, ctx->assignment, ctx->scores, s));
+  CK(launch_lpt_dispatch(t, ctx->dq, ctx->bq, ctx->termA, ctx->termP, ctx->key, ctx->cp, B, ctx->opt.lpt_enabled,
+                         ctx->opt.update_enabled, s));
   tm.mark();
-  ctx->launches += 3;
+  ctx->launches += 1;
   return RB_OK;
 }
 
@@ -213,7 +219,7 @@ rb_status run_path(rb_ctx* ctx, int B, int kind) {
   Timer tm(ctx);
   if (!graph) {
     if (kind != 2) {
-      rb_status st = enqueue_estimate(ctx, B, tm);
+      rb_status st = enqueue_estimate(ctx, B, kind == 0, tm);
       if (st != RB_OK) return st;
     }
     if (kind != 1) return enqueue_dispatch(ctx, B, kind == 2, tm);
@@ -226,7 +232,7 @@ rb_status run_path(rb_ctx* ctx, int B, int kind) {
     cudaGraph_t g = nullptr;
     CK(cudaStreamBeginCapture(ctx->stream, cudaStreamCaptureModeThreadLocal));
     rb_status st = RB_OK;
-    if (kind != 2) st = enqueue_estimate(ctx, B, tm);
+    if (kind != 2) st = enqueue_estimate(ctx, B, kind == 0, tm);
     if (st == RB_OK && kind != 1) st = enqueue_dispatch(ctx, B, kind == 2, tm);
     cudaError_t e = cudaStreamEndCapture(ctx->stream, &g);
     const int nodes = (int)(ctx->launches - before);
@@ -252,18 +258,21 @@ void collect_stage_times(rb_ctx* ctx, int kind) {
   if (!ctx->stage_timing) return;
   cudaStreamSynchronize(ctx->stream);
   for (float& v : ctx->stage_us) v = 0.0f;
-  // marks: estimate = 5 (4 intervals: stage, scan, merge, aggregate), dispatch = 2 more (score, dispatch)
-  const int first = (kind == 2) ? 4 : 0;
-  const int n_int = (kind == 0) ? 6 : (kind == 1 ? 4 : 2);
-  // kind 2 has no leading mark: its first interval start is unknown -> only the dispatch interval is reported
-  if (kind == 2) {
+  auto span = [&](int e0, int e1) {
     float ms = 0;
-    if (cudaEventElapsedTime(&ms, ctx->ev[0], ctx->ev[1]) == cudaSuccess) ctx->stage_us[5] = ms * 1000.0f;
-    return;
-  }
-  for (int j = 0; j < n_int; ++j) {
-    float ms = 0;
-    if (cudaEventElapsedTime(&ms, ctx->ev[j], ctx->ev[j + 1]) == cudaSuccess) ctx->stage_us[first + j] = ms * 1000.0f;
+    return cudaEventElapsedTime(&ms, ctx->ev[e0], ctx->ev[e1]) == cudaSuccess ? ms * 1000.0f : 0.0f;
+  };
+  // marks: estimate = 4 events (stage | scan | merge+aggregate), then dispatch = 2 more (score | dispatch)
+  if (kind != 2) {
+    ctx->stage_us[0] = span(0, 1);
+    ctx->stage_us[1] = span(1, 2);
+    ctx->stage_us[3] = span(2, 3);   // merge is fused into the finishing kernel: reported under "aggregate"
+    if (kind == 0) {
+      ctx->stage_us[4] = span(3, 4);
+      ctx->stage_us[5] = span(4, 5);
+    }
+  } else {
+    ctx->stage_us[5] = span(0, 1);   // no mark precedes the score kernel: only the dispatch interval is known
   }
 }
 
@@ -278,19 +287,48 @@ rb_status push_params(rb_ctx* ctx, const CallParams& cp) {
   return RB_OK;
 }
 
-struct CopyBack {
+// Resolves caller buffers into device pointers for the parameter block.  Host inputs are copied into the
+// context's staging buffer first; host outputs are produced in the staging buffer and copied back after the
+// kernels (Stager::finish).
+struct Stager {
   rb_ctx* ctx;
   bool any_host = false;
   cudaError_t err = cudaSuccess;
-  void out(void* dst, const void* src, size_t bytes) {
-    if (!dst || err != cudaSuccess) return;
-    any_host |= is_host_ptr(dst);
-    err = cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDefault, ctx->stream);
+  struct Back { void* dst; const void* src; size_t bytes; };
+  Back back[8];
+  int nback = 0;
+  template <typename T>
+  const T* in(const T* user, T* staging, size_t bytes) {
+    if (!is_host_ptr(user)) return user;
+    any_host = true;
+    if (err == cudaSuccess) err = cudaMemcpyAsync(staging, user, bytes, cudaMemcpyHostToDevice, ctx->stream);
+    return staging;
   }
-  void in(void* dst, const void* src, size_t bytes) {
-    if (err != cudaSuccess) return;
-    any_host |= is_host_ptr(src);
-    err = cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDefault, ctx->stream);
+  template <typename T>
+  T* out(T* user, T* staging, size_t bytes) {
+    if (!user) return nullptr;
+    if (!is_host_ptr(user)) return user;
+    any_host = true;
+    back[nback++] = Back{user, staging, bytes};
+    return staging;
+  }
+  // an output that the kernels always produce in `internal`: device callers get an extra copy through the
+  // parameter block, host callers a D2H copy afterwards
+  template <typename T>
+  T* out_internal(T* user, T* internal, size_t bytes) {
+    if (!user) return nullptr;
+    if (!is_host_ptr(user)) return user;
+    any_host = true;
+    back[nback++] = Back{user, internal, bytes};
+    return nullptr;
+  }
+  rb_status finish() {
+    for (int j = 0; j < nback && err == cudaSuccess; ++j)
+      err = cudaMemcpyAsync(back[j].dst, back[j].src, back[j].bytes, cudaMemcpyDeviceToHost, ctx->stream);
+    if (err != cudaSuccess) return fail(ctx, RB_ECUDA, "cudaMemcpyAsync (outputs)", err);
+    // host-side inputs must be consumed and host-side outputs complete before returning
+    if (any_host) CK(cudaStreamSynchronize(ctx->stream));
+    return RB_OK;
   }
 };
 
@@ -378,9 +416,7 @@ rb_status rb_create(rb_ctx** out, const void* bank_emb, const float* bank_qualit
       for (size_t r0 = 0; r0 < (size_t)N; r0 += chunk_rows) {
         const size_t rows = std::min(chunk_rows, (size_t)N - r0);
         CK(cudaMemcpyAsync(tmp, (const float*)bank_emb + r0 * d, rows * d * 4, cudaMemcpyDefault, s));
-        // one "row" of rows*d elements: the staging kernel is a plain elementwise RNE conversion
-        CK(launch_stage_queries(tmp, b16 + r0 * d, 1, 1, (int)std::min<size_t>(rows * d, (size_t)INT32_MAX), s));
-        if (rows * d > (size_t)INT32_MAX) return fail(ctx, RB_EINVAL, "conversion chunk too large");
+        CK(launch_convert_bf16(tmp, b16 + r0 * d, rows * d, s));
       }
       CK(cudaStreamSynchronize(s));
       cudaFree(tmp);
@@ -403,10 +439,10 @@ rb_status rb_create(rb_ctx** out, const void* bank_emb, const float* bank_qualit
   ALLOC(ctx->cp, 1);
   ALLOC(ctx->cand_sim, mb * ctx->kc);
   ALLOC(ctx->cand_idx, mb * ctx->kc);
-  ALLOC(ctx->nn_idx, mb * k);
-  ALLOC(ctx->nn_sim, mb * k);
   ALLOC(ctx->pred_q, mb * M);
   ALLOC(ctx->pred_l, mb * M);
+  ALLOC(ctx->stage_q, mb * M);
+  ALLOC(ctx->stage_l, mb * M);
   ALLOC(ctx->termA, mb * M);
   ALLOC(ctx->termP, mb * M);
   ALLOC(ctx->key, mb);
@@ -433,6 +469,12 @@ rb_status rb_create(rb_ctx** out, const void* bank_emb, const float* bank_qualit
     if (st != RB_OK) return st;
     CK(scan_tc_prepare());
   }
+  {
+    const size_t fin = std::max(finish_smem_bytes(ctx->num_sms, ctx->kcap), finish_smem_bytes(1, ctx->kc));
+    CK(finish_prepare(fin));
+  }
+  ALLOC(ctx->scratch_nn_idx, mb * k);
+  ALLOC(ctx->scratch_nn_sim, mb * k);
 #undef ALLOC
   CK(cudaStreamSynchronize(s));   // the caller may free its buffers on return
   return RB_OK;
@@ -507,11 +549,16 @@ rb_status rb_set_state(rb_ctx* ctx, const float* queued_tokens, const int32_t* r
 rb_status rb_get_state(rb_ctx* ctx, float* queued_tokens, int32_t* running) {
   if (!ctx) return RB_EINVAL;
   if (ctx->I == 0) return fail(ctx, RB_ESTATE, "rb_get_state before rb_set_instances");
-  CopyBack cb{ctx};
-  cb.out(queued_tokens, ctx->dq, ctx->I * 4);
-  cb.out(running, ctx->bq, ctx->I * 4);
-  if (cb.err != cudaSuccess) return fail(ctx, RB_ECUDA, "cudaMemcpyAsync", cb.err);
-  if (cb.any_host) CK(cudaStreamSynchronize(ctx->stream));
+  bool any_host = false;
+  if (queued_tokens) {
+    any_host |= is_host_ptr(queued_tokens);
+    CK(cudaMemcpyAsync(queued_tokens, ctx->dq, ctx->I * 4, cudaMemcpyDefault, ctx->stream));
+  }
+  if (running) {
+    any_host |= is_host_ptr(running);
+    CK(cudaMemcpyAsync(running, ctx->bq, ctx->I * 4, cudaMemcpyDefault, ctx->stream));
+  }
+  if (any_host) CK(cudaStreamSynchronize(ctx->stream));
   return RB_OK;
 }
 
@@ -533,26 +580,27 @@ rb_status rb_decide(rb_ctx* ctx, const float* query_emb, const int32_t* prompt_l
   if (B < 1 || B > ctx->opt.max_batch) return fail(ctx, RB_EINVAL, "B out of range [1,max_batch]");
   rb_status st = check_weights(ctx, w);
   if (st != RB_OK) return st;
-  const CallParams cp{w[0], w[1], w[2], 1};
-  CopyBack cb{ctx};
-  cb.in(ctx->q32, query_emb, (size_t)B * ctx->d * 4);
-  cb.in(ctx->plen, prompt_len, (size_t)B * 4);
-  if (cb.err != cudaSuccess) return fail(ctx, RB_ECUDA, "cudaMemcpyAsync (inputs)", cb.err);
+  const size_t bm = (size_t)B * ctx->M * 4, bk = (size_t)B * ctx->k * 4;
+  Stager sg{ctx};
+  CallParams cp{};
+  cp.w_qual = w[0]; cp.w_lat = w[1]; cp.w_cost = w[2]; cp.commit = 1;
+  cp.query = sg.in(query_emb, ctx->q32, (size_t)B * ctx->d * 4);
+  cp.plen = sg.in(prompt_len, ctx->plen, (size_t)B * 4);
+  cp.q_src = ctx->pred_q;
+  cp.l_src = ctx->pred_l;
+  cp.assignment = sg.out(assignment, ctx->assignment, (size_t)B * 4);
+  cp.scores = sg.out(scores, ctx->scores, (size_t)B * ctx->I * 4);
+  cp.pred_q = sg.out_internal(pred_quality, ctx->pred_q, bm);
+  cp.pred_l = sg.out_internal(pred_outlen, ctx->pred_l, bm);
+  cp.nn_idx = sg.out(nn_idx, ctx->scratch_nn_idx, bk);
+  cp.nn_sim = sg.out(nn_sim, ctx->scratch_nn_sim, bk);
+  if (sg.err != cudaSuccess) return fail(ctx, RB_ECUDA, "cudaMemcpyAsync (inputs)", sg.err);
   st = push_params(ctx, cp);
   if (st != RB_OK) return st;
   st = run_path(ctx, B, 0);
   if (st != RB_OK) return st;
-  cb.out(assignment, ctx->assignment, (size_t)B * 4);
-  cb.out(scores, ctx->scores, (size_t)B * ctx->I * 4);
-  cb.out(pred_quality, ctx->pred_q, (size_t)B * ctx->M * 4);
-  cb.out(pred_outlen, ctx->pred_l, (size_t)B * ctx->M * 4);
-  cb.out(nn_idx, ctx->nn_idx, (size_t)B * ctx->k * 4);
-  cb.out(nn_sim, ctx->nn_sim, (size_t)B * ctx->k * 4);
-  if (cb.err != cudaSuccess) return fail(ctx, RB_ECUDA, "cudaMemcpyAsync (outputs)", cb.err);
   collect_stage_times(ctx, 0);
-  // host-side inputs must be consumed and host-side outputs complete before returning
-  if (cb.any_host) CK(cudaStreamSynchronize(ctx->stream));
-  return RB_OK;
+  return sg.finish();
 }
 
 rb_status rb_estimate(rb_ctx* ctx, const float* query_emb, int32_t B, float* pred_quality, float* pred_outlen,
@@ -560,19 +608,21 @@ rb_status rb_estimate(rb_ctx* ctx, const float* query_emb, int32_t B, float* pre
   if (!ctx) return RB_EINVAL;
   if (!query_emb) return fail(ctx, RB_EINVAL, "NULL argument");
   if (B < 1 || B > ctx->opt.max_batch) return fail(ctx, RB_EINVAL, "B out of range [1,max_batch]");
-  CopyBack cb{ctx};
-  cb.in(ctx->q32, query_emb, (size_t)B * ctx->d * 4);
-  if (cb.err != cudaSuccess) return fail(ctx, RB_ECUDA, "cudaMemcpyAsync (inputs)", cb.err);
-  rb_status st = run_path(ctx, B, 1);
+  const size_t bm = (size_t)B * ctx->M * 4, bk = (size_t)B * ctx->k * 4;
+  Stager sg{ctx};
+  CallParams cp{};
+  cp.query = sg.in(query_emb, ctx->q32, (size_t)B * ctx->d * 4);
+  cp.pred_q = sg.out_internal(pred_quality, ctx->pred_q, bm);
+  cp.pred_l = sg.out_internal(pred_outlen, ctx->pred_l, bm);
+  cp.nn_idx = sg.out(nn_idx, ctx->scratch_nn_idx, bk);
+  cp.nn_sim = sg.out(nn_sim, ctx->scratch_nn_sim, bk);
+  if (sg.err != cudaSuccess) return fail(ctx, RB_ECUDA, "cudaMemcpyAsync (inputs)", sg.err);
+  rb_status st = push_params(ctx, cp);
   if (st != RB_OK) return st;
-  cb.out(pred_quality, ctx->pred_q, (size_t)B * ctx->M * 4);
-  cb.out(pred_outlen, ctx->pred_l, (size_t)B * ctx->M * 4);
-  cb.out(nn_idx, ctx->nn_idx, (size_t)B * ctx->k * 4);
-  cb.out(nn_sim, ctx->nn_sim, (size_t)B * ctx->k * 4);
-  if (cb.err != cudaSuccess) return fail(ctx, RB_ECUDA, "cudaMemcpyAsync (outputs)", cb.err);
+  st = run_path(ctx, B, 1);
+  if (st != RB_OK) return st;
   collect_stage_times(ctx, 1);
-  if (cb.any_host) CK(cudaStreamSynchronize(ctx->stream));
-  return RB_OK;
+  return sg.finish();
 }
 
 rb_status rb_decide_from_predictions(rb_ctx* ctx, const float* quality, const float* outlen, const int32_t* prompt_len,
@@ -584,24 +634,24 @@ rb_status rb_decide_from_predictions(rb_ctx* ctx, const float* quality, const fl
   if (B < 1 || B > ctx->opt.max_batch) return fail(ctx, RB_EINVAL, "B out of range [1,max_batch]");
   rb_status st = check_weights(ctx, w);
   if (st != RB_OK) return st;
-  const CallParams cp{w[0], w[1], w[2], commit ? 1 : 0};
-  CopyBack cb{ctx};
-  cb.in(ctx->pred_q, quality, (size_t)B * ctx->M * 4);
-  cb.in(ctx->pred_l, outlen, (size_t)B * ctx->M * 4);
-  cb.in(ctx->plen, prompt_len, (size_t)B * 4);
-  if (cb.err != cudaSuccess) return fail(ctx, RB_ECUDA, "cudaMemcpyAsync (inputs)", cb.err);
+  const size_t bm = (size_t)B * ctx->M * 4, bi = (size_t)B * ctx->I * 4;
+  Stager sg{ctx};
+  CallParams cp{};
+  cp.w_qual = w[0]; cp.w_lat = w[1]; cp.w_cost = w[2]; cp.commit = commit ? 1 : 0;
+  cp.q_src = sg.in(quality, ctx->stage_q, bm);
+  cp.l_src = sg.in(outlen, ctx->stage_l, bm);
+  cp.plen = sg.in(prompt_len, ctx->plen, (size_t)B * 4);
+  cp.assignment = sg.out(assignment, ctx->assignment, (size_t)B * 4);
+  cp.scores = sg.out(scores, ctx->scores, bi);
+  cp.scores0 = sg.out(scores0, ctx->scores0, bi);
+  cp.order = sg.out(order, ctx->order, (size_t)B * 4);
+  if (sg.err != cudaSuccess) return fail(ctx, RB_ECUDA, "cudaMemcpyAsync (inputs)", sg.err);
   st = push_params(ctx, cp);
   if (st != RB_OK) return st;
   st = run_path(ctx, B, 2);
   if (st != RB_OK) return st;
-  cb.out(assignment, ctx->assignment, (size_t)B * 4);
-  cb.out(scores, ctx->scores, (size_t)B * ctx->I * 4);
-  cb.out(scores0, ctx->scores0, (size_t)B * ctx->I * 4);
-  cb.out(order, ctx->order, (size_t)B * 4);
-  if (cb.err != cudaSuccess) return fail(ctx, RB_ECUDA, "cudaMemcpyAsync (outputs)", cb.err);
   collect_stage_times(ctx, 2);
-  if (cb.any_host) CK(cudaStreamSynchronize(ctx->stream));
-  return RB_OK;
+  return sg.finish();
 }
 
 rb_status rb_set_stage_timing(rb_ctx* ctx, int32_t enabled) {
@@ -632,7 +682,7 @@ void rb_destroy(rb_ctx* ctx) {
   for (auto& kv : ctx->graphs) cudaGraphExecDestroy(kv.second);
   void* ptrs[] = {ctx->bank, ctx->bank_quality, ctx->bank_outlen, ctx->tier, ctx->cap, ctx->present, ctx->price_in,
                   ctx->price_out, ctx->pre, ctx->dec, ctx->slope, ctx->dq, ctx->bq, ctx->q32, ctx->qs, ctx->plen, ctx->cp,
-                  ctx->part_sim, ctx->part_idx, ctx->sims, ctx->cand_sim, ctx->cand_idx, ctx->nn_idx, ctx->nn_sim,
+                  ctx->part_sim, ctx->part_idx, ctx->sims, ctx->cand_sim, ctx->cand_idx, ctx->scratch_nn_idx, ctx->scratch_nn_sim, ctx->stage_q, ctx->stage_l,
                   ctx->pred_q, ctx->pred_l, ctx->termA, ctx->termP, ctx->key, ctx->order, ctx->assignment, ctx->scores,
                   ctx->scores0};
   for (void* p : ptrs) cudaFree(p);

@@ -28,49 +28,84 @@ struct InstTable {
   const int32_t* present;  // [M] 1 if the tier has an instance
 };
 
-// Per-call parameters that change between graph replays live in device memory.
+// Per-call parameters live in device memory so that a captured graph can be replayed with new weights and new
+// caller buffers.  Every pointer is a DEVICE pointer: the caller's own buffer, or the context's staging buffer
+// when the caller passed host memory.  Optional outputs are NULL when not wanted.
 struct CallParams {
   float w_qual, w_lat, w_cost;
   int32_t commit;
+  const float* query;      // [B x d] fp32 prompt embeddings
+  const int32_t* plen;     // [B]
+  const float* q_src;      // [B x M] predicted quality the score/dispatch stages consume
+  const float* l_src;      // [B x M] predicted output length, likewise
+  int32_t* assignment;     // [B]
+  float* scores;           // [B x I] or NULL
+  float* scores0;          // [B x I] or NULL
+  int32_t* order;          // [B] or NULL
+  float* pred_q;           // [B x M] or NULL: extra copy of the estimate for the caller
+  float* pred_l;
+  int32_t* nn_idx;         // [B x k] or NULL
+  float* nn_sim;
 };
 
 // ---- launchers (each returns the cudaError of its launch) ---------------------------------------------
-// a0: fp32 queries -> bf16 staging [Bpad x d], rows >= B zeroed.
-cudaError_t launch_stage_queries(const float* q, __nv_bfloat16* qs, int B, int Bpad, int d, cudaStream_t s);
+// fp32 -> bf16 (RNE), n elements (bank conversion in rb_create).
+cudaError_t launch_convert_bf16(const float* in, __nv_bfloat16* out, size_t n, cudaStream_t s);
 
-// a1 (bf16): tcgen05 scan.  part_* are [grid][KCAP][Bpad] (sim fp32 / idx int32, idx -1 = empty).
-// Returns the grid size used through *grid_out.  kcap in {16,32,64}.
+// a0: cp->query (fp32) -> bf16 staging [Bpad x d], rows >= B zeroed.
+cudaError_t launch_stage_queries(const CallParams* cp, __nv_bfloat16* qs, int B, int Bpad, int d, cudaStream_t s);
+
+// a1 (bf16): tcgen05 scan.  part_* are [grid][Bpad][KCAP] (sim fp32 / idx int32, idx -1 = empty), each list
+// sorted by (sim desc, idx asc).  Returns the grid size used through *grid_out.  kcap in {16,32,64}.
 cudaError_t launch_scan_tc(const CUtensorMap* tm_q, const CUtensorMap* tm_bank, int64_t N, int d, int B, int Bpad,
                            int kcap, int max_grid, float* part_sim, int32_t* part_idx, int* grid_out,
                            cudaStream_t s);
 size_t scan_tc_smem_bytes();
 cudaError_t scan_tc_prepare();  // opt in to the dynamic shared memory size; call once
 
-// a1 (fp32 storage): exact fp64-accumulated similarities of queries [r0, r0+nq) to sims [nq x N],
-// then per-query selection of the kc best (sim desc, idx asc) into cand_* [B x kc].
-cudaError_t launch_scan_f32(const float* bank, const float* q, int64_t N, int d, int nq, float* sims, cudaStream_t s);
+// a1 (fp32 storage): exact fp64-accumulated similarities of nq queries (q: [nq x d]) to sims [nq x N],
+// then per-query selection of the kc best (sim desc, idx asc) into cand_* [nq x kc].
+cudaError_t launch_scan_f32(const float* bank, const CallParams* cp, int r0, int64_t N, int d, int nq, float* sims,
+                            cudaStream_t s);
 cudaError_t launch_select_f32(const float* sims, int64_t N, int nq, int kc, float* cand_sim, int32_t* cand_idx,
                               cudaStream_t s);
 
-// a2: merge the per-CTA partial lists into cand_* [B x kc], best first.
-cudaError_t launch_merge(const float* part_sim, const int32_t* part_idx, int grid, int kcap, int Bpad, int B, int kc,
-                         int64_t N, float* cand_sim, int32_t* cand_idx, cudaStream_t s);
+// a2 + a3 (+ a4 when with_terms): one CTA per query merges the nlists sorted partial lists
+// (part_* [nlists][Bpad][kcap]) into the kc best, re-ranks them exactly (bf16 storage, rerank != 0), keeps k,
+// aggregates the labels with distance weights and, when with_terms, derives the per-(request, tier) terms
+// A, P and the LPT key.  pred_q / pred_l are the context's [B x M] buffers; copies for the caller go through cp.
+struct FinishArgs {
+  const float* part_sim;
+  const int32_t* part_idx;
+  int nlists, kcap, Bpad, kc, k;
+  int64_t N;
+  const __nv_bfloat16* bank;
+  const __nv_bfloat16* qs;
+  int d, rerank;
+  const float* bank_quality;
+  const float* bank_outlen;
+  int M, weight_mode;
+  float eps;
+  int with_terms;
+  float* pred_q;
+  float* pred_l;
+  float* termA;
+  float* termP;
+  float* key;
+};
+cudaError_t launch_finish(const FinishArgs& a, InstTable t, const CallParams* cp, int B, cudaStream_t s);
+size_t finish_smem_bytes(int nlists, int kcap);
+cudaError_t finish_prepare(size_t max_smem);
 
-// a3: optional exact re-rank of the kc candidates (bf16 storage), keep k, distance weights, label gather.
-cudaError_t launch_aggregate(const __nv_bfloat16* bank, const __nv_bfloat16* qs, int d, int rerank, const float* cand_sim,
-                             const int32_t* cand_idx, int kc, int k, const float* bank_quality, const float* bank_outlen,
-                             int M, int weight_mode, float eps, int B, int32_t* nn_idx, float* nn_sim, float* pred_q,
-                             float* pred_l, cudaStream_t s);
+// a4+a5 from caller-supplied predictions (cp->q_src, cp->l_src): per-(request, tier) terms, LPT keys and the
+// batch-start score matrix (cp->scores0 when non-NULL).
+cudaError_t launch_score(InstTable t, const float* dq, const int32_t* bq, const CallParams* cp, int B, float* termA,
+                         float* termP, float* key, cudaStream_t s);
 
-// a4+a5: per-(request, tier) terms, LPT keys, batch-start score matrix.
-cudaError_t launch_score(InstTable t, const float* dq, const int32_t* bq, const float* pred_q, const float* pred_l,
-                         const int32_t* plen, const CallParams* cp, int B, float* termA, float* termP, float* key,
-                         float* scores0, cudaStream_t s);
-
-// a6+a7: LPT sort + greedy dispatch with dead-reckoned updates (single CTA).
-cudaError_t launch_dispatch(InstTable t, float* dq, int32_t* bq, const float* pred_l, const float* termA,
-                            const float* termP, const float* key, const CallParams* cp, int B, int lpt_enabled,
-                            int update_enabled, int32_t* order, int32_t* assignment, float* scores, cudaStream_t s);
+// a6+a7: LPT sort + greedy dispatch with dead-reckoned updates, one CTA.
+cudaError_t launch_lpt_dispatch(InstTable t, float* dq, int32_t* bq, const float* termA, const float* termP,
+                                const float* key, const CallParams* cp, int B, int lpt_enabled, int update_enabled,
+                                cudaStream_t s);
 
 // a8: dead reckoning between batches.
 cudaError_t launch_advance(InstTable t, float* dq, int32_t* bq, float elapsed_ms, cudaStream_t s);

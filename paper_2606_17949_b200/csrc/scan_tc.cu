@@ -4,7 +4,7 @@
 // Definition ("queries a ... KNN index (k=10) over the 14,919-prompt training split"; DESIGN.md
 // readings 1, 3, 4): s[r,n] = <q~_r, e~_n> over the bf16-rounded vectors; keep, per query, the best entries in
 // the order (s descending, n ascending).  Here each CTA keeps the best KCAP of its own slab of bank rows; the
-// cross-CTA merge is merge.cu and the exact re-rank is aggregate.cu.
+// cross-CTA merge and the exact re-rank are finish_kernel (estimate.cu).
 //
 // Shape of the kernel (one persistent CTA per SM, 6 warps):
 //   warp 0   TMA producer: cp.async.bulk.tensor tiles of the bank (64 rows x 64 bf16, 128B swizzle) and of the
@@ -246,16 +246,20 @@ scan_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__
         const uint32_t acc = it & 1, aph = (it >> 1) & 1;
         const int r = mt * kTileM + tl;
         const bool warp_active = (mt * kTileM + quarter * 32) < B;   // warp-uniform
-        const size_t pbase = ((size_t)blockIdx.x * KCAP) * (size_t)Bpad + (size_t)r;
+        const size_t pbase = ((size_t)blockIdx.x * (size_t)Bpad + (size_t)r) * KCAP;   // [grid][Bpad][KCAP]
+        float4* ps4 = reinterpret_cast<float4*>(part_sim + pbase);
+        int4* pi4 = reinterpret_cast<int4*>(part_idx + pbase);
         if (warp_active) {
           if (tile == 0) {
 #pragma unroll
             for (int j = 0; j < KCAP; ++j) { v[j] = -INFINITY; ix[j] = -1; }
           } else if (n_mt > 1) {
 #pragma unroll
-            for (int j = 0; j < KCAP; ++j) {
-              v[j] = part_sim[pbase + (size_t)j * Bpad];
-              ix[j] = part_idx[pbase + (size_t)j * Bpad];
+            for (int j = 0; j < KCAP / 4; ++j) {
+              const float4 a = ps4[j];
+              const int4 b = pi4[j];
+              v[4 * j] = a.x; v[4 * j + 1] = a.y; v[4 * j + 2] = a.z; v[4 * j + 3] = a.w;
+              ix[4 * j] = b.x; ix[4 * j + 1] = b.y; ix[4 * j + 2] = b.z; ix[4 * j + 3] = b.w;
             }
           }
         }
@@ -307,9 +311,9 @@ scan_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__
         if (lane == 0) mbar_arrive(&tempty[acc]);
         if (warp_active && r < B && (n_mt > 1 || tile == ntiles - 1)) {
 #pragma unroll
-          for (int j = 0; j < KCAP; ++j) {
-            part_sim[pbase + (size_t)j * Bpad] = v[j];
-            part_idx[pbase + (size_t)j * Bpad] = ix[j];
+          for (int j = 0; j < KCAP / 4; ++j) {
+            ps4[j] = make_float4(v[4 * j], v[4 * j + 1], v[4 * j + 2], v[4 * j + 3]);
+            pi4[j] = make_int4(ix[4 * j], ix[4 * j + 1], ix[4 * j + 2], ix[4 * j + 3]);
           }
         }
       }
