@@ -77,6 +77,9 @@ typedef struct {
   int32_t update_enabled; /* 1: dead-reckoning update after each dispatch; 0: none. default 1    */
   int32_t max_batch;      /* largest B any later call may pass (scratch sizing).          default 4096    */
   int32_t use_graph;      /* 1: replay the decision as a captured CUDA graph.             default 1       */
+  int32_t scan_list;      /* RB_BF16 only: entries the bank scan keeps per (CTA, query): 4|8|16|32|64, or 0 = */
+                          /* chosen from the bank size.  Lists shorter than k+slack are exact all the same:  */
+                          /* a slab whose list might hide neighbours is searched again.   default 0       */
   void* stream;           /* cudaStream_t all work is ordered on; NULL = legacy default stream            */
 } rb_options;
 

@@ -125,6 +125,10 @@ select_f32_kernel(const float* __restrict__ sims, int64_t N, int kc, float* __re
 //  merge   the nlists partial lists (each sorted by key, descending) are copied to shared memory as 64-bit
 //          keys; thread c owns list c and exposes its head; kc rounds of a block-wide maximum (REDUX on the
 //          high and low words, one barrier per round) pop the kc best in order.
+//  rescan  the scan may keep fewer entries per (CTA, query) than kc (short lists make its warm-up cheap).  A list
+//          whose every entry was popped may hide further members of the top kc; the bank rows of such a slab
+//          (rare: several of a query's kc best in one of ~148 slabs) are searched again here, exactly, and the
+//          merge is redone over the untouched lists' candidates and the slab's own best kc.
 //  re-rank (bf16 storage): the kc candidates' similarities are recomputed from the stored bf16 rows with fp64
 //          accumulation (products of bf16 values are exact), rounded once to fp32, re-ordered by
 //          (s desc, n asc); the best k are the neighbours.
@@ -135,10 +139,69 @@ select_f32_kernel(const float* __restrict__ sims, int64_t N, int kc, float* __re
 //          c1 = (float)l*pin; c2 = L*pout; C = c1 + c2; Cmax over tiers that have an instance;
 //          ct = Cmax > 0 ? 1 - C/Cmax : 0; A = wq*Q + wc*ct; P = pre*(float)l; key = max_m L
 constexpr int kFinThreads = 512;
+constexpr int kFinWarps = kFinThreads / 32;
+constexpr int kMaxFlag = 16;                      // flagged lists per query <= kc / kcap
+constexpr int kMerge2Stride = 64;                 // second merge: kFinWarps + 1 lists of up to kMaxK keys
+
+// s = fl32( sum_c (double)x[c]*(double)e[c] ) of two bf16 rows, the 32 lanes' fp64 partials added by shuffles.
+__device__ __forceinline__ float exact_sim_bf16(const uint4* __restrict__ qrow, const uint4* __restrict__ brow, int nvec,
+                                                int lane) {
+  double acc = 0.0;
+#pragma unroll 4
+  for (int vidx = lane; vidx < nvec; vidx += 32) {
+    const uint4 xb = qrow[vidx], eb = brow[vidx];
+    const __nv_bfloat162* xp = reinterpret_cast<const __nv_bfloat162*>(&xb);
+    const __nv_bfloat162* ep = reinterpret_cast<const __nv_bfloat162*>(&eb);
+#pragma unroll
+    for (int h = 0; h < 4; ++h) {
+      const float2 xf = __bfloat1622float2(xp[h]), ef = __bfloat1622float2(ep[h]);
+      acc = fma((double)xf.x, (double)ef.x, acc);
+      acc = fma((double)xf.y, (double)ef.y, acc);
+    }
+  }
+  for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+  return (float)acc;
+}
+
+// Block-wide k-way merge: thread c < nl owns the sorted list keys[c*stride .. c*stride+len); pops the kc largest
+// keys into out_key[0..kc) (0 = exhausted) and the list each came from into out_src.  Returns how many entries
+// of the caller's own list were popped.  All kFinThreads threads must call.
+__device__ int kway_merge(const unsigned long long* keys, int nl, int stride, int len, int kc,
+                          uint32_t (*s_red)[kFinWarps][2], unsigned long long* out_key, int* out_src) {
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  int pos = 0;
+  unsigned long long hk = (tid < nl) ? keys[(size_t)tid * stride] : 0ull;
+  for (int j = 0; j < kc; ++j) {
+    const uint32_t hi = (uint32_t)(hk >> 32), lo = (uint32_t)hk;
+    const uint32_t whi = __reduce_max_sync(0xffffffffu, hi);
+    const uint32_t wlo = __reduce_max_sync(0xffffffffu, hi == whi ? lo : 0u);
+    if (lane == 0) { s_red[j & 1][warp][0] = whi; s_red[j & 1][warp][1] = wlo; }
+    __syncthreads();
+    const uint32_t xhi = lane < kFinWarps ? s_red[j & 1][lane][0] : 0u;
+    const uint32_t xlo = lane < kFinWarps ? s_red[j & 1][lane][1] : 0u;
+    const uint32_t ghi = __reduce_max_sync(0xffffffffu, xhi);
+    const uint32_t glo = __reduce_max_sync(0xffffffffu, xhi == ghi ? xlo : 0u);
+    const unsigned long long win = ((unsigned long long)ghi << 32) | glo;
+    if (win != 0ull && hk == win) {   // keys are distinct: exactly one owner
+      out_key[j] = win;
+      out_src[j] = tid;
+      ++pos;
+      hk = pos < len ? keys[(size_t)tid * stride + pos] : 0ull;
+    }
+    if (win == 0ull && tid == 0) { out_key[j] = 0ull; out_src[j] = -1; }
+  }
+  __syncthreads();
+  return pos;
+}
+
 __global__ void __launch_bounds__(kFinThreads)
 finish_kernel(FinishArgs a, InstTable t, const CallParams* __restrict__ cp) {
-  extern __shared__ unsigned long long s_keys[];   // [nlists][kcap]
-  __shared__ uint32_t s_red[2][kFinThreads / 32][2];
+  extern __shared__ unsigned long long s_keys[];   // max([nlists][kcap], [kFinWarps + 1][kMerge2Stride])
+  __shared__ uint32_t s_red[2][kFinWarps][2];
+  __shared__ unsigned long long s_cand[kMaxK];
+  __shared__ int s_src[kMaxK];
+  __shared__ int s_nflag;
+  __shared__ int s_flag[kMaxFlag];
   __shared__ float s_sim[kMaxK];
   __shared__ int32_t s_idx[kMaxK];
   __shared__ float o_sim[kMaxK];
@@ -147,11 +210,14 @@ finish_kernel(FinishArgs a, InstTable t, const CallParams* __restrict__ cp) {
   __shared__ float sQ[kMaxM], sL[kMaxM], sC[kMaxM];
   const int r = blockIdx.x;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  constexpr int nwarps = kFinThreads / 32;
+  constexpr int nwarps = kFinWarps;
   const int kc = a.kc, k = a.k, kcap = a.kcap, M = a.M;
+  const uint4* qrow = reinterpret_cast<const uint4*>(a.qs + (size_t)r * a.d);
+  const int nvec = a.d / 8;   // d % 8 == 0
 
   // ---- merge ----
   const int total = a.nlists * kcap;
+  if (tid == 0) s_nflag = 0;
   for (int e = tid; e < total; e += kFinThreads) {
     const int c = e / kcap, j = e - c * kcap;
     const size_t off = ((size_t)c * a.Bpad + r) * kcap + j;
@@ -159,53 +225,68 @@ finish_kernel(FinishArgs a, InstTable t, const CallParams* __restrict__ cp) {
     s_keys[e] = (id >= 0 && (int64_t)id < a.N) ? make_key(a.part_sim[off], id) : 0ull;
   }
   __syncthreads();
-  int pos = 0;
-  unsigned long long hk = (tid < a.nlists) ? s_keys[(size_t)tid * kcap] : 0ull;
-  for (int j = 0; j < kc; ++j) {
-    const uint32_t hi = (uint32_t)(hk >> 32), lo = (uint32_t)hk;
-    const uint32_t whi = __reduce_max_sync(0xffffffffu, hi);
-    const uint32_t wlo = __reduce_max_sync(0xffffffffu, hi == whi ? lo : 0u);
-    if (lane == 0) { s_red[j & 1][warp][0] = whi; s_red[j & 1][warp][1] = wlo; }
+  const int popped = kway_merge(s_keys, a.nlists, kcap, kcap, kc, s_red, s_cand, s_src);
+
+  // ---- rescan of slabs whose list was popped completely ----
+  const bool flagged = a.rescan && tid < a.nlists && popped == kcap;
+  if (__syncthreads_or(flagged)) {
+    if (flagged) {
+      const int p = atomicAdd(&s_nflag, 1);
+      if (p < kMaxFlag) s_flag[p] = tid;
+    }
     __syncthreads();
-    const uint32_t xhi = lane < nwarps ? s_red[j & 1][lane][0] : 0u;
-    const uint32_t xlo = lane < nwarps ? s_red[j & 1][lane][1] : 0u;
-    const uint32_t ghi = __reduce_max_sync(0xffffffffu, xhi);
-    const uint32_t glo = __reduce_max_sync(0xffffffffu, xhi == ghi ? xlo : 0u);
-    const unsigned long long win = ((unsigned long long)ghi << 32) | glo;
-    if (win != 0ull && hk == win) {   // keys are distinct: exactly one owner
-      ++pos;
-      hk = pos < kcap ? s_keys[(size_t)tid * kcap + pos] : 0ull;
+    const int nflag = min(s_nflag, kMaxFlag);
+    // every warp keeps the best kc of the rows it visits: rank l in lane l (a) and rank 32+l (b)
+    unsigned long long la = 0, lb = 0, thr = 0;
+    const int64_t units = (a.N + kBoxN - 1) / kBoxN;
+    for (int f = 0; f < nflag; ++f) {
+      const int c = s_flag[f];
+      const int64_t row0 = units * c / a.nlists * kBoxN;
+      int64_t row1 = units * (c + 1) / a.nlists * kBoxN;
+      if (row1 > a.N) row1 = a.N;
+      for (int64_t n = row0 + warp; n < row1; n += nwarps) {
+        const float sx = exact_sim_bf16(qrow, reinterpret_cast<const uint4*>(a.bank + (size_t)n * a.d), nvec, lane);
+        const unsigned long long x = make_key(sx, (int32_t)n);
+        if (sx == sx && x > thr) {
+          const int p = __popc(__ballot_sync(0xffffffffu, la > x)) + __popc(__ballot_sync(0xffffffffu, lb > x));
+          const unsigned long long a_up = __shfl_up_sync(0xffffffffu, la, 1), b_up = __shfl_up_sync(0xffffffffu, lb, 1);
+          const unsigned long long a_last = __shfl_sync(0xffffffffu, la, 31);
+          const unsigned long long b_prev = (lane == 0) ? a_last : b_up;
+          la = (lane < p) ? la : ((lane == p) ? x : a_up);
+          lb = (lane + 32 < p) ? lb : ((lane + 32 == p) ? x : b_prev);
+          thr = (kc <= 32) ? __shfl_sync(0xffffffffu, la, kc - 1) : __shfl_sync(0xffffffffu, lb, kc - 33);
+        }
+      }
     }
+    __syncthreads();   // s_keys is rewritten: lists 0..nwarps-1 = the warps' lists, list nwarps = untouched candidates
+    s_keys[(size_t)warp * kMerge2Stride + lane] = la;
+    s_keys[(size_t)warp * kMerge2Stride + 32 + lane] = lb;
     if (tid == 0) {
-      s_sim[j] = win ? f32_unordered(ghi) : -INFINITY;
-      s_idx[j] = win ? (int32_t)(0xffffffffu - glo) : -1;
+      int o = 0;
+      for (int j = 0; j < kc; ++j) {
+        bool from_flagged = false;
+        for (int f = 0; f < nflag; ++f) from_flagged |= (s_src[j] == s_flag[f]);
+        if (s_cand[j] != 0ull && !from_flagged) s_keys[(size_t)nwarps * kMerge2Stride + o++] = s_cand[j];
+      }
+      for (; o < kMerge2Stride; ++o) s_keys[(size_t)nwarps * kMerge2Stride + o] = 0ull;
     }
+    __syncthreads();
+    kway_merge(s_keys, nwarps + 1, kMerge2Stride, kMerge2Stride, kc, s_red, s_cand, s_src);
+  }
+  if (tid < kc) {
+    const unsigned long long key = s_cand[tid];
+    s_sim[tid] = key ? f32_unordered((uint32_t)(key >> 32)) : -INFINITY;
+    s_idx[tid] = key ? (int32_t)(0xffffffffu - (uint32_t)key) : -1;
   }
   __syncthreads();
 
   // ---- exact re-rank ----
   if (a.rerank) {
-    const uint4* qrow = reinterpret_cast<const uint4*>(a.qs + (size_t)r * a.d);
-    const int nvec = a.d / 8;   // d % 8 == 0
     for (int c = warp; c < kc; c += nwarps) {
       const int32_t id = s_idx[c];
       if (id < 0) continue;
-      const uint4* brow = reinterpret_cast<const uint4*>(a.bank + (size_t)id * a.d);
-      double acc = 0.0;
-#pragma unroll 4
-      for (int vidx = lane; vidx < nvec; vidx += 32) {
-        const uint4 xb = qrow[vidx], eb = brow[vidx];
-        const __nv_bfloat162* xp = reinterpret_cast<const __nv_bfloat162*>(&xb);
-        const __nv_bfloat162* ep = reinterpret_cast<const __nv_bfloat162*>(&eb);
-#pragma unroll
-        for (int h = 0; h < 4; ++h) {
-          const float2 xf = __bfloat1622float2(xp[h]), ef = __bfloat1622float2(ep[h]);
-          acc = fma((double)xf.x, (double)ef.x, acc);
-          acc = fma((double)xf.y, (double)ef.y, acc);
-        }
-      }
-      for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
-      if (lane == 0) s_sim[c] = (float)acc;
+      const float sx = exact_sim_bf16(qrow, reinterpret_cast<const uint4*>(a.bank + (size_t)id * a.d), nvec, lane);
+      if (lane == 0) s_sim[c] = sx;
     }
     __syncthreads();
   }
@@ -317,7 +398,10 @@ cudaError_t launch_select_f32(const float* sims, int64_t N, int nq, int kc, floa
   return cudaGetLastError();
 }
 
-size_t finish_smem_bytes(int nlists, int kcap) { return (size_t)nlists * kcap * sizeof(unsigned long long); }
+size_t finish_smem_bytes(int nlists, int kcap) {
+  const size_t n1 = (size_t)nlists * kcap, n2 = (size_t)(kFinWarps + 1) * kMerge2Stride;
+  return (n1 > n2 ? n1 : n2) * sizeof(unsigned long long);
+}
 
 cudaError_t finish_prepare(size_t max_smem) {
   return cudaFuncSetAttribute(finish_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)max_smem);

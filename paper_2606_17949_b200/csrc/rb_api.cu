@@ -21,7 +21,7 @@ using namespace rb;
 struct rb_ctx {
   // problem
   int64_t N = 0;
-  int d = 0, M = 0, k = 0, kc = 0, kcap = 0;
+  int d = 0, M = 0, k = 0, kc = 0, kcap = 0, ks = 0;   // kc = k + slack; kcap >= kc; ks = entries the scan keeps
   rb_options opt{};
   cudaStream_t stream = nullptr;
   bool own_stream = false;
@@ -171,10 +171,11 @@ rb_status enqueue_estimate(rb_ctx* ctx, int B, bool with_terms, Timer& tm) {
     CK(launch_stage_queries(ctx->cp, ctx->qs, B, Bpad, ctx->d, s));
     tm.mark();
     int grid = 0;
-    CK(launch_scan_tc(&ctx->tm_q, &ctx->tm_bank, ctx->N, ctx->d, B, Bpad, ctx->kcap, ctx->num_sms, ctx->part_sim,
+    CK(launch_scan_tc(&ctx->tm_q, &ctx->tm_bank, ctx->N, ctx->d, B, Bpad, ctx->ks, ctx->num_sms, ctx->part_sim,
                       ctx->part_idx, &grid, s));
     tm.mark();
-    fa.part_sim = ctx->part_sim; fa.part_idx = ctx->part_idx; fa.nlists = grid; fa.kcap = ctx->kcap; fa.Bpad = Bpad;
+    fa.part_sim = ctx->part_sim; fa.part_idx = ctx->part_idx; fa.nlists = grid; fa.kcap = ctx->ks; fa.Bpad = Bpad;
+    fa.rescan = ctx->ks < ctx->kc ? 1 : 0;
     fa.bank = (const __nv_bfloat16*)ctx->bank; fa.qs = ctx->qs; fa.rerank = ctx->opt.rerank_slack > 0 ? 1 : 0;
     ctx->launches += 2;
   } else {
@@ -348,6 +349,7 @@ void rb_options_default(rb_options* opt) {
   opt->update_enabled = 1;
   opt->max_batch = 4096;
   opt->use_graph = 1;
+  opt->scan_list = 0;
   opt->stream = nullptr;
 }
 
@@ -367,6 +369,9 @@ rb_status rb_create(rb_ctx** out, const void* bank_emb, const float* bank_qualit
   if (opt.max_batch < 1 || opt.max_batch > 4096) return RB_EINVAL;
   if (!(opt.dist_eps >= 0.0f) || !std::isfinite(opt.dist_eps)) return RB_EINVAL;
   if (opt.weight_mode != 0 && opt.weight_mode != 1) return RB_EINVAL;
+  if (opt.scan_list != 0 && opt.scan_list != 4 && opt.scan_list != 8 && opt.scan_list != 16 && opt.scan_list != 32 &&
+      opt.scan_list != 64)
+    return RB_EINVAL;
 
   int dev = 0;
   cudaDeviceProp prop{};
@@ -382,6 +387,18 @@ rb_status rb_create(rb_ctx** out, const void* bank_emb, const float* bank_qualit
   ctx->kc = k + opt.rerank_slack;
   ctx->kcap = ctx->kc <= 16 ? 16 : (ctx->kc <= 32 ? 32 : 64);
   ctx->num_sms = prop.multiProcessorCount;
+  {
+    // Entries the scan keeps per (CTA, query).  Short lists make the scan's warm-up cheap (its cost is in the
+    // first few hundred rows of a slab); the finishing kernel searches a slab again, exactly, in the rare case
+    // that a short list may hide members of the top kc.  Long slabs amortise a full-length list.
+    const int64_t units = (N + kBoxN - 1) / kBoxN;
+    const int64_t grid = units < ctx->num_sms ? units : ctx->num_sms;
+    const int64_t rows_per_cta = N / grid;
+    int ks = opt.scan_list;
+    if (ks == 0) ks = rows_per_cta >= 16384 ? ctx->kcap : (rows_per_cta >= 2048 ? 8 : 4);
+    if (ks > ctx->kcap) ks = ctx->kcap;
+    ctx->ks = ks;
+  }
   ctx->Bpad_max = (opt.max_batch + kTileM - 1) / kTileM * kTileM;
   *out = ctx;   // from here on errors keep the context so that rb_last_error works; caller destroys it
 
@@ -470,7 +487,7 @@ rb_status rb_create(rb_ctx** out, const void* bank_emb, const float* bank_qualit
     CK(scan_tc_prepare());
   }
   {
-    const size_t fin = std::max(finish_smem_bytes(ctx->num_sms, ctx->kcap), finish_smem_bytes(1, ctx->kc));
+    const size_t fin = std::max(finish_smem_bytes(ctx->num_sms, ctx->ks), finish_smem_bytes(1, ctx->kc));
     CK(finish_prepare(fin));
   }
   ALLOC(ctx->scratch_nn_idx, mb * k);

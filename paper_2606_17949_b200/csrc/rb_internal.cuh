@@ -56,7 +56,8 @@ cudaError_t launch_convert_bf16(const float* in, __nv_bfloat16* out, size_t n, c
 cudaError_t launch_stage_queries(const CallParams* cp, __nv_bfloat16* qs, int B, int Bpad, int d, cudaStream_t s);
 
 // a1 (bf16): tcgen05 scan.  part_* are [grid][Bpad][KCAP] (sim fp32 / idx int32, idx -1 = empty), each list
-// sorted by (sim desc, idx asc).  Returns the grid size used through *grid_out.  kcap in {16,32,64}.
+// sorted by (sim desc, idx asc).  Returns the grid size used through *grid_out.  kcap in {4,8,16,32,64}; bank
+// rows are split over the CTAs in units of kBoxN rows: CTA c owns units [units*c/grid, units*(c+1)/grid).
 cudaError_t launch_scan_tc(const CUtensorMap* tm_q, const CUtensorMap* tm_bank, int64_t N, int d, int B, int Bpad,
                            int kcap, int max_grid, float* part_sim, int32_t* part_idx, int* grid_out,
                            cudaStream_t s);
@@ -82,6 +83,7 @@ struct FinishArgs {
   const __nv_bfloat16* bank;
   const __nv_bfloat16* qs;
   int d, rerank;
+  int rescan;               // 1: lists are shorter than kc -> slabs whose list was popped completely are searched again
   const float* bank_quality;
   const float* bank_outlen;
   int M, weight_mode;

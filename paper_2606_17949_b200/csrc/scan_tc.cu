@@ -23,6 +23,20 @@
 namespace rb {
 namespace {
 
+#ifdef RB_TRACE   // development aid (_work harness): per-CTA timestamps of the pipeline roles; compiled out otherwise
+__device__ unsigned long long rb_trace_buf[148 * 512];
+__device__ __forceinline__ void trace(int slot) {
+  if (slot < 512) {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    rb_trace_buf[blockIdx.x * 512 + slot] = t;
+  }
+}
+#define RB_TR(slot) trace(slot)
+#else
+#define RB_TR(slot)
+#endif
+
 constexpr int kStages = 4;
 constexpr int kABytes = kTileM * kTileK * 2;       // 16 KB: 128 queries x 64 bf16
 constexpr int kBoxBytes = kBoxN * kTileK * 2;      //  8 KB: 64 bank rows x 64 bf16
@@ -128,6 +142,8 @@ __device__ __forceinline__ void list_insert(float (&v)[K], int32_t (&ix)[K], flo
   ix[0] = top ? id : ix[0];
 }
 
+__device__ __forceinline__ bool tl_trace_end(int tid) { return tid == 128; }   // epilogue thread of query 0
+
 template <int KCAP>
 __global__ void __launch_bounds__(kThreads, 1)
 scan_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_bank, int64_t N, int d,
@@ -153,6 +169,7 @@ scan_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__
   const int64_t row0 = u0 * kBoxN;
   const int ntiles = (nunits + 3) / 4;
 
+  if (threadIdx.x == 0) RB_TR(0);
   if (warp == 0 && lane == 0) {
     asm volatile("prefetch.tensormap [%0];" ::"l"(&tm_q) : "memory");
     asm volatile("prefetch.tensormap [%0];" ::"l"(&tm_bank) : "memory");
@@ -175,6 +192,7 @@ scan_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot;
+  if (threadIdx.x == 0) RB_TR(1);
 
   if (warp == 0) {
     // ===== TMA producer =====
@@ -193,6 +211,7 @@ scan_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__
             mbar_arrive_expect_tx(&full[s], kABytes + nun * kBoxBytes);
             tma_load_2d(sa, &tm_q, kc * kTileK, mt * kTileM, &full[s]);
             for (int u = 0; u < nun; ++u) tma_load_2d(sb + u * kBoxBytes, &tm_bank, kc * kTileK, n0 + u * kBoxN, &full[s]);
+            RB_TR(16 + kit);
           }
         }
       }
@@ -215,6 +234,7 @@ scan_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__
             const uint32_t ph = (kit / kStages) & 1;
             mbar_wait(&full[s], ph);
             tc_fence_after();
+            RB_TR(96 + kit);
             const uint32_t sa = smem_u32(smem + s * kStageBytes);
             const uint64_t adesc = make_smem_desc(sa);
             const uint64_t bdesc = make_smem_desc(sa + kABytes);
@@ -226,6 +246,7 @@ scan_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__
             tc_commit(&empty[s]);
           }
           tc_commit(&tfull[acc]);
+          RB_TR(176 + it);
         }
       }
     }
@@ -265,6 +286,7 @@ scan_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__
         }
         mbar_wait(&tfull[acc], aph);
         tc_fence_after();
+        if (tl == 0) RB_TR(192 + it);
         if (warp_active) {
           float thr = (r < B) ? v[KCAP - 1] : INFINITY;   // padding lanes never collect
           const uint32_t taddr = tmem_base + ((uint32_t)(quarter * 32) << 16) + acc * kTileN;
@@ -308,6 +330,7 @@ scan_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__
         }
         tc_fence_before();
         __syncwarp();
+        if (tl == 0) RB_TR(208 + it);
         if (lane == 0) mbar_arrive(&tempty[acc]);
         if (warp_active && r < B && (n_mt > 1 || tile == ntiles - 1)) {
 #pragma unroll
@@ -320,8 +343,10 @@ scan_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__
     }
   }
 
+  if (tl_trace_end(threadIdx.x)) RB_TR(2);
   tc_fence_before();
   __syncthreads();
+  if (threadIdx.x == 0) RB_TR(3);
   if (warp == 1) {
     tc_fence_after();
     asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(512) : "memory");
@@ -334,6 +359,10 @@ size_t scan_tc_smem_bytes() { return kSmemBytes; }
 
 cudaError_t scan_tc_prepare() {
   cudaError_t e;
+  e = cudaFuncSetAttribute(scan_tc_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
+  if (e != cudaSuccess) return e;
+  e = cudaFuncSetAttribute(scan_tc_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
+  if (e != cudaSuccess) return e;
   e = cudaFuncSetAttribute(scan_tc_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
   if (e != cudaSuccess) return e;
   e = cudaFuncSetAttribute(scan_tc_kernel<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
@@ -346,7 +375,11 @@ cudaError_t launch_scan_tc(const CUtensorMap* tm_q, const CUtensorMap* tm_bank, 
   const int64_t units = (N + kBoxN - 1) / kBoxN;
   const int grid = (int)(units < max_grid ? units : max_grid);
   if (grid_out) *grid_out = grid;
-  if (kcap == 16)
+  if (kcap == 4)
+    scan_tc_kernel<4><<<grid, kThreads, kSmemBytes, s>>>(*tm_q, *tm_bank, N, d, B, Bpad, part_sim, part_idx);
+  else if (kcap == 8)
+    scan_tc_kernel<8><<<grid, kThreads, kSmemBytes, s>>>(*tm_q, *tm_bank, N, d, B, Bpad, part_sim, part_idx);
+  else if (kcap == 16)
     scan_tc_kernel<16><<<grid, kThreads, kSmemBytes, s>>>(*tm_q, *tm_bank, N, d, B, Bpad, part_sim, part_idx);
   else if (kcap == 32)
     scan_tc_kernel<32><<<grid, kThreads, kSmemBytes, s>>>(*tm_q, *tm_bank, N, d, B, Bpad, part_sim, part_idx);

@@ -7,7 +7,7 @@ from . import binding as rb
 
 class Router:
     def __init__(self, bank_emb, bank_quality, bank_outlen, k, *, store="bf16", rerank_slack=None, weight_mode=0,
-                 dist_eps=1e-6, lpt_enabled=1, update_enabled=1, max_batch=4096, use_graph=1, device="cuda"):
+                 dist_eps=1e-6, lpt_enabled=1, update_enabled=1, max_batch=4096, use_graph=1, scan_list=0, device="cuda"):
         N, d = bank_emb.shape
         M = bank_quality.shape[1]
         opt = rb.rb_options_default()
@@ -21,6 +21,7 @@ class Router:
         opt.update_enabled = update_enabled
         opt.max_batch = max_batch
         opt.use_graph = use_graph
+        opt.scan_list = scan_list
         self.device = torch.device(device)
         self.stream = torch.cuda.Stream(device=self.device)
         opt.stream = self.stream.cuda_stream

@@ -17,8 +17,11 @@ def _router(bank, cfg, **kw):
     return Router(bank["emb"], bank["quality"], bank["outlen"], cfg.k, store=cfg.store, **kw)
 
 
-def _setup(cfg, device="cuda", B=None, **kw):
+def _setup(cfg, device="cuda", B=None, sort_bank=False, **kw):
     bank = synth.make_bank(cfg, device=device)
+    if sort_bank:   # rows of one mixture component become contiguous: a query's neighbours share one CTA's slab
+        order = torch.argsort(bank["comp"], stable=True)
+        bank = {k_: v[order].contiguous() for k_, v in bank.items()}
     it = synth.make_instances(cfg.I, cfg.M)
     queued, running = synth.make_state(cfg.I, it["cap"], cfg.seed)
     query = synth.make_queries(cfg, B=B, device=device)
@@ -72,6 +75,20 @@ def test_bf16_scan_parity_ragged(orc, N, d, B, slack):
     tol = 0.0 if slack > 0 else 4e-6   # re-ranked similarities are exact; raw tensor-core sums are not
     g, near, log = _full_parity(orc, cfg, synth.PRESETS["balanced"], sim_tol=tol, rerank_slack=slack, max_batch=512)
     assert len(near) <= max(1, B // 20), log
+
+
+@pytest.mark.parametrize("scan_list", [4, 8, 16])
+@pytest.mark.parametrize("N,B,k,slack", [(20000, 24, 10, 6), (3000, 7, 10, 0), (150000, 130, 32, 8)])
+def test_short_scan_lists_rescan_clustered_bank(orc, scan_list, N, B, k, slack):
+    """The scan keeps only scan_list entries per (CTA, query); with the bank sorted by mixture component all of a
+    query's neighbours sit in one or two slabs, so the finishing kernel must search those slabs again
+    (exactly) to stay correct.  Also run on the unsorted bank, where the rescan is (almost) never taken."""
+    cfg = dataclasses.replace(synth.CONFIGS["C2"], N=N, d=128, B=B, k=k, Kc=8, seed=21)
+    tol = 0.0 if slack > 0 else 4e-6
+    for sort_bank in (True, False):
+        g, near, log = _full_parity(orc, cfg, synth.PRESETS["balanced"], sim_tol=tol, rerank_slack=slack, max_batch=256,
+                                    scan_list=scan_list, sort_bank=sort_bank)
+        assert len(near) <= max(1, B // 20), log
 
 
 def test_bf16_k32_and_uniform_weights(orc):
