@@ -220,6 +220,12 @@ def run_ours(args):
         torch.cuda.synchronize()
 
     # ---- leg 1: device-resident inputs, CUDA events per step on the library's stream ---------------------------
+    # untimed: one decision per distinct batch size, so that every CUDA graph the stream needs is captured
+    # and instantiated before the timed region (capture is a one-off host cost per batch size)
+    for B in sorted(set(sizes)):
+        rb.rb_decide(rt.ctx, allq[:B], allp[:B], B, weights[0], assign_dev[:B])
+    rt.sync()
+    rt.set_state(queued, running)
     for j in range(W):
         flush()
         step_device(j)
@@ -312,7 +318,8 @@ def run_ours(args):
                       "warm (bank 153.6 MB vs 126 MB L2)", "graph": "CUDA graph replay per B",
                       "parallelism": "replicas only" if world > 1 else "single GPU"},
            "decision_us": {"mean": round(float(step_ms.mean()) * 1e3, 2), "p50": round(float(np.median(step_ms)) * 1e3, 2),
-                           "p99": round(float(np.percentile(step_ms, 99)) * 1e3, 2)},
+                           "p99": round(float(np.percentile(step_ms, 99)) * 1e3, 2),
+                           "max": round(float(step_ms.max()) * 1e3, 2)},
            "e2e": {"value": round(units / e2e_max, 1), "unit": UNIT, "h2d_bytes_per_step": round(h2d, 1),
                    "d2h_bytes_per_step": round(d2h, 1), "us_per_decision": round(e2e_max / K * 1e6, 2)},
            "gpu_launches": int(launches), "clocks": sampler.summary(), "roofline": roofline,

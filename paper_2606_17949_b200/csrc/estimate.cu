@@ -22,12 +22,13 @@ __device__ __forceinline__ unsigned long long make_key(float sim, int32_t idx) {
 
 // ---- a0 ---------------------------------------------------------------------------------------------
 __global__ void stage_queries_kernel(const CallParams* __restrict__ cp, __nv_bfloat16* __restrict__ qs, int B, int Bpad,
-                                     int d) {
+                                     int d, int group) {
   const float* __restrict__ q = cp->query;
   const size_t n = (size_t)Bpad * d;
   for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
-    const size_t r = i / d;
-    qs[i] = (r < (size_t)B) ? __float2bfloat16_rn(q[i]) : __float2bfloat16_rn(0.0f);
+    const size_t row = i / d, c = i - row * d;
+    const size_t r = row % group;   // replicas of query r at rows r, group + r, ...
+    qs[i] = (r < (size_t)B) ? __float2bfloat16_rn(q[r * d + c]) : __float2bfloat16_rn(0.0f);
   }
 }
 __global__ void convert_bf16_kernel(const float* __restrict__ in, __nv_bfloat16* __restrict__ out, size_t n) {
@@ -138,10 +139,10 @@ select_f32_kernel(const float* __restrict__ sims, int64_t N, int kc, float* __re
 //  terms   (with_terms; Eq. 2, Eq. 1):
 //          c1 = (float)l*pin; c2 = L*pout; C = c1 + c2; Cmax over tiers that have an instance;
 //          ct = Cmax > 0 ? 1 - C/Cmax : 0; A = wq*Q + wc*ct; P = pre*(float)l; key = max_m L
-constexpr int kFinThreads = 512;
-constexpr int kFinWarps = kFinThreads / 32;
+constexpr int kFinThreadsMax = 1024;              // 512 threads, or 1024 when there are more than 512 lists
+constexpr int kFinWarpsMax = kFinThreadsMax / 32;
 constexpr int kMaxFlag = 16;                      // flagged lists per query <= kc / kcap
-constexpr int kMerge2Stride = 64;                 // second merge: kFinWarps + 1 lists of up to kMaxK keys
+constexpr int kMerge2Stride = 64;                 // second merge: nwarps + 1 lists of up to kMaxK keys
 
 // s = fl32( sum_c (double)x[c]*(double)e[c] ) of two bf16 rows, the 32 lanes' fp64 partials added by shuffles.
 __device__ __forceinline__ float exact_sim_bf16(const uint4* __restrict__ qrow, const uint4* __restrict__ brow, int nvec,
@@ -165,10 +166,10 @@ __device__ __forceinline__ float exact_sim_bf16(const uint4* __restrict__ qrow, 
 
 // Block-wide k-way merge: thread c < nl owns the sorted list keys[c*stride .. c*stride+len); pops the kc largest
 // keys into out_key[0..kc) (0 = exhausted) and the list each came from into out_src.  Returns how many entries
-// of the caller's own list were popped.  All kFinThreads threads must call.
+// of the caller's own list were popped.  All threads of the block must call.
 __device__ int kway_merge(const unsigned long long* keys, int nl, int stride, int len, int kc,
-                          uint32_t (*s_red)[kFinWarps][2], unsigned long long* out_key, int* out_src) {
-  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+                          uint32_t (*s_red)[kFinWarpsMax][2], unsigned long long* out_key, int* out_src) {
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, kFinWarps = blockDim.x >> 5;
   int pos = 0;
   unsigned long long hk = (tid < nl) ? keys[(size_t)tid * stride] : 0ull;
   for (int j = 0; j < kc; ++j) {
@@ -194,10 +195,10 @@ __device__ int kway_merge(const unsigned long long* keys, int nl, int stride, in
   return pos;
 }
 
-__global__ void __launch_bounds__(kFinThreads)
+__global__ void __launch_bounds__(kFinThreadsMax)
 finish_kernel(FinishArgs a, InstTable t, const CallParams* __restrict__ cp) {
-  extern __shared__ unsigned long long s_keys[];   // max([nlists][kcap], [kFinWarps + 1][kMerge2Stride])
-  __shared__ uint32_t s_red[2][kFinWarps][2];
+  extern __shared__ unsigned long long s_keys[];   // max([nlists][kcap], [nwarps + 1][kMerge2Stride])
+  __shared__ uint32_t s_red[2][kFinWarpsMax][2];
   __shared__ unsigned long long s_cand[kMaxK];
   __shared__ int s_src[kMaxK];
   __shared__ int s_nflag;
@@ -207,10 +208,20 @@ finish_kernel(FinishArgs a, InstTable t, const CallParams* __restrict__ cp) {
   __shared__ float o_sim[kMaxK];
   __shared__ int32_t o_idx[kMaxK];
   __shared__ float s_w[kMaxK];
+  __shared__ int o_pos[kMaxK];
+  __shared__ float s_lab[kMaxK][2 * kMaxM];         // labels of the kc candidates: [quality(M) | outlen(M)]
   __shared__ float sQ[kMaxM], sL[kMaxM], sC[kMaxM];
   const int r = blockIdx.x;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  constexpr int nwarps = kFinWarps;
+  const int kFinThreads = blockDim.x, nwarps = blockDim.x >> 5;
+  // coefficients of the score terms: requested now, consumed at the very end (their latency hides behind the merge)
+  float c_pin = 0.0f, c_pout = 0.0f, c_pre = 0.0f, c_ell = 0.0f;
+  if (a.with_terms && tid < a.M) {
+    c_pin = t.price_in[tid];
+    c_pout = t.price_out[tid];
+    c_pre = t.pre[tid];
+    c_ell = (float)cp->plen[r];
+  }
   const int kc = a.kc, k = a.k, kcap = a.kcap, M = a.M;
   const uint4* qrow = reinterpret_cast<const uint4*>(a.qs + (size_t)r * a.d);
   const int nvec = a.d / 8;   // d % 8 == 0
@@ -235,14 +246,27 @@ finish_kernel(FinishArgs a, InstTable t, const CallParams* __restrict__ cp) {
       if (p < kMaxFlag) s_flag[p] = tid;
     }
     __syncthreads();
-    const int nflag = min(s_nflag, kMaxFlag);
+    if (tid == 0) {   // lists -> CTAs (slabs), each once
+      const int nl = min(s_nflag, kMaxFlag);
+      int nc = 0;
+      for (int f = 0; f < nl; ++f) {
+        const int c = s_flag[f] / a.lists_per_cta;
+        bool seen = false;
+        for (int g = 0; g < nc; ++g) seen |= (s_flag[g] == c);
+        if (!seen) s_flag[nc++] = c;
+      }
+      s_nflag = nc;
+    }
+    __syncthreads();
+    const int nflag = s_nflag;
+    const int nctas = a.nlists / a.lists_per_cta;
     // every warp keeps the best kc of the rows it visits: rank l in lane l (a) and rank 32+l (b)
     unsigned long long la = 0, lb = 0, thr = 0;
     const int64_t units = (a.N + kBoxN - 1) / kBoxN;
     for (int f = 0; f < nflag; ++f) {
       const int c = s_flag[f];
-      const int64_t row0 = units * c / a.nlists * kBoxN;
-      int64_t row1 = units * (c + 1) / a.nlists * kBoxN;
+      const int64_t row0 = units * c / nctas * kBoxN;
+      int64_t row1 = units * (c + 1) / nctas * kBoxN;
       if (row1 > a.N) row1 = a.N;
       for (int64_t n = row0 + warp; n < row1; n += nwarps) {
         const float sx = exact_sim_bf16(qrow, reinterpret_cast<const uint4*>(a.bank + (size_t)n * a.d), nvec, lane);
@@ -265,7 +289,7 @@ finish_kernel(FinishArgs a, InstTable t, const CallParams* __restrict__ cp) {
       int o = 0;
       for (int j = 0; j < kc; ++j) {
         bool from_flagged = false;
-        for (int f = 0; f < nflag; ++f) from_flagged |= (s_src[j] == s_flag[f]);
+        for (int f = 0; f < nflag; ++f) from_flagged |= (s_src[j] / a.lists_per_cta == s_flag[f]);
         if (s_cand[j] != 0ull && !from_flagged) s_keys[(size_t)nwarps * kMerge2Stride + o++] = s_cand[j];
       }
       for (; o < kMerge2Stride; ++o) s_keys[(size_t)nwarps * kMerge2Stride + o] = 0ull;
@@ -280,6 +304,19 @@ finish_kernel(FinishArgs a, InstTable t, const CallParams* __restrict__ cp) {
   }
   __syncthreads();
 
+  // labels of all kc candidates are requested before the re-rank and parked after it (independent gathers)
+  float lv[4];
+  const int nlab = kc * 2 * M;   // <= 64 * 32 = 4 * 512
+#pragma unroll
+  for (int u = 0; u < 4; ++u) {
+    const int e = tid + u * kFinThreads;
+    lv[u] = 0.0f;
+    if (e < nlab) {
+      const int c = e / (2 * M), col = e - c * 2 * M;
+      const int32_t id = s_idx[c];
+      if (id >= 0) lv[u] = (col < M) ? a.bank_quality[(size_t)id * M + col] : a.bank_outlen[(size_t)id * M + col - M];
+    }
+  }
   // ---- exact re-rank ----
   if (a.rerank) {
     for (int c = warp; c < kc; c += nwarps) {
@@ -302,6 +339,12 @@ finish_kernel(FinishArgs a, InstTable t, const CallParams* __restrict__ cp) {
     }
     o_sim[rank] = s_sim[tid];
     o_idx[rank] = id;
+    o_pos[rank] = tid;
+  }
+#pragma unroll
+  for (int u = 0; u < 4; ++u) {
+    const int e = tid + u * kFinThreads;
+    if (e < nlab) s_lab[e / (2 * M)][e % (2 * M)] = lv[u];
   }
   __syncthreads();
   // ---- weights ----
@@ -325,12 +368,11 @@ finish_kernel(FinishArgs a, InstTable t, const CallParams* __restrict__ cp) {
   // ---- aggregate: thread m < M -> quality, M <= thread < 2M -> output length ----
   if (tid < 2 * M) {
     const int m = tid % M;
-    const float* lab = (tid < M) ? a.bank_quality : a.bank_outlen;
     float num = 0.0f, den = 0.0f;
     for (int j = 0; j < k; ++j) {
       const float w = s_w[j];
       if (o_idx[j] < 0) continue;
-      const float p = __fmul_rn(w, lab[(size_t)o_idx[j] * M + m]);
+      const float p = __fmul_rn(w, s_lab[o_pos[j]][tid]);
       num = __fadd_rn(num, p);
       den = __fadd_rn(den, w);
     }
@@ -348,8 +390,7 @@ finish_kernel(FinishArgs a, InstTable t, const CallParams* __restrict__ cp) {
   if (!a.with_terms) return;
   __syncthreads();
   // ---- per-(request, tier) terms ----
-  const float ell = (float)cp->plen[r];
-  if (tid < M) sC[tid] = __fadd_rn(__fmul_rn(ell, t.price_in[tid]), __fmul_rn(sL[tid], t.price_out[tid]));
+  if (tid < M) sC[tid] = __fadd_rn(__fmul_rn(c_ell, c_pin), __fmul_rn(sL[tid], c_pout));
   __syncthreads();
   if (tid < M) {
     const int m = tid;
@@ -363,7 +404,7 @@ finish_kernel(FinishArgs a, InstTable t, const CallParams* __restrict__ cp) {
     }
     const float ct = (Cmax > 0.0f) ? __fsub_rn(1.0f, __fdiv_rn(sC[m], Cmax)) : 0.0f;
     a.termA[(size_t)r * M + m] = __fadd_rn(__fmul_rn(cp->w_qual, sQ[m]), __fmul_rn(cp->w_cost, ct));
-    a.termP[(size_t)r * M + m] = __fmul_rn(t.pre[m], ell);
+    a.termP[(size_t)r * M + m] = __fmul_rn(c_pre, c_ell);
     if (m == 0) a.key[r] = __fadd_rn(kmax, 0.0f);   // -0 -> +0 so that the sort key order equals float order
   }
 }
@@ -377,11 +418,11 @@ cudaError_t launch_convert_bf16(const float* in, __nv_bfloat16* out, size_t n, c
   return cudaGetLastError();
 }
 
-cudaError_t launch_stage_queries(const CallParams* cp, __nv_bfloat16* qs, int B, int Bpad, int d, cudaStream_t s) {
+cudaError_t launch_stage_queries(const CallParams* cp, __nv_bfloat16* qs, int B, int Bpad, int d, int rep, cudaStream_t s) {
   const size_t n = (size_t)Bpad * d;
   int blocks = (int)((n + 255) / 256);
   if (blocks > 148 * 8) blocks = 148 * 8;
-  stage_queries_kernel<<<blocks, 256, 0, s>>>(cp, qs, B, Bpad, d);
+  stage_queries_kernel<<<blocks, 256, 0, s>>>(cp, qs, B, Bpad, d, rep > 1 ? kTileM / rep : Bpad);
   return cudaGetLastError();
 }
 
@@ -399,7 +440,7 @@ cudaError_t launch_select_f32(const float* sims, int64_t N, int nq, int kc, floa
 }
 
 size_t finish_smem_bytes(int nlists, int kcap) {
-  const size_t n1 = (size_t)nlists * kcap, n2 = (size_t)(kFinWarps + 1) * kMerge2Stride;
+  const size_t n1 = (size_t)nlists * kcap, n2 = (size_t)(kFinWarpsMax + 1) * kMerge2Stride;
   return (n1 > n2 ? n1 : n2) * sizeof(unsigned long long);
 }
 
@@ -408,7 +449,7 @@ cudaError_t finish_prepare(size_t max_smem) {
 }
 
 cudaError_t launch_finish(const FinishArgs& a, InstTable t, const CallParams* cp, int B, cudaStream_t s) {
-  finish_kernel<<<B, kFinThreads, finish_smem_bytes(a.nlists, a.kcap), s>>>(a, t, cp);
+  finish_kernel<<<B, a.nlists > 512 ? 1024 : 512, finish_smem_bytes(a.nlists, a.kcap), s>>>(a, t, cp);
   return cudaGetLastError();
 }
 

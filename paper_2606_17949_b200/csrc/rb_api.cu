@@ -34,6 +34,7 @@ struct rb_ctx {
   int I = 0;
   int32_t *tier = nullptr, *cap = nullptr, *present = nullptr;
   float *price_in = nullptr, *price_out = nullptr, *pre = nullptr, *dec = nullptr, *slope = nullptr;
+  float *dec_i = nullptr, *slope_i = nullptr;   // [I] per-instance copies of the tier coefficients
   float* dq = nullptr;
   int32_t* bq = nullptr;
   // per-call staging + scratch (sized by max_batch)
@@ -107,7 +108,7 @@ cudaError_t dev_alloc(T** p, size_t n) {
 InstTable table_of(const rb_ctx* c) {
   InstTable t;
   t.I = c->I; t.M = c->M; t.tier = c->tier; t.cap = c->cap; t.price_in = c->price_in; t.price_out = c->price_out;
-  t.pre = c->pre; t.dec = c->dec; t.slope = c->slope; t.present = c->present;
+  t.pre = c->pre; t.dec = c->dec; t.slope = c->slope; t.present = c->present; t.dec_i = c->dec_i; t.slope_i = c->slope_i;
   return t;
 }
 
@@ -168,13 +169,14 @@ rb_status enqueue_estimate(rb_ctx* ctx, int B, bool with_terms, Timer& tm) {
   fa.pred_q = ctx->pred_q; fa.pred_l = ctx->pred_l; fa.termA = ctx->termA; fa.termP = ctx->termP; fa.key = ctx->key;
   if (ctx->opt.store_dtype == RB_BF16) {
     tm.mark();
-    CK(launch_stage_queries(ctx->cp, ctx->qs, B, Bpad, ctx->d, s));
+    const int rep = scan_tc_replicas(B);
+    CK(launch_stage_queries(ctx->cp, ctx->qs, B, Bpad, ctx->d, rep, s));
     tm.mark();
     int grid = 0;
     CK(launch_scan_tc(&ctx->tm_q, &ctx->tm_bank, ctx->N, ctx->d, B, Bpad, ctx->ks, ctx->num_sms, ctx->part_sim,
                       ctx->part_idx, &grid, s));
     tm.mark();
-    fa.part_sim = ctx->part_sim; fa.part_idx = ctx->part_idx; fa.nlists = grid; fa.kcap = ctx->ks; fa.Bpad = Bpad;
+    fa.part_sim = ctx->part_sim; fa.part_idx = ctx->part_idx; fa.nlists = grid * rep; fa.lists_per_cta = rep; fa.kcap = ctx->ks; fa.Bpad = Bpad;
     fa.rescan = ctx->ks < ctx->kc ? 1 : 0;
     fa.bank = (const __nv_bfloat16*)ctx->bank; fa.qs = ctx->qs; fa.rerank = ctx->opt.rerank_slack > 0 ? 1 : 0;
     ctx->launches += 2;
@@ -190,7 +192,7 @@ rb_status enqueue_estimate(rb_ctx* ctx, int B, bool with_terms, Timer& tm) {
     }
     tm.mark();
     // the selected candidates are one already-merged list per query: [1][B][kc]
-    fa.part_sim = ctx->cand_sim; fa.part_idx = ctx->cand_idx; fa.nlists = 1; fa.kcap = ctx->kc; fa.Bpad = B;
+    fa.part_sim = ctx->cand_sim; fa.part_idx = ctx->cand_idx; fa.nlists = 1; fa.lists_per_cta = 1; fa.kcap = ctx->kc; fa.Bpad = B;
     fa.bank = nullptr; fa.qs = nullptr; fa.rerank = 0;
   }
   CK(launch_finish(fa, table_of(ctx), ctx->cp, B, s));
@@ -475,10 +477,14 @@ rb_status rb_create(rb_ctx** out, const void* bank_emb, const float* bank_qualit
   ALLOC(ctx->pre, kMaxM);
   ALLOC(ctx->dec, kMaxM);
   ALLOC(ctx->slope, kMaxM);
+  ALLOC(ctx->dec_i, kMaxI);
+  ALLOC(ctx->slope_i, kMaxI);
   if (opt.store_dtype == RB_BF16) {
     ALLOC(ctx->qs, (size_t)ctx->Bpad_max * d);
-    ALLOC(ctx->part_sim, (size_t)ctx->num_sms * ctx->kcap * ctx->Bpad_max);
-    ALLOC(ctx->part_idx, (size_t)ctx->num_sms * ctx->kcap * ctx->Bpad_max);
+    // [grid * rep][Bpad][ks]: rep = 4 replicas only when Bpad = 128
+    const size_t part_n = (size_t)ctx->num_sms * ctx->kcap * std::max<size_t>(ctx->Bpad_max, 4 * kTileM);
+    ALLOC(ctx->part_sim, part_n);
+    ALLOC(ctx->part_idx, part_n);
     CK(cudaMemsetAsync(ctx->qs, 0, (size_t)ctx->Bpad_max * d * 2, s));
     rb_status st = encode_map(ctx, &ctx->tm_bank, ctx->bank, (uint64_t)N, (uint64_t)d, kBoxN);
     if (st != RB_OK) return st;
@@ -487,8 +493,9 @@ rb_status rb_create(rb_ctx** out, const void* bank_emb, const float* bank_qualit
     CK(scan_tc_prepare());
   }
   {
-    const size_t fin = std::max(finish_smem_bytes(ctx->num_sms, ctx->ks), finish_smem_bytes(1, ctx->kc));
+    const size_t fin = std::max(finish_smem_bytes(ctx->num_sms * 4, ctx->ks), finish_smem_bytes(1, ctx->kc));
     CK(finish_prepare(fin));
+    CK(lpt_dispatch_prepare());
   }
   ALLOC(ctx->scratch_nn_idx, mb * k);
   ALLOC(ctx->scratch_nn_sim, mb * k);
@@ -517,6 +524,8 @@ rb_status rb_set_instances(rb_ctx* ctx, int32_t I, const int32_t* tier, const in
       return fail(ctx, RB_EINVAL, "latency head coefficients must be finite, >= 0");
     pre[m] = heads[m].prefill_ms_per_tok; dec[m] = heads[m].decode_ms_per_tok; slope[m] = heads[m].batch_slope;
   }
+  std::vector<float> dec_i(I), slope_i(I);
+  for (int i = 0; i < I; ++i) { dec_i[i] = dec[tier[i]]; slope_i[i] = slope[tier[i]]; }
   cudaStream_t s = ctx->stream;
   // scores buffers depend on I
   if (I != ctx->I) {
@@ -541,6 +550,8 @@ rb_status rb_set_instances(rb_ctx* ctx, int32_t I, const int32_t* tier, const in
   CK(cudaMemcpyAsync(ctx->pre, pre, M * 4, cudaMemcpyHostToDevice, s));
   CK(cudaMemcpyAsync(ctx->dec, dec, M * 4, cudaMemcpyHostToDevice, s));
   CK(cudaMemcpyAsync(ctx->slope, slope, M * 4, cudaMemcpyHostToDevice, s));
+  CK(cudaMemcpyAsync(ctx->dec_i, dec_i.data(), I * 4, cudaMemcpyHostToDevice, s));
+  CK(cudaMemcpyAsync(ctx->slope_i, slope_i.data(), I * 4, cudaMemcpyHostToDevice, s));
   CK(cudaMemsetAsync(ctx->dq, 0, kMaxI * 4, s));
   CK(cudaMemsetAsync(ctx->bq, 0, kMaxI * 4, s));
   CK(cudaStreamSynchronize(s));   // stack arrays above are read by pageable copies
@@ -698,7 +709,7 @@ void rb_destroy(rb_ctx* ctx) {
   if (ctx->stream) cudaStreamSynchronize(ctx->stream);
   for (auto& kv : ctx->graphs) cudaGraphExecDestroy(kv.second);
   void* ptrs[] = {ctx->bank, ctx->bank_quality, ctx->bank_outlen, ctx->tier, ctx->cap, ctx->present, ctx->price_in,
-                  ctx->price_out, ctx->pre, ctx->dec, ctx->slope, ctx->dq, ctx->bq, ctx->q32, ctx->qs, ctx->plen, ctx->cp,
+                  ctx->price_out, ctx->pre, ctx->dec, ctx->slope, ctx->dec_i, ctx->slope_i, ctx->dq, ctx->bq, ctx->q32, ctx->qs, ctx->plen, ctx->cp,
                   ctx->part_sim, ctx->part_idx, ctx->sims, ctx->cand_sim, ctx->cand_idx, ctx->scratch_nn_idx, ctx->scratch_nn_sim, ctx->stage_q, ctx->stage_l,
                   ctx->pred_q, ctx->pred_l, ctx->termA, ctx->termP, ctx->key, ctx->order, ctx->assignment, ctx->scores,
                   ctx->scores0};

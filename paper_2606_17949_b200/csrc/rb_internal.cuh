@@ -26,6 +26,8 @@ struct InstTable {
   const float* dec;        // [M]
   const float* slope;      // [M]
   const int32_t* present;  // [M] 1 if the tier has an instance
+  const float* dec_i;      // [I] dec[tier[i]]   (per-instance copies: no dependent lookups in the dispatch loop)
+  const float* slope_i;    // [I] slope[tier[i]]
 };
 
 // Per-call parameters live in device memory so that a captured graph can be replayed with new weights and new
@@ -52,10 +54,12 @@ struct CallParams {
 // fp32 -> bf16 (RNE), n elements (bank conversion in rb_create).
 cudaError_t launch_convert_bf16(const float* in, __nv_bfloat16* out, size_t n, cudaStream_t s);
 
-// a0: cp->query (fp32) -> bf16 staging [Bpad x d], rows >= B zeroed.
-cudaError_t launch_stage_queries(const CallParams* cp, __nv_bfloat16* qs, int B, int Bpad, int d, cudaStream_t s);
+// a0: cp->query (fp32) -> bf16 staging [Bpad x d]; rep copies of the B queries at rows j*(128/rep) + r (rep > 1 only
+// when Bpad = 128), all other rows zero.
+cudaError_t launch_stage_queries(const CallParams* cp, __nv_bfloat16* qs, int B, int Bpad, int d, int rep, cudaStream_t s);
+int scan_tc_replicas(int B);   // 4 (B <= 32), 2 (B <= 64), 1: query replicas over the TMEM lane quarters
 
-// a1 (bf16): tcgen05 scan.  part_* are [grid][Bpad][KCAP] (sim fp32 / idx int32, idx -1 = empty), each list
+// a1 (bf16): tcgen05 scan.  part_* are [grid * rep][Bpad][KCAP] (sim fp32 / idx int32, idx -1 = empty), each list
 // sorted by (sim desc, idx asc).  Returns the grid size used through *grid_out.  kcap in {4,8,16,32,64}; bank
 // rows are split over the CTAs in units of kBoxN rows: CTA c owns units [units*c/grid, units*(c+1)/grid).
 cudaError_t launch_scan_tc(const CUtensorMap* tm_q, const CUtensorMap* tm_bank, int64_t N, int d, int B, int Bpad,
@@ -78,7 +82,8 @@ cudaError_t launch_select_f32(const float* sims, int64_t N, int nq, int kc, floa
 struct FinishArgs {
   const float* part_sim;
   const int32_t* part_idx;
-  int nlists, kcap, Bpad, kc, k;
+  int nlists, kcap, Bpad, kc, k;   // nlists = grid * lists_per_cta
+  int lists_per_cta;
   int64_t N;
   const __nv_bfloat16* bank;
   const __nv_bfloat16* qs;
@@ -108,6 +113,8 @@ cudaError_t launch_score(InstTable t, const float* dq, const int32_t* bq, const 
 cudaError_t launch_lpt_dispatch(InstTable t, float* dq, int32_t* bq, const float* termA, const float* termP,
                                 const float* key, const CallParams* cp, int B, int lpt_enabled, int update_enabled,
                                 cudaStream_t s);
+
+cudaError_t lpt_dispatch_prepare();  // opt in to the dynamic shared memory size; call once
 
 // a8: dead reckoning between batches.
 cudaError_t launch_advance(InstTable t, float* dq, int32_t* bq, float elapsed_ms, cudaStream_t s);

@@ -17,7 +17,8 @@
 //            shared-memory buffer, then insert them into a sorted register list in warp lock-step.
 // Bank rows are split over CTAs in units of 64 rows; a CTA walks its slab in tiles of 256 rows and, for
 // B > 128, revisits each tile once per 128-query m-tile (bank tile then comes from L2), carrying the lists
-// through global memory between visits.
+// through global memory between visits.  For B <= 64 the queries are replicated over the lane quarters so that
+// all four epilogue warps share the columns of a tile (the epilogue of a short slab is latency-bound).
 #include "rb_internal.cuh"
 
 namespace rb {
@@ -44,7 +45,7 @@ constexpr int kBBytes = kTileN * kTileK * 2;       // 32 KB
 constexpr int kStageBytes = kABytes + kBBytes;     // 48 KB
 constexpr int kCandSlots = 32;                     // one tcgen05.ld chunk can yield at most 32 survivors
 constexpr int kThreads = 192;
-constexpr int kSmemBytes = kStages * kStageBytes + kCandSlots * kTileM * 5 + 256 + 1024;
+constexpr int kSmemBytes = kStages * kStageBytes + kCandSlots * kTileM * 8 + 256 + 1024;
 
 // ---- PTX wrappers --------------------------------------------------------------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -142,17 +143,56 @@ __device__ __forceinline__ void list_insert(float (&v)[K], int32_t (&ix)[K], flo
   ix[0] = top ? id : ix[0];
 }
 
+// One tcgen05.ld chunk (32 similarities of this thread's query against bank rows n0+c0 ..) folded into the
+// thread's sorted list.  Steady state: no lane of the warp holds a similarity above its threshold and the chunk
+// costs one max tree and one vote.  Otherwise the survivors (rare after warm-up) are parked in shared memory
+// and inserted in warp lock-step: every lane inserts its p-th survivor in the same iteration, so there is one
+// copy of the insertion code (the epilogue runs on few warps; its code must stay small).
+template <int K>
+__device__ __forceinline__ void fold_chunk(const uint32_t (&regs)[32], int c0, int c_end, int n0, float (&v)[K],
+                                           int32_t (&ix)[K], float& thr, uint2* cand, int tl) {
+  const bool full = c0 + 32 <= c_end;   // warp-uniform
+  float m0 = -INFINITY, m1 = -INFINITY, m2 = -INFINITY, m3 = -INFINITY;
+#pragma unroll
+  for (int j = 0; j < 32; j += 4) {
+    m0 = fmaxf(m0, (full || c0 + j + 0 < c_end) ? __uint_as_float(regs[j + 0]) : -INFINITY);
+    m1 = fmaxf(m1, (full || c0 + j + 1 < c_end) ? __uint_as_float(regs[j + 1]) : -INFINITY);
+    m2 = fmaxf(m2, (full || c0 + j + 2 < c_end) ? __uint_as_float(regs[j + 2]) : -INFINITY);
+    m3 = fmaxf(m3, (full || c0 + j + 3 < c_end) ? __uint_as_float(regs[j + 3]) : -INFINITY);
+  }
+  const float m = fmaxf(fmaxf(m0, m1), fmaxf(m2, m3));
+  if (!__any_sync(0xffffffffu, m > thr)) return;
+  int cnt = 0;
+#pragma unroll
+  for (int j = 0; j < 32; ++j) {
+    const float s = __uint_as_float(regs[j]);
+    if ((full || c0 + j < c_end) && s > thr) {
+      cand[cnt * kTileM + tl] = make_uint2(regs[j], (uint32_t)(c0 + j));
+      ++cnt;
+    }
+  }
+  uint2 nxt = cand[tl];
+  for (int p = 0; __any_sync(0xffffffffu, p < cnt); ++p) {
+    const uint2 cur = nxt;
+    nxt = cand[min(p + 1, kCandSlots - 1) * kTileM + tl];   // next survivor's slot is read while this one is inserted
+    const float s = __uint_as_float(cur.x);
+    if (p < cnt && s > thr) {
+      list_insert<K>(v, ix, s, n0 + (int)cur.y);
+      thr = v[K - 1];
+    }
+  }
+}
+
 __device__ __forceinline__ bool tl_trace_end(int tid) { return tid == 128; }   // epilogue thread of query 0
 
 template <int KCAP>
 __global__ void __launch_bounds__(kThreads, 1)
 scan_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_bank, int64_t N, int d,
-               int B, int Bpad, float* __restrict__ part_sim, int32_t* __restrict__ part_idx) {
+               int B, int Bpad, int rep, float* __restrict__ part_sim, int32_t* __restrict__ part_idx) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);   // 128B swizzle wants 1024 B alignment
-  float* cand_s = (float*)(smem + kStages * kStageBytes);
-  uint8_t* cand_c = (uint8_t*)(cand_s + kCandSlots * kTileM);
-  uint64_t* bars = (uint64_t*)(cand_c + kCandSlots * kTileM);
+  uint2* cand = (uint2*)(smem + kStages * kStageBytes);   // [kCandSlots][128]: (similarity bits, column)
+  uint64_t* bars = (uint64_t*)(cand + kCandSlots * kTileM);
   uint64_t* full = bars;                  // [kStages] TMA bytes landed
   uint64_t* empty = bars + kStages;       // [kStages] MMAs that read the slot retired
   uint64_t* tfull = bars + 2 * kStages;   // [2] accumulator complete
@@ -253,8 +293,15 @@ scan_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__
     __syncwarp();
   } else {
     // ===== epilogue: fused per-query top-KCAP =====
+    // rep = 4 (B <= 32) / 2 (B <= 64): the staged queries are replicated over the TMEM lane quarters, so each
+    // quarter's warp sees every query and folds its own share of the tile's columns into its own list
+    // (list index = CTA * rep + replica).  rep = 1: one query per TMEM lane, all columns.
     const int quarter = warp & 3;              // TMEM lane quarter this warp may read
-    const int tl = quarter * 32 + lane;        // TMEM lane = query row inside the m-tile
+    const int tl = quarter * 32 + lane;        // TMEM lane inside the m-tile
+    const int group = kTileM / rep;            // lanes per replica
+    const int replica = tl / group;
+    const int col_lo = replica * (kTileN / rep);
+    const int col_hi = col_lo + kTileN / rep;
     float v[KCAP];
     int32_t ix[KCAP];
     uint32_t it = 0;
@@ -263,11 +310,12 @@ scan_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__
       const int nun = min(4, nunits - tile * 4);
       const int ncols = nun * kBoxN;
       const int nvalid = (int)min((int64_t)ncols, N - (int64_t)n0);   // rows >= N are TMA zero fill
+      const int c_end = min(col_hi, nvalid);
       for (int mt = 0; mt < n_mt; ++mt, ++it) {
         const uint32_t acc = it & 1, aph = (it >> 1) & 1;
-        const int r = mt * kTileM + tl;
-        const bool warp_active = (mt * kTileM + quarter * 32) < B;   // warp-uniform
-        const size_t pbase = ((size_t)blockIdx.x * (size_t)Bpad + (size_t)r) * KCAP;   // [grid][Bpad][KCAP]
+        const int r = mt * kTileM + (tl - replica * group);
+        const bool warp_active = (mt * kTileM + (quarter * 32) % group) < B;   // warp-uniform
+        const size_t pbase = (((size_t)blockIdx.x * rep + replica) * (size_t)Bpad + (size_t)r) * KCAP;
         float4* ps4 = reinterpret_cast<float4*>(part_sim + pbase);
         int4* pi4 = reinterpret_cast<int4*>(part_idx + pbase);
         if (warp_active) {
@@ -290,41 +338,22 @@ scan_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__
         if (warp_active) {
           float thr = (r < B) ? v[KCAP - 1] : INFINITY;   // padding lanes never collect
           const uint32_t taddr = tmem_base + ((uint32_t)(quarter * 32) << 16) + acc * kTileN;
-          for (int c0 = 0; c0 < nvalid; c0 += 32) {
-            uint32_t regs[32];
-            tmem_ld32(taddr + c0, regs);
-            tmem_ld_wait();
-            int cnt = 0;
-            if (c0 + 32 <= nvalid) {
-#pragma unroll
-              for (int j = 0; j < 32; ++j) {
-                const float s = __uint_as_float(regs[j]);
-                if (s > thr) {
-                  cand_s[cnt * kTileM + tl] = s;
-                  cand_c[cnt * kTileM + tl] = (uint8_t)(c0 + j);
-                  ++cnt;
-                }
-              }
-            } else {
-#pragma unroll
-              for (int j = 0; j < 32; ++j) {
-                const float s = __uint_as_float(regs[j]);
-                if ((c0 + j < nvalid) && s > thr) {
-                  cand_s[cnt * kTileM + tl] = s;
-                  cand_c[cnt * kTileM + tl] = (uint8_t)(c0 + j);
-                  ++cnt;
-                }
-              }
+          if constexpr (KCAP <= 16) {   // two loads in flight per wait; longer lists need the registers
+            for (int c0 = col_lo; c0 < c_end; c0 += 64) {
+              uint32_t ra[32], rb[32];
+              const bool two = c0 + 32 < c_end;   // warp-uniform; the accumulator holds a multiple of 64 columns
+              tmem_ld32(taddr + c0, ra);
+              if (two) tmem_ld32(taddr + c0 + 32, rb);
+              tmem_ld_wait();
+              fold_chunk<KCAP>(ra, c0, c_end, n0, v, ix, thr, cand, tl);
+              if (two) fold_chunk<KCAP>(rb, c0 + 32, c_end, n0, v, ix, thr, cand, tl);
             }
-            // lock-step drain: every lane inserts its p-th survivor in the same iteration
-            for (int p = 0; __any_sync(0xffffffffu, p < cnt); ++p) {
-              if (p < cnt) {
-                const float s = cand_s[p * kTileM + tl];
-                if (s > thr) {
-                  list_insert<KCAP>(v, ix, s, n0 + (int)cand_c[p * kTileM + tl]);
-                  thr = v[KCAP - 1];
-                }
-              }
+          } else {
+            for (int c0 = col_lo; c0 < c_end; c0 += 32) {
+              uint32_t ra[32];
+              tmem_ld32(taddr + c0, ra);
+              tmem_ld_wait();
+              fold_chunk<KCAP>(ra, c0, c_end, n0, v, ix, thr, cand, tl);
             }
           }
         }
@@ -370,21 +399,24 @@ cudaError_t scan_tc_prepare() {
   return cudaFuncSetAttribute(scan_tc_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
 }
 
+int scan_tc_replicas(int B) { return B <= 32 ? 4 : (B <= 64 ? 2 : 1); }
+
 cudaError_t launch_scan_tc(const CUtensorMap* tm_q, const CUtensorMap* tm_bank, int64_t N, int d, int B, int Bpad,
                            int kcap, int max_grid, float* part_sim, int32_t* part_idx, int* grid_out, cudaStream_t s) {
   const int64_t units = (N + kBoxN - 1) / kBoxN;
   const int grid = (int)(units < max_grid ? units : max_grid);
+  const int rep = scan_tc_replicas(B);
   if (grid_out) *grid_out = grid;
-  if (kcap == 4)
-    scan_tc_kernel<4><<<grid, kThreads, kSmemBytes, s>>>(*tm_q, *tm_bank, N, d, B, Bpad, part_sim, part_idx);
-  else if (kcap == 8)
-    scan_tc_kernel<8><<<grid, kThreads, kSmemBytes, s>>>(*tm_q, *tm_bank, N, d, B, Bpad, part_sim, part_idx);
-  else if (kcap == 16)
-    scan_tc_kernel<16><<<grid, kThreads, kSmemBytes, s>>>(*tm_q, *tm_bank, N, d, B, Bpad, part_sim, part_idx);
-  else if (kcap == 32)
-    scan_tc_kernel<32><<<grid, kThreads, kSmemBytes, s>>>(*tm_q, *tm_bank, N, d, B, Bpad, part_sim, part_idx);
-  else
-    scan_tc_kernel<64><<<grid, kThreads, kSmemBytes, s>>>(*tm_q, *tm_bank, N, d, B, Bpad, part_sim, part_idx);
+#define RB_SCAN_LAUNCH(KC) \
+  scan_tc_kernel<KC><<<grid, kThreads, kSmemBytes, s>>>(*tm_q, *tm_bank, N, d, B, Bpad, rep, part_sim, part_idx)
+  switch (kcap) {
+    case 4: RB_SCAN_LAUNCH(4); break;
+    case 8: RB_SCAN_LAUNCH(8); break;
+    case 16: RB_SCAN_LAUNCH(16); break;
+    case 32: RB_SCAN_LAUNCH(32); break;
+    default: RB_SCAN_LAUNCH(64); break;
+  }
+#undef RB_SCAN_LAUNCH
   return cudaGetLastError();
 }
 
