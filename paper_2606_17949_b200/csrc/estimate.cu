@@ -23,6 +23,7 @@ __device__ __forceinline__ unsigned long long make_key(float sim, int32_t idx) {
 // ---- a0 ---------------------------------------------------------------------------------------------
 __global__ void stage_queries_kernel(const CallParams* __restrict__ cp, __nv_bfloat16* __restrict__ qs, int B, int Bpad,
                                      int d, int group) {
+  launch_dependents();
   const float* __restrict__ q = cp->query;
   const size_t n = (size_t)Bpad * d;
   for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
@@ -164,6 +165,29 @@ __device__ __forceinline__ float exact_sim_bf16(const uint4* __restrict__ qrow, 
   return (float)acc;
 }
 
+// Warp-level k-way merge: lane l owns the sorted list keys[(first + l)*stride ..] (l < nl <= 32) and the warp
+// pops the kc largest keys, in order, into out_key / out_src (the owning list's index).  No block barrier.
+__device__ __forceinline__ void warp_kway_merge(const unsigned long long* keys, int first, int nl, int stride, int len,
+                                                int kc, unsigned long long* out_key, int* out_src) {
+  const int lane = threadIdx.x & 31;
+  const unsigned long long* mine = keys + (size_t)(first + lane) * stride;
+  int pos = 0;
+  unsigned long long hk = (lane < nl) ? mine[0] : 0ull;
+  for (int j = 0; j < kc; ++j) {
+    const uint32_t hi = (uint32_t)(hk >> 32), lo = (uint32_t)hk;
+    const uint32_t ghi = __reduce_max_sync(0xffffffffu, hi);
+    const uint32_t glo = __reduce_max_sync(0xffffffffu, hi == ghi ? lo : 0u);
+    const unsigned long long win = ((unsigned long long)ghi << 32) | glo;
+    if (win != 0ull && hk == win) {   // keys are distinct: exactly one owner
+      out_key[j] = win;
+      out_src[j] = first + lane;
+      ++pos;
+      hk = pos < len ? mine[pos] : 0ull;
+    }
+    if (win == 0ull && lane == 0) { out_key[j] = 0ull; out_src[j] = -1; }
+  }
+}
+
 // Block-wide k-way merge: thread c < nl owns the sorted list keys[c*stride .. c*stride+len); pops the kc largest
 // keys into out_key[0..kc) (0 = exhausted) and the list each came from into out_src.  Returns how many entries
 // of the caller's own list were popped.  All threads of the block must call.
@@ -229,6 +253,8 @@ finish_kernel(FinishArgs a, InstTable t, const CallParams* __restrict__ cp) {
   // ---- merge ----
   const int total = a.nlists * kcap;
   if (tid == 0) s_nflag = 0;
+  launch_dependents();
+  grid_dependency_wait();   // the partial lists come from the preceding kernel
   for (int e = tid; e < total; e += kFinThreads) {
     const int c = e / kcap, j = e - c * kcap;
     const size_t off = ((size_t)c * a.Bpad + r) * kcap + j;
@@ -236,14 +262,55 @@ finish_kernel(FinishArgs a, InstTable t, const CallParams* __restrict__ cp) {
     s_keys[e] = (id >= 0 && (int64_t)id < a.N) ? make_key(a.part_sim[off], id) : 0ull;
   }
   __syncthreads();
-  const int popped = kway_merge(s_keys, a.nlists, kcap, kcap, kc, s_red, s_cand, s_src);
+  // two levels, no barrier inside either: every warp pops the kc best of its own share of the lists (lane = list),
+  // then warp 0 pops the kc best of the warps' results (lane = warp)
+  unsigned long long* w_key = s_keys + total;                         // [nwarps][kMerge2Stride]
+  int* w_src = reinterpret_cast<int*>(w_key + (size_t)nwarps * kMerge2Stride);   // [nwarps][kMerge2Stride]
+  {
+    const int per = (a.nlists + nwarps - 1) / nwarps;                 // <= 32 by the choice of the block size
+    const int first = warp * per;
+    const int nl = max(0, min(per, a.nlists - first));
+    warp_kway_merge(s_keys, first, nl, kcap, kcap, kc, w_key + (size_t)warp * kMerge2Stride,
+                    w_src + (size_t)warp * kMerge2Stride);
+  }
+  __syncthreads();
+  if (warp == 0) {
+    // out_src of this level is the warp whose list the key came from; its position in that list is the number
+    // of keys already taken from it, which recovers the original list index
+    const unsigned long long* mine = w_key + (size_t)lane * kMerge2Stride;
+    int pos = 0;
+    unsigned long long hk = (lane < nwarps) ? mine[0] : 0ull;
+    for (int j = 0; j < kc; ++j) {
+      const uint32_t hi = (uint32_t)(hk >> 32), lo = (uint32_t)hk;
+      const uint32_t ghi = __reduce_max_sync(0xffffffffu, hi);
+      const uint32_t glo = __reduce_max_sync(0xffffffffu, hi == ghi ? lo : 0u);
+      const unsigned long long win = ((unsigned long long)ghi << 32) | glo;
+      if (win != 0ull && hk == win) {
+        s_cand[j] = win;
+        s_src[j] = w_src[(size_t)lane * kMerge2Stride + pos];
+        ++pos;
+        hk = pos < kc ? mine[pos] : 0ull;
+      }
+      if (win == 0ull && lane == 0) { s_cand[j] = 0ull; s_src[j] = -1; }
+    }
+  }
+  __syncthreads();
 
   // ---- rescan of slabs whose list was popped completely ----
-  const bool flagged = a.rescan && tid < a.nlists && popped == kcap;
+  // (a list of kcap entries all of which are among the kc best may hide further members)
+  bool flagged = false;
+  if (a.rescan && tid < kc && s_src[tid] >= 0) {
+    int same = 0, earlier = 0;
+    for (int j = 0; j < kc; ++j) {
+      same += (s_src[j] == s_src[tid]);
+      earlier += (j < tid && s_src[j] == s_src[tid]);
+    }
+    flagged = (same == kcap) && (earlier == 0);
+  }
   if (__syncthreads_or(flagged)) {
     if (flagged) {
       const int p = atomicAdd(&s_nflag, 1);
-      if (p < kMaxFlag) s_flag[p] = tid;
+      if (p < kMaxFlag) s_flag[p] = s_src[tid];
     }
     __syncthreads();
     if (tid == 0) {   // lists -> CTAs (slabs), each once
@@ -440,8 +507,10 @@ cudaError_t launch_select_f32(const float* sims, int64_t N, int nq, int kc, floa
 }
 
 size_t finish_smem_bytes(int nlists, int kcap) {
-  const size_t n1 = (size_t)nlists * kcap, n2 = (size_t)(kFinWarpsMax + 1) * kMerge2Stride;
-  return (n1 > n2 ? n1 : n2) * sizeof(unsigned long long);
+  // keys of all lists + the warps' merged lists (keys and sources); the rescan's second merge reuses the front
+  const size_t n1 = (size_t)nlists * kcap * 8 + (size_t)kFinWarpsMax * kMerge2Stride * 12;
+  const size_t n2 = (size_t)(kFinWarpsMax + 1) * kMerge2Stride * 8;
+  return n1 > n2 ? n1 : n2;
 }
 
 cudaError_t finish_prepare(size_t max_smem) {
@@ -449,8 +518,9 @@ cudaError_t finish_prepare(size_t max_smem) {
 }
 
 cudaError_t launch_finish(const FinishArgs& a, InstTable t, const CallParams* cp, int B, cudaStream_t s) {
-  finish_kernel<<<B, a.nlists > 512 ? 1024 : 512, finish_smem_bytes(a.nlists, a.kcap), s>>>(a, t, cp);
-  return cudaGetLastError();
+  const cudaError_t e = launch_chained(finish_kernel, dim3(B), dim3(a.nlists > 512 ? 1024 : 512),
+                                       finish_smem_bytes(a.nlists, a.kcap), s, a, t, cp);
+  return e != cudaSuccess ? e : cudaGetLastError();
 }
 
 }  // namespace rb

@@ -50,6 +50,31 @@ struct CallParams {
   float* nn_sim;
 };
 
+// ---- programmatic dependent launch ---------------------------------------------------------------------------
+// Consecutive kernels of one decision are chained with programmatic stream serialization: a kernel lets its
+// successor start (launch_dependents, first thing) so that the successor's launch latency and prologue overlap
+// with it, and waits (grid_dependency_wait) before it touches anything its predecessor produces.  Both are
+// no-ops for a kernel launched without the attribute.
+#ifdef __CUDACC__
+__device__ __forceinline__ void launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void grid_dependency_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
+template <typename... KArgs, typename... Args>
+cudaError_t launch_chained(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t s, Args... args) {
+  cudaLaunchConfig_t cfg{};
+  cfg.gridDim = grid;
+  cfg.blockDim = block;
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = s;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at;
+  cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
+}
+#endif
+
 // ---- launchers (each returns the cudaError of its launch) ---------------------------------------------
 // fp32 -> bf16 (RNE), n elements (bank conversion in rb_create).
 cudaError_t launch_convert_bf16(const float* in, __nv_bfloat16* out, size_t n, cudaStream_t s);

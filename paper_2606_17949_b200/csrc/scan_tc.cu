@@ -209,6 +209,7 @@ scan_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__
   const int64_t row0 = u0 * kBoxN;
   const int ntiles = (nunits + 3) / 4;
 
+  launch_dependents();
   if (threadIdx.x == 0) RB_TR(0);
   if (warp == 0 && lane == 0) {
     asm volatile("prefetch.tensormap [%0];" ::"l"(&tm_q) : "memory");
@@ -237,6 +238,7 @@ scan_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__
   if (warp == 0) {
     // ===== TMA producer =====
     if (lane == 0) {
+      grid_dependency_wait();   // the staged queries come from the preceding kernel
       uint32_t kit = 0;
       for (int tile = 0; tile < ntiles; ++tile) {
         const int n0 = (int)(row0 + (int64_t)tile * kTileN);
@@ -407,8 +409,10 @@ cudaError_t launch_scan_tc(const CUtensorMap* tm_q, const CUtensorMap* tm_bank, 
   const int grid = (int)(units < max_grid ? units : max_grid);
   const int rep = scan_tc_replicas(B);
   if (grid_out) *grid_out = grid;
-#define RB_SCAN_LAUNCH(KC) \
-  scan_tc_kernel<KC><<<grid, kThreads, kSmemBytes, s>>>(*tm_q, *tm_bank, N, d, B, Bpad, rep, part_sim, part_idx)
+  cudaError_t e = cudaSuccess;
+#define RB_SCAN_LAUNCH(KC)                                                                                          \
+  e = launch_chained(scan_tc_kernel<KC>, dim3(grid), dim3(kThreads), kSmemBytes, s, *tm_q, *tm_bank, N, d, B, Bpad, rep, \
+                     part_sim, part_idx)
   switch (kcap) {
     case 4: RB_SCAN_LAUNCH(4); break;
     case 8: RB_SCAN_LAUNCH(8); break;
@@ -417,7 +421,7 @@ cudaError_t launch_scan_tc(const CUtensorMap* tm_q, const CUtensorMap* tm_bank, 
     default: RB_SCAN_LAUNCH(64); break;
   }
 #undef RB_SCAN_LAUNCH
-  return cudaGetLastError();
+  return e != cudaSuccess ? e : cudaGetLastError();
 }
 
 }  // namespace rb
