@@ -56,6 +56,7 @@ def parse_args(argv=None):
     ap.add_argument("--l2", default="flush", choices=["flush", "warm"],
                     help="flush: read a 3x-L2 buffer before every timed step; warm: back-to-back steps")
     ap.add_argument("--no-scan-c4", action="store_true", help="skip the C4 (10M x 384) bank-scan roofline leg")
+    ap.add_argument("--only-scan-c4", action="store_true", help="run only the C4 bank-scan leg (profiling runs)")
     ap.add_argument("--skip-cpu", action="store_true", help="skip the cpu_baseline / parity leg (profiling runs)")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="budget of the cpu_baseline sample")
     return ap.parse_args(argv)
@@ -186,6 +187,10 @@ def run_ours(args):
     dev = torch.device("cuda", local_rank if world > 1 else 0)
     torch.cuda.set_device(dev)
 
+    if args.only_scan_c4:
+        out = scan_c4(synth, Router, dev, measured_peaks()[0])
+        print(json.dumps(out))
+        return out
     cfg = synth.CONFIGS["C2"]
     K, W = args.steps, max(args.warmup, 3)
     sizes, elapsed, weights = c2_stream(cfg, W + K, seed_shift=rank)

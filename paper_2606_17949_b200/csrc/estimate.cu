@@ -7,6 +7,20 @@
 namespace rb {
 namespace {
 
+#ifdef RB_TRACE   // development aid (_work harness): timestamps of the finishing kernel's phases; compiled out otherwise
+__device__ unsigned long long rb_fin_trace[64 * 32];
+__device__ __forceinline__ void fin_trace(int slot) {
+  if (threadIdx.x == 0 && blockIdx.x < 64) {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    rb_fin_trace[blockIdx.x * 32 + slot] = t;
+  }
+}
+#define RB_FT(slot) fin_trace(slot)
+#else
+#define RB_FT(slot)
+#endif
+
 // Total order of candidates: similarity descending, bank index ascending (reading 3), as one 64-bit key whose
 // unsigned order is that order (larger key = better).  Key 0 is below every real candidate.
 __device__ __forceinline__ uint32_t f32_ordered(float f) {
@@ -250,6 +264,7 @@ finish_kernel(FinishArgs a, InstTable t, const CallParams* __restrict__ cp) {
   const uint4* qrow = reinterpret_cast<const uint4*>(a.qs + (size_t)r * a.d);
   const int nvec = a.d / 8;   // d % 8 == 0
 
+  RB_FT(0);
   // ---- merge ----
   const int total = a.nlists * kcap;
   if (tid == 0) s_nflag = 0;
@@ -262,6 +277,7 @@ finish_kernel(FinishArgs a, InstTable t, const CallParams* __restrict__ cp) {
     s_keys[e] = (id >= 0 && (int64_t)id < a.N) ? make_key(a.part_sim[off], id) : 0ull;
   }
   __syncthreads();
+  RB_FT(1);
   // two levels, no barrier inside either: every warp pops the kc best of its own share of the lists (lane = list),
   // then warp 0 pops the kc best of the warps' results (lane = warp)
   unsigned long long* w_key = s_keys + total;                         // [nwarps][kMerge2Stride]
@@ -274,6 +290,7 @@ finish_kernel(FinishArgs a, InstTable t, const CallParams* __restrict__ cp) {
                     w_src + (size_t)warp * kMerge2Stride);
   }
   __syncthreads();
+  RB_FT(2);
   if (warp == 0) {
     // out_src of this level is the warp whose list the key came from; its position in that list is the number
     // of keys already taken from it, which recovers the original list index
@@ -296,6 +313,7 @@ finish_kernel(FinishArgs a, InstTable t, const CallParams* __restrict__ cp) {
   }
   __syncthreads();
 
+  RB_FT(3);
   // ---- rescan of slabs whose list was popped completely ----
   // (a list of kcap entries all of which are among the kc best may hide further members)
   bool flagged = false;
@@ -371,6 +389,7 @@ finish_kernel(FinishArgs a, InstTable t, const CallParams* __restrict__ cp) {
   }
   __syncthreads();
 
+  RB_FT(4);
   // labels of all kc candidates are requested before the re-rank and parked after it (independent gathers)
   float lv[4];
   const int nlab = kc * 2 * M;   // <= 64 * 32 = 4 * 512
@@ -384,6 +403,7 @@ finish_kernel(FinishArgs a, InstTable t, const CallParams* __restrict__ cp) {
       if (id >= 0) lv[u] = (col < M) ? a.bank_quality[(size_t)id * M + col] : a.bank_outlen[(size_t)id * M + col - M];
     }
   }
+  RB_FT(5);
   // ---- exact re-rank ----
   if (a.rerank) {
     for (int c = warp; c < kc; c += nwarps) {
@@ -394,6 +414,7 @@ finish_kernel(FinishArgs a, InstTable t, const CallParams* __restrict__ cp) {
     }
     __syncthreads();
   }
+  RB_FT(6);
   // rank by counting (keys are distinct because indices are)
   if (tid < kc) {
     const int32_t id = s_idx[tid];
@@ -414,6 +435,7 @@ finish_kernel(FinishArgs a, InstTable t, const CallParams* __restrict__ cp) {
     if (e < nlab) s_lab[e / (2 * M)][e % (2 * M)] = lv[u];
   }
   __syncthreads();
+  RB_FT(7);
   // ---- weights ----
   if (tid < k) {
     const float s = o_sim[tid];
@@ -432,6 +454,7 @@ finish_kernel(FinishArgs a, InstTable t, const CallParams* __restrict__ cp) {
     if (cp->nn_sim) cp->nn_sim[(size_t)r * k + tid] = s;
   }
   __syncthreads();
+  RB_FT(8);
   // ---- aggregate: thread m < M -> quality, M <= thread < 2M -> output length ----
   if (tid < 2 * M) {
     const int m = tid % M;
@@ -454,6 +477,7 @@ finish_kernel(FinishArgs a, InstTable t, const CallParams* __restrict__ cp) {
       if (cp->pred_l) cp->pred_l[(size_t)r * M + m] = pred;
     }
   }
+  RB_FT(9);
   if (!a.with_terms) return;
   __syncthreads();
   // ---- per-(request, tier) terms ----
@@ -474,6 +498,7 @@ finish_kernel(FinishArgs a, InstTable t, const CallParams* __restrict__ cp) {
     a.termP[(size_t)r * M + m] = __fmul_rn(c_pre, c_ell);
     if (m == 0) a.key[r] = __fadd_rn(kmax, 0.0f);   // -0 -> +0 so that the sort key order equals float order
   }
+  RB_FT(10);
 }
 
 }  // namespace
