@@ -8,7 +8,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "librouteb.so")
-SOURCES = ["rb_api.cu", "scan_tc.cu", "estimate.cu", "score_dispatch.cu"]
+SOURCES = ["rb_api.cu", "scan_tc.cu", "scan_tc2.cu", "estimate.cu", "score_dispatch.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC",
          "-diag-suppress", "177"]
@@ -23,7 +23,7 @@ def _stale(target, deps):
 
 def build(force=False, verbose=False):
     os.makedirs(OBJ, exist_ok=True)
-    headers = [os.path.join(CSRC, "rb_internal.cuh"), os.path.join(HERE, "..", "include", "routebalance.h")]
+    headers = [os.path.join(CSRC, "rb_internal.cuh"), os.path.join(CSRC, "tc_scan.cuh"), os.path.join(HERE, "..", "include", "routebalance.h")]
     jobs = []
     objs = []
     for src in SOURCES:

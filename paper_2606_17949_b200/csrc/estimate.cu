@@ -347,11 +347,11 @@ finish_kernel(FinishArgs a, InstTable t, const CallParams* __restrict__ cp) {
     const int nctas = a.nlists / a.lists_per_cta;
     // every warp keeps the best kc of the rows it visits: rank l in lane l (a) and rank 32+l (b)
     unsigned long long la = 0, lb = 0, thr = 0;
-    const int64_t units = (a.N + kBoxN - 1) / kBoxN;
+    const int64_t units = (a.N + a.slab_unit - 1) / a.slab_unit;
     for (int f = 0; f < nflag; ++f) {
       const int c = s_flag[f];
-      const int64_t row0 = units * c / nctas * kBoxN;
-      int64_t row1 = units * (c + 1) / nctas * kBoxN;
+      const int64_t row0 = units * c / nctas * a.slab_unit;
+      int64_t row1 = units * (c + 1) / nctas * a.slab_unit;
       if (row1 > a.N) row1 = a.N;
       for (int64_t n = row0 + warp; n < row1; n += nwarps) {
         const float sx = exact_sim_bf16(qrow, reinterpret_cast<const uint4*>(a.bank + (size_t)n * a.d), nvec, lane);

@@ -169,14 +169,28 @@ rb_status enqueue_estimate(rb_ctx* ctx, int B, bool with_terms, Timer& tm) {
   fa.pred_q = ctx->pred_q; fa.pred_l = ctx->pred_l; fa.termA = ctx->termA; fa.termP = ctx->termP; fa.key = ctx->key;
   if (ctx->opt.store_dtype == RB_BF16) {
     tm.mark();
-    const int rep = scan_tc_replicas(B);
-    CK(launch_stage_queries(ctx->cp, ctx->qs, B, Bpad, ctx->d, rep, s));
-    tm.mark();
-    int grid = 0;
-    CK(launch_scan_tc(&ctx->tm_q, &ctx->tm_bank, ctx->N, ctx->d, B, Bpad, ctx->ks, ctx->num_sms, ctx->part_sim,
-                      ctx->part_idx, &grid, s));
-    tm.mark();
-    fa.part_sim = ctx->part_sim; fa.part_idx = ctx->part_idx; fa.nlists = grid * rep; fa.lists_per_cta = rep; fa.kcap = ctx->ks; fa.Bpad = Bpad;
+    if (B > kTileM && ctx->num_sms >= 2) {
+      // tensor-bound regime: CTA pairs, 256-query m-tiles
+      const int Bpad2 = (B + 2 * kTileM - 1) / (2 * kTileM) * (2 * kTileM);
+      CK(launch_stage_queries(ctx->cp, ctx->qs, B, Bpad2, ctx->d, 1, s));
+      tm.mark();
+      int ncl = 0;
+      CK(launch_scan_tc2(&ctx->tm_q, &ctx->tm_bank, ctx->N, ctx->d, B, Bpad2, ctx->ks, ctx->num_sms, ctx->part_sim,
+                         ctx->part_idx, &ncl, s));
+      tm.mark();
+      fa.part_sim = ctx->part_sim; fa.part_idx = ctx->part_idx; fa.nlists = ncl; fa.lists_per_cta = 1; fa.kcap = ctx->ks;
+      fa.Bpad = Bpad2; fa.slab_unit = kTileN;
+    } else {
+      const int rep = scan_tc_replicas(B, ctx->ks, ctx->num_sms);
+      CK(launch_stage_queries(ctx->cp, ctx->qs, B, Bpad, ctx->d, rep, s));
+      tm.mark();
+      int grid = 0;
+      CK(launch_scan_tc(&ctx->tm_q, &ctx->tm_bank, ctx->N, ctx->d, B, Bpad, ctx->ks, ctx->num_sms, ctx->part_sim,
+                        ctx->part_idx, &grid, s));
+      tm.mark();
+      fa.part_sim = ctx->part_sim; fa.part_idx = ctx->part_idx; fa.nlists = grid * rep; fa.lists_per_cta = rep; fa.kcap = ctx->ks;
+      fa.Bpad = Bpad; fa.slab_unit = kBoxN;
+    }
     fa.rescan = ctx->ks < ctx->kc ? 1 : 0;
     fa.bank = (const __nv_bfloat16*)ctx->bank; fa.qs = ctx->qs; fa.rerank = ctx->opt.rerank_slack > 0 ? 1 : 0;
     ctx->launches += 2;
@@ -193,6 +207,7 @@ rb_status enqueue_estimate(rb_ctx* ctx, int B, bool with_terms, Timer& tm) {
     tm.mark();
     // the selected candidates are one already-merged list per query: [1][B][kc]
     fa.part_sim = ctx->cand_sim; fa.part_idx = ctx->cand_idx; fa.nlists = 1; fa.lists_per_cta = 1; fa.kcap = ctx->kc; fa.Bpad = B;
+    fa.slab_unit = kBoxN;
     fa.bank = nullptr; fa.qs = nullptr; fa.rerank = 0;
   }
   CK(launch_finish(fa, table_of(ctx), ctx->cp, B, s));
@@ -401,7 +416,7 @@ rb_status rb_create(rb_ctx** out, const void* bank_emb, const float* bank_qualit
     if (ks > ctx->kcap) ks = ctx->kcap;
     ctx->ks = ks;
   }
-  ctx->Bpad_max = (opt.max_batch + kTileM - 1) / kTileM * kTileM;
+  ctx->Bpad_max = opt.max_batch <= kTileM ? kTileM : (opt.max_batch + 2 * kTileM - 1) / (2 * kTileM) * (2 * kTileM);
   *out = ctx;   // from here on errors keep the context so that rb_last_error works; caller destroys it
 
   if (opt.stream) {
@@ -491,9 +506,11 @@ rb_status rb_create(rb_ctx** out, const void* bank_emb, const float* bank_qualit
     st = encode_map(ctx, &ctx->tm_q, ctx->qs, (uint64_t)ctx->Bpad_max, (uint64_t)d, kTileM);
     if (st != RB_OK) return st;
     CK(scan_tc_prepare());
+    CK(scan_tc2_prepare());
   }
   {
-    const size_t fin = std::max(finish_smem_bytes(ctx->num_sms * 4, ctx->ks), finish_smem_bytes(1, ctx->kc));
+    const size_t fin = std::max(finish_smem_bytes(ctx->num_sms * scan_tc_replicas(1, ctx->ks, ctx->num_sms), ctx->ks),
+                                finish_smem_bytes(1, ctx->kc));
     CK(finish_prepare(fin));
     CK(lpt_dispatch_prepare());
   }

@@ -82,7 +82,9 @@ cudaError_t launch_convert_bf16(const float* in, __nv_bfloat16* out, size_t n, c
 // a0: cp->query (fp32) -> bf16 staging [Bpad x d]; rep copies of the B queries at rows j*(128/rep) + r (rep > 1 only
 // when Bpad = 128), all other rows zero.
 cudaError_t launch_stage_queries(const CallParams* cp, __nv_bfloat16* qs, int B, int Bpad, int d, int rep, cudaStream_t s);
-int scan_tc_replicas(int B);   // 4 (B <= 32), 2 (B <= 64), 1: query replicas over the TMEM lane quarters
+// query replicas over the TMEM lane quarters: 4 (B <= 32), 2 (B <= 64), 1; halved while the finishing kernel could not
+// hold max_grid * replicas lists of kcap entries in shared memory (long lists: k = 32)
+int scan_tc_replicas(int B, int kcap, int max_grid);
 
 // a1 (bf16): tcgen05 scan.  part_* are [grid * rep][Bpad][KCAP] (sim fp32 / idx int32, idx -1 = empty), each list
 // sorted by (sim desc, idx asc).  Returns the grid size used through *grid_out.  kcap in {4,8,16,32,64}; bank
@@ -92,6 +94,15 @@ cudaError_t launch_scan_tc(const CUtensorMap* tm_q, const CUtensorMap* tm_bank, 
                            cudaStream_t s);
 size_t scan_tc_smem_bytes();
 cudaError_t scan_tc_prepare();  // opt in to the dynamic shared memory size; call once
+
+// a1 (bf16, B > 128): the same scan on CTA pairs (tcgen05 cta_group::2, 256 queries x 256 bank rows per MMA tile).
+// Bpad is a multiple of 256.  part_* are [clusters][Bpad][KCAP]; cluster c owns the 256-row tiles
+// [tiles*c/clusters, tiles*(c+1)/clusters).  Returns the number of clusters through *clusters_out.
+cudaError_t launch_scan_tc2(const CUtensorMap* tm_q, const CUtensorMap* tm_bank, int64_t N, int d, int B, int Bpad,
+                            int kcap, int max_grid, float* part_sim, int32_t* part_idx, int* clusters_out,
+                            cudaStream_t s);
+int scan_tc2_clusters(int64_t N, int max_grid);
+cudaError_t scan_tc2_prepare();
 
 // a1 (fp32 storage): exact fp64-accumulated similarities of nq queries (q: [nq x d]) to sims [nq x N],
 // then per-query selection of the kc best (sim desc, idx asc) into cand_* [nq x kc].
@@ -109,6 +120,7 @@ struct FinishArgs {
   const int32_t* part_idx;
   int nlists, kcap, Bpad, kc, k;   // nlists = grid * lists_per_cta
   int lists_per_cta;
+  int slab_unit;            // rows per slab unit: slab c = rows [units*c/nslabs, units*(c+1)/nslabs) * slab_unit
   int64_t N;
   const __nv_bfloat16* bank;
   const __nv_bfloat16* qs;

@@ -91,6 +91,27 @@ def test_short_scan_lists_rescan_clustered_bank(orc, scan_list, N, B, k, slack):
         assert len(near) <= max(1, B // 20), log
 
 
+@pytest.mark.parametrize("N,d,B,k,slack", [(40000, 128, 129, 10, 6), (300, 64, 256, 10, 6), (25000, 192, 600, 10, 0),
+                                            (19001, 64, 1030, 32, 8), (256 * 74 * 3 + 100, 64, 257, 5, 3)])
+def test_bf16_pair_scan_large_batches(orc, N, d, B, k, slack):
+    """B > 128 runs the CTA-pair scan (tcgen05 cta_group::2, 256-query m-tiles): one and several m-pairs, a
+    half-empty last pair, fewer 256-row tiles than clusters (N = 300), a ragged last tile, K tails (d = 192)."""
+    cfg = dataclasses.replace(synth.CONFIGS["C2"], N=N, d=d, B=B, k=k, Kc=16, seed=31)
+    tol = 0.0 if slack > 0 else 4e-6
+    for sort_bank in (False, True):
+        g, near, log = _full_parity(orc, cfg, synth.PRESETS["balanced"], sim_tol=tol, rerank_slack=slack, max_batch=1100,
+                                    sort_bank=sort_bank)
+        assert len(near) <= max(1, B // 20), log
+
+
+@pytest.mark.parametrize("B", [8, 40, 130, 300])
+def test_k32_full_length_scan_lists(orc, B):
+    """k = 32 with slack 8 keeps 64-entry lists in the scan when slabs are long (C4: 67k rows per CTA); forced here
+    with scan_list = 64 on a small bank.  The finishing kernel's shared memory bounds the query replicas."""
+    cfg = dataclasses.replace(synth.CONFIGS["C2"], N=30000, d=128, B=B, k=32, Kc=16, seed=32)
+    _full_parity(orc, cfg, synth.PRESETS["balanced"], rerank_slack=8, max_batch=512, scan_list=64)
+
+
 def test_bf16_k32_and_uniform_weights(orc):
     cfg = dataclasses.replace(synth.CONFIGS["C2"], N=30000, d=384, B=40, k=32, Kc=16, seed=12)
     _full_parity(orc, cfg, synth.PRESETS["quality"], rerank_slack=8, max_batch=64)
