@@ -36,8 +36,9 @@ __device__ __forceinline__ unsigned long long make_key(float sim, int32_t idx) {
 
 // ---- a0 ---------------------------------------------------------------------------------------------
 __global__ void stage_queries_kernel(const CallParams* __restrict__ cp, __nv_bfloat16* __restrict__ qs, int B, int Bpad,
-                                     int d, int group) {
+                                     int d, int group, uint32_t* __restrict__ gthr, int n_gthr) {
   launch_dependents();
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n_gthr; i += gridDim.x * blockDim.x) gthr[i] = 0u;
   const float* __restrict__ q = cp->query;
   const size_t n = (size_t)Bpad * d;
   for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
@@ -510,11 +511,12 @@ cudaError_t launch_convert_bf16(const float* in, __nv_bfloat16* out, size_t n, c
   return cudaGetLastError();
 }
 
-cudaError_t launch_stage_queries(const CallParams* cp, __nv_bfloat16* qs, int B, int Bpad, int d, int rep, cudaStream_t s) {
+cudaError_t launch_stage_queries(const CallParams* cp, __nv_bfloat16* qs, int B, int Bpad, int d, int rep, uint32_t* gthr,
+                                 int n_gthr, cudaStream_t s) {
   const size_t n = (size_t)Bpad * d;
   int blocks = (int)((n + 255) / 256);
   if (blocks > 148 * 8) blocks = 148 * 8;
-  stage_queries_kernel<<<blocks, 256, 0, s>>>(cp, qs, B, Bpad, d, rep > 1 ? kTileM / rep : Bpad);
+  stage_queries_kernel<<<blocks, 256, 0, s>>>(cp, qs, B, Bpad, d, rep > 1 ? kTileM / rep : Bpad, gthr, n_gthr);
   return cudaGetLastError();
 }
 

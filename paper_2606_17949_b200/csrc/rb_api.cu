@@ -46,6 +46,7 @@ struct rb_ctx {
   CallParams* cp_ring = nullptr;    // pinned host ring feeding cp; slot reuse is guarded by cp_ev
   cudaEvent_t cp_ev[64]{};
   uint64_t cp_seq = 0;
+  uint32_t* gthr = nullptr;         // [Bpad_max] cross-slab admission thresholds of the scan (cleared per decision)
   float* part_sim = nullptr;        // [num_sms][kcap][Bpad_max]
   int32_t* part_idx = nullptr;
   float* sims = nullptr;            // fp32 storage only: [kF32Group x N]
@@ -172,17 +173,18 @@ rb_status enqueue_estimate(rb_ctx* ctx, int B, bool with_terms, Timer& tm) {
     if (B > kTileM && ctx->num_sms >= 2) {
       // tensor-bound regime: CTA pairs, 256-query m-tiles
       const int Bpad2 = (B + 2 * kTileM - 1) / (2 * kTileM) * (2 * kTileM);
-      CK(launch_stage_queries(ctx->cp, ctx->qs, B, Bpad2, ctx->d, 1, s));
+      CK(launch_stage_queries(ctx->cp, ctx->qs, B, Bpad2, ctx->d, 1, ctx->gthr,
+                              Bpad2 * (1 + scan_tc2_clusters(ctx->N, ctx->num_sms)), s));
       tm.mark();
       int ncl = 0;
-      CK(launch_scan_tc2(&ctx->tm_q, &ctx->tm_bank, ctx->N, ctx->d, B, Bpad2, ctx->ks, ctx->num_sms, ctx->part_sim,
-                         ctx->part_idx, &ncl, s));
+      CK(launch_scan_tc2(&ctx->tm_q, &ctx->tm_bank, ctx->N, ctx->d, B, Bpad2, ctx->kcap, ctx->kc, ctx->num_sms, ctx->part_sim,
+                         ctx->part_idx, ctx->gthr, &ncl, s));
       tm.mark();
-      fa.part_sim = ctx->part_sim; fa.part_idx = ctx->part_idx; fa.nlists = ncl; fa.lists_per_cta = 1; fa.kcap = ctx->ks;
-      fa.Bpad = Bpad2; fa.slab_unit = kTileN;
+      fa.part_sim = ctx->part_sim; fa.part_idx = ctx->part_idx; fa.nlists = ncl; fa.lists_per_cta = 1; fa.kcap = ctx->kcap;
+      fa.Bpad = Bpad2; fa.slab_unit = kTileN; fa.rescan = 0;   // full-length lists (K >= k + slack): nothing hidden
     } else {
       const int rep = scan_tc_replicas(B, ctx->ks, ctx->num_sms);
-      CK(launch_stage_queries(ctx->cp, ctx->qs, B, Bpad, ctx->d, rep, s));
+      CK(launch_stage_queries(ctx->cp, ctx->qs, B, Bpad, ctx->d, rep, ctx->gthr, Bpad, s));
       tm.mark();
       int grid = 0;
       CK(launch_scan_tc(&ctx->tm_q, &ctx->tm_bank, ctx->N, ctx->d, B, Bpad, ctx->ks, ctx->num_sms, ctx->part_sim,
@@ -191,7 +193,7 @@ rb_status enqueue_estimate(rb_ctx* ctx, int B, bool with_terms, Timer& tm) {
       fa.part_sim = ctx->part_sim; fa.part_idx = ctx->part_idx; fa.nlists = grid * rep; fa.lists_per_cta = rep; fa.kcap = ctx->ks;
       fa.Bpad = Bpad; fa.slab_unit = kBoxN;
     }
-    fa.rescan = ctx->ks < ctx->kc ? 1 : 0;
+    if (!(B > kTileM && ctx->num_sms >= 2)) fa.rescan = ctx->ks < ctx->kc ? 1 : 0;
     fa.bank = (const __nv_bfloat16*)ctx->bank; fa.qs = ctx->qs; fa.rerank = ctx->opt.rerank_slack > 0 ? 1 : 0;
     ctx->launches += 2;
   } else {
@@ -496,6 +498,7 @@ rb_status rb_create(rb_ctx** out, const void* bank_emb, const float* bank_qualit
   ALLOC(ctx->slope_i, kMaxI);
   if (opt.store_dtype == RB_BF16) {
     ALLOC(ctx->qs, (size_t)ctx->Bpad_max * d);
+    ALLOC(ctx->gthr, (size_t)ctx->Bpad_max * (2 + ctx->num_sms / 2));
     // [grid * rep][Bpad][ks]: rep = 4 replicas only when Bpad = 128
     const size_t part_n = (size_t)ctx->num_sms * ctx->kcap * std::max<size_t>(ctx->Bpad_max, 4 * kTileM);
     ALLOC(ctx->part_sim, part_n);
@@ -509,8 +512,8 @@ rb_status rb_create(rb_ctx** out, const void* bank_emb, const float* bank_qualit
     CK(scan_tc2_prepare());
   }
   {
-    const size_t fin = std::max(finish_smem_bytes(ctx->num_sms * scan_tc_replicas(1, ctx->ks, ctx->num_sms), ctx->ks),
-                                finish_smem_bytes(1, ctx->kc));
+    const size_t fin = std::max({finish_smem_bytes(ctx->num_sms * scan_tc_replicas(1, ctx->ks, ctx->num_sms), ctx->ks),
+                                 finish_smem_bytes(ctx->num_sms / 2 + 1, ctx->kcap), finish_smem_bytes(1, ctx->kc)});
     CK(finish_prepare(fin));
     CK(lpt_dispatch_prepare());
   }
@@ -727,7 +730,7 @@ void rb_destroy(rb_ctx* ctx) {
   for (auto& kv : ctx->graphs) cudaGraphExecDestroy(kv.second);
   void* ptrs[] = {ctx->bank, ctx->bank_quality, ctx->bank_outlen, ctx->tier, ctx->cap, ctx->present, ctx->price_in,
                   ctx->price_out, ctx->pre, ctx->dec, ctx->slope, ctx->dec_i, ctx->slope_i, ctx->dq, ctx->bq, ctx->q32, ctx->qs, ctx->plen, ctx->cp,
-                  ctx->part_sim, ctx->part_idx, ctx->sims, ctx->cand_sim, ctx->cand_idx, ctx->scratch_nn_idx, ctx->scratch_nn_sim, ctx->stage_q, ctx->stage_l,
+                  ctx->part_sim, ctx->part_idx, ctx->gthr, ctx->sims, ctx->cand_sim, ctx->cand_idx, ctx->scratch_nn_idx, ctx->scratch_nn_sim, ctx->stage_q, ctx->stage_l,
                   ctx->pred_q, ctx->pred_l, ctx->termA, ctx->termP, ctx->key, ctx->order, ctx->assignment, ctx->scores,
                   ctx->scores0};
   for (void* p : ptrs) cudaFree(p);

@@ -80,8 +80,9 @@ cudaError_t launch_chained(void (*kernel)(KArgs...), dim3 grid, dim3 block, size
 cudaError_t launch_convert_bf16(const float* in, __nv_bfloat16* out, size_t n, cudaStream_t s);
 
 // a0: cp->query (fp32) -> bf16 staging [Bpad x d]; rep copies of the B queries at rows j*(128/rep) + r (rep > 1 only
-// when Bpad = 128), all other rows zero.
-cudaError_t launch_stage_queries(const CallParams* cp, __nv_bfloat16* qs, int B, int Bpad, int d, int rep, cudaStream_t s);
+// when Bpad = 128), all other rows zero.  Also clears gthr [n_gthr] (the scan's cross-slab thresholds).
+cudaError_t launch_stage_queries(const CallParams* cp, __nv_bfloat16* qs, int B, int Bpad, int d, int rep, uint32_t* gthr,
+                                 int n_gthr, cudaStream_t s);
 // query replicas over the TMEM lane quarters: 4 (B <= 32), 2 (B <= 64), 1; halved while the finishing kernel could not
 // hold max_grid * replicas lists of kcap entries in shared memory (long lists: k = 32)
 int scan_tc_replicas(int B, int kcap, int max_grid);
@@ -98,9 +99,11 @@ cudaError_t scan_tc_prepare();  // opt in to the dynamic shared memory size; cal
 // a1 (bf16, B > 128): the same scan on CTA pairs (tcgen05 cta_group::2, 256 queries x 256 bank rows per MMA tile).
 // Bpad is a multiple of 256.  part_* are [clusters][Bpad][KCAP]; cluster c owns the 256-row tiles
 // [tiles*c/clusters, tiles*(c+1)/clusters).  Returns the number of clusters through *clusters_out.
+// gthr [(1 + clusters) x Bpad] must be zero at launch (launch_stage_queries clears it): cross-slab admission
+// thresholds ([Bpad] best K-th best of any slab, then per slab the (kc+15)/16-th best it has seen so far).
 cudaError_t launch_scan_tc2(const CUtensorMap* tm_q, const CUtensorMap* tm_bank, int64_t N, int d, int B, int Bpad,
-                            int kcap, int max_grid, float* part_sim, int32_t* part_idx, int* clusters_out,
-                            cudaStream_t s);
+                            int kcap, int kc, int max_grid, float* part_sim, int32_t* part_idx, uint32_t* gthr,
+                            int* clusters_out, cudaStream_t s);
 int scan_tc2_clusters(int64_t N, int max_grid);
 cudaError_t scan_tc2_prepare();
 

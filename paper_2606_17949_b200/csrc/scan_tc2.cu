@@ -18,20 +18,39 @@
 //            columns of the accumulator.
 // A cluster owns a contiguous slab of whole 256-row tiles and visits every m-pair per tile (the bank tile comes
 // from L2 after the first visit).  The per-(slab, query) lists live in global memory (L2); a visit needs only
-// the list's last similarity (the admission threshold) and touches the list itself only when a candidate
-// beats it -- rare after the first tiles.
+// the admission threshold (shared memory) and touches the list itself only when a candidate beats it.
+// Thresholds are shared ACROSS slabs: a slab that has K = KCAP >= k + slack entries for a query publishes its
+// K-th best similarity (atomicMax on gthr[query]); that value bounds the query's global K-th best from below, so
+// every slab may drop what is strictly below it without changing the merged result.  This turns the
+// K ln(rows per slab) insertions per (slab, query) of independent streaming top-K lists into about
+// K ln(rows seen by all slabs together) per query, which keeps the epilogue off the tensor pipe's time line.
 #include "rb_internal.cuh"
 #include "tc_scan.cuh"
 
 namespace rb {
 namespace {
 
+#ifdef RB_PROF   // development aid (_work harness): per-warp cycle and event counters; compiled out otherwise
+__device__ unsigned long long rb_prof[148 * 8 * 8];
+#define RB_PC_DECL unsigned long long pc_[8] = {0, 0, 0, 0, 0, 0, 0, 0}
+#define RB_PC(slot, val) pc_[slot] += (unsigned long long)(val)
+#define RB_PC_FLUSH do { if (lane == 0) { for (int q_ = 0; q_ < 8; ++q_) rb_prof[(blockIdx.x * 8 + warp) * 8 + q_] += pc_[q_]; } } while (0)
+#define RB_CLK() clock64()
+#else
+#define RB_PC_DECL
+#define RB_PC(slot, val)
+#define RB_PC_FLUSH
+#define RB_CLK() 0ll
+#endif
+
 constexpr int kStages2 = 6;
 constexpr int kA2Bytes = kTileM * kTileK * 2;            // 16 KB: this CTA's 128 queries x 64 bf16
 constexpr int kB2Bytes = (kTileN / 2) * kTileK * 2;      // 16 KB: this CTA's 128 of the tile's 256 bank rows
 constexpr int kStage2Bytes = kA2Bytes + kB2Bytes;        // 32 KB
 constexpr int kThreads2 = 192;
-constexpr int kSmem2Bytes = kStages2 * kStage2Bytes + kCandSlots * kTileM * 8 + 256 + 1024;
+constexpr int kCand2Slots = 16;                           // parked survivors per thread
+constexpr int kMaxPairs = 16;                             // m-pairs of one decision: B <= 4096
+constexpr int kSmem2Bytes = kStages2 * kStage2Bytes + kCand2Slots * kTileM * 8 + 2 * kMaxPairs * kTileM * 4 + 256 + 1024;
 constexpr int kPairM = 2 * kTileM;                        // queries per m-pair
 
 __device__ __forceinline__ uint32_t cluster_ctarank() {
@@ -49,8 +68,11 @@ __device__ __forceinline__ uint32_t mapa_u32(uint32_t saddr, uint32_t rank) {
   asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(saddr), "r"(rank));
   return r;
 }
+// Arrive on a barrier of another CTA of the cluster.  Relaxed: what the arrival publishes is that this warp's
+// tcgen05.ld reads of the accumulator have completed (tcgen05.wait::ld + tcgen05.fence::before_thread_sync order
+// them before it); no ordinary memory is handed over, and a release at cluster scope costs ~1500 clocks per visit.
 __device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_addr) {
-  asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
+  asm volatile("mbarrier.arrive.relaxed.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
 }
 // TMA tile load of a CTA pair: data into this CTA's shared memory, bytes counted on the barrier at bar_cluster_addr
 // (the leader's).
@@ -77,62 +99,103 @@ __device__ __forceinline__ void tc_mma_pair(uint32_t d_tmem, uint64_t adesc, uin
       : "memory");
 }
 
-// One tcgen05.ld chunk folded into the thread's list, the list itself fetched from global memory only when this
-// thread has a candidate above its threshold (tc_scan.cuh: fold_chunk is the register-resident variant).
+// Per-thread state of one visit (one accumulator of one m-pair): the admission threshold, the survivors parked
+// in shared memory, and the thread's list, which is fetched from global memory when the first survivor appears
+// and consumed only when the survivors are inserted -- normally after the accumulator has been released, so that
+// neither the L2 round trip nor the insertion sits on the tensor pipe's time line.
 template <int K>
-__device__ __forceinline__ void fold_chunk_lazy(const uint32_t (&regs)[32], int c0, int c_end, int n0, float (&v)[K],
-                                                int32_t (&ix)[K], float& thr, bool& loaded, const float4* ps4,
-                                                const int4* pi4, uint2* cand, int tl) {
-  const bool full = c0 + 32 <= c_end;   // warp-uniform
-  float m0 = -INFINITY, m1 = -INFINITY, m2 = -INFINITY, m3 = -INFINITY;
-#pragma unroll
-  for (int j = 0; j < 32; j += 4) {
-    m0 = fmaxf(m0, (full || c0 + j + 0 < c_end) ? __uint_as_float(regs[j + 0]) : -INFINITY);
-    m1 = fmaxf(m1, (full || c0 + j + 1 < c_end) ? __uint_as_float(regs[j + 1]) : -INFINITY);
-    m2 = fmaxf(m2, (full || c0 + j + 2 < c_end) ? __uint_as_float(regs[j + 2]) : -INFINITY);
-    m3 = fmaxf(m3, (full || c0 + j + 3 < c_end) ? __uint_as_float(regs[j + 3]) : -INFINITY);
-  }
-  const float m = fmaxf(fmaxf(m0, m1), fmaxf(m2, m3));
-  if (!__any_sync(0xffffffffu, m > thr)) return;
-  int cnt = 0;
-#pragma unroll
-  for (int j = 0; j < 32; ++j) {
-    const float s = __uint_as_float(regs[j]);
-    if ((full || c0 + j < c_end) && s > thr) {
-      cand[cnt * kTileM + tl] = make_uint2(regs[j], (uint32_t)(c0 + j));
-      ++cnt;
-    }
-  }
-  if (cnt > 0 && !loaded) {
+struct Visit {
+  float v[K];
+  int32_t ix[K];
+  float thr;
+  int cnt;        // survivors parked
+  bool loaded;    // list requested (or initialised)
+};
+
+// Inserts the parked survivors (scan order) into the list, in warp lock-step: every lane inserts its p-th
+// survivor in the same iteration.
+template <int K>
+__device__ __forceinline__ void request_list(Visit<K>& st, const float4* ps4, const int4* pi4) {
+  if (st.cnt > 0 && !st.loaded) {
 #pragma unroll
     for (int j = 0; j < K / 4; ++j) {
       const float4 a = ps4[j];
       const int4 b = pi4[j];
-      v[4 * j] = a.x; v[4 * j + 1] = a.y; v[4 * j + 2] = a.z; v[4 * j + 3] = a.w;
-      ix[4 * j] = b.x; ix[4 * j + 1] = b.y; ix[4 * j + 2] = b.z; ix[4 * j + 3] = b.w;
+      st.v[4 * j] = a.x; st.v[4 * j + 1] = a.y; st.v[4 * j + 2] = a.z; st.v[4 * j + 3] = a.w;
+      st.ix[4 * j] = b.x; st.ix[4 * j + 1] = b.y; st.ix[4 * j + 2] = b.z; st.ix[4 * j + 3] = b.w;
     }
-    loaded = true;
+    st.loaded = true;
   }
+}
+template <int K>
+__device__ __forceinline__ void drain(Visit<K>& st, const float4* ps4, const int4* pi4, const uint2* cand, int tl, int n0) {
+  request_list<K>(st, ps4, pi4);
   uint2 nxt = cand[tl];
-  for (int p = 0; __any_sync(0xffffffffu, p < cnt); ++p) {
+  for (int p = 0; __any_sync(0xffffffffu, p < st.cnt); ++p) {
     const uint2 cur = nxt;
-    nxt = cand[min(p + 1, kCandSlots - 1) * kTileM + tl];
+    nxt = cand[min(p + 1, kCand2Slots - 1) * kTileM + tl];
     const float s = __uint_as_float(cur.x);
-    if (p < cnt && s > thr) {
-      list_insert<K>(v, ix, s, n0 + (int)cur.y);
-      thr = v[K - 1];
+    if (p < st.cnt && s > st.thr) {
+      list_insert<K>(st.v, st.ix, s, n0 + (int)cur.y);
+      st.thr = fmaxf(st.thr, st.v[K - 1]);
     }
   }
+  st.cnt = 0;
+}
+
+// One tcgen05.ld chunk (32 similarities of this thread's query against bank rows n0 + c0 ..).  Steady state: no
+// lane of the warp holds a similarity above its threshold: one max tree and one vote.  Otherwise the survivors
+// are parked, 8 columns at a time; the queue (kCand2Slots per thread) is drained early only when a lane could
+// overflow it, which happens in the first tiles of a slab, while the lists fill.
+template <int K>
+__device__ __forceinline__ void park_chunk(const uint32_t (&regs)[32], int c0, int c_end, int n0, Visit<K>& st,
+                                           const float4* ps4, const int4* pi4, uint2* cand, int tl) {
+  const bool full = c0 + 32 <= c_end;   // warp-uniform
+  float m0 = -INFINITY, m1 = -INFINITY, m2 = -INFINITY, m3 = -INFINITY;
+  if (full) {
+#pragma unroll
+    for (int j = 0; j < 32; j += 4) {
+      m0 = fmaxf(m0, __uint_as_float(regs[j + 0]));
+      m1 = fmaxf(m1, __uint_as_float(regs[j + 1]));
+      m2 = fmaxf(m2, __uint_as_float(regs[j + 2]));
+      m3 = fmaxf(m3, __uint_as_float(regs[j + 3]));
+    }
+  } else {
+#pragma unroll
+    for (int j = 0; j < 32; j += 4) {
+      m0 = fmaxf(m0, (c0 + j + 0 < c_end) ? __uint_as_float(regs[j + 0]) : -INFINITY);
+      m1 = fmaxf(m1, (c0 + j + 1 < c_end) ? __uint_as_float(regs[j + 1]) : -INFINITY);
+      m2 = fmaxf(m2, (c0 + j + 2 < c_end) ? __uint_as_float(regs[j + 2]) : -INFINITY);
+      m3 = fmaxf(m3, (c0 + j + 3 < c_end) ? __uint_as_float(regs[j + 3]) : -INFINITY);
+    }
+  }
+  const float m = fmaxf(fmaxf(m0, m1), fmaxf(m2, m3));
+  if (!__any_sync(0xffffffffu, m > st.thr)) return;
+#pragma unroll
+  for (int g = 0; g < 4; ++g) {
+    if (__any_sync(0xffffffffu, st.cnt > kCand2Slots - 8)) drain<K>(st, ps4, pi4, cand, tl, n0);
+#pragma unroll
+    for (int j = 8 * g; j < 8 * g + 8; ++j) {
+      const float s = __uint_as_float(regs[j]);
+      if ((full || c0 + j < c_end) && s > st.thr) {
+        cand[st.cnt * kTileM + tl] = make_uint2(regs[j], (uint32_t)(c0 + j));
+        ++st.cnt;
+      }
+    }
+  }
+  request_list<K>(st, ps4, pi4);   // nothing waits for it here
 }
 
 template <int KCAP>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads2, 1)
 scan_tc2_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_bank, int64_t N, int d,
-                int B, int Bpad, float* part_sim, int32_t* part_idx) {
+                int B, int Bpad, float* part_sim, int32_t* part_idx, uint32_t* gthr, int pub_j, int pub_groups) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
   uint2* cand = (uint2*)(smem + kStages2 * kStage2Bytes);
-  uint64_t* bars = (uint64_t*)(cand + kCandSlots * kTileM);
+  float* thr_s = (float*)(cand + kCand2Slots * kTileM);   // [n_mp][128] K-th best similarity of this CTA's lists
+  uint32_t* gl_s = (uint32_t*)(thr_s + kMaxPairs * kTileM);   // [n_mp][128] pooled lower bound (ordered), see refresh
+  uint64_t* bars = (uint64_t*)(gl_s + kMaxPairs * kTileM);
   uint64_t* full = bars;                   // [kStages2] leader's: both CTAs' TMA bytes landed
   uint64_t* empty = bars + kStages2;       // [kStages2] own: the MMAs that read the slot retired
   uint64_t* tfull = bars + 2 * kStages2;   // [2] own: accumulator complete
@@ -140,6 +203,7 @@ scan_tc2_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant_
   uint32_t* tmem_slot = (uint32_t*)(tempty + 2);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  RB_PC_DECL;
   const uint32_t rank = cluster_ctarank();
   const int cl = blockIdx.x >> 1, ncl = gridDim.x >> 1;
   const int n_mp = Bpad / kPairM;
@@ -211,13 +275,17 @@ scan_tc2_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant_
       for (int tile = 0; tile < ntiles; ++tile) {
         for (int mp = 0; mp < n_mp; ++mp, ++it) {
           const uint32_t acc = it & 1, aph = (it >> 1) & 1;
+          const long long m0_ = RB_CLK();
           mbar_wait(&tempty[acc], aph ^ 1);
+          { const long long dw_ = RB_CLK() - m0_; RB_PC(0, dw_); const int bk_ = tile == 0 ? 2 : (tile == 1 ? 3 : (tile < 4 ? 4 : (tile < 8 ? 5 : (tile < 16 ? 6 : 7)))); RB_PC(bk_, dw_); }
           tc_fence_after();
           const uint32_t d_tmem = tmem_base + acc * kTileN;
           for (int kc = 0; kc < nk; ++kc, ++kit) {
             const int s = kit % kStages2;
             const uint32_t ph = (kit / kStages2) & 1;
+            const long long m1_ = RB_CLK();
             mbar_wait(&full[s], ph);
+            RB_PC(1, RB_CLK() - m1_);
             tc_fence_after();
             const uint32_t sa = smem_u32(smem + s * kStage2Bytes);
             const uint64_t adesc = make_smem_desc(sa);
@@ -237,12 +305,15 @@ scan_tc2_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant_
     const int quarter = warp & 3;
     const int tl = quarter * 32 + lane;
     const uint32_t tempty_leader[2] = {mapa_u32(smem_u32(&tempty[0]), 0), mapa_u32(smem_u32(&tempty[1]), 0)};
-    float v[KCAP];
-    int32_t ix[KCAP];
+    Visit<KCAP> st;
+    grid_dependency_wait();   // gthr was cleared by the preceding kernel
+    uint32_t g_cur = 0;       // best published lower bound of this visit's query, fetched during the previous visit
     uint32_t it = 0;
+    int next_refresh = 1;     // tiles 1, 2, 3, 4, 6, 9, 13, 19, ...: the bound moves slowly once many rows are pooled
     for (int tile = 0; tile < ntiles; ++tile) {
       const int n0 = (int)(row0 + (int64_t)tile * kTileN);
       const int c_end = (int)min((int64_t)kTileN, N - (int64_t)n0);   // rows >= N are TMA zero fill
+      if (tile > next_refresh) next_refresh = next_refresh + max(1, next_refresh >> 1);
       for (int mp = 0; mp < n_mp; ++mp, ++it) {
         const uint32_t acc = it & 1, aph = (it >> 1) & 1;
         const int r = mp * kPairM + (int)rank * kTileM + tl;
@@ -250,55 +321,123 @@ scan_tc2_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant_
         const size_t pbase = ((size_t)cl * (size_t)Bpad + (size_t)r) * KCAP;
         float4* ps4 = reinterpret_cast<float4*>(part_sim + pbase);
         int4* pi4 = reinterpret_cast<int4*>(part_idx + pbase);
-        bool loaded = false;
-        float thr = INFINITY;   // padding lanes never collect
-        if (warp_active && r < B) {
+        const int r_nxt = ((mp + 1 == n_mp) ? 0 : mp + 1) * kPairM + (int)rank * kTileM + tl;
+        const uint32_t g_nxt = (r_nxt < B) ? *reinterpret_cast<volatile uint32_t*>(gthr + r_nxt) : 0u;
+        st.cnt = 0;
+        st.loaded = false;
+        st.thr = INFINITY;   // padding lanes never collect
+        if (r < B) {
+          float own = -INFINITY;   // K-th best of this (slab, query) list so far
+          uint32_t gl = 0;         // pooled bound of this query (ordered; 0 = none)
           if (tile == 0) {
 #pragma unroll
-            for (int j = 0; j < KCAP; ++j) { v[j] = -INFINITY; ix[j] = -1; }
-            loaded = true;
-            thr = -INFINITY;
+            for (int j = 0; j < KCAP; ++j) { st.v[j] = -INFINITY; st.ix[j] = -1; }
+            st.loaded = true;
+            gl_s[mp * kTileM + tl] = 0u;
           } else {
-            thr = *reinterpret_cast<volatile float*>(part_sim + pbase + KCAP - 1);
+            own = thr_s[mp * kTileM + tl];
+            gl = gl_s[mp * kTileM + tl];
           }
+          if (tile == next_refresh) {
+            // Pooled bound over the slabs (every slab publishes its pub_j-th best per query): the slabs form
+            // pub_groups groups; the best published value of a group stands for pub_j entries >= it in ONE slab,
+            // so the minimum over the groups has pub_groups * pub_j >= k + slack distinct entries at or above it.
+            const volatile uint32_t* pub = gthr + (size_t)Bpad + r;
+            uint32_t tau = 0xffffffffu;
+            for (int g = 0; g < pub_groups; ++g) {
+              uint32_t mx = 0;
+#pragma unroll 5
+              for (int c = g; c < ncl; c += pub_groups) {
+                const uint32_t x = pub[(size_t)c * Bpad];
+                mx = x > mx ? x : mx;
+              }
+              tau = mx < tau ? mx : tau;
+            }
+            gl = tau > gl ? tau : gl;
+            gl_s[mp * kTileM + tl] = gl;
+          }
+          // Admission threshold: above the list's own K-th best (strictly: an equal similarity met later has a
+          // larger index), and not below what bounds the query's GLOBAL (k + slack)-th best from below: the pooled
+          // bound, and the best K-th best any single slab has published (an EQUAL similarity may still belong to
+          // the global best, hence the -1 in the ordered domain).
+          uint32_t ge = g_cur > gl ? g_cur : gl;
+          ge = ge ? ge - 1u : 0u;
+          const uint32_t lo = f32_ordered(own);
+          st.thr = f32_unordered(lo > ge ? lo : ge);
         }
+        const long long e0_ = RB_CLK();
         mbar_wait(&tfull[acc], aph);
+        const long long e1_ = RB_CLK();
+        RB_PC(0, e1_ - e0_);
         tc_fence_after();
+        long long lb_ = e1_;
         if (warp_active) {
+          // the accumulator always holds 256 columns (columns >= c_end are similarities to zero-filled rows)
           const uint32_t taddr = tmem_base + ((uint32_t)(quarter * 32) << 16) + acc * kTileN;
           if constexpr (KCAP <= 16) {
-            for (int c0 = 0; c0 < c_end; c0 += 64) {
-              uint32_t ra[32], rb[32];
-              const bool two = c0 + 32 < c_end;
-              tmem_ld32(taddr + c0, ra);
-              if (two) tmem_ld32(taddr + c0 + 32, rb);
+            // TMEM reads (64 B/clk) bound the visit: the next 64 columns are in flight while these are folded
+            uint32_t ra[32], rb[32], rc[32], rd[32];
+            tmem_ld32(taddr, ra);
+            tmem_ld32(taddr + 32, rb);
+            const long long la_ = RB_CLK();
+            RB_PC(5, la_ - e1_);
+#pragma unroll 1
+            for (int c0 = 0; c0 < kTileN; c0 += 128) {
               tmem_ld_wait();
-              fold_chunk_lazy<KCAP>(ra, c0, c_end, n0, v, ix, thr, loaded, ps4, pi4, cand, tl);
-              if (two) fold_chunk_lazy<KCAP>(rb, c0 + 32, c_end, n0, v, ix, thr, loaded, ps4, pi4, cand, tl);
+              tmem_ld32(taddr + c0 + 64, rc);
+              tmem_ld32(taddr + c0 + 96, rd);
+              if (c0 < c_end) park_chunk<KCAP>(ra, c0, c_end, n0, st, ps4, pi4, cand, tl);
+              if (c0 + 32 < c_end) park_chunk<KCAP>(rb, c0 + 32, c_end, n0, st, ps4, pi4, cand, tl);
+              tmem_ld_wait();
+              if (c0 + 128 < kTileN) {
+                tmem_ld32(taddr + c0 + 128, ra);
+                tmem_ld32(taddr + c0 + 160, rb);
+              }
+              if (c0 + 64 < c_end) park_chunk<KCAP>(rc, c0 + 64, c_end, n0, st, ps4, pi4, cand, tl);
+              if (c0 + 96 < c_end) park_chunk<KCAP>(rd, c0 + 96, c_end, n0, st, ps4, pi4, cand, tl);
             }
+            lb_ = RB_CLK();
+            RB_PC(7, lb_ - la_);
           } else {
             for (int c0 = 0; c0 < c_end; c0 += 32) {
               uint32_t ra[32];
               tmem_ld32(taddr + c0, ra);
               tmem_ld_wait();
-              fold_chunk_lazy<KCAP>(ra, c0, c_end, n0, v, ix, thr, loaded, ps4, pi4, cand, tl);
+              park_chunk<KCAP>(ra, c0, c_end, n0, st, ps4, pi4, cand, tl);
             }
           }
         }
         tc_fence_before();
         __syncwarp();
-        if (lane == 0) mbar_arrive_cluster(tempty_leader[acc]);
-        if (loaded) {
+        if (lane == 0) mbar_arrive_cluster(tempty_leader[acc]);   // accumulator released; now the insertions
+        const long long e2_ = RB_CLK();
+        RB_PC(1, e2_ - e1_);
+        RB_PC(6, e2_ - lb_);
+        RB_PC(3, 1);
+        {
+          const int anyd_ = __any_sync(0xffffffffu, st.cnt > 0) ? 1 : 0;
+          RB_PC(4, anyd_);
+        }
+        if (warp_active && __any_sync(0xffffffffu, st.cnt > 0)) drain<KCAP>(st, ps4, pi4, cand, tl, n0);
+        if (st.loaded) {
 #pragma unroll
           for (int j = 0; j < KCAP / 4; ++j) {
-            ps4[j] = make_float4(v[4 * j], v[4 * j + 1], v[4 * j + 2], v[4 * j + 3]);
-            pi4[j] = make_int4(ix[4 * j], ix[4 * j + 1], ix[4 * j + 2], ix[4 * j + 3]);
+            ps4[j] = make_float4(st.v[4 * j], st.v[4 * j + 1], st.v[4 * j + 2], st.v[4 * j + 3]);
+            pi4[j] = make_int4(st.ix[4 * j], st.ix[4 * j + 1], st.ix[4 * j + 2], st.ix[4 * j + 3]);
           }
+          const float own = st.v[KCAP - 1];
+          thr_s[mp * kTileM + tl] = own;
+          if (own > -INFINITY) atomicMax(gthr + r, f32_ordered(own));
+          const float pj = pub_j == 1 ? st.v[0] : (pub_j == 2 ? st.v[1] : (pub_j == 3 ? st.v[2] : st.v[3]));
+          if (pj > -INFINITY) gthr[(size_t)Bpad * (1 + cl) + r] = f32_ordered(pj);
         }
+        RB_PC(2, RB_CLK() - e2_);
+        g_cur = g_nxt;
       }
     }
   }
 
+  RB_PC_FLUSH;
   tc_fence_before();
   cluster_sync_all();   // the leader's MMAs read the peer's shared memory and write its TMEM: leave together
   if (warp == 1) {
@@ -308,6 +447,17 @@ scan_tc2_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant_
 }
 
 }  // namespace
+
+#ifdef RB_PROF
+extern "C" void rb_prof_read(unsigned long long* out, int reset) {
+  cudaDeviceSynchronize();
+  cudaMemcpyFromSymbol(out, rb_prof, sizeof(unsigned long long) * 148 * 8 * 8);
+  if (reset) {
+    static unsigned long long z[148 * 8 * 8];
+    cudaMemcpyToSymbol(rb_prof, z, sizeof z);
+  }
+}
+#endif
 
 cudaError_t scan_tc2_prepare() {
   cudaError_t e;
@@ -329,13 +479,15 @@ int scan_tc2_clusters(int64_t N, int max_grid) {
 }
 
 cudaError_t launch_scan_tc2(const CUtensorMap* tm_q, const CUtensorMap* tm_bank, int64_t N, int d, int B, int Bpad,
-                            int kcap, int max_grid, float* part_sim, int32_t* part_idx, int* clusters_out, cudaStream_t s) {
+                            int kcap, int kc, int max_grid, float* part_sim, int32_t* part_idx, uint32_t* gthr,
+                            int* clusters_out, cudaStream_t s) {
   const int ncl = scan_tc2_clusters(N, max_grid);
   if (clusters_out) *clusters_out = ncl;
+  const int pub_j = (kc + 15) / 16, pub_groups = (kc + pub_j - 1) / pub_j;   // pub_groups * pub_j >= kc
   cudaError_t e = cudaSuccess;
 #define RB_SCAN2_LAUNCH(KC)                                                                                       \
   e = launch_chained(scan_tc2_kernel<KC>, dim3(2 * ncl), dim3(kThreads2), kSmem2Bytes, s, *tm_q, *tm_bank, N, d, B, Bpad, \
-                     part_sim, part_idx)
+                     part_sim, part_idx, gthr, pub_j, pub_groups)
   switch (kcap) {
     case 4: RB_SCAN2_LAUNCH(4); break;
     case 8: RB_SCAN2_LAUNCH(8); break;
