@@ -47,7 +47,7 @@ constexpr int kStages2 = 6;
 constexpr int kA2Bytes = kTileM * kTileK * 2;            // 16 KB: this CTA's 128 queries x 64 bf16
 constexpr int kB2Bytes = (kTileN / 2) * kTileK * 2;      // 16 KB: this CTA's 128 of the tile's 256 bank rows
 constexpr int kStage2Bytes = kA2Bytes + kB2Bytes;        // 32 KB
-constexpr int kThreads2 = 192;
+constexpr int kThreads2 = 256;                            // 6 pipeline warps + 2 bound refreshers
 constexpr int kCand2Slots = 16;                           // parked survivors per thread
 constexpr int kMaxPairs = 16;                             // m-pairs of one decision: B <= 4096
 constexpr int kSmem2Bytes = kStages2 * kStage2Bytes + kCand2Slots * kTileM * 8 + 2 * kMaxPairs * kTileM * 4 + 256 + 1024;
@@ -201,6 +201,7 @@ scan_tc2_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant_
   uint64_t* tfull = bars + 2 * kStages2;   // [2] own: accumulator complete
   uint64_t* tempty = tfull + 2;            // [2] leader's: accumulator drained by the 8 epilogue warps of the pair
   uint32_t* tmem_slot = (uint32_t*)(tempty + 2);
+  int* epi_done = (int*)(tmem_slot + 1);   // epilogue warps that have finished
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   RB_PC_DECL;
@@ -227,6 +228,8 @@ scan_tc2_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant_
     }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
+  if (threadIdx.x == 32) *epi_done = 0;
+  for (int i = threadIdx.x; i < kMaxPairs * kTileM; i += kThreads2) gl_s[i] = 0u;
   if (warp == 1) {
     asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)), "r"(512)
                  : "memory");
@@ -300,7 +303,7 @@ scan_tc2_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant_
       }
     }
     __syncwarp();
-  } else {
+  } else if (warp < 6) {
     // ===== epilogue (both CTAs): fused per-query top-KCAP =====
     const int quarter = warp & 3;
     const int tl = quarter * 32 + lane;
@@ -309,11 +312,9 @@ scan_tc2_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant_
     grid_dependency_wait();   // gthr was cleared by the preceding kernel
     uint32_t g_cur = 0;       // best published lower bound of this visit's query, fetched during the previous visit
     uint32_t it = 0;
-    int next_refresh = 1;     // tiles 1, 2, 3, 4, 6, 9, 13, 19, ...: the bound moves slowly once many rows are pooled
     for (int tile = 0; tile < ntiles; ++tile) {
       const int n0 = (int)(row0 + (int64_t)tile * kTileN);
       const int c_end = (int)min((int64_t)kTileN, N - (int64_t)n0);   // rows >= N are TMA zero fill
-      if (tile > next_refresh) next_refresh = next_refresh + max(1, next_refresh >> 1);
       for (int mp = 0; mp < n_mp; ++mp, ++it) {
         const uint32_t acc = it & 1, aph = (it >> 1) & 1;
         const int r = mp * kPairM + (int)rank * kTileM + tl;
@@ -333,28 +334,9 @@ scan_tc2_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant_
 #pragma unroll
             for (int j = 0; j < KCAP; ++j) { st.v[j] = -INFINITY; st.ix[j] = -1; }
             st.loaded = true;
-            gl_s[mp * kTileM + tl] = 0u;
           } else {
             own = thr_s[mp * kTileM + tl];
-            gl = gl_s[mp * kTileM + tl];
-          }
-          if (tile == next_refresh) {
-            // Pooled bound over the slabs (every slab publishes its pub_j-th best per query): the slabs form
-            // pub_groups groups; the best published value of a group stands for pub_j entries >= it in ONE slab,
-            // so the minimum over the groups has pub_groups * pub_j >= k + slack distinct entries at or above it.
-            const volatile uint32_t* pub = gthr + (size_t)Bpad + r;
-            uint32_t tau = 0xffffffffu;
-            for (int g = 0; g < pub_groups; ++g) {
-              uint32_t mx = 0;
-#pragma unroll 5
-              for (int c = g; c < ncl; c += pub_groups) {
-                const uint32_t x = pub[(size_t)c * Bpad];
-                mx = x > mx ? x : mx;
-              }
-              tau = mx < tau ? mx : tau;
-            }
-            gl = tau > gl ? tau : gl;
-            gl_s[mp * kTileM + tl] = gl;
+            gl = *reinterpret_cast<volatile uint32_t*>(gl_s + mp * kTileM + tl);   // written by the refresher warp
           }
           // Admission threshold: above the list's own K-th best (strictly: an equal similarity met later has a
           // larger index), and not below what bounds the query's GLOBAL (k + slack)-th best from below: the pooled
@@ -433,6 +415,50 @@ scan_tc2_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant_
         }
         RB_PC(2, RB_CLK() - e2_);
         g_cur = g_nxt;
+      }
+    }
+    __syncwarp();
+    if (lane == 0) atomicAdd(epi_done, 1);
+  } else {
+    // ===== bound refresher (both CTAs) =====
+    // Every slab publishes, per query, the pub_j-th best similarity it has met (gthr + Bpad * (1 + slab)).  The
+    // G-th largest of those values over all slabs, G = pub_groups, has G * pub_j >= k + slack entries of the bank
+    // at or above it, so it bounds the query's global (k + slack)-th best from below -- with ~74 slabs it is close
+    // to the threshold a single stream over all rows seen so far would have.  This warp recomputes it for the
+    // CTA's queries round and round until the epilogue is done; the epilogue reads it from shared memory.
+    grid_dependency_wait();
+    const volatile int* done = epi_done;
+    while (*done < 4) {
+      for (int mp = 0; mp < n_mp && *done < 4; ++mp) {
+        for (int q4 = (warp - 6) * 2; q4 < (warp - 6) * 2 + 2; ++q4) {   // each refresher warp serves 64 of the 128 queries
+          const int tq = q4 * 32 + lane;
+          const int r = mp * kPairM + (int)rank * kTileM + tq;
+          if (mp * kPairM + (int)rank * kTileM + q4 * 32 >= B) break;   // warp-uniform
+          uint32_t top[16];   // the G largest published values, descending (G <= 16)
+#pragma unroll
+          for (int j = 0; j < 16; ++j) top[j] = 0u;
+          if (r < B) {
+            const volatile uint32_t* pub = gthr + (size_t)Bpad + r;
+#pragma unroll 2
+            for (int c = 0; c < ncl; ++c) {
+              const uint32_t x = pub[(size_t)c * Bpad];
+              if (x > top[15]) {
+#pragma unroll
+                for (int j = 15; j >= 1; --j) {
+                  const bool up = x > top[j - 1];
+                  top[j] = up ? top[j - 1] : (x > top[j] ? x : top[j]);
+                }
+                top[0] = x > top[0] ? x : top[0];
+              }
+            }
+            uint32_t tau = top[0];
+#pragma unroll
+            for (int j = 1; j < 16; ++j) tau = (j < pub_groups) ? top[j] : tau;
+            if (pub_groups > 16) tau = 0u;
+            const uint32_t old = gl_s[mp * kTileM + tq];
+            if (tau > old) gl_s[mp * kTileM + tq] = tau;
+          }
+        }
       }
     }
   }
