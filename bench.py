@@ -57,6 +57,8 @@ def parse_args(argv=None):
                     help="flush: read a 3x-L2 buffer before every timed step; warm: back-to-back steps")
     ap.add_argument("--no-scan-c4", action="store_true", help="skip the C4 (10M x 384) bank-scan roofline leg")
     ap.add_argument("--only-scan-c4", action="store_true", help="run only the C4 bank-scan leg (profiling runs)")
+    ap.add_argument("--only-scan-c3", action="store_true", help="run only the C3 tensor-bound scan leg (profiling runs)")
+    ap.add_argument("--no-large", action="store_true", help="skip the C3 (tensor-bound scan) and C5 (weight sweep) legs")
     ap.add_argument("--skip-cpu", action="store_true", help="skip the cpu_baseline / parity leg (profiling runs)")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="budget of the cpu_baseline sample")
     return ap.parse_args(argv)
@@ -189,6 +191,10 @@ def run_ours(args):
 
     if args.only_scan_c4:
         out = scan_c4(synth, Router, dev, measured_peaks()[0])
+        print(json.dumps(out))
+        return out
+    if args.only_scan_c3:
+        out = scan_c3(synth, Router, dev)
         print(json.dumps(out))
         return out
     cfg = synth.CONFIGS["C2"]
@@ -339,6 +345,9 @@ def run_ours(args):
         torch.cuda.empty_cache()
         if not args.no_scan_c4:
             out["scan_c4"] = scan_c4(synth, Router, dev, hbm_peak)
+        if not args.no_large:
+            out["scan_c3"] = scan_c3(synth, Router, dev)
+            out["sweep_c5"] = sweep_c5(synth, Router, dev)
     else:
         rt.close()
     if dist is not None:
@@ -413,6 +422,95 @@ def scan_c4(synth, Router, dev, hbm_peak):
             "bytes_per_launch": int(nbytes), "achieved": round(ach, 1), "unit": "GB/s", "peak": hbm_peak,
             "frac": round(ach / hbm_peak, 4), "frac_of_nominal_8TBs": round(ach / 8000.0, 4),
             "traffic": recorded_traffic("c4"), "l2": "bank 7.68 GB >> 126 MB L2"}
+
+
+def measured_tensor_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            j = json.load(f)
+        return float(j.get("bf16_tflops", 1590.0)), float(j.get("bf16_tflops_sustained", j.get("bf16_tflops", 1590.0))), \
+            "measured (MEASURED_PEAKS.json)"
+    return 1590.0, 1590.0, "fallback (B200_PROFILING.md)"
+
+
+def scan_c3(synth, Router, dev):
+    """BASELINE.json configs[2]: N=1M x d=1024 bf16 bank (2.05 GB), B=1024, k=10: the CTA-pair scan kernel alone
+    against the tensor roofline (2*B*N*d flop per launch, true B)."""
+    import torch
+    cfg = synth.CONFIGS["C3"]
+    bank = synth.make_bank(cfg, device=dev)
+    q = synth.make_queries(cfg, device=dev)
+    torch.cuda.synchronize()
+    rt = Router(bank["emb"], bank["quality"], bank["outlen"], cfg.k, store="bf16", max_batch=cfg.B, device=dev)
+    for _ in range(3):
+        rt.estimate(q)
+    rt.sync()
+    rt.set_stage_timing(1)
+    us, fin = [], []
+    for _ in range(10):
+        rt.estimate(q)
+        st = rt.stage_us()
+        us.append(st["scan"])
+        fin.append(st["aggregate"])
+    rt.close()
+    t = float(np.mean(us))
+    flop = 2.0 * cfg.B * cfg.N * cfg.d
+    ach = flop / (t * 1e-6) / 1e12
+    burst, sustained, src = measured_tensor_peaks()
+    return {"workload": "C3 N=1M d=1024 bf16 B=1024 k=10 (Zipf 1.1 over 256 components)", "kernel": "scan_tc2_kernel",
+            "bound": "tensor", "launch_us": round(t, 1), "flop_per_launch": flop, "achieved": round(ach, 1),
+            "unit": "TFLOP/s", "peak": burst, "frac": round(ach / burst, 4), "peak_sustained": sustained,
+            "frac_of_sustained": round(ach / sustained, 4), "peak_source": src,
+            "finish_us": round(float(np.mean(fin)), 1), "traffic": recorded_traffic("c3")}
+
+
+def sweep_c5(synth, Router, dev):
+    """BASELINE.json configs[4]: one KNN + aggregate for B=1024 requests (N=1M x d=768), then all 66 points of
+    the 3-simplex at step 0.1 through rb_decide_from_predictions(commit=0) from the same dead-reckoned state:
+    score + LPT dispatch timed in isolation (CUDA events on the library's stream, one pair per point)."""
+    import torch
+    cfg = synth.CONFIGS["C5"]
+    bank = synth.make_bank(cfg, device=dev)
+    q = synth.make_queries(cfg, device=dev)
+    plen = synth.make_prompt_len(cfg, device=dev)
+    it = synth.make_instances(cfg.I, cfg.M)
+    queued, running = synth.make_state(cfg.I, it["cap"], cfg.seed)
+    torch.cuda.synchronize()
+    rt = Router(bank["emb"], bank["quality"], bank["outlen"], cfg.k, store="bf16", max_batch=cfg.B, device=dev)
+    rt.set_instances(**it)
+    rt.set_state(queued, running)
+    for _ in range(2):
+        est = rt.estimate(q)
+    rt.sync()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(rt.stream)
+    est = rt.estimate(q)
+    e1.record(rt.stream)
+    rt.sync()
+    est_us = e0.elapsed_time(e1) * 1e3
+    pts = synth.simplex_points(0.1)
+    rt.decide_from_predictions(est["pred_quality"], est["pred_outlen"], plen, pts[0], commit=0)   # graph capture
+    rt.sync()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in pts]
+    tiers = torch.tensor(it["tier"], device=dev)
+    shares = []
+    for (a, b), w in zip(ev, pts):
+        a.record(rt.stream)
+        o = rt.decide_from_predictions(est["pred_quality"], est["pred_outlen"], plen, w, commit=0)
+        b.record(rt.stream)
+        rt.sync()
+        shares.append(torch.bincount(tiers[o["assignment"].long()], minlength=cfg.M).tolist())
+    us = np.array([a.elapsed_time(b) * 1e3 for a, b in ev])
+    rt.close()
+    corners = {("%.1f,%.1f,%.1f" % w): sh for w, sh in zip(pts, shares) if max(w) == 1.0}
+    return {"workload": "C5 N=1M d=768 bf16 B=1024 I=256 M=8, 66 simplex points, commit=0",
+            "estimate_us": round(est_us, 1), "points": len(pts), "score_dispatch_us_mean": round(float(us.mean()), 1),
+            "score_dispatch_us_p50": round(float(np.median(us)), 1), "score_dispatch_us_max": round(float(us.max()), 1),
+            "us_per_request_step": round(float(us.mean()) / cfg.B, 4),
+            "requests_per_s_score_dispatch": round(cfg.B / (float(us.mean()) * 1e-6), 1),
+            "tier_share_at_corners(qual,lat,cost)": corners,
+            "paper_context": "paper scoring loop: 12.8/14.3/22.5 us at |I|=13/100/500 per request on CPU (P:L119)"}
 
 
 # ---- reference arm = the oracle ---------------------------------------------------------------------------------

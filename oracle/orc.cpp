@@ -23,6 +23,7 @@
 
 #include <algorithm>
 #include <cmath>
+#include <climits>
 #include <cstdint>
 #include <cstring>
 #include <numeric>
@@ -149,65 +150,105 @@ int orc_aggregate(const int32_t* nn_idx, const float* nn_sim, const float* bank_
 }
 
 // One row of Eq. 1 for request r against the state (dq, bq).
-//   P:L92-95 Eq. 2   C[r,m] = l_r * c_in[m] + L^[r,m] * c_out[m]
+//   P:L92-95 Eq. 2   C[r,i] = l_r * c_in[m(i)] + L^[r,m(i)] * c_out[m(i)]; "a pre-scoring filter keeps only candidates
+//                    whose predicted total cost ... fits within" the request's budget: J_r = {i : C[r,i] <= b_r}.
+//                    Reading 24 (the paper is silent on an empty J_r): then J_r = {i : C[r,i] = min_j C[r,j]}, the
+//                    cheapest candidates.  No budget (has_budget = 0) or b_r = +inf: J_r = all instances.
 //   P:L119           T[r,i] = tpot_i * (d_i/b_i + L^[r,m(i)]); "if the instance has a free decode slot only
 //                    the second term applies" (reading 11: free <=> b_i < cap_i); reading 9: linear head
 //                    tpot_i = dec*(1+slope*b_i); reading 10: plus a prefill term pre*l_r (pre = 0 -> paper).
+//                    latency_mode 1 (P:L227 arm 4, "static per-tier prior (nominal TPOT x predicted length; zero
+//                    telemetry)"): T[r,i] = dec[m(i)] * L^[r,m(i)].
 //   P:L82-90 Eq. 1   S = w_qual*Q^ + w_cost*(1 - C/max_j C) + w_lat*(1 - T/max_j T), maxima over the
-//                    request's candidates j (reading 13), a zero maximum makes the term 0 (reading 14);
+//                    request's candidates j in J_r (reading 13), a zero maximum makes the term 0 (reading 14);
 //                    summed in Eq. 1's order (reading 15): (w_q*Q + w_c*cost) + w_l*lat.
+//                    Instances outside J_r get S = -inf (they are never chosen).
 static void score_row(int I, int M, const int32_t* tier, const int32_t* cap, const float* price_in,
                       const float* price_out, const float* pre, const float* dec, const float* slope,
                       const float* dq, const int32_t* bq, const float* Q, const float* L, int32_t ell,
-                      const float* w /*qual,lat,cost*/, float* S) {
+                      const float* w /*qual,lat,cost*/, int has_budget, float budget, int latency_mode, float* S,
+                      float* T_out /*I or NULL*/, char* cand_out /*I or NULL*/) {
   (void)M;
   std::vector<float> C(I), T(I);
-  float Cmax = 0.0f, Tmax = 0.0f;
-  bool first = true;
+  std::vector<char> cand(I, 1);
   for (int i = 0; i < I; ++i) {
     int t = tier[i];
     float c1 = (float)ell * price_in[t];
     float c2 = L[t] * price_out[t];
     C[i] = c1 + c2;
-    float a = slope[t] * (float)bq[i];
-    a = 1.0f + a;
-    float tpot = dec[t] * a;
-    float wait = (bq[i] < cap[i]) ? 0.0f : dq[i] / (float)bq[i];
-    float u = wait + L[t];
-    float v = tpot * u;
-    float p = pre[t] * (float)ell;
-    T[i] = p + v;
+    if (latency_mode == 1) {
+      T[i] = dec[t] * L[t];
+    } else {
+      float a = slope[t] * (float)bq[i];
+      a = 1.0f + a;
+      float tpot = dec[t] * a;
+      float wait = (bq[i] < cap[i]) ? 0.0f : dq[i] / (float)bq[i];
+      float u = wait + L[t];
+      float v = tpot * u;
+      float p = pre[t] * (float)ell;
+      T[i] = p + v;
+    }
+  }
+  if (has_budget) {
+    bool any = false;
+    for (int i = 0; i < I; ++i) {
+      cand[i] = (C[i] <= budget) ? 1 : 0;
+      any = any || cand[i];
+    }
+    if (!any) {
+      float Cmin = C[0];
+      for (int i = 1; i < I; ++i) Cmin = std::min(Cmin, C[i]);
+      for (int i = 0; i < I; ++i) cand[i] = (C[i] == Cmin) ? 1 : 0;
+    }
+  }
+  float Cmax = 0.0f, Tmax = 0.0f;
+  bool first = true;
+  for (int i = 0; i < I; ++i) {
+    if (!cand[i]) continue;
     if (first || C[i] > Cmax) Cmax = C[i];
     if (first || T[i] > Tmax) Tmax = T[i];
     first = false;
   }
   for (int i = 0; i < I; ++i) {
     int t = tier[i];
-    float ct = (Cmax > 0.0f) ? 1.0f - (C[i] / Cmax) : 0.0f;
-    float lt = (Tmax > 0.0f) ? 1.0f - (T[i] / Tmax) : 0.0f;
-    float t1 = w[0] * Q[t];
-    float t2 = w[2] * ct;
-    float A = t1 + t2;
-    float t3 = w[1] * lt;
-    S[i] = A + t3;
+    if (!cand[i]) {
+      S[i] = -INFINITY;
+    } else {
+      float ct = (Cmax > 0.0f) ? 1.0f - (C[i] / Cmax) : 0.0f;
+      float lt = (Tmax > 0.0f) ? 1.0f - (T[i] / Tmax) : 0.0f;
+      float t1 = w[0] * Q[t];
+      float t2 = w[2] * ct;
+      float A = t1 + t2;
+      float t3 = w[1] * lt;
+      S[i] = A + t3;
+    }
+    if (T_out) T_out[i] = T[i];
+    if (cand_out) cand_out[i] = cand[i];
   }
 }
 
-// Steps 6-9: Algorithm 1 (caption P:L109, prose P:L111).
+// Steps 6-9: Algorithm 1 (caption P:L109, prose P:L111), with the optional pieces of
+// SURVEY 8(f) #1 and #2 as arguments whose defaults (budget = NULL, update_mode = 1, tiebreak_mode = 0,
+// latency_mode = 0) give the deployed mechanism.
 //   key_r = max_m L^[r,m] over tiers that have an instance (reading 16/23), requests dispatched by
 //   (key descending, r ascending) when lpt_enabled, else in input order.
-//   Each dispatch: S[r,:] from the CURRENT local state; i* = first in the order (S descending, d ascending,
-//   i ascending) (reading 17); then, if update_enabled, d[i*] += L^[r,m(i*)] and the decode batch
-//   grows by one while a slot is free (reading 18).
+//   Each dispatch: S[r,:] from the CURRENT local state; i* = first candidate in the order
+//     tiebreak_mode 0: (S descending, d ascending, i ascending)  -- reading 17, "the scheduler's reactive
+//                      shortest-queue tiebreak" (P:L227 arm 2)
+//     tiebreak_mode 1: (S descending, T^ ascending, i ascending) -- "a predictive T^-argmin tiebreak" (arm 3);
+//   then update_mode 1: d[i*] += L^[r,m(i*)] and the decode batch grows by one while a slot is free
+//   (reading 18); update_mode 2: d only (P:L121 literally); update_mode 0: no update.
+//   max_tokens[r] ("max_tokens clamped to the remaining budget"): floor((b_r - l_r*c_in)/c_out) at the chosen
+//   model's prices, clamped to [0, 2^31-128]; INT32_MAX when r has no finite budget (or c_out = 0 and the input fits).
 //   scores0 = S[r,:] of every request from the batch-start state (reading 19).
-// dq/bq in: batch-start state; dq_out/bq_out: state after the batch (equal to the input when !update).
-int orc_decide_from_predictions(int I, int M, const int32_t* tier, const int32_t* cap,
-                                const float* price_in, const float* price_out, const float* pre,
-                                const float* dec, const float* slope, const float* dq_in,
-                                const int32_t* bq_in, const float* quality, const float* outlen,
-                                const int32_t* prompt_len, int B, const float* w, int lpt_enabled,
-                                int update_enabled, int32_t* assignment, float* scores, float* scores0,
-                                int32_t* order, float* dq_out, int32_t* bq_out) {
+// dq/bq in: batch-start state; dq_out/bq_out: state after the batch (equal to the input when update_mode = 0).
+int orc_dispatch(int I, int M, const int32_t* tier, const int32_t* cap, const float* price_in,
+                 const float* price_out, const float* pre, const float* dec, const float* slope,
+                 const float* dq_in, const int32_t* bq_in, const float* quality, const float* outlen,
+                 const int32_t* prompt_len, int B, const float* w, const float* budget /*B or NULL*/,
+                 int lpt_enabled, int update_mode, int tiebreak_mode, int latency_mode, int32_t* assignment,
+                 float* scores, float* scores0, int32_t* order, int32_t* max_tokens, float* dq_out,
+                 int32_t* bq_out) {
   std::vector<float> dq(dq_in, dq_in + I);
   std::vector<int32_t> bq(bq_in, bq_in + I);
   std::vector<char> present(M, 0);
@@ -231,10 +272,12 @@ int orc_decide_from_predictions(int I, int M, const int32_t* tier, const int32_t
     std::stable_sort(ord.begin(), ord.end(), [&](int32_t a, int32_t b) { return key[a] > key[b]; });
   }
 
-  std::vector<float> S(I);
+  std::vector<float> S(I), T(I);
+  std::vector<char> cand(I);
   for (int r = 0; r < B; ++r) {
-    score_row(I, M, tier, cap, price_in, price_out, pre, dec, slope, dq_in, bq_in,
-              quality + (int64_t)r * M, outlen + (int64_t)r * M, prompt_len[r], w, S.data());
+    score_row(I, M, tier, cap, price_in, price_out, pre, dec, slope, dq_in, bq_in, quality + (int64_t)r * M,
+              outlen + (int64_t)r * M, prompt_len[r], w, budget != nullptr, budget ? budget[r] : 0.0f, latency_mode,
+              S.data(), nullptr, nullptr);
     if (scores0) std::copy(S.begin(), S.end(), scores0 + (int64_t)r * I);
   }
 
@@ -242,23 +285,58 @@ int orc_decide_from_predictions(int I, int M, const int32_t* tier, const int32_t
     int r = ord[j];
     const float* Q = quality + (int64_t)r * M;
     const float* L = outlen + (int64_t)r * M;
-    score_row(I, M, tier, cap, price_in, price_out, pre, dec, slope, dq.data(), bq.data(), Q, L,
-              prompt_len[r], w, S.data());
-    int best = 0;
-    for (int i = 1; i < I; ++i) {
-      if (S[i] > S[best] || (S[i] == S[best] && dq[i] < dq[best])) best = i;
+    score_row(I, M, tier, cap, price_in, price_out, pre, dec, slope, dq.data(), bq.data(), Q, L, prompt_len[r], w,
+              budget != nullptr, budget ? budget[r] : 0.0f, latency_mode, S.data(), T.data(), cand.data());
+    int best = -1;
+    for (int i = 0; i < I; ++i) {
+      if (!cand[i]) continue;
+      if (best < 0) { best = i; continue; }
+      float ti = tiebreak_mode == 1 ? T[i] : dq[i];
+      float tb = tiebreak_mode == 1 ? T[best] : dq[best];
+      if (S[i] > S[best] || (S[i] == S[best] && ti < tb)) best = i;
     }
     assignment[r] = best;
     if (scores) std::copy(S.begin(), S.end(), scores + (int64_t)r * I);
     if (order) order[j] = r;
-    if (update_enabled) {
+    if (max_tokens) {
+      int32_t mt = INT32_MAX;
+      if (budget && budget[r] < INFINITY) {
+        int t = tier[best];
+        float c1 = (float)prompt_len[r] * price_in[t];
+        float rem = budget[r] - c1;
+        if (price_out[t] > 0.0f) {
+          float q = rem / price_out[t];
+          q = std::floor(q);
+          q = std::max(q, 0.0f);
+          q = std::min(q, 2147483520.0f);
+          mt = (q == q) ? (int32_t)q : 0;
+        } else {
+          mt = (rem >= 0.0f) ? INT32_MAX : 0;
+        }
+      }
+      max_tokens[r] = mt;
+    }
+    if (update_mode != 0) {
       dq[best] = dq[best] + L[tier[best]];
-      if (bq[best] < cap[best]) bq[best] += 1;
+      if (update_mode == 1 && bq[best] < cap[best]) bq[best] += 1;
     }
   }
   if (dq_out) std::copy(dq.begin(), dq.end(), dq_out);
   if (bq_out) std::copy(bq.begin(), bq.end(), bq_out);
   return 0;
+}
+
+// The deployed mechanism: no budgets, reactive tie-break, live latency, update of d and b.
+int orc_decide_from_predictions(int I, int M, const int32_t* tier, const int32_t* cap,
+                                const float* price_in, const float* price_out, const float* pre,
+                                const float* dec, const float* slope, const float* dq_in,
+                                const int32_t* bq_in, const float* quality, const float* outlen,
+                                const int32_t* prompt_len, int B, const float* w, int lpt_enabled,
+                                int update_enabled, int32_t* assignment, float* scores, float* scores0,
+                                int32_t* order, float* dq_out, int32_t* bq_out) {
+  return orc_dispatch(I, M, tier, cap, price_in, price_out, pre, dec, slope, dq_in, bq_in, quality, outlen,
+                      prompt_len, B, w, nullptr, lpt_enabled, update_enabled ? 1 : 0, 0, 0, assignment, scores,
+                      scores0, order, nullptr, dq_out, bq_out);
 }
 
 // Step 10 (BASELINE.json rb_advance_state; reading 22: the drain rule is ours, the paper re-reads telemetry):

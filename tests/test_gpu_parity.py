@@ -282,3 +282,74 @@ def test_c4_bank_scan_sampled_parity(orc):
     parity.check_predictions(orc, out["pred_quality"][rows], out["pred_outlen"][rows], out["nn_idx"][rows],
                              out["nn_sim"][rows], oi, os_, near, qn, ln)
     assert len(near) <= 2, log
+
+
+def _sampled_estimate_parity(orc, cfg, bank, query, out, rows, max_near):
+    bank_np = parity.bank_to_numpy(bank["emb"])
+    qn, ln = bank["quality"].cpu().numpy(), bank["outlen"].cpu().numpy()
+    log = []
+    oi, os_, near = parity.check_topk(orc, bank_np, query.cpu().numpy()[rows], "bf16", cfg.k, out["nn_idx"][rows],
+                                      out["nn_sim"][rows], 0.0, log)
+    parity.check_predictions(orc, out["pred_quality"][rows], out["pred_outlen"][rows], out["nn_idx"][rows],
+                             out["nn_sim"][rows], oi, os_, near, qn, ln)
+    assert len(near) <= max_near, log
+
+
+def test_c3_full_size_sampled_parity(orc):
+    """BASELINE.json configs[2] at full size (N=1M, d=1024 bf16, M=8, I=256, B=1024, Zipf-skewed topics) through
+    rb_decide in the launch shape bench.py's scan_c3 leg times (CTA-pair scan): 12 sampled queries against the
+    oracle's brute-force scan, and the whole dispatch (B=1024 x I=256) against the oracle from the GPU's predictions."""
+    cfg = synth.CONFIGS["C3"]
+    bank, it, queued, running, query, plen, rt = _setup(cfg, max_batch=cfg.B)
+    w = synth.PRESETS["balanced"]
+    g = _np(rt.decide(query, plen, w))
+    state = rt.get_state()
+    rt.close()
+    rows = [0, 1, 127, 128, 255, 256, 511, 640, 777, 900, 1022, 1023]
+    _sampled_estimate_parity(orc, cfg, bank, query, g, rows, 2)
+    parity.check_dispatch(orc, orc.Instances(**it), queued.numpy(), running.numpy(), g["pred_quality"], g["pred_outlen"],
+                          plen.cpu().numpy(), w, g, state_after=(state[0].numpy(), state[1].numpy()))
+    # properties that hold at any size: neighbours distinct and in range, similarities sorted, predictions in the labels' range
+    assert (g["nn_idx"] >= 0).all() and (g["nn_idx"] < cfg.N).all()
+    assert (np.diff(g["nn_sim"], axis=1) <= 0).all()
+    assert (g["pred_quality"] >= 0).all() and (g["pred_quality"] <= 1).all()
+    assert (g["pred_outlen"] >= 1).all() and (g["pred_outlen"] <= 8192).all()
+
+
+@pytest.mark.parametrize("B,k,slack", [(4096, 32, 8), (512, 10, 6), (1, 32, 8)])
+def test_c4_large_batch_sampled_parity(orc, B, k, slack):
+    """BASELINE.json configs[3] sweep ends: N=10M x d=384 bf16 with B=4096 / k=32 (tensor-bound, CTA-pair scan),
+    B=512 / k=10 and B=1 / k=32: 6 sampled queries each against the oracle's brute-force scan of the whole bank."""
+    cfg = dataclasses.replace(synth.CONFIGS["C4"], k=k)
+    bank = synth.make_bank(cfg, device="cuda")
+    query = synth.make_queries(cfg, B=B, device="cuda")
+    torch.cuda.synchronize()
+    rt = _router(bank, cfg, max_batch=B, rerank_slack=slack)
+    out = _np(rt.estimate(query))
+    rt.close()
+    rows = sorted(set([0, B // 7, B // 3, B // 2, (3 * B) // 4, B - 1]))
+    _sampled_estimate_parity(orc, cfg, bank, query, out, rows, 2)
+    assert (out["nn_idx"] >= 0).all() and (out["nn_idx"] < cfg.N).all()
+    assert (np.diff(out["nn_sim"], axis=1) <= 0).all()
+
+
+def test_c5_weight_sweep_all_66_points_bit_exact(orc):
+    """BASELINE.json configs[4]: N=1M x d=768, B=1024, I=256, M=8.  One estimate, then every point of the 3-simplex at
+    step 0.1 through rb_decide_from_predictions(commit=0) from the same state: assignment, order, scores and scores0
+    against the oracle for all 66 points; the state must be untouched afterwards."""
+    cfg = synth.CONFIGS["C5"]
+    bank, it, queued, running, query, plen, rt = _setup(cfg, max_batch=cfg.B)
+    est = rt.estimate(query)
+    rt.sync()
+    _sampled_estimate_parity(orc, cfg, bank, query, _np(est), [0, 300, 700, 1023], 1)
+    inst = orc.Instances(**it)
+    pq, pl = est["pred_quality"].cpu().numpy(), est["pred_outlen"].cpu().numpy()
+    pts = synth.simplex_points(0.1)
+    assert len(pts) == 66
+    for w in pts:
+        g = _np(rt.decide_from_predictions(est["pred_quality"], est["pred_outlen"], plen, w, commit=0))
+        ref = parity.check_dispatch(orc, inst, queued.numpy(), running.numpy(), pq, pl, plen.cpu().numpy(), w, g)
+        assert np.array_equal(g["scores"], ref["scores"]) and np.array_equal(g["scores0"], ref["scores0"])
+    s = rt.get_state()
+    assert np.array_equal(s[0].numpy(), queued.numpy()) and np.array_equal(s[1].numpy(), running.numpy())
+    rt.close()
