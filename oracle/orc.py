@@ -140,6 +140,35 @@ def decide_from_predictions(inst, queued, running, quality, outlen, prompt_len, 
     return dict(assignment=assignment, scores=scores, scores0=scores0, order=order, queued=dq, running=bq)
 
 
+def dispatch(inst, queued, running, quality, outlen, prompt_len, w, budget=None, lpt_enabled=1, update_mode=1,
+             tiebreak_mode=0, latency_mode=0):
+    """orc_dispatch: the score + LPT greedy stage with the optional budget admission filter (Eq. 2) and the
+    isolation-arm modes.  Returns dict(assignment, scores, scores0, order, max_tokens, queued, running)."""
+    quality = _f32(quality)
+    outlen = _f32(outlen)
+    prompt_len = _i32(prompt_len)
+    queued = _f32(queued)
+    running = _i32(running)
+    w = _f32(w)
+    bud = None if budget is None else _f32(budget)
+    B, M = quality.shape
+    assert M == inst.M
+    I = inst.I
+    assignment = np.empty(B, dtype=np.int32)
+    scores = np.empty((B, I), dtype=np.float32)
+    scores0 = np.empty((B, I), dtype=np.float32)
+    order = np.empty(B, dtype=np.int32)
+    max_tokens = np.empty(B, dtype=np.int32)
+    dq = np.empty(I, dtype=np.float32)
+    bq = np.empty(I, dtype=np.int32)
+    lib().orc_dispatch(I, M, _p(inst.tier), _p(inst.cap), _p(inst.price_in), _p(inst.price_out), _p(inst.pre),
+                       _p(inst.dec), _p(inst.slope), _p(queued), _p(running), _p(quality), _p(outlen), _p(prompt_len),
+                       B, _p(w), _p(bud), int(lpt_enabled), int(update_mode), int(tiebreak_mode), int(latency_mode),
+                       _p(assignment), _p(scores), _p(scores0), _p(order), _p(max_tokens), _p(dq), _p(bq))
+    return dict(assignment=assignment, scores=scores, scores0=scores0, order=order, max_tokens=max_tokens, queued=dq,
+                running=bq)
+
+
 def advance_state(inst, queued, running, elapsed_ms):
     dq = _f32(queued).copy()
     bq = _i32(running).copy()
