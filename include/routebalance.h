@@ -74,12 +74,19 @@ typedef struct {
   int32_t rerank_slack;   /* RB_BF16 only: the scan keeps k+slack candidates per query, their similarities */
                           /* are recomputed exactly (fp64 accumulate) and the best k kept. default 6       */
   int32_t lpt_enabled;    /* 1: dispatch in LPT order; 0: in input order.         default 1       */
-  int32_t update_enabled; /* 1: dead-reckoning update after each dispatch; 0: none. default 1    */
+  int32_t update_enabled; /* dead-reckoning update after each dispatch: 1: d += L^ and the decode batch   */
+                          /* grows by one while a slot is free (default); 2: d only (P:L121 literally); 0: none   */
   int32_t max_batch;      /* largest B any later call may pass (scratch sizing).          default 4096    */
   int32_t use_graph;      /* 1: replay the decision as a captured CUDA graph.             default 1       */
   int32_t scan_list;      /* RB_BF16 only: entries the bank scan keeps per (CTA, query): 4|8|16|32|64, or 0 = */
                           /* chosen from the bank size.  Lists shorter than k+slack are exact all the same:  */
                           /* a slab whose list might hide neighbours is searched again.   default 0       */
+  int32_t tiebreak_mode;  /* ties of the argmax over S: 0 (default): smaller queued_tokens d_i, then smaller i --  */
+                          /* "the scheduler's reactive shortest-queue tiebreak" (P:L227 arm 2); 1: smaller T^[r,i], */
+                          /* then smaller i -- "a predictive T^-argmin tiebreak" (arm 3)                           */
+  int32_t latency_mode;   /* 0 (default): live latency head over the dead-reckoned state;                */
+                          /* 1: static per-tier prior T^ = decode_ms_per_tok * L^ ("nominal TPOT x predicted       */
+                          /* length; zero telemetry", P:L227 arm 4): no wait, batch-slope or prefill term          */
   void* stream;           /* cudaStream_t all work is ordered on; NULL = legacy default stream            */
 } rb_options;
 
@@ -136,6 +143,20 @@ rb_status rb_decide(rb_ctx* ctx, const float* query_emb, const int32_t* prompt_l
                     const float w[3], int32_t* assignment, float* scores, float* pred_quality,
                     float* pred_outlen, int32_t* nn_idx, float* nn_sim);
 
+/* rb_decide with the per-request cost budgets of Eq. 2: "a pre-scoring filter keeps only candidates whose
+ * predicted total cost (input tokens plus KNN-predicted output length, at the model's rates) fits within it":
+ * the candidates of request r are the instances i with C^[r,i] = l_r*c_in[m(i)] + L^[r,m(i)]*c_out[m(i)] <= budget[r];
+ * the maxima of Eq. 1 and the argmax run over the candidates; if nothing fits, the cheapest instances are the
+ * candidates (the paper is silent; reading 24).  Filtered instances are reported with S = -inf.
+ *   budget      [host|device] B fp32, same unit as price * tokens; +inf = unconstrained; NULL = no filter (rb_decide)
+ *   max_tokens  [host|device] B int32 or NULL: floor((budget[r] - l_r*c_in)/c_out) at the chosen model's prices,
+ *               clamped to [0, 2147483520] -- the dispatch-time clamp of P:L97 ("max_tokens clamped to the remaining
+ *               budget"); INT32_MAX where budget[r] is +inf (or c_out = 0 and the prompt fits)
+ * Budgets must not be NaN.  Everything else as rb_decide. */
+rb_status rb_decide_budgeted(rb_ctx* ctx, const float* query_emb, const int32_t* prompt_len, const float* budget,
+                             int32_t B, const float w[3], int32_t* assignment, int32_t* max_tokens, float* scores,
+                             float* pred_quality, float* pred_outlen, int32_t* nn_idx, float* nn_sim);
+
 /* The score + dispatch stages alone, from caller-supplied predictions (quality, outlen: B x M fp32,
  * [host|device]).  commit = 0 leaves the dead-reckoned state untouched (weight sweeps from one state).
  *   scores0 [host|device] B x I or NULL: S[r,:] of every request evaluated from the batch-start state
@@ -144,6 +165,12 @@ rb_status rb_decide_from_predictions(rb_ctx* ctx, const float* quality, const fl
                                      const int32_t* prompt_len, int32_t B, const float w[3],
                                      int32_t commit, int32_t* assignment, float* scores,
                                      float* scores0, int32_t* order);
+
+/* rb_decide_from_predictions with budgets; budget / max_tokens as in rb_decide_budgeted. */
+rb_status rb_decide_from_predictions_budgeted(rb_ctx* ctx, const float* quality, const float* outlen,
+                                              const int32_t* prompt_len, const float* budget, int32_t B, const float w[3],
+                                              int32_t commit, int32_t* assignment, int32_t* max_tokens, float* scores,
+                                              float* scores0, int32_t* order);
 
 /* The estimate stage alone (KNN scan + merge + aggregate); outputs as in rb_decide, any may be NULL. */
 rb_status rb_estimate(rb_ctx* ctx, const float* query_emb, int32_t B, float* pred_quality,

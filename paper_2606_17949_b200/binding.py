@@ -26,7 +26,7 @@ RB_OK, RB_EINVAL, RB_ECUDA, RB_ENOMEM, RB_ESTATE, RB_EUNSUPPORTED = range(6)
 RB_F32, RB_BF16 = 0, 1
 _STATUS = {0: "RB_OK", 1: "RB_EINVAL", 2: "RB_ECUDA", 3: "RB_ENOMEM", 4: "RB_ESTATE", 5: "RB_EUNSUPPORTED"}
 EXPORTS = ["rb_options_default", "rb_create", "rb_set_instances", "rb_set_state", "rb_get_state", "rb_advance_state",
-           "rb_decide", "rb_decide_from_predictions", "rb_estimate", "rb_set_stage_timing", "rb_last_stage_us",
+           "rb_decide", "rb_decide_budgeted", "rb_decide_from_predictions", "rb_decide_from_predictions_budgeted", "rb_estimate", "rb_set_stage_timing", "rb_last_stage_us",
            "rb_launch_count", "rb_sync", "rb_last_error", "rb_destroy"]
 
 
@@ -34,7 +34,8 @@ class rb_options(ctypes.Structure):
     _fields_ = [("bank_dtype", ctypes.c_int32), ("store_dtype", ctypes.c_int32), ("weight_mode", ctypes.c_int32),
                 ("dist_eps", ctypes.c_float), ("rerank_slack", ctypes.c_int32), ("lpt_enabled", ctypes.c_int32),
                 ("update_enabled", ctypes.c_int32), ("max_batch", ctypes.c_int32), ("use_graph", ctypes.c_int32),
-                ("scan_list", ctypes.c_int32), ("stream", ctypes.c_void_p)]
+                ("scan_list", ctypes.c_int32), ("tiebreak_mode", ctypes.c_int32), ("latency_mode", ctypes.c_int32),
+                ("stream", ctypes.c_void_p)]
 
 
 class rb_lat_head(ctypes.Structure):
@@ -58,6 +59,9 @@ _lib.rb_get_state.argtypes = [_vp, _vp, _vp]
 _lib.rb_advance_state.argtypes = [_vp, _f]
 _lib.rb_decide.argtypes = [_vp, _vp, _vp, _i32, ctypes.POINTER(_f * 3), _vp, _vp, _vp, _vp, _vp, _vp]
 _lib.rb_decide_from_predictions.argtypes = [_vp, _vp, _vp, _vp, _i32, ctypes.POINTER(_f * 3), _i32, _vp, _vp, _vp, _vp]
+_lib.rb_decide_budgeted.argtypes = [_vp, _vp, _vp, _vp, _i32, ctypes.POINTER(_f * 3), _vp, _vp, _vp, _vp, _vp, _vp, _vp]
+_lib.rb_decide_from_predictions_budgeted.argtypes = [_vp, _vp, _vp, _vp, _vp, _i32, ctypes.POINTER(_f * 3), _i32, _vp, _vp,
+                                                     _vp, _vp, _vp]
 _lib.rb_estimate.argtypes = [_vp, _vp, _i32, _vp, _vp, _vp, _vp]
 _lib.rb_set_stage_timing.argtypes = [_vp, _i32]
 _lib.rb_last_stage_us.argtypes = [_vp, ctypes.POINTER(_f * 6)]
@@ -161,6 +165,24 @@ def rb_decide_from_predictions(ctx, quality, outlen, prompt_len, B, w, commit, a
     _check(ctx, _lib.rb_decide_from_predictions(ctx, _ptr(quality, f32), _ptr(outlen, f32), _ptr(prompt_len, i32), B,
                                                 _w3(w), int(commit), _ptr(assignment, i32), _ptr(scores, f32),
                                                 _ptr(scores0, f32), _ptr(order, i32)))
+
+
+def rb_decide_budgeted(ctx, query_emb, prompt_len, budget, B, w, assignment, max_tokens=None, scores=None,
+                       pred_quality=None, pred_outlen=None, nn_idx=None, nn_sim=None):
+    f32, i32 = (torch.float32, torch.int32) if torch else (np.float32, np.int32)
+    _check(ctx, _lib.rb_decide_budgeted(ctx, _ptr(query_emb, f32), _ptr(prompt_len, i32), _ptr(budget, f32), B, _w3(w),
+                                        _ptr(assignment, i32), _ptr(max_tokens, i32), _ptr(scores, f32),
+                                        _ptr(pred_quality, f32), _ptr(pred_outlen, f32), _ptr(nn_idx, i32),
+                                        _ptr(nn_sim, f32)))
+
+
+def rb_decide_from_predictions_budgeted(ctx, quality, outlen, prompt_len, budget, B, w, commit, assignment,
+                                        max_tokens=None, scores=None, scores0=None, order=None):
+    f32, i32 = (torch.float32, torch.int32) if torch else (np.float32, np.int32)
+    _check(ctx, _lib.rb_decide_from_predictions_budgeted(ctx, _ptr(quality, f32), _ptr(outlen, f32),
+                                                         _ptr(prompt_len, i32), _ptr(budget, f32), B, _w3(w),
+                                                         int(commit), _ptr(assignment, i32), _ptr(max_tokens, i32),
+                                                         _ptr(scores, f32), _ptr(scores0, f32), _ptr(order, i32)))
 
 
 def rb_estimate(ctx, query_emb, B, pred_quality=None, pred_outlen=None, nn_idx=None, nn_sim=None):

@@ -254,12 +254,15 @@ finish_kernel(FinishArgs a, InstTable t, const CallParams* __restrict__ cp) {
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int kFinThreads = blockDim.x, nwarps = blockDim.x >> 5;
   // coefficients of the score terms: requested now, consumed at the very end (their latency hides behind the merge)
-  float c_pin = 0.0f, c_pout = 0.0f, c_pre = 0.0f, c_ell = 0.0f;
+  float c_pin = 0.0f, c_pout = 0.0f, c_pre = 0.0f, c_ell = 0.0f, c_budget = 0.0f;
+  bool has_budget = false;
   if (a.with_terms && tid < a.M) {
     c_pin = t.price_in[tid];
     c_pout = t.price_out[tid];
     c_pre = t.pre[tid];
     c_ell = (float)cp->plen[r];
+    has_budget = cp->budget != nullptr;
+    if (has_budget) c_budget = cp->budget[r];
   }
   const int kc = a.kc, k = a.k, kcap = a.kcap, M = a.M;
   const uint4* qrow = reinterpret_cast<const uint4*>(a.qs + (size_t)r * a.d);
@@ -486,18 +489,11 @@ finish_kernel(FinishArgs a, InstTable t, const CallParams* __restrict__ cp) {
   __syncthreads();
   if (tid < M) {
     const int m = tid;
-    float Cmax = 0.0f, kmax = 0.0f;
-    bool first = true;
-    for (int j = 0; j < M; ++j) {
-      if (!t.present[j]) continue;
-      if (first || sC[j] > Cmax) Cmax = sC[j];
-      if (first || sL[j] > kmax) kmax = sL[j];
-      first = false;
-    }
-    const float ct = (Cmax > 0.0f) ? __fsub_rn(1.0f, __fdiv_rn(sC[m], Cmax)) : 0.0f;
-    a.termA[(size_t)r * M + m] = __fadd_rn(__fmul_rn(cp->w_qual, sQ[m]), __fmul_rn(cp->w_cost, ct));
+    float kmax;
+    const float A = tier_term_A(m, M, t.present, sC, sL, sQ[m], cp->w_qual, cp->w_cost, has_budget, c_budget, &kmax);
+    a.termA[(size_t)r * M + m] = A;
     a.termP[(size_t)r * M + m] = __fmul_rn(c_pre, c_ell);
-    if (m == 0) a.key[r] = __fadd_rn(kmax, 0.0f);   // -0 -> +0 so that the sort key order equals float order
+    if (m == 0) a.key[r] = kmax;
   }
   RB_FT(10);
 }

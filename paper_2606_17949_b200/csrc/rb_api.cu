@@ -57,7 +57,8 @@ struct rb_ctx {
   float *pred_q = nullptr, *pred_l = nullptr;   // [max_batch x M] the estimate, consumed by score/dispatch
   float *stage_q = nullptr, *stage_l = nullptr; // [max_batch x M] staging of caller-supplied predictions (host)
   float *termA = nullptr, *termP = nullptr, *key = nullptr;
-  int32_t *order = nullptr, *assignment = nullptr;
+  int32_t *order = nullptr, *assignment = nullptr, *max_tokens = nullptr;
+  float* budget = nullptr;          // [max_batch] staging of host budgets
   float *scores = nullptr, *scores0 = nullptr;  // [max_batch x I], allocated by rb_set_instances
   CUtensorMap tm_q{}, tm_bank{};
   // graphs: key = B * 4 + kind (0 decide, 1 estimate, 2 from_predictions)
@@ -104,6 +105,13 @@ bool is_host_ptr(const void* p) {
 template <typename T>
 cudaError_t dev_alloc(T** p, size_t n) {
   return cudaMalloc((void**)p, (n ? n : 1) * sizeof(T));
+}
+
+DispatchModes modes_of(const rb_ctx* c) {
+  DispatchModes m;
+  m.lpt_enabled = c->opt.lpt_enabled; m.update_mode = c->opt.update_enabled; m.tiebreak_mode = c->opt.tiebreak_mode;
+  m.latency_mode = c->opt.latency_mode;
+  return m;
 }
 
 InstTable table_of(const rb_ctx* c) {
@@ -222,12 +230,11 @@ rb_status enqueue_dispatch(rb_ctx* ctx, int B, bool from_predictions, Timer& tm)
   cudaStream_t s = ctx->stream;
   InstTable t = table_of(ctx);
   if (from_predictions) {
-    CK(launch_score(t, ctx->dq, ctx->bq, ctx->cp, B, ctx->termA, ctx->termP, ctx->key, s));
+    CK(launch_score(t, ctx->dq, ctx->bq, ctx->cp, B, ctx->termA, ctx->termP, ctx->key, modes_of(ctx), s));
     ctx->launches += 1;
   }
   tm.mark();
-  CK(launch_lpt_dispatch(t, ctx->dq, ctx->bq, ctx->termA, ctx->termP, ctx->key, ctx->cp, B, ctx->opt.lpt_enabled,
-                         ctx->opt.update_enabled, s));
+  CK(launch_lpt_dispatch(t, ctx->dq, ctx->bq, ctx->termA, ctx->termP, ctx->key, ctx->cp, B, modes_of(ctx), s));
   tm.mark();
   ctx->launches += 1;
   return RB_OK;
@@ -315,7 +322,7 @@ struct Stager {
   bool any_host = false;
   cudaError_t err = cudaSuccess;
   struct Back { void* dst; const void* src; size_t bytes; };
-  Back back[8];
+  Back back[10];
   int nback = 0;
   template <typename T>
   const T* in(const T* user, T* staging, size_t bytes) {
@@ -369,6 +376,8 @@ void rb_options_default(rb_options* opt) {
   opt->max_batch = 4096;
   opt->use_graph = 1;
   opt->scan_list = 0;
+  opt->tiebreak_mode = 0;
+  opt->latency_mode = 0;
   opt->stream = nullptr;
 }
 
@@ -388,6 +397,10 @@ rb_status rb_create(rb_ctx** out, const void* bank_emb, const float* bank_qualit
   if (opt.max_batch < 1 || opt.max_batch > 4096) return RB_EINVAL;
   if (!(opt.dist_eps >= 0.0f) || !std::isfinite(opt.dist_eps)) return RB_EINVAL;
   if (opt.weight_mode != 0 && opt.weight_mode != 1) return RB_EINVAL;
+  if (opt.update_enabled < 0 || opt.update_enabled > 2) return RB_EINVAL;
+  if (opt.tiebreak_mode != 0 && opt.tiebreak_mode != 1) return RB_EINVAL;
+  if (opt.latency_mode != 0 && opt.latency_mode != 1) return RB_EINVAL;
+  opt.lpt_enabled = opt.lpt_enabled ? 1 : 0;
   if (opt.scan_list != 0 && opt.scan_list != 4 && opt.scan_list != 8 && opt.scan_list != 16 && opt.scan_list != 32 &&
       opt.scan_list != 64)
     return RB_EINVAL;
@@ -484,6 +497,8 @@ rb_status rb_create(rb_ctx** out, const void* bank_emb, const float* bank_qualit
   ALLOC(ctx->key, mb);
   ALLOC(ctx->order, mb);
   ALLOC(ctx->assignment, mb);
+  ALLOC(ctx->max_tokens, mb);
+  ALLOC(ctx->budget, mb);
   ALLOC(ctx->tier, kMaxI);
   ALLOC(ctx->cap, kMaxI);
   ALLOC(ctx->dq, kMaxI);
@@ -622,6 +637,13 @@ rb_status rb_advance_state(rb_ctx* ctx, float elapsed_ms) {
 rb_status rb_decide(rb_ctx* ctx, const float* query_emb, const int32_t* prompt_len, int32_t B, const float w[3],
                     int32_t* assignment, float* scores, float* pred_quality, float* pred_outlen, int32_t* nn_idx,
                     float* nn_sim) {
+  return rb_decide_budgeted(ctx, query_emb, prompt_len, nullptr, B, w, assignment, nullptr, scores, pred_quality,
+                            pred_outlen, nn_idx, nn_sim);
+}
+
+rb_status rb_decide_budgeted(rb_ctx* ctx, const float* query_emb, const int32_t* prompt_len, const float* budget,
+                             int32_t B, const float w[3], int32_t* assignment, int32_t* max_tokens, float* scores,
+                             float* pred_quality, float* pred_outlen, int32_t* nn_idx, float* nn_sim) {
   if (!ctx) return RB_EINVAL;
   if (ctx->I == 0) return fail(ctx, RB_ESTATE, "rb_decide before rb_set_instances");
   if (!query_emb || !prompt_len || !assignment) return fail(ctx, RB_EINVAL, "NULL argument");
@@ -636,7 +658,9 @@ rb_status rb_decide(rb_ctx* ctx, const float* query_emb, const int32_t* prompt_l
   cp.plen = sg.in(prompt_len, ctx->plen, (size_t)B * 4);
   cp.q_src = ctx->pred_q;
   cp.l_src = ctx->pred_l;
+  cp.budget = budget ? sg.in(budget, ctx->budget, (size_t)B * 4) : nullptr;
   cp.assignment = sg.out(assignment, ctx->assignment, (size_t)B * 4);
+  cp.max_tokens = sg.out(max_tokens, ctx->max_tokens, (size_t)B * 4);
   cp.scores = sg.out(scores, ctx->scores, (size_t)B * ctx->I * 4);
   cp.pred_q = sg.out_internal(pred_quality, ctx->pred_q, bm);
   cp.pred_l = sg.out_internal(pred_outlen, ctx->pred_l, bm);
@@ -676,6 +700,14 @@ rb_status rb_estimate(rb_ctx* ctx, const float* query_emb, int32_t B, float* pre
 rb_status rb_decide_from_predictions(rb_ctx* ctx, const float* quality, const float* outlen, const int32_t* prompt_len,
                                      int32_t B, const float w[3], int32_t commit, int32_t* assignment, float* scores,
                                      float* scores0, int32_t* order) {
+  return rb_decide_from_predictions_budgeted(ctx, quality, outlen, prompt_len, nullptr, B, w, commit, assignment, nullptr,
+                                             scores, scores0, order);
+}
+
+rb_status rb_decide_from_predictions_budgeted(rb_ctx* ctx, const float* quality, const float* outlen,
+                                              const int32_t* prompt_len, const float* budget, int32_t B, const float w[3],
+                                              int32_t commit, int32_t* assignment, int32_t* max_tokens, float* scores,
+                                              float* scores0, int32_t* order) {
   if (!ctx) return RB_EINVAL;
   if (ctx->I == 0) return fail(ctx, RB_ESTATE, "rb_decide_from_predictions before rb_set_instances");
   if (!quality || !outlen || !prompt_len || !assignment) return fail(ctx, RB_EINVAL, "NULL argument");
@@ -689,7 +721,9 @@ rb_status rb_decide_from_predictions(rb_ctx* ctx, const float* quality, const fl
   cp.q_src = sg.in(quality, ctx->stage_q, bm);
   cp.l_src = sg.in(outlen, ctx->stage_l, bm);
   cp.plen = sg.in(prompt_len, ctx->plen, (size_t)B * 4);
+  cp.budget = budget ? sg.in(budget, ctx->budget, (size_t)B * 4) : nullptr;
   cp.assignment = sg.out(assignment, ctx->assignment, (size_t)B * 4);
+  cp.max_tokens = sg.out(max_tokens, ctx->max_tokens, (size_t)B * 4);
   cp.scores = sg.out(scores, ctx->scores, bi);
   cp.scores0 = sg.out(scores0, ctx->scores0, bi);
   cp.order = sg.out(order, ctx->order, (size_t)B * 4);
@@ -732,7 +766,7 @@ void rb_destroy(rb_ctx* ctx) {
                   ctx->price_out, ctx->pre, ctx->dec, ctx->slope, ctx->dec_i, ctx->slope_i, ctx->dq, ctx->bq, ctx->q32, ctx->qs, ctx->plen, ctx->cp,
                   ctx->part_sim, ctx->part_idx, ctx->gthr, ctx->sims, ctx->cand_sim, ctx->cand_idx, ctx->scratch_nn_idx, ctx->scratch_nn_sim, ctx->stage_q, ctx->stage_l,
                   ctx->pred_q, ctx->pred_l, ctx->termA, ctx->termP, ctx->key, ctx->order, ctx->assignment, ctx->scores,
-                  ctx->scores0};
+                  ctx->scores0, ctx->max_tokens, ctx->budget};
   for (void* p : ptrs) cudaFree(p);
   for (auto& e : ctx->ev)
     if (e) cudaEventDestroy(e);

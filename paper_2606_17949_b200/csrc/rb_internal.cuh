@@ -48,6 +48,16 @@ struct CallParams {
   float* pred_l;
   int32_t* nn_idx;         // [B x k] or NULL
   float* nn_sim;
+  const float* budget;     // [B] per-request cost budgets (Eq. 2) or NULL: no admission filter
+  int32_t* max_tokens;     // [B] or NULL: output-token clamp of the chosen instance
+};
+
+// Dispatch modes (rb_options; SURVEY 8(f) #2, P:L227 isolation arms, P:L266 ablations).
+struct DispatchModes {
+  int32_t lpt_enabled;     // 1: LPT order; 0: input order
+  int32_t update_mode;     // 0: none; 1: d += L^ and b = min(b+1, cap) (default); 2: d only (P:L121 literally)
+  int32_t tiebreak_mode;   // 0: (S desc, d asc, i asc) reactive shortest queue; 1: (S desc, T^ asc, i asc) predictive
+  int32_t latency_mode;    // 0: live head over the dead-reckoned state; 1: static prior T^ = dec * L^ (arm 4)
 };
 
 // ---- programmatic dependent launch ---------------------------------------------------------------------------
@@ -58,6 +68,40 @@ struct CallParams {
 #ifdef __CUDACC__
 __device__ __forceinline__ void launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 __device__ __forceinline__ void grid_dependency_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
+// a4: per-(request, tier) term A[m] = w_q*Q^ + w_c*(1 - C/Cmax) of Eq. 1, with the admission filter of
+// Eq. 2: tier m is a candidate iff it has an instance and C[m] <= budget; if no tier fits, the cheapest
+// present tiers are the candidates (reading 24).  Cmax runs over the candidates ("normalized by their
+// candidate maxima").  Non-candidates get A = -inf, which the score and dispatch kernels read as "filtered out".
+// Also returns the LPT key max_m L^ over present tiers (budgets do not enter it).  sC / sL: [M] in shared memory.
+__device__ __forceinline__ float tier_term_A(int m, int M, const int32_t* __restrict__ present, const float* sC,
+                                             const float* sL, float Q, float wq, float wc, bool has_budget, float budget,
+                                             float* key_out) {
+  float kmax = 0.0f, Cmin = 0.0f;
+  bool first = true, any = false;
+  for (int j = 0; j < M; ++j) {
+    if (!present[j]) continue;
+    if (first || sL[j] > kmax) kmax = sL[j];
+    if (first || sC[j] < Cmin) Cmin = sC[j];
+    first = false;
+    any = any || !has_budget || sC[j] <= budget;
+  }
+  float Cmax = 0.0f;
+  first = true;
+  bool mine = false;
+  for (int j = 0; j < M; ++j) {
+    if (!present[j]) continue;
+    const bool cand = any ? (!has_budget || sC[j] <= budget) : (sC[j] == Cmin);
+    if (!cand) continue;
+    if (first || sC[j] > Cmax) Cmax = sC[j];
+    first = false;
+    if (j == m) mine = true;
+  }
+  *key_out = __fadd_rn(kmax, 0.0f);   // -0 -> +0 so that the sort key order equals float order
+  if (!mine) return -INFINITY;
+  const float ct = (Cmax > 0.0f) ? __fsub_rn(1.0f, __fdiv_rn(sC[m], Cmax)) : 0.0f;
+  return __fadd_rn(__fmul_rn(wq, Q), __fmul_rn(wc, ct));
+}
 
 template <typename... KArgs, typename... Args>
 cudaError_t launch_chained(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t s, Args... args) {
@@ -147,12 +191,11 @@ cudaError_t finish_prepare(size_t max_smem);
 // a4+a5 from caller-supplied predictions (cp->q_src, cp->l_src): per-(request, tier) terms, LPT keys and the
 // batch-start score matrix (cp->scores0 when non-NULL).
 cudaError_t launch_score(InstTable t, const float* dq, const int32_t* bq, const CallParams* cp, int B, float* termA,
-                         float* termP, float* key, cudaStream_t s);
+                         float* termP, float* key, DispatchModes modes, cudaStream_t s);
 
 // a6+a7: LPT sort + greedy dispatch with dead-reckoned updates, one CTA.
 cudaError_t launch_lpt_dispatch(InstTable t, float* dq, int32_t* bq, const float* termA, const float* termP,
-                                const float* key, const CallParams* cp, int B, int lpt_enabled, int update_enabled,
-                                cudaStream_t s);
+                                const float* key, const CallParams* cp, int B, DispatchModes modes, cudaStream_t s);
 
 cudaError_t lpt_dispatch_prepare();  // opt in to the dynamic shared memory size; call once
 

@@ -7,7 +7,8 @@ from . import binding as rb
 
 class Router:
     def __init__(self, bank_emb, bank_quality, bank_outlen, k, *, store="bf16", rerank_slack=None, weight_mode=0,
-                 dist_eps=1e-6, lpt_enabled=1, update_enabled=1, max_batch=4096, use_graph=1, scan_list=0, device="cuda"):
+                 dist_eps=1e-6, lpt_enabled=1, update_enabled=1, max_batch=4096, use_graph=1, scan_list=0, tiebreak_mode=0,
+                 latency_mode=0, device="cuda"):
         N, d = bank_emb.shape
         M = bank_quality.shape[1]
         opt = rb.rb_options_default()
@@ -22,6 +23,8 @@ class Router:
         opt.max_batch = max_batch
         opt.use_graph = use_graph
         opt.scan_list = scan_list
+        opt.tiebreak_mode = tiebreak_mode
+        opt.latency_mode = latency_mode
         self.device = torch.device(device)
         self.stream = torch.cuda.Stream(device=self.device)
         opt.stream = self.stream.cuda_stream
@@ -62,9 +65,10 @@ class Router:
     def _buf(self, shape, dtype, device):
         return torch.empty(shape, dtype=dtype, device=device)
 
-    def decide(self, query, prompt_len, w, want=("scores", "pred", "nn"), out_device=None):
+    def decide(self, query, prompt_len, w, want=("scores", "pred", "nn"), out_device=None, budget=None):
         """query [B,d] float32, prompt_len [B] int32 (host or device).  Outputs land on out_device
-        (default: where the query lives).  Returns a dict of tensors."""
+        (default: where the query lives).  budget [B] float32: per-request cost budgets (Eq. 2); adds max_tokens.
+        Returns a dict of tensors."""
         B = query.shape[0]
         dev = out_device if out_device is not None else query.device
         out = {"assignment": self._buf((B,), torch.int32, dev)}
@@ -76,6 +80,12 @@ class Router:
         if "nn" in want:
             out["nn_idx"] = self._buf((B, self.k), torch.int32, dev)
             out["nn_sim"] = self._buf((B, self.k), torch.float32, dev)
+        if budget is not None:
+            out["max_tokens"] = self._buf((B,), torch.int32, dev)
+            rb.rb_decide_budgeted(self.ctx, query, prompt_len, budget, B, w, out["assignment"], out["max_tokens"],
+                                  out.get("scores"), out.get("pred_quality"), out.get("pred_outlen"), out.get("nn_idx"),
+                                  out.get("nn_sim"))
+            return out
         rb.rb_decide(self.ctx, query, prompt_len, B, w, out["assignment"], out.get("scores"), out.get("pred_quality"),
                      out.get("pred_outlen"), out.get("nn_idx"), out.get("nn_sim"))
         return out
@@ -89,11 +99,17 @@ class Router:
         rb.rb_estimate(self.ctx, query, B, out["pred_quality"], out["pred_outlen"], out["nn_idx"], out["nn_sim"])
         return out
 
-    def decide_from_predictions(self, quality, outlen, prompt_len, w, commit=0, out_device=None):
+    def decide_from_predictions(self, quality, outlen, prompt_len, w, commit=0, out_device=None, budget=None):
         B = quality.shape[0]
         dev = out_device if out_device is not None else quality.device
         out = {"assignment": self._buf((B,), torch.int32, dev), "scores": self._buf((B, self.I), torch.float32, dev),
                "scores0": self._buf((B, self.I), torch.float32, dev), "order": self._buf((B,), torch.int32, dev)}
+        if budget is not None:
+            out["max_tokens"] = self._buf((B,), torch.int32, dev)
+            rb.rb_decide_from_predictions_budgeted(self.ctx, quality, outlen, prompt_len, budget, B, w, commit,
+                                                   out["assignment"], out["max_tokens"], out["scores"], out["scores0"],
+                                                   out["order"])
+            return out
         rb.rb_decide_from_predictions(self.ctx, quality, outlen, prompt_len, B, w, commit, out["assignment"],
                                       out["scores"], out["scores0"], out["order"])
         return out

@@ -353,3 +353,92 @@ def test_c5_weight_sweep_all_66_points_bit_exact(orc):
     s = rt.get_state()
     assert np.array_equal(s[0].numpy(), queued.numpy()) and np.array_equal(s[1].numpy(), running.numpy())
     rt.close()
+
+
+def _random_budgets(rng, it, L, plen, frac_inf=0.25):
+    """Budgets around each request's own tier costs (below the cheapest -> fallback, between tiers, above all),
+    kept 1 % away from every cost so that fp32 admission is unambiguous; a share unconstrained (+inf)."""
+    pin, pout = np.asarray(it["price_in"], np.float32), np.asarray(it["price_out"], np.float32)
+    tiers = sorted(set(it["tier"]))
+    bud = np.empty(len(plen), np.float32)
+    for r in range(len(plen)):
+        C = np.unique((np.float32(plen[r]) * pin[tiers] + L[r, tiers] * pout[tiers]).astype(np.float32))
+        pick = rng.integers(0, len(C) + 1)
+        bud[r] = C[0] * 0.5 if pick == 0 else (C[-1] * 1.01 if pick == len(C) else 0.5 * (C[pick - 1] + C[pick]))
+        if rng.uniform() < frac_inf:
+            bud[r] = np.inf
+    return bud
+
+
+@pytest.mark.parametrize("I,M,B", [(13, 4, 16), (64, 4, 200), (256, 8, 1024), (33, 3, 50)])
+@pytest.mark.parametrize("upd,tb,lat", [(1, 0, 0), (2, 0, 0), (1, 1, 0), (1, 0, 1), (2, 1, 1), (0, 1, 0)])
+def test_budget_filter_and_dispatch_modes_bit_exact(orc, I, M, B, upd, tb, lat):
+    """SURVEY 8(f) #1 + #2: Eq. 2 admission filter (per-request budgets incl. the nothing-fits fallback and +inf),
+    max_tokens clamp, tie-break / latency / update modes: everything bit-exact against orc_dispatch."""
+    from paper_2606_17949_b200.router import Router
+    rng = np.random.default_rng(7 * I + B + 100 * upd + 10 * tb + lat)
+    it = synth.make_instances(I, M, cap=int(rng.integers(1, 9)))
+    bank = dict(emb=torch.randn(64, 16), quality=torch.rand(64, M), outlen=torch.rand(64, M) * 100 + 1)
+    rt = Router(bank["emb"].cuda(), bank["quality"].cuda(), bank["outlen"].cuda(), 4, store="f32", max_batch=B,
+                update_enabled=upd, tiebreak_mode=tb, latency_mode=lat)
+    rt.set_instances(**it)
+    queued = rng.integers(0, 20001, I).astype(np.float32)
+    queued[: I // 3] = queued[0]         # equal queues -> the index decides
+    running = np.minimum(rng.integers(0, 12, I), it["cap"]).astype(np.int32)
+    Q = rng.uniform(0, 1, (B, M)).astype(np.float32)
+    L = rng.lognormal(5.5, 0.7, (B, M)).astype(np.float32)
+    plen = rng.integers(1, 4000, B).astype(np.int32)
+    bud = _random_budgets(rng, it, L, plen)
+    inst = orc.Instances(**it)
+    for w in [synth.PRESETS["balanced"], (1.0, 0.0, 0.0), (0.5, 0.0, 0.5), (0.0, 1.0, 0.0), (0.0, 0.0, 1.0)]:
+        for budget in (bud, None):
+            rt.set_state(torch.from_numpy(queued), torch.from_numpy(running))
+            out = rt.decide_from_predictions(torch.from_numpy(Q).cuda(), torch.from_numpy(L).cuda(),
+                                             torch.from_numpy(plen).cuda(), w, commit=1,
+                                             budget=None if budget is None else torch.from_numpy(budget).cuda())
+            g = _np(out)
+            ref = orc.dispatch(inst, queued, running, Q, L, plen, w, budget=budget, update_mode=upd, tiebreak_mode=tb,
+                               latency_mode=lat)
+            for key in ("assignment", "order", "scores", "scores0"):
+                assert np.array_equal(g[key], ref[key]), (key, w, budget is None)
+            if budget is not None:
+                assert np.array_equal(g["max_tokens"], ref["max_tokens"])
+                fits = (g["scores"] > -np.inf).any(axis=1)
+                assert fits.all()
+            s = rt.get_state()
+            assert np.array_equal(s[0].numpy(), ref["queued"]) and np.array_equal(s[1].numpy(), ref["running"])
+    rt.close()
+
+
+def test_decide_budgeted_full_path(orc):
+    """rb_decide_budgeted end to end (bf16 scan -> finish kernel's terms with the filter -> dispatch), device and host
+    buffers, graph replay: predictions against the oracle, then the dispatch against orc_dispatch from the GPU's own
+    predictions."""
+    cfg = dataclasses.replace(synth.CONFIGS["C2"], N=20000, d=128, B=48, Kc=16, seed=21)
+    bank, it, queued, running, query, plen, rt = _setup(cfg, max_batch=64)
+    rng = np.random.default_rng(3)
+    w = synth.PRESETS["quality"]
+    est = _np(rt.estimate(query))
+    bud = torch.from_numpy(_random_budgets(rng, it, est["pred_outlen"], plen.cpu().numpy()))
+    inst = orc.Instances(**it)
+    for host in (False, True):
+        rt.set_state(queued, running)
+        q, p, b = (query.cpu(), plen.cpu(), bud) if host else (query, plen, bud.cuda())
+        for _ in range(2):                    # second call replays the captured graph
+            rt.set_state(queued, running)
+            g = _np(rt.decide(q, p, w, budget=b))
+        assert np.array_equal(g["pred_outlen"], est["pred_outlen"]) and np.array_equal(g["pred_quality"], est["pred_quality"])
+        ref = orc.dispatch(inst, queued.numpy(), running.numpy(), g["pred_quality"], g["pred_outlen"], plen.cpu().numpy(), w,
+                           budget=bud.numpy())
+        for key in ("assignment", "scores", "max_tokens"):
+            assert np.array_equal(g[key], ref[key]), key
+        s = rt.get_state()
+        assert np.array_equal(s[0].numpy(), ref["queued"]) and np.array_equal(s[1].numpy(), ref["running"])
+    # no budget through the same entry point == rb_decide
+    rt.set_state(queued, running)
+    g0 = _np(rt.decide(query, plen, w))
+    rt.set_state(queued, running)
+    g1 = _np(rt.decide(query, plen, w, budget=torch.full((cfg.B,), float("inf"), device="cuda")))
+    assert np.array_equal(g0["assignment"], g1["assignment"]) and np.array_equal(g0["scores"], g1["scores"])
+    assert (g1["max_tokens"] == 2**31 - 1).all()
+    rt.close()
