@@ -149,6 +149,42 @@ int orc_aggregate(const int32_t* nn_idx, const float* nn_sim, const float* bank_
   return 0;
 }
 
+// Gradient-boosted TPOT head ("For each (model, GPU) tier we train one XGBoost TPOT head"; P:L131 telemetry:
+// "queue depth, pending decode work, active sequences, KV-cache pressure, recent service rate").  The paper's trained
+// boosters are not available, so the forest is an INPUT; what is restated here is the evaluation rule of an XGBoost
+// regression forest (reading 9b):
+//   features of instance i:  x[0] = (float)b_i (active sequences), x[1] = d_i (pending decode work),
+//                            x[2+j] = aux[i, j], the remaining telemetry fields, constant during a batch
+//   node: feature >= 0 -> internal, go to `left` if x[feature] < value else to `right`; feature < 0 -> leaf `value`
+//   prediction of tier t:    p = base[t]; for each tree of the tier, in order: p = p + leaf(tree, x)   (fp32)
+//   tpot_i = max(p, 1e-6)   (a TPOT is positive; the floor keeps T^ and the drain rule finite for any forest)
+struct orc_forest {
+  const int32_t* node_feature;
+  const float* node_value;
+  const int32_t* node_left;
+  const int32_t* node_right;
+  const int32_t* tree_root;        // [n_trees] index of each tree's root node
+  const int32_t* tier_tree_begin;  // [M+1] trees of tier t: tree_root[tier_tree_begin[t] .. tier_tree_begin[t+1])
+  const float* base;               // [M]
+  int32_t n_features;              // F = 2 + Fa
+  const float* aux;                // [I x Fa] or NULL when Fa = 0
+};
+
+static float gbdt_tpot(const orc_forest* f, int t, int32_t b, float d, int i) {
+  const int Fa = f->n_features - 2;
+  float p = f->base[t];
+  for (int tr = f->tier_tree_begin[t]; tr < f->tier_tree_begin[t + 1]; ++tr) {
+    int n = f->tree_root[tr];
+    while (f->node_feature[n] >= 0) {
+      int c = f->node_feature[n];
+      float x = (c == 0) ? (float)b : (c == 1) ? d : f->aux[(int64_t)i * Fa + (c - 2)];
+      n = (x < f->node_value[n]) ? f->node_left[n] : f->node_right[n];
+    }
+    p = p + f->node_value[n];
+  }
+  return std::max(p, 1e-6f);
+}
+
 // One row of Eq. 1 for request r against the state (dq, bq).
 //   P:L92-95 Eq. 2   C[r,i] = l_r * c_in[m(i)] + L^[r,m(i)] * c_out[m(i)]; "a pre-scoring filter keeps only candidates
 //                    whose predicted total cost ... fits within" the request's budget: J_r = {i : C[r,i] <= b_r}.
@@ -159,6 +195,8 @@ int orc_aggregate(const int32_t* nn_idx, const float* nn_sim, const float* bank_
 //                    tpot_i = dec*(1+slope*b_i); reading 10: plus a prefill term pre*l_r (pre = 0 -> paper).
 //                    latency_mode 1 (P:L227 arm 4, "static per-tier prior (nominal TPOT x predicted length; zero
 //                    telemetry)"): T[r,i] = dec[m(i)] * L^[r,m(i)].
+//                    latency_mode 2: tpot_i from the tier's gradient-boosted head (gbdt_tpot above) instead of the
+//                    linear stand-in; the rest of the formula is unchanged.
 //   P:L82-90 Eq. 1   S = w_qual*Q^ + w_cost*(1 - C/max_j C) + w_lat*(1 - T/max_j T), maxima over the
 //                    request's candidates j in J_r (reading 13), a zero maximum makes the term 0 (reading 14);
 //                    summed in Eq. 1's order (reading 15): (w_q*Q + w_c*cost) + w_l*lat.
@@ -166,8 +204,8 @@ int orc_aggregate(const int32_t* nn_idx, const float* nn_sim, const float* bank_
 static void score_row(int I, int M, const int32_t* tier, const int32_t* cap, const float* price_in,
                       const float* price_out, const float* pre, const float* dec, const float* slope,
                       const float* dq, const int32_t* bq, const float* Q, const float* L, int32_t ell,
-                      const float* w /*qual,lat,cost*/, int has_budget, float budget, int latency_mode, float* S,
-                      float* T_out /*I or NULL*/, char* cand_out /*I or NULL*/) {
+                      const float* w /*qual,lat,cost*/, int has_budget, float budget, int latency_mode,
+                      const orc_forest* forest, float* S, float* T_out /*I or NULL*/, char* cand_out /*I or NULL*/) {
   (void)M;
   std::vector<float> C(I), T(I);
   std::vector<char> cand(I, 1);
@@ -179,9 +217,14 @@ static void score_row(int I, int M, const int32_t* tier, const int32_t* cap, con
     if (latency_mode == 1) {
       T[i] = dec[t] * L[t];
     } else {
-      float a = slope[t] * (float)bq[i];
-      a = 1.0f + a;
-      float tpot = dec[t] * a;
+      float tpot;
+      if (latency_mode == 2) {   // reading 9b: the tier's boosted TPOT head over the instance's telemetry
+        tpot = gbdt_tpot(forest, t, bq[i], dq[i], i);
+      } else {
+        float a = slope[t] * (float)bq[i];
+        a = 1.0f + a;
+        tpot = dec[t] * a;
+      }
       float wait = (bq[i] < cap[i]) ? 0.0f : dq[i] / (float)bq[i];
       float u = wait + L[t];
       float v = tpot * u;
@@ -242,13 +285,14 @@ static void score_row(int I, int M, const int32_t* tier, const int32_t* cap, con
 //   model's prices, clamped to [0, 2^31-128]; INT32_MAX when r has no finite budget (or c_out = 0 and the input fits).
 //   scores0 = S[r,:] of every request from the batch-start state (reading 19).
 // dq/bq in: batch-start state; dq_out/bq_out: state after the batch (equal to the input when update_mode = 0).
-int orc_dispatch(int I, int M, const int32_t* tier, const int32_t* cap, const float* price_in,
-                 const float* price_out, const float* pre, const float* dec, const float* slope,
-                 const float* dq_in, const int32_t* bq_in, const float* quality, const float* outlen,
-                 const int32_t* prompt_len, int B, const float* w, const float* budget /*B or NULL*/,
-                 int lpt_enabled, int update_mode, int tiebreak_mode, int latency_mode, int32_t* assignment,
-                 float* scores, float* scores0, int32_t* order, int32_t* max_tokens, float* dq_out,
-                 int32_t* bq_out) {
+int orc_dispatch_gbdt(int I, int M, const int32_t* tier, const int32_t* cap, const float* price_in,
+                      const float* price_out, const float* pre, const float* dec, const float* slope,
+                      const float* dq_in, const int32_t* bq_in, const float* quality, const float* outlen,
+                      const int32_t* prompt_len, int B, const float* w, const float* budget /*B or NULL*/,
+                      int lpt_enabled, int update_mode, int tiebreak_mode, int latency_mode,
+                      const orc_forest* forest /*latency_mode 2*/, int32_t* assignment, float* scores,
+                      float* scores0, int32_t* order, int32_t* max_tokens, float* dq_out, int32_t* bq_out) {
+  if (latency_mode == 2 && forest == nullptr) return 1;
   std::vector<float> dq(dq_in, dq_in + I);
   std::vector<int32_t> bq(bq_in, bq_in + I);
   std::vector<char> present(M, 0);
@@ -277,7 +321,7 @@ int orc_dispatch(int I, int M, const int32_t* tier, const int32_t* cap, const fl
   for (int r = 0; r < B; ++r) {
     score_row(I, M, tier, cap, price_in, price_out, pre, dec, slope, dq_in, bq_in, quality + (int64_t)r * M,
               outlen + (int64_t)r * M, prompt_len[r], w, budget != nullptr, budget ? budget[r] : 0.0f, latency_mode,
-              S.data(), nullptr, nullptr);
+              forest, S.data(), nullptr, nullptr);
     if (scores0) std::copy(S.begin(), S.end(), scores0 + (int64_t)r * I);
   }
 
@@ -286,7 +330,7 @@ int orc_dispatch(int I, int M, const int32_t* tier, const int32_t* cap, const fl
     const float* Q = quality + (int64_t)r * M;
     const float* L = outlen + (int64_t)r * M;
     score_row(I, M, tier, cap, price_in, price_out, pre, dec, slope, dq.data(), bq.data(), Q, L, prompt_len[r], w,
-              budget != nullptr, budget ? budget[r] : 0.0f, latency_mode, S.data(), T.data(), cand.data());
+              budget != nullptr, budget ? budget[r] : 0.0f, latency_mode, forest, S.data(), T.data(), cand.data());
     int best = -1;
     for (int i = 0; i < I; ++i) {
       if (!cand[i]) continue;
@@ -326,6 +370,25 @@ int orc_dispatch(int I, int M, const int32_t* tier, const int32_t* cap, const fl
   return 0;
 }
 
+int orc_dispatch(int I, int M, const int32_t* tier, const int32_t* cap, const float* price_in,
+                 const float* price_out, const float* pre, const float* dec, const float* slope,
+                 const float* dq_in, const int32_t* bq_in, const float* quality, const float* outlen,
+                 const int32_t* prompt_len, int B, const float* w, const float* budget /*B or NULL*/,
+                 int lpt_enabled, int update_mode, int tiebreak_mode, int latency_mode, int32_t* assignment,
+                 float* scores, float* scores0, int32_t* order, int32_t* max_tokens, float* dq_out,
+                 int32_t* bq_out) {
+  return orc_dispatch_gbdt(I, M, tier, cap, price_in, price_out, pre, dec, slope, dq_in, bq_in, quality, outlen,
+                           prompt_len, B, w, budget, lpt_enabled, update_mode, tiebreak_mode, latency_mode, nullptr,
+                           assignment, scores, scores0, order, max_tokens, dq_out, bq_out);
+}
+
+// tpot of every instance from the boosted head (what latency_mode 2 uses), for tests of the forest rule alone.
+int orc_gbdt_tpot(int I, const int32_t* tier, const orc_forest* forest, const float* dq, const int32_t* bq,
+                  float* tpot) {
+  for (int i = 0; i < I; ++i) tpot[i] = gbdt_tpot(forest, tier[i], bq[i], dq[i], i);
+  return 0;
+}
+
 // The deployed mechanism: no budgets, reactive tie-break, live latency, update of d and b.
 int orc_decide_from_predictions(int I, int M, const int32_t* tier, const int32_t* cap,
                                 const float* price_in, const float* price_out, const float* pre,
@@ -349,6 +412,22 @@ int orc_advance_state(int I, const int32_t* tier, const float* dec, const float*
     float a = slope[t] * (float)bq[i];
     a = 1.0f + a;
     float tpot = dec[t] * a;
+    float q = elapsed_ms / tpot;
+    float done = (float)bq[i] * q;
+    float d = dq[i] - done;
+    d = std::max(d, 0.0f);
+    dq[i] = d;
+    if (d == 0.0f) bq[i] = 0;
+  }
+  return 0;
+}
+
+// Step 10 with the boosted head: the same drain rule, tpot_i from gbdt_tpot.
+int orc_advance_state_gbdt(int I, const int32_t* tier, const orc_forest* forest, float elapsed_ms, float* dq,
+                           int32_t* bq) {
+  for (int i = 0; i < I; ++i) {
+    if (bq[i] <= 0) continue;
+    float tpot = gbdt_tpot(forest, tier[i], bq[i], dq[i], i);
     float q = elapsed_ms / tpot;
     float done = (float)bq[i] * q;
     float d = dq[i] - done;

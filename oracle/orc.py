@@ -140,8 +140,51 @@ def decide_from_predictions(inst, queued, running, quality, outlen, prompt_len, 
     return dict(assignment=assignment, scores=scores, scores0=scores0, order=order, queued=dq, running=bq)
 
 
+class _CForest(ctypes.Structure):
+    _fields_ = [("node_feature", ctypes.c_void_p), ("node_value", ctypes.c_void_p), ("node_left", ctypes.c_void_p),
+                ("node_right", ctypes.c_void_p), ("tree_root", ctypes.c_void_p), ("tier_tree_begin", ctypes.c_void_p),
+                ("base", ctypes.c_void_p), ("n_features", ctypes.c_int32), ("aux", ctypes.c_void_p)]
+
+
+class Forest:
+    """Plain record of a boosted TPOT head: node arrays (feature, value, left, right), tree_root [n_trees],
+    tier_tree_begin [M+1], base [M], n_features = 2 + Fa and the per-instance auxiliary telemetry aux [I, Fa]."""
+
+    def __init__(self, node_feature, node_value, node_left, node_right, tree_root, tier_tree_begin, base, n_features,
+                 aux=None):
+        self.node_feature = _i32(node_feature)
+        self.node_value = _f32(node_value)
+        self.node_left = _i32(node_left)
+        self.node_right = _i32(node_right)
+        self.tree_root = _i32(tree_root)
+        self.tier_tree_begin = _i32(tier_tree_begin)
+        self.base = _f32(base)
+        self.n_features = int(n_features)
+        self.aux = None if aux is None else _f32(aux)
+
+    def c(self):
+        return _CForest(_p(self.node_feature), _p(self.node_value), _p(self.node_left), _p(self.node_right),
+                        _p(self.tree_root), _p(self.tier_tree_begin), _p(self.base), self.n_features, _p(self.aux))
+
+
+def gbdt_tpot(inst, forest, queued, running):
+    queued, running = _f32(queued), _i32(running)
+    out = np.empty(inst.I, dtype=np.float32)
+    cf = forest.c()
+    lib().orc_gbdt_tpot(inst.I, _p(inst.tier), ctypes.byref(cf), _p(queued), _p(running), _p(out))
+    return out
+
+
+def advance_state_gbdt(inst, forest, queued, running, elapsed_ms):
+    dq = _f32(queued).copy()
+    bq = _i32(running).copy()
+    cf = forest.c()
+    lib().orc_advance_state_gbdt(inst.I, _p(inst.tier), ctypes.byref(cf), ctypes.c_float(elapsed_ms), _p(dq), _p(bq))
+    return dq, bq
+
+
 def dispatch(inst, queued, running, quality, outlen, prompt_len, w, budget=None, lpt_enabled=1, update_mode=1,
-             tiebreak_mode=0, latency_mode=0):
+             tiebreak_mode=0, latency_mode=0, forest=None):
     """orc_dispatch: the score + LPT greedy stage with the optional budget admission filter (Eq. 2) and the
     isolation-arm modes.  Returns dict(assignment, scores, scores0, order, max_tokens, queued, running)."""
     quality = _f32(quality)
@@ -161,10 +204,14 @@ def dispatch(inst, queued, running, quality, outlen, prompt_len, w, budget=None,
     max_tokens = np.empty(B, dtype=np.int32)
     dq = np.empty(I, dtype=np.float32)
     bq = np.empty(I, dtype=np.int32)
-    lib().orc_dispatch(I, M, _p(inst.tier), _p(inst.cap), _p(inst.price_in), _p(inst.price_out), _p(inst.pre),
-                       _p(inst.dec), _p(inst.slope), _p(queued), _p(running), _p(quality), _p(outlen), _p(prompt_len),
-                       B, _p(w), _p(bud), int(lpt_enabled), int(update_mode), int(tiebreak_mode), int(latency_mode),
-                       _p(assignment), _p(scores), _p(scores0), _p(order), _p(max_tokens), _p(dq), _p(bq))
+    cf = forest.c() if forest is not None else None
+    rc = lib().orc_dispatch_gbdt(I, M, _p(inst.tier), _p(inst.cap), _p(inst.price_in), _p(inst.price_out), _p(inst.pre),
+                                 _p(inst.dec), _p(inst.slope), _p(queued), _p(running), _p(quality), _p(outlen),
+                                 _p(prompt_len), B, _p(w), _p(bud), int(lpt_enabled), int(update_mode),
+                                 int(tiebreak_mode), int(latency_mode), ctypes.byref(cf) if cf is not None else None,
+                                 _p(assignment), _p(scores), _p(scores0), _p(order), _p(max_tokens), _p(dq), _p(bq))
+    if rc != 0:
+        raise ValueError("orc_dispatch_gbdt: latency_mode 2 needs a forest")
     return dict(assignment=assignment, scores=scores, scores0=scores0, order=order, max_tokens=max_tokens, queued=dq,
                 running=bq)
 

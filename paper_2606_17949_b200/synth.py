@@ -190,3 +190,69 @@ def simplex_points(step=0.1):
     """All weight vectors (w_qual, w_lat, w_cost) on the 3-simplex at the given step (66 points at 0.1)."""
     n = round(1.0 / step)
     return [(a / n, b / n, (n - a - b) / n) for a in range(n + 1) for b in range(n + 1 - a)]
+
+
+# ---- gradient-boosted TPOT heads (P:L119): the paper's trained boosters are unavailable, so forests are drawn ----
+def make_forest(M, dec, n_trees=32, depth=4, Fa=2, seed=0, stream=8, I=None):
+    """A random regression forest per tier in the node format of include/routebalance.h (rb_tree_node): features
+    x[0] = running b, x[1] = queued tokens d, x[2..] = auxiliary telemetry in [0,1].  Leaves are small corrections
+    around base[t] = dec[t], rising with b, so that the predicted TPOT stays positive and load-dependent.
+    Returns dict(node_feature, node_value, node_left, node_right, tree_root, tier_tree_begin, base, n_features, aux)."""
+    g = _gen(seed, stream, "cpu")
+    F = 2 + Fa
+    feat, val, left, right, roots, begin = [], [], [], [], [], [0]
+
+    def rnd():
+        return float(torch.rand((), generator=g))
+
+    def grow(t, level, lo_b, hi_b):
+        n = len(feat)
+        feat.append(-1), val.append(0.0), left.append(-1), right.append(-1)
+        if level == depth or (level >= 1 and rnd() < 0.15):
+            mid = 0.5 * (lo_b + hi_b) / 32.0
+            val[n] = dec[t] * 0.04 * (mid - 0.5 + 0.5 * (rnd() - 0.5))
+            return n
+        u = rnd()
+        c = 0 if u < 0.5 else (1 if u < 0.75 or Fa == 0 else 2 + int(rnd() * Fa) % Fa)
+        feat[n] = c
+        if c == 0:
+            thr = float(int(lo_b + rnd() * max(1.0, hi_b - lo_b))) + 0.5
+            val[n] = thr
+            left[n] = grow(t, level + 1, lo_b, min(hi_b, thr))
+            right[n] = grow(t, level + 1, max(lo_b, thr), hi_b)
+        else:
+            val[n] = rnd() * (20000.0 if c == 1 else 1.0)
+            left[n] = grow(t, level + 1, lo_b, hi_b)
+            right[n] = grow(t, level + 1, lo_b, hi_b)
+        return n
+
+    for t in range(M):
+        for _ in range(n_trees):
+            roots.append(grow(t, 0, 0.0, 32.0))
+        begin.append(len(roots))
+    aux = None
+    if I is not None and Fa > 0:
+        aux = torch.rand(I, Fa, generator=g)
+    return dict(node_feature=feat, node_value=val, node_left=left, node_right=right, tree_root=roots,
+                tier_tree_begin=begin, base=[float(x) for x in dec], n_features=F, aux=aux)
+
+
+def lookup_forest(M, dec, slope, bmax):
+    """One tree per tier that tabulates a function of the running batch b = 0..bmax (a chain of splits at b + 0.5);
+    the leaf of b holds the caller-supplied value table[t][b].  Used with table = the linear head's tpot to check that
+    the boosted-head path reproduces the linear one.  Returns (forest dict without leaf values filled, leaf_index[t][b])."""
+    feat, val, left, right, roots, begin, leaf_index = [], [], [], [], [], [0], []
+    for t in range(M):
+        roots.append(len(feat))
+        idx = []
+        for b in range(bmax):
+            n = len(feat)
+            feat.append(0), val.append(b + 0.5), left.append(n + 1), right.append(n + 2)
+            idx.append(len(feat))
+            feat.append(-1), val.append(0.0), left.append(-1), right.append(-1)
+        idx.append(len(feat))
+        feat.append(-1), val.append(0.0), left.append(-1), right.append(-1)
+        leaf_index.append(idx)
+        begin.append(len(roots))
+    return dict(node_feature=feat, node_value=val, node_left=left, node_right=right, tree_root=roots,
+                tier_tree_begin=begin, base=[0.0] * M, n_features=2, aux=None), leaf_index
