@@ -503,12 +503,34 @@ def sweep_c5(synth, Router, dev):
         shares.append(torch.bincount(tiers[o["assignment"].long()], minlength=cfg.M).tolist())
     us = np.array([a.elapsed_time(b) * 1e3 for a, b in ev])
     rt.close()
+    # the same sweep with the gradient-boosted TPOT head (latency_mode 2; synthetic forest: 64 trees of depth 5 per
+    # tier, 2 auxiliary telemetry features) -- the paper's head is a per-tier XGBoost booster
+    small = synth.make_bank(synth.CONFIGS["C1"], device=dev)
+    rt2 = Router(small["emb"].repeat(1, 1), small["quality"][:, :1].repeat(1, cfg.M), small["outlen"][:, :1].repeat(1, cfg.M),
+                 4, store="f32", max_batch=cfg.B, latency_mode=2, device=dev)
+    rt2.set_instances(**it)
+    fd = synth.make_forest(cfg.M, it["dec"], n_trees=64, depth=5, Fa=2, seed=cfg.seed, I=cfg.I)
+    aux = fd.pop("aux")
+    rt2.set_tpot_forest(aux=aux.to(dev), **fd)
+    rt2.set_state(queued, running)
+    rt2.decide_from_predictions(est["pred_quality"], est["pred_outlen"], plen, pts[0], commit=0)
+    rt2.sync()
+    ev2 = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in pts]
+    for (a, b), w in zip(ev2, pts):
+        a.record(rt2.stream)
+        rt2.decide_from_predictions(est["pred_quality"], est["pred_outlen"], plen, w, commit=0)
+        b.record(rt2.stream)
+    rt2.sync()
+    us2 = np.array([a.elapsed_time(b) * 1e3 for a, b in ev2])
+    rt2.close()
     corners = {("%.1f,%.1f,%.1f" % w): sh for w, sh in zip(pts, shares) if max(w) == 1.0}
     return {"workload": "C5 N=1M d=768 bf16 B=1024 I=256 M=8, 66 simplex points, commit=0",
             "estimate_us": round(est_us, 1), "points": len(pts), "score_dispatch_us_mean": round(float(us.mean()), 1),
             "score_dispatch_us_p50": round(float(np.median(us)), 1), "score_dispatch_us_max": round(float(us.max()), 1),
             "us_per_request_step": round(float(us.mean()) / cfg.B, 4),
             "requests_per_s_score_dispatch": round(cfg.B / (float(us.mean()) * 1e-6), 1),
+            "boosted_head": {"forest": "64 trees x depth 5 per tier, 4 features, synthetic", "score_dispatch_us_mean":
+                             round(float(us2.mean()), 1), "us_per_request_step": round(float(us2.mean()) / cfg.B, 4)},
             "tier_share_at_corners(qual,lat,cost)": corners,
             "paper_context": "paper scoring loop: 12.8/14.3/22.5 us at |I|=13/100/500 per request on CPU (P:L119)"}
 

@@ -84,7 +84,8 @@ typedef struct {
   int32_t tiebreak_mode;  /* ties of the argmax over S: 0 (default): smaller queued_tokens d_i, then smaller i --  */
                           /* "the scheduler's reactive shortest-queue tiebreak" (P:L227 arm 2); 1: smaller T^[r,i], */
                           /* then smaller i -- "a predictive T^-argmin tiebreak" (arm 3)                           */
-  int32_t latency_mode;   /* 0 (default): live latency head over the dead-reckoned state;                */
+  int32_t latency_mode;   /* 0 (default): live linear latency head over the dead-reckoned state;         */
+                          /* 2: live gradient-boosted TPOT head (rb_set_tpot_forest) in place of the linear one;   */
                           /* 1: static per-tier prior T^ = decode_ms_per_tok * L^ ("nominal TPOT x predicted       */
                           /* length; zero telemetry", P:L227 arm 4): no wait, batch-slope or prefill term          */
   void* stream;           /* cudaStream_t all work is ordered on; NULL = legacy default stream            */
@@ -116,6 +117,35 @@ rb_status rb_create(rb_ctx** out, const void* bank_emb, const float* bank_qualit
  *   1 <= I <= 1024.  May be called again at any time between decisions (tier loss). */
 rb_status rb_set_instances(rb_ctx* ctx, int32_t I, const int32_t* tier, const int32_t* cap,
                            const float* price_in, const float* price_out, const rb_lat_head* heads);
+
+/* Gradient-boosted TPOT head ("For each (model, GPU) tier we train one XGBoost TPOT head ... one XGBoost call
+ * per tier (not per instance)").  The trained boosters of the paper are not available: the forest is an input, and
+ * what the library implements is the evaluation rule of an XGBoost regression forest (reading 9b):
+ *   features of instance i  x[0] = (float)running_i, x[1] = queued_tokens_i (both dead-reckoned within a batch),
+ *                           x[2+j] = aux[i,j]: further telemetry (queue depth, KV-cache pressure, recent
+ *                           service rate), constant during a batch, set with rb_set_telemetry (default 0)
+ *   node                    feature >= 0: go to `left` if x[feature] < value, else to `right`; feature < 0: leaf `value`
+ *   tier t                  p = base[t]; for each tree of the tier in order: p = p + leaf   (fp32);  tpot = max(p, 1e-6)
+ * Used when rb_options.latency_mode = 2: tpot_i replaces decode_ms_per_tok*(1+batch_slope*b_i) in T^ and in
+ * rb_advance_state; the chosen instance's head is evaluated again after every dispatch.
+ *   nodes            [host] n_nodes; children of an internal node must have larger indices than the node
+ *   tree_root        [host] n_trees node indices
+ *   tier_tree_begin  [host] M+1: trees of tier t are tree_root[tier_tree_begin[t] .. tier_tree_begin[t+1]), <= 256 each
+ *   base             [host] M;  n_features = 2 + (aux columns), in [2,8]
+ * Errors: RB_EINVAL (ranges, non-finite values, backward links), RB_ENOMEM.  Decisions under latency_mode 2 return
+ * RB_ESTATE until a forest is set. */
+typedef struct {
+  int32_t feature;
+  float value;
+  int32_t left;
+  int32_t right;
+} rb_tree_node;
+rb_status rb_set_tpot_forest(rb_ctx* ctx, const rb_tree_node* nodes, int32_t n_nodes, const int32_t* tree_root,
+                             int32_t n_trees, const int32_t* tier_tree_begin, const float* base, int32_t n_features);
+
+/* Auxiliary telemetry features of the boosted head: aux [host|device] I x (n_features - 2) fp32, row i = instance i.
+ * Reset to 0 by rb_set_instances.  RB_ESTATE before rb_set_instances / rb_set_tpot_forest. */
+rb_status rb_set_telemetry(rb_ctx* ctx, const float* aux);
 
 /* Seeds the dead-reckoned state from telemetry: queued_tokens[i] = pending decode tokens
  * d_i >= 0 (finite), running[i] = decode batch size b_i >= 0.  Both [host|device], I entries. */

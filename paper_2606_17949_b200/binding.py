@@ -25,7 +25,7 @@ _lib = ctypes.CDLL(LIB_PATH)
 RB_OK, RB_EINVAL, RB_ECUDA, RB_ENOMEM, RB_ESTATE, RB_EUNSUPPORTED = range(6)
 RB_F32, RB_BF16 = 0, 1
 _STATUS = {0: "RB_OK", 1: "RB_EINVAL", 2: "RB_ECUDA", 3: "RB_ENOMEM", 4: "RB_ESTATE", 5: "RB_EUNSUPPORTED"}
-EXPORTS = ["rb_options_default", "rb_create", "rb_set_instances", "rb_set_state", "rb_get_state", "rb_advance_state",
+EXPORTS = ["rb_options_default", "rb_create", "rb_set_instances", "rb_set_tpot_forest", "rb_set_telemetry", "rb_set_state", "rb_get_state", "rb_advance_state",
            "rb_decide", "rb_decide_budgeted", "rb_decide_from_predictions", "rb_decide_from_predictions_budgeted", "rb_estimate", "rb_set_stage_timing", "rb_last_stage_us",
            "rb_launch_count", "rb_sync", "rb_last_error", "rb_destroy"]
 
@@ -43,6 +43,10 @@ class rb_lat_head(ctypes.Structure):
                 ("batch_slope", ctypes.c_float)]
 
 
+class rb_tree_node(ctypes.Structure):
+    _fields_ = [("feature", ctypes.c_int32), ("value", ctypes.c_float), ("left", ctypes.c_int32), ("right", ctypes.c_int32)]
+
+
 class RbError(RuntimeError):
     def __init__(self, status, msg):
         super().__init__("%s: %s" % (_STATUS.get(status, status), msg))
@@ -54,6 +58,8 @@ _lib.rb_options_default.argtypes = [ctypes.POINTER(rb_options)]
 _lib.rb_options_default.restype = None
 _lib.rb_create.argtypes = [ctypes.POINTER(_vp), _vp, _vp, _vp, _i64, _i32, _i32, _i32, ctypes.POINTER(rb_options)]
 _lib.rb_set_instances.argtypes = [_vp, _i32, _vp, _vp, _vp, _vp, ctypes.POINTER(rb_lat_head)]
+_lib.rb_set_tpot_forest.argtypes = [_vp, _vp, _i32, _vp, _i32, _vp, _vp, _i32]
+_lib.rb_set_telemetry.argtypes = [_vp, _vp]
 _lib.rb_set_state.argtypes = [_vp, _vp, _vp]
 _lib.rb_get_state.argtypes = [_vp, _vp, _vp]
 _lib.rb_advance_state.argtypes = [_vp, _f]
@@ -131,6 +137,23 @@ def rb_set_instances(ctx, tier, cap, price_in, price_out, heads):
     h = (rb_lat_head * len(heads))(*[rb_lat_head(*map(float, x)) for x in heads])
     _check(ctx, _lib.rb_set_instances(ctx, len(tier), tier.ctypes.data, cap.ctypes.data, pin.ctypes.data,
                                       pout.ctypes.data, h))
+
+
+def rb_set_tpot_forest(ctx, node_feature, node_value, node_left, node_right, tree_root, tier_tree_begin, base, n_features):
+    """Node arrays (four parallel sequences) are packed into rb_tree_node records."""
+    n = len(node_feature)
+    nodes = np.zeros(n, dtype=[("feature", np.int32), ("value", np.float32), ("left", np.int32), ("right", np.int32)])
+    nodes["feature"], nodes["value"], nodes["left"], nodes["right"] = node_feature, node_value, node_left, node_right
+    root = np.ascontiguousarray(tree_root, dtype=np.int32)
+    begin = np.ascontiguousarray(tier_tree_begin, dtype=np.int32)
+    b = np.ascontiguousarray(base, dtype=np.float32)
+    _check(ctx, _lib.rb_set_tpot_forest(ctx, nodes.ctypes.data, n, root.ctypes.data, len(root), begin.ctypes.data,
+                                        b.ctypes.data, int(n_features)))
+
+
+def rb_set_telemetry(ctx, aux):
+    f32 = torch.float32 if torch else np.float32
+    _check(ctx, _lib.rb_set_telemetry(ctx, _ptr(aux, f32)))
 
 
 def rb_set_state(ctx, queued_tokens, running):

@@ -59,6 +59,12 @@ struct rb_ctx {
   float *termA = nullptr, *termP = nullptr, *key = nullptr;
   int32_t *order = nullptr, *assignment = nullptr, *max_tokens = nullptr;
   float* budget = nullptr;          // [max_batch] staging of host budgets
+  // boosted TPOT head (latency_mode 2)
+  int4* f_nodes = nullptr;
+  int32_t *f_root = nullptr, *f_begin = nullptr;
+  float *f_base = nullptr, *f_aux = nullptr, *f_tpot0 = nullptr;
+  int f_features = 0;
+  bool has_forest = false;
   float *scores = nullptr, *scores0 = nullptr;  // [max_batch x I], allocated by rb_set_instances
   CUtensorMap tm_q{}, tm_bank{};
   // graphs: key = B * 4 + kind (0 decide, 1 estimate, 2 from_predictions)
@@ -112,6 +118,13 @@ DispatchModes modes_of(const rb_ctx* c) {
   m.lpt_enabled = c->opt.lpt_enabled; m.update_mode = c->opt.update_enabled; m.tiebreak_mode = c->opt.tiebreak_mode;
   m.latency_mode = c->opt.latency_mode;
   return m;
+}
+
+ForestDev forest_of(const rb_ctx* c) {
+  ForestDev f{};
+  f.nodes = c->f_nodes; f.tree_root = c->f_root; f.tier_begin = c->f_begin; f.base = c->f_base; f.aux = c->f_aux;
+  f.tpot0 = c->f_tpot0; f.n_features = c->f_features;
+  return f;
 }
 
 InstTable table_of(const rb_ctx* c) {
@@ -230,11 +243,15 @@ rb_status enqueue_dispatch(rb_ctx* ctx, int B, bool from_predictions, Timer& tm)
   cudaStream_t s = ctx->stream;
   InstTable t = table_of(ctx);
   if (from_predictions) {
-    CK(launch_score(t, ctx->dq, ctx->bq, ctx->cp, B, ctx->termA, ctx->termP, ctx->key, modes_of(ctx), s));
+    if (ctx->opt.latency_mode == 2) {
+      CK(launch_tpot_forest(t, forest_of(ctx), ctx->dq, ctx->bq, ctx->f_tpot0, -1.0f, s));
+      ctx->launches += 1;
+    }
+    CK(launch_score(t, ctx->dq, ctx->bq, ctx->cp, B, ctx->termA, ctx->termP, ctx->key, modes_of(ctx), forest_of(ctx), s));
     ctx->launches += 1;
   }
   tm.mark();
-  CK(launch_lpt_dispatch(t, ctx->dq, ctx->bq, ctx->termA, ctx->termP, ctx->key, ctx->cp, B, modes_of(ctx), s));
+  CK(launch_lpt_dispatch(t, ctx->dq, ctx->bq, ctx->termA, ctx->termP, ctx->key, ctx->cp, B, modes_of(ctx), forest_of(ctx), s));
   tm.mark();
   ctx->launches += 1;
   return RB_OK;
@@ -245,6 +262,10 @@ rb_status run_path(rb_ctx* ctx, int B, int kind) {
   const bool graph = ctx->opt.use_graph && !ctx->stage_timing;
   Timer tm(ctx);
   if (!graph) {
+    if (kind == 0 && ctx->opt.latency_mode == 2) {   // the head over the batch-start state; only the state feeds it
+      CK(launch_tpot_forest(table_of(ctx), forest_of(ctx), ctx->dq, ctx->bq, ctx->f_tpot0, -1.0f, ctx->stream));
+      ctx->launches += 1;
+    }
     if (kind != 2) {
       rb_status st = enqueue_estimate(ctx, B, kind == 0, tm);
       if (st != RB_OK) return st;
@@ -259,7 +280,12 @@ rb_status run_path(rb_ctx* ctx, int B, int kind) {
     cudaGraph_t g = nullptr;
     CK(cudaStreamBeginCapture(ctx->stream, cudaStreamCaptureModeThreadLocal));
     rb_status st = RB_OK;
-    if (kind != 2) st = enqueue_estimate(ctx, B, kind == 0, tm);
+    if (kind == 0 && ctx->opt.latency_mode == 2) {
+      if (launch_tpot_forest(table_of(ctx), forest_of(ctx), ctx->dq, ctx->bq, ctx->f_tpot0, -1.0f, ctx->stream) != cudaSuccess)
+        st = fail(ctx, RB_ECUDA, "launch_tpot_forest");
+      ctx->launches += 1;
+    }
+    if (st == RB_OK && kind != 2) st = enqueue_estimate(ctx, B, kind == 0, tm);
     if (st == RB_OK && kind != 1) st = enqueue_dispatch(ctx, B, kind == 2, tm);
     cudaError_t e = cudaStreamEndCapture(ctx->stream, &g);
     const int nodes = (int)(ctx->launches - before);
@@ -399,7 +425,7 @@ rb_status rb_create(rb_ctx** out, const void* bank_emb, const float* bank_qualit
   if (opt.weight_mode != 0 && opt.weight_mode != 1) return RB_EINVAL;
   if (opt.update_enabled < 0 || opt.update_enabled > 2) return RB_EINVAL;
   if (opt.tiebreak_mode != 0 && opt.tiebreak_mode != 1) return RB_EINVAL;
-  if (opt.latency_mode != 0 && opt.latency_mode != 1) return RB_EINVAL;
+  if (opt.latency_mode < 0 || opt.latency_mode > 2) return RB_EINVAL;
   opt.lpt_enabled = opt.lpt_enabled ? 1 : 0;
   if (opt.scan_list != 0 && opt.scan_list != 4 && opt.scan_list != 8 && opt.scan_list != 16 && opt.scan_list != 32 &&
       opt.scan_list != 64)
@@ -509,6 +535,9 @@ rb_status rb_create(rb_ctx** out, const void* bank_emb, const float* bank_qualit
   ALLOC(ctx->pre, kMaxM);
   ALLOC(ctx->dec, kMaxM);
   ALLOC(ctx->slope, kMaxM);
+  ALLOC(ctx->f_aux, (size_t)kMaxI * kMaxFeatures);
+  ALLOC(ctx->f_tpot0, kMaxI);
+  CK(cudaMemsetAsync(ctx->f_aux, 0, (size_t)kMaxI * kMaxFeatures * 4, s));
   ALLOC(ctx->dec_i, kMaxI);
   ALLOC(ctx->slope_i, kMaxI);
   if (opt.store_dtype == RB_BF16) {
@@ -589,8 +618,69 @@ rb_status rb_set_instances(rb_ctx* ctx, int32_t I, const int32_t* tier, const in
   CK(cudaMemcpyAsync(ctx->slope_i, slope_i.data(), I * 4, cudaMemcpyHostToDevice, s));
   CK(cudaMemsetAsync(ctx->dq, 0, kMaxI * 4, s));
   CK(cudaMemsetAsync(ctx->bq, 0, kMaxI * 4, s));
+  CK(cudaMemsetAsync(ctx->f_aux, 0, (size_t)kMaxI * kMaxFeatures * 4, s));
   CK(cudaStreamSynchronize(s));   // stack arrays above are read by pageable copies
   ctx->I = I;
+  return RB_OK;
+}
+
+rb_status rb_set_tpot_forest(rb_ctx* ctx, const rb_tree_node* nodes, int32_t n_nodes, const int32_t* tree_root,
+                             int32_t n_trees, const int32_t* tier_tree_begin, const float* base, int32_t n_features) {
+  if (!ctx) return RB_EINVAL;
+  if (!nodes || !tree_root || !tier_tree_begin || !base) return fail(ctx, RB_EINVAL, "NULL argument");
+  if (n_nodes < 1 || n_nodes > (1 << 22) || n_trees < 0) return fail(ctx, RB_EINVAL, "forest size out of range");
+  if (n_features < 2 || n_features > kMaxFeatures) return fail(ctx, RB_EINVAL, "n_features out of range [2,8]");
+  const int M = ctx->M;
+  if (tier_tree_begin[0] != 0 || tier_tree_begin[M] != n_trees) return fail(ctx, RB_EINVAL, "tier_tree_begin must span [0,n_trees]");
+  for (int m = 0; m < M; ++m) {
+    const int n = tier_tree_begin[m + 1] - tier_tree_begin[m];
+    if (n < 0 || n > kMaxTreesPerTier) return fail(ctx, RB_EINVAL, "trees per tier out of range [0,256]");
+    if (!std::isfinite(base[m])) return fail(ctx, RB_EINVAL, "base must be finite");
+  }
+  for (int j = 0; j < n_trees; ++j)
+    if (tree_root[j] < 0 || tree_root[j] >= n_nodes) return fail(ctx, RB_EINVAL, "tree_root out of range");
+  for (int n = 0; n < n_nodes; ++n) {
+    if (!std::isfinite(nodes[n].value)) return fail(ctx, RB_EINVAL, "node value must be finite");
+    if (nodes[n].feature < 0) continue;
+    if (nodes[n].feature >= n_features) return fail(ctx, RB_EINVAL, "node feature out of range");
+    // children after their parent: every walk is finite
+    if (nodes[n].left <= n || nodes[n].left >= n_nodes || nodes[n].right <= n || nodes[n].right >= n_nodes)
+      return fail(ctx, RB_EINVAL, "node children must lie after their parent and inside the node array");
+  }
+  cudaStream_t s = ctx->stream;
+  CK(cudaStreamSynchronize(s));
+  cudaFree(ctx->f_nodes); cudaFree(ctx->f_root); cudaFree(ctx->f_begin); cudaFree(ctx->f_base);
+  ctx->f_nodes = nullptr; ctx->f_root = ctx->f_begin = nullptr; ctx->f_base = nullptr;
+  ctx->has_forest = false;
+  static_assert(sizeof(rb_tree_node) == sizeof(int4), "rb_tree_node is read as int4");
+  if (dev_alloc(&ctx->f_nodes, (size_t)n_nodes) != cudaSuccess || dev_alloc(&ctx->f_root, (size_t)n_trees) != cudaSuccess ||
+      dev_alloc(&ctx->f_begin, (size_t)M + 1) != cudaSuccess || dev_alloc(&ctx->f_base, (size_t)M) != cudaSuccess) {
+    cudaGetLastError();
+    return fail(ctx, RB_ENOMEM, "cudaMalloc forest");
+  }
+  CK(cudaMemcpyAsync(ctx->f_nodes, nodes, (size_t)n_nodes * sizeof(rb_tree_node), cudaMemcpyHostToDevice, s));
+  CK(cudaMemcpyAsync(ctx->f_root, tree_root, (size_t)n_trees * 4, cudaMemcpyHostToDevice, s));
+  CK(cudaMemcpyAsync(ctx->f_begin, tier_tree_begin, (size_t)(M + 1) * 4, cudaMemcpyHostToDevice, s));
+  CK(cudaMemcpyAsync(ctx->f_base, base, (size_t)M * 4, cudaMemcpyHostToDevice, s));
+  CK(cudaStreamSynchronize(s));
+  if (n_features != ctx->f_features) CK(cudaMemsetAsync(ctx->f_aux, 0, (size_t)kMaxI * kMaxFeatures * 4, s));
+  ctx->f_features = n_features;
+  ctx->has_forest = true;
+  for (auto& kv : ctx->graphs) cudaGraphExecDestroy(kv.second);   // captured kernel arguments hold the old forest
+  ctx->graphs.clear();
+  ctx->graph_nodes.clear();
+  return RB_OK;
+}
+
+rb_status rb_set_telemetry(rb_ctx* ctx, const float* aux) {
+  if (!ctx) return RB_EINVAL;
+  if (ctx->I == 0) return fail(ctx, RB_ESTATE, "rb_set_telemetry before rb_set_instances");
+  if (!ctx->has_forest) return fail(ctx, RB_ESTATE, "rb_set_telemetry before rb_set_tpot_forest");
+  const int Fa = ctx->f_features - 2;
+  if (Fa == 0) return RB_OK;
+  if (!aux) return fail(ctx, RB_EINVAL, "NULL argument");
+  CK(cudaMemcpyAsync(ctx->f_aux, aux, (size_t)ctx->I * Fa * 4, cudaMemcpyDefault, ctx->stream));
+  if (is_host_ptr(aux)) CK(cudaStreamSynchronize(ctx->stream));
   return RB_OK;
 }
 
@@ -629,7 +719,12 @@ rb_status rb_advance_state(rb_ctx* ctx, float elapsed_ms) {
   if (!ctx) return RB_EINVAL;
   if (ctx->I == 0) return fail(ctx, RB_ESTATE, "rb_advance_state before rb_set_instances");
   if (!finite_nonneg(elapsed_ms)) return fail(ctx, RB_EINVAL, "elapsed_ms must be finite and >= 0");
-  CK(launch_advance(table_of(ctx), ctx->dq, ctx->bq, elapsed_ms, ctx->stream));
+  if (ctx->opt.latency_mode == 2) {
+    if (!ctx->has_forest) return fail(ctx, RB_ESTATE, "latency_mode 2 needs rb_set_tpot_forest first");
+    CK(launch_tpot_forest(table_of(ctx), forest_of(ctx), ctx->dq, ctx->bq, nullptr, elapsed_ms, ctx->stream));
+  } else {
+    CK(launch_advance(table_of(ctx), ctx->dq, ctx->bq, elapsed_ms, ctx->stream));
+  }
   ctx->launches += 1;
   return RB_OK;
 }
@@ -646,6 +741,7 @@ rb_status rb_decide_budgeted(rb_ctx* ctx, const float* query_emb, const int32_t*
                              float* pred_quality, float* pred_outlen, int32_t* nn_idx, float* nn_sim) {
   if (!ctx) return RB_EINVAL;
   if (ctx->I == 0) return fail(ctx, RB_ESTATE, "rb_decide before rb_set_instances");
+  if (ctx->opt.latency_mode == 2 && !ctx->has_forest) return fail(ctx, RB_ESTATE, "latency_mode 2 needs rb_set_tpot_forest first");
   if (!query_emb || !prompt_len || !assignment) return fail(ctx, RB_EINVAL, "NULL argument");
   if (B < 1 || B > ctx->opt.max_batch) return fail(ctx, RB_EINVAL, "B out of range [1,max_batch]");
   rb_status st = check_weights(ctx, w);
@@ -710,6 +806,7 @@ rb_status rb_decide_from_predictions_budgeted(rb_ctx* ctx, const float* quality,
                                               float* scores0, int32_t* order) {
   if (!ctx) return RB_EINVAL;
   if (ctx->I == 0) return fail(ctx, RB_ESTATE, "rb_decide_from_predictions before rb_set_instances");
+  if (ctx->opt.latency_mode == 2 && !ctx->has_forest) return fail(ctx, RB_ESTATE, "latency_mode 2 needs rb_set_tpot_forest first");
   if (!quality || !outlen || !prompt_len || !assignment) return fail(ctx, RB_EINVAL, "NULL argument");
   if (B < 1 || B > ctx->opt.max_batch) return fail(ctx, RB_EINVAL, "B out of range [1,max_batch]");
   rb_status st = check_weights(ctx, w);
@@ -766,7 +863,8 @@ void rb_destroy(rb_ctx* ctx) {
                   ctx->price_out, ctx->pre, ctx->dec, ctx->slope, ctx->dec_i, ctx->slope_i, ctx->dq, ctx->bq, ctx->q32, ctx->qs, ctx->plen, ctx->cp,
                   ctx->part_sim, ctx->part_idx, ctx->gthr, ctx->sims, ctx->cand_sim, ctx->cand_idx, ctx->scratch_nn_idx, ctx->scratch_nn_sim, ctx->stage_q, ctx->stage_l,
                   ctx->pred_q, ctx->pred_l, ctx->termA, ctx->termP, ctx->key, ctx->order, ctx->assignment, ctx->scores,
-                  ctx->scores0, ctx->max_tokens, ctx->budget};
+                  ctx->scores0, ctx->max_tokens, ctx->budget, ctx->f_nodes, ctx->f_root, ctx->f_begin, ctx->f_base, ctx->f_aux,
+                  ctx->f_tpot0};
   for (void* p : ptrs) cudaFree(p);
   for (auto& e : ctx->ev)
     if (e) cudaEventDestroy(e);

@@ -30,6 +30,19 @@ struct InstTable {
   const float* slope_i;    // [I] slope[tier[i]]
 };
 
+// Gradient-boosted TPOT head (reading 9b) as the kernels see it (device memory).
+constexpr int kMaxTreesPerTier = 256;
+constexpr int kMaxFeatures = 8;
+struct ForestDev {
+  const int4* nodes;           // (feature, value bits, left, right); feature < 0: leaf
+  const int32_t* tree_root;    // [n_trees]
+  const int32_t* tier_begin;   // [M+1]
+  const float* base;           // [M]
+  const float* aux;            // [I x (F-2)] auxiliary telemetry features
+  const float* tpot0;          // [I] head evaluated on the batch-start state (tpot_kernel)
+  int32_t n_features;
+};
+
 // Per-call parameters live in device memory so that a captured graph can be replayed with new weights and new
 // caller buffers.  Every pointer is a DEVICE pointer: the caller's own buffer, or the context's staging buffer
 // when the caller passed host memory.  Optional outputs are NULL when not wanted.
@@ -57,8 +70,22 @@ struct DispatchModes {
   int32_t lpt_enabled;     // 1: LPT order; 0: input order
   int32_t update_mode;     // 0: none; 1: d += L^ and b = min(b+1, cap) (default); 2: d only (P:L121 literally)
   int32_t tiebreak_mode;   // 0: (S desc, d asc, i asc) reactive shortest queue; 1: (S desc, T^ asc, i asc) predictive
-  int32_t latency_mode;    // 0: live head over the dead-reckoned state; 1: static prior T^ = dec * L^ (arm 4)
+  int32_t latency_mode;    // 0: live linear head over the dead-reckoned state; 1: static prior T^ = dec * L^ (arm 4);
+                           // 2: live gradient-boosted head (ForestDev)
 };
+
+#ifdef __CUDACC__
+// Leaf of one tree for the features (x0 = running, x1 = queued tokens, x2.. = aux): XGBoost's rule, left iff x < threshold.
+__device__ __forceinline__ float forest_leaf(const int4* __restrict__ nodes, int root, float xb, float xd,
+                                             const float* __restrict__ aux_i) {
+  int4 nd = __ldg(&nodes[root]);
+  while (nd.x >= 0) {
+    const float x = nd.x == 0 ? xb : (nd.x == 1 ? xd : __ldg(&aux_i[nd.x - 2]));
+    nd = __ldg(&nodes[(x < __int_as_float(nd.y)) ? nd.z : nd.w]);
+  }
+  return __int_as_float(nd.y);
+}
+#endif
 
 // ---- programmatic dependent launch ---------------------------------------------------------------------------
 // Consecutive kernels of one decision are chained with programmatic stream serialization: a kernel lets its
@@ -191,13 +218,20 @@ cudaError_t finish_prepare(size_t max_smem);
 // a4+a5 from caller-supplied predictions (cp->q_src, cp->l_src): per-(request, tier) terms, LPT keys and the
 // batch-start score matrix (cp->scores0 when non-NULL).
 cudaError_t launch_score(InstTable t, const float* dq, const int32_t* bq, const CallParams* cp, int B, float* termA,
-                         float* termP, float* key, DispatchModes modes, cudaStream_t s);
+                         float* termP, float* key, DispatchModes modes, ForestDev forest, cudaStream_t s);
 
 // a6+a7: LPT sort + greedy dispatch with dead-reckoned updates, one CTA.
 cudaError_t launch_lpt_dispatch(InstTable t, float* dq, int32_t* bq, const float* termA, const float* termP,
-                                const float* key, const CallParams* cp, int B, DispatchModes modes, cudaStream_t s);
+                                const float* key, const CallParams* cp, int B, DispatchModes modes, ForestDev forest,
+                                cudaStream_t s);
 
 cudaError_t lpt_dispatch_prepare();  // opt in to the dynamic shared memory size; call once
+
+// Boosted head over the current state: tpot_out[i] = max(base + sum of leaves (fp32, tree order), 1e-6) for every
+// instance (one CTA per instance, one thread per tree, sequential sum by thread 0).  elapsed_ms >= 0: also applies
+// the a8 drain rule with that tpot (rb_advance_state under latency_mode 2).
+cudaError_t launch_tpot_forest(InstTable t, ForestDev forest, float* dq, int32_t* bq, float* tpot_out, float elapsed_ms,
+                               cudaStream_t s);
 
 // a8: dead reckoning between batches.
 cudaError_t launch_advance(InstTable t, float* dq, int32_t* bq, float elapsed_ms, cudaStream_t s);

@@ -50,6 +50,13 @@ class Router:
         rb.rb_set_instances(self.ctx, tier, cap, price_in, price_out, list(zip(pre, dec, slope)))
         self.I = len(tier)
 
+    def set_tpot_forest(self, node_feature, node_value, node_left, node_right, tree_root, tier_tree_begin, base,
+                        n_features, aux=None):
+        rb.rb_set_tpot_forest(self.ctx, node_feature, node_value, node_left, node_right, tree_root, tier_tree_begin, base,
+                              n_features)
+        if aux is not None:
+            rb.rb_set_telemetry(self.ctx, aux.contiguous().float())
+
     def set_state(self, queued, running):
         rb.rb_set_state(self.ctx, queued.contiguous().float(), running.contiguous().to(torch.int32))
 

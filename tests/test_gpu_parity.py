@@ -442,3 +442,72 @@ def test_decide_budgeted_full_path(orc):
     assert np.array_equal(g0["assignment"], g1["assignment"]) and np.array_equal(g0["scores"], g1["scores"])
     assert (g1["max_tokens"] == 2**31 - 1).all()
     rt.close()
+
+
+def _forest_pair(orc, it, I, M, n_trees, depth, Fa, seed):
+    fd = synth.make_forest(M, it["dec"], n_trees=n_trees, depth=depth, Fa=Fa, seed=seed, I=I)
+    aux = fd.pop("aux")
+    of = orc.Forest(aux=None if aux is None else aux.numpy(), **fd)
+    return fd, aux, of
+
+
+@pytest.mark.parametrize("I,M,B,n_trees,depth,Fa", [(13, 4, 16, 32, 4, 2), (64, 4, 200, 100, 5, 3), (256, 8, 1024, 16, 3, 0),
+                                                    (33, 3, 50, 256, 2, 6), (5, 2, 9, 1, 0, 1)])
+@pytest.mark.parametrize("upd,tb", [(1, 0), (2, 1)])
+def test_boosted_tpot_head_bit_exact(orc, I, M, B, n_trees, depth, Fa, upd, tb):
+    """latency_mode 2 -- per-tier gradient-boosted TPOT head over (running, queued, aux telemetry),
+    re-evaluated for the chosen instance after every dispatch; scores0/scores/assignment/state and the between-batch
+    drain bit-exact against orc_dispatch_gbdt / orc_advance_state_gbdt, with and without budgets."""
+    from paper_2606_17949_b200.router import Router
+    rng = np.random.default_rng(11 * I + B + upd)
+    it = synth.make_instances(I, M, cap=int(rng.integers(2, 9)))
+    fd, aux, of = _forest_pair(orc, it, I, M, n_trees, depth, Fa, seed=I + B)
+    bank = dict(emb=torch.randn(64, 16), quality=torch.rand(64, M), outlen=torch.rand(64, M) * 100 + 1)
+    rt = Router(bank["emb"].cuda(), bank["quality"].cuda(), bank["outlen"].cuda(), 4, store="f32", max_batch=B,
+                update_enabled=upd, tiebreak_mode=tb, latency_mode=2)
+    rt.set_instances(**it)
+    with pytest.raises(Exception):
+        rt.decide_from_predictions(torch.rand(B, M).cuda(), torch.rand(B, M).cuda(), torch.ones(B, dtype=torch.int32).cuda(),
+                                   synth.PRESETS["balanced"])       # RB_ESTATE: no forest yet
+    rt.set_tpot_forest(aux=None if aux is None else aux.cuda(), **fd)
+    queued = rng.integers(0, 20001, I).astype(np.float32)
+    running = np.minimum(rng.integers(0, 12, I), it["cap"]).astype(np.int32)
+    Q = rng.uniform(0, 1, (B, M)).astype(np.float32)
+    L = rng.lognormal(5.5, 0.7, (B, M)).astype(np.float32)
+    plen = rng.integers(1, 4000, B).astype(np.int32)
+    bud = _random_budgets(rng, it, L, plen)
+    inst = orc.Instances(**it)
+    for w in [synth.PRESETS["balanced"], synth.PRESETS["latency"], (0.0, 1.0, 0.0)]:
+        for budget in (None, bud):
+            rt.set_state(torch.from_numpy(queued), torch.from_numpy(running))
+            rt.advance_state(41.5)
+            dq, bq = orc.advance_state_gbdt(inst, of, queued, running, np.float32(41.5))
+            g = _np(rt.decide_from_predictions(torch.from_numpy(Q).cuda(), torch.from_numpy(L).cuda(),
+                                               torch.from_numpy(plen).cuda(), w, commit=1,
+                                               budget=None if budget is None else torch.from_numpy(budget).cuda()))
+            ref = orc.dispatch(inst, dq, bq, Q, L, plen, w, budget=budget, update_mode=upd, tiebreak_mode=tb,
+                               latency_mode=2, forest=of)
+            for key in ("assignment", "order", "scores", "scores0"):
+                assert np.array_equal(g[key], ref[key]), (key, w, budget is None)
+            s = rt.get_state()
+            assert np.array_equal(s[0].numpy(), ref["queued"]) and np.array_equal(s[1].numpy(), ref["running"])
+    rt.close()
+
+
+def test_boosted_head_full_decide_path(orc):
+    """rb_decide under latency_mode 2 (graph replay: tpot kernel -> stage -> scan -> finish -> dispatch)."""
+    cfg = dataclasses.replace(synth.CONFIGS["C2"], N=20000, d=128, B=40, Kc=16, seed=22)
+    bank, it, queued, running, query, plen, rt = _setup(cfg, max_batch=64, latency_mode=2)
+    fd, aux, of = _forest_pair(orc, it, cfg.I, cfg.M, 48, 4, 2, seed=5)
+    rt.set_tpot_forest(aux=aux.cuda(), **fd)
+    inst = orc.Instances(**it)
+    w = synth.PRESETS["latency"]
+    for _ in range(2):
+        rt.set_state(queued, running)
+        g = _np(rt.decide(query, plen, w))
+    ref = orc.dispatch(inst, queued.numpy(), running.numpy(), g["pred_quality"], g["pred_outlen"], plen.cpu().numpy(), w,
+                       latency_mode=2, forest=of)
+    assert np.array_equal(g["assignment"], ref["assignment"]) and np.array_equal(g["scores"], ref["scores"])
+    s = rt.get_state()
+    assert np.array_equal(s[0].numpy(), ref["queued"]) and np.array_equal(s[1].numpy(), ref["running"])
+    rt.close()
