@@ -213,6 +213,11 @@ rb_status rb_estimate(rb_ctx* ctx, const float* query_emb, int32_t B, float* pre
 rb_status rb_set_stage_timing(rb_ctx* ctx, int32_t enabled);
 rb_status rb_last_stage_us(rb_ctx* ctx, float us[6]);
 
+/* Self-test of the dispatch kernel's branch-free fp32 division (reciprocal refinement without the compiler's range check;
+ * used only for operands inside the exponent window where it is exact, IEEE __fdiv_rn otherwise): compares it with the
+ * IEEE division bit for bit on n_pairs pseudo-random in-window operand pairs.  *mismatches [host] must come back 0. */
+rb_status rb_selftest_division(rb_ctx* ctx, uint64_t n_pairs, uint64_t seed, uint64_t* mismatches);
+
 /* Number of kernel launches (graph nodes count individually) issued by this context so far. */
 int64_t rb_launch_count(const rb_ctx* ctx);
 

@@ -38,6 +38,7 @@ __device__ __forceinline__ unsigned long long make_key(float sim, int32_t idx) {
 __global__ void stage_queries_kernel(const CallParams* __restrict__ cp, __nv_bfloat16* __restrict__ qs, int B, int Bpad,
                                      int d, int group, uint32_t* __restrict__ gthr, int n_gthr) {
   launch_dependents();
+  RB_TL_INIT(cp);
   for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n_gthr; i += gridDim.x * blockDim.x) gthr[i] = 0u;
   const float* __restrict__ q = cp->query;
   const size_t n = (size_t)Bpad * d;
@@ -46,6 +47,7 @@ __global__ void stage_queries_kernel(const CallParams* __restrict__ cp, __nv_bfl
     const size_t r = row % group;   // replicas of query r at rows r, group + r, ...
     qs[i] = (r < (size_t)B) ? __float2bfloat16_rn(q[r * d + c]) : __float2bfloat16_rn(0.0f);
   }
+  RB_TL_FLUSH(cp, 0, 1);
 }
 __global__ void convert_bf16_kernel(const float* __restrict__ in, __nv_bfloat16* __restrict__ out, size_t n) {
   for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x)
@@ -264,24 +266,66 @@ finish_kernel(FinishArgs a, InstTable t, const CallParams* __restrict__ cp) {
     has_budget = cp->budget != nullptr;
     if (has_budget) c_budget = cp->budget[r];
   }
+  const int c_present = (a.with_terms && tid < a.M) ? t.present[tid] : 0;
+  // caller-side output pointers and weights: read once, up front (every later use would be an L2 round trip)
+  float* const out_pq = cp->pred_q;
+  float* const out_pl = cp->pred_l;
+  int32_t* const out_nn_idx = cp->nn_idx;
+  float* const out_nn_sim = cp->nn_sim;
+  const float c_wq = cp->w_qual, c_wc = cp->w_cost;
   const int kc = a.kc, k = a.k, kcap = a.kcap, M = a.M;
   const uint4* qrow = reinterpret_cast<const uint4*>(a.qs + (size_t)r * a.d);
   const int nvec = a.d / 8;   // d % 8 == 0
 
   RB_FT(0);
+  RB_TL_INIT(cp);
+  RB_TL(cp, 34);
   // ---- merge ----
   const int total = a.nlists * kcap;
-  if (tid == 0) s_nflag = 0;
   launch_dependents();
   grid_dependency_wait();   // the partial lists come from the preceding kernel
-  for (int e = tid; e < total; e += kFinThreads) {
-    const int c = e / kcap, j = e - c * kcap;
-    const size_t off = ((size_t)c * a.Bpad + r) * kcap + j;
-    const int32_t id = a.part_idx[off];
-    s_keys[e] = (id >= 0 && (int64_t)id < a.N) ? make_key(a.part_sim[off], id) : 0ull;
+  if (tid == 0) s_nflag = 0;
+  RB_TL(cp, 36);
+  if (kcap & 3) {   // fp32-storage path: one already-merged list of kc entries per query
+    for (int e = tid; e < total; e += kFinThreads) {
+      const int c = e / kcap, j = e - c * kcap;
+      const size_t off = ((size_t)c * a.Bpad + r) * kcap + j;
+      const int32_t id = a.part_idx[off];
+      s_keys[e] = (id >= 0 && (int64_t)id < a.N) ? make_key(a.part_sim[off], id) : 0ull;
+    }
+  } else {
+    // a list's kcap entries are contiguous (kcap is a multiple of 4): one 16-byte load of similarities and one of
+    // indices per (list, quad); two quads in flight per thread
+    const int q4 = kcap >> 2, nquads = a.nlists * q4;
+    for (int e0 = tid; e0 < nquads; e0 += 2 * kFinThreads) {
+      float4 sv[2];
+      int4 iv[2];
+#pragma unroll
+      for (int u = 0; u < 2; ++u) {
+        const int e = e0 + u * kFinThreads;
+        if (e < nquads) {
+          const int c = e / q4, j4 = e - c * q4;
+          const size_t off = ((size_t)c * a.Bpad + r) * kcap + 4 * j4;
+          sv[u] = __ldcg(reinterpret_cast<const float4*>(a.part_sim + off));
+          iv[u] = __ldcg(reinterpret_cast<const int4*>(a.part_idx + off));
+        }
+      }
+#pragma unroll
+      for (int u = 0; u < 2; ++u) {
+        const int e = e0 + u * kFinThreads;
+        if (e < nquads) {
+          const float sx[4] = {sv[u].x, sv[u].y, sv[u].z, sv[u].w};
+          const int32_t ix[4] = {iv[u].x, iv[u].y, iv[u].z, iv[u].w};
+#pragma unroll
+          for (int h = 0; h < 4; ++h)
+            s_keys[4 * e + h] = (ix[h] >= 0 && (int64_t)ix[h] < a.N) ? make_key(sx[h], ix[h]) : 0ull;
+        }
+      }
+    }
   }
   __syncthreads();
   RB_FT(1);
+  RB_TL(cp, 38);
   // two levels, no barrier inside either: every warp pops the kc best of its own share of the lists (lane = list),
   // then warp 0 pops the kc best of the warps' results (lane = warp)
   unsigned long long* w_key = s_keys + total;                         // [nwarps][kMerge2Stride]
@@ -295,6 +339,7 @@ finish_kernel(FinishArgs a, InstTable t, const CallParams* __restrict__ cp) {
   }
   __syncthreads();
   RB_FT(2);
+  RB_TL(cp, 40);
   if (warp == 0) {
     // out_src of this level is the warp whose list the key came from; its position in that list is the number
     // of keys already taken from it, which recovers the original list index
@@ -318,6 +363,7 @@ finish_kernel(FinishArgs a, InstTable t, const CallParams* __restrict__ cp) {
   __syncthreads();
 
   RB_FT(3);
+  RB_TL(cp, 42);
   // ---- rescan of slabs whose list was popped completely ----
   // (a list of kcap entries all of which are among the kc best may hide further members)
   bool flagged = false;
@@ -394,6 +440,7 @@ finish_kernel(FinishArgs a, InstTable t, const CallParams* __restrict__ cp) {
   __syncthreads();
 
   RB_FT(4);
+  RB_TL(cp, 44);
   // labels of all kc candidates are requested before the re-rank and parked after it (independent gathers)
   float lv[4];
   const int nlab = kc * 2 * M;   // <= 64 * 32 = 4 * 512
@@ -408,6 +455,7 @@ finish_kernel(FinishArgs a, InstTable t, const CallParams* __restrict__ cp) {
     }
   }
   RB_FT(5);
+  RB_TL(cp, 46);
   // ---- exact re-rank ----
   if (a.rerank) {
     for (int c = warp; c < kc; c += nwarps) {
@@ -419,6 +467,7 @@ finish_kernel(FinishArgs a, InstTable t, const CallParams* __restrict__ cp) {
     __syncthreads();
   }
   RB_FT(6);
+  RB_TL(cp, 48);
   // rank by counting (keys are distinct because indices are)
   if (tid < kc) {
     const int32_t id = s_idx[tid];
@@ -440,6 +489,7 @@ finish_kernel(FinishArgs a, InstTable t, const CallParams* __restrict__ cp) {
   }
   __syncthreads();
   RB_FT(7);
+  RB_TL(cp, 50);
   // ---- weights ----
   if (tid < k) {
     const float s = o_sim[tid];
@@ -454,11 +504,12 @@ finish_kernel(FinishArgs a, InstTable t, const CallParams* __restrict__ cp) {
       w = __fdiv_rn(1.0f, __fadd_rn(dist, a.eps));
     }
     s_w[tid] = w;
-    if (cp->nn_idx) cp->nn_idx[(size_t)r * k + tid] = o_idx[tid];
-    if (cp->nn_sim) cp->nn_sim[(size_t)r * k + tid] = s;
+    if (out_nn_idx) out_nn_idx[(size_t)r * k + tid] = o_idx[tid];
+    if (out_nn_sim) out_nn_sim[(size_t)r * k + tid] = s;
   }
   __syncthreads();
   RB_FT(8);
+  RB_TL(cp, 52);
   // ---- aggregate: thread m < M -> quality, M <= thread < 2M -> output length ----
   if (tid < 2 * M) {
     const int m = tid % M;
@@ -474,15 +525,17 @@ finish_kernel(FinishArgs a, InstTable t, const CallParams* __restrict__ cp) {
     if (tid < M) {
       sQ[m] = pred;
       a.pred_q[(size_t)r * M + m] = pred;
-      if (cp->pred_q) cp->pred_q[(size_t)r * M + m] = pred;
+      if (out_pq) out_pq[(size_t)r * M + m] = pred;
     } else {
       sL[m] = pred;
       a.pred_l[(size_t)r * M + m] = pred;
-      if (cp->pred_l) cp->pred_l[(size_t)r * M + m] = pred;
+      if (out_pl) out_pl[(size_t)r * M + m] = pred;
     }
   }
   RB_FT(9);
+  RB_TL(cp, 54);
   if (!a.with_terms) return;
+  const uint32_t present = __ballot_sync(0xffffffffu, c_present != 0);   // warp 0's ballot covers tiers 0..M-1
   __syncthreads();
   // ---- per-(request, tier) terms ----
   if (tid < M) sC[tid] = __fadd_rn(__fmul_rn(c_ell, c_pin), __fmul_rn(sL[tid], c_pout));
@@ -490,12 +543,14 @@ finish_kernel(FinishArgs a, InstTable t, const CallParams* __restrict__ cp) {
   if (tid < M) {
     const int m = tid;
     float kmax;
-    const float A = tier_term_A(m, M, t.present, sC, sL, sQ[m], cp->w_qual, cp->w_cost, has_budget, c_budget, &kmax);
+    const float A = tier_term_A(m, M, present, sC, sL, sQ[m], c_wq, c_wc, has_budget, c_budget, &kmax);
     a.termA[(size_t)r * M + m] = A;
     a.termP[(size_t)r * M + m] = __fmul_rn(c_pre, c_ell);
     if (m == 0) a.key[r] = kmax;
   }
   RB_FT(10);
+  RB_TL(cp, 35);
+  RB_TL_FLUSH(cp, 32, 33);
 }
 
 }  // namespace

@@ -43,6 +43,9 @@ struct rb_ctx {
   __nv_bfloat16* qs = nullptr;      // [Bpad_max x d]
   int32_t* plen = nullptr;          // [max_batch]
   CallParams* cp = nullptr;
+#ifdef RB_TRACE
+  unsigned long long* timeline = nullptr;
+#endif
   CallParams* cp_ring = nullptr;    // pinned host ring feeding cp; slot reuse is guarded by cp_ev
   cudaEvent_t cp_ev[64]{};
   uint64_t cp_seq = 0;
@@ -59,6 +62,7 @@ struct rb_ctx {
   float *termA = nullptr, *termP = nullptr, *key = nullptr;
   int32_t *order = nullptr, *assignment = nullptr, *max_tokens = nullptr;
   float* budget = nullptr;          // [max_batch] staging of host budgets
+  uint8_t* arena = nullptr;         // one allocation behind all the small per-decision buffers
   // boosted TPOT head (latency_mode 2)
   int4* f_nodes = nullptr;
   int32_t *f_root = nullptr, *f_begin = nullptr;
@@ -334,6 +338,10 @@ rb_status push_params(rb_ctx* ctx, const CallParams& cp) {
   const int slot = (int)(ctx->cp_seq % 64);
   if (ctx->cp_seq >= 64) CK(cudaEventSynchronize(ctx->cp_ev[slot]));
   ctx->cp_ring[slot] = cp;
+#ifdef RB_TRACE
+  if (!ctx->timeline) CK(cudaMalloc((void**)&ctx->timeline, 128 * 8));
+  ctx->cp_ring[slot].timeline = ctx->timeline;
+#endif
   CK(cudaMemcpyAsync(ctx->cp, &ctx->cp_ring[slot], sizeof cp, cudaMemcpyHostToDevice, ctx->stream));
   CK(cudaEventRecord(ctx->cp_ev[slot], ctx->stream));
   ctx->cp_seq++;
@@ -510,36 +518,34 @@ rb_status rb_create(rb_ctx** out, const void* bank_emb, const float* bank_qualit
 
   const size_t mb = opt.max_batch;
   ALLOC(ctx->q32, mb * d);
-  ALLOC(ctx->plen, mb);
-  ALLOC(ctx->cp, 1);
-  ALLOC(ctx->cand_sim, mb * ctx->kc);
-  ALLOC(ctx->cand_idx, mb * ctx->kc);
-  ALLOC(ctx->pred_q, mb * M);
-  ALLOC(ctx->pred_l, mb * M);
-  ALLOC(ctx->stage_q, mb * M);
-  ALLOC(ctx->stage_l, mb * M);
-  ALLOC(ctx->termA, mb * M);
-  ALLOC(ctx->termP, mb * M);
-  ALLOC(ctx->key, mb);
-  ALLOC(ctx->order, mb);
-  ALLOC(ctx->assignment, mb);
-  ALLOC(ctx->max_tokens, mb);
-  ALLOC(ctx->budget, mb);
-  ALLOC(ctx->tier, kMaxI);
-  ALLOC(ctx->cap, kMaxI);
-  ALLOC(ctx->dq, kMaxI);
-  ALLOC(ctx->bq, kMaxI);
-  ALLOC(ctx->present, kMaxM);
-  ALLOC(ctx->price_in, kMaxM);
-  ALLOC(ctx->price_out, kMaxM);
-  ALLOC(ctx->pre, kMaxM);
-  ALLOC(ctx->dec, kMaxM);
-  ALLOC(ctx->slope, kMaxM);
-  ALLOC(ctx->f_aux, (size_t)kMaxI * kMaxFeatures);
-  ALLOC(ctx->f_tpot0, kMaxI);
-  CK(cudaMemsetAsync(ctx->f_aux, 0, (size_t)kMaxI * kMaxFeatures * 4, s));
-  ALLOC(ctx->dec_i, kMaxI);
-  ALLOC(ctx->slope_i, kMaxI);
+  // Everything a decision's latency-bound kernels touch (per-call parameters, instance table, state, per-request
+  // terms and outputs) lives in ONE allocation, packed: a cold kernel then pays for one or two TLB misses instead
+  // of one per buffer.
+  {
+    size_t off = 0;
+    auto take = [&](size_t bytes) { const size_t o = off; off = (off + bytes + 255) & ~(size_t)255; return o; };
+    const size_t o_cp = take(sizeof(CallParams)), o_plen = take(mb * 4), o_csim = take(mb * ctx->kc * 4),
+                 o_cidx = take(mb * ctx->kc * 4), o_pq = take(mb * M * 4), o_pl = take(mb * M * 4), o_sq = take(mb * M * 4),
+                 o_sl = take(mb * M * 4), o_ta = take(mb * M * 4), o_tp = take(mb * M * 4), o_key = take(mb * 4),
+                 o_ord = take(mb * 4), o_asg = take(mb * 4), o_mt = take(mb * 4), o_bud = take(mb * 4),
+                 o_tier = take(kMaxI * 4), o_cap = take(kMaxI * 4), o_dq = take(kMaxI * 4), o_bq = take(kMaxI * 4),
+                 o_pres = take(kMaxM * 4), o_pin = take(kMaxM * 4), o_pout = take(kMaxM * 4), o_pre = take(kMaxM * 4),
+                 o_dec = take(kMaxM * 4), o_slope = take(kMaxM * 4), o_deci = take(kMaxI * 4), o_slopei = take(kMaxI * 4),
+                 o_aux = take((size_t)kMaxI * kMaxFeatures * 4), o_tpot0 = take(kMaxI * 4);
+    ALLOC(ctx->arena, off);
+    uint8_t* a = ctx->arena;
+    ctx->cp = (CallParams*)(a + o_cp); ctx->plen = (int32_t*)(a + o_plen); ctx->cand_sim = (float*)(a + o_csim);
+    ctx->cand_idx = (int32_t*)(a + o_cidx); ctx->pred_q = (float*)(a + o_pq); ctx->pred_l = (float*)(a + o_pl);
+    ctx->stage_q = (float*)(a + o_sq); ctx->stage_l = (float*)(a + o_sl); ctx->termA = (float*)(a + o_ta);
+    ctx->termP = (float*)(a + o_tp); ctx->key = (float*)(a + o_key); ctx->order = (int32_t*)(a + o_ord);
+    ctx->assignment = (int32_t*)(a + o_asg); ctx->max_tokens = (int32_t*)(a + o_mt); ctx->budget = (float*)(a + o_bud);
+    ctx->tier = (int32_t*)(a + o_tier); ctx->cap = (int32_t*)(a + o_cap); ctx->dq = (float*)(a + o_dq);
+    ctx->bq = (int32_t*)(a + o_bq); ctx->present = (int32_t*)(a + o_pres); ctx->price_in = (float*)(a + o_pin);
+    ctx->price_out = (float*)(a + o_pout); ctx->pre = (float*)(a + o_pre); ctx->dec = (float*)(a + o_dec);
+    ctx->slope = (float*)(a + o_slope); ctx->dec_i = (float*)(a + o_deci); ctx->slope_i = (float*)(a + o_slopei);
+    ctx->f_aux = (float*)(a + o_aux); ctx->f_tpot0 = (float*)(a + o_tpot0);
+    CK(cudaMemsetAsync(ctx->arena, 0, off, s));
+  }
   if (opt.store_dtype == RB_BF16) {
     ALLOC(ctx->qs, (size_t)ctx->Bpad_max * d);
     ALLOC(ctx->gthr, (size_t)ctx->Bpad_max * (2 + ctx->num_sms / 2));
@@ -845,6 +851,35 @@ rb_status rb_last_stage_us(rb_ctx* ctx, float us[6]) {
   return RB_OK;
 }
 
+#ifdef RB_TRACE
+int rb_debug_timeline(rb_ctx* ctx, unsigned long long* out, int reset) {
+  cudaStreamSynchronize(ctx->stream);
+  if (!ctx->timeline) cudaMalloc((void**)&ctx->timeline, 128 * 8);
+  cudaMemcpy(out, ctx->timeline, 128 * 8, cudaMemcpyDeviceToHost);
+  if (reset) {
+    unsigned long long init[128];
+    for (int j = 0; j < 128; ++j) init[j] = (j & 1) ? 0ull : ~0ull;
+    cudaMemcpy(ctx->timeline, init, sizeof init, cudaMemcpyHostToDevice);
+  }
+  return 0;
+}
+#endif
+
+rb_status rb_selftest_division(rb_ctx* ctx, uint64_t n_pairs, uint64_t seed, uint64_t* mismatches) {
+  if (!ctx || !mismatches) return RB_EINVAL;
+  unsigned long long* dcount = nullptr;
+  CK(cudaMalloc((void**)&dcount, 8));
+  cudaError_t e = cudaMemsetAsync(dcount, 0, 8, ctx->stream);
+  if (e == cudaSuccess) e = launch_div_selftest(n_pairs, seed, dcount, ctx->stream);
+  unsigned long long h = 0;
+  if (e == cudaSuccess) e = cudaMemcpyAsync(&h, dcount, 8, cudaMemcpyDeviceToHost, ctx->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+  cudaFree(dcount);
+  if (e != cudaSuccess) return fail(ctx, RB_ECUDA, "rb_selftest_division", e);
+  *mismatches = h;
+  return RB_OK;
+}
+
 int64_t rb_launch_count(const rb_ctx* ctx) { return ctx ? ctx->launches : 0; }
 
 rb_status rb_sync(rb_ctx* ctx) {
@@ -859,12 +894,9 @@ void rb_destroy(rb_ctx* ctx) {
   if (!ctx) return;
   if (ctx->stream) cudaStreamSynchronize(ctx->stream);
   for (auto& kv : ctx->graphs) cudaGraphExecDestroy(kv.second);
-  void* ptrs[] = {ctx->bank, ctx->bank_quality, ctx->bank_outlen, ctx->tier, ctx->cap, ctx->present, ctx->price_in,
-                  ctx->price_out, ctx->pre, ctx->dec, ctx->slope, ctx->dec_i, ctx->slope_i, ctx->dq, ctx->bq, ctx->q32, ctx->qs, ctx->plen, ctx->cp,
-                  ctx->part_sim, ctx->part_idx, ctx->gthr, ctx->sims, ctx->cand_sim, ctx->cand_idx, ctx->scratch_nn_idx, ctx->scratch_nn_sim, ctx->stage_q, ctx->stage_l,
-                  ctx->pred_q, ctx->pred_l, ctx->termA, ctx->termP, ctx->key, ctx->order, ctx->assignment, ctx->scores,
-                  ctx->scores0, ctx->max_tokens, ctx->budget, ctx->f_nodes, ctx->f_root, ctx->f_begin, ctx->f_base, ctx->f_aux,
-                  ctx->f_tpot0};
+  void* ptrs[] = {ctx->bank, ctx->bank_quality, ctx->bank_outlen, ctx->arena, ctx->q32, ctx->qs, ctx->part_sim, ctx->part_idx,
+                  ctx->gthr, ctx->sims, ctx->scratch_nn_idx, ctx->scratch_nn_sim, ctx->scores, ctx->scores0, ctx->f_nodes,
+                  ctx->f_root, ctx->f_begin, ctx->f_base};
   for (void* p : ptrs) cudaFree(p);
   for (auto& e : ctx->ev)
     if (e) cudaEventDestroy(e);

@@ -63,6 +63,9 @@ struct CallParams {
   float* nn_sim;
   const float* budget;     // [B] per-request cost budgets (Eq. 2) or NULL: no admission filter
   int32_t* max_tokens;     // [B] or NULL: output-token clamp of the chosen instance
+#ifdef RB_TRACE
+  unsigned long long* timeline;   // development aid: [128] globaltimer stamps (even slots: earliest, odd: latest), then block 0's clock64 per slot
+#endif
 };
 
 // Dispatch modes (rb_options; SURVEY 8(f) #2, P:L227 isolation arms, P:L266 ablations).
@@ -93,6 +96,26 @@ __device__ __forceinline__ float forest_leaf(const int4* __restrict__ nodes, int
 // with it, and waits (grid_dependency_wait) before it touches anything its predecessor produces.  Both are
 // no-ops for a kernel launched without the attribute.
 #ifdef __CUDACC__
+#ifdef RB_TRACE   // development aid (_work harness): kernel/phase timestamps of one decision; compiled out otherwise
+// Thread 0 of every block keeps clock64 stamps in registers/shared memory (cheap); RB_TL_FLUSH writes block 0's
+// stamps to timeline[64 + slot] and one globaltimer pair (first slot: earliest over blocks, last: latest).
+struct TlBuf { long long c[32]; unsigned long long g0; };
+__device__ __forceinline__ unsigned long long tl_gtime() {
+  unsigned long long t;
+  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+  return t;
+}
+#define RB_TL_INIT(cp) __shared__ TlBuf tl_buf_; unsigned long long* const tl_ptr_ = (cp)->timeline; \
+  if (threadIdx.x == 0) { for (int q_ = 0; q_ < 32; ++q_) tl_buf_.c[q_] = 0; tl_buf_.g0 = tl_gtime(); }
+#define RB_TL(cp, slot) do { if (threadIdx.x == 0) tl_buf_.c[(slot) & 31] = clock64(); } while (0)
+#define RB_TL_FLUSH(cp, first, last) do { if (threadIdx.x == 0) { atomicMin(tl_ptr_ + (first), tl_buf_.g0); \
+  atomicMax(tl_ptr_ + (last), tl_gtime()); if (blockIdx.x == 0) for (int q_ = 0; q_ < 32; ++q_) if (tl_buf_.c[q_]) \
+  tl_ptr_[64 + ((first) & ~31) + q_] = (unsigned long long)tl_buf_.c[q_]; } } while (0)
+#else
+#define RB_TL_INIT(cp)
+#define RB_TL(cp, slot)
+#define RB_TL_FLUSH(cp, first, last)
+#endif
 __device__ __forceinline__ void launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 __device__ __forceinline__ void grid_dependency_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 
@@ -101,13 +124,14 @@ __device__ __forceinline__ void grid_dependency_wait() { asm volatile("griddepco
 // present tiers are the candidates (reading 24).  Cmax runs over the candidates ("normalized by their
 // candidate maxima").  Non-candidates get A = -inf, which the score and dispatch kernels read as "filtered out".
 // Also returns the LPT key max_m L^ over present tiers (budgets do not enter it).  sC / sL: [M] in shared memory.
-__device__ __forceinline__ float tier_term_A(int m, int M, const int32_t* __restrict__ present, const float* sC,
+// present: bit j set iff tier j has an instance.
+__device__ __forceinline__ float tier_term_A(int m, int M, uint32_t present, const float* sC,
                                              const float* sL, float Q, float wq, float wc, bool has_budget, float budget,
                                              float* key_out) {
   float kmax = 0.0f, Cmin = 0.0f;
   bool first = true, any = false;
   for (int j = 0; j < M; ++j) {
-    if (!present[j]) continue;
+    if (!((present >> j) & 1u)) continue;
     if (first || sL[j] > kmax) kmax = sL[j];
     if (first || sC[j] < Cmin) Cmin = sC[j];
     first = false;
@@ -117,7 +141,7 @@ __device__ __forceinline__ float tier_term_A(int m, int M, const int32_t* __rest
   first = true;
   bool mine = false;
   for (int j = 0; j < M; ++j) {
-    if (!present[j]) continue;
+    if (!((present >> j) & 1u)) continue;
     const bool cand = any ? (!has_budget || sC[j] <= budget) : (sC[j] == Cmin);
     if (!cand) continue;
     if (first || sC[j] > Cmax) Cmax = sC[j];
@@ -232,6 +256,9 @@ cudaError_t lpt_dispatch_prepare();  // opt in to the dynamic shared memory size
 // the a8 drain rule with that tpot (rb_advance_state under latency_mode 2).
 cudaError_t launch_tpot_forest(InstTable t, ForestDev forest, float* dq, int32_t* bq, float* tpot_out, float elapsed_ms,
                                cudaStream_t s);
+
+// Counts pairs on which the dispatch loop's branch-free division differs from the IEEE one (must be 0).
+cudaError_t launch_div_selftest(unsigned long long n, unsigned long long seed, unsigned long long* mismatches, cudaStream_t s);
 
 // a8: dead reckoning between batches.
 cudaError_t launch_advance(InstTable t, float* dq, int32_t* bq, float elapsed_ms, cudaStream_t s);

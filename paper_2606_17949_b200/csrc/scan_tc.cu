@@ -35,7 +35,15 @@ __device__ __forceinline__ void trace(int slot) {
   }
 }
 #define RB_TR(slot) trace(slot)
+__device__ unsigned long long rb_scan_tl[8];   // [0] earliest start, [1] latest end, [2] earliest first TMA issue, [3] latest last-epilogue end
+__device__ __forceinline__ void scan_tl(int slot) {
+  unsigned long long t;
+  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+  if (slot & 1) atomicMax(rb_scan_tl + slot, t); else atomicMin(rb_scan_tl + slot, t);
+}
+#define RB_STL(slot) scan_tl(slot)
 #else
+#define RB_STL(slot)
 #define RB_TR(slot)
 #endif
 
@@ -74,7 +82,7 @@ scan_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__
   const int ntiles = (nunits + 3) / 4;
 
   launch_dependents();
-  if (threadIdx.x == 0) RB_TR(0);
+  if (threadIdx.x == 0) { RB_TR(0); RB_STL(0); }
   if (warp == 0 && lane == 0) {
     asm volatile("prefetch.tensormap [%0];" ::"l"(&tm_q) : "memory");
     asm volatile("prefetch.tensormap [%0];" ::"l"(&tm_bank) : "memory");
@@ -103,6 +111,7 @@ scan_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__
     // ===== TMA producer =====
     if (lane == 0) {
       grid_dependency_wait();   // the staged queries come from the preceding kernel
+      RB_STL(2);
       uint32_t kit = 0;
       for (int tile = 0; tile < ntiles; ++tile) {
         const int n0 = (int)(row0 + (int64_t)tile * kTileN);
@@ -238,10 +247,10 @@ scan_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__
     }
   }
 
-  if (tl_trace_end(threadIdx.x)) RB_TR(2);
+  if (tl_trace_end(threadIdx.x)) { RB_TR(2); RB_STL(3); }
   tc_fence_before();
   __syncthreads();
-  if (threadIdx.x == 0) RB_TR(3);
+  if (threadIdx.x == 0) { RB_TR(3); RB_STL(1); }
   if (warp == 1) {
     tc_fence_after();
     asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(512) : "memory");
@@ -249,6 +258,18 @@ scan_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__
 }
 
 }  // namespace
+
+#ifdef RB_TRACE
+extern "C" int rb_debug_scan_timeline(unsigned long long* out, int reset) {
+  cudaDeviceSynchronize();
+  cudaMemcpyFromSymbol(out, rb_scan_tl, sizeof(rb_scan_tl));
+  if (reset) {
+    unsigned long long init[8] = {~0ull, 0, ~0ull, 0, ~0ull, 0, ~0ull, 0};
+    cudaMemcpyToSymbol(rb_scan_tl, init, sizeof(init));
+  }
+  return 0;
+}
+#endif
 
 size_t scan_tc_smem_bytes() { return kSmemBytes; }
 

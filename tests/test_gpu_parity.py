@@ -511,3 +511,14 @@ def test_boosted_head_full_decide_path(orc):
     s = rt.get_state()
     assert np.array_equal(s[0].numpy(), ref["queued"]) and np.array_equal(s[1].numpy(), ref["running"])
     rt.close()
+
+
+def test_dispatch_fast_division_is_ieee_exact():
+    """The dispatch loop divides with a branch-free reciprocal-refinement sequence inside a safe exponent window
+    (IEEE __fdiv_rn outside it): 2^31 pseudo-random in-window operand pairs, bit for bit against the IEEE division."""
+    from paper_2606_17949_b200 import binding as rb
+    from paper_2606_17949_b200.router import Router
+    rt = Router(torch.randn(64, 16).cuda(), torch.rand(64, 2).cuda(), torch.rand(64, 2).cuda() + 1, 4, store="f32", max_batch=4)
+    for seed in (0, 12345):
+        assert rb.rb_selftest_division(rt.ctx, 1 << 30, seed) == 0
+    rt.close()
