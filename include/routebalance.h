@@ -156,7 +156,9 @@ rb_status rb_get_state(rb_ctx* ctx, float* queued_tokens, int32_t* running);
 
 /* Dead reckoning between batches (BASELINE.json; the drain rule is this library's, reading 22):
  * every instance with b_i > 0 drains d_i <- max(0, d_i - b_i * elapsed_ms / tpot_i); b_i <- 0 when d_i
- * reaches 0.  elapsed_ms must be finite and >= 0. */
+ * reaches 0.  elapsed_ms must be finite and >= 0.
+ * The drain is applied in stream order before anything reads or writes the state; under the linear head it is deferred
+ * into the first kernel of the next rb_decide (no launch of its own), other calls apply it first. */
 rb_status rb_advance_state(rb_ctx* ctx, float elapsed_ms);
 
 /* One per-batch decision: estimate -> score -> LPT greedy dispatch, committing the dead-reckoned updates.

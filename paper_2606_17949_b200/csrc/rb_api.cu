@@ -69,6 +69,9 @@ struct rb_ctx {
   float *f_base = nullptr, *f_aux = nullptr, *f_tpot0 = nullptr;
   int f_features = 0;
   bool has_forest = false;
+  // rb_advance_state calls not yet applied on the device: the next rb_decide folds them into its first kernel
+  float pending_adv[kMaxPendingAdvance]{};
+  int n_pending = 0;
   float *scores = nullptr, *scores0 = nullptr;  // [max_batch x I], allocated by rb_set_instances
   CUtensorMap tm_q{}, tm_bank{};
   // graphs: key = B * 4 + kind (0 decide, 1 estimate, 2 from_predictions)
@@ -138,6 +141,16 @@ InstTable table_of(const rb_ctx* c) {
   return t;
 }
 
+// Applies the pending rb_advance_state calls with the standalone kernel (every path but rb_decide's bf16 pipeline).
+rb_status flush_pending(rb_ctx* ctx) {
+  for (int a = 0; a < ctx->n_pending; ++a) {
+    CK(launch_advance(table_of(ctx), ctx->dq, ctx->bq, ctx->pending_adv[a], ctx->stream));
+    ctx->launches += 1;
+  }
+  ctx->n_pending = 0;
+  return RB_OK;
+}
+
 rb_status encode_map(rb_ctx* ctx, CUtensorMap* map, void* base, uint64_t rows, uint64_t cols, uint32_t box_rows) {
   static PFN_cuTensorMapEncodeTiled_v12000 fn = nullptr;
   if (!fn) {
@@ -199,7 +212,7 @@ rb_status enqueue_estimate(rb_ctx* ctx, int B, bool with_terms, Timer& tm) {
       // tensor-bound regime: CTA pairs, 256-query m-tiles
       const int Bpad2 = (B + 2 * kTileM - 1) / (2 * kTileM) * (2 * kTileM);
       CK(launch_stage_queries(ctx->cp, ctx->qs, B, Bpad2, ctx->d, 1, ctx->gthr,
-                              Bpad2 * (1 + scan_tc2_clusters(ctx->N, ctx->num_sms)), s));
+                              Bpad2 * (1 + scan_tc2_clusters(ctx->N, ctx->num_sms)), table_of(ctx), ctx->dq, ctx->bq, s));
       tm.mark();
       int ncl = 0;
       CK(launch_scan_tc2(&ctx->tm_q, &ctx->tm_bank, ctx->N, ctx->d, B, Bpad2, ctx->kcap, ctx->kc, ctx->num_sms, ctx->part_sim,
@@ -209,7 +222,7 @@ rb_status enqueue_estimate(rb_ctx* ctx, int B, bool with_terms, Timer& tm) {
       fa.Bpad = Bpad2; fa.slab_unit = kTileN; fa.rescan = 0;   // full-length lists (K >= k + slack): nothing hidden
     } else {
       const int rep = scan_tc_replicas(B, ctx->ks, ctx->num_sms);
-      CK(launch_stage_queries(ctx->cp, ctx->qs, B, Bpad, ctx->d, rep, ctx->gthr, Bpad, s));
+      CK(launch_stage_queries(ctx->cp, ctx->qs, B, Bpad, ctx->d, rep, ctx->gthr, Bpad, table_of(ctx), ctx->dq, ctx->bq, s));
       tm.mark();
       int grid = 0;
       CK(launch_scan_tc(&ctx->tm_q, &ctx->tm_bank, ctx->N, ctx->d, B, Bpad, ctx->ks, ctx->num_sms, ctx->part_sim,
@@ -622,6 +635,7 @@ rb_status rb_set_instances(rb_ctx* ctx, int32_t I, const int32_t* tier, const in
   CK(cudaMemcpyAsync(ctx->slope, slope, M * 4, cudaMemcpyHostToDevice, s));
   CK(cudaMemcpyAsync(ctx->dec_i, dec_i.data(), I * 4, cudaMemcpyHostToDevice, s));
   CK(cudaMemcpyAsync(ctx->slope_i, slope_i.data(), I * 4, cudaMemcpyHostToDevice, s));
+  ctx->n_pending = 0;   // the state is reset
   CK(cudaMemsetAsync(ctx->dq, 0, kMaxI * 4, s));
   CK(cudaMemsetAsync(ctx->bq, 0, kMaxI * 4, s));
   CK(cudaMemsetAsync(ctx->f_aux, 0, (size_t)kMaxI * kMaxFeatures * 4, s));
@@ -699,6 +713,7 @@ rb_status rb_set_state(rb_ctx* ctx, const float* queued_tokens, const int32_t* r
     for (int i = 0; i < ctx->I; ++i)
       if (!finite_nonneg(queued_tokens[i]) || running[i] < 0) return fail(ctx, RB_EINVAL, "state must be finite, >= 0");
   }
+  ctx->n_pending = 0;   // advances before an overwrite of the whole state have no effect
   CK(cudaMemcpyAsync(ctx->dq, queued_tokens, ctx->I * 4, cudaMemcpyDefault, ctx->stream));
   CK(cudaMemcpyAsync(ctx->bq, running, ctx->I * 4, cudaMemcpyDefault, ctx->stream));
   if (host) CK(cudaStreamSynchronize(ctx->stream));
@@ -708,6 +723,10 @@ rb_status rb_set_state(rb_ctx* ctx, const float* queued_tokens, const int32_t* r
 rb_status rb_get_state(rb_ctx* ctx, float* queued_tokens, int32_t* running) {
   if (!ctx) return RB_EINVAL;
   if (ctx->I == 0) return fail(ctx, RB_ESTATE, "rb_get_state before rb_set_instances");
+  {
+    rb_status st = flush_pending(ctx);
+    if (st != RB_OK) return st;
+  }
   bool any_host = false;
   if (queued_tokens) {
     any_host |= is_host_ptr(queued_tokens);
@@ -729,7 +748,14 @@ rb_status rb_advance_state(rb_ctx* ctx, float elapsed_ms) {
     if (!ctx->has_forest) return fail(ctx, RB_ESTATE, "latency_mode 2 needs rb_set_tpot_forest first");
     CK(launch_tpot_forest(table_of(ctx), forest_of(ctx), ctx->dq, ctx->bq, nullptr, elapsed_ms, ctx->stream));
   } else {
-    CK(launch_advance(table_of(ctx), ctx->dq, ctx->bq, elapsed_ms, ctx->stream));
+    // deferred: the next rb_decide applies it in its first kernel (one launch less per decision); any other reader or
+    // writer of the state applies it first (flush_pending)
+    if (ctx->n_pending == kMaxPendingAdvance) {
+      rb_status st = flush_pending(ctx);
+      if (st != RB_OK) return st;
+    }
+    ctx->pending_adv[ctx->n_pending++] = elapsed_ms;
+    return RB_OK;
   }
   ctx->launches += 1;
   return RB_OK;
@@ -756,6 +782,14 @@ rb_status rb_decide_budgeted(rb_ctx* ctx, const float* query_emb, const int32_t*
   Stager sg{ctx};
   CallParams cp{};
   cp.w_qual = w[0]; cp.w_lat = w[1]; cp.w_cost = w[2]; cp.commit = 1;
+  if (ctx->opt.store_dtype == RB_BF16 && ctx->opt.latency_mode != 2) {
+    cp.n_adv = ctx->n_pending;   // applied by the staging kernel, ahead of everything that reads the state
+    for (int a = 0; a < ctx->n_pending; ++a) cp.adv_ms[a] = ctx->pending_adv[a];
+    ctx->n_pending = 0;
+  } else {
+    st = flush_pending(ctx);
+    if (st != RB_OK) return st;
+  }
   cp.query = sg.in(query_emb, ctx->q32, (size_t)B * ctx->d * 4);
   cp.plen = sg.in(prompt_len, ctx->plen, (size_t)B * 4);
   cp.q_src = ctx->pred_q;
@@ -821,6 +855,8 @@ rb_status rb_decide_from_predictions_budgeted(rb_ctx* ctx, const float* quality,
   Stager sg{ctx};
   CallParams cp{};
   cp.w_qual = w[0]; cp.w_lat = w[1]; cp.w_cost = w[2]; cp.commit = commit ? 1 : 0;
+  st = flush_pending(ctx);   // the score kernel's CTAs all read the state: it must be current before they start
+  if (st != RB_OK) return st;
   cp.q_src = sg.in(quality, ctx->stage_q, bm);
   cp.l_src = sg.in(outlen, ctx->stage_l, bm);
   cp.plen = sg.in(prompt_len, ctx->plen, (size_t)B * 4);

@@ -14,6 +14,7 @@ constexpr int kTileM = 128;        // queries per MMA tile (TMEM lanes)
 constexpr int kTileN = 256;        // bank rows per MMA tile (TMEM columns of one accumulator)
 constexpr int kBoxN = 64;          // bank rows per TMA box; slabs are multiples of this
 constexpr int kTileK = 64;         // bf16 per K chunk = one 128-byte swizzle row
+constexpr int kMaxPendingAdvance = 4;   // rb_advance_state calls a decision can absorb (CallParams::adv_ms)
 
 // Instance table + per-tier coefficients as the score/dispatch kernels see them (device memory).
 struct InstTable {
@@ -63,6 +64,8 @@ struct CallParams {
   float* nn_sim;
   const float* budget;     // [B] per-request cost budgets (Eq. 2) or NULL: no admission filter
   int32_t* max_tokens;     // [B] or NULL: output-token clamp of the chosen instance
+  int32_t n_adv;           // pending rb_advance_state calls folded into this decision's first kernel (<= kMaxPendingAdvance)
+  float adv_ms[4];         // their elapsed_ms, in call order
 #ifdef RB_TRACE
   unsigned long long* timeline;   // development aid: [128] globaltimer stamps (even slots: earliest, odd: latest), then block 0's clock64 per slot
 #endif
@@ -176,8 +179,9 @@ cudaError_t launch_convert_bf16(const float* in, __nv_bfloat16* out, size_t n, c
 
 // a0: cp->query (fp32) -> bf16 staging [Bpad x d]; rep copies of the B queries at rows j*(128/rep) + r (rep > 1 only
 // when Bpad = 128), all other rows zero.  Also clears gthr [n_gthr] (the scan's cross-slab thresholds).
+// Block 0 also applies the cp->n_adv pending state advances (a8's drain rule, linear head) to (dq, bq), in call order.
 cudaError_t launch_stage_queries(const CallParams* cp, __nv_bfloat16* qs, int B, int Bpad, int d, int rep, uint32_t* gthr,
-                                 int n_gthr, cudaStream_t s);
+                                 int n_gthr, InstTable t, float* dq, int32_t* bq, cudaStream_t s);
 // query replicas over the TMEM lane quarters: 4 (B <= 32), 2 (B <= 64), 1; halved while the finishing kernel could not
 // hold max_grid * replicas lists of kcap entries in shared memory (long lists: k = 32)
 int scan_tc_replicas(int B, int kcap, int max_grid);

@@ -522,3 +522,42 @@ def test_dispatch_fast_division_is_ieee_exact():
     for seed in (0, 12345):
         assert rb.rb_selftest_division(rt.ctx, 1 << 30, seed) == 0
     rt.close()
+
+
+def test_deferred_advance_is_applied_in_call_order(orc):
+    """rb_advance_state is deferred into the next rb_decide's first kernel; every other reader or writer of the state
+    must see it applied (or, for an overwrite, dropped): sequences of advances, reads, overwrites and both decision
+    entry points against the oracle's advance + dispatch, bit for bit."""
+    cfg = dataclasses.replace(synth.CONFIGS["C2"], N=6000, d=64, B=9, Kc=8, seed=31)
+    bank, it, queued, running, query, plen, rt = _setup(cfg, max_batch=16)
+    inst = orc.Instances(**it)
+    w = synth.PRESETS["balanced"]
+    dq, bq = queued.numpy().copy(), running.numpy().copy()
+    # six advances (more than a decision absorbs) then a read
+    for dt in (5.0, 17.5, 0.0, 250.0, 3.25, 40.0):
+        rt.advance_state(dt)
+        dq, bq = orc.advance_state(inst, dq, bq, np.float32(dt))
+    s = rt.get_state()
+    assert np.array_equal(s[0].numpy(), dq) and np.array_equal(s[1].numpy(), bq)
+    # advances, then a full decision: folded into the staging kernel
+    for dt in (12.0, 33.0, 8.5):
+        rt.advance_state(dt)
+        dq, bq = orc.advance_state(inst, dq, bq, np.float32(dt))
+    g = _np(rt.decide(query, plen, w))
+    ref = orc.dispatch(inst, dq, bq, g["pred_quality"], g["pred_outlen"], plen.cpu().numpy(), w)
+    assert np.array_equal(g["assignment"], ref["assignment"]) and np.array_equal(g["scores"], ref["scores"])
+    dq, bq = ref["queued"], ref["running"]
+    # an advance before decide_from_predictions is applied first
+    rt.advance_state(77.0)
+    dq, bq = orc.advance_state(inst, dq, bq, np.float32(77.0))
+    g2 = _np(rt.decide_from_predictions(torch.from_numpy(g["pred_quality"]).cuda(), torch.from_numpy(g["pred_outlen"]).cuda(),
+                                        plen, w, commit=1))
+    ref2 = orc.dispatch(inst, dq, bq, g["pred_quality"], g["pred_outlen"], plen.cpu().numpy(), w)
+    assert np.array_equal(g2["assignment"], ref2["assignment"]) and np.array_equal(g2["scores0"], ref2["scores0"])
+    # an advance followed by an overwrite of the state is dropped; an estimate in between leaves it pending
+    rt.advance_state(1000.0)
+    rt.estimate(query)
+    rt.set_state(queued, running)
+    s = rt.get_state()
+    assert np.array_equal(s[0].numpy(), queued.numpy()) and np.array_equal(s[1].numpy(), running.numpy())
+    rt.close()
