@@ -325,12 +325,24 @@ finish_kernel(FinishArgs a, InstTable t, const CallParams* __restrict__ cp) {
       for (int u = 0; u < 2; ++u) {
         const int e = e0 + u * kFinThreads;
         if (e < nquads) {
-          const int c = e / q4, j4 = e - c * q4;
-          const size_t off = ((size_t)c * a.Bpad + r) * kcap + 4 * j4;
-          sv[u] = __ldcg(reinterpret_cast<const float4*>(a.part_sim + off));
-          iv[u] = __ldcg(reinterpret_cast<const int4*>(a.part_idx + off));
+          if (a.records) {   // record e of this query: [4 similarities | 4 indices], contiguous over e
+            const uint4* rec = reinterpret_cast<const uint4*>(a.part_sim) + ((size_t)r * nquads + e) * 2;
+            const uint4 ua = __ldcg(rec), ub = __ldcg(rec + 1);
+            sv[u] = make_float4(__uint_as_float(ua.x), __uint_as_float(ua.y), __uint_as_float(ua.z), __uint_as_float(ua.w));
+            iv[u] = make_int4((int)ub.x, (int)ub.y, (int)ub.z, (int)ub.w);
+          } else {
+            const int c = e / q4, j4 = e - c * q4;
+            const size_t off = ((size_t)c * a.Bpad + r) * kcap + 4 * j4;
+            sv[u] = __ldcg(reinterpret_cast<const float4*>(a.part_sim + off));
+            iv[u] = __ldcg(reinterpret_cast<const int4*>(a.part_idx + off));
+          }
         }
       }
+#ifdef RB_TRACE
+      RB_TL(cp, 56);                                    // loads issued
+      if (sv[0].x == 12345.678f && iv[0].x == -77) tl_buf_.g0 = 0;   // (waits for the data)
+      RB_TL(cp, 58);                                    // loads returned
+#endif
 #pragma unroll
       for (int u = 0; u < 2; ++u) {
         const int e = e0 + u * kFinThreads;
@@ -535,6 +547,7 @@ finish_kernel(FinishArgs a, InstTable t, const CallParams* __restrict__ cp) {
   if (tid < 2 * M) {
     const int m = tid % M;
     float num = 0.0f, den = 0.0f;
+#pragma unroll 1   // executed once, by one warp, from a cold instruction cache: compact code beats unrolled code here
     for (int j = 0; j < k; ++j) {
       const float w = s_w[j];
       if (o_idx[j] < 0) continue;

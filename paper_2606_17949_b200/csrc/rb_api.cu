@@ -229,6 +229,7 @@ rb_status enqueue_estimate(rb_ctx* ctx, int B, bool with_terms, Timer& tm) {
                         ctx->part_idx, &grid, s));
       tm.mark();
       fa.part_sim = ctx->part_sim; fa.part_idx = ctx->part_idx; fa.nlists = grid * rep; fa.lists_per_cta = rep; fa.kcap = ctx->ks;
+      fa.records = 1;
       fa.Bpad = Bpad; fa.slab_unit = kBoxN;
     }
     if (!(B > kTileM && ctx->num_sms >= 2)) fa.rescan = ctx->ks < ctx->kc ? 1 : 0;
@@ -564,8 +565,8 @@ rb_status rb_create(rb_ctx** out, const void* bank_emb, const float* bank_qualit
     ALLOC(ctx->gthr, (size_t)ctx->Bpad_max * (2 + ctx->num_sms / 2));
     // [grid * rep][Bpad][ks]: rep = 4 replicas only when Bpad = 128
     const size_t part_n = (size_t)ctx->num_sms * ctx->kcap * std::max<size_t>(ctx->Bpad_max, 4 * kTileM);
-    ALLOC(ctx->part_sim, part_n);
-    ALLOC(ctx->part_idx, part_n);
+    ALLOC(ctx->part_sim, 2 * part_n);          // one allocation: [similarities | indices], or 32-byte records over all of it
+    ctx->part_idx = reinterpret_cast<int32_t*>(ctx->part_sim + part_n);
     CK(cudaMemsetAsync(ctx->qs, 0, (size_t)ctx->Bpad_max * d * 2, s));
     rb_status st = encode_map(ctx, &ctx->tm_bank, ctx->bank, (uint64_t)N, (uint64_t)d, kBoxN);
     if (st != RB_OK) return st;
@@ -930,7 +931,7 @@ void rb_destroy(rb_ctx* ctx) {
   if (!ctx) return;
   if (ctx->stream) cudaStreamSynchronize(ctx->stream);
   for (auto& kv : ctx->graphs) cudaGraphExecDestroy(kv.second);
-  void* ptrs[] = {ctx->bank, ctx->bank_quality, ctx->bank_outlen, ctx->arena, ctx->q32, ctx->qs, ctx->part_sim, ctx->part_idx,
+  void* ptrs[] = {ctx->bank, ctx->bank_quality, ctx->bank_outlen, ctx->arena, ctx->q32, ctx->qs, ctx->part_sim,
                   ctx->gthr, ctx->sims, ctx->scratch_nn_idx, ctx->scratch_nn_sim, ctx->scores, ctx->scores0, ctx->f_nodes,
                   ctx->f_root, ctx->f_begin, ctx->f_base};
   for (void* p : ptrs) cudaFree(p);

@@ -133,6 +133,7 @@ __device__ __forceinline__ float tier_term_A(int m, int M, uint32_t present, con
                                              float* key_out) {
   float kmax = 0.0f, Cmin = 0.0f;
   bool first = true, any = false;
+#pragma unroll 1   // cold, once-executed code: keep it compact
   for (int j = 0; j < M; ++j) {
     if (!((present >> j) & 1u)) continue;
     if (first || sL[j] > kmax) kmax = sL[j];
@@ -143,6 +144,7 @@ __device__ __forceinline__ float tier_term_A(int m, int M, uint32_t present, con
   float Cmax = 0.0f;
   first = true;
   bool mine = false;
+#pragma unroll 1
   for (int j = 0; j < M; ++j) {
     if (!((present >> j) & 1u)) continue;
     const bool cand = any ? (!has_budget || sC[j] <= budget) : (sC[j] == Cmin);
@@ -186,8 +188,9 @@ cudaError_t launch_stage_queries(const CallParams* cp, __nv_bfloat16* qs, int B,
 // hold max_grid * replicas lists of kcap entries in shared memory (long lists: k = 32)
 int scan_tc_replicas(int B, int kcap, int max_grid);
 
-// a1 (bf16): tcgen05 scan.  part_* are [grid * rep][Bpad][KCAP] (sim fp32 / idx int32, idx -1 = empty), each list
-// sorted by (sim desc, idx asc).  Returns the grid size used through *grid_out.  kcap in {4,8,16,32,64}; bank
+// a1 (bf16): tcgen05 scan.  The lists (sim fp32 / idx int32, idx -1 = empty, each sorted by (sim desc, idx asc)) are
+// written through part_sim as QUERY-MAJOR 32-byte records: record ((r * nlists + list) * KCAP/4 + quad) =
+// [4 similarities | 4 indices], nlists = grid * rep; part_sim must have room for nlists * Bpad * KCAP * 8 bytes.  Returns the grid size used through *grid_out.  kcap in {4,8,16,32,64}; bank
 // rows are split over the CTAs in units of kBoxN rows: CTA c owns units [units*c/grid, units*(c+1)/grid).
 cudaError_t launch_scan_tc(const CUtensorMap* tm_q, const CUtensorMap* tm_bank, int64_t N, int d, int B, int Bpad,
                            int kcap, int max_grid, float* part_sim, int32_t* part_idx, int* grid_out,
@@ -222,6 +225,8 @@ struct FinishArgs {
   const int32_t* part_idx;
   int nlists, kcap, Bpad, kc, k;   // nlists = grid * lists_per_cta
   int lists_per_cta;
+  int records;              // 1: part_sim holds the query-major 32-byte records of launch_scan_tc; 0: part_sim / part_idx
+                            //    are [nlists][Bpad][kcap] arrays
   int slab_unit;            // rows per slab unit: slab c = rows [units*c/nslabs, units*(c+1)/nslabs) * slab_unit
   int64_t N;
   const __nv_bfloat16* bank;

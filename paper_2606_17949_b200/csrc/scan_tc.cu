@@ -110,14 +110,33 @@ scan_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__
   if (warp == 0) {
     // ===== TMA producer =====
     if (lane == 0) {
-      grid_dependency_wait();   // the staged queries come from the preceding kernel
+      // The bank does not depend on the preceding (staging) kernel, the staged queries do: the first ring slots get
+      // their bank boxes before the dependency resolves, their query tiles after it -- the HBM stream starts while
+      // the staging kernel still runs.
+      const int per_tile = n_mt * nk;
+      const int total_it = ntiles * per_tile;
+      const int npre = min(kStages, total_it);
+      for (int kit = 0; kit < npre; ++kit) {
+        const int tile = kit / per_tile, kc = (kit - tile * per_tile) % nk;
+        const int n0 = (int)(row0 + (int64_t)tile * kTileN);
+        const int nun = min(4, nunits - tile * 4);
+        uint8_t* sb = smem + kit * kStageBytes + kABytes;
+        mbar_arrive_expect_tx(&full[kit], kABytes + nun * kBoxBytes);
+        for (int u = 0; u < nun; ++u) tma_load_2d(sb + u * kBoxBytes, &tm_bank, kc * kTileK, n0 + u * kBoxN, &full[kit]);
+      }
       RB_STL(2);
+      grid_dependency_wait();   // the staged queries come from the preceding kernel
+      for (int kit = 0; kit < npre; ++kit) {
+        const int tile = kit / per_tile, rem = kit - tile * per_tile;
+        tma_load_2d(smem + kit * kStageBytes, &tm_q, (rem % nk) * kTileK, (rem / nk) * kTileM, &full[kit]);
+      }
       uint32_t kit = 0;
       for (int tile = 0; tile < ntiles; ++tile) {
         const int n0 = (int)(row0 + (int64_t)tile * kTileN);
         const int nun = min(4, nunits - tile * 4);
         for (int mt = 0; mt < n_mt; ++mt) {
           for (int kc = 0; kc < nk; ++kc, ++kit) {
+            if ((int)kit < npre) continue;   // issued above
             const int s = kit % kStages;
             const uint32_t ph = (kit / kStages) & 1;
             mbar_wait(&empty[s], ph ^ 1);
@@ -190,9 +209,10 @@ scan_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__
         const uint32_t acc = it & 1, aph = (it >> 1) & 1;
         const int r = mt * kTileM + (tl - replica * group);
         const bool warp_active = (mt * kTileM + (quarter * 32) % group) < B;   // warp-uniform
-        const size_t pbase = (((size_t)blockIdx.x * rep + replica) * (size_t)Bpad + (size_t)r) * KCAP;
-        float4* ps4 = reinterpret_cast<float4*>(part_sim + pbase);
-        int4* pi4 = reinterpret_cast<int4*>(part_idx + pbase);
+        // query-major 32-byte records [similarities of a quad | their indices]: the finishing CTA of a query reads its
+        // lists as one contiguous stream of whole sectors (a half-written sector would cost it a DRAM fill)
+        const size_t pbase = ((size_t)r * ((size_t)gridDim.x * rep) + ((size_t)blockIdx.x * rep + replica)) * (KCAP / 4) * 2;
+        uint4* prec = reinterpret_cast<uint4*>(part_sim) + pbase;
         if (warp_active) {
           if (tile == 0) {
 #pragma unroll
@@ -200,8 +220,9 @@ scan_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__
           } else if (n_mt > 1) {
 #pragma unroll
             for (int j = 0; j < KCAP / 4; ++j) {
-              const float4 a = ps4[j];
-              const int4 b = pi4[j];
+              const uint4 ua = prec[2 * j], ub = prec[2 * j + 1];
+              const float4 a = make_float4(__uint_as_float(ua.x), __uint_as_float(ua.y), __uint_as_float(ua.z), __uint_as_float(ua.w));
+              const int4 b = make_int4((int)ub.x, (int)ub.y, (int)ub.z, (int)ub.w);
               v[4 * j] = a.x; v[4 * j + 1] = a.y; v[4 * j + 2] = a.z; v[4 * j + 3] = a.w;
               ix[4 * j] = b.x; ix[4 * j + 1] = b.y; ix[4 * j + 2] = b.z; ix[4 * j + 3] = b.w;
             }
@@ -239,8 +260,9 @@ scan_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__
         if (warp_active && r < B && (n_mt > 1 || tile == ntiles - 1)) {
 #pragma unroll
           for (int j = 0; j < KCAP / 4; ++j) {
-            ps4[j] = make_float4(v[4 * j], v[4 * j + 1], v[4 * j + 2], v[4 * j + 3]);
-            pi4[j] = make_int4(ix[4 * j], ix[4 * j + 1], ix[4 * j + 2], ix[4 * j + 3]);
+            prec[2 * j] = make_uint4(__float_as_uint(v[4 * j]), __float_as_uint(v[4 * j + 1]), __float_as_uint(v[4 * j + 2]),
+                                     __float_as_uint(v[4 * j + 3]));
+            prec[2 * j + 1] = make_uint4((uint32_t)ix[4 * j], (uint32_t)ix[4 * j + 1], (uint32_t)ix[4 * j + 2], (uint32_t)ix[4 * j + 3]);
           }
         }
       }
