@@ -338,11 +338,6 @@ finish_kernel(FinishArgs a, InstTable t, const CallParams* __restrict__ cp) {
           }
         }
       }
-#ifdef RB_TRACE
-      RB_TL(cp, 56);                                    // loads issued
-      if (sv[0].x == 12345.678f && iv[0].x == -77) tl_buf_.g0 = 0;   // (waits for the data)
-      RB_TL(cp, 58);                                    // loads returned
-#endif
 #pragma unroll
       for (int u = 0; u < 2; ++u) {
         const int e = e0 + u * kFinThreads;
