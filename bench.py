@@ -24,6 +24,10 @@ One JSON line is printed by rank 0:
                same stream
   scan_c4      BASELINE.json configs[3] (N=10M x d=384 bf16 = 7.68 GB, B=64): the scan kernel alone against
                the HBM roofline -- the north-star's ">= 70 % of the HBM roofline" figure (bank >> L2)
+  sweep_c4     the whole configs[3] sweep: B in {1, 8, 64, 512, 4096} x k in {10, 32}, GB/s and TFLOP/s of the scan
+  scan_c3      configs[2] (N=1M x d=1024, B=1024): the CTA-pair scan kernel against the tensor roofline
+  sweep_c5     configs[4]: 66 simplex points of score + LPT dispatch from fixed predictions (linear and boosted head)
+               (--no-large skips these three)
 
 --impl reference times the oracle alone (this tier has no reference implementation; the oracle is the
 reference arm).  With --gpus N > 1 (torchrun) every rank runs an independent replica of the router on its
@@ -346,6 +350,7 @@ def run_ours(args):
         if not args.no_scan_c4:
             out["scan_c4"] = scan_c4(synth, Router, dev, hbm_peak)
         if not args.no_large:
+            out["sweep_c4"] = sweep_c4(synth, Router, dev, hbm_peak)
             out["scan_c3"] = scan_c3(synth, Router, dev)
             out["sweep_c5"] = sweep_c5(synth, Router, dev)
     else:
@@ -422,6 +427,45 @@ def scan_c4(synth, Router, dev, hbm_peak):
             "bytes_per_launch": int(nbytes), "achieved": round(ach, 1), "unit": "GB/s", "peak": hbm_peak,
             "frac": round(ach / hbm_peak, 4), "frac_of_nominal_8TBs": round(ach / 8000.0, 4),
             "traffic": recorded_traffic("c4"), "l2": "bank 7.68 GB >> 126 MB L2"}
+
+
+def sweep_c4(synth, Router, dev, hbm_peak):
+    """BASELINE.json configs[3], the whole sweep: N=10M x d=384 bf16 (7.68 GB), B in {1, 8, 64, 512, 4096} x k in {10, 32}:
+    the scan kernel alone (CUDA events around it, stage timing mode), as GB/s against the HBM roofline and TFLOP/s
+    against the tensor roofline; whichever fraction is larger names the bound of that point."""
+    import dataclasses
+    import torch
+    burst, sustained, _ = measured_tensor_peaks()
+    base = synth.CONFIGS["C4"]
+    bank = synth.make_bank(base, device=dev)
+    rows = []
+    for k, slack in ((10, 6), (32, 8)):
+        cfg = dataclasses.replace(base, k=k)
+        rt = Router(bank["emb"], bank["quality"], bank["outlen"], k, store="bf16", rerank_slack=slack, max_batch=4096, device=dev)
+        for B in (1, 8, 64, 512, 4096):
+            q = synth.make_queries(cfg, B=B, device=dev)
+            torch.cuda.synchronize()
+            for _ in range(2):
+                rt.estimate(q)
+            rt.sync()
+            rt.set_stage_timing(1)
+            us, fin = [], []
+            for _ in range(5 if B >= 512 else 10):
+                rt.estimate(q)
+                st = rt.stage_us()
+                us.append(st["scan"])
+                fin.append(st["aggregate"])
+            rt.set_stage_timing(0)
+            t = float(np.mean(us))
+            gbs = (cfg.N * cfg.d * 2 + B * cfg.d * 2) / (t * 1e-6) / 1e9
+            tfs = 2.0 * B * cfg.N * cfg.d / (t * 1e-6) / 1e12
+            fh, ft = gbs / hbm_peak, tfs / burst
+            rows.append({"B": B, "k": k, "scan_us": round(t, 1), "finish_us": round(float(np.mean(fin)), 1),
+                         "GB/s": round(gbs, 1), "frac_hbm": round(fh, 4), "TFLOP/s": round(tfs, 1), "frac_tensor": round(ft, 4),
+                         "bound": "hbm" if fh >= ft else "tensor", "queries/s": round(B / ((t + float(np.mean(fin))) * 1e-6), 1)})
+        rt.close()
+    return {"workload": "C4 N=10M d=384 bf16 (7.68 GB >> L2), scan kernel alone", "hbm_peak_GB/s": hbm_peak,
+            "tensor_peak_TFLOP/s": burst, "rows": rows}
 
 
 def measured_tensor_peaks():

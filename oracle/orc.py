@@ -241,3 +241,27 @@ def scan_fast_f32(bank, query):
     lib().orc_scan_fast_f32(_p(bank), _p(query), ctypes.c_int64(bank.shape[0]), bank.shape[1],
                             query.shape[0], _p(best))
     return best
+
+
+def matching_replay(scores0, quota, greedy=None):
+    """Batch-level matching replay ("A batch-level matching (e.g. Hungarian) ... an offline replay over the logged
+    score matrices"; reading 26): the assignment a of the B requests to instances that maximises
+    sum_r S0[r, a(r)] over the batch-start score matrix, with at most quota[i] requests on instance i and no request on
+    an instance filtered out for it (S0 = -inf).  The definition written out: every instance becomes min(quota, B)
+    identical slots and the one-to-one assignment problem on requests x slots is solved by the library routine
+    (scipy.optimize.linear_sum_assignment = the Hungarian/Jonker-Volgenant method the paper names).
+    Returns dict(match [B] int32, objective float (fp64 sum of the chosen fp32 scores), diverged int or None)."""
+    from scipy.optimize import linear_sum_assignment
+    S = np.asarray(scores0, dtype=np.float32)
+    B, I = S.shape
+    quota = np.asarray(quota, dtype=np.int64)
+    if quota.shape != (I,) or (quota < 0).any() or quota.sum() < B:
+        raise ValueError("quota must be I non-negative counts summing to at least B")
+    owner = np.repeat(np.arange(I), np.minimum(quota, B))
+    cost = S.astype(np.float64)[:, owner]
+    rows, cols = linear_sum_assignment(cost, maximize=True)     # raises when no feasible assignment exists
+    match = np.empty(B, dtype=np.int32)
+    match[rows] = owner[cols]
+    objective = float(S.astype(np.float64)[np.arange(B), match].sum())
+    diverged = None if greedy is None else int((match != np.asarray(greedy)).sum())
+    return dict(match=match, objective=objective, diverged=diverged)
