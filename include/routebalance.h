@@ -204,6 +204,22 @@ rb_status rb_decide_from_predictions_budgeted(rb_ctx* ctx, const float* quality,
                                               int32_t commit, int32_t* assignment, int32_t* max_tokens, float* scores,
                                               float* scores0, int32_t* order);
 
+/* Batch-level matching replay ("A batch-level matching (e.g. Hungarian) would differ only through within-batch
+ * state updates, and an offline replay over the logged score matrices changes 15.6% of assignments").  Finds the
+ * assignment a of the B requests that maximises sum_r scores0[r, a(r)] with at most quota[i] requests on instance i and
+ * none on an instance filtered out for the request (score -inf) -- the Hungarian method in shortest-augmenting-path form
+ * on the transportation problem, fp64 duals, one CTA -- and counts the requests it places differently from `greedy`.
+ * The paper does not say how its replay bounds an instance's share of a batch: the quota is the caller's (DESIGN.md
+ * reading 26); quota[i] >= B for all i makes the optimum the row-wise argmax.  An offline tool, not on the decision path.
+ *   scores0     [host|device] B x I fp32: the batch-start score matrix (rb_decide_from_predictions' scores0)
+ *   quota       [host|device] I int32 >= 0
+ *   greedy      [host|device] B int32 or NULL: assignment to compare with
+ *   match       [host|device] B int32: the optimal assignment (one of them, if several tie)
+ *   objective   [host] or NULL: sum of the chosen scores (fp64);   n_diverged [host] or NULL: #{r : match[r] != greedy[r]}
+ * 1 <= B <= 4096.  RB_EINVAL when no feasible assignment exists.  Synchronises the context's stream. */
+rb_status rb_match_replay(rb_ctx* ctx, const float* scores0, int32_t B, const int32_t* quota, const int32_t* greedy,
+                          int32_t* match, double* objective, int32_t* n_diverged);
+
 /* The estimate stage alone (KNN scan + merge + aggregate); outputs as in rb_decide, any may be NULL. */
 rb_status rb_estimate(rb_ctx* ctx, const float* query_emb, int32_t B, float* pred_quality,
                       float* pred_outlen, int32_t* nn_idx, float* nn_sim);
@@ -214,6 +230,11 @@ rb_status rb_estimate(rb_ctx* ctx, const float* query_emb, int32_t B, float* pre
  *   us [host] 6 floats: stage (query staging), scan, merge, aggregate, score, dispatch. */
 rb_status rb_set_stage_timing(rb_ctx* ctx, int32_t enabled);
 rb_status rb_last_stage_us(rb_ctx* ctx, float us[6]);
+
+/* Duration of the bank-scan kernel of the most recent rb_decide / rb_estimate that ran with stage timing enabled, on
+ * the device's own clock: latest CTA end - earliest CTA start (globaltimer), in microseconds; 0 if not measured (fp32
+ * storage, B > 128, or stage timing off).  Unlike the event interval in rb_last_stage_us it holds no launch latency. */
+rb_status rb_last_scan_device_us(rb_ctx* ctx, float* us);
 
 /* Self-test of the dispatch kernel's branch-free fp32 division (reciprocal refinement without the compiler's range check;
  * used only for operands inside the exponent window where it is exact, IEEE __fdiv_rn otherwise): compares it with the

@@ -26,7 +26,7 @@ RB_OK, RB_EINVAL, RB_ECUDA, RB_ENOMEM, RB_ESTATE, RB_EUNSUPPORTED = range(6)
 RB_F32, RB_BF16 = 0, 1
 _STATUS = {0: "RB_OK", 1: "RB_EINVAL", 2: "RB_ECUDA", 3: "RB_ENOMEM", 4: "RB_ESTATE", 5: "RB_EUNSUPPORTED"}
 EXPORTS = ["rb_options_default", "rb_create", "rb_set_instances", "rb_set_tpot_forest", "rb_set_telemetry", "rb_set_state", "rb_get_state", "rb_advance_state",
-           "rb_decide", "rb_decide_budgeted", "rb_decide_from_predictions", "rb_decide_from_predictions_budgeted", "rb_estimate", "rb_set_stage_timing", "rb_last_stage_us", "rb_selftest_division",
+           "rb_decide", "rb_decide_budgeted", "rb_decide_from_predictions", "rb_decide_from_predictions_budgeted", "rb_estimate", "rb_match_replay", "rb_set_stage_timing", "rb_last_stage_us", "rb_last_scan_device_us", "rb_selftest_division",
            "rb_launch_count", "rb_sync", "rb_last_error", "rb_destroy"]
 
 
@@ -68,9 +68,11 @@ _lib.rb_decide_from_predictions.argtypes = [_vp, _vp, _vp, _vp, _i32, ctypes.POI
 _lib.rb_decide_budgeted.argtypes = [_vp, _vp, _vp, _vp, _i32, ctypes.POINTER(_f * 3), _vp, _vp, _vp, _vp, _vp, _vp, _vp]
 _lib.rb_decide_from_predictions_budgeted.argtypes = [_vp, _vp, _vp, _vp, _vp, _i32, ctypes.POINTER(_f * 3), _i32, _vp, _vp,
                                                      _vp, _vp, _vp]
+_lib.rb_match_replay.argtypes = [_vp, _vp, _i32, _vp, _vp, _vp, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(_i32)]
 _lib.rb_estimate.argtypes = [_vp, _vp, _i32, _vp, _vp, _vp, _vp]
 _lib.rb_set_stage_timing.argtypes = [_vp, _i32]
 _lib.rb_last_stage_us.argtypes = [_vp, ctypes.POINTER(_f * 6)]
+_lib.rb_last_scan_device_us.argtypes = [_vp, ctypes.POINTER(_f)]
 _lib.rb_selftest_division.argtypes = [_vp, ctypes.c_uint64, ctypes.c_uint64, ctypes.POINTER(ctypes.c_uint64)]
 _lib.rb_launch_count.argtypes = [_vp]
 _lib.rb_launch_count.restype = _i64
@@ -209,6 +211,15 @@ def rb_decide_from_predictions_budgeted(ctx, quality, outlen, prompt_len, budget
                                                          _ptr(scores, f32), _ptr(scores0, f32), _ptr(order, i32)))
 
 
+def rb_match_replay(ctx, scores0, B, quota, greedy, match):
+    """Returns (objective, n_diverged); match is filled in place."""
+    f32, i32 = (torch.float32, torch.int32) if torch else (np.float32, np.int32)
+    obj, div = ctypes.c_double(0.0), _i32(0)
+    _check(ctx, _lib.rb_match_replay(ctx, _ptr(scores0, f32), B, _ptr(quota, i32), _ptr(greedy, i32), _ptr(match, i32),
+                                     ctypes.byref(obj), ctypes.byref(div)))
+    return float(obj.value), int(div.value)
+
+
 def rb_estimate(ctx, query_emb, B, pred_quality=None, pred_outlen=None, nn_idx=None, nn_sim=None):
     f32, i32 = (torch.float32, torch.int32) if torch else (np.float32, np.int32)
     _check(ctx, _lib.rb_estimate(ctx, _ptr(query_emb, f32), B, _ptr(pred_quality, f32), _ptr(pred_outlen, f32),
@@ -223,6 +234,12 @@ def rb_last_stage_us(ctx):
     us = (_f * 6)()
     _check(ctx, _lib.rb_last_stage_us(ctx, ctypes.byref(us)))
     return dict(zip(["stage", "scan", "merge", "aggregate", "score", "dispatch"], list(us)))
+
+
+def rb_last_scan_device_us(ctx):
+    us = _f(0.0)
+    _check(ctx, _lib.rb_last_scan_device_us(ctx, ctypes.byref(us)))
+    return float(us.value)
 
 
 def rb_selftest_division(ctx, n_pairs, seed=0):

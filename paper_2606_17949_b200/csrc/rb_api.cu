@@ -81,6 +81,8 @@ struct rb_ctx {
   bool stage_timing = false;
   cudaEvent_t ev[8]{};
   float stage_us[6]{};
+  unsigned long long* dev_clock = nullptr;   // [2] scan kernel's earliest CTA start / latest CTA end (stage-timing mode)
+  float scan_device_us = 0.0f;
   std::string err;
 };
 
@@ -207,6 +209,10 @@ rb_status enqueue_estimate(rb_ctx* ctx, int B, bool with_terms, Timer& tm) {
   fa.weight_mode = ctx->opt.weight_mode; fa.eps = ctx->opt.dist_eps; fa.with_terms = with_terms ? 1 : 0;
   fa.pred_q = ctx->pred_q; fa.pred_l = ctx->pred_l; fa.termA = ctx->termA; fa.termP = ctx->termP; fa.key = ctx->key;
   if (ctx->opt.store_dtype == RB_BF16) {
+    if (ctx->stage_timing) {   // before the first mark: nothing but the kernels between the stage events
+      static const unsigned long long init[2] = {~0ull, 0ull};
+      CK(cudaMemcpyAsync(ctx->dev_clock, init, sizeof init, cudaMemcpyHostToDevice, s));
+    }
     tm.mark();
     if (B > kTileM && ctx->num_sms >= 2) {
       // tensor-bound regime: CTA pairs, 256-query m-tiles
@@ -226,7 +232,7 @@ rb_status enqueue_estimate(rb_ctx* ctx, int B, bool with_terms, Timer& tm) {
       tm.mark();
       int grid = 0;
       CK(launch_scan_tc(&ctx->tm_q, &ctx->tm_bank, ctx->N, ctx->d, B, Bpad, ctx->ks, ctx->num_sms, ctx->part_sim,
-                        ctx->part_idx, &grid, s));
+                        ctx->part_idx, &grid, ctx->stage_timing ? ctx->dev_clock : nullptr, s));
       tm.mark();
       fa.part_sim = ctx->part_sim; fa.part_idx = ctx->part_idx; fa.nlists = grid * rep; fa.lists_per_cta = rep; fa.kcap = ctx->ks;
       fa.records = 1;
@@ -329,6 +335,12 @@ void collect_stage_times(rb_ctx* ctx, int kind) {
   if (!ctx->stage_timing) return;
   cudaStreamSynchronize(ctx->stream);
   for (float& v : ctx->stage_us) v = 0.0f;
+  {
+    unsigned long long h[2] = {0, 0};
+    ctx->scan_device_us = 0.0f;
+    if (cudaMemcpy(h, ctx->dev_clock, sizeof h, cudaMemcpyDeviceToHost) == cudaSuccess && h[1] > h[0] && h[0] != ~0ull)
+      ctx->scan_device_us = (float)((double)(h[1] - h[0]) * 1e-3);
+  }
   auto span = [&](int e0, int e1) {
     float ms = 0;
     return cudaEventElapsedTime(&ms, ctx->ev[e0], ctx->ev[e1]) == cudaSuccess ? ms * 1000.0f : 0.0f;
@@ -491,6 +503,8 @@ rb_status rb_create(rb_ctx** out, const void* bank_emb, const float* bank_qualit
   for (auto& e : ctx->ev) CK(cudaEventCreate(&e));
   for (auto& e : ctx->cp_ev) CK(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
   CK(cudaMallocHost((void**)&ctx->cp_ring, 64 * sizeof(CallParams)));
+  CK(cudaMalloc((void**)&ctx->dev_clock, 16));
+  CK(cudaMemset(ctx->dev_clock, 0, 16));
   cudaStream_t s = ctx->stream;
   const size_t nd = (size_t)N * d;
 #define ALLOC(ptr, n)                                                                 \
@@ -902,6 +916,60 @@ int rb_debug_timeline(rb_ctx* ctx, unsigned long long* out, int reset) {
 }
 #endif
 
+rb_status rb_match_replay(rb_ctx* ctx, const float* scores0, int32_t B, const int32_t* quota, const int32_t* greedy,
+                          int32_t* match, double* objective, int32_t* n_diverged) {
+  if (!ctx) return RB_EINVAL;
+  if (ctx->I == 0) return fail(ctx, RB_ESTATE, "rb_match_replay before rb_set_instances");
+  if (!scores0 || !quota || !match) return fail(ctx, RB_EINVAL, "NULL argument");
+  if (B < 1 || B > 4096) return fail(ctx, RB_EINVAL, "B out of range [1,4096]");
+  const int I = ctx->I;
+  cudaStream_t s = ctx->stream;
+  // offline tool: scratch is allocated per call
+  const size_t nS = (size_t)B * I * 4;
+  uint8_t* scratch = nullptr;
+  const size_t o_S = 0, o_q = (nS + 255) & ~(size_t)255, o_g = o_q + (((size_t)I * 4 + 255) & ~(size_t)255),
+               o_m = o_g + (((size_t)B * 4 + 255) & ~(size_t)255), o_out = o_m + (((size_t)B * 4 + 255) & ~(size_t)255);
+  if (cudaMalloc((void**)&scratch, o_out + 256) != cudaSuccess) {
+    cudaGetLastError();
+    return fail(ctx, RB_ENOMEM, "cudaMalloc (match replay scratch)");
+  }
+  auto done = [&](rb_status st) { cudaFree(scratch); return st; };
+  const float* dS = scores0;
+  const int32_t* dq = quota;
+  const int32_t* dg = greedy;
+  int32_t* dm = match;
+  cudaError_t e = cudaSuccess;
+  if (is_host_ptr(scores0)) { dS = (const float*)(scratch + o_S); e = cudaMemcpyAsync(scratch + o_S, scores0, nS, cudaMemcpyHostToDevice, s); }
+  if (e == cudaSuccess && is_host_ptr(quota)) { dq = (const int32_t*)(scratch + o_q); e = cudaMemcpyAsync(scratch + o_q, quota, (size_t)I * 4, cudaMemcpyHostToDevice, s); }
+  if (e == cudaSuccess && greedy && is_host_ptr(greedy)) { dg = (const int32_t*)(scratch + o_g); e = cudaMemcpyAsync(scratch + o_g, greedy, (size_t)B * 4, cudaMemcpyHostToDevice, s); }
+  const bool host_match = is_host_ptr(match);
+  if (host_match) dm = (int32_t*)(scratch + o_m);
+  double* d_obj = (double*)(scratch + o_out);
+  int32_t* d_div = (int32_t*)(scratch + o_out + 8);
+  int32_t* d_status = (int32_t*)(scratch + o_out + 12);
+  if (e == cudaSuccess) e = match_replay_prepare();
+  if (e == cudaSuccess) e = launch_match_replay(dS, B, I, dq, dg, dm, d_obj, d_div, d_status, s);
+  ctx->launches += 1;
+  struct { double obj; int32_t div; int32_t status; } h{};
+  if (e == cudaSuccess) e = cudaMemcpyAsync(&h, d_obj, 16, cudaMemcpyDeviceToHost, s);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+  if (e != cudaSuccess) return done(fail(ctx, RB_ECUDA, "rb_match_replay", e));
+  if (h.status != 0) return done(fail(ctx, RB_EINVAL, "no feasible assignment: the quotas of the admissible instances do not cover the batch"));
+  if (host_match) {
+    e = cudaMemcpy(match, dm, (size_t)B * 4, cudaMemcpyDeviceToHost);
+    if (e != cudaSuccess) return done(fail(ctx, RB_ECUDA, "cudaMemcpy (match)", e));
+  }
+  if (objective) *objective = h.obj;
+  if (n_diverged) *n_diverged = greedy ? h.div : 0;
+  return done(RB_OK);
+}
+
+rb_status rb_last_scan_device_us(rb_ctx* ctx, float* us) {
+  if (!ctx || !us) return RB_EINVAL;
+  *us = ctx->scan_device_us;
+  return RB_OK;
+}
+
 rb_status rb_selftest_division(rb_ctx* ctx, uint64_t n_pairs, uint64_t seed, uint64_t* mismatches) {
   if (!ctx || !mismatches) return RB_EINVAL;
   unsigned long long* dcount = nullptr;
@@ -933,7 +1001,7 @@ void rb_destroy(rb_ctx* ctx) {
   for (auto& kv : ctx->graphs) cudaGraphExecDestroy(kv.second);
   void* ptrs[] = {ctx->bank, ctx->bank_quality, ctx->bank_outlen, ctx->arena, ctx->q32, ctx->qs, ctx->part_sim,
                   ctx->gthr, ctx->sims, ctx->scratch_nn_idx, ctx->scratch_nn_sim, ctx->scores, ctx->scores0, ctx->f_nodes,
-                  ctx->f_root, ctx->f_begin, ctx->f_base};
+                  ctx->f_root, ctx->f_begin, ctx->f_base, ctx->dev_clock};
   for (void* p : ptrs) cudaFree(p);
   for (auto& e : ctx->ev)
     if (e) cudaEventDestroy(e);

@@ -194,6 +194,7 @@ int scan_tc_replicas(int B, int kcap, int max_grid);
 // rows are split over the CTAs in units of kBoxN rows: CTA c owns units [units*c/grid, units*(c+1)/grid).
 cudaError_t launch_scan_tc(const CUtensorMap* tm_q, const CUtensorMap* tm_bank, int64_t N, int d, int B, int Bpad,
                            int kcap, int max_grid, float* part_sim, int32_t* part_idx, int* grid_out,
+                           unsigned long long* dev_clock /* NULL, or [2] = {~0, 0}: earliest CTA start / latest CTA end (globaltimer ns) */,
                            cudaStream_t s);
 size_t scan_tc_smem_bytes();
 cudaError_t scan_tc_prepare();  // opt in to the dynamic shared memory size; call once
@@ -268,6 +269,12 @@ cudaError_t launch_tpot_forest(InstTable t, ForestDev forest, float* dq, int32_t
 
 // Counts pairs on which the dispatch loop's branch-free division differs from the IEEE one (must be 0).
 cudaError_t launch_div_selftest(unsigned long long n, unsigned long long seed, unsigned long long* mismatches, cudaStream_t s);
+
+// Batch-level matching replay: quota-constrained optimum of sum_r S0[r, a(r)], one CTA.
+// All pointers device; *status = 1 when no feasible assignment exists.
+cudaError_t launch_match_replay(const float* S0, int B, int I, const int32_t* quota, const int32_t* greedy, int32_t* match,
+                                double* objective, int32_t* n_diverged, int32_t* status, cudaStream_t s);
+cudaError_t match_replay_prepare();
 
 // a8: dead reckoning between batches.
 cudaError_t launch_advance(InstTable t, float* dq, int32_t* bq, float elapsed_ms, cudaStream_t s);

@@ -60,7 +60,8 @@ __device__ __forceinline__ bool tl_trace_end(int tid) { return tid == 128; }   /
 template <int KCAP>
 __global__ void __launch_bounds__(kThreads, 1)
 scan_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_bank, int64_t N, int d,
-               int B, int Bpad, int rep, float* __restrict__ part_sim, int32_t* __restrict__ part_idx) {
+               int B, int Bpad, int rep, float* __restrict__ part_sim, int32_t* __restrict__ part_idx,
+               unsigned long long* __restrict__ dev_clock) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);   // 128B swizzle wants 1024 B alignment
   uint2* cand = (uint2*)(smem + kStages * kStageBytes);   // [kCandSlots][128]: (similarity bits, column)
@@ -83,6 +84,11 @@ scan_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__
 
   launch_dependents();
   if (threadIdx.x == 0) { RB_TR(0); RB_STL(0); }
+  if (dev_clock != nullptr && threadIdx.x == 0) {   // stage-timing mode: earliest CTA start on the device's own clock
+    unsigned long long t0;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t0));
+    atomicMin(dev_clock, t0);
+  }
   if (warp == 0 && lane == 0) {
     asm volatile("prefetch.tensormap [%0];" ::"l"(&tm_q) : "memory");
     asm volatile("prefetch.tensormap [%0];" ::"l"(&tm_bank) : "memory");
@@ -260,9 +266,13 @@ scan_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__
         if (warp_active && r < B && (n_mt > 1 || tile == ntiles - 1)) {
 #pragma unroll
           for (int j = 0; j < KCAP / 4; ++j) {
-            prec[2 * j] = make_uint4(__float_as_uint(v[4 * j]), __float_as_uint(v[4 * j + 1]), __float_as_uint(v[4 * j + 2]),
-                                     __float_as_uint(v[4 * j + 3]));
-            prec[2 * j + 1] = make_uint4((uint32_t)ix[4 * j], (uint32_t)ix[4 * j + 1], (uint32_t)ix[4 * j + 2], (uint32_t)ix[4 * j + 3]);
+            // one 256-bit store per record: the whole 32-byte sector in one transaction (two 16-byte stores would each be
+            // a partial-sector write that L2 has to complete from DRAM)
+            asm volatile("st.global.v8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};" ::"l"(prec + 2 * j),
+                         "r"(__float_as_uint(v[4 * j])), "r"(__float_as_uint(v[4 * j + 1])), "r"(__float_as_uint(v[4 * j + 2])),
+                         "r"(__float_as_uint(v[4 * j + 3])), "r"((uint32_t)ix[4 * j]), "r"((uint32_t)ix[4 * j + 1]),
+                         "r"((uint32_t)ix[4 * j + 2]), "r"((uint32_t)ix[4 * j + 3])
+                         : "memory");
           }
         }
       }
@@ -273,6 +283,11 @@ scan_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__
   tc_fence_before();
   __syncthreads();
   if (threadIdx.x == 0) { RB_TR(3); RB_STL(1); }
+  if (dev_clock != nullptr && threadIdx.x == 0) {   // ... and latest CTA end
+    unsigned long long t1;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t1));
+    atomicMax(dev_clock + 1, t1);
+  }
   if (warp == 1) {
     tc_fence_after();
     asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(512) : "memory");
@@ -315,7 +330,8 @@ int scan_tc_replicas(int B, int kcap, int max_grid) {
 }
 
 cudaError_t launch_scan_tc(const CUtensorMap* tm_q, const CUtensorMap* tm_bank, int64_t N, int d, int B, int Bpad,
-                           int kcap, int max_grid, float* part_sim, int32_t* part_idx, int* grid_out, cudaStream_t s) {
+                           int kcap, int max_grid, float* part_sim, int32_t* part_idx, int* grid_out,
+                           unsigned long long* dev_clock, cudaStream_t s) {
   const int64_t units = (N + kBoxN - 1) / kBoxN;
   const int grid = (int)(units < max_grid ? units : max_grid);
   const int rep = scan_tc_replicas(B, kcap, max_grid);
@@ -323,7 +339,7 @@ cudaError_t launch_scan_tc(const CUtensorMap* tm_q, const CUtensorMap* tm_bank, 
   cudaError_t e = cudaSuccess;
 #define RB_SCAN_LAUNCH(KC)                                                                                          \
   e = launch_chained(scan_tc_kernel<KC>, dim3(grid), dim3(kThreads), kSmemBytes, s, *tm_q, *tm_bank, N, d, B, Bpad, rep, \
-                     part_sim, part_idx)
+                     part_sim, part_idx, dev_clock)
   switch (kcap) {
     case 4: RB_SCAN_LAUNCH(4); break;
     case 8: RB_SCAN_LAUNCH(8); break;

@@ -121,6 +121,14 @@ class Router:
                                       out["scores"], out["scores0"], out["order"])
         return out
 
+    def match_replay(self, scores0, quota, greedy=None):
+        """Quota-constrained optimum of the batch-start score matrix; returns (match, objective, n_diverged)."""
+        B = scores0.shape[0]
+        match = torch.empty(B, dtype=torch.int32, device=scores0.device)
+        obj, div = rb.rb_match_replay(self.ctx, scores0.contiguous(), B, quota.contiguous().to(torch.int32),
+                                      None if greedy is None else greedy.contiguous().to(torch.int32), match)
+        return match, obj, div
+
     def sync(self):
         rb.rb_sync(self.ctx)
 
@@ -129,6 +137,9 @@ class Router:
 
     def stage_us(self):
         return rb.rb_last_stage_us(self.ctx)
+
+    def scan_device_us(self):
+        return rb.rb_last_scan_device_us(self.ctx)
 
     def set_stage_timing(self, on):
         rb.rb_set_stage_timing(self.ctx, on)

@@ -561,3 +561,69 @@ def test_deferred_advance_is_applied_in_call_order(orc):
     s = rt.get_state()
     assert np.array_equal(s[0].numpy(), queued.numpy()) and np.array_equal(s[1].numpy(), running.numpy())
     rt.close()
+
+
+@pytest.mark.parametrize("B,I,qmax", [(1, 1, 1), (6, 3, 3), (16, 13, 2), (64, 13, 8), (200, 64, 5), (1024, 256, 6), (300, 7, 60)])
+def test_match_replay_reaches_the_oracle_optimum(orc, B, I, qmax):
+    """quota-constrained optimum of the batch-start score matrix.  Several optimal assignments may
+    exist, so what is compared is what is unique -- the objective (fp64 sum of the chosen fp32 scores) -- and the rest
+    is checked for validity: quotas respected, no filtered (-inf) pair chosen, divergence count consistent."""
+    from paper_2606_17949_b200.router import Router
+    rng = np.random.default_rng(1000 + B + I)
+    M = min(4, I)
+    it = synth.make_instances(I, M)
+    rt = Router(torch.randn(64, 16).cuda(), torch.rand(64, M).cuda(), torch.rand(64, M).cuda() + 1, 4, store="f32", max_batch=8)
+    rt.set_instances(**it)
+    for trial in range(3):
+        S = rng.uniform(0, 1, (B, I)).astype(np.float32)
+        if trial == 1:
+            S = np.round(S * 8) / 8                                  # many exact ties
+        if trial == 2 and I > 1:
+            S[rng.uniform(size=S.shape) < 0.3] = -np.inf             # budget-filtered pairs
+            S[np.arange(B), rng.integers(0, I, B)] = rng.uniform(0, 1, B).astype(np.float32)   # every request keeps one
+        quota = rng.integers(0, qmax + 1, I)
+        while quota.sum() < B + I:
+            quota[rng.integers(0, I)] += 1
+        greedy = np.where(np.isfinite(S), S, -2).argmax(axis=1).astype(np.int32)
+        try:
+            ref = orc.matching_replay(S, quota, greedy)
+        except ValueError:
+            with pytest.raises(Exception):
+                rt.match_replay(torch.from_numpy(S).cuda(), torch.from_numpy(quota.astype(np.int32)).cuda())
+            continue
+        for host in (False, True):
+            St, qt, gt = torch.from_numpy(S), torch.from_numpy(quota.astype(np.int32)), torch.from_numpy(greedy)
+            if not host:
+                St, qt, gt = St.cuda(), qt.cuda(), gt.cuda()
+            match, obj, div = rt.match_replay(St, qt, gt)
+            m = match.cpu().numpy()
+            assert abs(obj - ref["objective"]) <= 1e-9 * B, (obj, ref["objective"])
+            assert abs(float(S.astype(np.float64)[np.arange(B), m].sum()) - obj) <= 1e-9 * B
+            assert (np.bincount(m, minlength=I) <= quota).all() and np.isfinite(S[np.arange(B), m]).all()
+            assert div == int((m != greedy).sum())
+    # loose quotas: the objective decomposes per request (P:L80) -> row-wise argmax, nothing diverges
+    S = rng.uniform(0, 1, (B, I)).astype(np.float32)
+    g = S.argmax(axis=1).astype(np.int32)
+    match, obj, div = rt.match_replay(torch.from_numpy(S).cuda(), torch.full((I,), B, dtype=torch.int32).cuda(), torch.from_numpy(g).cuda())
+    assert np.array_equal(match.cpu().numpy(), g) and div == 0
+    with pytest.raises(Exception):
+        rt.match_replay(torch.from_numpy(S).cuda(), torch.zeros(I, dtype=torch.int32).cuda())
+    rt.close()
+
+
+def test_match_replay_on_a_real_score_matrix(orc):
+    """The replay the paper describes: scores0 of a C5-shaped batch (B=1024, I=256) from the library itself, quota = 6
+    requests per instance; objective against the oracle, and the greedy-vs-matching divergence is reported."""
+    cfg = dataclasses.replace(synth.CONFIGS["C5"], N=50000, d=128)
+    bank, it, queued, running, query, plen, rt = _setup(cfg, max_batch=cfg.B)
+    est = rt.estimate(query)
+    w = synth.PRESETS["balanced"]
+    out = rt.decide_from_predictions(est["pred_quality"], est["pred_outlen"], plen, w, commit=0)
+    quota = torch.full((cfg.I,), 6, dtype=torch.int32, device="cuda")
+    match, obj, div = rt.match_replay(out["scores0"], quota, out["assignment"])
+    ref = orc.matching_replay(out["scores0"].cpu().numpy(), np.full(cfg.I, 6), out["assignment"].cpu().numpy())
+    assert abs(obj - ref["objective"]) <= 1e-9 * cfg.B
+    m = match.cpu().numpy()
+    assert (np.bincount(m, minlength=cfg.I) <= 6).all()
+    assert 0 <= div <= cfg.B
+    rt.close()
