@@ -63,6 +63,11 @@ struct rb_ctx {
   int32_t *order = nullptr, *assignment = nullptr, *max_tokens = nullptr;
   float* budget = nullptr;          // [max_batch] staging of host budgets
   uint8_t* arena = nullptr;         // one allocation behind all the small per-decision buffers
+  // Host callers of rb_decide: inputs are copied (host memcpy) into this pinned block, which the kernels read over the
+  // bus directly, and the assignment is written into it by the dispatch kernel -- no copy-engine transfers on the path.
+  uint8_t* h_zc = nullptr;          // pinned host block: [query | plen | budget | assignment]
+  uint8_t* d_zc = nullptr;          // the same block as the device addresses it
+  size_t zc_query_cap = 0, zc_off_plen = 0, zc_off_budget = 0, zc_off_assign = 0;
   // boosted TPOT head (latency_mode 2)
   int4* f_nodes = nullptr;
   int32_t *f_root = nullptr, *f_begin = nullptr;
@@ -384,6 +389,26 @@ struct Stager {
   struct Back { void* dst; const void* src; size_t bytes; };
   Back back[10];
   int nback = 0;
+  Back hback[2];   // host memcpys out of the pinned block, after the stream has drained
+  int nhback = 0;
+  // host input of at most `cap` bytes -> pinned block at `off`, read by the kernels in place
+  template <typename T>
+  const T* in_zc(const T* user, size_t off, size_t cap, T* staging, size_t bytes) {
+    if (!is_host_ptr(user)) return user;
+    if (ctx->h_zc == nullptr || bytes > cap) return in(user, staging, bytes);
+    any_host = true;
+    std::memcpy(ctx->h_zc + off, user, bytes);
+    return reinterpret_cast<const T*>(ctx->d_zc + off);
+  }
+  template <typename T>
+  T* out_zc(T* user, size_t off, T* staging, size_t bytes) {
+    if (!user) return nullptr;
+    if (!is_host_ptr(user)) return user;
+    if (ctx->h_zc == nullptr) return out(user, staging, bytes);
+    any_host = true;
+    hback[nhback++] = Back{user, ctx->h_zc + off, bytes};
+    return reinterpret_cast<T*>(ctx->d_zc + off);
+  }
   template <typename T>
   const T* in(const T* user, T* staging, size_t bytes) {
     if (!is_host_ptr(user)) return user;
@@ -415,6 +440,7 @@ struct Stager {
     if (err != cudaSuccess) return fail(ctx, RB_ECUDA, "cudaMemcpyAsync (outputs)", err);
     // host-side inputs must be consumed and host-side outputs complete before returning
     if (any_host) CK(cudaStreamSynchronize(ctx->stream));
+    for (int j = 0; j < nhback; ++j) std::memcpy(hback[j].dst, hback[j].src, hback[j].bytes);
     return RB_OK;
   }
 };
@@ -487,7 +513,9 @@ rb_status rb_create(rb_ctx** out, const void* bank_emb, const float* bank_qualit
     const int64_t grid = units < ctx->num_sms ? units : ctx->num_sms;
     const int64_t rows_per_cta = N / grid;
     int ks = opt.scan_list;
-    if (ks == 0) ks = rows_per_cta >= 16384 ? ctx->kcap : (rows_per_cta >= 2048 ? 8 : 4);
+    // (long slabs amortise the warm-up of a longer list, but past 16 entries the lock-step insertions of an
+    // epilogue warp -- about KS*ln(rows/KS) per query, each ~6*KS instructions -- outgrow the time a tile's bytes take)
+    if (ks == 0) ks = rows_per_cta >= 16384 ? std::min(ctx->kcap, 16) : (rows_per_cta >= 2048 ? 8 : 4);
     if (ks > ctx->kcap) ks = ctx->kcap;
     ctx->ks = ks;
   }
@@ -503,6 +531,23 @@ rb_status rb_create(rb_ctx** out, const void* bank_emb, const float* bank_qualit
   for (auto& e : ctx->ev) CK(cudaEventCreate(&e));
   for (auto& e : ctx->cp_ev) CK(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
   CK(cudaMallocHost((void**)&ctx->cp_ring, 64 * sizeof(CallParams)));
+  {
+    const size_t mbz = (size_t)opt.max_batch;
+    ctx->zc_query_cap = std::min<size_t>(mbz * d * 4, (size_t)1 << 20);
+    ctx->zc_off_plen = (ctx->zc_query_cap + 255) & ~(size_t)255;
+    ctx->zc_off_budget = ctx->zc_off_plen + ((mbz * 4 + 255) & ~(size_t)255);
+    ctx->zc_off_assign = ctx->zc_off_budget + ((mbz * 4 + 255) & ~(size_t)255);
+    const size_t total = ctx->zc_off_assign + ((mbz * 4 + 255) & ~(size_t)255);
+    if (cudaHostAlloc((void**)&ctx->h_zc, total, cudaHostAllocMapped) == cudaSuccess &&
+        cudaHostGetDevicePointer((void**)&ctx->d_zc, ctx->h_zc, 0) == cudaSuccess) {
+      std::memset(ctx->h_zc, 0, total);
+    } else {   // no mapped pinned memory: host callers go through the copy engine
+      cudaGetLastError();
+      if (ctx->h_zc) cudaFreeHost(ctx->h_zc);
+      ctx->h_zc = nullptr;
+      ctx->d_zc = nullptr;
+    }
+  }
   CK(cudaMalloc((void**)&ctx->dev_clock, 16));
   CK(cudaMemset(ctx->dev_clock, 0, 16));
   cudaStream_t s = ctx->stream;
@@ -805,12 +850,15 @@ rb_status rb_decide_budgeted(rb_ctx* ctx, const float* query_emb, const int32_t*
     st = flush_pending(ctx);
     if (st != RB_OK) return st;
   }
-  cp.query = sg.in(query_emb, ctx->q32, (size_t)B * ctx->d * 4);
-  cp.plen = sg.in(prompt_len, ctx->plen, (size_t)B * 4);
+  // (the fp32-storage scan reads every query from every block: it wants them in device memory)
+  cp.query = sg.in_zc(query_emb, 0, ctx->opt.store_dtype == RB_BF16 ? ctx->zc_query_cap : 0, ctx->q32, (size_t)B * ctx->d * 4);
+  cp.plen = sg.in_zc(prompt_len, ctx->zc_off_plen, (size_t)B * 4, ctx->plen, (size_t)B * 4);
   cp.q_src = ctx->pred_q;
   cp.l_src = ctx->pred_l;
-  cp.budget = budget ? sg.in(budget, ctx->budget, (size_t)B * 4) : nullptr;
-  cp.assignment = sg.out(assignment, ctx->assignment, (size_t)B * 4);
+  cp.budget = budget ? sg.in_zc(budget, ctx->zc_off_budget, (size_t)B * 4, ctx->budget, (size_t)B * 4) : nullptr;
+  // (with max_tokens the dispatch kernel reads the assignment back: it then stays in device memory)
+  cp.assignment = max_tokens ? sg.out(assignment, ctx->assignment, (size_t)B * 4)
+                             : sg.out_zc(assignment, ctx->zc_off_assign, ctx->assignment, (size_t)B * 4);
   cp.max_tokens = sg.out(max_tokens, ctx->max_tokens, (size_t)B * 4);
   cp.scores = sg.out(scores, ctx->scores, (size_t)B * ctx->I * 4);
   cp.pred_q = sg.out_internal(pred_quality, ctx->pred_q, bm);
@@ -1008,6 +1056,7 @@ void rb_destroy(rb_ctx* ctx) {
   for (auto& e : ctx->cp_ev)
     if (e) cudaEventDestroy(e);
   if (ctx->cp_ring) cudaFreeHost(ctx->cp_ring);
+  if (ctx->h_zc) cudaFreeHost(ctx->h_zc);
   if (ctx->own_stream) cudaStreamDestroy(ctx->stream);
   delete ctx;
 }
