@@ -326,6 +326,8 @@ finish_kernel(FinishArgs a, InstTable t, const CallParams* __restrict__ cp) {
         const int e = e0 + u * kFinThreads;
         if (e < nquads) {
           if (a.records) {   // record e of this query: [4 similarities | 4 indices], contiguous over e
+            // (a list-major layout of the same records was tried: the 4 KB stride between a query's records costs the
+            // finishing CTA ~3000 cycles more than this contiguous run)
             const uint4* rec = reinterpret_cast<const uint4*>(a.part_sim) + ((size_t)r * nquads + e) * 2;
             const uint4 ua = __ldcg(rec), ub = __ldcg(rec + 1);
             sv[u] = make_float4(__uint_as_float(ua.x), __uint_as_float(ua.y), __uint_as_float(ua.z), __uint_as_float(ua.w));

@@ -116,33 +116,16 @@ scan_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__
   if (warp == 0) {
     // ===== TMA producer =====
     if (lane == 0) {
-      // The bank does not depend on the preceding (staging) kernel, the staged queries do: the first ring slots get
-      // their bank boxes before the dependency resolves, their query tiles after it -- the HBM stream starts while
-      // the staging kernel still runs.
-      const int per_tile = n_mt * nk;
-      const int total_it = ntiles * per_tile;
-      const int npre = min(kStages, total_it);
-      for (int kit = 0; kit < npre; ++kit) {
-        const int tile = kit / per_tile, kc = (kit - tile * per_tile) % nk;
-        const int n0 = (int)(row0 + (int64_t)tile * kTileN);
-        const int nun = min(4, nunits - tile * 4);
-        uint8_t* sb = smem + kit * kStageBytes + kABytes;
-        mbar_arrive_expect_tx(&full[kit], kABytes + nun * kBoxBytes);
-        for (int u = 0; u < nun; ++u) tma_load_2d(sb + u * kBoxBytes, &tm_bank, kc * kTileK, n0 + u * kBoxN, &full[kit]);
-      }
+      grid_dependency_wait();   // the staged queries come from the preceding kernel (it ends about when this
+                                // kernel's prologue does: issuing bank boxes ahead of the wait only delayed the
+                                // first query tile behind them -- measured, reverted)
       RB_STL(2);
-      grid_dependency_wait();   // the staged queries come from the preceding kernel
-      for (int kit = 0; kit < npre; ++kit) {
-        const int tile = kit / per_tile, rem = kit - tile * per_tile;
-        tma_load_2d(smem + kit * kStageBytes, &tm_q, (rem % nk) * kTileK, (rem / nk) * kTileM, &full[kit]);
-      }
       uint32_t kit = 0;
       for (int tile = 0; tile < ntiles; ++tile) {
         const int n0 = (int)(row0 + (int64_t)tile * kTileN);
         const int nun = min(4, nunits - tile * 4);
         for (int mt = 0; mt < n_mt; ++mt) {
           for (int kc = 0; kc < nk; ++kc, ++kit) {
-            if ((int)kit < npre) continue;   // issued above
             const int s = kit % kStages;
             const uint32_t ph = (kit / kStages) & 1;
             mbar_wait(&empty[s], ph ^ 1);
