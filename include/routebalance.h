@@ -226,7 +226,8 @@ rb_status rb_estimate(rb_ctx* ctx, const float* query_emb, int32_t B, float* pre
 
 /* Device time of the stages of the most recent rb_decide / rb_estimate on this context, measured with
  * CUDA events on the context's stream (only when the call ran with stage timing enabled through
- * rb_set_stage_timing(ctx, 1), which also disables graph replay for that context).
+ * rb_set_stage_timing(ctx, 1); the decision is then replayed from a graph with event-record nodes between its kernels,
+ * which serialises them: each stage's interval is meaningful, their sum is longer than an untimed decision).
  *   us [host] 6 floats: stage (query staging), scan, merge, aggregate, score, dispatch. */
 rb_status rb_set_stage_timing(rb_ctx* ctx, int32_t enabled);
 rb_status rb_last_stage_us(rb_ctx* ctx, float us[6]);

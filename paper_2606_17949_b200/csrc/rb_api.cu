@@ -84,9 +84,11 @@ struct rb_ctx {
   std::unordered_map<int64_t, int> graph_nodes;
   int64_t launches = 0;
   bool stage_timing = false;
+  bool capturing = false;
   cudaEvent_t ev[8]{};
   float stage_us[6]{};
   unsigned long long* dev_clock = nullptr;   // [2] scan kernel's earliest CTA start / latest CTA end (stage-timing mode)
+  unsigned long long* dev_clock_init = nullptr;   // [2] = {~0, 0} in device memory
   float scan_device_us = 0.0f;
   std::string err;
 };
@@ -200,7 +202,8 @@ struct Timer {
   int idx = 0;
   explicit Timer(rb_ctx* c_) : c(c_) {}
   void mark() {
-    if (c->stage_timing) cudaEventRecord(c->ev[idx++], c->stream);
+    // (inside a capture the record becomes an event node of the graph; "external" keeps the event usable for timing)
+    if (c->stage_timing) cudaEventRecordWithFlags(c->ev[idx++], c->stream, c->capturing ? cudaEventRecordExternal : cudaEventRecordDefault);
   }
 };
 
@@ -215,8 +218,7 @@ rb_status enqueue_estimate(rb_ctx* ctx, int B, bool with_terms, Timer& tm) {
   fa.pred_q = ctx->pred_q; fa.pred_l = ctx->pred_l; fa.termA = ctx->termA; fa.termP = ctx->termP; fa.key = ctx->key;
   if (ctx->opt.store_dtype == RB_BF16) {
     if (ctx->stage_timing) {   // before the first mark: nothing but the kernels between the stage events
-      static const unsigned long long init[2] = {~0ull, 0ull};
-      CK(cudaMemcpyAsync(ctx->dev_clock, init, sizeof init, cudaMemcpyHostToDevice, s));
+      CK(cudaMemcpyAsync(ctx->dev_clock, ctx->dev_clock_init, 16, cudaMemcpyDeviceToDevice, s));
     }
     tm.mark();
     if (B > kTileM && ctx->num_sms >= 2) {
@@ -288,7 +290,11 @@ rb_status enqueue_dispatch(rb_ctx* ctx, int B, bool from_predictions, Timer& tm)
 
 // kind: 0 = estimate + dispatch, 1 = estimate, 2 = dispatch (+scores0)
 rb_status run_path(rb_ctx* ctx, int B, int kind) {
-  const bool graph = ctx->opt.use_graph && !ctx->stage_timing;
+  // With stage timing on, the same launch sequence is captured with event-record nodes between the kernels (a
+  // separate graph per shape): the stage intervals then hold graph-internal launch latencies like a decision's, not
+  // host-side ones.  The kernels lose their programmatic overlap across the event nodes, so the SUM of the stages is
+  // longer than a decision; each stage's own duration is what is read.
+  const bool graph = ctx->opt.use_graph != 0;
   Timer tm(ctx);
   if (!graph) {
     if (kind == 0 && ctx->opt.latency_mode == 2) {   // the head over the batch-start state; only the state feeds it
@@ -302,12 +308,13 @@ rb_status run_path(rb_ctx* ctx, int B, int kind) {
     if (kind != 1) return enqueue_dispatch(ctx, B, kind == 2, tm);
     return RB_OK;
   }
-  const int64_t gkey = (int64_t)B * 4 + kind;
+  const int64_t gkey = (int64_t)B * 8 + kind + (ctx->stage_timing ? 4 : 0);
   auto it = ctx->graphs.find(gkey);
   if (it == ctx->graphs.end()) {
     const int64_t before = ctx->launches;
     cudaGraph_t g = nullptr;
     CK(cudaStreamBeginCapture(ctx->stream, cudaStreamCaptureModeThreadLocal));
+    ctx->capturing = true;
     rb_status st = RB_OK;
     if (kind == 0 && ctx->opt.latency_mode == 2) {
       if (launch_tpot_forest(table_of(ctx), forest_of(ctx), ctx->dq, ctx->bq, ctx->f_tpot0, -1.0f, ctx->stream) != cudaSuccess)
@@ -317,6 +324,7 @@ rb_status run_path(rb_ctx* ctx, int B, int kind) {
     if (st == RB_OK && kind != 2) st = enqueue_estimate(ctx, B, kind == 0, tm);
     if (st == RB_OK && kind != 1) st = enqueue_dispatch(ctx, B, kind == 2, tm);
     cudaError_t e = cudaStreamEndCapture(ctx->stream, &g);
+    ctx->capturing = false;
     const int nodes = (int)(ctx->launches - before);
     ctx->launches = before;
     if (st != RB_OK) {
@@ -548,8 +556,12 @@ rb_status rb_create(rb_ctx** out, const void* bank_emb, const float* bank_qualit
       ctx->d_zc = nullptr;
     }
   }
-  CK(cudaMalloc((void**)&ctx->dev_clock, 16));
-  CK(cudaMemset(ctx->dev_clock, 0, 16));
+  CK(cudaMalloc((void**)&ctx->dev_clock, 32));
+  ctx->dev_clock_init = ctx->dev_clock + 2;
+  {
+    const unsigned long long init[4] = {0ull, 0ull, ~0ull, 0ull};
+    CK(cudaMemcpy(ctx->dev_clock, init, sizeof init, cudaMemcpyHostToDevice));
+  }
   cudaStream_t s = ctx->stream;
   const size_t nd = (size_t)N * d;
 #define ALLOC(ptr, n)                                                                 \
