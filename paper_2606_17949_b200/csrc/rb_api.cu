@@ -228,11 +228,15 @@ rb_status enqueue_estimate(rb_ctx* ctx, int B, bool with_terms, Timer& tm) {
                               Bpad2 * (1 + scan_tc2_clusters(ctx->N, ctx->num_sms)), table_of(ctx), ctx->dq, ctx->bq, s));
       tm.mark();
       int ncl = 0;
-      CK(launch_scan_tc2(&ctx->tm_q, &ctx->tm_bank, ctx->N, ctx->d, B, Bpad2, ctx->kcap, ctx->kc, ctx->num_sms, ctx->part_sim,
+      // lists of at most 16 entries per (cluster, query): longer ones put the sorted insertions (in global memory) on the
+      // tensor pipe's time line (k = 32: 0.54 of the tensor roofline with 64-entry lists); a cluster whose list is
+      // popped completely is searched again by the finishing kernel, as for the single-CTA scan
+      const int kcap2 = std::min(ctx->kcap, 16);
+      CK(launch_scan_tc2(&ctx->tm_q, &ctx->tm_bank, ctx->N, ctx->d, B, Bpad2, kcap2, ctx->kc, ctx->num_sms, ctx->part_sim,
                          ctx->part_idx, ctx->gthr, &ncl, s));
       tm.mark();
-      fa.part_sim = ctx->part_sim; fa.part_idx = ctx->part_idx; fa.nlists = ncl; fa.lists_per_cta = 1; fa.kcap = ctx->kcap;
-      fa.Bpad = Bpad2; fa.slab_unit = kTileN; fa.rescan = 0;   // full-length lists (K >= k + slack): nothing hidden
+      fa.part_sim = ctx->part_sim; fa.part_idx = ctx->part_idx; fa.nlists = ncl; fa.lists_per_cta = 1; fa.kcap = kcap2;
+      fa.Bpad = Bpad2; fa.slab_unit = kTileN; fa.rescan = kcap2 < ctx->kc ? 1 : 0;
     } else {
       const int rep = scan_tc_replicas(B, ctx->ks, ctx->num_sms);
       CK(launch_stage_queries(ctx->cp, ctx->qs, B, Bpad, ctx->d, rep, ctx->gthr, Bpad, table_of(ctx), ctx->dq, ctx->bq, s));

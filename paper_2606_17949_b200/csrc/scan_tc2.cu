@@ -189,7 +189,8 @@ __device__ __forceinline__ void park_chunk(const uint32_t (&regs)[32], int c0, i
 template <int KCAP>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads2, 1)
 scan_tc2_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_bank, int64_t N, int d,
-                int B, int Bpad, float* part_sim, int32_t* part_idx, uint32_t* gthr, int pub_j, int pub_groups) {
+                int B, int Bpad, float* part_sim, int32_t* part_idx, uint32_t* gthr, int pub_j, int pub_groups,
+                int publish_own) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
   uint2* cand = (uint2*)(smem + kStages2 * kStage2Bytes);
@@ -409,7 +410,8 @@ scan_tc2_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant_
           }
           const float own = st.v[KCAP - 1];
           thr_s[mp * kTileM + tl] = own;
-          if (own > -INFINITY) atomicMax(gthr + r, f32_ordered(own));
+          // (a list shorter than k + slack proves nothing about the global (k + slack)-th best: only the pooled bound then)
+          if (publish_own && own > -INFINITY) atomicMax(gthr + r, f32_ordered(own));
           const float pj = pub_j == 1 ? st.v[0] : (pub_j == 2 ? st.v[1] : (pub_j == 3 ? st.v[2] : st.v[3]));
           if (pj > -INFINITY) gthr[(size_t)Bpad * (1 + cl) + r] = f32_ordered(pj);
         }
@@ -513,7 +515,7 @@ cudaError_t launch_scan_tc2(const CUtensorMap* tm_q, const CUtensorMap* tm_bank,
   cudaError_t e = cudaSuccess;
 #define RB_SCAN2_LAUNCH(KC)                                                                                       \
   e = launch_chained(scan_tc2_kernel<KC>, dim3(2 * ncl), dim3(kThreads2), kSmem2Bytes, s, *tm_q, *tm_bank, N, d, B, Bpad, \
-                     part_sim, part_idx, gthr, pub_j, pub_groups)
+                     part_sim, part_idx, gthr, pub_j, pub_groups, kcap >= kc ? 1 : 0)
   switch (kcap) {
     case 4: RB_SCAN2_LAUNCH(4); break;
     case 8: RB_SCAN2_LAUNCH(8); break;
