@@ -24,6 +24,7 @@ One JSON line is printed by rank 0:
                same stream
   scan_c4      BASELINE.json configs[3] (N=10M x d=384 bf16 = 7.68 GB, B=64): the scan kernel alone against
                the HBM roofline -- the north-star's ">= 70 % of the HBM roofline" figure (bank >> L2)
+  p0_paper_shape  the paper's own bank / cluster shape over its k sweep and batch sizes (context row)
   sweep_c4     the whole configs[3] sweep: B in {1, 8, 64, 512, 4096} x k in {10, 32}, GB/s and TFLOP/s of the scan
   scan_c3      configs[2] (N=1M x d=1024, B=1024): the CTA-pair scan kernel against the tensor roofline
   sweep_c5     configs[4]: 66 simplex points of score + LPT dispatch from fixed predictions (linear and boosted head)
@@ -358,6 +359,7 @@ def run_ours(args):
         if not args.no_scan_c4:
             out["scan_c4"] = scan_c4(synth, Router, dev, hbm_peak)
         if not args.no_large:
+            out["p0_paper_shape"] = paper_shape_p0(synth, Router, dev)
             out["sweep_c4"] = sweep_c4(synth, Router, dev, hbm_peak)
             out["scan_c3"] = scan_c3(synth, Router, dev)
             out["sweep_c5"] = sweep_c5(synth, Router, dev)
@@ -475,6 +477,46 @@ def sweep_c4(synth, Router, dev, hbm_peak):
         rt.close()
     return {"workload": "C4 N=10M d=384 bf16 (7.68 GB >> L2), scan kernel alone", "hbm_peak_GB/s": hbm_peak,
             "tensor_peak_TFLOP/s": burst, "rows": rows}
+
+
+def paper_shape_p0(synth, Router, dev):
+    """The paper's own shape (context row, SURVEY 8d "P0"): bank 14,919 x 384, the 13 instances of Table 1
+    (P:L57-64), k in {5, 10, 20, 50}, B in {1, 16, 32} (the paper's fixed batch sizes): device time of
+    one whole decision (graph replay, L2 warm: the 11.5 MB bank is L2-resident), beside the paper's 28-32 ms per request
+    on its 96-core CPU host, sentence encoder included."""
+    import dataclasses
+    import torch
+    base = synth.CONFIGS["P0"]
+    it = synth.paper_cluster()
+    rows = []
+    for k in (5, 10, 20, 50):
+        cfg = dataclasses.replace(base, k=k, store="bf16")
+        bank = synth.make_bank(cfg, device=dev)
+        queued, running = synth.make_state(cfg.I, it["cap"], cfg.seed)
+        rt = Router(bank["emb"], bank["quality"], bank["outlen"], k, store="bf16", max_batch=32, device=dev)
+        rt.set_instances(**it)
+        rt.set_state(queued, running)
+        for B in (1, 16, 32):
+            q = synth.make_queries(cfg, B=B, device=dev)
+            p = synth.make_prompt_len(cfg, B=B, device=dev)
+            a = torch.empty(B, dtype=torch.int32, device=dev)
+            w = synth.PRESETS["balanced"]
+            from paper_2606_17949_b200 import binding as rb
+            for _ in range(5):
+                rb.rb_decide(rt.ctx, q, p, B, w, a)
+            rt.sync()
+            n = 100
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(rt.stream)
+            for _ in range(n):
+                rb.rb_decide(rt.ctx, q, p, B, w, a)
+            e1.record(rt.stream)
+            rt.sync()
+            us = e0.elapsed_time(e1) * 1e3 / n
+            rows.append({"k": k, "B": B, "decision_us": round(us, 1), "us_per_request": round(us / B, 2)})
+        rt.close()
+    return {"workload": "P0 paper-exact shape: N=14,919 d=384 bf16, Table 1 cluster (I=13, M=4), back-to-back decisions",
+            "rows": rows, "paper_context": "paper: 28-32 ms per request on its CPU host, encoder included (P:L133, Table 4)"}
 
 
 def measured_tensor_peaks():

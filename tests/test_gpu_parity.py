@@ -627,3 +627,32 @@ def test_match_replay_on_a_real_score_matrix(orc):
     assert (np.bincount(m, minlength=cfg.I) <= 6).all()
     assert 0 <= div <= cfg.B
     rt.close()
+
+
+@pytest.mark.parametrize("k,slack", [(5, 6), (20, 6), (50, 6), (50, 14)])
+@pytest.mark.parametrize("store", ["bf16", "f32"])
+def test_paper_shape_k_sweep(orc, k, slack, store):
+    """P0: the paper's own shape (bank of 14,919 prompts x 384, 13 instances of Table 1) over its k
+    sweep {5, 20, 50} at its fixed batch size 32, both storage modes, full parity."""
+    cfg = dataclasses.replace(synth.CONFIGS["P0"], k=k, store=store)
+    bank = synth.make_bank(cfg, device="cuda")
+    it = synth.paper_cluster()
+    queued, running = synth.make_state(cfg.I, it["cap"], cfg.seed)
+    query = synth.make_queries(cfg, device="cuda")
+    plen = synth.make_prompt_len(cfg, device="cuda")
+    torch.cuda.synchronize()
+    rt = _router(bank, cfg, max_batch=32, rerank_slack=slack if store == "bf16" else 0)
+    rt.set_instances(**it)
+    rt.set_state(queued, running)
+    w = synth.PRESETS["balanced"]
+    g = _np(rt.decide(query, plen, w))
+    bank_np = parity.bank_to_numpy(bank["emb"])
+    qn, ln = bank["quality"].cpu().numpy(), bank["outlen"].cpu().numpy()
+    log = []
+    oi, os_, near = parity.check_topk(orc, bank_np, query.cpu().numpy(), store, k, g["nn_idx"], g["nn_sim"], 0.0, log)
+    parity.check_predictions(orc, g["pred_quality"], g["pred_outlen"], g["nn_idx"], g["nn_sim"], oi, os_, near, qn, ln)
+    s = rt.get_state()
+    parity.check_dispatch(orc, orc.Instances(**it), queued.numpy(), running.numpy(), g["pred_quality"], g["pred_outlen"],
+                          plen.cpu().numpy(), w, g, state_after=(s[0].numpy(), s[1].numpy()))
+    assert len(near) <= 2, log
+    rt.close()
