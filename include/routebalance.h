@@ -25,7 +25,8 @@
  *   - Input buffers are consumed before the call returns (host pointers) or in stream order on the
  *     context's stream (device pointers).  The library never keeps a caller pointer.
  *   - Outputs to host pointers are complete when the call returns; outputs to device pointers are complete
- *     in stream order on the context's stream.
+ *     in stream order on the context's stream.  (rb_decide with host buffers returns as soon as the assignment has
+ *     reached host memory; work it queued behind that -- nothing a caller can observe -- may still be draining.)
  *   - All matrices are dense row-major.  Optional outputs may be NULL.
  *   - On any non-RB_OK return nothing the caller can observe has changed, except rb_last_error().
  *   - One context = one CUDA stream = one caller thread at a time.  Several contexts may coexist.

@@ -67,7 +67,12 @@ struct rb_ctx {
   // bus directly, and the assignment is written into it by the dispatch kernel -- no copy-engine transfers on the path.
   uint8_t* h_zc = nullptr;          // pinned host block: [query | plen | budget | assignment]
   uint8_t* d_zc = nullptr;          // the same block as the device addresses it
-  size_t zc_query_cap = 0, zc_off_plen = 0, zc_off_budget = 0, zc_off_assign = 0;
+  size_t zc_query_cap = 0, zc_off_plen = 0, zc_off_budget = 0, zc_off_assign = 0, zc_off_flag = 0;
+  uint32_t done_seq = 0;
+  // is_host_ptr results of the caller pointers seen last (a serving loop passes the same buffers again and again)
+  const void* ptr_cache[8]{};
+  bool ptr_cache_host[8]{};
+  int ptr_cache_next = 0;
   // boosted TPOT head (latency_mode 2)
   int4* f_nodes = nullptr;
   int32_t *f_root = nullptr, *f_begin = nullptr;
@@ -397,6 +402,17 @@ rb_status push_params(rb_ctx* ctx, const CallParams& cp) {
 struct Stager {
   rb_ctx* ctx;
   bool any_host = false;
+  bool wait_flag = false;    // completion is signalled through the pinned word (no stream synchronisation needed)
+  bool needs_sync = false;   // some host buffer went through the copy engine: the stream must drain
+  bool host(const void* p) {
+    for (int j = 0; j < 8; ++j)
+      if (ctx->ptr_cache[j] == p && p != nullptr) return ctx->ptr_cache_host[j];
+    const bool h = is_host_ptr(p);
+    ctx->ptr_cache[ctx->ptr_cache_next] = p;
+    ctx->ptr_cache_host[ctx->ptr_cache_next] = h;
+    ctx->ptr_cache_next = (ctx->ptr_cache_next + 1) & 7;
+    return h;
+  }
   cudaError_t err = cudaSuccess;
   struct Back { void* dst; const void* src; size_t bytes; };
   Back back[10];
@@ -406,7 +422,7 @@ struct Stager {
   // host input of at most `cap` bytes -> pinned block at `off`, read by the kernels in place
   template <typename T>
   const T* in_zc(const T* user, size_t off, size_t cap, T* staging, size_t bytes) {
-    if (!is_host_ptr(user)) return user;
+    if (!host(user)) return user;
     if (ctx->h_zc == nullptr || bytes > cap) return in(user, staging, bytes);
     any_host = true;
     std::memcpy(ctx->h_zc + off, user, bytes);
@@ -415,24 +431,27 @@ struct Stager {
   template <typename T>
   T* out_zc(T* user, size_t off, T* staging, size_t bytes) {
     if (!user) return nullptr;
-    if (!is_host_ptr(user)) return user;
+    if (!host(user)) return user;
     if (ctx->h_zc == nullptr) return out(user, staging, bytes);
     any_host = true;
+    wait_flag = true;
     hback[nhback++] = Back{user, ctx->h_zc + off, bytes};
     return reinterpret_cast<T*>(ctx->d_zc + off);
   }
   template <typename T>
   const T* in(const T* user, T* staging, size_t bytes) {
-    if (!is_host_ptr(user)) return user;
+    if (!host(user)) return user;
     any_host = true;
+    needs_sync = true;
     if (err == cudaSuccess) err = cudaMemcpyAsync(staging, user, bytes, cudaMemcpyHostToDevice, ctx->stream);
     return staging;
   }
   template <typename T>
   T* out(T* user, T* staging, size_t bytes) {
     if (!user) return nullptr;
-    if (!is_host_ptr(user)) return user;
+    if (!host(user)) return user;
     any_host = true;
+    needs_sync = true;
     back[nback++] = Back{user, staging, bytes};
     return staging;
   }
@@ -441,8 +460,9 @@ struct Stager {
   template <typename T>
   T* out_internal(T* user, T* internal, size_t bytes) {
     if (!user) return nullptr;
-    if (!is_host_ptr(user)) return user;
+    if (!host(user)) return user;
     any_host = true;
+    needs_sync = true;
     back[nback++] = Back{user, internal, bytes};
     return nullptr;
   }
@@ -451,7 +471,24 @@ struct Stager {
       err = cudaMemcpyAsync(back[j].dst, back[j].src, back[j].bytes, cudaMemcpyDeviceToHost, ctx->stream);
     if (err != cudaSuccess) return fail(ctx, RB_ECUDA, "cudaMemcpyAsync (outputs)", err);
     // host-side inputs must be consumed and host-side outputs complete before returning
-    if (any_host) CK(cudaStreamSynchronize(ctx->stream));
+    if (any_host) {
+      if (wait_flag && !needs_sync) {
+        // the dispatch kernel stores the call's sequence number into the pinned word after the assignment: poll it
+        // (a stream synchronisation costs several microseconds more); the stream is queried now and then so that
+        // a failed launch cannot hang the caller
+        volatile uint32_t* flag = reinterpret_cast<volatile uint32_t*>(ctx->h_zc + ctx->zc_off_flag);
+        for (uint32_t spins = 1; *flag != ctx->done_seq; ++spins) {
+          if ((spins & 0x3fff) == 0) {
+            const cudaError_t q = cudaStreamQuery(ctx->stream);
+            if (q == cudaSuccess) break;
+            if (q != cudaErrorNotReady) return fail(ctx, RB_ECUDA, "cudaStreamQuery", q);
+          }
+        }
+        if (*flag != ctx->done_seq) CK(cudaStreamSynchronize(ctx->stream));
+      } else {
+        CK(cudaStreamSynchronize(ctx->stream));
+      }
+    }
     for (int j = 0; j < nhback; ++j) std::memcpy(hback[j].dst, hback[j].src, hback[j].bytes);
     return RB_OK;
   }
@@ -549,7 +586,8 @@ rb_status rb_create(rb_ctx** out, const void* bank_emb, const float* bank_qualit
     ctx->zc_off_plen = (ctx->zc_query_cap + 255) & ~(size_t)255;
     ctx->zc_off_budget = ctx->zc_off_plen + ((mbz * 4 + 255) & ~(size_t)255);
     ctx->zc_off_assign = ctx->zc_off_budget + ((mbz * 4 + 255) & ~(size_t)255);
-    const size_t total = ctx->zc_off_assign + ((mbz * 4 + 255) & ~(size_t)255);
+    ctx->zc_off_flag = ctx->zc_off_assign + ((mbz * 4 + 255) & ~(size_t)255);
+    const size_t total = ctx->zc_off_flag + 256;
     if (cudaHostAlloc((void**)&ctx->h_zc, total, cudaHostAllocMapped) == cudaSuccess &&
         cudaHostGetDevicePointer((void**)&ctx->d_zc, ctx->h_zc, 0) == cudaSuccess) {
       std::memset(ctx->h_zc, 0, total);
@@ -882,6 +920,12 @@ rb_status rb_decide_budgeted(rb_ctx* ctx, const float* query_emb, const int32_t*
   cp.nn_idx = sg.out(nn_idx, ctx->scratch_nn_idx, bk);
   cp.nn_sim = sg.out(nn_sim, ctx->scratch_nn_sim, bk);
   if (sg.err != cudaSuccess) return fail(ctx, RB_ECUDA, "cudaMemcpyAsync (inputs)", sg.err);
+  if (sg.wait_flag && !sg.needs_sync && !ctx->stage_timing) {
+    cp.done_flag = reinterpret_cast<uint32_t*>(ctx->d_zc + ctx->zc_off_flag);
+    cp.done_seq = ++ctx->done_seq;
+  } else {
+    sg.needs_sync = sg.any_host;
+  }
   st = push_params(ctx, cp);
   if (st != RB_OK) return st;
   st = run_path(ctx, B, 0);

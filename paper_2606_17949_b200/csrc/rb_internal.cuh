@@ -64,6 +64,8 @@ struct CallParams {
   float* nn_sim;
   const float* budget;     // [B] per-request cost budgets (Eq. 2) or NULL: no admission filter
   int32_t* max_tokens;     // [B] or NULL: output-token clamp of the chosen instance
+  uint32_t* done_flag;     // pinned host word or NULL: the dispatch kernel stores done_seq there once the assignment is out
+  uint32_t done_seq;       //   (host callers wait on it instead of synchronising the stream)
   int32_t n_adv;           // pending rb_advance_state calls folded into this decision's first kernel (<= kMaxPendingAdvance)
   float adv_ms[4];         // their elapsed_ms, in call order
 #ifdef RB_TRACE
