@@ -656,3 +656,34 @@ def test_paper_shape_k_sweep(orc, k, slack, store):
                           plen.cpu().numpy(), w, g, state_after=(s[0].numpy(), s[1].numpy()))
     assert len(near) <= 2, log
     rt.close()
+
+
+@pytest.mark.parametrize("I,M,B", [(64, 4, 4096), (1024, 16, 4096), (256, 8, 3000)])
+def test_dispatch_at_maximum_batch(orc, I, M, B):
+    """Largest shapes the ABI admits (max_batch 4096, I 1024, M 16): the per-(request, tier) terms no longer fit shared
+    memory (global-memory path of the dispatch loop), the sort runs 4096 keys; with budgets; bit-exact."""
+    from paper_2606_17949_b200.router import Router
+    rng = np.random.default_rng(I + B)
+    it = synth.make_instances(I, M, cap=4)
+    rt = Router(torch.randn(64, 16).cuda(), torch.rand(64, M).cuda(), torch.rand(64, M).cuda() + 1, 4, store="f32", max_batch=B)
+    rt.set_instances(**it)
+    queued = rng.integers(0, 20001, I).astype(np.float32)
+    running = np.minimum(rng.integers(0, 12, I), it["cap"]).astype(np.int32)
+    Q = rng.uniform(0, 1, (B, M)).astype(np.float32)
+    L = rng.lognormal(5.5, 0.7, (B, M)).astype(np.float32)
+    L[B // 2] = L[3]
+    plen = rng.integers(1, 4000, B).astype(np.int32)
+    bud = _random_budgets(rng, it, L, plen)
+    inst = orc.Instances(**it)
+    for w, budget in ((synth.PRESETS["balanced"], None), (synth.PRESETS["cost"], bud)):
+        rt.set_state(torch.from_numpy(queued), torch.from_numpy(running))
+        g = _np(rt.decide_from_predictions(torch.from_numpy(Q).cuda(), torch.from_numpy(L).cuda(), torch.from_numpy(plen).cuda(),
+                                           w, commit=1, budget=None if budget is None else torch.from_numpy(budget).cuda()))
+        ref = orc.dispatch(inst, queued, running, Q, L, plen, w, budget=budget)
+        for key in ("assignment", "order", "scores", "scores0"):
+            assert np.array_equal(g[key], ref[key]), key
+        if budget is not None:
+            assert np.array_equal(g["max_tokens"], ref["max_tokens"])
+        s = rt.get_state()
+        assert np.array_equal(s[0].numpy(), ref["queued"]) and np.array_equal(s[1].numpy(), ref["running"])
+    rt.close()
