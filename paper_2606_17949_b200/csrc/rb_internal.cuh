@@ -93,6 +93,33 @@ __device__ __forceinline__ float forest_leaf(const int4* __restrict__ nodes, int
   }
   return __int_as_float(nd.y);
 }
+// Leaves of trees tr0 + lane, tr0 + lane + 32, ... < tr1 into out[tree - tr0]: every lane walks up to four trees at once
+// (a walk is a chain of dependent node loads; four independent chains hide most of their latency).
+__device__ __forceinline__ void forest_leaves_warp(const int4* __restrict__ nodes, const int32_t* __restrict__ tree_root,
+                                                   int tr0, int tr1, int lane, float xb, float xd,
+                                                   const float* __restrict__ aux_i, float* out) {
+  for (int base = tr0 + lane; base < tr1; base += 128) {
+    int4 nd[4];
+    bool live[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      live[u] = base + 32 * u < tr1;
+      nd[u] = live[u] ? __ldg(&nodes[__ldg(&tree_root[base + 32 * u])]) : make_int4(-1, 0, 0, 0);
+    }
+    while ((nd[0].x >= 0) | (nd[1].x >= 0) | (nd[2].x >= 0) | (nd[3].x >= 0)) {
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        if (nd[u].x >= 0) {
+          const float x = nd[u].x == 0 ? xb : (nd[u].x == 1 ? xd : __ldg(&aux_i[nd[u].x - 2]));
+          nd[u] = __ldg(&nodes[(x < __int_as_float(nd[u].y)) ? nd[u].z : nd[u].w]);
+        }
+      }
+    }
+#pragma unroll
+    for (int u = 0; u < 4; ++u)
+      if (live[u]) out[base + 32 * u - tr0] = __int_as_float(nd[u].y);
+  }
+}
 #endif
 
 // ---- programmatic dependent launch ---------------------------------------------------------------------------
