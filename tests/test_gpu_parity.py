@@ -687,3 +687,34 @@ def test_dispatch_at_maximum_batch(orc, I, M, B):
         s = rt.get_state()
         assert np.array_equal(s[0].numpy(), ref["queued"]) and np.array_equal(s[1].numpy(), ref["running"])
     rt.close()
+
+
+def test_deferred_advance_on_a_bank_that_does_not_fill_the_gpu(orc):
+    """On a small bank the scan occupies few SMs, so with programmatic dependent launch every kernel of a decision can be
+    resident at once: the dispatch kernel must still see the state advance its own decision's staging kernel applies.
+    300 advance + decide steps in lock-step with the oracle (state compared after every step)."""
+    cfg = dataclasses.replace(synth.CONFIGS["C2"], N=500, d=64, B=5, Kc=4, seed=41)
+    bank, it, queued, running, query, plen, rt = _setup(cfg, max_batch=8)
+    inst = orc.Instances(**it)
+    bank_np = parity.bank_to_numpy(bank["emb"])
+    qn, ln = bank["quality"].cpu().numpy(), bank["outlen"].cpu().numpy()
+    ref = orc.decide(bank_np, qn, ln, inst, queued.numpy(), running.numpy(), query.cpu().numpy(), plen.cpu().numpy(),
+                     synth.PRESETS["balanced"], cfg.k, store_dtype="bf16")
+    pq, pl = ref["pred_quality"], ref["pred_outlen"]
+    dq, bq = queued.numpy().copy(), running.numpy().copy()
+    rng = np.random.default_rng(2)
+    a = torch.empty(cfg.B, dtype=torch.int32, device="cuda")
+    from paper_2606_17949_b200 import binding as rb
+    for step in range(300):
+        dt = float(rng.choice([0.0, 3.0, 40.0, 900.0]))
+        w = list(synth.PRESETS.values())[step % 4]
+        rb.rb_advance_state(rt.ctx, dt)
+        rb.rb_decide(rt.ctx, query, plen, cfg.B, w, a)
+        dq, bq = orc.advance_state(inst, dq, bq, np.float32(dt))
+        r = orc.dispatch(inst, dq, bq, pq, pl, plen.cpu().numpy(), w)
+        dq, bq = r["queued"], r["running"]
+        if step % 25 == 24 or step < 5:
+            s = rt.get_state()
+            assert np.array_equal(a.cpu().numpy(), r["assignment"]), step
+            assert np.array_equal(s[0].numpy(), dq) and np.array_equal(s[1].numpy(), bq), step
+    rt.close()
