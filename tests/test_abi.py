@@ -52,3 +52,17 @@ def test_product_never_imports_oracle():
     for f in ("orc.cpp", "orc.py"):
         text = open(os.path.join(ROOT, "oracle", f)).read()
         assert not re.search(r"(import\s+paper_2606|from\s+paper_2606\S*\s+import|#include\s+\"[^\"]*(csrc|routebalance))", text), f
+
+
+def test_c_program_links_and_runs(tmp_path):
+    """include/routebalance.h is valid C99 and librouteb.so links from a plain C program (no Python, no torch):
+    defaults, argument validation and NULL handling through the C ABI, without a GPU."""
+    import subprocess
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    pkg = os.path.join(root, "paper_2606_17949_b200")
+    exe = str(tmp_path / "abi_check")
+    subprocess.run(["gcc", "-std=c99", "-Wall", "-Werror", "-I", os.path.join(root, "include"),
+                    os.path.join(pkg, "examples", "abi_check.c"), "-o", exe, "-L", pkg, "-lrouteb",
+                    "-Wl,-rpath," + pkg], check=True)
+    r = subprocess.run([exe], capture_output=True, text=True)
+    assert r.returncode == 0 and "abi ok" in r.stdout, (r.returncode, r.stdout, r.stderr)
