@@ -187,7 +187,7 @@ constexpr int kMerge2Stride = 64;                 // second merge: nwarps + 1 li
 __device__ __forceinline__ float exact_sim_bf16(const uint4* __restrict__ qrow, const uint4* __restrict__ brow, int nvec,
                                                 int lane) {
   double acc = 0.0;
-#pragma unroll 4
+#pragma unroll 2
   for (int vidx = lane; vidx < nvec; vidx += 32) {
     const uint4 xb = qrow[vidx], eb = brow[vidx];
     const __nv_bfloat162* xp = reinterpret_cast<const __nv_bfloat162*>(&xb);
