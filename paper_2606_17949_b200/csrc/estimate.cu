@@ -205,8 +205,10 @@ __device__ __forceinline__ float exact_sim_bf16(const uint4* __restrict__ qrow, 
 
 // Warp-level k-way merge: lane l owns the sorted list keys[(first + l)*stride ..] (l < nl <= 32) and the warp
 // pops the kc largest keys, in order, into out_key / out_src (the owning list's index).  No block barrier.
+// bound_hi: similarity (ordered bits) that every member of the query's kc best reaches (0 = none known): the warp stops
+// popping below it and pads the rest of its output with empty entries.
 __device__ __forceinline__ void warp_kway_merge(const unsigned long long* keys, int first, int nl, int stride, int len,
-                                                int kc, unsigned long long* out_key, int* out_src) {
+                                                int kc, unsigned long long* out_key, int* out_src, uint32_t bound_hi) {
   const int lane = threadIdx.x & 31;
   const unsigned long long* mine = keys + (size_t)(first + lane) * stride;
   int pos = 0;
@@ -214,6 +216,10 @@ __device__ __forceinline__ void warp_kway_merge(const unsigned long long* keys, 
   for (int j = 0; j < kc; ++j) {
     const uint32_t hi = (uint32_t)(hk >> 32), lo = (uint32_t)hk;
     const uint32_t ghi = __reduce_max_sync(0xffffffffu, hi);
+    if (ghi < bound_hi) {   // warp-uniform: nothing left here can be among the kc best
+      for (int jj = j + lane; jj < kc; jj += 32) { out_key[jj] = 0ull; out_src[jj] = -1; }
+      break;
+    }
     const uint32_t glo = __reduce_max_sync(0xffffffffu, hi == ghi ? lo : 0u);
     const unsigned long long win = ((unsigned long long)ghi << 32) | glo;
     if (win != 0ull && hk == win) {   // keys are distinct: exactly one owner
@@ -264,6 +270,7 @@ finish_kernel(FinishArgs a, InstTable t, const CallParams* __restrict__ cp) {
   __shared__ unsigned long long s_cand[kMaxK];
   __shared__ int s_src[kMaxK];
   __shared__ int s_nflag;
+  __shared__ uint32_t s_wbest[kFinWarpsMax];
   __shared__ int s_flag[kMaxFlag];
   __shared__ float s_sim[kMaxK];
   __shared__ int32_t s_idx[kMaxK];
@@ -364,8 +371,28 @@ finish_kernel(FinishArgs a, InstTable t, const CallParams* __restrict__ cp) {
     const int per = (a.nlists + nwarps - 1) / nwarps;                 // <= 32 by the choice of the block size
     const int first = warp * per;
     const int nl = max(0, min(per, a.nlists - first));
+    // Admission bound: the kc-th largest of the warps' best similarities is reached by kc distinct candidates, so
+    // every member of the kc best reaches it too -- a warp then pops two or three entries instead of kc.
+    uint32_t bound = 0u;
+    if (nwarps >= kc) {   // block-uniform
+      const uint32_t head = lane < nl ? (uint32_t)(s_keys[(size_t)(first + lane) * kcap] >> 32) : 0u;
+      const uint32_t wbest = __reduce_max_sync(0xffffffffu, head);
+      if (lane == 0) s_wbest[warp] = wbest;
+      __syncthreads();
+      uint32_t v = lane < nwarps ? s_wbest[lane] : 0u;
+#pragma unroll
+      for (int size = 2; size <= 32; size <<= 1) {
+#pragma unroll
+        for (int stride = size >> 1; stride > 0; stride >>= 1) {
+          const uint32_t other = __shfl_xor_sync(0xffffffffu, v, stride);
+          const bool keep_max = ((lane & stride) == 0) == ((lane & size) == 0);   // descending
+          v = (keep_max == (v > other)) ? v : other;
+        }
+      }
+      bound = __shfl_sync(0xffffffffu, v, kc - 1);
+    }
     warp_kway_merge(s_keys, first, nl, kcap, kcap, kc, w_key + (size_t)warp * kMerge2Stride,
-                    w_src + (size_t)warp * kMerge2Stride);
+                    w_src + (size_t)warp * kMerge2Stride, bound);
   }
   __syncthreads();
   RB_FT(2);
