@@ -207,11 +207,12 @@ __device__ __forceinline__ float exact_sim_bf16(const uint4* __restrict__ qrow, 
 // pops the kc largest keys, in order, into out_key / out_src (the owning list's index).  No block barrier.
 // bound_hi: similarity (ordered bits) that every member of the query's kc best reaches (0 = none known): the warp stops
 // popping below it and pads the rest of its output with empty entries.
-__device__ __forceinline__ void warp_kway_merge(const unsigned long long* keys, int first, int nl, int stride, int len,
-                                                int kc, unsigned long long* out_key, int* out_src, uint32_t bound_hi) {
+// Returns the number of entries popped (warp-uniform).
+__device__ __forceinline__ int warp_kway_merge(const unsigned long long* keys, int first, int nl, int stride, int len,
+                                               int kc, unsigned long long* out_key, int* out_src, uint32_t bound_hi) {
   const int lane = threadIdx.x & 31;
   const unsigned long long* mine = keys + (size_t)(first + lane) * stride;
-  int pos = 0;
+  int pos = 0, npop = 0;
   unsigned long long hk = (lane < nl) ? mine[0] : 0ull;
   for (int j = 0; j < kc; ++j) {
     const uint32_t hi = (uint32_t)(hk >> 32), lo = (uint32_t)hk;
@@ -220,6 +221,7 @@ __device__ __forceinline__ void warp_kway_merge(const unsigned long long* keys, 
       for (int jj = j + lane; jj < kc; jj += 32) { out_key[jj] = 0ull; out_src[jj] = -1; }
       break;
     }
+    npop += ghi != 0u;
     const uint32_t glo = __reduce_max_sync(0xffffffffu, hi == ghi ? lo : 0u);
     const unsigned long long win = ((unsigned long long)ghi << 32) | glo;
     if (win != 0ull && hk == win) {   // keys are distinct: exactly one owner
@@ -230,6 +232,7 @@ __device__ __forceinline__ void warp_kway_merge(const unsigned long long* keys, 
     }
     if (win == 0ull && lane == 0) { out_key[j] = 0ull; out_src[j] = -1; }
   }
+  return npop;
 }
 
 // Block-wide k-way merge: thread c < nl owns the sorted list keys[c*stride .. c*stride+len); pops the kc largest
@@ -271,6 +274,9 @@ finish_kernel(FinishArgs a, InstTable t, const CallParams* __restrict__ cp) {
   __shared__ int s_src[kMaxK];
   __shared__ int s_nflag;
   __shared__ uint32_t s_wbest[kFinWarpsMax];
+  __shared__ int s_wcnt[kFinWarpsMax];                // entries each warp popped at the first level
+  __shared__ unsigned long long s_skey[64];           // first-level survivors, compacted (second level by counting)
+  __shared__ int s_ssrc[64];
   __shared__ int s_flag[kMaxFlag];
   __shared__ float s_sim[kMaxK];
   __shared__ int32_t s_idx[kMaxK];
@@ -391,8 +397,9 @@ finish_kernel(FinishArgs a, InstTable t, const CallParams* __restrict__ cp) {
       }
       bound = __shfl_sync(0xffffffffu, v, kc - 1);
     }
-    warp_kway_merge(s_keys, first, nl, kcap, kcap, kc, w_key + (size_t)warp * kMerge2Stride,
-                    w_src + (size_t)warp * kMerge2Stride, bound);
+    const int npop = warp_kway_merge(s_keys, first, nl, kcap, kcap, kc, w_key + (size_t)warp * kMerge2Stride,
+                                     w_src + (size_t)warp * kMerge2Stride, bound);
+    if (lane == 0) s_wcnt[warp] = npop;
   }
   __syncthreads();
   RB_FT(2);
@@ -401,6 +408,34 @@ finish_kernel(FinishArgs a, InstTable t, const CallParams* __restrict__ cp) {
     // out_src of this level is the warp whose list the key came from; its position in that list is the number
     // of keys already taken from it, which recovers the original list index
     const unsigned long long* mine = w_key + (size_t)lane * kMerge2Stride;
+    // With the admission bound the warps hand over a few dozen entries in all: rank them by counting (keys are
+    // distinct) instead of kc sequential pops.  More than 64 (no bound, or a bank sorted by topic): the pops below.
+    const int cnt = lane < nwarps ? s_wcnt[lane] : 0;
+    int incl = cnt;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const int up = __shfl_up_sync(0xffffffffu, incl, o);
+      if (lane >= o) incl += up;
+    }
+    const int total = __shfl_sync(0xffffffffu, incl, 31);
+    if (total <= 64) {
+      const int off = incl - cnt;
+      for (int q = 0; q < cnt; ++q) {
+        s_skey[off + q] = mine[q];
+        s_ssrc[off + q] = w_src[(size_t)lane * kMerge2Stride + q];
+      }
+      __syncwarp();
+      const unsigned long long k0 = lane < total ? s_skey[lane] : 0ull, k1 = lane + 32 < total ? s_skey[lane + 32] : 0ull;
+      int rk0 = 0, rk1 = 0;
+      for (int q = 0; q < total; ++q) {
+        const unsigned long long o = s_skey[q];
+        rk0 += o > k0;
+        rk1 += o > k1;
+      }
+      if (lane < total && rk0 < kc) { s_cand[rk0] = k0; s_src[rk0] = s_ssrc[lane]; }
+      if (lane + 32 < total && rk1 < kc) { s_cand[rk1] = k1; s_src[rk1] = s_ssrc[lane + 32]; }
+      for (int j = total + lane; j < kc; j += 32) { s_cand[j] = 0ull; s_src[j] = -1; }
+    } else {
     int pos = 0;
     unsigned long long hk = (lane < nwarps) ? mine[0] : 0ull;
     for (int j = 0; j < kc; ++j) {
@@ -415,6 +450,7 @@ finish_kernel(FinishArgs a, InstTable t, const CallParams* __restrict__ cp) {
         hk = pos < kc ? mine[pos] : 0ull;
       }
       if (win == 0ull && lane == 0) { s_cand[j] = 0ull; s_src[j] = -1; }
+    }
     }
   }
   __syncthreads();
