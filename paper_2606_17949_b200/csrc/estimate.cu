@@ -274,6 +274,7 @@ finish_kernel(FinishArgs a, InstTable t, const CallParams* __restrict__ cp) {
   __shared__ int s_src[kMaxK];
   __shared__ int s_nflag;
   __shared__ uint32_t s_wbest[kFinWarpsMax];
+  __shared__ int s_maxcnt;
   __shared__ int s_wcnt[kFinWarpsMax];                // entries each warp popped at the first level
   __shared__ unsigned long long s_skey[64];           // first-level survivors, compacted (second level by counting)
   __shared__ int s_ssrc[64];
@@ -418,6 +419,9 @@ finish_kernel(FinishArgs a, InstTable t, const CallParams* __restrict__ cp) {
       if (lane >= o) incl += up;
     }
     const int total = __shfl_sync(0xffffffffu, incl, 31);
+    // a list can only have been popped completely if its warp popped at least kcap entries
+    const int maxcnt = (int)__reduce_max_sync(0xffffffffu, (uint32_t)cnt);
+    if (lane == 0) s_maxcnt = maxcnt;
     if (total <= 64) {
       const int off = incl - cnt;
       for (int q = 0; q < cnt; ++q) {
@@ -460,7 +464,7 @@ finish_kernel(FinishArgs a, InstTable t, const CallParams* __restrict__ cp) {
   // ---- rescan of slabs whose list was popped completely ----
   // (a list of kcap entries all of which are among the kc best may hide further members)
   bool flagged = false;
-  if (a.rescan && tid < kc && s_src[tid] >= 0) {
+  if (a.rescan && s_maxcnt >= kcap && tid < kc && s_src[tid] >= 0) {
     int same = 0, earlier = 0;
     for (int j = 0; j < kc; ++j) {
       same += (s_src[j] == s_src[tid]);
