@@ -694,7 +694,8 @@ cudaError_t finish_prepare(size_t max_smem) {
 }
 
 cudaError_t launch_finish(const FinishArgs& a, InstTable t, const CallParams* cp, int B, cudaStream_t s) {
-  const cudaError_t e = launch_chained(finish_kernel, dim3(B), dim3(a.nlists > 512 ? 1024 : 512),
+  // 32 warps from 257 lists on: the first-level merges' admission bound needs at least k + slack warps to bite
+  const cudaError_t e = launch_chained(finish_kernel, dim3(B), dim3(a.nlists > 256 ? 1024 : 512),
                                        finish_smem_bytes(a.nlists, a.kcap), s, a, t, cp);
   return e != cudaSuccess ? e : cudaGetLastError();
 }
