@@ -35,9 +35,10 @@ __device__ __forceinline__ unsigned long long make_key(float sim, int32_t idx) {
 }
 
 // ---- a0 ---------------------------------------------------------------------------------------------
-__global__ void stage_queries_kernel(const CallParams* __restrict__ cp, __nv_bfloat16* __restrict__ qs, int B, int Bpad,
+__global__ void stage_queries_kernel(const __grid_constant__ CallParams cpv, __nv_bfloat16* __restrict__ qs, int B, int Bpad,
                                      int d, int group, uint32_t* __restrict__ gthr, int n_gthr, InstTable t,
                                      float* __restrict__ dq, int32_t* __restrict__ bq) {
+  const CallParams* __restrict__ cp = &cpv;   // the per-call parameters travel as a kernel argument (constant bank)
   launch_dependents();
   if (blockIdx.x == 0) {
     // a8 folded in: rb_advance_state calls since the last decision (reading 22; same arithmetic as advance_kernel):
@@ -82,9 +83,10 @@ constexpr int kF32Rows = 128;   // bank rows per block, one per thread
 constexpr int kF32Q = 8;        // queries per register group
 constexpr int kF32Chunk = 64;   // columns staged per step
 __global__ void __launch_bounds__(kF32Rows)
-scan_f32_kernel(const float* __restrict__ bank, const CallParams* __restrict__ cp, int r0, int64_t N, int d, int nq,
+scan_f32_kernel(const float* __restrict__ bank, const __grid_constant__ CallParams cpv, int r0, int64_t N, int d, int nq,
                 float* __restrict__ sims) {
   __shared__ float xs[kF32Q][kF32Chunk];
+  const CallParams* __restrict__ cp = &cpv;
   const float* __restrict__ q = cp->query + (size_t)r0 * d;
   const int64_t n = (int64_t)blockIdx.x * kF32Rows + threadIdx.x;
   const float* row = bank + (n < N ? n : N - 1) * (int64_t)d;
@@ -267,7 +269,8 @@ __device__ int kway_merge(const unsigned long long* keys, int nl, int stride, in
 }
 
 __global__ void __launch_bounds__(kFinThreadsMax)
-finish_kernel(FinishArgs a, InstTable t, const CallParams* __restrict__ cp) {
+finish_kernel(FinishArgs a, InstTable t, const __grid_constant__ CallParams cpv) {
+  const CallParams* __restrict__ cp = &cpv;   // per-call parameters: a kernel argument (constant bank), not a device block
   extern __shared__ unsigned long long s_keys[];   // max([nlists][kcap], [nwarps + 1][kMerge2Stride])
   __shared__ uint32_t s_red[2][kFinWarpsMax][2];
   __shared__ unsigned long long s_cand[kMaxK];
@@ -660,7 +663,7 @@ cudaError_t launch_convert_bf16(const float* in, __nv_bfloat16* out, size_t n, c
   return cudaGetLastError();
 }
 
-cudaError_t launch_stage_queries(const CallParams* cp, __nv_bfloat16* qs, int B, int Bpad, int d, int rep, uint32_t* gthr,
+cudaError_t launch_stage_queries(const CallParams& cp, __nv_bfloat16* qs, int B, int Bpad, int d, int rep, uint32_t* gthr,
                                  int n_gthr, InstTable t, float* dq, int32_t* bq, cudaStream_t s) {
   const size_t n = (size_t)Bpad * d;
   int blocks = (int)((n + 255) / 256);
@@ -669,7 +672,7 @@ cudaError_t launch_stage_queries(const CallParams* cp, __nv_bfloat16* qs, int B,
   return cudaGetLastError();
 }
 
-cudaError_t launch_scan_f32(const float* bank, const CallParams* cp, int r0, int64_t N, int d, int nq, float* sims,
+cudaError_t launch_scan_f32(const float* bank, const CallParams& cp, int r0, int64_t N, int d, int nq, float* sims,
                             cudaStream_t s) {
   const int blocks = (int)((N + kF32Rows - 1) / kF32Rows);
   scan_f32_kernel<<<blocks, kF32Rows, 0, s>>>(bank, cp, r0, N, d, nq, sims);
@@ -680,6 +683,15 @@ cudaError_t launch_select_f32(const float* sims, int64_t N, int nq, int kc, floa
                               cudaStream_t s) {
   select_f32_kernel<<<nq, 256, 0, s>>>(sims, N, kc, cand_sim, cand_idx);
   return cudaGetLastError();
+}
+
+// Position and count of the arguments of this file's kernels that carry the per-call parameters (graph replays update
+// that one argument): returns the index of the CallParams argument, or -1 if func is not one of them.
+int estimate_cp_arg(const void* func, int* nargs) {
+  if (func == (const void*)stage_queries_kernel) { *nargs = 11; return 0; }
+  if (func == (const void*)scan_f32_kernel) { *nargs = 7; return 1; }
+  if (func == (const void*)finish_kernel) { *nargs = 3; return 2; }
+  return -1;
 }
 
 size_t finish_smem_bytes(int nlists, int kcap) {
@@ -693,7 +705,7 @@ cudaError_t finish_prepare(size_t max_smem) {
   return cudaFuncSetAttribute(finish_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)max_smem);
 }
 
-cudaError_t launch_finish(const FinishArgs& a, InstTable t, const CallParams* cp, int B, cudaStream_t s) {
+cudaError_t launch_finish(const FinishArgs& a, InstTable t, const CallParams& cp, int B, cudaStream_t s) {
   // 32 warps from 257 lists on: the first-level merges' admission bound needs at least k + slack warps to bite
   const cudaError_t e = launch_chained(finish_kernel, dim3(B), dim3(a.nlists > 256 ? 1024 : 512),
                                        finish_smem_bytes(a.nlists, a.kcap), s, a, t, cp);

@@ -42,13 +42,10 @@ struct rb_ctx {
   float* q32 = nullptr;             // [max_batch x d]
   __nv_bfloat16* qs = nullptr;      // [Bpad_max x d]
   int32_t* plen = nullptr;          // [max_batch]
-  CallParams* cp = nullptr;
+  CallParams cp_cur{};              // per-call parameters of the call being enqueued (passed to the kernels by value)
 #ifdef RB_TRACE
   unsigned long long* timeline = nullptr;
 #endif
-  CallParams* cp_ring = nullptr;    // pinned host ring feeding cp; slot reuse is guarded by cp_ev
-  cudaEvent_t cp_ev[64]{};
-  uint64_t cp_seq = 0;
   uint32_t* gthr = nullptr;         // [Bpad_max] cross-slab admission thresholds of the scan (cleared per decision)
   float* part_sim = nullptr;        // [num_sms][kcap][Bpad_max]
   int32_t* part_idx = nullptr;
@@ -85,8 +82,22 @@ struct rb_ctx {
   float *scores = nullptr, *scores0 = nullptr;  // [max_batch x I], allocated by rb_set_instances
   CUtensorMap tm_q{}, tm_bank{};
   // graphs: key = B * 4 + kind (0 decide, 1 estimate, 2 from_predictions)
-  std::unordered_map<int64_t, cudaGraphExec_t> graphs;
-  std::unordered_map<int64_t, int> graph_nodes;
+  // One captured graph per decision shape.  The per-call parameters are an argument of the kernels that need them; a
+  // replay rewrites that one argument of those kernel nodes (cudaGraphExecKernelNodeSetParams) -- no transfer of any
+  // kind sits between the host and the decision's first kernel.
+  struct CpNode {
+    cudaGraphNode_t node;
+    cudaKernelNodeParams params;
+    std::vector<void*> args;   // the node's argument pointers, with args[cp_index] redirected to cp_cur
+    int cp_index;
+  };
+  struct GraphRec {
+    cudaGraph_t graph = nullptr;
+    cudaGraphExec_t exec = nullptr;
+    int nodes = 0;
+    std::vector<CpNode> cp_nodes;
+  };
+  std::unordered_map<int64_t, GraphRec> graphs;
   int64_t launches = 0;
   bool stage_timing = false;
   bool capturing = false;
@@ -146,6 +157,14 @@ ForestDev forest_of(const rb_ctx* c) {
   f.nodes = c->f_nodes; f.tree_root = c->f_root; f.tier_begin = c->f_begin; f.base = c->f_base; f.aux = c->f_aux;
   f.tpot0 = c->f_tpot0; f.n_features = c->f_features;
   return f;
+}
+
+void drop_graphs(rb_ctx* c) {
+  for (auto& kv : c->graphs) {
+    cudaGraphExecDestroy(kv.second.exec);
+    cudaGraphDestroy(kv.second.graph);
+  }
+  c->graphs.clear();
 }
 
 InstTable table_of(const rb_ctx* c) {
@@ -229,7 +248,7 @@ rb_status enqueue_estimate(rb_ctx* ctx, int B, bool with_terms, Timer& tm) {
     if (B > kTileM && ctx->num_sms >= 2) {
       // tensor-bound regime: CTA pairs, 256-query m-tiles
       const int Bpad2 = (B + 2 * kTileM - 1) / (2 * kTileM) * (2 * kTileM);
-      CK(launch_stage_queries(ctx->cp, ctx->qs, B, Bpad2, ctx->d, 1, ctx->gthr,
+      CK(launch_stage_queries(ctx->cp_cur, ctx->qs, B, Bpad2, ctx->d, 1, ctx->gthr,
                               Bpad2 * (1 + scan_tc2_clusters(ctx->N, ctx->num_sms)), table_of(ctx), ctx->dq, ctx->bq, s));
       tm.mark();
       int ncl = 0;
@@ -244,7 +263,7 @@ rb_status enqueue_estimate(rb_ctx* ctx, int B, bool with_terms, Timer& tm) {
       fa.Bpad = Bpad2; fa.slab_unit = kTileN; fa.rescan = kcap2 < ctx->kc ? 1 : 0;
     } else {
       const int rep = scan_tc_replicas(B, ctx->ks, ctx->num_sms);
-      CK(launch_stage_queries(ctx->cp, ctx->qs, B, Bpad, ctx->d, rep, ctx->gthr, Bpad, table_of(ctx), ctx->dq, ctx->bq, s));
+      CK(launch_stage_queries(ctx->cp_cur, ctx->qs, B, Bpad, ctx->d, rep, ctx->gthr, Bpad, table_of(ctx), ctx->dq, ctx->bq, s));
       tm.mark();
       int grid = 0;
       CK(launch_scan_tc(&ctx->tm_q, &ctx->tm_bank, ctx->N, ctx->d, B, Bpad, ctx->ks, ctx->num_sms, ctx->part_sim,
@@ -262,7 +281,7 @@ rb_status enqueue_estimate(rb_ctx* ctx, int B, bool with_terms, Timer& tm) {
     tm.mark();
     for (int r0 = 0; r0 < B; r0 += kF32Group) {
       const int nq = (B - r0 < kF32Group) ? (B - r0) : kF32Group;
-      CK(launch_scan_f32((const float*)ctx->bank, ctx->cp, r0, ctx->N, ctx->d, nq, ctx->sims, s));
+      CK(launch_scan_f32((const float*)ctx->bank, ctx->cp_cur, r0, ctx->N, ctx->d, nq, ctx->sims, s));
       CK(launch_select_f32(ctx->sims, ctx->N, nq, ctx->kc, ctx->cand_sim + (size_t)r0 * ctx->kc,
                            ctx->cand_idx + (size_t)r0 * ctx->kc, s));
       ctx->launches += 2;
@@ -273,7 +292,7 @@ rb_status enqueue_estimate(rb_ctx* ctx, int B, bool with_terms, Timer& tm) {
     fa.slab_unit = kBoxN;
     fa.bank = nullptr; fa.qs = nullptr; fa.rerank = 0;
   }
-  CK(launch_finish(fa, table_of(ctx), ctx->cp, B, s));
+  CK(launch_finish(fa, table_of(ctx), ctx->cp_cur, B, s));
   ctx->launches += 1;
   tm.mark();
   return RB_OK;
@@ -287,11 +306,11 @@ rb_status enqueue_dispatch(rb_ctx* ctx, int B, bool from_predictions, Timer& tm)
       CK(launch_tpot_forest(t, forest_of(ctx), ctx->dq, ctx->bq, ctx->f_tpot0, -1.0f, s));
       ctx->launches += 1;
     }
-    CK(launch_score(t, ctx->dq, ctx->bq, ctx->cp, B, ctx->termA, ctx->termP, ctx->key, modes_of(ctx), forest_of(ctx), s));
+    CK(launch_score(t, ctx->dq, ctx->bq, ctx->cp_cur, B, ctx->termA, ctx->termP, ctx->key, modes_of(ctx), forest_of(ctx), s));
     ctx->launches += 1;
   }
   tm.mark();
-  CK(launch_lpt_dispatch(t, ctx->dq, ctx->bq, ctx->termA, ctx->termP, ctx->key, ctx->cp, B, modes_of(ctx), forest_of(ctx), s));
+  CK(launch_lpt_dispatch(t, ctx->dq, ctx->bq, ctx->termA, ctx->termP, ctx->key, ctx->cp_cur, B, modes_of(ctx), forest_of(ctx), s));
   tm.mark();
   ctx->launches += 1;
   return RB_OK;
@@ -341,15 +360,45 @@ rb_status run_path(rb_ctx* ctx, int B, int kind) {
       return st;
     }
     if (e != cudaSuccess) return fail(ctx, RB_ECUDA, "cudaStreamEndCapture", e);
-    cudaGraphExec_t ge = nullptr;
-    e = cudaGraphInstantiate(&ge, g, 0);
-    cudaGraphDestroy(g);
-    if (e != cudaSuccess) return fail(ctx, RB_ECUDA, "cudaGraphInstantiate", e);
-    it = ctx->graphs.emplace(gkey, ge).first;
-    ctx->graph_nodes[gkey] = nodes;
+    rb_ctx::GraphRec rec;
+    rec.graph = g;
+    rec.nodes = nodes;
+    e = cudaGraphInstantiate(&rec.exec, g, 0);
+    if (e != cudaSuccess) {
+      cudaGraphDestroy(g);
+      return fail(ctx, RB_ECUDA, "cudaGraphInstantiate", e);
+    }
+    // the kernel nodes that take the per-call parameters, and where
+    size_t nn = 0;
+    CK(cudaGraphGetNodes(g, nullptr, &nn));
+    std::vector<cudaGraphNode_t> all(nn);
+    CK(cudaGraphGetNodes(g, all.data(), &nn));
+    for (cudaGraphNode_t node : all) {
+      cudaGraphNodeType ty;
+      CK(cudaGraphNodeGetType(node, &ty));
+      if (ty != cudaGraphNodeTypeKernel) continue;
+      rb_ctx::CpNode cn{};
+      CK(cudaGraphKernelNodeGetParams(node, &cn.params));
+      int nargs = 0;
+      int idx = estimate_cp_arg(cn.params.func, &nargs);
+      if (idx < 0) idx = dispatch_cp_arg(cn.params.func, &nargs);
+      if (idx < 0) continue;
+      cn.node = node;
+      cn.cp_index = idx;
+      cn.args.assign(cn.params.kernelParams, cn.params.kernelParams + nargs);   // values stay owned by the node
+      rec.cp_nodes.push_back(std::move(cn));
+    }
+    it = ctx->graphs.emplace(gkey, std::move(rec)).first;
+  } else {
+    // replay: the same graph with this call's parameters
+    for (rb_ctx::CpNode& cn : it->second.cp_nodes) {
+      cn.args[cn.cp_index] = &ctx->cp_cur;
+      cn.params.kernelParams = cn.args.data();
+      CK(cudaGraphExecKernelNodeSetParams(it->second.exec, cn.node, &cn.params));
+    }
   }
-  CK(cudaGraphLaunch(it->second, ctx->stream));
-  ctx->launches += ctx->graph_nodes[gkey];
+  CK(cudaGraphLaunch(it->second.exec, ctx->stream));
+  ctx->launches += it->second.nodes;
   return RB_OK;
 }
 
@@ -381,18 +430,13 @@ void collect_stage_times(rb_ctx* ctx, int kind) {
   }
 }
 
-// Per-call parameters travel host -> device through a pinned ring so that the copy is truly asynchronous.
+// The call's parameters: kept in the context while its kernels are enqueued (they receive them by value).
 rb_status push_params(rb_ctx* ctx, const CallParams& cp) {
-  const int slot = (int)(ctx->cp_seq % 64);
-  if (ctx->cp_seq >= 64) CK(cudaEventSynchronize(ctx->cp_ev[slot]));
-  ctx->cp_ring[slot] = cp;
+  ctx->cp_cur = cp;
 #ifdef RB_TRACE
   if (!ctx->timeline) CK(cudaMalloc((void**)&ctx->timeline, 128 * 8));
-  ctx->cp_ring[slot].timeline = ctx->timeline;
+  ctx->cp_cur.timeline = ctx->timeline;
 #endif
-  CK(cudaMemcpyAsync(ctx->cp, &ctx->cp_ring[slot], sizeof cp, cudaMemcpyHostToDevice, ctx->stream));
-  CK(cudaEventRecord(ctx->cp_ev[slot], ctx->stream));
-  ctx->cp_seq++;
   return RB_OK;
 }
 
@@ -578,8 +622,6 @@ rb_status rb_create(rb_ctx** out, const void* bank_emb, const float* bank_qualit
     ctx->own_stream = true;
   }
   for (auto& e : ctx->ev) CK(cudaEventCreate(&e));
-  for (auto& e : ctx->cp_ev) CK(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
-  CK(cudaMallocHost((void**)&ctx->cp_ring, 64 * sizeof(CallParams)));
   {
     const size_t mbz = (size_t)opt.max_batch;
     ctx->zc_query_cap = std::min<size_t>(mbz * d * 4, (size_t)1 << 20);
@@ -651,7 +693,7 @@ rb_status rb_create(rb_ctx** out, const void* bank_emb, const float* bank_qualit
   {
     size_t off = 0;
     auto take = [&](size_t bytes) { const size_t o = off; off = (off + bytes + 255) & ~(size_t)255; return o; };
-    const size_t o_cp = take(sizeof(CallParams)), o_plen = take(mb * 4), o_csim = take(mb * ctx->kc * 4),
+    const size_t o_plen = take(mb * 4), o_csim = take(mb * ctx->kc * 4),
                  o_cidx = take(mb * ctx->kc * 4), o_pq = take(mb * M * 4), o_pl = take(mb * M * 4), o_sq = take(mb * M * 4),
                  o_sl = take(mb * M * 4), o_ta = take(mb * M * 4), o_tp = take(mb * M * 4), o_key = take(mb * 4),
                  o_ord = take(mb * 4), o_asg = take(mb * 4), o_mt = take(mb * 4), o_bud = take(mb * 4),
@@ -661,7 +703,7 @@ rb_status rb_create(rb_ctx** out, const void* bank_emb, const float* bank_qualit
                  o_aux = take((size_t)kMaxI * kMaxFeatures * 4), o_tpot0 = take(kMaxI * 4);
     ALLOC(ctx->arena, off);
     uint8_t* a = ctx->arena;
-    ctx->cp = (CallParams*)(a + o_cp); ctx->plen = (int32_t*)(a + o_plen); ctx->cand_sim = (float*)(a + o_csim);
+    ctx->plen = (int32_t*)(a + o_plen); ctx->cand_sim = (float*)(a + o_csim);
     ctx->cand_idx = (int32_t*)(a + o_cidx); ctx->pred_q = (float*)(a + o_pq); ctx->pred_l = (float*)(a + o_pl);
     ctx->stage_q = (float*)(a + o_sq); ctx->stage_l = (float*)(a + o_sl); ctx->termA = (float*)(a + o_ta);
     ctx->termP = (float*)(a + o_tp); ctx->key = (float*)(a + o_key); ctx->order = (int32_t*)(a + o_ord);
@@ -735,9 +777,7 @@ rb_status rb_set_instances(rb_ctx* ctx, int32_t I, const int32_t* tier, const in
       ctx->I = 0;
       return fail(ctx, RB_ENOMEM, "cudaMalloc scores");
     }
-    for (auto& kv : ctx->graphs) cudaGraphExecDestroy(kv.second);   // grid shapes depend on I
-    ctx->graphs.clear();
-    ctx->graph_nodes.clear();
+    drop_graphs(ctx);   // grid shapes depend on I
   }
   CK(cudaMemcpyAsync(ctx->tier, tier, I * 4, cudaMemcpyHostToDevice, s));
   CK(cudaMemcpyAsync(ctx->cap, cap, I * 4, cudaMemcpyHostToDevice, s));
@@ -800,9 +840,7 @@ rb_status rb_set_tpot_forest(rb_ctx* ctx, const rb_tree_node* nodes, int32_t n_n
   if (n_features != ctx->f_features) CK(cudaMemsetAsync(ctx->f_aux, 0, (size_t)kMaxI * kMaxFeatures * 4, s));
   ctx->f_features = n_features;
   ctx->has_forest = true;
-  for (auto& kv : ctx->graphs) cudaGraphExecDestroy(kv.second);   // captured kernel arguments hold the old forest
-  ctx->graphs.clear();
-  ctx->graph_nodes.clear();
+  drop_graphs(ctx);   // captured kernel arguments hold the old forest
   return RB_OK;
 }
 
@@ -1106,16 +1144,13 @@ const char* rb_last_error(const rb_ctx* ctx) { return ctx ? ctx->err.c_str() : "
 void rb_destroy(rb_ctx* ctx) {
   if (!ctx) return;
   if (ctx->stream) cudaStreamSynchronize(ctx->stream);
-  for (auto& kv : ctx->graphs) cudaGraphExecDestroy(kv.second);
+  drop_graphs(ctx);
   void* ptrs[] = {ctx->bank, ctx->bank_quality, ctx->bank_outlen, ctx->arena, ctx->q32, ctx->qs, ctx->part_sim,
                   ctx->gthr, ctx->sims, ctx->scratch_nn_idx, ctx->scratch_nn_sim, ctx->scores, ctx->scores0, ctx->f_nodes,
                   ctx->f_root, ctx->f_begin, ctx->f_base, ctx->dev_clock};
   for (void* p : ptrs) cudaFree(p);
   for (auto& e : ctx->ev)
     if (e) cudaEventDestroy(e);
-  for (auto& e : ctx->cp_ev)
-    if (e) cudaEventDestroy(e);
-  if (ctx->cp_ring) cudaFreeHost(ctx->cp_ring);
   if (ctx->h_zc) cudaFreeHost(ctx->h_zc);
   if (ctx->own_stream) cudaStreamDestroy(ctx->stream);
   delete ctx;

@@ -211,7 +211,7 @@ cudaError_t launch_convert_bf16(const float* in, __nv_bfloat16* out, size_t n, c
 // a0: cp->query (fp32) -> bf16 staging [Bpad x d]; rep copies of the B queries at rows j*(128/rep) + r (rep > 1 only
 // when Bpad = 128), all other rows zero.  Also clears gthr [n_gthr] (the scan's cross-slab thresholds).
 // Block 0 also applies the cp->n_adv pending state advances (a8's drain rule, linear head) to (dq, bq), in call order.
-cudaError_t launch_stage_queries(const CallParams* cp, __nv_bfloat16* qs, int B, int Bpad, int d, int rep, uint32_t* gthr,
+cudaError_t launch_stage_queries(const CallParams& cp, __nv_bfloat16* qs, int B, int Bpad, int d, int rep, uint32_t* gthr,
                                  int n_gthr, InstTable t, float* dq, int32_t* bq, cudaStream_t s);
 // query replicas over the TMEM lane quarters: 4 (B <= 32), 2 (B <= 64), 1; halved while the finishing kernel could not
 // hold max_grid * replicas lists of kcap entries in shared memory (long lists: k = 32)
@@ -241,7 +241,7 @@ cudaError_t scan_tc2_prepare();
 
 // a1 (fp32 storage): exact fp64-accumulated similarities of nq queries (q: [nq x d]) to sims [nq x N],
 // then per-query selection of the kc best (sim desc, idx asc) into cand_* [nq x kc].
-cudaError_t launch_scan_f32(const float* bank, const CallParams* cp, int r0, int64_t N, int d, int nq, float* sims,
+cudaError_t launch_scan_f32(const float* bank, const CallParams& cp, int r0, int64_t N, int d, int nq, float* sims,
                             cudaStream_t s);
 cudaError_t launch_select_f32(const float* sims, int64_t N, int nq, int kc, float* cand_sim, int32_t* cand_idx,
                               cudaStream_t s);
@@ -274,18 +274,20 @@ struct FinishArgs {
   float* termP;
   float* key;
 };
-cudaError_t launch_finish(const FinishArgs& a, InstTable t, const CallParams* cp, int B, cudaStream_t s);
+cudaError_t launch_finish(const FinishArgs& a, InstTable t, const CallParams& cp, int B, cudaStream_t s);
+int estimate_cp_arg(const void* func, int* nargs);   // which argument of a kernel of estimate.cu holds the CallParams (-1: none)
+int dispatch_cp_arg(const void* func, int* nargs);   // likewise for score_dispatch.cu
 size_t finish_smem_bytes(int nlists, int kcap);
 cudaError_t finish_prepare(size_t max_smem);
 
 // a4+a5 from caller-supplied predictions (cp->q_src, cp->l_src): per-(request, tier) terms, LPT keys and the
 // batch-start score matrix (cp->scores0 when non-NULL).
-cudaError_t launch_score(InstTable t, const float* dq, const int32_t* bq, const CallParams* cp, int B, float* termA,
+cudaError_t launch_score(InstTable t, const float* dq, const int32_t* bq, const CallParams& cp, int B, float* termA,
                          float* termP, float* key, DispatchModes modes, ForestDev forest, cudaStream_t s);
 
 // a6+a7: LPT sort + greedy dispatch with dead-reckoned updates, one CTA.
 cudaError_t launch_lpt_dispatch(InstTable t, float* dq, int32_t* bq, const float* termA, const float* termP,
-                                const float* key, const CallParams* cp, int B, DispatchModes modes, ForestDev forest,
+                                const float* key, const CallParams& cp, int B, DispatchModes modes, ForestDev forest,
                                 cudaStream_t s);
 
 cudaError_t lpt_dispatch_prepare();  // opt in to the dynamic shared memory size; call once
