@@ -457,3 +457,62 @@ int orc_scan_fast_f32(const float* bank, const float* query, int64_t N, int d, i
 }
 
 }  // extern "C"
+
+// ---- pipeline mode: "Equation 1 is bypassed, a pluggable estimator first picks a model ..., and a dispatcher
+// (round-robin, shortest-queue, or random) places the request within that model's replica pool."  The model choice is an
+// INPUT here (the paper's model-picking estimators are comparison systems); what is stated is the three dispatchers,
+// in input order, over the same dead-reckoned state and with the same update as the greedy pass (reading 18):
+//   policy 0 round-robin    the tier's instances in index order, a cursor per tier that persists across batches
+//   policy 1 shortest queue  the tier's instance with the smallest d_i, ties -> smaller i
+//   policy 2 random          member (splitmix64(seed + counter) mod n_m) of the tier's instances in index order; counter =
+//                            number of requests placed so far (persists across batches), so both sides draw the same numbers
+// A request whose tier has no instance gets assignment -1 and changes nothing.
+extern "C" {
+
+static inline uint64_t splitmix64(uint64_t x) {
+  x += 0x9e3779b97f4a7c15ull;
+  x = (x ^ (x >> 30)) * 0xbf58476d1ce4e5b9ull;
+  x = (x ^ (x >> 27)) * 0x94d049bb133111ebull;
+  return x ^ (x >> 31);
+}
+
+uint64_t orc_splitmix64(uint64_t x) { return splitmix64(x); }
+
+int orc_pipeline_dispatch(int I, int M, const int32_t* tier, const int32_t* cap, const float* dq_in, const int32_t* bq_in,
+                          const int32_t* model, const float* outlen /*B x M or NULL: no update*/, int B, int policy,
+                          uint64_t seed, uint64_t* counter /*in/out*/, int32_t* cursor /*M, in/out*/, int32_t* assignment,
+                          float* dq_out, int32_t* bq_out) {
+  std::vector<float> dq(dq_in, dq_in + I);
+  std::vector<int32_t> bq(bq_in, bq_in + I);
+  for (int r = 0; r < B; ++r) {
+    const int m = model[r];
+    std::vector<int> members;
+    if (m >= 0 && m < M)
+      for (int i = 0; i < I; ++i)
+        if (tier[i] == m) members.push_back(i);
+    if (members.empty()) { assignment[r] = -1; continue; }
+    const int n = (int)members.size();
+    int pick;
+    if (policy == 0) {
+      pick = members[cursor[m] % n];
+      cursor[m] = (cursor[m] + 1) % n;
+    } else if (policy == 1) {
+      pick = members[0];
+      for (int i : members)
+        if (dq[i] < dq[pick]) pick = i;
+    } else {
+      pick = members[(int)(splitmix64(seed + *counter) % (uint64_t)n)];
+    }
+    *counter += 1;
+    assignment[r] = pick;
+    if (outlen) {
+      dq[pick] = dq[pick] + outlen[(int64_t)r * M + m];
+      if (bq[pick] < cap[pick]) bq[pick] += 1;
+    }
+  }
+  if (dq_out) std::copy(dq.begin(), dq.end(), dq_out);
+  if (bq_out) std::copy(bq.begin(), bq.end(), bq_out);
+  return 0;
+}
+
+}  // extern "C"

@@ -265,3 +265,23 @@ def matching_replay(scores0, quota, greedy=None):
     objective = float(S.astype(np.float64)[np.arange(B), match].sum())
     diverged = None if greedy is None else int((match != np.asarray(greedy)).sum())
     return dict(match=match, objective=objective, diverged=diverged)
+
+
+def splitmix64(x):
+    lib().orc_splitmix64.restype = ctypes.c_uint64
+    return int(lib().orc_splitmix64(ctypes.c_uint64(x)))
+
+
+def pipeline_dispatch(inst, queued, running, model, outlen, policy, seed=0, counter=0, cursor=None):
+    """Pipeline-mode dispatchers.  Returns dict(assignment, queued, running, counter, cursor)."""
+    queued, running, model = _f32(queued), _i32(running), _i32(model)
+    B = model.shape[0]
+    ol = None if outlen is None else _f32(outlen)
+    cur = np.zeros(inst.M, dtype=np.int32) if cursor is None else _i32(cursor).copy()
+    cnt = ctypes.c_uint64(counter)
+    a = np.empty(B, dtype=np.int32)
+    dq = np.empty(inst.I, dtype=np.float32)
+    bq = np.empty(inst.I, dtype=np.int32)
+    lib().orc_pipeline_dispatch(inst.I, inst.M, _p(inst.tier), _p(inst.cap), _p(queued), _p(running), _p(model), _p(ol), B,
+                                int(policy), ctypes.c_uint64(seed), ctypes.byref(cnt), _p(cur), _p(a), _p(dq), _p(bq))
+    return dict(assignment=a, queued=dq, running=bq, counter=int(cnt.value), cursor=cur)
