@@ -205,6 +205,21 @@ rb_status rb_decide_from_predictions_budgeted(rb_ctx* ctx, const float* quality,
                                               int32_t commit, int32_t* assignment, int32_t* max_tokens, float* scores,
                                               float* scores0, int32_t* order);
 
+/* Pipeline mode ("Equation 1 is bypassed, a pluggable estimator first picks a model ..., and a dispatcher
+ * (round-robin, shortest-queue, or random) places the request within that model's replica pool").  The model choice is
+ * the caller's (the paper's model-picking estimators are comparison systems, out of scope); the library places each
+ * request, in input order, inside the chosen tier's replica pool and applies the greedy pass's dead-reckoning update.
+ *   model       [host|device] B int32: tier chosen for each request, in [0,M)
+ *   outlen      [host|device] B x M fp32 predicted output lengths, or NULL: no dead-reckoning update
+ *   policy      0 round-robin (instances of the tier in index order; one cursor per tier, kept across calls),
+ *               1 shortest queue (smallest queued_tokens, ties -> smaller index),
+ *               2 random (member splitmix64(seed + n) mod pool size, n = requests placed so far on this context)
+ *   commit      0: leave the state, cursors and draw counter untouched
+ *   assignment  [host|device] B int32; -1 for a request whose tier has no instance
+ * Cursors and the draw counter are reset by rb_set_instances. */
+rb_status rb_dispatch_pipeline(rb_ctx* ctx, const int32_t* model, const float* outlen, int32_t B, int32_t policy,
+                               uint64_t seed, int32_t commit, int32_t* assignment);
+
 /* Batch-level matching replay ("A batch-level matching (e.g. Hungarian) would differ only through within-batch
  * state updates, and an offline replay over the logged score matrices changes 15.6% of assignments").  Finds the
  * assignment a of the B requests that maximises sum_r scores0[r, a(r)] with at most quota[i] requests on instance i and

@@ -8,7 +8,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "librouteb.so")
-SOURCES = ["rb_api.cu", "scan_tc.cu", "scan_tc2.cu", "estimate.cu", "score_dispatch.cu", "match_replay.cu"]
+SOURCES = ["rb_api.cu", "scan_tc.cu", "scan_tc2.cu", "estimate.cu", "score_dispatch.cu", "match_replay.cu", "pipeline_dispatch.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC",
          "-diag-suppress", "177"]

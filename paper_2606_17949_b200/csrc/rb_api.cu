@@ -60,6 +60,8 @@ struct rb_ctx {
   int32_t *order = nullptr, *assignment = nullptr, *max_tokens = nullptr;
   float* budget = nullptr;          // [max_batch] staging of host budgets
   uint8_t* arena = nullptr;         // one allocation behind all the small per-decision buffers
+  int32_t *members = nullptr, *tstart = nullptr, *pipe_cursor = nullptr;   // pipeline mode: tier membership, cursors
+  unsigned long long* pipe_counter = nullptr;
   // Host callers of rb_decide: inputs are copied (host memcpy) into this pinned block, which the kernels read over the
   // bus directly, and the assignment is written into it by the dispatch kernel -- no copy-engine transfers on the path.
   uint8_t* h_zc = nullptr;          // pinned host block: [query | plen | budget | assignment]
@@ -700,7 +702,8 @@ rb_status rb_create(rb_ctx** out, const void* bank_emb, const float* bank_qualit
                  o_tier = take(kMaxI * 4), o_cap = take(kMaxI * 4), o_dq = take(kMaxI * 4), o_bq = take(kMaxI * 4),
                  o_pres = take(kMaxM * 4), o_pin = take(kMaxM * 4), o_pout = take(kMaxM * 4), o_pre = take(kMaxM * 4),
                  o_dec = take(kMaxM * 4), o_slope = take(kMaxM * 4), o_deci = take(kMaxI * 4), o_slopei = take(kMaxI * 4),
-                 o_aux = take((size_t)kMaxI * kMaxFeatures * 4), o_tpot0 = take(kMaxI * 4);
+                 o_aux = take((size_t)kMaxI * kMaxFeatures * 4), o_tpot0 = take(kMaxI * 4), o_mem = take(kMaxI * 4),
+                 o_tst = take((kMaxM + 1) * 4), o_cur = take(kMaxM * 4), o_cnt = take(8);
     ALLOC(ctx->arena, off);
     uint8_t* a = ctx->arena;
     ctx->plen = (int32_t*)(a + o_plen); ctx->cand_sim = (float*)(a + o_csim);
@@ -713,6 +716,8 @@ rb_status rb_create(rb_ctx** out, const void* bank_emb, const float* bank_qualit
     ctx->price_out = (float*)(a + o_pout); ctx->pre = (float*)(a + o_pre); ctx->dec = (float*)(a + o_dec);
     ctx->slope = (float*)(a + o_slope); ctx->dec_i = (float*)(a + o_deci); ctx->slope_i = (float*)(a + o_slopei);
     ctx->f_aux = (float*)(a + o_aux); ctx->f_tpot0 = (float*)(a + o_tpot0);
+    ctx->members = (int32_t*)(a + o_mem); ctx->tstart = (int32_t*)(a + o_tst); ctx->pipe_cursor = (int32_t*)(a + o_cur);
+    ctx->pipe_counter = (unsigned long long*)(a + o_cnt);
     CK(cudaMemsetAsync(ctx->arena, 0, off, s));
   }
   if (opt.store_dtype == RB_BF16) {
@@ -765,6 +770,13 @@ rb_status rb_set_instances(rb_ctx* ctx, int32_t I, const int32_t* tier, const in
   }
   std::vector<float> dec_i(I), slope_i(I);
   for (int i = 0; i < I; ++i) { dec_i[i] = dec[tier[i]]; slope_i[i] = slope[tier[i]]; }
+  std::vector<int32_t> members, tstart(kMaxM + 1, 0);   // pipeline mode: instances by (tier, index)
+  for (int m = 0; m < M; ++m) {
+    tstart[m] = (int32_t)members.size();
+    for (int i = 0; i < I; ++i)
+      if (tier[i] == m) members.push_back(i);
+  }
+  for (int m = M; m <= kMaxM; ++m) tstart[m] = (int32_t)members.size();
   cudaStream_t s = ctx->stream;
   // scores buffers depend on I
   if (I != ctx->I) {
@@ -790,6 +802,10 @@ rb_status rb_set_instances(rb_ctx* ctx, int32_t I, const int32_t* tier, const in
   CK(cudaMemcpyAsync(ctx->dec_i, dec_i.data(), I * 4, cudaMemcpyHostToDevice, s));
   CK(cudaMemcpyAsync(ctx->slope_i, slope_i.data(), I * 4, cudaMemcpyHostToDevice, s));
   ctx->n_pending = 0;   // the state is reset
+  CK(cudaMemcpyAsync(ctx->members, members.data(), I * 4, cudaMemcpyHostToDevice, s));
+  CK(cudaMemcpyAsync(ctx->tstart, tstart.data(), (kMaxM + 1) * 4, cudaMemcpyHostToDevice, s));
+  CK(cudaMemsetAsync(ctx->pipe_cursor, 0, kMaxM * 4, s));
+  CK(cudaMemsetAsync(ctx->pipe_counter, 0, 8, s));
   CK(cudaMemsetAsync(ctx->dq, 0, kMaxI * 4, s));
   CK(cudaMemsetAsync(ctx->bq, 0, kMaxI * 4, s));
   CK(cudaMemsetAsync(ctx->f_aux, 0, (size_t)kMaxI * kMaxFeatures * 4, s));
@@ -1061,6 +1077,27 @@ int rb_debug_timeline(rb_ctx* ctx, unsigned long long* out, int reset) {
   return 0;
 }
 #endif
+
+rb_status rb_dispatch_pipeline(rb_ctx* ctx, const int32_t* model, const float* outlen, int32_t B, int32_t policy,
+                               uint64_t seed, int32_t commit, int32_t* assignment) {
+  if (!ctx) return RB_EINVAL;
+  if (ctx->I == 0) return fail(ctx, RB_ESTATE, "rb_dispatch_pipeline before rb_set_instances");
+  if (!model || !assignment) return fail(ctx, RB_EINVAL, "NULL argument");
+  if (B < 1 || B > ctx->opt.max_batch) return fail(ctx, RB_EINVAL, "B out of range [1,max_batch]");
+  if (policy < 0 || policy > 2) return fail(ctx, RB_EINVAL, "policy must be 0 (round-robin), 1 (shortest queue) or 2 (random)");
+  rb_status st = flush_pending(ctx);
+  if (st != RB_OK) return st;
+  Stager sg{ctx};
+  const int32_t* d_model = sg.in(model, ctx->order, (size_t)B * 4);
+  const float* d_outlen = outlen ? sg.in(outlen, ctx->stage_l, (size_t)B * ctx->M * 4) : nullptr;
+  int32_t* d_assign = sg.out(assignment, ctx->assignment, (size_t)B * 4);
+  if (sg.err != cudaSuccess) return fail(ctx, RB_ECUDA, "cudaMemcpyAsync (inputs)", sg.err);
+  CK(launch_pipeline_dispatch(table_of(ctx), ctx->members, ctx->tstart, ctx->dq, ctx->bq, d_model, d_outlen, B, policy,
+                              (unsigned long long)seed, ctx->pipe_counter, ctx->pipe_cursor, commit ? 1 : 0, d_assign,
+                              ctx->stream));
+  ctx->launches += 1;
+  return sg.finish();
+}
 
 rb_status rb_match_replay(rb_ctx* ctx, const float* scores0, int32_t B, const int32_t* quota, const int32_t* greedy,
                           int32_t* match, double* objective, int32_t* n_diverged) {

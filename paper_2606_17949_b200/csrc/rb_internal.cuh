@@ -307,6 +307,13 @@ cudaError_t launch_match_replay(const float* S0, int B, int I, const int32_t* qu
                                 double* objective, int32_t* n_diverged, int32_t* status, cudaStream_t s);
 cudaError_t match_replay_prepare();
 
+// Pipeline-mode dispatchers, one warp; members / tstart: instances sorted by (tier, index) and the start of each
+// tier's run; counter / cursor: device-resident draw counter and per-tier round-robin cursors.
+cudaError_t launch_pipeline_dispatch(InstTable t, const int32_t* members, const int32_t* tstart, float* dq, int32_t* bq,
+                                     const int32_t* model, const float* outlen, int B, int policy, unsigned long long seed,
+                                     unsigned long long* counter, int32_t* cursor, int commit, int32_t* assignment,
+                                     cudaStream_t s);
+
 // a8: dead reckoning between batches.
 cudaError_t launch_advance(InstTable t, float* dq, int32_t* bq, float elapsed_ms, cudaStream_t s);
 

@@ -121,6 +121,14 @@ class Router:
                                       out["scores"], out["scores0"], out["order"])
         return out
 
+    def dispatch_pipeline(self, model, outlen, policy, seed=0, commit=1):
+        """Pipeline-mode dispatchers: model [B] int32 tiers, outlen [B,M] or None; returns assignment [B]."""
+        B = model.shape[0]
+        a = torch.empty(B, dtype=torch.int32, device=model.device)
+        rb.rb_dispatch_pipeline(self.ctx, model.contiguous().to(torch.int32), None if outlen is None else outlen.contiguous().float(),
+                                B, policy, seed, commit, a)
+        return a
+
     def match_replay(self, scores0, quota, greedy=None):
         """Quota-constrained optimum of the batch-start score matrix; returns (match, objective, n_diverged)."""
         B = scores0.shape[0]

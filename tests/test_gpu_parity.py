@@ -718,3 +718,42 @@ def test_deferred_advance_on_a_bank_that_does_not_fill_the_gpu(orc):
             assert np.array_equal(a.cpu().numpy(), r["assignment"]), step
             assert np.array_equal(s[0].numpy(), dq) and np.array_equal(s[1].numpy(), bq), step
     rt.close()
+
+
+@pytest.mark.parametrize("I,M,B", [(13, 4, 16), (64, 4, 200), (256, 8, 1024), (6, 3, 9)])
+@pytest.mark.parametrize("policy", [0, 1, 2])
+def test_pipeline_mode_dispatchers(orc, I, M, B, policy):
+    """P:L135 pipeline mode: round-robin / shortest-queue / random placement inside the chosen model's replica pool, three
+    consecutive batches (cursors, draw counter and dead-reckoned state persist), bit-exact against the oracle; commit=0
+    leaves everything untouched; a tier without instances places nothing."""
+    from paper_2606_17949_b200.router import Router
+    rng = np.random.default_rng(50 + I + policy)
+    it = synth.make_instances(I, M, cap=4)
+    if I == 6:
+        it["tier"] = [0, 1, 0, 1, 0, 1]          # tier 2 has no instance
+    rt = Router(torch.randn(64, 16).cuda(), torch.rand(64, M).cuda(), torch.rand(64, M).cuda() + 1, 4, store="f32", max_batch=B)
+    rt.set_instances(**it)
+    inst = orc.Instances(**it)
+    dq = rng.integers(0, 5000, I).astype(np.float32)
+    dq[: I // 2] = dq[0]
+    bq = np.minimum(rng.integers(0, 6, I), it["cap"]).astype(np.int32)
+    rt.set_state(torch.from_numpy(dq), torch.from_numpy(bq))
+    counter, cursor = 0, None
+    for batch in range(3):
+        model = rng.integers(0, M, B).astype(np.int32)
+        L = rng.lognormal(5.0, 0.5, (B, M)).astype(np.float32)
+        use_len = batch != 1
+        dry = _np({"a": rt.dispatch_pipeline(torch.from_numpy(model).cuda(), torch.from_numpy(L).cuda(), policy, seed=9, commit=0)})
+        ref = orc.pipeline_dispatch(inst, dq, bq, model, L if use_len else None, policy, seed=9, counter=counter, cursor=cursor)
+        a = rt.dispatch_pipeline(torch.from_numpy(model) if batch == 2 else torch.from_numpy(model).cuda(),
+                                 (torch.from_numpy(L) if batch == 2 else torch.from_numpy(L).cuda()) if use_len else None, policy, seed=9)
+        rt.sync()   # the library works on its own stream
+        assert np.array_equal(a.cpu().numpy(), ref["assignment"]), (batch, policy)
+        if use_len:
+            assert np.array_equal(dry["a"], ref["assignment"])      # commit=0 had changed nothing
+        if I == 6:
+            assert ((a.cpu().numpy() == -1) == (model == 2)).all()
+        dq, bq, counter, cursor = ref["queued"], ref["running"], ref["counter"], ref["cursor"]
+        s = rt.get_state()
+        assert np.array_equal(s[0].numpy(), dq) and np.array_equal(s[1].numpy(), bq)
+    rt.close()
