@@ -757,3 +757,13 @@ def test_pipeline_mode_dispatchers(orc, I, M, B, policy):
         s = rt.get_state()
         assert np.array_equal(s[0].numpy(), dq) and np.array_equal(s[1].numpy(), bq)
     rt.close()
+
+
+@pytest.mark.parametrize("k,slack,M,I,B,d", [(40, 8, 16, 40, 20, 128), (58, 6, 16, 7, 3, 64), (10, 6, 16, 100, 70, 8), (64, 0, 2, 5, 9, 72)])
+def test_full_path_at_the_limits_of_k_and_M(orc, k, slack, M, I, B, d):
+    """Largest neighbour counts (k + slack = 64), most tiers (M = 16: 32 label columns per candidate), smallest and odd
+    embedding widths (d = 8, 72), through the whole rb_decide path against the oracle."""
+    cfg = dataclasses.replace(synth.CONFIGS["C2"], N=9000, d=d, M=M, I=I, B=B, k=k, Kc=8, seed=61)
+    tol = 0.0 if slack > 0 else 4e-6
+    g, near, log = _full_parity(orc, cfg, synth.PRESETS["balanced"], sim_tol=tol, rerank_slack=slack, max_batch=128)
+    assert len(near) <= max(1, B // 10), log
