@@ -174,8 +174,18 @@ def rb_advance_state(ctx, elapsed_ms):
     _check(ctx, _lib.rb_advance_state(ctx, float(elapsed_ms)))
 
 
+_W3_CACHE = {}
+
+
 def _w3(w):
-    return ctypes.byref((_f * 3)(*[float(x) for x in w]))
+    """(w_qual, w_lat, w_cost) as a C float[3]; the handful of weight vectors a caller uses are marshalled once."""
+    key = tuple(w)
+    arr = _W3_CACHE.get(key)
+    if arr is None:
+        if len(_W3_CACHE) > 4096:
+            _W3_CACHE.clear()
+        arr = _W3_CACHE[key] = (_f * 3)(*[float(x) for x in key])
+    return ctypes.byref(arr)
 
 
 def rb_decide(ctx, query_emb, prompt_len, B, w, assignment, scores=None, pred_quality=None, pred_outlen=None,
