@@ -767,3 +767,32 @@ def test_full_path_at_the_limits_of_k_and_M(orc, k, slack, M, I, B, d):
     tol = 0.0 if slack > 0 else 4e-6
     g, near, log = _full_parity(orc, cfg, synth.PRESETS["balanced"], sim_tol=tol, rerank_slack=slack, max_batch=128)
     assert len(near) <= max(1, B // 10), log
+
+
+def test_contexts_release_their_memory():
+    """rb_destroy frees everything a context owns (device, pinned host, graphs): 30 create / decide / destroy cycles leave
+    the device's free memory where it was."""
+    from paper_2606_17949_b200.router import Router
+    cfg = dataclasses.replace(synth.CONFIGS["C2"], N=20000, d=128, B=16, Kc=8, seed=71)
+    bank = synth.make_bank(cfg, device="cuda")
+    it = synth.make_instances(cfg.I, cfg.M)
+    query = synth.make_queries(cfg, device="cuda")
+    plen = synth.make_prompt_len(cfg, device="cuda")
+
+    def cycle():
+        rt = Router(bank["emb"], bank["quality"], bank["outlen"], cfg.k, store="bf16", max_batch=64)
+        rt.set_instances(**it)
+        rt.decide(query, plen, synth.PRESETS["balanced"])
+        rt.decide(query.cpu(), plen.cpu(), synth.PRESETS["cost"])
+        rt.estimate(query[:3])
+        rt.sync()
+        rt.close()
+
+    cycle()
+    torch.cuda.synchronize()
+    free0, _ = torch.cuda.mem_get_info()
+    for _ in range(30):
+        cycle()
+    torch.cuda.synchronize()
+    free1, _ = torch.cuda.mem_get_info()
+    assert free0 - free1 < 32 * 1024 * 1024, (free0, free1)
