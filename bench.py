@@ -409,7 +409,24 @@ def cpu_baseline_and_parity(args, cfg, bank, it, queued, running, rt, rb, synth)
         n_dec += 1
     s = rt.get_state()
     state_equal = bool(np.array_equal(s[0].numpy(), dq) and np.array_equal(s[1].numpy(), bq))
-    cpu = {"value": round(done_req / t_cpu, 2), "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle",
+    # where the oracle's time goes (one window of 16 requests): stage split with all threads, the scan with one thread, and
+    # -- separately labelled, never used for parity -- the same brute-force scan with a vectorisable fp32 accumulator
+    nthreads = orc.num_threads()
+    q16, p16 = allq[:16].numpy(), allp[:16].numpy()
+    t0 = time.perf_counter(); ni, ns = orc.knn(bank_np, q16, cfg.k, store_dtype="bf16"); t_knn = time.perf_counter() - t0
+    t0 = time.perf_counter(); pq_, pl_ = orc.aggregate(ni, ns, qn, ln); t_agg = time.perf_counter() - t0
+    t0 = time.perf_counter(); orc.decide_from_predictions(inst, dq, bq, pq_, pl_, p16, weights[0]); t_disp = time.perf_counter() - t0
+    orc.set_num_threads(1)
+    t0 = time.perf_counter(); orc.knn(bank_np, q16[:2], cfg.k, store_dtype="bf16"); t_knn1 = (time.perf_counter() - t0) / 2
+    orc.set_num_threads(nthreads)
+    bank_f32 = orc.bf16_bits_to_f32(bank_np)
+    t0 = time.perf_counter(); orc.scan_fast_f32(bank_f32, q16[:4]); t_fast = (time.perf_counter() - t0) / 4
+    split = {"window": "16 requests", "knn_ms": round(t_knn * 1e3, 2), "aggregate_ms": round(t_agg * 1e3, 3),
+             "score_dispatch_ms": round(t_disp * 1e3, 3), "knn_ms_per_query_1_thread": round(t_knn1 * 1e3, 1),
+             "fast_fp32_scan_ms_per_query_1_thread": round(t_fast * 1e3, 1),
+             "note": "fast_fp32_scan: same brute-force scan, fp32 accumulator the compiler may vectorise (oracle built -O2; "
+                     "not used for parity)"}
+    cpu = {"value": round(done_req / t_cpu, 2), "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle", "split": split,
            "sample": "first %d decisions (%d requests) of a C2 stream, full oracle (fp64-accumulated brute-force KNN "
                      "+ aggregate + score + LPT), %.1f s" % (n_dec, done_req, t_cpu),
            "ms_per_decision": round(t_cpu / n_dec * 1e3, 2)}

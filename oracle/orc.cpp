@@ -74,6 +74,15 @@ int orc_num_threads(void) {
 #endif
 }
 
+// Sets the thread count of the neighbour search (bench.py's 1-thread figure); no arithmetic.
+int orc_set_num_threads(int n) {
+#ifdef _OPENMP
+  if (n >= 1) omp_set_num_threads(n);
+#endif
+  (void)n;
+  return 0;
+}
+
 // Rounds n fp32 values to bf16 (RNE); out receives the raw 16-bit patterns.
 int orc_round_bf16(const float* in, uint16_t* out, int64_t n) {
   for (int64_t i = 0; i < n; ++i) out[i] = f32_to_bf16_rne(in[i]);

@@ -52,6 +52,10 @@ def num_threads():
     return int(lib().orc_num_threads())
 
 
+def set_num_threads(n):
+    lib().orc_set_num_threads(int(n))
+
+
 def round_bf16(x):
     """fp32 array -> raw bf16 bit patterns (uint16), round-to-nearest-even."""
     x = _f32(x)
