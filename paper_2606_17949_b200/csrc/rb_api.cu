@@ -83,7 +83,7 @@ struct rb_ctx {
   int n_pending = 0;
   float *scores = nullptr, *scores0 = nullptr;  // [max_batch x I], allocated by rb_set_instances
   CUtensorMap tm_q{}, tm_bank{};
-  // graphs: key = B * 4 + kind (0 decide, 1 estimate, 2 from_predictions)
+  // graphs: key = B * 8 + kind (0 decide, 1 estimate, 2 from_predictions) + 4 if stage timing is on
   // One captured graph per decision shape.  The per-call parameters are an argument of the kernels that need them; a
   // replay rewrites that one argument of those kernel nodes (cudaGraphExecKernelNodeSetParams) -- no transfer of any
   // kind sits between the host and the decision's first kernel.
