@@ -64,6 +64,7 @@ def parse_args(argv=None):
     ap.add_argument("--only-scan-c4", action="store_true", help="run only the C4 bank-scan leg (profiling runs)")
     ap.add_argument("--c4-batch", type=int, default=64, help="B of the --only-scan-c4 leg (1..4096)")
     ap.add_argument("--only-scan-c3", action="store_true", help="run only the C3 tensor-bound scan leg (profiling runs)")
+    ap.add_argument("--only-sweep-c5", action="store_true", help="run only the C5 weight-sweep leg (profiling runs)")
     ap.add_argument("--no-large", action="store_true", help="skip the C3 (tensor-bound scan) and C5 (weight sweep) legs")
     ap.add_argument("--skip-cpu", action="store_true", help="skip the cpu_baseline / parity leg (profiling runs)")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="budget of the cpu_baseline sample")
@@ -201,6 +202,10 @@ def run_ours(args):
         return out
     if args.only_scan_c3:
         out = scan_c3(synth, Router, dev)
+        print(json.dumps(out))
+        return out
+    if args.only_sweep_c5:
+        out = sweep_c5(synth, Router, dev)
         print(json.dumps(out))
         return out
     cfg = synth.CONFIGS["C2"]
@@ -619,6 +624,28 @@ def sweep_c5(synth, Router, dev):
         rt.sync()
         shares.append(torch.bincount(tiers[o["assignment"].long()], minlength=cfg.M).tolist())
     us = np.array([a.elapsed_time(b) * 1e3 for a, b in ev])
+    # the same 66 points in ONE call (rb_sweep_weights: one CTA per point) -- the passes are independent
+    per_point = []
+    for w in pts:
+        o = rt.decide_from_predictions(est["pred_quality"], est["pred_outlen"], plen, w, commit=0)
+        rt.sync()   # torch's own stream copies what the library's stream wrote
+        per_point.append(o["assignment"].clone())
+    W = np.asarray(pts, dtype=np.float32)
+    for _ in range(2):
+        swept = rt.sweep_weights(est["pred_quality"], est["pred_outlen"], plen, W)
+    rt.sync()
+    sw = []
+    for _ in range(5):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(rt.stream)
+        swept = rt.sweep_weights(est["pred_quality"], est["pred_outlen"], plen, W)
+        b.record(rt.stream)
+        rt.sync()
+        sw.append(a.elapsed_time(b) * 1e3)
+    sweep_same = bool(all(torch.equal(swept[j], per_point[j]) for j in range(len(pts))))
+    sweep = {"call": "rb_sweep_weights, 66 points concurrently (one CTA per point)", "us_all_points": round(float(np.median(sw)), 1),
+             "us_per_point": round(float(np.median(sw)) / len(pts), 2), "equals_per_point_calls": sweep_same,
+             "speedup_vs_per_point_calls": round(float(us.sum()) / float(np.median(sw)), 1)}
     # batch-level matching replay (the paper reports 15.6 % of assignments changed, quality -0.002) of the balanced
     # point's batch-start score matrix; quota = the load the greedy pass itself put on each instance, so the matching
     # differs from greedy only through the within-batch state updates
@@ -665,6 +692,7 @@ def sweep_c5(synth, Router, dev):
             "score_dispatch_us_p50": round(float(np.median(us)), 1), "score_dispatch_us_max": round(float(us.max()), 1),
             "us_per_request_step": round(float(us.mean()) / cfg.B, 4),
             "requests_per_s_score_dispatch": round(cfg.B / (float(us.mean()) * 1e-6), 1),
+            "sweep_one_call": sweep,
             "boosted_head": {"forest": "64 trees x depth 5 per tier, 4 features, synthetic", "score_dispatch_us_mean":
                              round(float(us2.mean()), 1), "us_per_request_step": round(float(us2.mean()) / cfg.B, 4)},
             "matching_replay": replay,

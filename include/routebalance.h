@@ -205,6 +205,19 @@ rb_status rb_decide_from_predictions_budgeted(rb_ctx* ctx, const float* quality,
                                               int32_t commit, int32_t* assignment, int32_t* max_tokens, float* scores,
                                               float* scores0, int32_t* order);
 
+/* Weight sweep ("RouteBalance sweeps 16 weight tuples on the simplex"; "turning only the weight vector,
+ * RouteBalance traces a monotone frontier"): P independent score + dispatch passes over the same predictions from the
+ * same dead-reckoned state, one per weight vector, none committed.  Point p's result equals that of
+ * rb_decide_from_predictions_budgeted(..., w + 3p, commit = 0, ...); the passes are independent, so they run
+ * concurrently -- one CTA per point -- and a whole sweep costs about one pass.
+ *   quality, outlen, prompt_len, budget   as rb_decide_from_predictions_budgeted (budget NULL: no filter)
+ *   w           [host] P x 3 fp32 (qual, lat, cost per row), each row on the 3-simplex; 1 <= P <= 65535
+ *   assignment  [host|device] P x B int32, row p = the assignment under w[p]
+ * The state, the pipeline cursors and the captured graphs are left untouched.  Scratch of P*B*(2M+2)*4 bytes is kept
+ * by the context (grown on demand, released by rb_destroy). */
+rb_status rb_sweep_weights(rb_ctx* ctx, const float* quality, const float* outlen, const int32_t* prompt_len,
+                           const float* budget, int32_t B, const float* w, int32_t P, int32_t* assignment);
+
 /* Pipeline mode ("Equation 1 is bypassed, a pluggable estimator first picks a model ..., and a dispatcher
  * (round-robin, shortest-queue, or random) places the request within that model's replica pool").  The model choice is
  * the caller's (the paper's model-picking estimators are comparison systems, out of scope); the library places each

@@ -62,6 +62,8 @@ struct rb_ctx {
   uint8_t* arena = nullptr;         // one allocation behind all the small per-decision buffers
   int32_t *members = nullptr, *tstart = nullptr, *pipe_cursor = nullptr;   // pipeline mode: tier membership, cursors
   unsigned long long* pipe_counter = nullptr;
+  uint8_t* sweep_buf = nullptr;     // rb_sweep_weights: [P x 3] weights | [P][B x M] termA | termP | [P][B] key | assignment
+  size_t sweep_cap = 0;
   // Host callers of rb_decide: inputs are copied (host memcpy) into this pinned block, which the kernels read over the
   // bus directly, and the assignment is written into it by the dispatch kernel -- no copy-engine transfers on the path.
   uint8_t* h_zc = nullptr;          // pinned host block: [query | plen | budget | assignment]
@@ -1052,6 +1054,63 @@ rb_status rb_decide_from_predictions_budgeted(rb_ctx* ctx, const float* quality,
   return sg.finish();
 }
 
+rb_status rb_sweep_weights(rb_ctx* ctx, const float* quality, const float* outlen, const int32_t* prompt_len,
+                           const float* budget, int32_t B, const float* w, int32_t P, int32_t* assignment) {
+  if (!ctx) return RB_EINVAL;
+  if (ctx->I == 0) return fail(ctx, RB_ESTATE, "rb_sweep_weights before rb_set_instances");
+  if (ctx->opt.latency_mode == 2 && !ctx->has_forest) return fail(ctx, RB_ESTATE, "latency_mode 2 needs rb_set_tpot_forest first");
+  if (!quality || !outlen || !prompt_len || !w || !assignment) return fail(ctx, RB_EINVAL, "NULL argument");
+  if (B < 1 || B > ctx->opt.max_batch) return fail(ctx, RB_EINVAL, "B out of range [1,max_batch]");
+  if (P < 1 || P > 65535) return fail(ctx, RB_EINVAL, "P out of range [1,65535]");
+  if (is_host_ptr(w) == false) return fail(ctx, RB_EINVAL, "w must be host memory");
+  rb_status st = RB_OK;
+  for (int p = 0; p < P; ++p)
+    if ((st = check_weights(ctx, w + 3 * p)) != RB_OK) return st;
+  st = flush_pending(ctx);
+  if (st != RB_OK) return st;
+  // per-point scratch, grown on demand
+  const size_t pb = (size_t)P * B, pbm = pb * ctx->M;
+  auto al = [](size_t x) { return (x + 255) & ~(size_t)255; };
+  const size_t o_w = 0, o_a = al((size_t)P * 12), o_p = o_a + al(pbm * 4), o_k = o_p + al(pbm * 4), o_asg = o_k + al(pb * 4),
+               need = o_asg + al(pb * 4);
+  if (need > ctx->sweep_cap) {
+    CK(cudaStreamSynchronize(ctx->stream));
+    if (ctx->sweep_buf) cudaFree(ctx->sweep_buf);
+    ctx->sweep_buf = nullptr;
+    ctx->sweep_cap = 0;
+    cudaError_t e = cudaMalloc((void**)&ctx->sweep_buf, need);
+    if (e != cudaSuccess) { cudaGetLastError(); return fail(ctx, RB_ENOMEM, "cudaMalloc sweep scratch", e); }
+    ctx->sweep_cap = need;
+  }
+  uint8_t* sb = ctx->sweep_buf;
+  CK(cudaMemcpyAsync(sb + o_w, w, (size_t)P * 12, cudaMemcpyHostToDevice, ctx->stream));
+  const size_t bm = (size_t)B * ctx->M * 4;
+  Stager sg{ctx};
+  CallParams cp{};
+  cp.commit = 0;
+  cp.q_src = sg.in(quality, ctx->stage_q, bm);
+  cp.l_src = sg.in(outlen, ctx->stage_l, bm);
+  cp.plen = sg.in(prompt_len, ctx->plen, (size_t)B * 4);
+  cp.budget = budget ? sg.in(budget, ctx->budget, (size_t)B * 4) : nullptr;
+  cp.assignment = sg.out(assignment, reinterpret_cast<int32_t*>(sb + o_asg), pb * 4);
+  cp.sweep_w = reinterpret_cast<const float*>(sb + o_w);
+  if (sg.err != cudaSuccess) return fail(ctx, RB_ECUDA, "cudaMemcpyAsync (inputs)", sg.err);
+  st = push_params(ctx, cp);
+  if (st != RB_OK) return st;
+  InstTable t = table_of(ctx);
+  float* termA = reinterpret_cast<float*>(sb + o_a);
+  float* termP = reinterpret_cast<float*>(sb + o_p);
+  float* key = reinterpret_cast<float*>(sb + o_k);
+  if (ctx->opt.latency_mode == 2) {
+    CK(launch_tpot_forest(t, forest_of(ctx), ctx->dq, ctx->bq, ctx->f_tpot0, -1.0f, ctx->stream));
+    ctx->launches += 1;
+  }
+  CK(launch_score(t, ctx->dq, ctx->bq, ctx->cp_cur, B, termA, termP, key, modes_of(ctx), forest_of(ctx), ctx->stream, P));
+  CK(launch_lpt_dispatch(t, ctx->dq, ctx->bq, termA, termP, key, ctx->cp_cur, B, modes_of(ctx), forest_of(ctx), ctx->stream, P));
+  ctx->launches += 2;
+  return sg.finish();
+}
+
 rb_status rb_set_stage_timing(rb_ctx* ctx, int32_t enabled) {
   if (!ctx) return RB_EINVAL;
   ctx->stage_timing = enabled != 0;
@@ -1184,7 +1243,7 @@ void rb_destroy(rb_ctx* ctx) {
   drop_graphs(ctx);
   void* ptrs[] = {ctx->bank, ctx->bank_quality, ctx->bank_outlen, ctx->arena, ctx->q32, ctx->qs, ctx->part_sim,
                   ctx->gthr, ctx->sims, ctx->scratch_nn_idx, ctx->scratch_nn_sim, ctx->scores, ctx->scores0, ctx->f_nodes,
-                  ctx->f_root, ctx->f_begin, ctx->f_base, ctx->dev_clock};
+                  ctx->f_root, ctx->f_begin, ctx->f_base, ctx->dev_clock, ctx->sweep_buf};
   for (void* p : ptrs) cudaFree(p);
   for (auto& e : ctx->ev)
     if (e) cudaEventDestroy(e);

@@ -68,6 +68,8 @@ struct CallParams {
   uint32_t done_seq;       //   (host callers wait on it instead of synchronising the stream)
   int32_t n_adv;           // pending rb_advance_state calls folded into this decision's first kernel (<= kMaxPendingAdvance)
   float adv_ms[4];         // their elapsed_ms, in call order
+  const float* sweep_w;    // weight sweep (rb_sweep_weights): [P x 3] weights, point p = the CTA's grid coordinate; the
+                           //   term, key and assignment arrays are then [P][...]; NULL: the w_* fields above
 #ifdef RB_TRACE
   unsigned long long* timeline;   // development aid: [128] globaltimer stamps (even slots: earliest, odd: latest), then block 0's clock64 per slot
 #endif
@@ -283,12 +285,12 @@ cudaError_t finish_prepare(size_t max_smem);
 // a4+a5 from caller-supplied predictions (cp->q_src, cp->l_src): per-(request, tier) terms, LPT keys and the
 // batch-start score matrix (cp->scores0 when non-NULL).
 cudaError_t launch_score(InstTable t, const float* dq, const int32_t* bq, const CallParams& cp, int B, float* termA,
-                         float* termP, float* key, DispatchModes modes, ForestDev forest, cudaStream_t s);
+                         float* termP, float* key, DispatchModes modes, ForestDev forest, cudaStream_t s, int points = 1);
 
 // a6+a7: LPT sort + greedy dispatch with dead-reckoned updates, one CTA.
 cudaError_t launch_lpt_dispatch(InstTable t, float* dq, int32_t* bq, const float* termA, const float* termP,
                                 const float* key, const CallParams& cp, int B, DispatchModes modes, ForestDev forest,
-                                cudaStream_t s);
+                                cudaStream_t s, int points = 1);
 
 cudaError_t lpt_dispatch_prepare();  // opt in to the dynamic shared memory size; call once
 

@@ -121,6 +121,15 @@ class Router:
                                       out["scores"], out["scores0"], out["order"])
         return out
 
+    def sweep_weights(self, quality, outlen, prompt_len, weights, budget=None, out_device=None):
+        """P weight vectors over the same predictions and state, none committed: assignment [P, B]."""
+        B = quality.shape[0]
+        w = torch.as_tensor(weights, dtype=torch.float32, device="cpu").reshape(-1, 3).contiguous()
+        dev = out_device if out_device is not None else quality.device
+        a = torch.empty((w.shape[0], B), dtype=torch.int32, device=dev)
+        rb.rb_sweep_weights(self.ctx, quality, outlen, prompt_len, budget, B, w, w.shape[0], a)
+        return a
+
     def dispatch_pipeline(self, model, outlen, policy, seed=0, commit=1):
         """Pipeline-mode dispatchers: model [B] int32 tiers, outlen [B,M] or None; returns assignment [B]."""
         B = model.shape[0]

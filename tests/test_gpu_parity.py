@@ -796,3 +796,58 @@ def test_contexts_release_their_memory():
     torch.cuda.synchronize()
     free1, _ = torch.cuda.mem_get_info()
     assert free0 - free1 < 32 * 1024 * 1024, (free0, free1)
+
+
+@pytest.mark.parametrize("I,M,B,P,modes", [(13, 4, 16, 66, {}), (256, 8, 1024, 66, {}), (64, 4, 200, 231, {}),
+                                            (40, 4, 70, 21, dict(update_enabled=2, tiebreak_mode=1)),
+                                            (13, 4, 33, 6, dict(latency_mode=1, lpt_enabled=0)), (300, 16, 5, 300, {})])
+def test_weight_sweep_equals_one_pass_per_point(orc, I, M, B, P, modes):
+    """rb_sweep_weights (the weight sweep behind the frontier): P simplex points over the same predictions and
+    state in one call, one CTA per point; every row equals the oracle's uncommitted pass under that row's weights, with
+    and without budgets, device and host buffers; the state is left untouched and a pending advance is applied first."""
+    from paper_2606_17949_b200.router import Router
+    rng = np.random.default_rng(1000 + I + B)
+    it = synth.make_instances(I, M, cap=int(rng.integers(2, 9)))
+    rt = Router(torch.randn(64, 16).cuda(), torch.rand(64, M).cuda(), torch.rand(64, M).cuda() + 1, 4, store="f32", max_batch=B,
+                **modes)
+    rt.set_instances(**it)
+    inst = orc.Instances(**it)
+    queued = rng.integers(0, 20001, I).astype(np.float32)
+    queued[: I // 3] = queued[0]                       # replicas with equal state: exact ties
+    running = np.minimum(rng.integers(0, 12, I), it["cap"]).astype(np.int32)
+    Q = rng.uniform(0, 1, (B, M)).astype(np.float32)
+    L = rng.lognormal(5.5, 0.7, (B, M)).astype(np.float32)
+    plen = rng.integers(1, 4000, B).astype(np.int32)
+    bud = _random_budgets(rng, it, L, plen)
+    if P in (66, 231, 21, 6):
+        step = {66: 0.1, 231: 0.05, 21: 0.2, 6: 0.5}[P]
+        W = np.asarray(synth.simplex_points(step), dtype=np.float32)
+    else:
+        W = rng.dirichlet((1.0, 1.0, 1.0), P).astype(np.float32)
+        W[:, 2] = 1.0 - W[:, 0] - W[:, 1]
+        W = np.clip(W, 0.0, 1.0)
+    assert W.shape == (P, 3)
+    rt.set_state(torch.from_numpy(queued), torch.from_numpy(running))
+    rt.advance_state(23.0)
+    dq, bq = orc.advance_state(inst, queued, running, np.float32(23.0))
+    omodes = dict(lpt_enabled=modes.get("lpt_enabled", 1), update_mode=modes.get("update_enabled", 1),
+                  tiebreak_mode=modes.get("tiebreak_mode", 0), latency_mode=modes.get("latency_mode", 0))
+    for budget, host in ((None, False), (bud, False), (bud, True)):
+        dev = (lambda a: torch.from_numpy(a)) if host else (lambda a: torch.from_numpy(a).cuda())
+        a = rt.sweep_weights(dev(Q), dev(L), dev(plen), W, budget=None if budget is None else dev(budget))
+        rt.sync()
+        a = a.cpu().numpy()
+        for p in range(P):
+            ref = orc.dispatch(inst, dq, bq, Q, L, plen, W[p], budget=budget, **omodes)
+            assert np.array_equal(a[p], ref["assignment"]), (p, W[p], budget is None, host)
+        s = rt.get_state()
+        assert np.array_equal(s[0].numpy(), dq) and np.array_equal(s[1].numpy(), bq)
+    # the same context still takes ordinary decisions afterwards (graphs, scratch untouched)
+    g = _np(rt.decide_from_predictions(torch.from_numpy(Q).cuda(), torch.from_numpy(L).cuda(), torch.from_numpy(plen).cuda(),
+                                       tuple(W[P // 2]), commit=1))
+    ref = orc.dispatch(inst, dq, bq, Q, L, plen, W[P // 2], **omodes)
+    assert np.array_equal(g["assignment"], ref["assignment"])
+    with pytest.raises(Exception):
+        rt.sweep_weights(torch.from_numpy(Q).cuda(), torch.from_numpy(L).cuda(), torch.from_numpy(plen).cuda(),
+                         np.array([[0.5, 0.6, 0.1]], dtype=np.float32))        # not on the simplex
+    rt.close()
