@@ -646,6 +646,27 @@ def sweep_c5(synth, Router, dev):
     sweep = {"call": "rb_sweep_weights, 66 points concurrently (one CTA per point)", "us_all_points": round(float(np.median(sw)), 1),
              "us_per_point": round(float(np.median(sw)) / len(pts), 2), "equals_per_point_calls": sweep_same,
              "speedup_vs_per_point_calls": round(float(us.sum()) / float(np.median(sw)), 1)}
+    # frontier table: what the chosen instances look like per weight vector -- means over the batch of the
+    # predicted quality, predicted cost and predicted latency (batch-start state) of each request's chosen instance.
+    # Reporting glue in torch on the sweep's assignments; not part of the decision path.
+    dq0, bq0 = rt.get_state()
+    dq0, bq0 = dq0.to(dev), bq0.to(dev).float()
+    t_dec, t_pre, t_slope = (torch.tensor(it[k_], device=dev, dtype=torch.float32)[tiers] for k_ in ("dec", "pre", "slope"))
+    capf = torch.tensor(it["cap"], device=dev, dtype=torch.float32)
+    pin, pout = (torch.tensor(it[k_], device=dev, dtype=torch.float32) for k_ in ("price_in", "price_out"))
+    tpot_i = t_dec * (1 + t_slope * bq0)
+    wait_i = torch.where(bq0 < capf, torch.zeros_like(dq0), dq0 / bq0.clamp(min=1))
+    ar = torch.arange(cfg.B, device=dev)
+    frontier = {}
+    for j, w in enumerate(pts):
+        if max(w) == 1.0 or w in ((0.8, 0.1, 0.1), (0.1, 0.8, 0.1), (0.1, 0.1, 0.8)) or (abs(w[0] - 0.3) < 1e-9 and abs(w[1] - 0.3) < 1e-9):
+            a_ = swept[j].long()
+            m_ = tiers[a_]
+            Lh = est["pred_outlen"][ar, m_]
+            frontier["%.1f,%.1f,%.1f" % w] = {
+                "mean_Q": round(float(est["pred_quality"][ar, m_].mean()), 4),
+                "mean_C": round(float((plen.float() * pin[m_] + Lh * pout[m_]).mean()), 2),
+                "mean_T_ms_batch_start": round(float((t_pre[a_] * plen.float() + tpot_i[a_] * (wait_i[a_] + Lh)).mean()), 1)}
     # batch-level matching replay (the paper reports 15.6 % of assignments changed, quality -0.002) of the balanced
     # point's batch-start score matrix; quota = the load the greedy pass itself put on each instance, so the matching
     # differs from greedy only through the within-batch state updates
@@ -693,6 +714,7 @@ def sweep_c5(synth, Router, dev):
             "us_per_request_step": round(float(us.mean()) / cfg.B, 4),
             "requests_per_s_score_dispatch": round(cfg.B / (float(us.mean()) * 1e-6), 1),
             "sweep_one_call": sweep,
+            "frontier(qual,lat,cost)": frontier,
             "boosted_head": {"forest": "64 trees x depth 5 per tier, 4 features, synthetic", "score_dispatch_us_mean":
                              round(float(us2.mean()), 1), "us_per_request_step": round(float(us2.mean()) / cfg.B, 4)},
             "matching_replay": replay,
