@@ -851,3 +851,43 @@ def test_weight_sweep_equals_one_pass_per_point(orc, I, M, B, P, modes):
         rt.sweep_weights(torch.from_numpy(Q).cuda(), torch.from_numpy(L).cuda(), torch.from_numpy(plen).cuda(),
                          np.array([[0.5, 0.6, 0.1]], dtype=np.float32))        # not on the simplex
     rt.close()
+
+
+def test_c2_stream_10k_decisions_lockstep(orc):
+    """SURVEY 8(d), C2 as specified: 10,000 consecutive decisions of the paper-shaped stream at full size (N=100k, d=768
+    bf16, I=13; Poisson windows at 12 then 30 req/s, rb_advance_state between them, the four presets in turn) in the
+    launch configuration bench.py times.  Score / LPT / dead-reckoned state are checked in lock-step on ALL decisions
+    (bit-exact, given the GPU's predictions); neighbours and predictions against the brute-force oracle on every 10th."""
+    import bench
+    cfg = synth.CONFIGS["C2"]
+    n_dec = 10000
+    sizes, elapsed, weights = bench.c2_stream(cfg, n_dec)
+    n_req = sum(sizes)
+    bank, it, queued, running, _, _, rt = _setup(cfg, B=1, max_batch=64)
+    allq = synth.make_queries(cfg, B=n_req, device="cuda")
+    allp = synth.make_prompt_len(cfg, B=n_req, device="cuda")
+    torch.cuda.synchronize()
+    allp_np = allp.cpu().numpy()
+    bank_np = parity.bank_to_numpy(bank["emb"])
+    qn, ln = bank["quality"].cpu().numpy(), bank["outlen"].cpu().numpy()
+    inst = orc.Instances(**it)
+    dq, bq = queued.numpy().copy(), running.numpy().copy()
+    off, near_rows, knn_rows, log = 0, 0, 0, []
+    for j, (B, dt, w) in enumerate(zip(sizes, elapsed, weights)):
+        rt.advance_state(dt)
+        dq, bq = orc.advance_state(inst, dq, bq, np.float32(dt))
+        g = _np(rt.decide(allq[off:off + B], allp[off:off + B], w, want=("pred", "nn")))
+        if j % 10 == 0:
+            q_np = allq[off:off + B].cpu().numpy()
+            oi, os_, near = parity.check_topk(orc, bank_np, q_np, cfg.store, cfg.k, g["nn_idx"], g["nn_sim"], 0.0, log)
+            parity.check_predictions(orc, g["pred_quality"], g["pred_outlen"], g["nn_idx"], g["nn_sim"], oi, os_, near, qn, ln)
+            near_rows += len(near)
+            knn_rows += B
+        s = rt.get_state()
+        ref = parity.check_dispatch(orc, inst, dq, bq, g["pred_quality"], g["pred_outlen"], allp_np[off:off + B], w, g,
+                                    state_after=(s[0].numpy(), s[1].numpy()))
+        dq, bq = ref["queued"], ref["running"]
+        off += B
+    assert off == n_req and 4 <= min(sizes) and max(sizes) <= 64
+    assert near_rows <= max(3, knn_rows // 200), (near_rows, knn_rows, log[:5])   # documented near-ties only, and rare
+    rt.close()
