@@ -289,7 +289,7 @@ finish_kernel(FinishArgs a, InstTable t, const __grid_constant__ CallParams cpv)
   __shared__ float s_w[kMaxK];
   __shared__ int o_pos[kMaxK];
   __shared__ float s_lab[kMaxK][2 * kMaxM];         // labels of the kc candidates: [quality(M) | outlen(M)]
-  __shared__ float sQ[kMaxM], sL[kMaxM], sC[kMaxM];
+  __shared__ float sQ[kMaxM], sL[kMaxM];
   const int r = blockIdx.x;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int kFinThreads = blockDim.x, nwarps = blockDim.x >> 5;
@@ -635,19 +635,21 @@ finish_kernel(FinishArgs a, InstTable t, const __grid_constant__ CallParams cpv)
   }
   RB_FT(9);
   RB_TL(cp, 54);
-  if (!a.with_terms) return;
-  const uint32_t present = __ballot_sync(0xffffffffu, c_present != 0);   // warp 0's ballot covers tiers 0..M-1
-  __syncthreads();
-  // ---- per-(request, tier) terms ----
-  if (tid < M) sC[tid] = __fadd_rn(__fmul_rn(c_ell, c_pin), __fmul_rn(sL[tid], c_pout));
-  __syncthreads();
-  if (tid < M) {
-    const int m = tid;
+  if (!a.with_terms || warp != 0) return;
+  // ---- per-(request, tier) terms: warp 0 alone (2M <= 32: the predictions above were all written by its lanes) ----
+  const uint32_t present = __ballot_sync(0xffffffffu, c_present != 0);   // lanes 0..M-1 hold the tiers' flags
+  __syncwarp();
+  {
+    const int m = lane < M ? lane : 0;
+    const float L = sL[m];
+    const float C = __fadd_rn(__fmul_rn(c_ell, c_pin), __fmul_rn(L, c_pout));
     float kmax;
-    const float A = tier_term_A(m, M, present, sC, sL, sQ[m], c_wq, c_wc, has_budget, c_budget, &kmax);
-    a.termA[(size_t)r * M + m] = A;
-    a.termP[(size_t)r * M + m] = __fmul_rn(c_pre, c_ell);
-    if (m == 0) a.key[r] = kmax;
+    const float A = tier_term_A_warp(lane, present, C, L, sQ[m], c_wq, c_wc, has_budget, c_budget, &kmax);
+    if (lane < M) {
+      a.termA[(size_t)r * M + lane] = A;
+      a.termP[(size_t)r * M + lane] = __fmul_rn(c_pre, c_ell);
+      if (lane == 0) a.key[r] = kmax;
+    }
   }
   RB_FT(10);
   RB_TL(cp, 35);

@@ -157,36 +157,32 @@ __device__ __forceinline__ void grid_dependency_wait() { asm volatile("griddepco
 // Eq. 2: tier m is a candidate iff it has an instance and C[m] <= budget; if no tier fits, the cheapest
 // present tiers are the candidates (reading 24).  Cmax runs over the candidates ("normalized by their
 // candidate maxima").  Non-candidates get A = -inf, which the score and dispatch kernels read as "filtered out".
-// Also returns the LPT key max_m L^ over present tiers (budgets do not enter it).  sC / sL: [M] in shared memory.
-// present: bit j set iff tier j has an instance.
-__device__ __forceinline__ float tier_term_A(int m, int M, uint32_t present, const float* sC,
-                                             const float* sL, float Q, float wq, float wc, bool has_budget, float budget,
-                                             float* key_out) {
-  float kmax = 0.0f, Cmin = 0.0f;
-  bool first = true, any = false;
-#pragma unroll 1   // cold, once-executed code: keep it compact
-  for (int j = 0; j < M; ++j) {
-    if (!((present >> j) & 1u)) continue;
-    if (first || sL[j] > kmax) kmax = sL[j];
-    if (first || sC[j] < Cmin) Cmin = sC[j];
-    first = false;
-    any = any || !has_budget || sC[j] <= budget;
-  }
-  float Cmax = 0.0f;
-  first = true;
-  bool mine = false;
-#pragma unroll 1
-  for (int j = 0; j < M; ++j) {
-    if (!((present >> j) & 1u)) continue;
-    const bool cand = any ? (!has_budget || sC[j] <= budget) : (sC[j] == Cmin);
-    if (!cand) continue;
-    if (first || sC[j] > Cmax) Cmax = sC[j];
-    first = false;
-    if (j == m) mine = true;
-  }
+// Also returns the LPT key max_m L^ over present tiers (budgets do not enter it).
+// Warp-collective: all 32 lanes call it; lane j < M carries tier j's cost C and predicted length L (other lanes are
+// ignored: their bit of `present` is clear), present: bit j set iff tier j has an instance.  The maxima and the minimum
+// over tiers are warp reductions on the order-preserving integer image of the floats (max and min are exact, so the
+// result equals a sequential scan over the tiers); returns lane j's A[j].
+__device__ __forceinline__ uint32_t rb_f2o(float f) {   // larger float <=> larger uint
+  const uint32_t u = __float_as_uint(f);
+  return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
+}
+__device__ __forceinline__ float rb_o2f(uint32_t o) {
+  return __uint_as_float((o & 0x80000000u) ? (o & 0x7fffffffu) : ~o);
+}
+__device__ __forceinline__ float tier_term_A_warp(int lane, uint32_t present, float C, float L, float Q, float wq, float wc,
+                                                  bool has_budget, float budget, float* key_out) {
+  const bool here = (present >> lane) & 1u;
+  const uint32_t okmax = __reduce_max_sync(0xffffffffu, here ? rb_f2o(L) : 0u);
+  const uint32_t ocmin = __reduce_min_sync(0xffffffffu, here ? rb_f2o(C) : 0xffffffffu);
+  const float kmax = present ? rb_o2f(okmax) : 0.0f, Cmin = present ? rb_o2f(ocmin) : 0.0f;
+  const bool fits = here && (!has_budget || C <= budget);
+  const bool any = __any_sync(0xffffffffu, fits);
+  const bool cand = any ? fits : (here && C == Cmin);
+  const uint32_t ocmax = __reduce_max_sync(0xffffffffu, cand ? rb_f2o(C) : 0u);
+  const float Cmax = __any_sync(0xffffffffu, cand) ? rb_o2f(ocmax) : 0.0f;
   *key_out = __fadd_rn(kmax, 0.0f);   // -0 -> +0 so that the sort key order equals float order
-  if (!mine) return -INFINITY;
-  const float ct = (Cmax > 0.0f) ? __fsub_rn(1.0f, __fdiv_rn(sC[m], Cmax)) : 0.0f;
+  if (!cand) return -INFINITY;
+  const float ct = (Cmax > 0.0f) ? __fsub_rn(1.0f, __fdiv_rn(C, Cmax)) : 0.0f;
   return __fadd_rn(__fmul_rn(wq, Q), __fmul_rn(wc, ct));
 }
 
