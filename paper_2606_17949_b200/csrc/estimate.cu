@@ -568,19 +568,27 @@ finish_kernel(FinishArgs a, InstTable t, const __grid_constant__ CallParams cpv)
   }
   RB_FT(6);
   RB_TL(cp, 48);
-  // rank by counting (keys are distinct because indices are)
-  if (tid < kc) {
-    const int32_t id = s_idx[tid];
-    const unsigned long long me = (id < 0) ? 0ull : make_key(s_sim[tid], id);
+  // rank by counting (keys are distinct because indices are): warp c ranks candidate c, lane j compares candidate j
+  for (int c = warp; c < kc; c += nwarps) {
+    const int32_t id = s_idx[c];
+    const float sc = s_sim[c];
+    const unsigned long long me = (id < 0) ? 0ull : make_key(sc, id);
     int rank = 0;
-    for (int j = 0; j < kc; ++j) {
-      const int32_t oj = s_idx[j];
-      const unsigned long long other = (oj < 0) ? 0ull : make_key(s_sim[j], oj);
-      rank += (other > me) || (other == me && j < tid);
+    for (int j0 = 0; j0 < kc; j0 += 32) {
+      const int j = j0 + lane;
+      bool ahead = false;
+      if (j < kc) {
+        const int32_t oj = s_idx[j];
+        const unsigned long long other = (oj < 0) ? 0ull : make_key(s_sim[j], oj);
+        ahead = (other > me) || (other == me && j < c);
+      }
+      rank += __popc(__ballot_sync(0xffffffffu, ahead));
     }
-    o_sim[rank] = s_sim[tid];
-    o_idx[rank] = id;
-    o_pos[rank] = tid;
+    if (lane == 0) {
+      o_sim[rank] = sc;
+      o_idx[rank] = id;
+      o_pos[rank] = c;
+    }
   }
 #pragma unroll
   for (int u = 0; u < 4; ++u) {
