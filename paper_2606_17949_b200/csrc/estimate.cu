@@ -588,6 +588,21 @@ finish_kernel(FinishArgs a, InstTable t, const __grid_constant__ CallParams cpv)
       o_sim[rank] = sc;
       o_idx[rank] = id;
       o_pos[rank] = c;
+      if (rank < k) {   // ---- weight of the rank-th neighbour (the warps' square roots and divisions overlap) ----
+        float w = 1.0f;
+        if (id < 0) {
+          w = 0.0f;   // fewer than k rows reachable (cannot happen for k <= N); keeps the gather in bounds
+        } else if (a.weight_mode == 0) {
+          const float tt = __fmul_rn(2.0f, sc);
+          float u = __fsub_rn(2.0f, tt);
+          u = fmaxf(u, 0.0f);
+          const float dist = __fsqrt_rn(u);
+          w = __fdiv_rn(1.0f, __fadd_rn(dist, a.eps));
+        }
+        s_w[rank] = w;
+        if (out_nn_idx) out_nn_idx[(size_t)r * k + rank] = id;
+        if (out_nn_sim) out_nn_sim[(size_t)r * k + rank] = sc;
+      }
     }
   }
 #pragma unroll
@@ -598,34 +613,16 @@ finish_kernel(FinishArgs a, InstTable t, const __grid_constant__ CallParams cpv)
   __syncthreads();
   RB_FT(7);
   RB_TL(cp, 50);
-  // ---- weights ----
-  if (tid < k) {
-    const float s = o_sim[tid];
-    float w = 1.0f;
-    if (o_idx[tid] < 0) {
-      w = 0.0f;   // fewer than k rows reachable (cannot happen for k <= N); keeps the gather in bounds
-    } else if (a.weight_mode == 0) {
-      const float tt = __fmul_rn(2.0f, s);
-      float u = __fsub_rn(2.0f, tt);
-      u = fmaxf(u, 0.0f);
-      const float dist = __fsqrt_rn(u);
-      w = __fdiv_rn(1.0f, __fadd_rn(dist, a.eps));
-    }
-    s_w[tid] = w;
-    if (out_nn_idx) out_nn_idx[(size_t)r * k + tid] = o_idx[tid];
-    if (out_nn_sim) out_nn_sim[(size_t)r * k + tid] = s;
-  }
-  __syncthreads();
   RB_FT(8);
   RB_TL(cp, 52);
   // ---- aggregate: thread m < M -> quality, M <= thread < 2M -> output length ----
   if (tid < 2 * M) {
     const int m = tid % M;
     float num = 0.0f, den = 0.0f;
-#pragma unroll 1   // executed once, by one warp, from a cold instruction cache: compact code beats unrolled code here
+    // (a missing neighbour -- fewer than k rows reachable -- has weight 0 and position 0: it adds +0 to both sums)
+#pragma unroll 4   // the loads of four neighbours in flight; the two sums stay sequential (canonical order)
     for (int j = 0; j < k; ++j) {
       const float w = s_w[j];
-      if (o_idx[j] < 0) continue;
       const float p = __fmul_rn(w, s_lab[o_pos[j]][tid]);
       num = __fadd_rn(num, p);
       den = __fadd_rn(den, w);
