@@ -541,12 +541,15 @@ finish_kernel(FinishArgs a, InstTable t, const __grid_constant__ CallParams cpv)
 
   RB_FT(4);
   RB_TL(cp, 44);
-  // labels of all kc candidates are requested before the re-rank and parked after it (independent gathers)
+  // labels of all kc candidates are requested before the re-rank and parked after it (independent gathers); the
+  // threads are rotated by half a block so that, for the usual handful of candidates, the label gathers are issued
+  // by the upper warps while the lower ones (warp c = candidate c) already fetch their bank rows
+  const int tid_lab = (tid + (kFinThreads >> 1)) & (kFinThreads - 1);   // the block size is a power of two
   float lv[4];
   const int nlab = kc * 2 * M;   // <= 64 * 32 = 4 * 512
 #pragma unroll
   for (int u = 0; u < 4; ++u) {
-    const int e = tid + u * kFinThreads;
+    const int e = tid_lab + u * kFinThreads;
     lv[u] = 0.0f;
     if (e < nlab) {
       const int c = e / (2 * M), col = e - c * 2 * M;
@@ -607,7 +610,7 @@ finish_kernel(FinishArgs a, InstTable t, const __grid_constant__ CallParams cpv)
   }
 #pragma unroll
   for (int u = 0; u < 4; ++u) {
-    const int e = tid + u * kFinThreads;
+    const int e = tid_lab + u * kFinThreads;
     if (e < nlab) s_lab[e / (2 * M)][e % (2 * M)] = lv[u];
   }
   __syncthreads();
