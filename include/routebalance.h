@@ -74,6 +74,8 @@ typedef struct {
   float dist_eps;         /* eps above.                                                   default 1e-6    */
   int32_t rerank_slack;   /* RB_BF16 only: the scan keeps k+slack candidates per query, their similarities */
                           /* are recomputed exactly (fp64 accumulate) and the best k kept. default 6       */
+                          /* 0: no re-rank; similarities are the tensor core's fp32 sums (within 4e-6), and  */
+                          /* inverse-distance weights amplify that as a neighbour's similarity nears 1.      */
   int32_t lpt_enabled;    /* 1: dispatch in LPT order; 0: in input order.         default 1       */
   int32_t update_enabled; /* dead-reckoning update after each dispatch: 1: d += L^ and the decode batch   */
                           /* grows by one while a slot is free (default); 2: d only (P:L121 literally); 0: none   */

@@ -49,7 +49,7 @@ def _full_parity(orc, cfg, w, B=None, sim_tol=0.0, **kw):
     log = []
     oi, os_, near = parity.check_topk(orc, bank_np, query_np, cfg.store, cfg.k, g["nn_idx"], g["nn_sim"], sim_tol, log)
     parity.check_predictions(orc, g["pred_quality"], g["pred_outlen"], g["nn_idx"], g["nn_sim"], oi, os_, near, qn, ln,
-                             weight_mode=kw.get("weight_mode", 0))
+                             weight_mode=kw.get("weight_mode", 0), raw_sums=sim_tol > 0)
     inst = orc.Instances(**it)
     state = rt.get_state()
     parity.check_dispatch(orc, inst, queued.numpy(), running.numpy(), g["pred_quality"], g["pred_outlen"], plen_np, w, g,
