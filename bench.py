@@ -429,8 +429,9 @@ def cpu_baseline_and_parity(args, cfg, bank, it, queued, running, rt, rb, synth)
     split = {"window": "16 requests", "knn_ms": round(t_knn * 1e3, 2), "aggregate_ms": round(t_agg * 1e3, 3),
              "score_dispatch_ms": round(t_disp * 1e3, 3), "knn_ms_per_query_1_thread": round(t_knn1 * 1e3, 1),
              "fast_fp32_scan_ms_per_query_1_thread": round(t_fast * 1e3, 1),
-             "note": "fast_fp32_scan: same brute-force scan, fp32 accumulator the compiler may vectorise (oracle built -O2; "
-                     "not used for parity)"}
+             "note": "fast_fp32_scan: same brute-force scan over an fp32 copy of the bank (307 MB per query), fp32 accumulator, "
+                     "omp-simd reduction (AVX2 where the host has it): one thread streams the bank at memory speed; not used "
+                     "for parity"}
     cpu = {"value": round(done_req / t_cpu, 2), "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle", "split": split,
            "sample": "first %d decisions (%d requests) of a C2 stream, full oracle (fp64-accumulated brute-force KNN "
                      "+ aggregate + score + LPT), %.1f s" % (n_dec, done_req, t_cpu),

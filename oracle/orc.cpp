@@ -448,20 +448,34 @@ int orc_advance_state_gbdt(int I, const int32_t* tier, const orc_forest* forest,
 }
 
 // A second, separately labelled CPU figure for bench.py only (never used for parity): the same brute-force
-// scan with an fp32 accumulator the compiler may vectorise.  Returns the index of the best row per query.
-int orc_scan_fast_f32(const float* bank, const float* query, int64_t N, int d, int B, int32_t* best) {
-  for (int r = 0; r < B; ++r) {
-    float bs = -INFINITY;
-    int32_t bi = 0;
-    const float* x = query + (int64_t)r * d;
-    for (int64_t n = 0; n < N; ++n) {
-      const float* e = bank + n * d;
-      float acc = 0.0f;
-      for (int c = 0; c < d; ++c) acc += x[c] * e[c];
-      if (acc > bs) { bs = acc; bi = (int32_t)n; }
-    }
-    best[r] = bi;
+// scan with an fp32 accumulator whose sum the compiler may reorder and vectorise (omp simd reduction; AVX2 when the
+// host has it).  Returns the index of the best row per query.
+#define ORC_FAST_SCAN_BODY                                              \
+  for (int r = 0; r < B; ++r) {                                         \
+    float bs = -INFINITY;                                               \
+    int32_t bi = 0;                                                     \
+    const float* x = query + (int64_t)r * d;                            \
+    for (int64_t n = 0; n < N; ++n) {                                   \
+      const float* e = bank + n * d;                                    \
+      float acc = 0.0f;                                                 \
+      _Pragma("omp simd reduction(+ : acc)")                            \
+      for (int c = 0; c < d; ++c) acc += x[c] * e[c];                   \
+      if (acc > bs) { bs = acc; bi = (int32_t)n; }                      \
+    }                                                                   \
+    best[r] = bi;                                                       \
   }
+}  // extern "C"
+__attribute__((target("avx2"))) static void scan_fast_avx2(const float* bank, const float* query, int64_t N, int d, int B,
+                                                           int32_t* best) {
+  ORC_FAST_SCAN_BODY
+}
+static void scan_fast_base(const float* bank, const float* query, int64_t N, int d, int B, int32_t* best) {
+  ORC_FAST_SCAN_BODY
+}
+extern "C" {
+int orc_scan_fast_f32(const float* bank, const float* query, int64_t N, int d, int B, int32_t* best) {
+  if (__builtin_cpu_supports("avx2")) scan_fast_avx2(bank, query, N, d, B, best);
+  else scan_fast_base(bank, query, N, d, B, best);
   return 0;
 }
 
