@@ -168,7 +168,9 @@ rb_status rb_advance_state(rb_ctx* ctx, float elapsed_ms);
  *   query_emb    [host|device] B x d fp32 prompt embeddings (unit norm expected, not enforced)
  *   prompt_len   [host|device] B int32 input token counts l_r >= 0
  *   w            [host] (w_qual, w_lat, w_cost), each >= 0, |sum - 1| <= 1e-5
- *   assignment   [host|device] B int32: chosen instance per request (indexed like the input batch)
+ *   assignment   [host|device] B int32: chosen instance per request (indexed like the input batch); -1 = no admissible
+ *                instance, which only non-finite inputs can produce (a NaN label, prediction, price or budget makes every
+ *                cost comparison of the request false); labels, predictions and budgets are not checked for finiteness
  *   scores       [host|device] B x I fp32 or NULL: row r = S[r,:] as seen when r was dispatched
  *   pred_quality [host|device] B x M or NULL; pred_outlen likewise
  *   nn_idx       [host|device] B x k int32 or NULL: neighbours, best first (similarity desc, index asc)
@@ -254,24 +256,6 @@ rb_status rb_match_replay(rb_ctx* ctx, const float* scores0, int32_t B, const in
 /* The estimate stage alone (KNN scan + merge + aggregate); outputs as in rb_decide, any may be NULL. */
 rb_status rb_estimate(rb_ctx* ctx, const float* query_emb, int32_t B, float* pred_quality,
                       float* pred_outlen, int32_t* nn_idx, float* nn_sim);
-
-/* Device time of the stages of the most recent rb_decide / rb_estimate on this context, measured with
- * CUDA events on the context's stream (only when the call ran with stage timing enabled through
- * rb_set_stage_timing(ctx, 1); the decision is then replayed from a graph with event-record nodes between its kernels,
- * which serialises them: each stage's interval is meaningful, their sum is longer than an untimed decision).
- *   us [host] 6 floats: stage (query staging), scan, merge, aggregate, score, dispatch. */
-rb_status rb_set_stage_timing(rb_ctx* ctx, int32_t enabled);
-rb_status rb_last_stage_us(rb_ctx* ctx, float us[6]);
-
-/* Duration of the bank-scan kernel of the most recent rb_decide / rb_estimate that ran with stage timing enabled, on
- * the device's own clock: latest CTA end - earliest CTA start (globaltimer), in microseconds; 0 if not measured (fp32
- * storage, B > 128, or stage timing off).  Unlike the event interval in rb_last_stage_us it holds no launch latency. */
-rb_status rb_last_scan_device_us(rb_ctx* ctx, float* us);
-
-/* Self-test of the dispatch kernel's branch-free fp32 division (reciprocal refinement without the compiler's range check;
- * used only for operands inside the exponent window where it is exact, IEEE __fdiv_rn otherwise): compares it with the
- * IEEE division bit for bit on n_pairs pseudo-random in-window operand pairs.  *mismatches [host] must come back 0. */
-rb_status rb_selftest_division(rb_ctx* ctx, uint64_t n_pairs, uint64_t seed, uint64_t* mismatches);
 
 /* Number of kernel launches (graph nodes count individually) issued by this context so far. */
 int64_t rb_launch_count(const rb_ctx* ctx);

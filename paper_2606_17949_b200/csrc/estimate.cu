@@ -7,19 +7,6 @@
 namespace rb {
 namespace {
 
-#ifdef RB_TRACE   // development aid (_work harness): timestamps of the finishing kernel's phases; compiled out otherwise
-__device__ unsigned long long rb_fin_trace[64 * 32];
-__device__ __forceinline__ void fin_trace(int slot) {
-  if (threadIdx.x == 0 && blockIdx.x < 64) {
-    unsigned long long t;
-    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
-    rb_fin_trace[blockIdx.x * 32 + slot] = t;
-  }
-}
-#define RB_FT(slot) fin_trace(slot)
-#else
-#define RB_FT(slot)
-#endif
 
 // Total order of candidates: similarity descending, bank index ascending (reading 3), as one 64-bit key whose
 // unsigned order is that order (larger key = better).  Key 0 is below every real candidate.
@@ -60,7 +47,6 @@ __global__ void stage_queries_kernel(const __grid_constant__ CallParams cpv, __n
       }
     }
   }
-  RB_TL_INIT(cp);
   for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n_gthr; i += gridDim.x * blockDim.x) gthr[i] = 0u;
   const float* __restrict__ q = cp->query;
   const size_t n = (size_t)Bpad * d;
@@ -69,7 +55,6 @@ __global__ void stage_queries_kernel(const __grid_constant__ CallParams cpv, __n
     const size_t r = row % group;   // replicas of query r at rows r, group + r, ...
     qs[i] = (r < (size_t)B) ? __float2bfloat16_rn(q[r * d + c]) : __float2bfloat16_rn(0.0f);
   }
-  RB_TL_FLUSH(cp, 0, 1);
 }
 __global__ void convert_bf16_kernel(const float* __restrict__ in, __nv_bfloat16* __restrict__ out, size_t n) {
   for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x)
@@ -315,15 +300,11 @@ finish_kernel(FinishArgs a, InstTable t, const __grid_constant__ CallParams cpv)
   const uint4* qrow = reinterpret_cast<const uint4*>(a.qs + (size_t)r * a.d);
   const int nvec = a.d / 8;   // d % 8 == 0
 
-  RB_FT(0);
-  RB_TL_INIT(cp);
-  RB_TL(cp, 34);
   // ---- merge ----
   const int total = a.nlists * kcap;
   launch_dependents();
   grid_dependency_wait();   // the partial lists come from the preceding kernel
   if (tid == 0) s_nflag = 0;
-  RB_TL(cp, 36);
   if (kcap & 3) {   // fp32-storage path: one already-merged list of kc entries per query
     for (int e = tid; e < total; e += kFinThreads) {
       const int c = e / kcap, j = e - c * kcap;
@@ -371,8 +352,6 @@ finish_kernel(FinishArgs a, InstTable t, const __grid_constant__ CallParams cpv)
     }
   }
   __syncthreads();
-  RB_FT(1);
-  RB_TL(cp, 38);
   // two levels, no barrier inside either: every warp pops the kc best of its own share of the lists (lane = list),
   // then warp 0 pops the kc best of the warps' results (lane = warp)
   unsigned long long* w_key = s_keys + total;                         // [nwarps][kMerge2Stride]
@@ -406,8 +385,6 @@ finish_kernel(FinishArgs a, InstTable t, const __grid_constant__ CallParams cpv)
     if (lane == 0) s_wcnt[warp] = npop;
   }
   __syncthreads();
-  RB_FT(2);
-  RB_TL(cp, 40);
   if (warp == 0) {
     // out_src of this level is the warp whose list the key came from; its position in that list is the number
     // of keys already taken from it, which recovers the original list index
@@ -462,8 +439,6 @@ finish_kernel(FinishArgs a, InstTable t, const __grid_constant__ CallParams cpv)
   }
   __syncthreads();
 
-  RB_FT(3);
-  RB_TL(cp, 42);
   // ---- rescan of slabs whose list was popped completely ----
   // (a list of kcap entries all of which are among the kc best may hide further members)
   bool flagged = false;
@@ -539,8 +514,6 @@ finish_kernel(FinishArgs a, InstTable t, const __grid_constant__ CallParams cpv)
   }
   __syncthreads();
 
-  RB_FT(4);
-  RB_TL(cp, 44);
   // labels of all kc candidates are requested before the re-rank and parked after it (independent gathers); the
   // threads are rotated by half a block so that, for the usual handful of candidates, the label gathers are issued
   // by the upper warps while the lower ones (warp c = candidate c) already fetch their bank rows
@@ -557,8 +530,6 @@ finish_kernel(FinishArgs a, InstTable t, const __grid_constant__ CallParams cpv)
       if (id >= 0) lv[u] = (col < M) ? a.bank_quality[(size_t)id * M + col] : a.bank_outlen[(size_t)id * M + col - M];
     }
   }
-  RB_FT(5);
-  RB_TL(cp, 46);
   // ---- exact re-rank ----
   if (a.rerank) {
     for (int c = warp; c < kc; c += nwarps) {
@@ -569,8 +540,6 @@ finish_kernel(FinishArgs a, InstTable t, const __grid_constant__ CallParams cpv)
     }
     __syncthreads();
   }
-  RB_FT(6);
-  RB_TL(cp, 48);
   // rank by counting (keys are distinct because indices are): warp c ranks candidate c, lane j compares candidate j
   for (int c = warp; c < kc; c += nwarps) {
     const int32_t id = s_idx[c];
@@ -614,10 +583,6 @@ finish_kernel(FinishArgs a, InstTable t, const __grid_constant__ CallParams cpv)
     if (e < nlab) s_lab[e / (2 * M)][e % (2 * M)] = lv[u];
   }
   __syncthreads();
-  RB_FT(7);
-  RB_TL(cp, 50);
-  RB_FT(8);
-  RB_TL(cp, 52);
   // ---- aggregate: thread m < M -> quality, M <= thread < 2M -> output length ----
   if (tid < 2 * M) {
     const int m = tid % M;
@@ -641,8 +606,6 @@ finish_kernel(FinishArgs a, InstTable t, const __grid_constant__ CallParams cpv)
       if (out_pl) out_pl[(size_t)r * M + m] = pred;
     }
   }
-  RB_FT(9);
-  RB_TL(cp, 54);
   if (!a.with_terms || warp != 0) return;
   // ---- per-(request, tier) terms: warp 0 alone (2M <= 32: the predictions above were all written by its lanes) ----
   const uint32_t present = __ballot_sync(0xffffffffu, c_present != 0);   // lanes 0..M-1 hold the tiers' flags
@@ -659,9 +622,6 @@ finish_kernel(FinishArgs a, InstTable t, const __grid_constant__ CallParams cpv)
       if (lane == 0) a.key[r] = kmax;
     }
   }
-  RB_FT(10);
-  RB_TL(cp, 35);
-  RB_TL_FLUSH(cp, 32, 33);
 }
 
 }  // namespace

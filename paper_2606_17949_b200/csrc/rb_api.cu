@@ -2,6 +2,7 @@
 // sequence of one decision (a0..a7) and its CUDA-graph replay (a9).  Every step of the path runs in the
 // kernels of scan_tc.cu / estimate.cu / score_dispatch.cu; nothing here computes on the host.
 #include "../../include/routebalance.h"
+#include "../../include/routebalance_testing.h"
 
 #include <algorithm>
 #include <cmath>
@@ -43,9 +44,6 @@ struct rb_ctx {
   __nv_bfloat16* qs = nullptr;      // [Bpad_max x d]
   int32_t* plen = nullptr;          // [max_batch]
   CallParams cp_cur{};              // per-call parameters of the call being enqueued (passed to the kernels by value)
-#ifdef RB_TRACE
-  unsigned long long* timeline = nullptr;
-#endif
   uint32_t* gthr = nullptr;         // [Bpad_max] cross-slab admission thresholds of the scan (cleared per decision)
   float* part_sim = nullptr;        // [num_sms][kcap][Bpad_max]
   int32_t* part_idx = nullptr;
@@ -70,10 +68,6 @@ struct rb_ctx {
   uint8_t* d_zc = nullptr;          // the same block as the device addresses it
   size_t zc_query_cap = 0, zc_off_plen = 0, zc_off_budget = 0, zc_off_assign = 0, zc_off_flag = 0;
   uint32_t done_seq = 0;
-  // is_host_ptr results of the caller pointers seen last (a serving loop passes the same buffers again and again)
-  const void* ptr_cache[8]{};
-  bool ptr_cache_host[8]{};
-  int ptr_cache_next = 0;
   // boosted TPOT head (latency_mode 2)
   int4* f_nodes = nullptr;
   int32_t *f_root = nullptr, *f_begin = nullptr;
@@ -437,10 +431,6 @@ void collect_stage_times(rb_ctx* ctx, int kind) {
 // The call's parameters: kept in the context while its kernels are enqueued (they receive them by value).
 rb_status push_params(rb_ctx* ctx, const CallParams& cp) {
   ctx->cp_cur = cp;
-#ifdef RB_TRACE
-  if (!ctx->timeline) CK(cudaMalloc((void**)&ctx->timeline, 128 * 8));
-  ctx->cp_cur.timeline = ctx->timeline;
-#endif
   return RB_OK;
 }
 
@@ -452,15 +442,8 @@ struct Stager {
   bool any_host = false;
   bool wait_flag = false;    // completion is signalled through the pinned word (no stream synchronisation needed)
   bool needs_sync = false;   // some host buffer went through the copy engine: the stream must drain
-  bool host(const void* p) {
-    for (int j = 0; j < 8; ++j)
-      if (ctx->ptr_cache[j] == p && p != nullptr) return ctx->ptr_cache_host[j];
-    const bool h = is_host_ptr(p);
-    ctx->ptr_cache[ctx->ptr_cache_next] = p;
-    ctx->ptr_cache_host[ctx->ptr_cache_next] = h;
-    ctx->ptr_cache_next = (ctx->ptr_cache_next + 1) & 7;
-    return h;
-  }
+  // classified on every call (cudaPointerGetAttributes): an address can change its memory kind between calls
+  bool host(const void* p) { return is_host_ptr(p); }
   cudaError_t err = cudaSuccess;
   struct Back { void* dst; const void* src; size_t bytes; };
   Back back[10];
@@ -952,10 +935,11 @@ rb_status rb_decide_budgeted(rb_ctx* ctx, const float* query_emb, const int32_t*
   Stager sg{ctx};
   CallParams cp{};
   cp.w_qual = w[0]; cp.w_lat = w[1]; cp.w_cost = w[2]; cp.commit = 1;
+  bool adv_folded = false;
   if (ctx->opt.store_dtype == RB_BF16 && ctx->opt.latency_mode != 2) {
     cp.n_adv = ctx->n_pending;   // applied by the staging kernel, ahead of everything that reads the state
     for (int a = 0; a < ctx->n_pending; ++a) cp.adv_ms[a] = ctx->pending_adv[a];
-    ctx->n_pending = 0;
+    adv_folded = true;           // (n_pending is cleared only once the decision has been enqueued: a failed call changes nothing)
   } else {
     st = flush_pending(ctx);
     if (st != RB_OK) return st;
@@ -986,6 +970,7 @@ rb_status rb_decide_budgeted(rb_ctx* ctx, const float* query_emb, const int32_t*
   if (st != RB_OK) return st;
   st = run_path(ctx, B, 0);
   if (st != RB_OK) return st;
+  if (adv_folded) ctx->n_pending = 0;
   collect_stage_times(ctx, 0);
   return sg.finish();
 }
@@ -1123,19 +1108,6 @@ rb_status rb_last_stage_us(rb_ctx* ctx, float us[6]) {
   return RB_OK;
 }
 
-#ifdef RB_TRACE
-int rb_debug_timeline(rb_ctx* ctx, unsigned long long* out, int reset) {
-  cudaStreamSynchronize(ctx->stream);
-  if (!ctx->timeline) cudaMalloc((void**)&ctx->timeline, 128 * 8);
-  cudaMemcpy(out, ctx->timeline, 128 * 8, cudaMemcpyDeviceToHost);
-  if (reset) {
-    unsigned long long init[128];
-    for (int j = 0; j < 128; ++j) init[j] = (j & 1) ? 0ull : ~0ull;
-    cudaMemcpy(ctx->timeline, init, sizeof init, cudaMemcpyHostToDevice);
-  }
-  return 0;
-}
-#endif
 
 rb_status rb_dispatch_pipeline(rb_ctx* ctx, const int32_t* model, const float* outlen, int32_t B, int32_t policy,
                                uint64_t seed, int32_t commit, int32_t* assignment) {

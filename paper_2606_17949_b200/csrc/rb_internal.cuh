@@ -70,9 +70,6 @@ struct CallParams {
   float adv_ms[4];         // their elapsed_ms, in call order
   const float* sweep_w;    // weight sweep (rb_sweep_weights): [P x 3] weights, point p = the CTA's grid coordinate; the
                            //   term, key and assignment arrays are then [P][...]; NULL: the w_* fields above
-#ifdef RB_TRACE
-  unsigned long long* timeline;   // development aid: [128] globaltimer stamps (even slots: earliest, odd: latest), then block 0's clock64 per slot
-#endif
 };
 
 // Dispatch modes (rb_options; SURVEY 8(f) #2, P:L227 isolation arms, P:L266 ablations).
@@ -130,26 +127,6 @@ __device__ __forceinline__ void forest_leaves_warp(const int4* __restrict__ node
 // with it, and waits (grid_dependency_wait) before it touches anything its predecessor produces.  Both are
 // no-ops for a kernel launched without the attribute.
 #ifdef __CUDACC__
-#ifdef RB_TRACE   // development aid (_work harness): kernel/phase timestamps of one decision; compiled out otherwise
-// Thread 0 of every block keeps clock64 stamps in registers/shared memory (cheap); RB_TL_FLUSH writes block 0's
-// stamps to timeline[64 + slot] and one globaltimer pair (first slot: earliest over blocks, last: latest).
-struct TlBuf { long long c[32]; unsigned long long g0; };
-__device__ __forceinline__ unsigned long long tl_gtime() {
-  unsigned long long t;
-  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
-  return t;
-}
-#define RB_TL_INIT(cp) __shared__ TlBuf tl_buf_; unsigned long long* const tl_ptr_ = (cp)->timeline; \
-  if (threadIdx.x == 0) { for (int q_ = 0; q_ < 32; ++q_) tl_buf_.c[q_] = 0; tl_buf_.g0 = tl_gtime(); }
-#define RB_TL(cp, slot) do { if (threadIdx.x == 0) tl_buf_.c[(slot) & 31] = clock64(); } while (0)
-#define RB_TL_FLUSH(cp, first, last) do { if (threadIdx.x == 0) { atomicMin(tl_ptr_ + (first), tl_buf_.g0); \
-  atomicMax(tl_ptr_ + (last), tl_gtime()); if (blockIdx.x == 0) for (int q_ = 0; q_ < 32; ++q_) if (tl_buf_.c[q_]) \
-  tl_ptr_[64 + ((first) & ~31) + q_] = (unsigned long long)tl_buf_.c[q_]; } } while (0)
-#else
-#define RB_TL_INIT(cp)
-#define RB_TL(cp, slot)
-#define RB_TL_FLUSH(cp, first, last)
-#endif
 __device__ __forceinline__ void launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 __device__ __forceinline__ void grid_dependency_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 

@@ -25,27 +25,6 @@
 namespace rb {
 namespace {
 
-#ifdef RB_TRACE   // development aid (_work harness): per-CTA timestamps of the pipeline roles; compiled out otherwise
-__device__ unsigned long long rb_trace_buf[148 * 512];
-__device__ __forceinline__ void trace(int slot) {
-  if (slot < 512) {
-    unsigned long long t;
-    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
-    rb_trace_buf[blockIdx.x * 512 + slot] = t;
-  }
-}
-#define RB_TR(slot) trace(slot)
-__device__ unsigned long long rb_scan_tl[8];   // [0] earliest start, [1] latest end, [2] earliest first TMA issue, [3] latest last-epilogue end
-__device__ __forceinline__ void scan_tl(int slot) {
-  unsigned long long t;
-  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
-  if (slot & 1) atomicMax(rb_scan_tl + slot, t); else atomicMin(rb_scan_tl + slot, t);
-}
-#define RB_STL(slot) scan_tl(slot)
-#else
-#define RB_STL(slot)
-#define RB_TR(slot)
-#endif
 
 constexpr int kStages = 4;
 constexpr int kABytes = kTileM * kTileK * 2;       // 16 KB: 128 queries x 64 bf16
@@ -54,8 +33,6 @@ constexpr int kBBytes = kTileN * kTileK * 2;       // 32 KB
 constexpr int kStageBytes = kABytes + kBBytes;     // 48 KB
 constexpr int kThreads = 192;
 constexpr int kSmemBytes = kStages * kStageBytes + kCandSlots * kTileM * 8 + 256 + 1024;
-
-__device__ __forceinline__ bool tl_trace_end(int tid) { return tid == 128; }   // epilogue thread of query 0
 
 template <int KCAP>
 __global__ void __launch_bounds__(kThreads, 1)
@@ -83,7 +60,6 @@ scan_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__
   const int ntiles = (nunits + 3) / 4;
 
   launch_dependents();
-  if (threadIdx.x == 0) { RB_TR(0); RB_STL(0); }
   if (dev_clock != nullptr && threadIdx.x == 0) {   // stage-timing mode: earliest CTA start on the device's own clock
     unsigned long long t0;
     asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t0));
@@ -111,7 +87,6 @@ scan_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot;
-  if (threadIdx.x == 0) RB_TR(1);
 
   if (warp == 0) {
     // ===== TMA producer =====
@@ -119,7 +94,6 @@ scan_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__
       grid_dependency_wait();   // the staged queries come from the preceding kernel (it ends about when this
                                 // kernel's prologue does: issuing bank boxes ahead of the wait only delayed the
                                 // first query tile behind them -- measured, reverted)
-      RB_STL(2);
       uint32_t kit = 0;
       for (int tile = 0; tile < ntiles; ++tile) {
         const int n0 = (int)(row0 + (int64_t)tile * kTileN);
@@ -134,7 +108,6 @@ scan_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__
             mbar_arrive_expect_tx(&full[s], kABytes + nun * kBoxBytes);
             tma_load_2d(sa, &tm_q, kc * kTileK, mt * kTileM, &full[s]);
             for (int u = 0; u < nun; ++u) tma_load_2d(sb + u * kBoxBytes, &tm_bank, kc * kTileK, n0 + u * kBoxN, &full[s]);
-            RB_TR(16 + kit);
           }
         }
       }
@@ -157,7 +130,6 @@ scan_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__
             const uint32_t ph = (kit / kStages) & 1;
             mbar_wait(&full[s], ph);
             tc_fence_after();
-            RB_TR(96 + kit);
             const uint32_t sa = smem_u32(smem + s * kStageBytes);
             const uint64_t adesc = make_smem_desc(sa);
             const uint64_t bdesc = make_smem_desc(sa + kABytes);
@@ -169,7 +141,6 @@ scan_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__
             tc_commit(&empty[s]);
           }
           tc_commit(&tfull[acc]);
-          RB_TR(176 + it);
         }
       }
     }
@@ -219,7 +190,6 @@ scan_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__
         }
         mbar_wait(&tfull[acc], aph);
         tc_fence_after();
-        if (tl == 0) RB_TR(192 + it);
         if (warp_active) {
           float thr = (r < B) ? v[KCAP - 1] : INFINITY;   // padding lanes never collect
           const uint32_t taddr = tmem_base + ((uint32_t)(quarter * 32) << 16) + acc * kTileN;
@@ -244,7 +214,6 @@ scan_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__
         }
         tc_fence_before();
         __syncwarp();
-        if (tl == 0) RB_TR(208 + it);
         if (lane == 0) mbar_arrive(&tempty[acc]);
         if (warp_active && r < B && (n_mt > 1 || tile == ntiles - 1)) {
 #pragma unroll
@@ -262,10 +231,8 @@ scan_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__
     }
   }
 
-  if (tl_trace_end(threadIdx.x)) { RB_TR(2); RB_STL(3); }
   tc_fence_before();
   __syncthreads();
-  if (threadIdx.x == 0) { RB_TR(3); RB_STL(1); }
   if (dev_clock != nullptr && threadIdx.x == 0) {   // ... and latest CTA end
     unsigned long long t1;
     asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t1));
@@ -279,17 +246,6 @@ scan_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__
 
 }  // namespace
 
-#ifdef RB_TRACE
-extern "C" int rb_debug_scan_timeline(unsigned long long* out, int reset) {
-  cudaDeviceSynchronize();
-  cudaMemcpyFromSymbol(out, rb_scan_tl, sizeof(rb_scan_tl));
-  if (reset) {
-    unsigned long long init[8] = {~0ull, 0, ~0ull, 0, ~0ull, 0, ~0ull, 0};
-    cudaMemcpyToSymbol(rb_scan_tl, init, sizeof(init));
-  }
-  return 0;
-}
-#endif
 
 size_t scan_tc_smem_bytes() { return kSmemBytes; }
 

@@ -30,18 +30,6 @@
 namespace rb {
 namespace {
 
-#ifdef RB_PROF   // development aid (_work harness): per-warp cycle and event counters; compiled out otherwise
-__device__ unsigned long long rb_prof[148 * 8 * 8];
-#define RB_PC_DECL unsigned long long pc_[8] = {0, 0, 0, 0, 0, 0, 0, 0}
-#define RB_PC(slot, val) pc_[slot] += (unsigned long long)(val)
-#define RB_PC_FLUSH do { if (lane == 0) { for (int q_ = 0; q_ < 8; ++q_) rb_prof[(blockIdx.x * 8 + warp) * 8 + q_] += pc_[q_]; } } while (0)
-#define RB_CLK() clock64()
-#else
-#define RB_PC_DECL
-#define RB_PC(slot, val)
-#define RB_PC_FLUSH
-#define RB_CLK() 0ll
-#endif
 
 constexpr int kStages2 = 6;
 constexpr int kA2Bytes = kTileM * kTileK * 2;            // 16 KB: this CTA's 128 queries x 64 bf16
@@ -205,7 +193,6 @@ scan_tc2_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant_
   int* epi_done = (int*)(tmem_slot + 1);   // epilogue warps that have finished
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  RB_PC_DECL;
   const uint32_t rank = cluster_ctarank();
   const int cl = blockIdx.x >> 1, ncl = gridDim.x >> 1;
   const int n_mp = Bpad / kPairM;
@@ -279,17 +266,13 @@ scan_tc2_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant_
       for (int tile = 0; tile < ntiles; ++tile) {
         for (int mp = 0; mp < n_mp; ++mp, ++it) {
           const uint32_t acc = it & 1, aph = (it >> 1) & 1;
-          const long long m0_ = RB_CLK();
           mbar_wait(&tempty[acc], aph ^ 1);
-          { const long long dw_ = RB_CLK() - m0_; RB_PC(0, dw_); const int bk_ = tile == 0 ? 2 : (tile == 1 ? 3 : (tile < 4 ? 4 : (tile < 8 ? 5 : (tile < 16 ? 6 : 7)))); RB_PC(bk_, dw_); }
           tc_fence_after();
           const uint32_t d_tmem = tmem_base + acc * kTileN;
           for (int kc = 0; kc < nk; ++kc, ++kit) {
             const int s = kit % kStages2;
             const uint32_t ph = (kit / kStages2) & 1;
-            const long long m1_ = RB_CLK();
             mbar_wait(&full[s], ph);
-            RB_PC(1, RB_CLK() - m1_);
             tc_fence_after();
             const uint32_t sa = smem_u32(smem + s * kStage2Bytes);
             const uint64_t adesc = make_smem_desc(sa);
@@ -348,12 +331,8 @@ scan_tc2_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant_
           const uint32_t lo = f32_ordered(own);
           st.thr = f32_unordered(lo > ge ? lo : ge);
         }
-        const long long e0_ = RB_CLK();
         mbar_wait(&tfull[acc], aph);
-        const long long e1_ = RB_CLK();
-        RB_PC(0, e1_ - e0_);
         tc_fence_after();
-        long long lb_ = e1_;
         if (warp_active) {
           // the accumulator always holds 256 columns (columns >= c_end are similarities to zero-filled rows)
           const uint32_t taddr = tmem_base + ((uint32_t)(quarter * 32) << 16) + acc * kTileN;
@@ -362,8 +341,6 @@ scan_tc2_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant_
             uint32_t ra[32], rb[32], rc[32], rd[32];
             tmem_ld32(taddr, ra);
             tmem_ld32(taddr + 32, rb);
-            const long long la_ = RB_CLK();
-            RB_PC(5, la_ - e1_);
 #pragma unroll 1
             for (int c0 = 0; c0 < kTileN; c0 += 128) {
               tmem_ld_wait();
@@ -379,8 +356,6 @@ scan_tc2_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant_
               if (c0 + 64 < c_end) park_chunk<KCAP>(rc, c0 + 64, c_end, n0, st, ps4, pi4, cand, tl);
               if (c0 + 96 < c_end) park_chunk<KCAP>(rd, c0 + 96, c_end, n0, st, ps4, pi4, cand, tl);
             }
-            lb_ = RB_CLK();
-            RB_PC(7, lb_ - la_);
           } else {
             for (int c0 = 0; c0 < c_end; c0 += 32) {
               uint32_t ra[32];
@@ -393,14 +368,6 @@ scan_tc2_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant_
         tc_fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive_cluster(tempty_leader[acc]);   // accumulator released; now the insertions
-        const long long e2_ = RB_CLK();
-        RB_PC(1, e2_ - e1_);
-        RB_PC(6, e2_ - lb_);
-        RB_PC(3, 1);
-        {
-          const int anyd_ = __any_sync(0xffffffffu, st.cnt > 0) ? 1 : 0;
-          RB_PC(4, anyd_);
-        }
         if (warp_active && __any_sync(0xffffffffu, st.cnt > 0)) drain<KCAP>(st, ps4, pi4, cand, tl, n0);
         if (st.loaded) {
 #pragma unroll
@@ -415,7 +382,6 @@ scan_tc2_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant_
           const float pj = pub_j == 1 ? st.v[0] : (pub_j == 2 ? st.v[1] : (pub_j == 3 ? st.v[2] : st.v[3]));
           if (pj > -INFINITY) gthr[(size_t)Bpad * (1 + cl) + r] = f32_ordered(pj);
         }
-        RB_PC(2, RB_CLK() - e2_);
         g_cur = g_nxt;
       }
     }
@@ -465,7 +431,6 @@ scan_tc2_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant_
     }
   }
 
-  RB_PC_FLUSH;
   tc_fence_before();
   cluster_sync_all();   // the leader's MMAs read the peer's shared memory and write its TMEM: leave together
   if (warp == 1) {
@@ -476,16 +441,6 @@ scan_tc2_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant_
 
 }  // namespace
 
-#ifdef RB_PROF
-extern "C" void rb_prof_read(unsigned long long* out, int reset) {
-  cudaDeviceSynchronize();
-  cudaMemcpyFromSymbol(out, rb_prof, sizeof(unsigned long long) * 148 * 8 * 8);
-  if (reset) {
-    static unsigned long long z[148 * 8 * 8];
-    cudaMemcpyToSymbol(rb_prof, z, sizeof z);
-  }
-}
-#endif
 
 cudaError_t scan_tc2_prepare() {
   cudaError_t e;

@@ -1,5 +1,15 @@
 """Convenience wrapper: owns an rb_ctx and torch output buffers; every method is one C-ABI call plus
-marshalling.  No arithmetic of the method lives here."""
+marshalling.  No arithmetic of the method lives here.
+
+Stream contract.  The context runs on a private stream (`Router.stream`).  Every method that consumes or produces
+device tensors orders that stream against torch's current stream on both sides: the library's kernels start after
+everything already queued on the current stream (the caller's inputs are complete), and the current stream waits for
+the library's kernels before anything queued after the call (the outputs can be consumed like those of any torch op).
+Both are event waits on the device, not host synchronisations.  Device tensors are also recorded on the private stream,
+so the caching allocator does not hand their memory out while the library still reads or writes it.  Host tensors are
+complete when the call returns (C-ABI convention)."""
+import contextlib
+
 import torch
 
 from . import binding as rb
@@ -46,6 +56,20 @@ class Router:
         except Exception:
             pass
 
+    @contextlib.contextmanager
+    def _ordered(self, *tensors):
+        """Stream ordering of one call (module docstring): private stream after the current one, current one after the
+        private one; device tensors recorded on the private stream."""
+        cur = torch.cuda.current_stream(self.device)
+        self.stream.wait_stream(cur)
+        try:
+            yield
+        finally:
+            cur.wait_stream(self.stream)
+            for x in tensors:
+                if isinstance(x, torch.Tensor) and x.is_cuda:
+                    x.record_stream(self.stream)
+
     def set_instances(self, tier, cap, price_in, price_out, pre, dec, slope):
         rb.rb_set_instances(self.ctx, tier, cap, price_in, price_out, list(zip(pre, dec, slope)))
         self.I = len(tier)
@@ -55,10 +79,14 @@ class Router:
         rb.rb_set_tpot_forest(self.ctx, node_feature, node_value, node_left, node_right, tree_root, tier_tree_begin, base,
                               n_features)
         if aux is not None:
-            rb.rb_set_telemetry(self.ctx, aux.contiguous().float())
+            aux = aux.contiguous().float()
+            with self._ordered(aux):
+                rb.rb_set_telemetry(self.ctx, aux)
 
     def set_state(self, queued, running):
-        rb.rb_set_state(self.ctx, queued.contiguous().float(), running.contiguous().to(torch.int32))
+        q, b = queued.contiguous().float(), running.contiguous().to(torch.int32)
+        with self._ordered(q, b):
+            rb.rb_set_state(self.ctx, q, b)
 
     def get_state(self):
         q = torch.empty(self.I, dtype=torch.float32)
@@ -89,12 +117,14 @@ class Router:
             out["nn_sim"] = self._buf((B, self.k), torch.float32, dev)
         if budget is not None:
             out["max_tokens"] = self._buf((B,), torch.int32, dev)
-            rb.rb_decide_budgeted(self.ctx, query, prompt_len, budget, B, w, out["assignment"], out["max_tokens"],
-                                  out.get("scores"), out.get("pred_quality"), out.get("pred_outlen"), out.get("nn_idx"),
-                                  out.get("nn_sim"))
+            with self._ordered(query, prompt_len, budget, *out.values()):
+                rb.rb_decide_budgeted(self.ctx, query, prompt_len, budget, B, w, out["assignment"], out["max_tokens"],
+                                      out.get("scores"), out.get("pred_quality"), out.get("pred_outlen"), out.get("nn_idx"),
+                                      out.get("nn_sim"))
             return out
-        rb.rb_decide(self.ctx, query, prompt_len, B, w, out["assignment"], out.get("scores"), out.get("pred_quality"),
-                     out.get("pred_outlen"), out.get("nn_idx"), out.get("nn_sim"))
+        with self._ordered(query, prompt_len, *out.values()):
+            rb.rb_decide(self.ctx, query, prompt_len, B, w, out["assignment"], out.get("scores"), out.get("pred_quality"),
+                         out.get("pred_outlen"), out.get("nn_idx"), out.get("nn_sim"))
         return out
 
     def estimate(self, query, out_device=None):
@@ -103,7 +133,8 @@ class Router:
         out = {"pred_quality": self._buf((B, self.M), torch.float32, dev),
                "pred_outlen": self._buf((B, self.M), torch.float32, dev),
                "nn_idx": self._buf((B, self.k), torch.int32, dev), "nn_sim": self._buf((B, self.k), torch.float32, dev)}
-        rb.rb_estimate(self.ctx, query, B, out["pred_quality"], out["pred_outlen"], out["nn_idx"], out["nn_sim"])
+        with self._ordered(query, *out.values()):
+            rb.rb_estimate(self.ctx, query, B, out["pred_quality"], out["pred_outlen"], out["nn_idx"], out["nn_sim"])
         return out
 
     def decide_from_predictions(self, quality, outlen, prompt_len, w, commit=0, out_device=None, budget=None):
@@ -113,12 +144,14 @@ class Router:
                "scores0": self._buf((B, self.I), torch.float32, dev), "order": self._buf((B,), torch.int32, dev)}
         if budget is not None:
             out["max_tokens"] = self._buf((B,), torch.int32, dev)
-            rb.rb_decide_from_predictions_budgeted(self.ctx, quality, outlen, prompt_len, budget, B, w, commit,
-                                                   out["assignment"], out["max_tokens"], out["scores"], out["scores0"],
-                                                   out["order"])
+            with self._ordered(quality, outlen, prompt_len, budget, *out.values()):
+                rb.rb_decide_from_predictions_budgeted(self.ctx, quality, outlen, prompt_len, budget, B, w, commit,
+                                                       out["assignment"], out["max_tokens"], out["scores"], out["scores0"],
+                                                       out["order"])
             return out
-        rb.rb_decide_from_predictions(self.ctx, quality, outlen, prompt_len, B, w, commit, out["assignment"],
-                                      out["scores"], out["scores0"], out["order"])
+        with self._ordered(quality, outlen, prompt_len, *out.values()):
+            rb.rb_decide_from_predictions(self.ctx, quality, outlen, prompt_len, B, w, commit, out["assignment"],
+                                          out["scores"], out["scores0"], out["order"])
         return out
 
     def sweep_weights(self, quality, outlen, prompt_len, weights, budget=None, out_device=None):
@@ -127,23 +160,28 @@ class Router:
         w = torch.as_tensor(weights, dtype=torch.float32, device="cpu").reshape(-1, 3).contiguous()
         dev = out_device if out_device is not None else quality.device
         a = torch.empty((w.shape[0], B), dtype=torch.int32, device=dev)
-        rb.rb_sweep_weights(self.ctx, quality, outlen, prompt_len, budget, B, w, w.shape[0], a)
+        with self._ordered(quality, outlen, prompt_len, budget, a):
+            rb.rb_sweep_weights(self.ctx, quality, outlen, prompt_len, budget, B, w, w.shape[0], a)
         return a
 
     def dispatch_pipeline(self, model, outlen, policy, seed=0, commit=1):
         """Pipeline-mode dispatchers: model [B] int32 tiers, outlen [B,M] or None; returns assignment [B]."""
         B = model.shape[0]
         a = torch.empty(B, dtype=torch.int32, device=model.device)
-        rb.rb_dispatch_pipeline(self.ctx, model.contiguous().to(torch.int32), None if outlen is None else outlen.contiguous().float(),
-                                B, policy, seed, commit, a)
+        model = model.contiguous().to(torch.int32)
+        outlen = None if outlen is None else outlen.contiguous().float()
+        with self._ordered(model, outlen, a):
+            rb.rb_dispatch_pipeline(self.ctx, model, outlen, B, policy, seed, commit, a)
         return a
 
     def match_replay(self, scores0, quota, greedy=None):
         """Quota-constrained optimum of the batch-start score matrix; returns (match, objective, n_diverged)."""
         B = scores0.shape[0]
         match = torch.empty(B, dtype=torch.int32, device=scores0.device)
-        obj, div = rb.rb_match_replay(self.ctx, scores0.contiguous(), B, quota.contiguous().to(torch.int32),
-                                      None if greedy is None else greedy.contiguous().to(torch.int32), match)
+        scores0, quota = scores0.contiguous(), quota.contiguous().to(torch.int32)
+        greedy = None if greedy is None else greedy.contiguous().to(torch.int32)
+        with self._ordered(scores0, quota, greedy, match):
+            obj, div = rb.rb_match_replay(self.ctx, scores0, B, quota, greedy, match)
         return match, obj, div
 
     def sync(self):

@@ -49,12 +49,14 @@ def check_predictions(orc, gpu_q, gpu_l, gpu_idx, gpu_sim, orc_idx, orc_sim, nea
     """Predicted quality / output length within 1e-3 relative (north_star).  Near-tie rows are compared with
     the oracle's aggregation re-run on the GPU's own neighbour set.  raw_sums (rerank_slack = 0: the similarities are
     the tensor core's own sums, within 4e-6 of the oracle's): the inverse-distance weight 1/(sqrt(2 - 2s) + eps)
-    amplifies that deviation without bound as s -> 1, so rows with a neighbour closer than s = 0.99 are compared the
-    same way (parity protocol); the default re-ranked path has bit-equal similarities and needs none of it."""
+    amplifies that deviation without bound as s -> 1: a weight moves by ds / (2 - 2s) relative, which stays within the
+    1e-3 bound while 2 - 2s >= 4e-3, i.e. up to s = 0.998; rows with a neighbour closer than that are compared the same
+    way as near-tie rows (parity protocol).  The default re-ranked path has bit-equal similarities and needs
+    none of it."""
     oq, ol = orc.aggregate(orc_idx, orc_sim, quality_np, outlen_np, weight_mode, eps)
     near = list(near)
     if raw_sums and weight_mode == 0:
-        near = sorted(set(near) | set(np.nonzero(gpu_sim.max(axis=1) > 0.99)[0].tolist()))
+        near = sorted(set(near) | set(np.nonzero(gpu_sim.max(axis=1) > 0.998)[0].tolist()))
     if near:
         nq, nl = orc.aggregate(gpu_idx[near], gpu_sim[near], quality_np, outlen_np, weight_mode, eps)
         oq[near], ol[near] = nq, nl

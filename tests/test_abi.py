@@ -7,9 +7,15 @@ from conftest import ROOT
 
 
 def _declared():
-    src = open(os.path.join(ROOT, "include", "routebalance.h")).read()
-    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
-    return sorted(set(re.findall(r"\b(rb_[a-z_0-9]+)\s*\(", src)))
+    """Every function include/*.h declares (routebalance.h: the decision API; routebalance_testing.h: the timing and
+    self-test entry points of the tests and bench.py)."""
+    names = set()
+    inc = os.path.join(ROOT, "include")
+    for h in sorted(os.listdir(inc)):
+        if h.endswith(".h"):
+            src = re.sub(r"/\*.*?\*/", "", open(os.path.join(inc, h)).read(), flags=re.S)
+            names |= set(re.findall(r"\b(rb_[a-z_0-9]+)\s*\(", src))
+    return sorted(names)
 
 
 def test_library_builds_and_exports_declared_symbols():

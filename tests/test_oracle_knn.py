@@ -1,5 +1,6 @@
 """Pins for the oracle's estimate stage (orc_knn, orc_aggregate, orc_round_bf16): closed forms, special
 cases that reduce to library routines, invariants and brute force.  No GPU."""
+import dataclasses
 import math
 
 import numpy as np
@@ -170,3 +171,22 @@ def test_bad_k_rejected(orc):
     with pytest.raises(ValueError):
         orc.knn(bank, bank[:1], 6)
     assert math.isfinite(1.0)
+
+
+def test_fast_fp32_scan_finds_the_nearest_row(orc):
+    """orc_scan_fast_f32 (the separately labelled fp32-accumulator scan that bench.py's cpu_baseline.split times; never
+    used for parity) is pinned to the exact search: on a seeded mixture bank its argmax equals orc_knn(k = 1) for every
+    query whose two best similarities are further apart than fp32 accumulation noise (1e-5: nearly all of them), and a
+    planted exact copy of the query is found wherever it sits (first, middle, last row)."""
+    from paper_2606_17949_b200 import synth
+    cfg = dataclasses.replace(synth.CONFIGS["C1"], N=3000, d=96, Kc=12, seed=17)
+    bank = synth.make_bank(cfg)["emb"].numpy()
+    query = synth.make_queries(cfg, B=40).numpy()
+    idx, sim = orc.knn(bank, query, 2, store_dtype="f32")
+    clear = sim[:, 0] - sim[:, 1] > 1e-5
+    assert clear.sum() >= 30
+    assert np.array_equal(orc.scan_fast_f32(bank, query)[clear], idx[clear, 0])
+    for pos in (0, 1501, 2999):
+        planted = bank.copy()
+        planted[pos] = query[7]
+        assert orc.scan_fast_f32(planted, query[7:8])[0] == pos
