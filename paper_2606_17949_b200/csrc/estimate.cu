@@ -148,14 +148,18 @@ select_f32_kernel(const float* __restrict__ sims, int64_t N, int kc, float* __re
 }
 
 // ---- a2 + a3 + a4 ---------------------------------------------------------------------------------------
-// One CTA per query.
-//  merge   the nlists partial lists (each sorted by key, descending) are copied to shared memory as 64-bit
-//          keys; thread c owns list c and exposes its head; kc rounds of a block-wide maximum (REDUX on the
-//          high and low words, one barrier per round) pop the kc best in order.
+// One CTA per query.  The kernel is bound by the length of its once-executed instruction stream (a cold kernel
+// fetches every instruction it executes, and an SM's instruction cache holds 32 KB), so every phase is a short rolled
+// loop and the rare cases live in functions that are not inlined.
+//  load    the query's partial lists (sorted by key, descending) become 64-bit keys in shared memory.
+//  bound   every 8 lanes form a group; the kc-th largest group maximum is reached by kc distinct entries, so every
+//          member of the kc best reaches it too (admission bound).
+//  select  entries at or above the bound (a few dozen) are compacted and ranked by counting (keys are distinct);
+//          more survivors than slots (equal similarities, a bank sorted by topic): kc rounds of a block-wide maximum.
 //  rescan  the scan may keep fewer entries per (CTA, query) than kc (short lists make its warm-up cheap).  A list
-//          whose every entry was popped may hide further members of the top kc; the bank rows of such a slab
-//          (rare: several of a query's kc best in one of ~148 slabs) are searched again here, exactly, and the
-//          merge is redone over the untouched lists' candidates and the slab's own best kc.
+//          whose last entry made the kc best may hide further members; the bank rows of such a slab (rare: several of
+//          a query's kc best in one of ~148 slabs) are searched again here, exactly, and the selection is redone over
+//          the other slabs' candidates and the slab's own best.
 //  re-rank (bf16 storage): the kc candidates' similarities are recomputed from the stored bf16 rows with fp64
 //          accumulation (products of bf16 values are exact), rounded once to fp32, re-ordered by
 //          (s desc, n asc); the best k are the neighbours.
@@ -165,10 +169,12 @@ select_f32_kernel(const float* __restrict__ sims, int64_t N, int kc, float* __re
 //  terms   (with_terms; Eq. 2, Eq. 1):
 //          c1 = (float)l*pin; c2 = L*pout; C = c1 + c2; Cmax over tiers that have an instance;
 //          ct = Cmax > 0 ? 1 - C/Cmax : 0; A = wq*Q + wc*ct; P = pre*(float)l; key = max_m L
-constexpr int kFinThreadsMax = 1024;              // 512 threads, or 1024 when there are more than 512 lists
+constexpr int kFinThreadsMax = 1024;
 constexpr int kFinWarpsMax = kFinThreadsMax / 32;
 constexpr int kMaxFlag = 16;                      // flagged lists per query <= kc / kcap
-constexpr int kMerge2Stride = 64;                 // second merge: nwarps + 1 lists of up to kMaxK keys
+constexpr int kSurvMax = 256;                     // survivors of the admission bound that are ranked by counting
+constexpr int kGroupsMax = kFinThreadsMax / 8;    // admission groups: 8 lanes each
+constexpr int kRescanKeep = 64;                   // entries every warp keeps of a slab it searches again (>= kMaxK)
 
 // s = fl32( sum_c (double)x[c]*(double)e[c] ) of two bf16 rows, the 32 lanes' fp64 partials added by shuffles.
 __device__ __forceinline__ float exact_sim_bf16(const uint4* __restrict__ qrow, const uint4* __restrict__ brow, int nvec,
@@ -190,357 +196,285 @@ __device__ __forceinline__ float exact_sim_bf16(const uint4* __restrict__ qrow, 
   return (float)acc;
 }
 
-// Warp-level k-way merge: lane l owns the sorted list keys[(first + l)*stride ..] (l < nl <= 32) and the warp
-// pops the kc largest keys, in order, into out_key / out_src (the owning list's index).  No block barrier.
-// bound_hi: similarity (ordered bits) that every member of the query's kc best reaches (0 = none known): the warp stops
-// popping below it and pads the rest of its output with empty entries.
-// Returns the number of entries popped (warp-uniform).
-__device__ __forceinline__ int warp_kway_merge(const unsigned long long* keys, int first, int nl, int stride, int len,
-                                               int kc, unsigned long long* out_key, int* out_src, uint32_t bound_hi) {
-  const int lane = threadIdx.x & 31;
-  const unsigned long long* mine = keys + (size_t)(first + lane) * stride;
-  int pos = 0, npop = 0;
-  unsigned long long hk = (lane < nl) ? mine[0] : 0ull;
+// kc rounds of a block-wide maximum over distinct 64-bit keys: each round takes the largest key below the previous
+// pick (keys [n] in shared memory; 0 = empty).  Result in out[0..kc), descending (0 = exhausted).  All threads of the
+// block must call.  Rare path: kept out of line.
+__device__ __noinline__ void block_select_topk(const unsigned long long* keys, int n, int kc,
+                                               uint32_t (*s_red)[kFinWarpsMax][2], unsigned long long* out) {
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, nwarps = blockDim.x >> 5;
+  unsigned long long prev = ~0ull;
+#pragma unroll 1
   for (int j = 0; j < kc; ++j) {
-    const uint32_t hi = (uint32_t)(hk >> 32), lo = (uint32_t)hk;
-    const uint32_t ghi = __reduce_max_sync(0xffffffffu, hi);
-    if (ghi < bound_hi) {   // warp-uniform: nothing left here can be among the kc best
-      for (int jj = j + lane; jj < kc; jj += 32) { out_key[jj] = 0ull; out_src[jj] = -1; }
-      break;
+    unsigned long long best = 0ull;
+    for (int e = tid; e < n; e += blockDim.x) {
+      const unsigned long long key = keys[e];
+      if (key < prev && key > best) best = key;
     }
-    npop += ghi != 0u;
-    const uint32_t glo = __reduce_max_sync(0xffffffffu, hi == ghi ? lo : 0u);
-    const unsigned long long win = ((unsigned long long)ghi << 32) | glo;
-    if (win != 0ull && hk == win) {   // keys are distinct: exactly one owner
-      out_key[j] = win;
-      out_src[j] = first + lane;
-      ++pos;
-      hk = pos < len ? mine[pos] : 0ull;
-    }
-    if (win == 0ull && lane == 0) { out_key[j] = 0ull; out_src[j] = -1; }
-  }
-  return npop;
-}
-
-// Block-wide k-way merge: thread c < nl owns the sorted list keys[c*stride .. c*stride+len); pops the kc largest
-// keys into out_key[0..kc) (0 = exhausted) and the list each came from into out_src.  Returns how many entries
-// of the caller's own list were popped.  All threads of the block must call.
-__device__ int kway_merge(const unsigned long long* keys, int nl, int stride, int len, int kc,
-                          uint32_t (*s_red)[kFinWarpsMax][2], unsigned long long* out_key, int* out_src) {
-  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, kFinWarps = blockDim.x >> 5;
-  int pos = 0;
-  unsigned long long hk = (tid < nl) ? keys[(size_t)tid * stride] : 0ull;
-  for (int j = 0; j < kc; ++j) {
-    const uint32_t hi = (uint32_t)(hk >> 32), lo = (uint32_t)hk;
+    const uint32_t hi = (uint32_t)(best >> 32), lo = (uint32_t)best;
     const uint32_t whi = __reduce_max_sync(0xffffffffu, hi);
     const uint32_t wlo = __reduce_max_sync(0xffffffffu, hi == whi ? lo : 0u);
     if (lane == 0) { s_red[j & 1][warp][0] = whi; s_red[j & 1][warp][1] = wlo; }
     __syncthreads();
-    const uint32_t xhi = lane < kFinWarps ? s_red[j & 1][lane][0] : 0u;
-    const uint32_t xlo = lane < kFinWarps ? s_red[j & 1][lane][1] : 0u;
+    const uint32_t xhi = lane < nwarps ? s_red[j & 1][lane][0] : 0u;
+    const uint32_t xlo = lane < nwarps ? s_red[j & 1][lane][1] : 0u;
     const uint32_t ghi = __reduce_max_sync(0xffffffffu, xhi);
     const uint32_t glo = __reduce_max_sync(0xffffffffu, xhi == ghi ? xlo : 0u);
-    const unsigned long long win = ((unsigned long long)ghi << 32) | glo;
-    if (win != 0ull && hk == win) {   // keys are distinct: exactly one owner
-      out_key[j] = win;
-      out_src[j] = tid;
-      ++pos;
-      hk = pos < len ? keys[(size_t)tid * stride + pos] : 0ull;
-    }
-    if (win == 0ull && tid == 0) { out_key[j] = 0ull; out_src[j] = -1; }
+    prev = ((unsigned long long)ghi << 32) | glo;
+    if (tid == 0) out[j] = prev;
+    if (prev == 0ull) prev = 1ull;   // exhausted: later rounds find nothing (key 0 is below every real candidate)
   }
   __syncthreads();
-  return pos;
+}
+
+// Rows [row0, row1) of slab c (the scan's split of the bank: slab c = units [units*c/nslabs, units*(c+1)/nslabs)).
+__device__ __forceinline__ void slab_rows(const FinishArgs& a, int c, int nslabs, int64_t* row0, int64_t* row1) {
+  const int64_t units = (a.N + a.slab_unit - 1) / a.slab_unit;
+  *row0 = units * c / nslabs * a.slab_unit;
+  int64_t r1 = units * (c + 1) / nslabs * a.slab_unit;
+  *row1 = r1 > a.N ? a.N : r1;
+}
+
+// The slabs whose list may hide members of the kc best (last entry at or above kstar, the kc-th best key found) are
+// searched again with exact similarities; s_cand becomes the kc best of those slabs' rows and of the candidates that
+// came from the other slabs.  s_keys is overwritten ([nwarps][kRescanKeep] + [kc]).  All threads must call; rare path.
+__device__ __noinline__ void rescan_slabs(const FinishArgs& a, const uint4* qrow, int nvec, unsigned long long kstar,
+                                          unsigned long long* s_keys, unsigned long long* s_cand,
+                                          uint32_t (*s_red)[kFinWarpsMax][2], int* s_flag, int* s_nflag) {
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, nwarps = blockDim.x >> 5;
+  const int kc = a.kc, kcap = a.kcap;
+  if (tid == 0) *s_nflag = 0;
+  __syncthreads();
+  for (int l = tid; l < a.nlists; l += blockDim.x) {
+    const unsigned long long last = s_keys[(size_t)l * kcap + kcap - 1];
+    if (last != 0ull && last >= kstar) {
+      const int p = atomicAdd(s_nflag, 1);
+      if (p < kMaxFlag) s_flag[p] = l / a.lists_per_cta;
+    }
+  }
+  __syncthreads();
+  if (tid == 0) {   // lists -> slabs, each once
+    const int nl = min(*s_nflag, kMaxFlag);
+    int nc = 0;
+    for (int f = 0; f < nl; ++f) {
+      const int c = s_flag[f];
+      bool seen = false;
+      for (int g = 0; g < nc; ++g) seen |= (s_flag[g] == c);
+      if (!seen) s_flag[nc++] = c;
+    }
+    *s_nflag = nc;
+  }
+  __syncthreads();
+  const int nflag = *s_nflag;
+  const int nslabs = a.nlists / a.lists_per_cta;
+  // every warp keeps the best 64 of the rows it visits: rank l in lane l (la) and rank 32 + l (lb)
+  unsigned long long la = 0, lb = 0, thr = 0;
+  for (int f = 0; f < nflag; ++f) {
+    int64_t row0, row1;
+    slab_rows(a, s_flag[f], nslabs, &row0, &row1);
+    for (int64_t n = row0 + warp; n < row1; n += nwarps) {
+      const float sx = exact_sim_bf16(qrow, reinterpret_cast<const uint4*>(a.bank + (size_t)n * a.d), nvec, lane);
+      const unsigned long long x = make_key(sx, (int32_t)n);
+      if (sx == sx && x > thr) {
+        const int p = __popc(__ballot_sync(0xffffffffu, la > x)) + __popc(__ballot_sync(0xffffffffu, lb > x));
+        const unsigned long long a_up = __shfl_up_sync(0xffffffffu, la, 1), b_up = __shfl_up_sync(0xffffffffu, lb, 1);
+        const unsigned long long a_last = __shfl_sync(0xffffffffu, la, 31);
+        const unsigned long long b_prev = (lane == 0) ? a_last : b_up;
+        la = (lane < p) ? la : ((lane == p) ? x : a_up);
+        lb = (lane + 32 < p) ? lb : ((lane + 32 == p) ? x : b_prev);
+        thr = (kc <= 32) ? __shfl_sync(0xffffffffu, la, kc - 1) : __shfl_sync(0xffffffffu, lb, kc - 33);
+      }
+    }
+  }
+  __syncthreads();   // everybody is done with the list keys
+  s_keys[(size_t)warp * kRescanKeep + lane] = la;
+  s_keys[(size_t)warp * kRescanKeep + 32 + lane] = lb;
+  if (tid < kc) {    // candidates from the other slabs stay in the running
+    const unsigned long long key = s_cand[tid];
+    bool from_flagged = false;
+    if (key != 0ull) {
+      const int64_t n = (int64_t)(0xffffffffu - (uint32_t)key);
+      for (int f = 0; f < nflag; ++f) {
+        int64_t row0, row1;
+        slab_rows(a, s_flag[f], nslabs, &row0, &row1);
+        from_flagged |= (n >= row0 && n < row1);
+      }
+    }
+    s_keys[(size_t)nwarps * kRescanKeep + tid] = from_flagged ? 0ull : key;
+  }
+  __syncthreads();
+  block_select_topk(s_keys, nwarps * kRescanKeep + kc, kc, s_red, s_cand);
 }
 
 __global__ void __launch_bounds__(kFinThreadsMax)
 finish_kernel(FinishArgs a, InstTable t, const __grid_constant__ CallParams cpv) {
   const CallParams* __restrict__ cp = &cpv;   // per-call parameters: a kernel argument (constant bank), not a device block
-  extern __shared__ unsigned long long s_keys[];   // max([nlists][kcap], [nwarps + 1][kMerge2Stride])
+  extern __shared__ unsigned long long s_keys[];   // max([nlists][kcap], [nwarps][kRescanKeep] + [kMaxK])
   __shared__ uint32_t s_red[2][kFinWarpsMax][2];
+  __shared__ uint32_t s_gmax[kGroupsMax];
+  __shared__ unsigned long long s_surv[kSurvMax];
   __shared__ unsigned long long s_cand[kMaxK];
-  __shared__ int s_src[kMaxK];
-  __shared__ int s_nflag;
-  __shared__ uint32_t s_wbest[kFinWarpsMax];
-  __shared__ int s_maxcnt;
-  __shared__ int s_wcnt[kFinWarpsMax];                // entries each warp popped at the first level
-  __shared__ unsigned long long s_skey[64];           // first-level survivors, compacted (second level by counting)
-  __shared__ int s_ssrc[64];
+  __shared__ int s_nsurv, s_nflag;
+  __shared__ uint32_t s_tau;
   __shared__ int s_flag[kMaxFlag];
   __shared__ float s_sim[kMaxK];
   __shared__ int32_t s_idx[kMaxK];
-  __shared__ float o_sim[kMaxK];
-  __shared__ int32_t o_idx[kMaxK];
   __shared__ float s_w[kMaxK];
-  __shared__ int o_pos[kMaxK];
   __shared__ float s_lab[kMaxK][2 * kMaxM];         // labels of the kc candidates: [quality(M) | outlen(M)]
+  __shared__ int s_pos[kMaxK];                      // candidate at each final rank
   __shared__ float sQ[kMaxM], sL[kMaxM];
   const int r = blockIdx.x;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  const int kFinThreads = blockDim.x, nwarps = blockDim.x >> 5;
+  const int nthreads = blockDim.x, nwarps = blockDim.x >> 5;
   // coefficients of the score terms: requested now, consumed at the very end (their latency hides behind the merge)
   float c_pin = 0.0f, c_pout = 0.0f, c_pre = 0.0f, c_ell = 0.0f, c_budget = 0.0f;
   bool has_budget = false;
+  int c_present = 0;
   if (a.with_terms && tid < a.M) {
     c_pin = t.price_in[tid];
     c_pout = t.price_out[tid];
     c_pre = t.pre[tid];
+    c_present = t.present[tid];
     c_ell = (float)cp->plen[r];
     has_budget = cp->budget != nullptr;
     if (has_budget) c_budget = cp->budget[r];
   }
-  const int c_present = (a.with_terms && tid < a.M) ? t.present[tid] : 0;
-  // caller-side output pointers and weights: read once, up front (every later use would be an L2 round trip)
+  const int kc = a.kc, k = a.k, kcap = a.kcap, M = a.M;
+  const uint4* qrow = reinterpret_cast<const uint4*>(a.qs + (size_t)r * a.d);
+  const int nvec = a.d / 8;   // d % 8 == 0
+  const int total = a.nlists * kcap;
+  if (tid == 0) s_nsurv = 0;
+  launch_dependents();
+  grid_dependency_wait();   // the partial lists come from the preceding kernel
+
+  // ---- load: lists -> keys in shared memory; every thread remembers the best similarity it has seen ----
+  uint32_t tmax = 0u;
+  if (kcap & 3) {   // one already-merged list per query, entry by entry ([nlists][Bpad][kcap] arrays)
+    for (int e = tid; e < total; e += nthreads) {
+      const int c = e / kcap, j = e - c * kcap;
+      const size_t off = ((size_t)c * a.Bpad + r) * kcap + j;
+      const int32_t id = a.part_idx[off];
+      const unsigned long long key = (id >= 0 && (int64_t)id < a.N) ? make_key(a.part_sim[off], id) : 0ull;
+      s_keys[e] = key;
+      tmax = max(tmax, (uint32_t)(key >> 32));
+    }
+  } else {
+    // a list's kcap entries are contiguous (kcap is a multiple of 4): one quad = 4 similarities + 4 indices per step
+    const int q4 = kcap >> 2, nquads = a.nlists * q4;
+#pragma unroll 1
+    for (int e = tid; e < nquads; e += nthreads) {
+      uint4 ua, ub;
+      if (a.records) {   // record e of this query: [4 similarities | 4 indices], contiguous over e (one run per query)
+        const uint4* rec = reinterpret_cast<const uint4*>(a.part_sim) + ((size_t)r * nquads + e) * 2;
+        ua = __ldcg(rec);
+        ub = __ldcg(rec + 1);
+      } else {
+        const int c = e / q4, j4 = e - c * q4;
+        const size_t off = ((size_t)c * a.Bpad + r) * kcap + 4 * j4;
+        ua = __ldcg(reinterpret_cast<const uint4*>(a.part_sim + off));
+        ub = __ldcg(reinterpret_cast<const uint4*>(a.part_idx + off));
+      }
+      const uint32_t sx[4] = {ua.x, ua.y, ua.z, ua.w};
+      const uint32_t ix[4] = {ub.x, ub.y, ub.z, ub.w};
+#pragma unroll
+      for (int h = 0; h < 4; ++h) {
+        const int32_t id = (int32_t)ix[h];
+        const unsigned long long key = (id >= 0 && (int64_t)id < a.N) ? make_key(__uint_as_float(sx[h]), id) : 0ull;
+        s_keys[4 * e + h] = key;
+        tmax = max(tmax, (uint32_t)(key >> 32));
+      }
+    }
+  }
+  // ---- bound: kc-th largest of the 8-lane group maxima ----
+  tmax = max(tmax, __shfl_xor_sync(0xffffffffu, tmax, 1));
+  tmax = max(tmax, __shfl_xor_sync(0xffffffffu, tmax, 2));
+  tmax = max(tmax, __shfl_xor_sync(0xffffffffu, tmax, 4));
+  const int ngroups = nthreads >> 3;
+  if ((lane & 7) == 0) s_gmax[tid >> 3] = tmax;
+  if (tid == 0) s_tau = 0u;
+  __syncthreads();
+  if (tid < ngroups && ngroups >= kc) {
+    const uint32_t mine = s_gmax[tid];
+    int rank = 0;
+#pragma unroll 4
+    for (int g = 0; g < ngroups; ++g) {
+      const uint32_t o = s_gmax[g];
+      rank += (o > mine) || (o == mine && g < tid);
+    }
+    if (rank == kc - 1) s_tau = mine;   // ranks are distinct: exactly one writer
+  }
+  __syncthreads();
+  // ---- select: survivors of the bound, compacted ----
+  const uint32_t tau = s_tau;
+  // (every thread revisits the entries it wrote itself: quads tid, tid + nthreads, ...)
+  if (kcap & 3) {
+    for (int e = tid; e < total; e += nthreads) {
+      const unsigned long long key = s_keys[e];
+      if (key != 0ull && (uint32_t)(key >> 32) >= tau) {
+        const int p = atomicAdd(&s_nsurv, 1);
+        if (p < kSurvMax) s_surv[p] = key;
+      }
+    }
+  } else {
+    const int nquads = total >> 2;
+#pragma unroll 1
+    for (int e = tid; e < nquads; e += nthreads) {
+#pragma unroll 1
+      for (int h = 0; h < 4; ++h) {   // a list is sorted: stop at the first entry below the bound
+        const unsigned long long key = s_keys[4 * e + h];
+        if (key == 0ull || (uint32_t)(key >> 32) < tau) break;
+        const int p = atomicAdd(&s_nsurv, 1);
+        if (p < kSurvMax) s_surv[p] = key;
+      }
+    }
+  }
+  __syncthreads();
+  const int nsurv = s_nsurv;
+  if (nsurv <= kSurvMax) {
+    // rank by counting: thread c ranks survivor c
+    if (tid < kc) s_cand[tid] = 0ull;
+    __syncthreads();
+    if (tid < nsurv) {
+      const unsigned long long mine = s_surv[tid];
+      int rank = 0;
+#pragma unroll 4
+      for (int j = 0; j < nsurv; ++j) rank += s_surv[j] > mine;
+      if (rank < kc) s_cand[rank] = mine;
+    }
+    __syncthreads();
+  } else {
+    block_select_topk(s_keys, total, kc, s_red, s_cand);
+  }
+  // ---- rescan of slabs whose list may hide members ----
+  if (a.rescan) {
+    const unsigned long long kstar = s_cand[kc - 1];
+    bool flagged = false;
+    for (int l = tid; l < a.nlists; l += nthreads) {
+      const unsigned long long last = s_keys[(size_t)l * kcap + kcap - 1];
+      flagged |= (last != 0ull && last >= kstar);
+    }
+    if (__syncthreads_or(flagged)) rescan_slabs(a, qrow, nvec, kstar, s_keys, s_cand, s_red, s_flag, &s_nflag);
+  }
+
+  // ---- exact re-rank: warp c recomputes candidate c (and gathers its labels meanwhile) ----
   float* const out_pq = cp->pred_q;
   float* const out_pl = cp->pred_l;
   int32_t* const out_nn_idx = cp->nn_idx;
   float* const out_nn_sim = cp->nn_sim;
-  const float c_wq = cp->w_qual, c_wc = cp->w_cost;
-  const int kc = a.kc, k = a.k, kcap = a.kcap, M = a.M;
-  const uint4* qrow = reinterpret_cast<const uint4*>(a.qs + (size_t)r * a.d);
-  const int nvec = a.d / 8;   // d % 8 == 0
-
-  // ---- merge ----
-  const int total = a.nlists * kcap;
-  launch_dependents();
-  grid_dependency_wait();   // the partial lists come from the preceding kernel
-  if (tid == 0) s_nflag = 0;
-  if (kcap & 3) {   // fp32-storage path: one already-merged list of kc entries per query
-    for (int e = tid; e < total; e += kFinThreads) {
-      const int c = e / kcap, j = e - c * kcap;
-      const size_t off = ((size_t)c * a.Bpad + r) * kcap + j;
-      const int32_t id = a.part_idx[off];
-      s_keys[e] = (id >= 0 && (int64_t)id < a.N) ? make_key(a.part_sim[off], id) : 0ull;
-    }
-  } else {
-    // a list's kcap entries are contiguous (kcap is a multiple of 4): one 16-byte load of similarities and one of
-    // indices per (list, quad); two quads in flight per thread
-    const int q4 = kcap >> 2, nquads = a.nlists * q4;
-    for (int e0 = tid; e0 < nquads; e0 += 2 * kFinThreads) {
-      float4 sv[2];
-      int4 iv[2];
-#pragma unroll
-      for (int u = 0; u < 2; ++u) {
-        const int e = e0 + u * kFinThreads;
-        if (e < nquads) {
-          if (a.records) {   // record e of this query: [4 similarities | 4 indices], contiguous over e
-            // (a list-major layout of the same records was tried: the 4 KB stride between a query's records costs the
-            // finishing CTA ~3000 cycles more than this contiguous run)
-            const uint4* rec = reinterpret_cast<const uint4*>(a.part_sim) + ((size_t)r * nquads + e) * 2;
-            const uint4 ua = __ldcg(rec), ub = __ldcg(rec + 1);
-            sv[u] = make_float4(__uint_as_float(ua.x), __uint_as_float(ua.y), __uint_as_float(ua.z), __uint_as_float(ua.w));
-            iv[u] = make_int4((int)ub.x, (int)ub.y, (int)ub.z, (int)ub.w);
-          } else {
-            const int c = e / q4, j4 = e - c * q4;
-            const size_t off = ((size_t)c * a.Bpad + r) * kcap + 4 * j4;
-            sv[u] = __ldcg(reinterpret_cast<const float4*>(a.part_sim + off));
-            iv[u] = __ldcg(reinterpret_cast<const int4*>(a.part_idx + off));
-          }
-        }
-      }
-#pragma unroll
-      for (int u = 0; u < 2; ++u) {
-        const int e = e0 + u * kFinThreads;
-        if (e < nquads) {
-          const float sx[4] = {sv[u].x, sv[u].y, sv[u].z, sv[u].w};
-          const int32_t ix[4] = {iv[u].x, iv[u].y, iv[u].z, iv[u].w};
-#pragma unroll
-          for (int h = 0; h < 4; ++h)
-            s_keys[4 * e + h] = (ix[h] >= 0 && (int64_t)ix[h] < a.N) ? make_key(sx[h], ix[h]) : 0ull;
-        }
-      }
-    }
+#pragma unroll 1
+  for (int c = warp; c < kc; c += nwarps) {
+    const unsigned long long key = s_cand[c];
+    const int32_t id = key ? (int32_t)(0xffffffffu - (uint32_t)key) : -1;
+    float sx = key ? f32_unordered((uint32_t)(key >> 32)) : -INFINITY;
+    float lv = 0.0f;   // the candidate's labels are requested first: independent of the bank row's loads
+    if (id >= 0 && lane < 2 * M) lv = (lane < M) ? a.bank_quality[(size_t)id * M + lane] : a.bank_outlen[(size_t)id * M + lane - M];
+    if (id >= 0 && a.rerank) sx = exact_sim_bf16(qrow, reinterpret_cast<const uint4*>(a.bank + (size_t)id * a.d), nvec, lane);
+    if (lane == 0) { s_sim[c] = sx; s_idx[c] = id; }
+    if (lane < 2 * M) s_lab[c][lane] = lv;
   }
   __syncthreads();
-  // two levels, no barrier inside either: every warp pops the kc best of its own share of the lists (lane = list),
-  // then warp 0 pops the kc best of the warps' results (lane = warp)
-  unsigned long long* w_key = s_keys + total;                         // [nwarps][kMerge2Stride]
-  int* w_src = reinterpret_cast<int*>(w_key + (size_t)nwarps * kMerge2Stride);   // [nwarps][kMerge2Stride]
-  {
-    const int per = (a.nlists + nwarps - 1) / nwarps;                 // <= 32 by the choice of the block size
-    const int first = warp * per;
-    const int nl = max(0, min(per, a.nlists - first));
-    // Admission bound: the kc-th largest of the warps' best similarities is reached by kc distinct candidates, so
-    // every member of the kc best reaches it too -- a warp then pops two or three entries instead of kc.
-    uint32_t bound = 0u;
-    if (nwarps >= kc) {   // block-uniform
-      const uint32_t head = lane < nl ? (uint32_t)(s_keys[(size_t)(first + lane) * kcap] >> 32) : 0u;
-      const uint32_t wbest = __reduce_max_sync(0xffffffffu, head);
-      if (lane == 0) s_wbest[warp] = wbest;
-      __syncthreads();
-      uint32_t v = lane < nwarps ? s_wbest[lane] : 0u;
-#pragma unroll
-      for (int size = 2; size <= 32; size <<= 1) {
-#pragma unroll
-        for (int stride = size >> 1; stride > 0; stride >>= 1) {
-          const uint32_t other = __shfl_xor_sync(0xffffffffu, v, stride);
-          const bool keep_max = ((lane & stride) == 0) == ((lane & size) == 0);   // descending
-          v = (keep_max == (v > other)) ? v : other;
-        }
-      }
-      bound = __shfl_sync(0xffffffffu, v, kc - 1);
-    }
-    const int npop = warp_kway_merge(s_keys, first, nl, kcap, kcap, kc, w_key + (size_t)warp * kMerge2Stride,
-                                     w_src + (size_t)warp * kMerge2Stride, bound);
-    if (lane == 0) s_wcnt[warp] = npop;
-  }
-  __syncthreads();
-  if (warp == 0) {
-    // out_src of this level is the warp whose list the key came from; its position in that list is the number
-    // of keys already taken from it, which recovers the original list index
-    const unsigned long long* mine = w_key + (size_t)lane * kMerge2Stride;
-    // With the admission bound the warps hand over a few dozen entries in all: rank them by counting (keys are
-    // distinct) instead of kc sequential pops.  More than 64 (no bound, or a bank sorted by topic): the pops below.
-    const int cnt = lane < nwarps ? s_wcnt[lane] : 0;
-    int incl = cnt;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-      const int up = __shfl_up_sync(0xffffffffu, incl, o);
-      if (lane >= o) incl += up;
-    }
-    const int total = __shfl_sync(0xffffffffu, incl, 31);
-    // a list can only have been popped completely if its warp popped at least kcap entries
-    const int maxcnt = (int)__reduce_max_sync(0xffffffffu, (uint32_t)cnt);
-    if (lane == 0) s_maxcnt = maxcnt;
-    if (total <= 64) {
-      const int off = incl - cnt;
-      for (int q = 0; q < cnt; ++q) {
-        s_skey[off + q] = mine[q];
-        s_ssrc[off + q] = w_src[(size_t)lane * kMerge2Stride + q];
-      }
-      __syncwarp();
-      const unsigned long long k0 = lane < total ? s_skey[lane] : 0ull, k1 = lane + 32 < total ? s_skey[lane + 32] : 0ull;
-      int rk0 = 0, rk1 = 0;
-      for (int q = 0; q < total; ++q) {
-        const unsigned long long o = s_skey[q];
-        rk0 += o > k0;
-        rk1 += o > k1;
-      }
-      if (lane < total && rk0 < kc) { s_cand[rk0] = k0; s_src[rk0] = s_ssrc[lane]; }
-      if (lane + 32 < total && rk1 < kc) { s_cand[rk1] = k1; s_src[rk1] = s_ssrc[lane + 32]; }
-      for (int j = total + lane; j < kc; j += 32) { s_cand[j] = 0ull; s_src[j] = -1; }
-    } else {
-    int pos = 0;
-    unsigned long long hk = (lane < nwarps) ? mine[0] : 0ull;
-    for (int j = 0; j < kc; ++j) {
-      const uint32_t hi = (uint32_t)(hk >> 32), lo = (uint32_t)hk;
-      const uint32_t ghi = __reduce_max_sync(0xffffffffu, hi);
-      const uint32_t glo = __reduce_max_sync(0xffffffffu, hi == ghi ? lo : 0u);
-      const unsigned long long win = ((unsigned long long)ghi << 32) | glo;
-      if (win != 0ull && hk == win) {
-        s_cand[j] = win;
-        s_src[j] = w_src[(size_t)lane * kMerge2Stride + pos];
-        ++pos;
-        hk = pos < kc ? mine[pos] : 0ull;
-      }
-      if (win == 0ull && lane == 0) { s_cand[j] = 0ull; s_src[j] = -1; }
-    }
-    }
-  }
-  __syncthreads();
-
-  // ---- rescan of slabs whose list was popped completely ----
-  // (a list of kcap entries all of which are among the kc best may hide further members)
-  bool flagged = false;
-  if (a.rescan && s_maxcnt >= kcap && tid < kc && s_src[tid] >= 0) {
-    int same = 0, earlier = 0;
-    for (int j = 0; j < kc; ++j) {
-      same += (s_src[j] == s_src[tid]);
-      earlier += (j < tid && s_src[j] == s_src[tid]);
-    }
-    flagged = (same == kcap) && (earlier == 0);
-  }
-  if (__syncthreads_or(flagged)) {
-    if (flagged) {
-      const int p = atomicAdd(&s_nflag, 1);
-      if (p < kMaxFlag) s_flag[p] = s_src[tid];
-    }
-    __syncthreads();
-    if (tid == 0) {   // lists -> CTAs (slabs), each once
-      const int nl = min(s_nflag, kMaxFlag);
-      int nc = 0;
-      for (int f = 0; f < nl; ++f) {
-        const int c = s_flag[f] / a.lists_per_cta;
-        bool seen = false;
-        for (int g = 0; g < nc; ++g) seen |= (s_flag[g] == c);
-        if (!seen) s_flag[nc++] = c;
-      }
-      s_nflag = nc;
-    }
-    __syncthreads();
-    const int nflag = s_nflag;
-    const int nctas = a.nlists / a.lists_per_cta;
-    // every warp keeps the best kc of the rows it visits: rank l in lane l (a) and rank 32+l (b)
-    unsigned long long la = 0, lb = 0, thr = 0;
-    const int64_t units = (a.N + a.slab_unit - 1) / a.slab_unit;
-    for (int f = 0; f < nflag; ++f) {
-      const int c = s_flag[f];
-      const int64_t row0 = units * c / nctas * a.slab_unit;
-      int64_t row1 = units * (c + 1) / nctas * a.slab_unit;
-      if (row1 > a.N) row1 = a.N;
-      for (int64_t n = row0 + warp; n < row1; n += nwarps) {
-        const float sx = exact_sim_bf16(qrow, reinterpret_cast<const uint4*>(a.bank + (size_t)n * a.d), nvec, lane);
-        const unsigned long long x = make_key(sx, (int32_t)n);
-        if (sx == sx && x > thr) {
-          const int p = __popc(__ballot_sync(0xffffffffu, la > x)) + __popc(__ballot_sync(0xffffffffu, lb > x));
-          const unsigned long long a_up = __shfl_up_sync(0xffffffffu, la, 1), b_up = __shfl_up_sync(0xffffffffu, lb, 1);
-          const unsigned long long a_last = __shfl_sync(0xffffffffu, la, 31);
-          const unsigned long long b_prev = (lane == 0) ? a_last : b_up;
-          la = (lane < p) ? la : ((lane == p) ? x : a_up);
-          lb = (lane + 32 < p) ? lb : ((lane + 32 == p) ? x : b_prev);
-          thr = (kc <= 32) ? __shfl_sync(0xffffffffu, la, kc - 1) : __shfl_sync(0xffffffffu, lb, kc - 33);
-        }
-      }
-    }
-    __syncthreads();   // s_keys is rewritten: lists 0..nwarps-1 = the warps' lists, list nwarps = untouched candidates
-    s_keys[(size_t)warp * kMerge2Stride + lane] = la;
-    s_keys[(size_t)warp * kMerge2Stride + 32 + lane] = lb;
-    if (tid == 0) {
-      int o = 0;
-      for (int j = 0; j < kc; ++j) {
-        bool from_flagged = false;
-        for (int f = 0; f < nflag; ++f) from_flagged |= (s_src[j] / a.lists_per_cta == s_flag[f]);
-        if (s_cand[j] != 0ull && !from_flagged) s_keys[(size_t)nwarps * kMerge2Stride + o++] = s_cand[j];
-      }
-      for (; o < kMerge2Stride; ++o) s_keys[(size_t)nwarps * kMerge2Stride + o] = 0ull;
-    }
-    __syncthreads();
-    kway_merge(s_keys, nwarps + 1, kMerge2Stride, kMerge2Stride, kc, s_red, s_cand, s_src);
-  }
-  if (tid < kc) {
-    const unsigned long long key = s_cand[tid];
-    s_sim[tid] = key ? f32_unordered((uint32_t)(key >> 32)) : -INFINITY;
-    s_idx[tid] = key ? (int32_t)(0xffffffffu - (uint32_t)key) : -1;
-  }
-  __syncthreads();
-
-  // labels of all kc candidates are requested before the re-rank and parked after it (independent gathers); the
-  // threads are rotated by half a block so that, for the usual handful of candidates, the label gathers are issued
-  // by the upper warps while the lower ones (warp c = candidate c) already fetch their bank rows
-  const int tid_lab = (tid + (kFinThreads >> 1)) & (kFinThreads - 1);   // the block size is a power of two
-  float lv[4];
-  const int nlab = kc * 2 * M;   // <= 64 * 32 = 4 * 512
-#pragma unroll
-  for (int u = 0; u < 4; ++u) {
-    const int e = tid_lab + u * kFinThreads;
-    lv[u] = 0.0f;
-    if (e < nlab) {
-      const int c = e / (2 * M), col = e - c * 2 * M;
-      const int32_t id = s_idx[c];
-      if (id >= 0) lv[u] = (col < M) ? a.bank_quality[(size_t)id * M + col] : a.bank_outlen[(size_t)id * M + col - M];
-    }
-  }
-  // ---- exact re-rank ----
-  if (a.rerank) {
-    for (int c = warp; c < kc; c += nwarps) {
-      const int32_t id = s_idx[c];
-      if (id < 0) continue;
-      const float sx = exact_sim_bf16(qrow, reinterpret_cast<const uint4*>(a.bank + (size_t)id * a.d), nvec, lane);
-      if (lane == 0) s_sim[c] = sx;
-    }
-    __syncthreads();
-  }
-  // rank by counting (keys are distinct because indices are): warp c ranks candidate c, lane j compares candidate j
+  // rank by counting (keys are distinct because indices are): warp c ranks candidate c, lane j compares candidate j;
+  // lane 0 then computes the weight of the rank-th neighbour (the warps' square roots and divisions overlap)
+#pragma unroll 1
   for (int c = warp; c < kc; c += nwarps) {
     const int32_t id = s_idx[c];
     const float sc = s_sim[c];
@@ -556,14 +490,12 @@ finish_kernel(FinishArgs a, InstTable t, const __grid_constant__ CallParams cpv)
       }
       rank += __popc(__ballot_sync(0xffffffffu, ahead));
     }
-    if (lane == 0) {
-      o_sim[rank] = sc;
-      o_idx[rank] = id;
-      o_pos[rank] = c;
-      if (rank < k) {   // ---- weight of the rank-th neighbour (the warps' square roots and divisions overlap) ----
+    if (rank < k) {
+      if (lane == 0) {
+        s_pos[rank] = c;
         float w = 1.0f;
         if (id < 0) {
-          w = 0.0f;   // fewer than k rows reachable (cannot happen for k <= N); keeps the gather in bounds
+          w = 0.0f;   // fewer than k rows reachable (cannot happen for k <= N); adds +0 to both sums
         } else if (a.weight_mode == 0) {
           const float tt = __fmul_rn(2.0f, sc);
           float u = __fsub_rn(2.0f, tt);
@@ -577,37 +509,31 @@ finish_kernel(FinishArgs a, InstTable t, const __grid_constant__ CallParams cpv)
       }
     }
   }
-#pragma unroll
-  for (int u = 0; u < 4; ++u) {
-    const int e = tid_lab + u * kFinThreads;
-    if (e < nlab) s_lab[e / (2 * M)][e % (2 * M)] = lv[u];
-  }
   __syncthreads();
-  // ---- aggregate: thread m < M -> quality, M <= thread < 2M -> output length ----
-  if (tid < 2 * M) {
-    const int m = tid % M;
+  if (warp != 0) return;
+  // ---- aggregate: lane m < M -> quality, M <= lane < 2M -> output length ----
+  if (lane < 2 * M) {
     float num = 0.0f, den = 0.0f;
-    // (a missing neighbour -- fewer than k rows reachable -- has weight 0 and position 0: it adds +0 to both sums)
-#pragma unroll 4   // the loads of four neighbours in flight; the two sums stay sequential (canonical order)
+#pragma unroll 4   // four neighbours' loads in flight; the two sums stay sequential (canonical order)
     for (int j = 0; j < k; ++j) {
       const float w = s_w[j];
-      const float p = __fmul_rn(w, s_lab[o_pos[j]][tid]);
+      const float p = __fmul_rn(w, s_lab[s_pos[j]][lane]);
       num = __fadd_rn(num, p);
       den = __fadd_rn(den, w);
     }
     const float pred = __fdiv_rn(num, den);
-    if (tid < M) {
-      sQ[m] = pred;
-      a.pred_q[(size_t)r * M + m] = pred;
-      if (out_pq) out_pq[(size_t)r * M + m] = pred;
+    if (lane < M) {
+      sQ[lane] = pred;
+      a.pred_q[(size_t)r * M + lane] = pred;
+      if (out_pq) out_pq[(size_t)r * M + lane] = pred;
     } else {
-      sL[m] = pred;
-      a.pred_l[(size_t)r * M + m] = pred;
-      if (out_pl) out_pl[(size_t)r * M + m] = pred;
+      sL[lane - M] = pred;
+      a.pred_l[(size_t)r * M + lane - M] = pred;
+      if (out_pl) out_pl[(size_t)r * M + lane - M] = pred;
     }
   }
-  if (!a.with_terms || warp != 0) return;
-  // ---- per-(request, tier) terms: warp 0 alone (2M <= 32: the predictions above were all written by its lanes) ----
+  if (!a.with_terms) return;
+  // ---- per-(request, tier) terms: lane = tier ----
   const uint32_t present = __ballot_sync(0xffffffffu, c_present != 0);   // lanes 0..M-1 hold the tiers' flags
   __syncwarp();
   {
@@ -615,7 +541,7 @@ finish_kernel(FinishArgs a, InstTable t, const __grid_constant__ CallParams cpv)
     const float L = sL[m];
     const float C = __fadd_rn(__fmul_rn(c_ell, c_pin), __fmul_rn(L, c_pout));
     float kmax;
-    const float A = tier_term_A_warp(lane, present, C, L, sQ[m], c_wq, c_wc, has_budget, c_budget, &kmax);
+    const float A = tier_term_A_warp(lane, present, C, L, sQ[m], cp->w_qual, cp->w_cost, has_budget, c_budget, &kmax);
     if (lane < M) {
       a.termA[(size_t)r * M + lane] = A;
       a.termP[(size_t)r * M + lane] = __fmul_rn(c_pre, c_ell);
@@ -665,9 +591,9 @@ int estimate_cp_arg(const void* func, int* nargs) {
 }
 
 size_t finish_smem_bytes(int nlists, int kcap) {
-  // keys of all lists + the warps' merged lists (keys and sources); the rescan's second merge reuses the front
-  const size_t n1 = (size_t)nlists * kcap * 8 + (size_t)kFinWarpsMax * kMerge2Stride * 12;
-  const size_t n2 = (size_t)(kFinWarpsMax + 1) * kMerge2Stride * 8;
+  // keys of all lists; the rescan reuses the space for the warps' own lists and the other slabs' candidates
+  const size_t n1 = (size_t)nlists * kcap * 8;
+  const size_t n2 = (size_t)(kFinWarpsMax * kRescanKeep + kMaxK) * 8;
   return n1 > n2 ? n1 : n2;
 }
 
@@ -676,9 +602,10 @@ cudaError_t finish_prepare(size_t max_smem) {
 }
 
 cudaError_t launch_finish(const FinishArgs& a, InstTable t, const CallParams& cp, int B, cudaStream_t s) {
-  // 32 warps from 257 lists on: the first-level merges' admission bound needs at least k + slack warps to bite
-  const cudaError_t e = launch_chained(finish_kernel, dim3(B), dim3(a.nlists > 256 ? 1024 : 512),
-                                       finish_smem_bytes(a.nlists, a.kcap), s, a, t, cp);
+  // one thread per quad of list entries where that fits; at least 16 warps (one per candidate of the re-rank)
+  const int nquads = a.nlists * ((a.kcap + 3) / 4);
+  const int threads = nquads <= 512 ? 512 : (nquads >= 1024 ? 1024 : (nquads + 31) / 32 * 32);
+  const cudaError_t e = launch_chained(finish_kernel, dim3(B), dim3(threads), finish_smem_bytes(a.nlists, a.kcap), s, a, t, cp);
   return e != cudaSuccess ? e : cudaGetLastError();
 }
 
