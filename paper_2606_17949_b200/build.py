@@ -23,7 +23,7 @@ def _stale(target, deps):
 
 def build(force=False, verbose=False):
     os.makedirs(OBJ, exist_ok=True)
-    headers = [os.path.join(CSRC, "rb_internal.cuh"), os.path.join(CSRC, "tc_scan.cuh"), os.path.join(HERE, "..", "include", "routebalance.h")]
+    headers = [os.path.join(CSRC, "rb_internal.cuh"), os.path.join(CSRC, "tc_scan.cuh"), os.path.join(CSRC, "finish_body.cuh"), os.path.join(HERE, "..", "include", "routebalance.h")]
     jobs = []
     objs = []
     for src in SOURCES:

@@ -721,8 +721,10 @@ rb_status rb_create(rb_ctx** out, const void* bank_emb, const float* bank_qualit
     CK(scan_tc2_prepare());
   }
   {
-    const size_t fin = std::max({finish_smem_bytes(ctx->num_sms * scan_tc_replicas(1, ctx->ks, ctx->num_sms), ctx->ks),
-                                 finish_smem_bytes(ctx->num_sms / 2 + 1, ctx->kcap), finish_smem_bytes(1, ctx->kc)});
+    const int rr = opt.rerank_slack > 0 ? 1 : 0;
+    const size_t fin = std::max({finish_smem_bytes(ctx->num_sms * scan_tc_replicas(1, ctx->ks, ctx->num_sms), ctx->ks, ctx->kc, d, rr),
+                                 finish_smem_bytes(ctx->num_sms / 2 + 1, ctx->kcap, ctx->kc, d, rr),
+                                 finish_smem_bytes(1, ctx->kc, ctx->kc, d, rr)});
     CK(finish_prepare(fin));
     CK(lpt_dispatch_prepare());
   }

@@ -127,6 +127,39 @@ __device__ __forceinline__ void forest_leaves_warp(const int4* __restrict__ node
 // with it, and waits (grid_dependency_wait) before it touches anything its predecessor produces.  Both are
 // no-ops for a kernel launched without the attribute.
 #ifdef __CUDACC__
+// ---- mbarrier / bulk-copy PTX wrappers shared by the scan kernels and the finishing code --------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+  const uint32_t addr = smem_u32(bar);
+  uint32_t ok;
+  do {
+    asm volatile(
+        "{\n\t.reg .pred P1;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%1], %2;\n\t"
+        "selp.b32 %0, 1, 0, P1;\n\t}"
+        : "=r"(ok)
+        : "r"(addr), "r"(parity)
+        : "memory");
+  } while (!ok);
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("{\n\t.reg .b64 st;\n\tmbarrier.arrive.expect_tx.shared::cta.b64 st, [%0], %1;\n\t}" ::"r"(smem_u32(bar)),
+               "r"(bytes)
+               : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+  asm volatile("{\n\t.reg .b64 st;\n\tmbarrier.arrive.shared::cta.b64 st, [%0];\n\t}" ::"r"(smem_u32(bar)) : "memory");
+}
+// 1-D bulk copy global -> shared (bytes a multiple of 16, both addresses 16-byte aligned), completion on an mbarrier.
+__device__ __forceinline__ void bulk_load_1d(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),
+               "l"(src), "r"(bytes), "r"(smem_u32(bar))
+               : "memory");
+}
 __device__ __forceinline__ void launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 __device__ __forceinline__ void grid_dependency_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 
@@ -252,7 +285,7 @@ struct FinishArgs {
 cudaError_t launch_finish(const FinishArgs& a, InstTable t, const CallParams& cp, int B, cudaStream_t s);
 int estimate_cp_arg(const void* func, int* nargs);   // which argument of a kernel of estimate.cu holds the CallParams (-1: none)
 int dispatch_cp_arg(const void* func, int* nargs);   // likewise for score_dispatch.cu
-size_t finish_smem_bytes(int nlists, int kcap);
+size_t finish_smem_bytes(int nlists, int kcap, int kc, int d, int rerank);
 cudaError_t finish_prepare(size_t max_smem);
 
 // a4+a5 from caller-supplied predictions (cp->q_src, cp->l_src): per-(request, tier) terms, LPT keys and the
