@@ -164,6 +164,18 @@ rb_status rb_get_state(rb_ctx* ctx, float* queued_tokens, int32_t* running);
  * into the first kernel of the next rb_decide (no launch of its own), other calls apply it first. */
 rb_status rb_advance_state(rb_ctx* ctx, float elapsed_ms);
 
+/* Adaptive batch size (§4.1: "Batch size is adaptive -- larger when more instances are busy, smaller when idle";
+ * P:L191 §6.3: "Adaptive sizing ties t_form to cluster busyness").  The paper states no rule; this library's
+ * (reading 27), evaluated on the current dead-reckoned state (pending rb_advance_state calls applied first):
+ *   an instance is busy when it has no free decode slot, running_i >= cap_i (the condition of the wait term);
+ *   n_busy = number of busy instances;   target = bs_min + floor((bs_max - bs_min) * n_busy / I).
+ * An idle cluster gives bs_min, a saturated one bs_max; bs_min = bs_max is the fixed batch size of the paper's
+ * "adaptive-off" ablation.  A stream driver closes the next batch when it holds `target` requests (or its first
+ * request has waited long enough) -- paper_2606_17949_b200/stream.py is one.
+ *   target  [host|device] 1 int32;   n_busy [host|device] 1 int32 or NULL
+ * 1 <= bs_min <= bs_max, else RB_EINVAL.  Host outputs synchronise the context's stream. */
+rb_status rb_batch_target(rb_ctx* ctx, int32_t bs_min, int32_t bs_max, int32_t* target, int32_t* n_busy);
+
 /* One per-batch decision: estimate -> score -> LPT greedy dispatch, committing the dead-reckoned updates.
  *   query_emb    [host|device] B x d fp32 prompt embeddings (unit norm expected, not enforced)
  *   prompt_len   [host|device] B int32 input token counts l_r >= 0

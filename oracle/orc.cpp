@@ -431,6 +431,25 @@ int orc_advance_state(int I, const int32_t* tier, const float* dec, const float*
   return 0;
 }
 
+// Adaptive batch size ("Batch size is adaptive -- larger when more instances are busy, smaller when idle"; P:L191
+// "Adaptive sizing ties t_form to cluster busyness").  The paper gives no rule; reading 27:
+//   an instance is busy  <=>  it has no free decode slot, b_i >= cap_i (the condition under which the wait term of
+//                             P:L119 applies, reading 11);
+//   n_busy = #{i : b_i >= cap_i};
+//   target = bs_min + floor((bs_max - bs_min) * n_busy / I)          (integers)
+// so that an idle cluster gives bs_min, a saturated one bs_max, and bs_min = bs_max is the ablation's fixed batch size
+// ("adaptive-off", "Fixed batch size ... bs=1 / 16 / 32").
+int orc_batch_target(int I, const int32_t* cap, const int32_t* bq, int bs_min, int bs_max, int32_t* target,
+                     int32_t* n_busy) {
+  if (I < 1 || bs_min < 1 || bs_max < bs_min) return 1;
+  int busy = 0;
+  for (int i = 0; i < I; ++i)
+    if (bq[i] >= cap[i]) busy += 1;
+  *target = (int32_t)(bs_min + ((int64_t)(bs_max - bs_min) * busy) / I);
+  if (n_busy) *n_busy = busy;
+  return 0;
+}
+
 // Step 10 with the boosted head: the same drain rule, tpot_i from gbdt_tpot.
 int orc_advance_state_gbdt(int I, const int32_t* tier, const orc_forest* forest, float elapsed_ms, float* dq,
                            int32_t* bq) {

@@ -228,6 +228,18 @@ def advance_state(inst, queued, running, elapsed_ms):
     return dq, bq
 
 
+def batch_target(inst, running, bs_min, bs_max):
+    """Adaptive batch size (reading 27): returns (target, n_busy)."""
+    running = _i32(running)
+    target = ctypes.c_int32(0)
+    busy = ctypes.c_int32(0)
+    rc = lib().orc_batch_target(inst.I, _p(inst.cap), _p(running), int(bs_min), int(bs_max), ctypes.byref(target),
+                                ctypes.byref(busy))
+    if rc != 0:
+        raise ValueError("orc_batch_target: need I >= 1 and 1 <= bs_min <= bs_max")
+    return int(target.value), int(busy.value)
+
+
 def decide(bank, bank_quality, bank_outlen, inst, queued, running, query, prompt_len, w, k,
            store_dtype="bf16", weight_mode=0, eps=1e-6, lpt_enabled=1, update_enabled=1):
     """The whole per-batch decision: KNN -> aggregate -> score -> LPT greedy dispatch."""

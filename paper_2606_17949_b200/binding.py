@@ -26,7 +26,7 @@ RB_OK, RB_EINVAL, RB_ECUDA, RB_ENOMEM, RB_ESTATE, RB_EUNSUPPORTED = range(6)
 RB_F32, RB_BF16 = 0, 1
 _STATUS = {0: "RB_OK", 1: "RB_EINVAL", 2: "RB_ECUDA", 3: "RB_ENOMEM", 4: "RB_ESTATE", 5: "RB_EUNSUPPORTED"}
 EXPORTS = ["rb_options_default", "rb_create", "rb_set_instances", "rb_set_tpot_forest", "rb_set_telemetry", "rb_set_state", "rb_get_state", "rb_advance_state",
-           "rb_decide", "rb_decide_budgeted", "rb_decide_from_predictions", "rb_decide_from_predictions_budgeted", "rb_sweep_weights", "rb_estimate", "rb_dispatch_pipeline", "rb_match_replay", "rb_set_stage_timing", "rb_last_stage_us", "rb_last_scan_device_us", "rb_selftest_division",
+           "rb_batch_target", "rb_decide", "rb_decide_budgeted", "rb_decide_from_predictions", "rb_decide_from_predictions_budgeted", "rb_sweep_weights", "rb_estimate", "rb_dispatch_pipeline", "rb_match_replay", "rb_set_stage_timing", "rb_last_stage_us", "rb_last_scan_device_us", "rb_selftest_division",
            "rb_launch_count", "rb_sync", "rb_last_error", "rb_destroy"]
 
 
@@ -63,6 +63,7 @@ _lib.rb_set_telemetry.argtypes = [_vp, _vp]
 _lib.rb_set_state.argtypes = [_vp, _vp, _vp]
 _lib.rb_get_state.argtypes = [_vp, _vp, _vp]
 _lib.rb_advance_state.argtypes = [_vp, _f]
+_lib.rb_batch_target.argtypes = [_vp, _i32, _i32, _vp, _vp]
 _lib.rb_decide.argtypes = [_vp, _vp, _vp, _i32, ctypes.POINTER(_f * 3), _vp, _vp, _vp, _vp, _vp, _vp]
 _lib.rb_decide_from_predictions.argtypes = [_vp, _vp, _vp, _vp, _i32, ctypes.POINTER(_f * 3), _i32, _vp, _vp, _vp, _vp]
 _lib.rb_decide_budgeted.argtypes = [_vp, _vp, _vp, _vp, _i32, ctypes.POINTER(_f * 3), _vp, _vp, _vp, _vp, _vp, _vp, _vp]
@@ -173,6 +174,14 @@ def rb_get_state(ctx, queued_tokens, running):
 
 def rb_advance_state(ctx, elapsed_ms):
     _check(ctx, _lib.rb_advance_state(ctx, float(elapsed_ms)))
+
+
+def rb_batch_target(ctx, bs_min, bs_max):
+    """Adaptive batch size on the current state (reading 27): returns (target, n_busy) as Python ints
+    (host outputs: the call synchronises the context's stream)."""
+    out = (ctypes.c_int32 * 2)()
+    _check(ctx, _lib.rb_batch_target(ctx, int(bs_min), int(bs_max), ctypes.addressof(out), ctypes.addressof(out) + 4))
+    return int(out[0]), int(out[1])
 
 
 _W3_CACHE = {}

@@ -916,6 +916,25 @@ rb_status rb_advance_state(rb_ctx* ctx, float elapsed_ms) {
   return RB_OK;
 }
 
+rb_status rb_batch_target(rb_ctx* ctx, int32_t bs_min, int32_t bs_max, int32_t* target, int32_t* n_busy) {
+  if (!ctx) return RB_EINVAL;
+  if (ctx->I == 0) return fail(ctx, RB_ESTATE, "rb_batch_target before rb_set_instances");
+  if (!target) return fail(ctx, RB_EINVAL, "NULL argument");
+  if (bs_min < 1 || bs_max < bs_min) return fail(ctx, RB_EINVAL, "need 1 <= bs_min <= bs_max");
+  rb_status st = flush_pending(ctx);   // the rule reads the current state
+  if (st != RB_OK) return st;
+  const bool h_t = is_host_ptr(target), h_b = n_busy && is_host_ptr(n_busy);
+  int32_t* d_out = ctx->order;   // two words of per-decision scratch (free between decisions)
+  int32_t* d_t = h_t ? d_out : target;
+  int32_t* d_b = n_busy ? (h_b ? d_out + 1 : n_busy) : nullptr;
+  CK(launch_batch_target(table_of(ctx), ctx->bq, bs_min, bs_max, d_t, d_b, ctx->stream));
+  ctx->launches += 1;
+  if (h_t) CK(cudaMemcpyAsync(target, d_t, 4, cudaMemcpyDeviceToHost, ctx->stream));
+  if (h_b) CK(cudaMemcpyAsync(n_busy, d_b, 4, cudaMemcpyDeviceToHost, ctx->stream));
+  if (h_t || h_b) CK(cudaStreamSynchronize(ctx->stream));
+  return RB_OK;
+}
+
 rb_status rb_decide(rb_ctx* ctx, const float* query_emb, const int32_t* prompt_len, int32_t B, const float w[3],
                     int32_t* assignment, float* scores, float* pred_quality, float* pred_outlen, int32_t* nn_idx,
                     float* nn_sim) {

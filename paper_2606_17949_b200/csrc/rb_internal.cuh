@@ -322,6 +322,10 @@ cudaError_t launch_pipeline_dispatch(InstTable t, const int32_t* members, const 
                                      unsigned long long* counter, int32_t* cursor, int commit, int32_t* assignment,
                                      cudaStream_t s);
 
+// Adaptive batch size (reading 27): *target = bs_min + floor((bs_max - bs_min) * n_busy / I), n_busy = #{b_i >= cap_i}.
+cudaError_t launch_batch_target(InstTable t, const int32_t* bq, int bs_min, int bs_max, int32_t* target, int32_t* n_busy,
+                                cudaStream_t s);
+
 // a8: dead reckoning between batches.
 cudaError_t launch_advance(InstTable t, float* dq, int32_t* bq, float elapsed_ms, cudaStream_t s);
 

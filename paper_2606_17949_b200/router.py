@@ -97,6 +97,10 @@ class Router:
     def advance_state(self, elapsed_ms):
         rb.rb_advance_state(self.ctx, elapsed_ms)
 
+    def batch_target(self, bs_min, bs_max):
+        """Adaptive batch size: (target, n_busy) from the current dead-reckoned state."""
+        return rb.rb_batch_target(self.ctx, bs_min, bs_max)
+
     def _buf(self, shape, dtype, device):
         return torch.empty(shape, dtype=dtype, device=device)
 

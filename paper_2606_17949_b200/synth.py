@@ -150,6 +150,15 @@ def make_state(I, cap, seed, stream=5):
     return queued, running
 
 
+def poisson_arrivals_ms(rate, n_req, seed, stream=9):
+    """Arrival times (ms, float64, non-decreasing) of n_req requests of a Poisson stream at `rate` requests per second
+    (Poisson arrivals at 6-30 req/s) -- the input of the stream driver (stream.py)."""
+    import numpy as np
+    g = _gen(seed, stream, "cpu")
+    gaps = torch.empty(n_req).exponential_(rate, generator=g).double()
+    return (torch.cumsum(gaps, 0) * 1000.0).numpy().astype(np.float64)
+
+
 def poisson_windows(rate, n_decisions, seed, max_b=64, min_b=4, max_age=0.5, stream=6):
     """Batch windows of a Poisson arrival stream: a batch closes when it holds max_b requests or
     (>= min_b requests and age >= max_age seconds).  Returns lists (B_j, elapsed_ms_j)."""

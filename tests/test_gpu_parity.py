@@ -937,3 +937,46 @@ def test_c2_stream_10k_decisions_lockstep(orc):
     assert off == n_req and 4 <= min(sizes) and max(sizes) <= 64
     assert near_rows <= max(3, knn_rows // 200), (near_rows, knn_rows, log[:5])   # documented near-ties only, and rare
     rt.close()
+
+
+def test_adaptive_batch_rule_and_stream_driver_lockstep(orc):
+    """SURVEY 8(f) #4, second half: the adaptive batch-size rule (rb_batch_target; reading 27) and the
+    stream driver (stream.py) that forms its windows with it.  A Poisson stream of 1500 requests at 30 req/s over a
+    cluster whose instances saturate and drain (cap = 4): the rule's target and busy count, every assignment and the state
+    after every decision equal the oracle's, window by window; the targets really move with the load; and the
+    fixed-batch-size off-switch (bs_min = bs_max) gives windows of that size."""
+    from paper_2606_17949_b200 import binding as rb, stream
+    from stream_backends import LockstepBackend
+    cfg = dataclasses.replace(synth.CONFIGS["C2"], N=20000, d=128, Kc=16, seed=51)
+    n_req = 1500
+    bank = synth.make_bank(cfg, device="cuda")
+    it = synth.make_instances(cfg.I, cfg.M, cap=4)
+    queued, running = synth.make_state(cfg.I, it["cap"], cfg.seed)
+    q = synth.make_queries(cfg, B=n_req, device="cuda")
+    p = synth.make_prompt_len(cfg, B=n_req, device="cuda")
+    arrivals = synth.poisson_arrivals_ms(30.0, n_req, seed=cfg.seed)
+    torch.cuda.synchronize()
+    rt = _router(bank, cfg, max_batch=64)
+    rt.set_instances(**it)
+    inst = orc.Instances(**it)
+    presets = list(synth.PRESETS.values())
+    for bs_min, bs_max in ((4, 64), (16, 16)):
+        rt.set_state(queued, running)
+        gpu = stream.RouterBackend(rt, q, p, want_predictions=True)
+        both = LockstepBackend(orc, gpu, inst, queued.numpy(), running.numpy(), p.cpu().numpy())
+        res = stream.drive(both, arrivals, lambda j: presets[j % 4], bs_min=bs_min, bs_max=bs_max, max_wait_ms=500.0)
+        assert res.hi[-1] == n_req and both.windows == len(res.lo)
+        if bs_min != bs_max:
+            assert min(res.target) < max(res.target), "the load never moved the batch size"
+            assert min(res.n_busy) < max(res.n_busy)
+        else:
+            assert set(res.target) == {16}
+    # device outputs, and argument checking
+    out = torch.zeros(2, dtype=torch.int32, device="cuda")
+    assert rb._lib.rb_batch_target(rt.ctx, 4, 64, out.data_ptr(), out.data_ptr() + 4) == rb.RB_OK
+    rt.sync()
+    assert tuple(out.tolist()) == rt.batch_target(4, 64)
+    for lo, hi in ((0, 4), (8, 4)):
+        with pytest.raises(rb.RbError):
+            rt.batch_target(lo, hi)
+    rt.close()
