@@ -46,7 +46,6 @@ __device__ __forceinline__ unsigned long long fin_key(float sim, int32_t idx) {
 struct FinScratch {
   uint32_t red[2][kFinWarpsMax][2];
   uint32_t gmax[kFinThreadsMax];
-  int grank[kFinThreadsMax];
   unsigned long long surv[kSurvMax];
   unsigned long long cand[kMaxK];
   float w[kMaxK];
@@ -57,6 +56,7 @@ struct FinScratch {
   float Q[kMaxM], L[kMaxM];
   int flag[kMaxFlag];
   int nsurv, nflag;
+  uint32_t tau;
 };
 
 // s = fl32( sum_c (double)x[c]*(double)e[c] ) of two bf16 rows (nvec uint4 of 8 values each, nvec <= 128), the 32
@@ -131,7 +131,7 @@ __device__ __forceinline__ void slab_rows(const FinishArgs& a, int c, int nslabs
 // The slabs whose list may hide members of the kc best (last entry at or above kstar, the kc-th best key found) are
 // searched again with exact similarities; S.cand becomes the kc best of those slabs' rows and of the candidates that
 // came from the other slabs.  s_keys is overwritten ([nwarps][kRescanKeep] + [kc]).  All threads must call; rare path.
-__device__ __noinline__ void rescan_slabs(const FinishArgs& a, const uint4* qrow, int nvec, unsigned long long kstar,
+__device__ __noinline__ void rescan_slabs(const FinishArgs a, const uint4* qrow, int nvec, unsigned long long kstar,
                                           unsigned long long* s_keys, FinScratch& S) {
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, nwarps = blockDim.x >> 5;
   const int kc = a.kc, kcap = a.kcap;
@@ -207,11 +207,11 @@ __host__ __device__ inline size_t fin_keys_bytes(int nlists, int kcap) {
 }
 
 // Steps a2-a4 for query r; every thread of the CTA (blockDim.x a multiple of 32, at least 64, at most kFinThreadsMax)
-// must call it, after the lists are visible.  s_keys: fin_keys_bytes() of shared memory; S: scratch.  On return warp 0
-// has written the predictions (and terms) of the query; the other warps pass through.
-// Cost model the phases are written to: an SM issues 4 instructions per cycle over all its warps, so work that every
-// warp repeats is paid for nwarps times; a dependent shared-memory load, shuffle or vote costs 20-30 cycles, a barrier
-// of 19 warps ~100.
+// must call it, after the lists are visible.  s_keys: fin_keys_bytes() of shared memory, 16-byte aligned; S: scratch.
+// On return warp 0 has written the predictions (and terms) of the query; the other warps pass through.
+// What the phases are written to (ncu on the C2 workload): the kernel is bound by the NUMBER of warp instructions --
+// 19 warps share 4 issue slots and every instruction of a phase that all warps run is paid 19 times -- and by the
+// dependent shared-memory / shuffle / vote latencies (20-30 cycles each) between its barriers.
 __device__ __forceinline__ void finish_query(const FinishArgs& a, const InstTable& t, const CallParams* __restrict__ cp,
                                              int r, unsigned long long* s_keys, FinScratch& S) {
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -233,85 +233,62 @@ __device__ __forceinline__ void finish_query(const FinishArgs& a, const InstTabl
     has_budget = cp->budget != nullptr;
     if (has_budget) c_budget = cp->budget[r];
   }
-  if (tid == 0) S.nsurv = 0;
+  if (tid == 0) { S.nsurv = 0; S.tau = 0u; }
   if (tid < kc) S.cand[tid] = 0ull;
 
   // ---- load: lists -> keys in shared memory; every thread remembers the best similarity it has seen ----
   uint32_t tmax = 0u;
-  const bool quads = (kcap & 3) == 0;
-  if (!quads) {   // one already-merged list per query, entry by entry ([nlists][Bpad][kcap] arrays)
+  const bool quads = a.records != 0;   // query-major records of 4 ready-made keys (scan_tc.cu): one item = one quad
+  const int step = quads ? 4 : 1, nitems = total / step;
+  if (quads) {
+    const uint4* rec = reinterpret_cast<const uint4*>(a.part_sim) + (size_t)r * nitems * 2;
+    uint4* dst = reinterpret_cast<uint4*>(s_keys);
+#pragma unroll 1
+    for (int e = tid; e < nitems; e += nthreads) {
+      const uint4 ua = __ldcg(rec + 2 * e), ub = __ldcg(rec + 2 * e + 1);   // (lo, hi) x 4
+      dst[2 * e] = ua;
+      dst[2 * e + 1] = ub;
+      tmax = max(max(tmax, ua.y), max(ua.w, max(ub.y, ub.w)));
+    }
+  } else {   // [nlists][Bpad][kcap] similarity / index arrays (CTA-pair scan, fp32-storage scan), entry by entry
+#pragma unroll 1
     for (int e = tid; e < total; e += nthreads) {
       const int c = e / kcap, j = e - c * kcap;
       const size_t off = ((size_t)c * a.Bpad + r) * kcap + j;
-      const int32_t id = a.part_idx[off];
-      const unsigned long long key = (id >= 0 && (int64_t)id < a.N) ? fin_key(a.part_sim[off], id) : 0ull;
+      const int32_t id = __ldcg(a.part_idx + off);
+      const unsigned long long key = ((uint32_t)id < (uint32_t)a.N) ? fin_key(__ldcg(a.part_sim + off), id) : 0ull;
       s_keys[e] = key;
       tmax = max(tmax, (uint32_t)(key >> 32));
-    }
-  } else {
-    // a list's kcap entries are contiguous (kcap is a multiple of 4): one quad = 4 similarities + 4 indices per step
-    const int q4 = kcap >> 2, nquads = a.nlists * q4;
-#pragma unroll 1
-    for (int e = tid; e < nquads; e += nthreads) {
-      uint4 ua, ub;
-      if (a.records) {   // record e of this query: [4 similarities | 4 indices], contiguous over e (one run per query)
-        const uint4* rec = reinterpret_cast<const uint4*>(a.part_sim) + ((size_t)r * nquads + e) * 2;
-        ua = __ldcg(rec);
-        ub = __ldcg(rec + 1);
-      } else {
-        const int c = e / q4, j4 = e - c * q4;
-        const size_t off = ((size_t)c * a.Bpad + r) * kcap + 4 * j4;
-        ua = __ldcg(reinterpret_cast<const uint4*>(a.part_sim + off));
-        ub = __ldcg(reinterpret_cast<const uint4*>(a.part_idx + off));
-      }
-      const uint32_t sx[4] = {ua.x, ua.y, ua.z, ua.w};
-      const uint32_t ix[4] = {ub.x, ub.y, ub.z, ub.w};
-#pragma unroll
-      for (int h = 0; h < 4; ++h) {
-        const int32_t id = (int32_t)ix[h];
-        const unsigned long long key = (id >= 0 && (int64_t)id < a.N) ? fin_key(__uint_as_float(sx[h]), id) : 0ull;
-        s_keys[4 * e + h] = key;
-        tmax = max(tmax, (uint32_t)(key >> 32));
-      }
     }
   }
   // ---- bound: the threads that hold entries form groups of 8 lanes (fewer lanes while that leaves under 2 kc
   // groups); the kc-th largest group maximum is reached by kc distinct entries, so every member of the kc best
-  // reaches it too.  With ~32 entries per group about kc + 4 entries survive.  The groups are ranked by counting, the
-  // G x G comparisons spread over all threads of the CTA (thread = group x slice of the other groups). ----
-  const int step = quads ? 4 : 1, nitems = total / step;
+  // reaches it too.  With ~32 entries per group about kc + 4 entries survive.  The groups are ranked by counting: the
+  // lanes of a group share its G comparisons and add their counts up by shuffles. ----
   const int nact = min(nthreads, nitems);   // threads that loaded something
   int glanes = 8;
   while (glanes > 1 && (nact + glanes - 1) / glanes < 2 * kc) glanes >>= 1;
   for (int o = 1; o < glanes; o <<= 1) tmax = max(tmax, __shfl_xor_sync(0xffffffffu, tmax, o));
   const int ngroups = (nact + glanes - 1) / glanes;   // <= kFinThreadsMax
   const bool bounded = ngroups >= kc && total > kSurvMax;   // (a small input is ranked whole)
-  if ((lane & (glanes - 1)) == 0 && tid < nact) S.gmax[tid / glanes] = tmax;
-  if (tid < ngroups) S.grank[tid] = 0;
+  const int g = tid / glanes;
+  if ((tid & (glanes - 1)) == 0 && g < ngroups) S.gmax[g] = tmax;
   __syncthreads();
-  uint32_t tau = 0u;
   if (bounded) {
-    const int slices = nthreads / ngroups;   // >= 1
-    if (tid < ngroups * slices) {
-      const int g = tid % ngroups, s = tid / ngroups;
-      const uint32_t mine = S.gmax[g];
-      int ahead = 0;
-#pragma unroll 4
-      for (int j = s; j < ngroups; j += slices) {
+    int ahead = 0;
+    if (g < ngroups) {
+#pragma unroll 2
+      for (int j = tid & (glanes - 1); j < ngroups; j += glanes) {
         const uint32_t o = S.gmax[j];
-        ahead += (o > mine) || (o == mine && j < g);
+        ahead += (o > tmax) || (o == tmax && j < g);
       }
-      if (ahead) atomicAdd(&S.grank[g], ahead);
     }
+    for (int o = 1; o < glanes; o <<= 1) ahead += __shfl_xor_sync(0xffffffffu, ahead, o);
+    if ((tid & (glanes - 1)) == 0 && g < ngroups && ahead == kc - 1) S.tau = tmax;   // ranks are distinct: one writer
     __syncthreads();
-    // every warp looks the group of rank kc - 1 up by itself (ranks are distinct: one hit)
-    for (int g0 = 0; g0 < ngroups; g0 += 32) {
-      const int g = g0 + lane;
-      const uint32_t hit = __ballot_sync(0xffffffffu, g < ngroups && S.grank[g] == kc - 1);
-      if (hit) tau = S.gmax[g0 + __ffs(hit) - 1];
-    }
   }
   // ---- select: survivors of the bound, compacted (one shared-memory atomic per warp and step; any order) ----
+  const uint32_t tau = S.tau;
   bool maybe_hidden = false;   // a list whose LAST entry reaches the bound may be popped completely
 #pragma unroll 1
   for (int e0 = 0; e0 < nitems; e0 += nthreads) {   // every thread revisits the entries it wrote itself
@@ -343,18 +320,18 @@ __device__ __forceinline__ void finish_query(const FinishArgs& a, const InstTabl
   const int any_hidden = __syncthreads_or(maybe_hidden);
   const int nsurv = S.nsurv;
   if (nsurv <= kSurvMax) {
-    // rank by counting (keys are distinct): the warp takes survivors warp, warp + nwarps, ...; lane j compares survivor j0 + j
-#pragma unroll 1
-    for (int c = warp; c < nsurv; c += nwarps) {
-      const unsigned long long mine = S.surv[c];
-      int rank = 0;
-#pragma unroll 1
-      for (int j0 = 0; j0 < nsurv; j0 += 32) {
-        const int j = j0 + lane;
-        rank += __popc(__ballot_sync(0xffffffffu, j < nsurv && S.surv[j] > mine));
-      }
-      if (rank < kc && lane == 0) S.cand[rank] = mine;
+    // rank by counting (keys are distinct): `sl` adjacent lanes share the comparisons of one survivor
+    int sl = 32;
+    while (sl > 1 && nsurv * sl > nthreads) sl >>= 1;
+    const int c = tid / sl, s = tid & (sl - 1);
+    const unsigned long long mine = c < nsurv ? S.surv[c] : 0ull;
+    int ahead = 0;
+    if (c < nsurv) {
+#pragma unroll 2
+      for (int j = s; j < nsurv; j += sl) ahead += S.surv[j] > mine;
     }
+    for (int o = 1; o < sl; o <<= 1) ahead += __shfl_xor_sync(0xffffffffu, ahead, o);
+    if (s == 0 && c < nsurv && ahead < kc) S.cand[ahead] = mine;
     __syncthreads();
   } else {
     block_select_topk(s_keys, total, kc, S.red, S.cand);

@@ -179,12 +179,15 @@ scan_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__
             for (int j = 0; j < KCAP; ++j) { v[j] = -INFINITY; ix[j] = -1; }
           } else if (n_mt > 1) {
 #pragma unroll
-            for (int j = 0; j < KCAP / 4; ++j) {
+            for (int j = 0; j < KCAP / 4; ++j) {   // records hold keys (see the store below): decode them
               const uint4 ua = prec[2 * j], ub = prec[2 * j + 1];
-              const float4 a = make_float4(__uint_as_float(ua.x), __uint_as_float(ua.y), __uint_as_float(ua.z), __uint_as_float(ua.w));
-              const int4 b = make_int4((int)ub.x, (int)ub.y, (int)ub.z, (int)ub.w);
-              v[4 * j] = a.x; v[4 * j + 1] = a.y; v[4 * j + 2] = a.z; v[4 * j + 3] = a.w;
-              ix[4 * j] = b.x; ix[4 * j + 1] = b.y; ix[4 * j + 2] = b.z; ix[4 * j + 3] = b.w;
+              const uint32_t lo[4] = {ua.x, ua.z, ub.x, ub.z}, hi[4] = {ua.y, ua.w, ub.y, ub.w};
+#pragma unroll
+              for (int h = 0; h < 4; ++h) {
+                const bool real = (lo[h] | hi[h]) != 0u;
+                v[4 * j + h] = real ? f32_unordered(hi[h]) : -INFINITY;
+                ix[4 * j + h] = real ? (int32_t)(0xffffffffu - lo[h]) : -1;
+              }
             }
           }
         }
@@ -218,12 +221,19 @@ scan_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__
         if (warp_active && r < B && (n_mt > 1 || tile == ntiles - 1)) {
 #pragma unroll
           for (int j = 0; j < KCAP / 4; ++j) {
-            // one 256-bit store per record: the whole 32-byte sector in one transaction (two 16-byte stores would each be
+            // A record = the finishing kernel's 64-bit keys of a quad of entries, ready made: high word = the similarity's
+            // order-preserving integer image, low word = ~index (larger key = better; 0 = empty slot).
+            // One 256-bit store per record: the whole 32-byte sector in one transaction (two 16-byte stores would each be
             // a partial-sector write that L2 has to complete from DRAM)
-            asm volatile("st.global.v8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};" ::"l"(prec + 2 * j),
-                         "r"(__float_as_uint(v[4 * j])), "r"(__float_as_uint(v[4 * j + 1])), "r"(__float_as_uint(v[4 * j + 2])),
-                         "r"(__float_as_uint(v[4 * j + 3])), "r"((uint32_t)ix[4 * j]), "r"((uint32_t)ix[4 * j + 1]),
-                         "r"((uint32_t)ix[4 * j + 2]), "r"((uint32_t)ix[4 * j + 3])
+            uint32_t kw[8];
+#pragma unroll
+            for (int h = 0; h < 4; ++h) {
+              const bool real = ix[4 * j + h] >= 0;
+              kw[2 * h] = real ? 0xffffffffu - (uint32_t)ix[4 * j + h] : 0u;
+              kw[2 * h + 1] = real ? f32_ordered(v[4 * j + h]) : 0u;
+            }
+            asm volatile("st.global.v8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};" ::"l"(prec + 2 * j), "r"(kw[0]), "r"(kw[1]),
+                         "r"(kw[2]), "r"(kw[3]), "r"(kw[4]), "r"(kw[5]), "r"(kw[6]), "r"(kw[7])
                          : "memory");
           }
         }
