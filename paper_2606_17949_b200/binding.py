@@ -35,7 +35,7 @@ class rb_options(ctypes.Structure):
                 ("dist_eps", ctypes.c_float), ("rerank_slack", ctypes.c_int32), ("lpt_enabled", ctypes.c_int32),
                 ("update_enabled", ctypes.c_int32), ("max_batch", ctypes.c_int32), ("use_graph", ctypes.c_int32),
                 ("scan_list", ctypes.c_int32), ("tiebreak_mode", ctypes.c_int32), ("latency_mode", ctypes.c_int32),
-                ("stream", ctypes.c_void_p)]
+                ("pipeline", ctypes.c_int32), ("stream", ctypes.c_void_p)]
 
 
 class rb_lat_head(ctypes.Structure):

@@ -24,30 +24,9 @@ __device__ __forceinline__ unsigned long long make_key(float sim, int32_t idx) {
 
 // ---- a0 ---------------------------------------------------------------------------------------------
 __global__ void stage_queries_kernel(const __grid_constant__ CallParams cpv, __nv_bfloat16* __restrict__ qs, int B, int Bpad,
-                                     int d, int group, uint32_t* __restrict__ gthr, int n_gthr, InstTable t,
-                                     float* __restrict__ dq, int32_t* __restrict__ bq) {
+                                     int d, int group, uint32_t* __restrict__ gthr, int n_gthr) {
   const CallParams* __restrict__ cp = &cpv;   // the per-call parameters travel as a kernel argument (constant bank)
   launch_dependents();
-  if (blockIdx.x == 0) {
-    // a8 folded in: rb_advance_state calls since the last decision (reading 22; same arithmetic as advance_kernel):
-    //   tpot = dec*(1 + slope*(float)b); q = dt/tpot; done = (float)b*q; d = max(d - done, 0); if d == 0: b = 0   (b > 0 only)
-    const int n_adv = cp->n_adv;
-    if (n_adv > 0) {
-      for (int i = threadIdx.x; i < t.I; i += blockDim.x) {
-        float dd = dq[i];
-        int b = bq[i];
-        const float dec = t.dec_i[i], slope = t.slope_i[i];
-        for (int a = 0; a < n_adv && b > 0; ++a) {
-          const float tpot = __fmul_rn(dec, __fadd_rn(1.0f, __fmul_rn(slope, (float)b)));
-          const float done = __fmul_rn((float)b, __fdiv_rn(cp->adv_ms[a], tpot));
-          dd = fmaxf(__fsub_rn(dd, done), 0.0f);
-          if (dd == 0.0f) b = 0;
-        }
-        dq[i] = dd;
-        bq[i] = b;
-      }
-    }
-  }
   for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n_gthr; i += gridDim.x * blockDim.x) gthr[i] = 0u;
   const float* __restrict__ q = cp->query;
   const size_t n = (size_t)Bpad * d;
@@ -168,11 +147,11 @@ cudaError_t launch_convert_bf16(const float* in, __nv_bfloat16* out, size_t n, c
 }
 
 cudaError_t launch_stage_queries(const CallParams& cp, __nv_bfloat16* qs, int B, int Bpad, int d, int rep, uint32_t* gthr,
-                                 int n_gthr, InstTable t, float* dq, int32_t* bq, cudaStream_t s) {
+                                 int n_gthr, cudaStream_t s) {
   const size_t n = (size_t)Bpad * d;
   int blocks = (int)((n + 255) / 256);
   if (blocks > 148 * 8) blocks = 148 * 8;
-  stage_queries_kernel<<<blocks, 256, 0, s>>>(cp, qs, B, Bpad, d, rep > 1 ? kTileM / rep : Bpad, gthr, n_gthr, t, dq, bq);
+  stage_queries_kernel<<<blocks, 256, 0, s>>>(cp, qs, B, Bpad, d, rep > 1 ? kTileM / rep : Bpad, gthr, n_gthr);
   return cudaGetLastError();
 }
 
@@ -192,7 +171,7 @@ cudaError_t launch_select_f32(const float* sims, int64_t N, int nq, int kc, floa
 // Position and count of the arguments of this file's kernels that carry the per-call parameters (graph replays update
 // that one argument): returns the index of the CallParams argument, or -1 if func is not one of them.
 int estimate_cp_arg(const void* func, int* nargs) {
-  if (func == (const void*)stage_queries_kernel) { *nargs = 11; return 0; }
+  if (func == (const void*)stage_queries_kernel) { *nargs = 8; return 0; }
   if (func == (const void*)scan_f32_kernel) { *nargs = 7; return 1; }
   if (func == (const void*)finish_kernel) { *nargs = 3; return 2; }
   return -1;

@@ -55,6 +55,21 @@ struct rb_ctx {
   float *pred_q = nullptr, *pred_l = nullptr;   // [max_batch x M] the estimate, consumed by score/dispatch
   float *stage_q = nullptr, *stage_l = nullptr; // [max_batch x M] staging of caller-supplied predictions (host)
   float *termA = nullptr, *termP = nullptr, *key = nullptr;
+  // Pipelined decisions (rb_options.pipeline): a second set of everything a decision's estimate hands to its dispatch
+  // side (staged queries + their tensor map, partial lists, predictions, terms, keys), an internal stream for the front
+  // half (staging + scan) and the events that order the two halves and the reuse of a set.
+  struct Slot {
+    __nv_bfloat16* qs = nullptr;
+    CUtensorMap tm_q{};
+    float* part_sim = nullptr;
+    int32_t* part_idx = nullptr;
+    float *pred_q = nullptr, *pred_l = nullptr, *termA = nullptr, *termP = nullptr, *key = nullptr;
+    cudaEvent_t ev_front = nullptr;   // front half (staging + scan) done, recorded on the front stream
+    cudaEvent_t ev_back = nullptr;    // back half (finish + dispatch) done, recorded on the context's stream
+  } slot[2];
+  cudaStream_t front = nullptr;       // low-priority internal stream of the front halves
+  uint64_t pipe_seq = 0;              // pipelined decisions issued so far (slot = seq & 1)
+  bool front_busy = false;            // a front half may still be running on the internal stream
   int32_t *order = nullptr, *assignment = nullptr, *max_tokens = nullptr;
   float* budget = nullptr;          // [max_batch] staging of host budgets
   uint8_t* arena = nullptr;         // one allocation behind all the small per-decision buffers
@@ -230,126 +245,120 @@ struct Timer {
 };
 
 // with_terms: the finishing kernel also derives the score terms (rb_decide); otherwise estimate only.
-rb_status enqueue_estimate(rb_ctx* ctx, int B, bool with_terms, Timer& tm) {
-  cudaStream_t s = ctx->stream;
+// sl: buffer set.  part: kAll = staging + scan + finish on stream s; kFront = staging + scan; kBack = finish.
+enum EstimatePart { kAll = 0, kFront = 1, kBack = 2 };
+rb_status enqueue_estimate(rb_ctx* ctx, int B, bool with_terms, Timer& tm, int sl = 0, EstimatePart part = kAll,
+                           cudaStream_t s = nullptr) {
+  if (!s) s = ctx->stream;
+  rb_ctx::Slot& S = ctx->slot[sl];
   const int Bpad = (B + kTileM - 1) / kTileM * kTileM;
   FinishArgs fa{};
   fa.kc = ctx->kc; fa.k = ctx->k; fa.N = ctx->N; fa.d = ctx->d;
   fa.bank_quality = ctx->bank_quality; fa.bank_outlen = ctx->bank_outlen; fa.M = ctx->M;
   fa.weight_mode = ctx->opt.weight_mode; fa.eps = ctx->opt.dist_eps; fa.with_terms = with_terms ? 1 : 0;
-  fa.pred_q = ctx->pred_q; fa.pred_l = ctx->pred_l; fa.termA = ctx->termA; fa.termP = ctx->termP; fa.key = ctx->key;
+  fa.pred_q = S.pred_q; fa.pred_l = S.pred_l; fa.termA = S.termA; fa.termP = S.termP; fa.key = S.key;
+  const bool front = part != kBack, back = part != kFront;
   if (ctx->opt.store_dtype == RB_BF16) {
-    if (ctx->stage_timing) {   // before the first mark: nothing but the kernels between the stage events
+    if (ctx->stage_timing && front) {   // before the first mark: nothing but the kernels between the stage events
       CK(cudaMemcpyAsync(ctx->dev_clock, ctx->dev_clock_init, 16, cudaMemcpyDeviceToDevice, s));
     }
-    tm.mark();
+    if (front) tm.mark();
     if (B > kTileM && ctx->num_sms >= 2) {
       // tensor-bound regime: CTA pairs, 256-query m-tiles
       const int Bpad2 = (B + 2 * kTileM - 1) / (2 * kTileM) * (2 * kTileM);
-      CK(launch_stage_queries(ctx->cp_cur, ctx->qs, B, Bpad2, ctx->d, 1, ctx->gthr,
-                              Bpad2 * (1 + scan_tc2_clusters(ctx->N, ctx->num_sms)), table_of(ctx), ctx->dq, ctx->bq, s));
-      tm.mark();
-      int ncl = 0;
+      const int ncl = scan_tc2_clusters(ctx->N, ctx->num_sms);
       // lists of at most 16 entries per (cluster, query): longer ones put the sorted insertions (in global memory) on the
       // tensor pipe's time line (k = 32: 0.54 of the tensor roofline with 64-entry lists); a cluster whose list is
       // popped completely is searched again by the finishing kernel, as for the single-CTA scan
       const int kcap2 = std::min(ctx->kcap, 16);
-      CK(launch_scan_tc2(&ctx->tm_q, &ctx->tm_bank, ctx->N, ctx->d, B, Bpad2, kcap2, ctx->kc, ctx->num_sms, ctx->part_sim,
-                         ctx->part_idx, ctx->gthr, &ncl, s));
-      tm.mark();
-      fa.part_sim = ctx->part_sim; fa.part_idx = ctx->part_idx; fa.nlists = ncl; fa.lists_per_cta = 1; fa.kcap = kcap2;
+      if (front) {
+        CK(launch_stage_queries(ctx->cp_cur, S.qs, B, Bpad2, ctx->d, 1, ctx->gthr, Bpad2 * (1 + ncl), s));
+        tm.mark();
+        int ncl_used = 0;
+        CK(launch_scan_tc2(&S.tm_q, &ctx->tm_bank, ctx->N, ctx->d, B, Bpad2, kcap2, ctx->kc, ctx->num_sms, S.part_sim,
+                           S.part_idx, ctx->gthr, &ncl_used, s));
+        tm.mark();
+        ctx->launches += 2;
+      }
+      fa.part_sim = S.part_sim; fa.part_idx = S.part_idx; fa.nlists = ncl; fa.lists_per_cta = 1; fa.kcap = kcap2;
       fa.Bpad = Bpad2; fa.slab_unit = kTileN; fa.rescan = kcap2 < ctx->kc ? 1 : 0;
     } else {
       const int rep = scan_tc_replicas(B, ctx->ks, ctx->num_sms);
-      CK(launch_stage_queries(ctx->cp_cur, ctx->qs, B, Bpad, ctx->d, rep, ctx->gthr, Bpad, table_of(ctx), ctx->dq, ctx->bq, s));
-      tm.mark();
-      int grid = 0;
-      CK(launch_scan_tc(&ctx->tm_q, &ctx->tm_bank, ctx->N, ctx->d, B, Bpad, ctx->ks, ctx->num_sms, ctx->part_sim,
-                        ctx->part_idx, &grid, ctx->stage_timing ? ctx->dev_clock : nullptr, s));
-      tm.mark();
-      fa.part_sim = ctx->part_sim; fa.part_idx = ctx->part_idx; fa.nlists = grid * rep; fa.lists_per_cta = rep; fa.kcap = ctx->ks;
+      const int64_t units = (ctx->N + kBoxN - 1) / kBoxN;
+      const int grid = (int)(units < ctx->num_sms ? units : ctx->num_sms);   // what launch_scan_tc uses
+      if (front) {
+        CK(launch_stage_queries(ctx->cp_cur, S.qs, B, Bpad, ctx->d, rep, ctx->gthr, 0, s));
+        tm.mark();
+        int grid_used = 0;
+        CK(launch_scan_tc(&S.tm_q, &ctx->tm_bank, ctx->N, ctx->d, B, Bpad, ctx->ks, ctx->num_sms, S.part_sim, S.part_idx,
+                          &grid_used, ctx->stage_timing ? ctx->dev_clock : nullptr, s));
+        tm.mark();
+        ctx->launches += 2;
+      }
+      fa.part_sim = S.part_sim; fa.part_idx = S.part_idx; fa.nlists = grid * rep; fa.lists_per_cta = rep; fa.kcap = ctx->ks;
       fa.records = 1;
       fa.Bpad = Bpad; fa.slab_unit = kBoxN;
+      fa.rescan = ctx->ks < ctx->kc ? 1 : 0;
     }
-    if (!(B > kTileM && ctx->num_sms >= 2)) fa.rescan = ctx->ks < ctx->kc ? 1 : 0;
-    fa.bank = (const __nv_bfloat16*)ctx->bank; fa.qs = ctx->qs; fa.rerank = ctx->opt.rerank_slack > 0 ? 1 : 0;
-    ctx->launches += 2;
+    fa.bank = (const __nv_bfloat16*)ctx->bank; fa.qs = S.qs; fa.rerank = ctx->opt.rerank_slack > 0 ? 1 : 0;
   } else {
-    tm.mark();
-    tm.mark();
-    for (int r0 = 0; r0 < B; r0 += kF32Group) {
-      const int nq = (B - r0 < kF32Group) ? (B - r0) : kF32Group;
-      CK(launch_scan_f32((const float*)ctx->bank, ctx->cp_cur, r0, ctx->N, ctx->d, nq, ctx->sims, s));
-      CK(launch_select_f32(ctx->sims, ctx->N, nq, ctx->kc, ctx->cand_sim + (size_t)r0 * ctx->kc,
-                           ctx->cand_idx + (size_t)r0 * ctx->kc, s));
-      ctx->launches += 2;
+    if (front) {
+      tm.mark();
+      tm.mark();
+      for (int r0 = 0; r0 < B; r0 += kF32Group) {
+        const int nq = (B - r0 < kF32Group) ? (B - r0) : kF32Group;
+        CK(launch_scan_f32((const float*)ctx->bank, ctx->cp_cur, r0, ctx->N, ctx->d, nq, ctx->sims, s));
+        CK(launch_select_f32(ctx->sims, ctx->N, nq, ctx->kc, ctx->cand_sim + (size_t)r0 * ctx->kc,
+                             ctx->cand_idx + (size_t)r0 * ctx->kc, s));
+        ctx->launches += 2;
+      }
+      tm.mark();
     }
-    tm.mark();
     // the selected candidates are one already-merged list per query: [1][B][kc]
     fa.part_sim = ctx->cand_sim; fa.part_idx = ctx->cand_idx; fa.nlists = 1; fa.lists_per_cta = 1; fa.kcap = ctx->kc; fa.Bpad = B;
     fa.slab_unit = kBoxN;
     fa.bank = nullptr; fa.qs = nullptr; fa.rerank = 0;
   }
-  CK(launch_finish(fa, table_of(ctx), ctx->cp_cur, B, s));
-  ctx->launches += 1;
-  tm.mark();
+  if (back) {
+    CK(launch_finish(fa, table_of(ctx), ctx->cp_cur, B, s));
+    ctx->launches += 1;
+    tm.mark();
+  }
   return RB_OK;
 }
 
-rb_status enqueue_dispatch(rb_ctx* ctx, int B, bool from_predictions, Timer& tm) {
+rb_status enqueue_dispatch(rb_ctx* ctx, int B, bool from_predictions, Timer& tm, int sl = 0) {
   cudaStream_t s = ctx->stream;
+  rb_ctx::Slot& S = ctx->slot[sl];
   InstTable t = table_of(ctx);
   if (from_predictions) {
     if (ctx->opt.latency_mode == 2) {
       CK(launch_tpot_forest(t, forest_of(ctx), ctx->dq, ctx->bq, ctx->f_tpot0, -1.0f, s));
       ctx->launches += 1;
     }
-    CK(launch_score(t, ctx->dq, ctx->bq, ctx->cp_cur, B, ctx->termA, ctx->termP, ctx->key, modes_of(ctx), forest_of(ctx), s));
+    CK(launch_score(t, ctx->dq, ctx->bq, ctx->cp_cur, B, S.termA, S.termP, S.key, modes_of(ctx), forest_of(ctx), s));
     ctx->launches += 1;
   }
   tm.mark();
-  CK(launch_lpt_dispatch(t, ctx->dq, ctx->bq, ctx->termA, ctx->termP, ctx->key, ctx->cp_cur, B, modes_of(ctx), forest_of(ctx), s));
+  CK(launch_lpt_dispatch(t, ctx->dq, ctx->bq, S.termA, S.termP, S.key, ctx->cp_cur, B, modes_of(ctx), forest_of(ctx), s));
   tm.mark();
   ctx->launches += 1;
   return RB_OK;
 }
 
-// kind: 0 = estimate + dispatch, 1 = estimate, 2 = dispatch (+scores0)
-rb_status run_path(rb_ctx* ctx, int B, int kind) {
-  // With stage timing on, the same launch sequence is captured with event-record nodes between the kernels (a
-  // separate graph per shape): the stage intervals then hold graph-internal launch latencies like a decision's, not
-  // host-side ones.  The kernels lose their programmatic overlap across the event nodes, so the SUM of the stages is
-  // longer than a decision; each stage's own duration is what is read.
-  const bool graph = ctx->opt.use_graph != 0;
-  Timer tm(ctx);
-  if (!graph) {
-    if (kind == 0 && ctx->opt.latency_mode == 2) {   // the head over the batch-start state; only the state feeds it
-      CK(launch_tpot_forest(table_of(ctx), forest_of(ctx), ctx->dq, ctx->bq, ctx->f_tpot0, -1.0f, ctx->stream));
-      ctx->launches += 1;
-    }
-    if (kind != 2) {
-      rb_status st = enqueue_estimate(ctx, B, kind == 0, tm);
-      if (st != RB_OK) return st;
-    }
-    if (kind != 1) return enqueue_dispatch(ctx, B, kind == 2, tm);
-    return RB_OK;
-  }
-  const int64_t gkey = (int64_t)B * 8 + kind + (ctx->stage_timing ? 4 : 0);
+// Runs the launch sequence `enqueue` on stream s as a CUDA graph: captured and instantiated the first time a key is seen,
+// replayed afterwards with this call's parameters (the per-call parameters are an argument of the kernels that need them;
+// a replay rewrites that one argument of those kernel nodes, cudaGraphExecKernelNodeSetParams).
+template <typename F>
+rb_status graph_run(rb_ctx* ctx, int64_t gkey, cudaStream_t s, F&& enqueue) {
   auto it = ctx->graphs.find(gkey);
   if (it == ctx->graphs.end()) {
     const int64_t before = ctx->launches;
     cudaGraph_t g = nullptr;
-    CK(cudaStreamBeginCapture(ctx->stream, cudaStreamCaptureModeThreadLocal));
+    CK(cudaStreamBeginCapture(s, cudaStreamCaptureModeThreadLocal));
     ctx->capturing = true;
-    rb_status st = RB_OK;
-    if (kind == 0 && ctx->opt.latency_mode == 2) {
-      if (launch_tpot_forest(table_of(ctx), forest_of(ctx), ctx->dq, ctx->bq, ctx->f_tpot0, -1.0f, ctx->stream) != cudaSuccess)
-        st = fail(ctx, RB_ECUDA, "launch_tpot_forest");
-      ctx->launches += 1;
-    }
-    if (st == RB_OK && kind != 2) st = enqueue_estimate(ctx, B, kind == 0, tm);
-    if (st == RB_OK && kind != 1) st = enqueue_dispatch(ctx, B, kind == 2, tm);
-    cudaError_t e = cudaStreamEndCapture(ctx->stream, &g);
+    rb_status st = enqueue();
+    cudaError_t e = cudaStreamEndCapture(s, &g);
     ctx->capturing = false;
     const int nodes = (int)(ctx->launches - before);
     ctx->launches = before;
@@ -395,8 +404,59 @@ rb_status run_path(rb_ctx* ctx, int B, int kind) {
       CK(cudaGraphExecKernelNodeSetParams(it->second.exec, cn.node, &cn.params));
     }
   }
-  CK(cudaGraphLaunch(it->second.exec, ctx->stream));
+  CK(cudaGraphLaunch(it->second.exec, s));
   ctx->launches += it->second.nodes;
+  return RB_OK;
+}
+
+int64_t graph_key(const rb_ctx* ctx, int B, int kind, int sl) {
+  return (((int64_t)B * 8 + kind) * 2 + sl) * 2 + (ctx->stage_timing ? 1 : 0);
+}
+
+// kind: 0 = estimate + dispatch, 1 = estimate, 2 = dispatch (+scores0)
+rb_status run_path(rb_ctx* ctx, int B, int kind) {
+  // With stage timing on, the same launch sequence is captured with event-record nodes between the kernels (a
+  // separate graph per shape): the stage intervals then hold graph-internal launch latencies like a decision's, not
+  // host-side ones.  The kernels lose their programmatic overlap across the event nodes, so the SUM of the stages is
+  // longer than a decision; each stage's own duration is what is read.
+  Timer tm(ctx);
+  auto enqueue = [&]() -> rb_status {
+    if (kind == 0 && ctx->opt.latency_mode == 2) {   // the head over the batch-start state; only the state feeds it
+      if (launch_tpot_forest(table_of(ctx), forest_of(ctx), ctx->dq, ctx->bq, ctx->f_tpot0, -1.0f, ctx->stream) != cudaSuccess)
+        return fail(ctx, RB_ECUDA, "launch_tpot_forest");
+      ctx->launches += 1;
+    }
+    rb_status st = RB_OK;
+    if (kind != 2) st = enqueue_estimate(ctx, B, kind == 0, tm);
+    if (st == RB_OK && kind != 1) st = enqueue_dispatch(ctx, B, kind == 2, tm);
+    return st;
+  };
+  rb_status st = ctx->opt.use_graph ? graph_run(ctx, graph_key(ctx, B, kind, 0), ctx->stream, enqueue) : enqueue();
+  // (a later pipelined decision's front half must not start on this buffer set before this work is done)
+  if (st == RB_OK && ctx->front && kind != 2) CK(cudaEventRecord(ctx->slot[0].ev_back, ctx->stream));
+  return st;
+}
+
+// rb_decide in throughput mode (rb_options.pipeline): the front half of the decision (staging + bank scan) goes to the
+// internal low-priority stream, the back half (finishing + dispatch) to the context's stream, joined by events; the two
+// buffer sets alternate, so the front half of this call overlaps the back half of the call before it.
+rb_status run_pipelined(rb_ctx* ctx, int B) {
+  const int sl = (int)(ctx->pipe_seq & 1);
+  rb_ctx::Slot& S = ctx->slot[sl];
+  Timer tm(ctx);
+  CK(cudaStreamWaitEvent(ctx->front, S.ev_back, 0));   // the back half that last read this buffer set is done
+  rb_status st = graph_run(ctx, graph_key(ctx, B, 3, sl), ctx->front,
+                           [&]() -> rb_status { return enqueue_estimate(ctx, B, true, tm, sl, kFront, ctx->front); });
+  if (st != RB_OK) return st;
+  CK(cudaEventRecord(S.ev_front, ctx->front));
+  CK(cudaStreamWaitEvent(ctx->stream, S.ev_front, 0));
+  st = graph_run(ctx, graph_key(ctx, B, 4, sl), ctx->stream, [&]() -> rb_status {
+    rb_status s1 = enqueue_estimate(ctx, B, true, tm, sl, kBack, ctx->stream);
+    return s1 != RB_OK ? s1 : enqueue_dispatch(ctx, B, false, tm, sl);
+  });
+  if (st != RB_OK) return st;
+  CK(cudaEventRecord(S.ev_back, ctx->stream));
+  ctx->pipe_seq += 1;
   return RB_OK;
 }
 
@@ -544,6 +604,7 @@ void rb_options_default(rb_options* opt) {
   opt->scan_list = 0;
   opt->tiebreak_mode = 0;
   opt->latency_mode = 0;
+  opt->pipeline = 0;
   opt->stream = nullptr;
 }
 
@@ -567,6 +628,7 @@ rb_status rb_create(rb_ctx** out, const void* bank_emb, const float* bank_qualit
   if (opt.tiebreak_mode != 0 && opt.tiebreak_mode != 1) return RB_EINVAL;
   if (opt.latency_mode < 0 || opt.latency_mode > 2) return RB_EINVAL;
   opt.lpt_enabled = opt.lpt_enabled ? 1 : 0;
+  opt.pipeline = (opt.pipeline && opt.store_dtype == RB_BF16) ? 1 : 0;
   if (opt.scan_list != 0 && opt.scan_list != 4 && opt.scan_list != 8 && opt.scan_list != 16 && opt.scan_list != 32 &&
       opt.scan_list != 64)
     return RB_EINVAL;
@@ -689,6 +751,10 @@ rb_status rb_create(rb_ctx** out, const void* bank_emb, const float* bank_qualit
                  o_dec = take(kMaxM * 4), o_slope = take(kMaxM * 4), o_deci = take(kMaxI * 4), o_slopei = take(kMaxI * 4),
                  o_aux = take((size_t)kMaxI * kMaxFeatures * 4), o_tpot0 = take(kMaxI * 4), o_mem = take(kMaxI * 4),
                  o_tst = take((kMaxM + 1) * 4), o_cur = take(kMaxM * 4), o_cnt = take(8);
+    // second set of what an estimate hands to its dispatch side (pipelined decisions of at most 128 requests)
+    const size_t m1 = opt.pipeline ? (size_t)kTileM : 0;
+    const size_t o_pq1 = take(m1 * M * 4), o_pl1 = take(m1 * M * 4), o_ta1 = take(m1 * M * 4), o_tp1 = take(m1 * M * 4),
+                 o_key1 = take(m1 * 4);
     ALLOC(ctx->arena, off);
     uint8_t* a = ctx->arena;
     ctx->plen = (int32_t*)(a + o_plen); ctx->cand_sim = (float*)(a + o_csim);
@@ -703,6 +769,11 @@ rb_status rb_create(rb_ctx** out, const void* bank_emb, const float* bank_qualit
     ctx->f_aux = (float*)(a + o_aux); ctx->f_tpot0 = (float*)(a + o_tpot0);
     ctx->members = (int32_t*)(a + o_mem); ctx->tstart = (int32_t*)(a + o_tst); ctx->pipe_cursor = (int32_t*)(a + o_cur);
     ctx->pipe_counter = (unsigned long long*)(a + o_cnt);
+    {
+      rb_ctx::Slot& S1 = ctx->slot[1];
+      S1.pred_q = (float*)(a + o_pq1); S1.pred_l = (float*)(a + o_pl1); S1.termA = (float*)(a + o_ta1);
+      S1.termP = (float*)(a + o_tp1); S1.key = (float*)(a + o_key1);
+    }
     CK(cudaMemsetAsync(ctx->arena, 0, off, s));
   }
   if (opt.store_dtype == RB_BF16) {
@@ -717,8 +788,31 @@ rb_status rb_create(rb_ctx** out, const void* bank_emb, const float* bank_qualit
     if (st != RB_OK) return st;
     st = encode_map(ctx, &ctx->tm_q, ctx->qs, (uint64_t)ctx->Bpad_max, (uint64_t)d, kTileM);
     if (st != RB_OK) return st;
+    if (opt.pipeline) {
+      // second buffer set, for batches of at most 128 requests (larger ones are not pipelined)
+      rb_ctx::Slot& S1 = ctx->slot[1];
+      ALLOC(S1.qs, (size_t)kTileM * d);
+      const size_t part_n1 = (size_t)ctx->num_sms * ctx->kcap * 4 * kTileM;
+      ALLOC(S1.part_sim, 2 * part_n1);
+      S1.part_idx = reinterpret_cast<int32_t*>(S1.part_sim + part_n1);
+      CK(cudaMemsetAsync(S1.qs, 0, (size_t)kTileM * d * 2, s));
+      st = encode_map(ctx, &S1.tm_q, S1.qs, (uint64_t)kTileM, (uint64_t)d, kTileM);
+      if (st != RB_OK) return st;
+      int lo = 0, hi = 0;
+      CK(cudaDeviceGetStreamPriorityRange(&lo, &hi));   // lo = least priority
+      CK(cudaStreamCreateWithPriority(&ctx->front, cudaStreamNonBlocking, lo));
+      for (int j = 0; j < 2; ++j) {
+        CK(cudaEventCreateWithFlags(&ctx->slot[j].ev_front, cudaEventDisableTiming));
+        CK(cudaEventCreateWithFlags(&ctx->slot[j].ev_back, cudaEventDisableTiming));
+      }
+    }
     CK(scan_tc_prepare());
     CK(scan_tc2_prepare());
+  }
+  {
+    rb_ctx::Slot& S0 = ctx->slot[0];   // the primary buffer set
+    S0.qs = ctx->qs; S0.tm_q = ctx->tm_q; S0.part_sim = ctx->part_sim; S0.part_idx = ctx->part_idx;
+    S0.pred_q = ctx->pred_q; S0.pred_l = ctx->pred_l; S0.termA = ctx->termA; S0.termP = ctx->termP; S0.key = ctx->key;
   }
   {
     const int rr = opt.rerank_slack > 0 ? 1 : 0;
@@ -987,9 +1081,17 @@ rb_status rb_decide_budgeted(rb_ctx* ctx, const float* query_emb, const int32_t*
   } else {
     sg.needs_sync = sg.any_host;
   }
+  // throughput mode: device buffers only (host buffers make the call synchronous anyway), at most one 128-query tile
+  const bool pipelined = ctx->front != nullptr && !sg.any_host && B <= kTileM && adv_folded && !ctx->stage_timing &&
+                         ctx->opt.use_graph != 0;
+  if (pipelined) {
+    const rb_ctx::Slot& S = ctx->slot[ctx->pipe_seq & 1];
+    cp.q_src = S.pred_q;
+    cp.l_src = S.pred_l;
+  }
   st = push_params(ctx, cp);
   if (st != RB_OK) return st;
-  st = run_path(ctx, B, 0);
+  st = pipelined ? run_pipelined(ctx, B) : run_path(ctx, B, 0);
   if (st != RB_OK) return st;
   if (adv_folded) ctx->n_pending = 0;
   collect_stage_times(ctx, 0);
@@ -1232,12 +1334,20 @@ const char* rb_last_error(const rb_ctx* ctx) { return ctx ? ctx->err.c_str() : "
 
 void rb_destroy(rb_ctx* ctx) {
   if (!ctx) return;
+  if (ctx->front) cudaStreamSynchronize(ctx->front);
   if (ctx->stream) cudaStreamSynchronize(ctx->stream);
   drop_graphs(ctx);
   void* ptrs[] = {ctx->bank, ctx->bank_quality, ctx->bank_outlen, ctx->arena, ctx->q32, ctx->qs, ctx->part_sim,
                   ctx->gthr, ctx->sims, ctx->scratch_nn_idx, ctx->scratch_nn_sim, ctx->scores, ctx->scores0, ctx->f_nodes,
                   ctx->f_root, ctx->f_begin, ctx->f_base, ctx->dev_clock, ctx->sweep_buf};
   for (void* p : ptrs) cudaFree(p);
+  cudaFree(ctx->slot[1].qs);
+  cudaFree(ctx->slot[1].part_sim);
+  for (auto& sl : ctx->slot) {
+    if (sl.ev_front) cudaEventDestroy(sl.ev_front);
+    if (sl.ev_back) cudaEventDestroy(sl.ev_back);
+  }
+  if (ctx->front) cudaStreamDestroy(ctx->front);
   for (auto& e : ctx->ev)
     if (e) cudaEventDestroy(e);
   if (ctx->h_zc) cudaFreeHost(ctx->h_zc);

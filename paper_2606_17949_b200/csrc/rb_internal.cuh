@@ -66,7 +66,7 @@ struct CallParams {
   int32_t* max_tokens;     // [B] or NULL: output-token clamp of the chosen instance
   uint32_t* done_flag;     // pinned host word or NULL: the dispatch kernel stores done_seq there once the assignment is out
   uint32_t done_seq;       //   (host callers wait on it instead of synchronising the stream)
-  int32_t n_adv;           // pending rb_advance_state calls folded into this decision's first kernel (<= kMaxPendingAdvance)
+  int32_t n_adv;           // pending rb_advance_state calls folded into this decision's dispatch kernel (<= kMaxPendingAdvance)
   float adv_ms[4];         // their elapsed_ms, in call order
   const float* sweep_w;    // weight sweep (rb_sweep_weights): [P x 3] weights, point p = the CTA's grid coordinate; the
                            //   term, key and assignment arrays are then [P][...]; NULL: the w_* fields above
@@ -218,9 +218,8 @@ cudaError_t launch_convert_bf16(const float* in, __nv_bfloat16* out, size_t n, c
 
 // a0: cp->query (fp32) -> bf16 staging [Bpad x d]; rep copies of the B queries at rows j*(128/rep) + r (rep > 1 only
 // when Bpad = 128), all other rows zero.  Also clears gthr [n_gthr] (the scan's cross-slab thresholds).
-// Block 0 also applies the cp->n_adv pending state advances (a8's drain rule, linear head) to (dq, bq), in call order.
 cudaError_t launch_stage_queries(const CallParams& cp, __nv_bfloat16* qs, int B, int Bpad, int d, int rep, uint32_t* gthr,
-                                 int n_gthr, InstTable t, float* dq, int32_t* bq, cudaStream_t s);
+                                 int n_gthr, cudaStream_t s);
 // query replicas over the TMEM lane quarters: 4 (B <= 32), 2 (B <= 64), 1; halved while the finishing kernel could not
 // hold max_grid * replicas lists of kcap entries in shared memory (long lists: k = 32)
 int scan_tc_replicas(int B, int kcap, int max_grid);

@@ -12,7 +12,7 @@ int main(void) {
   rb_options_default(&opt);
   if (opt.bank_dtype != RB_F32 || opt.store_dtype != RB_BF16 || opt.weight_mode != 0 || opt.rerank_slack != 6 ||
       opt.lpt_enabled != 1 || opt.update_enabled != 1 || opt.max_batch != 4096 || opt.use_graph != 1 ||
-      opt.scan_list != 0 || opt.tiebreak_mode != 0 || opt.latency_mode != 0 || opt.stream != NULL) {
+      opt.scan_list != 0 || opt.tiebreak_mode != 0 || opt.latency_mode != 0 || opt.pipeline != 0 || opt.stream != NULL) {
     printf("defaults differ from the header\n");
     return 1;
   }

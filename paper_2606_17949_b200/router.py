@@ -18,7 +18,7 @@ from . import binding as rb
 class Router:
     def __init__(self, bank_emb, bank_quality, bank_outlen, k, *, store="bf16", rerank_slack=None, weight_mode=0,
                  dist_eps=1e-6, lpt_enabled=1, update_enabled=1, max_batch=4096, use_graph=1, scan_list=0, tiebreak_mode=0,
-                 latency_mode=0, device="cuda"):
+                 latency_mode=0, pipeline=0, device="cuda"):
         N, d = bank_emb.shape
         M = bank_quality.shape[1]
         opt = rb.rb_options_default()
@@ -35,6 +35,7 @@ class Router:
         opt.scan_list = scan_list
         opt.tiebreak_mode = tiebreak_mode
         opt.latency_mode = latency_mode
+        opt.pipeline = pipeline
         self.device = torch.device(device)
         self.stream = torch.cuda.Stream(device=self.device)
         opt.stream = self.stream.cuda_stream

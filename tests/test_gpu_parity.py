@@ -980,3 +980,77 @@ def test_adaptive_batch_rule_and_stream_driver_lockstep(orc):
         with pytest.raises(rb.RbError):
             rt.batch_target(lo, hi)
     rt.close()
+
+
+def test_pipelined_decisions_equal_unpipelined_ones(orc):
+    """rb_options.pipeline (throughput mode: the bank scan of a decision overlaps the finishing and dispatch stages of the
+    one before it, two buffer sets alternating): a stream of 300 decisions of varying size with rb_advance_state between
+    them, estimate-only calls, state reads and a budgeted call mixed in, gives bit for bit the outputs and the final state
+    of the same calls on an unpipelined context; and the first 40 decisions are checked against the oracle in lock-step."""
+    cfg = dataclasses.replace(synth.CONFIGS["C2"], N=30000, d=256, Kc=16, seed=61)
+    bank = synth.make_bank(cfg, device="cuda")
+    it = synth.make_instances(cfg.I, cfg.M, cap=6)
+    queued, running = synth.make_state(cfg.I, it["cap"], cfg.seed)
+    rng = np.random.default_rng(61)
+    sizes = [int(x) for x in rng.integers(1, 129, 300)]
+    q = synth.make_queries(cfg, B=sum(sizes), device="cuda")
+    p = synth.make_prompt_len(cfg, B=sum(sizes), device="cuda")
+    torch.cuda.synchronize()
+    presets = list(synth.PRESETS.values())
+    outs = []
+    for pipeline in (0, 1):
+        rt = _router(bank, cfg, max_batch=128, pipeline=pipeline)
+        rt.set_instances(**it)
+        rt.set_state(queued, running)
+        rec, off = [], 0
+        for j, B in enumerate(sizes):
+            rt.advance_state(float(3.0 + (j % 7)))
+            if j % 5 == 4:
+                rt.advance_state(1.5)                      # two pending advances folded into one decision
+            qq, pp = q[off:off + B], p[off:off + B]
+            if j % 37 == 36:
+                bud = torch.full((B,), 1e9, device="cuda")
+                o = rt.decide(qq, pp, presets[j % 4], budget=bud)
+            else:
+                o = rt.decide(qq, pp, presets[j % 4])
+            rec.append({k_: v.clone() for k_, v in o.items()})
+            if j % 23 == 22:
+                e = rt.estimate(qq[:min(B, 9)])            # an unpipelined call in between
+                rec.append({k_: v.clone() for k_, v in e.items()})
+            if j % 41 == 40:
+                s = rt.get_state()
+                rec.append({"dq": s[0].clone(), "bq": s[1].clone()})
+            off += B
+        rt.sync()
+        s = rt.get_state()
+        rec.append({"dq": s[0].clone(), "bq": s[1].clone()})
+        outs.append(rec)
+        rt.close()
+    assert len(outs[0]) == len(outs[1])
+    for a, b in zip(*outs):
+        assert a.keys() == b.keys()
+        for key in a:
+            assert torch.equal(a[key].cpu(), b[key].cpu()), key
+    # lock-step against the oracle (predictions from the GPU, DESIGN.md parity protocol), pipelined context
+    rt = _router(bank, cfg, max_batch=128, pipeline=1)
+    rt.set_instances(**it)
+    rt.set_state(queued, running)
+    inst = orc.Instances(**it)
+    dq, bq = queued.numpy().copy(), running.numpy().copy()
+    off, res = 0, []
+    for j, B in enumerate(sizes[:40]):
+        rt.advance_state(float(3.0 + (j % 7)))
+        res.append(rt.decide(q[off:off + B], p[off:off + B], presets[j % 4]))   # no synchronisation: calls pile up
+        off += B
+    rt.sync()
+    off = 0
+    for j, B in enumerate(sizes[:40]):
+        g = {k_: v.cpu().numpy() for k_, v in res[j].items()}
+        dq, bq = orc.advance_state(inst, dq, bq, np.float32(3.0 + (j % 7)))
+        ref = parity.check_dispatch(orc, inst, dq, bq, g["pred_quality"], g["pred_outlen"], p[off:off + B].cpu().numpy(),
+                                    presets[j % 4], g)
+        dq, bq = ref["queued"], ref["running"]
+        off += B
+    s = rt.get_state()
+    assert np.array_equal(s[0].numpy(), dq) and np.array_equal(s[1].numpy(), bq)
+    rt.close()
