@@ -11,8 +11,13 @@ Poisson arrivals at 12 and 30 req/s batched into windows of 4..64 requests, the 
 All inputs are seeded synthetic stand-ins for the paper's dataset (paper_2606_17949_b200/synth.py).
 
 One JSON line is printed by rank 0:
-  value        requests routed per second, inputs resident in HBM, device time (CUDA events on the library's
-               stream, one pair per step, L2 flushed between steps by default), whole job over all ranks
+  value        requests routed per second, inputs resident in HBM: the K timed steps issued back to back on a context in
+               throughput mode (rb_options.pipeline: the scan of a decision overlaps the finishing and dispatch stages of
+               the one before it), device time between one CUDA-event pair on the library's stream, whole job over all
+               ranks.  The bank (153.6 MB) is larger than L2 (126 MB): no flush between steps.
+  decision_us  latency of ONE decision (unpipelined context, L2 flushed before every decision, CUDA events around each):
+               median / p99 over at least 300 decisions whatever --steps says; unpipelined_flushed_requests_per_s is the
+               throughput that figure gives (the round-1 definition of value)
   e2e          the same through the C ABI with pinned HOST buffers: H2D of the step's queries and prompt
                lengths and D2H of the assignment inside the timed region (wall clock per call; the call
                returns when the host output is complete)
@@ -96,6 +101,40 @@ def bank_to_numpy(emb):
     if e.dtype == torch.bfloat16:
         return e.view(torch.int16).numpy().view(np.uint16)
     return e.numpy()
+
+
+def c2_config(cfg, world):
+    """The `config` object of the JSON line: the same dict from both arms (the reference arm's bounded sample is
+    described under its cpu_baseline.sample, not here)."""
+    return {"workload": "C2 paper-shaped stream (BASELINE.json configs[1])", "N": cfg.N, "d": cfg.d, "M": cfg.M,
+            "I": cfg.I, "k": cfg.k, "B": "windows of 4..64 requests (mean ~12.6)", "bank": "bf16 153.6 MB",
+            "arrivals": "Poisson 12 req/s (first half of the steps) and 30 req/s (second half)",
+            "weights": "quality/latency/cost/balanced presets in turn", "rerank_slack": 6,
+            "l2": "bank (153.6 MB) larger than L2 (126 MB), steps back to back; the per-decision latency leg flushes L2 "
+                  "before every decision",
+            "graph": "CUDA graph replay per B", "parallelism": "replicas only" if world > 1 else "single GPU"}
+
+
+def read_only_peak_gbs(rt, rb):
+    """Read-only streaming bandwidth of this GPU (rb_testing_read_bandwidth: a plain coalesced 16-byte-load kernel over
+    2 GiB, best of 10): the ceiling a read-dominated kernel can reach; MEASURED_PEAKS.json's figure is a copy (read +
+    write) and sits below it."""
+    return rb.rb_testing_read_bandwidth(rt.ctx, 2 << 30, 10)
+
+
+def c_harness_e2e(N, d, B, I, steps=300):
+    """examples/e2e_bench.c: rb_advance_state + rb_decide from host buffers through the C ABI, no Python on the path."""
+    import subprocess
+    import tempfile
+    pkg = os.path.join(ROOT, "paper_2606_17949_b200")
+    exe = os.path.join(tempfile.mkdtemp(), "e2e_bench")
+    try:
+        subprocess.run(["gcc", "-std=c99", "-O2", "-I", os.path.join(ROOT, "include"), os.path.join(pkg, "examples", "e2e_bench.c"),
+                        "-o", exe, "-L", pkg, "-lrouteb", "-lm", "-Wl,-rpath," + pkg], check=True, capture_output=True)
+        r = subprocess.run([exe, str(N), str(d), str(B), str(I), str(steps)], capture_output=True, text=True, timeout=300)
+        return json.loads(r.stdout.strip().splitlines()[-1])
+    except Exception as e:   # reported, never fatal for the bench line
+        return {"error": repr(e)[:200]}
 
 
 # ---- the C2 stream (pure input generation; no arithmetic of the method) -------------------------------------
@@ -221,19 +260,27 @@ def run_ours(args):
     rt = Router(bank["emb"], bank["quality"], bank["outlen"], cfg.k, store="bf16", max_batch=64, device=dev)
     rt.set_instances(**it)
     rt.set_state(queued, running)
+    rtp = Router(bank["emb"], bank["quality"], bank["outlen"], cfg.k, store="bf16", max_batch=64, pipeline=1, device=dev)
+    rtp.set_instances(**it)
+    rtp.set_state(queued, running)
     offs = np.concatenate([[0], np.cumsum(sizes)]).astype(np.int64)
     assign_dev = torch.empty(64, dtype=torch.int32, device=dev)
-    flush_buf = torch.ones(3 * L2_BYTES // 4, dtype=torch.float32, device=dev) if args.l2 == "flush" else None
+    assign_all = torch.empty(int(offs[-1]), dtype=torch.int32, device=dev)
+    flush_buf = torch.ones(3 * L2_BYTES // 4, dtype=torch.float32, device=dev)
 
     def flush():
-        if flush_buf is not None:
-            with torch.cuda.stream(rt.stream):
-                flush_buf.sum()          # read-only sweep of 3x L2: evicts the bank without leaving dirty lines
+        with torch.cuda.stream(rt.stream):
+            flush_buf.sum()          # read-only sweep of 3x L2: evicts the bank without leaving dirty lines
 
-    def step_device(j):
-        B = sizes[j]
-        rb.rb_advance_state(rt.ctx, elapsed[j])
-        rb.rb_decide(rt.ctx, allq[offs[j]:offs[j + 1]], allp[offs[j]:offs[j + 1]], B, weights[j], assign_dev[:B])
+    # the steps' device buffers are views prepared beforehand: slicing torch tensors is Python overhead, not the library's
+    qv = [allq[offs[j]:offs[j + 1]] for j in range(W + K)]
+    pv = [allp[offs[j]:offs[j + 1]] for j in range(W + K)]
+    av = [assign_all[offs[j]:offs[j + 1]] for j in range(W + K)]
+
+    def step_device(j, r=None, out=None):
+        r = rt if r is None else r
+        rb.rb_advance_state(r.ctx, elapsed[j])
+        rb.rb_decide(r.ctx, qv[j], pv[j], sizes[j], weights[j], assign_dev[:sizes[j]] if out is None else av[j])
 
     def barrier():
         torch.cuda.synchronize()
@@ -241,44 +288,62 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    # ---- leg 1: device-resident inputs, CUDA events per step on the library's stream ---------------------------
+    # ---- leg 1: device-resident inputs, K steps back to back in throughput mode, one event pair ----------------
     # untimed: one decision per distinct batch size, so that every CUDA graph the stream needs is captured
-    # and instantiated before the timed region (capture is a one-off host cost per batch size)
-    for B in sorted(set(sizes)):
-        rb.rb_decide(rt.ctx, allq[:B], allp[:B], B, weights[0], assign_dev[:B])
-    rt.sync()
-    rt.set_state(queued, running)
+    # and instantiated before the timed region (capture is a one-off host cost per batch size and buffer set)
+    for r in (rt, rtp):
+        for B in sorted(set(sizes)):
+            for _ in range(2):
+                rb.rb_decide(r.ctx, allq[:B], allp[:B], B, weights[0], assign_dev[:B])
+        r.sync()
+        r.set_state(queued, running)
     for j in range(W):
-        flush()
-        step_device(j)
+        step_device(j, rtp, assign_all)
     barrier()
-    ev0 = [torch.cuda.Event(enable_timing=True) for _ in range(K)]
-    ev1 = [torch.cuda.Event(enable_timing=True) for _ in range(K)]
-    launches0 = rt.launch_count()
+    ev_a, ev_b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    launches0 = rtp.launch_count()
     sampler = ClockSampler(dev.index or 0)
     with sampler:
         wall0 = time.perf_counter()
+        ev_a.record(rtp.stream)
         for j in range(K):
-            flush()
-            ev0[j].record(rt.stream)
-            step_device(W + j)
-            ev1[j].record(rt.stream)
+            step_device(W + j, rtp, assign_all)
+        ev_b.record(rtp.stream)
         barrier()
         wall = time.perf_counter() - wall0
+        launches = rtp.launch_count() - launches0
         if wall < 0.5:   # keep the GPU under the same load a little longer so that the sampler sees it
             t_end = time.perf_counter() + (0.5 - wall)
-            j = 0
             while time.perf_counter() < t_end:
-                flush()
-                rb.rb_estimate(rt.ctx, allq[:sizes[0]], sizes[0])
-                j += 1
-            torch.cuda.synchronize()
-    launches = rt.launch_count() - launches0
-    step_ms = np.array([a.elapsed_time(b) for a, b in zip(ev0, ev1)])
-    dev_seconds = float(step_ms.sum()) / 1e3
+                for j in range(W, W + min(K, 50)):
+                    step_device(j, rtp, assign_all)
+                rtp.sync()
+    dev_seconds = ev_a.elapsed_time(ev_b) / 1e3
     timed_req = int(sum(sizes[W:W + K]))
     t_max, units = reduce_over_ranks(dist, dev, dev_seconds, timed_req)
     value = units / t_max
+
+    # ---- leg 1b: latency of one decision: unpipelined context, L2 flushed, one event pair per decision, >= 300 of them
+    nlat = max(K, 300)
+    sz_l, el_l, w_l = c2_stream(cfg, nlat, seed_shift=rank + 7)
+    q_l = synth.make_queries(cfg, B=sum(sz_l), device=dev, stream=13 + 100 * rank)
+    p_l = synth.make_prompt_len(cfg, B=sum(sz_l), device=dev, stream=14 + 100 * rank)
+    off_l = np.concatenate([[0], np.cumsum(sz_l)]).astype(np.int64)
+    rt.set_state(queued, running)
+    ev0 = [torch.cuda.Event(enable_timing=True) for _ in range(nlat)]
+    ev1 = [torch.cuda.Event(enable_timing=True) for _ in range(nlat)]
+    for j in range(nlat + 5):
+        jj = max(0, j - 5)          # the first five repeat decision 0 untimed
+        flush()
+        if j >= 5:
+            ev0[jj].record(rt.stream)
+        rb.rb_advance_state(rt.ctx, el_l[jj])
+        rb.rb_decide(rt.ctx, q_l[off_l[jj]:off_l[jj + 1]], p_l[off_l[jj]:off_l[jj + 1]], sz_l[jj], w_l[jj], assign_dev[:sz_l[jj]])
+        if j >= 5:
+            ev1[jj].record(rt.stream)
+    barrier()
+    step_ms = np.array([a.elapsed_time(b) for a, b in zip(ev0, ev1)])
+    lat_req_per_s = float(sum(sz_l)) / (float(step_ms.sum()) / 1e3)
 
     # ---- leg 2: end to end through the C ABI with pinned host buffers ------------------------------------------
     q_host = allq[offs[W]:].cpu().pin_memory()
@@ -325,6 +390,7 @@ def run_ours(args):
             stage_sum[k_] = stage_sum.get(k_, 0.0) + v
     rt.set_stage_timing(0)
     hbm_peak, tf_peak, peak_src = measured_peaks()
+    read_peak = read_only_peak_gbs(rt, rb)
     mean_B = float(np.mean(sizes[W:W + nscan]))
     scan_bytes = cfg.N * cfg.d * 2 + mean_B * cfg.d * 2
     scan_mean_us = float(np.mean(scan_us))
@@ -333,6 +399,11 @@ def run_ours(args):
                 "unit": "GB/s", "frac": round(achieved / hbm_peak, 4), "traffic": recorded_traffic("c2"),
                 "bytes_per_launch": int(scan_bytes), "launch_us": round(scan_mean_us, 2), "peak_source": peak_src,
                 "frac_of_nominal_8TBs": round(achieved / 8000.0, 4),
+                "read_only_peak": {"GB/s": round(read_peak, 1), "frac": round(achieved / read_peak, 4),
+                                   "note": "a plain 16-byte-load streaming kernel over 2 GiB on this GPU: the ceiling of a read-only stream; the copy "
+                                           "bandwidth above (read + write) sits below it, so a read-dominated kernel can "
+                                           "show frac > 1 against the copy figure -- against this one it cannot"},
+                "frac_exceeds_1": bool(achieved / hbm_peak > 1.0),
                 "device_clock": {"launch_us": round(float(np.mean(scan_dev_us)), 2),
                                  "achieved": round(scan_bytes / (float(np.mean(scan_dev_us)) * 1e-6) / 1e9, 1),
                                  "frac": round(scan_bytes / (float(np.mean(scan_dev_us)) * 1e-6) / 1e9 / hbm_peak, 4),
@@ -343,35 +414,51 @@ def run_ours(args):
     out = {"metric": METRIC, "value": round(value, 1), "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
            "ms_per_step": round(t_max / K * 1e3, 5), "higher_is_better": True,
            "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
-           "config": {"workload": "C2 paper-shaped stream (BASELINE.json configs[1])", "N": cfg.N, "d": cfg.d, "M": cfg.M,
-                      "I": cfg.I, "k": cfg.k, "B": "4..64 (mean %.1f)" % (timed_req / K), "bank": "bf16 153.6 MB",
-                      "arrivals": "Poisson 12 req/s (first half of the steps) and 30 req/s (second half)",
-                      "weights": "quality/latency/cost/balanced presets in turn", "rerank_slack": 6,
-                      "l2": "flushed before every step (read of a 3x-L2 buffer)" if args.l2 == "flush" else
-                      "warm (bank 153.6 MB vs 126 MB L2)", "graph": "CUDA graph replay per B",
-                      "parallelism": "replicas only" if world > 1 else "single GPU"},
+           "config": c2_config(cfg, world),
+           "timed_region": {"mode": "throughput (rb_options.pipeline): the K decisions back to back, one CUDA-event pair",
+                            "mean_B": round(timed_req / K, 2), "us_per_decision": round(t_max / K * 1e6, 2)},
            "decision_us": {"mean": round(float(step_ms.mean()) * 1e3, 2), "p50": round(float(np.median(step_ms)) * 1e3, 2),
                            "p99": round(float(np.percentile(step_ms, 99)) * 1e3, 2),
-                           "max": round(float(step_ms.max()) * 1e3, 2)},
+                           "max": round(float(step_ms.max()) * 1e3, 2), "decisions": int(nlat),
+                           "mode": "one decision at a time, unpipelined context, L2 flushed before each",
+                           "unpipelined_flushed_requests_per_s": round(lat_req_per_s, 1)},
            "e2e": {"value": round(units / e2e_max, 1), "unit": UNIT, "h2d_bytes_per_step": round(h2d, 1),
                    "d2h_bytes_per_step": round(d2h, 1), "us_per_decision": round(e2e_max / K * 1e6, 2)},
            "gpu_launches": int(launches), "clocks": sampler.summary(), "roofline": roofline,
            "paper_context": "paper: ~32 ms per decision at 12 req/s on its 96-core CPU host, encoder included (P:L7)"}
 
+    rtp.close()
     if rank == 0 and world == 1:
         if not args.skip_cpu:
             out["cpu_baseline"], out["parity"] = cpu_baseline_and_parity(args, cfg, bank, it, queued, running, rt, rb,
                                                                          synth)
+        out["adaptive_stream"] = adaptive_stream_leg(cfg, bank, it, queued, running, synth, Router, dev)
+        per_config = {}
+        if not args.skip_cpu:
+            orc_bank = (bank_to_numpy(bank["emb"]), bank["quality"].cpu().numpy(), bank["outlen"].cpu().numpy())
+            per_config["C2 B=64 (largest window)"] = decision_stats(rt, rb, synth, cfg, 64, dev, it=it, flush_buf=flush_buf,
+                                                                    orc_bank=orc_bank, oracle_queries=4)
+            per_config["C2 B=12 (mean window)"] = decision_stats(rt, rb, synth, cfg, 12, dev, it=it, flush_buf=flush_buf,
+                                                                 orc_bank=orc_bank, oracle_queries=4)
+            del orc_bank
         rt.close()
         del bank, rt, flush_buf
         torch.cuda.empty_cache()
+        out["e2e"]["c_harness"] = c_harness_e2e(cfg.N, cfg.d, 12, cfg.I)
+        torch.cuda.empty_cache()
+        if not args.skip_cpu:
+            per_config.update(small_configs(synth, Router, rb, dev))
         if not args.no_scan_c4:
             out["scan_c4"] = scan_c4(synth, Router, dev, hbm_peak)
         if not args.no_large:
             out["p0_paper_shape"] = paper_shape_p0(synth, Router, dev)
-            out["sweep_c4"] = sweep_c4(synth, Router, dev, hbm_peak)
-            out["scan_c3"] = scan_c3(synth, Router, dev)
-            out["sweep_c5"] = sweep_c5(synth, Router, dev)
+            out["sweep_c4"] = sweep_c4(synth, Router, dev, hbm_peak, rb=rb, with_oracle=not args.skip_cpu)
+            out["scan_c3"] = scan_c3(synth, Router, dev, rb=rb, with_oracle=not args.skip_cpu)
+            out["sweep_c5"] = sweep_c5(synth, Router, dev, rb=rb, with_oracle=not args.skip_cpu)
+            for key, leg in (("C4 N=10M", "sweep_c4"), ("C3", "scan_c3"), ("C5", "sweep_c5")):
+                for name, d_ in out[leg].pop("decisions", {}).items():
+                    per_config["%s %s" % (key, name)] = d_
+        out["per_config"] = per_config
     else:
         rt.close()
     if dist is not None:
@@ -440,6 +527,125 @@ def cpu_baseline_and_parity(args, cfg, bank, it, queued, running, rt, rb, synth)
     return cpu, par
 
 
+def adaptive_stream_leg(cfg, bank, it, queued, running, synth, Router, dev, n_req=6000):
+    """the C2 stream with windows formed by the adaptive batch-size rule (rb_batch_target) through the
+    stream driver (stream.py), beside the fixed batch sizes of the paper's ablation: decisions per second of the
+    driver loop (wall clock; the rule's read-back synchronises once per window) and the batch wait it gives."""
+    import torch
+    from paper_2606_17949_b200 import stream
+    rows = []
+    q = synth.make_queries(cfg, B=n_req, device=dev, stream=23)
+    p = synth.make_prompt_len(cfg, B=n_req, device=dev, stream=24)
+    presets = list(synth.PRESETS.values())
+    rt = Router(bank["emb"], bank["quality"], bank["outlen"], cfg.k, store="bf16", max_batch=64, device=dev)
+    rt.set_instances(**it)
+    for rate in (12.0, 30.0):
+        arrivals = synth.poisson_arrivals_ms(rate, n_req, seed=cfg.seed)
+        for name, lo, hi in (("adaptive 4..64", 4, 64), ("fixed 16", 16, 16), ("fixed 32", 32, 32)):
+            rt.set_state(queued, running)
+            be = stream.RouterBackend(rt, q, p)
+            stream.drive(be, arrivals[:400], lambda j: presets[j % 4], bs_min=lo, bs_max=hi, max_wait_ms=500.0)   # graphs
+            rt.set_state(queued, running)
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            res = stream.drive(be, arrivals, lambda j: presets[j % 4], bs_min=lo, bs_max=hi, max_wait_ms=500.0)
+            rt.sync()
+            wall = time.perf_counter() - t0
+            wait = res.batch_wait_ms(arrivals)
+            rows.append({"arrivals_per_s": rate, "rule": name, "windows": len(res.lo), "mean_B": round(n_req / len(res.lo), 2),
+                         "mean_target": round(float(np.mean(res.target)), 2), "mean_busy": round(float(np.mean(res.n_busy)), 2),
+                         "driver_decisions_per_s": round(len(res.lo) / wall, 1), "driver_requests_per_s": round(n_req / wall, 1),
+                         "batch_wait_ms_mean": round(float(wait.mean()), 2), "batch_wait_ms_p99": round(float(np.percentile(wait, 99)), 2)})
+    rt.close()
+    return {"workload": "C2 bank, %d Poisson requests per cell, max wait 500 ms" % n_req, "rows": rows,
+            "paper_context": "paper Table 4: batch wait 48-101 ms at 6-30 req/s with its ~30 ms decisions (P:L195-201); "
+                             "adaptive-off costs 0.4-6.0 % E2E (P:L266)"}
+
+
+def decision_stats(rt, rb, synth, cfg, B, dev, it=None, n=200, flush_buf=None, orc_bank=None, oracle_queries=2):
+    """One config's decision figures: median / p99 device time of rb_advance_state + rb_decide over n decisions
+    (a CUDA-event pair around each, graph replay; L2 flushed before each when flush_buf is given -- banks larger than L2
+    need none), requests per second at the median, per-kernel time (stage-timing mode, 10 decisions), and the oracle's time
+    for the same decision on the host cores (brute-force KNN of `oracle_queries` of the B queries, extrapolated to B and
+    labelled so, plus the full aggregate + score + dispatch)."""
+    import torch
+    if it is None:
+        it = synth.make_instances(cfg.I, cfg.M)
+    queued, running = synth.make_state(cfg.I, it["cap"], cfg.seed)
+    rt.set_instances(**it)
+    rt.set_state(queued, running)
+    q = synth.make_queries(cfg, B=B, device=dev)
+    p = synth.make_prompt_len(cfg, B=B, device=dev)
+    a = torch.empty(B, dtype=torch.int32, device=dev)
+    pq = torch.empty(B, cfg.M, dtype=torch.float32, device=dev)
+    pl = torch.empty(B, cfg.M, dtype=torch.float32, device=dev)
+    w = synth.PRESETS["balanced"]
+    torch.cuda.synchronize()
+    for _ in range(5):
+        rb.rb_advance_state(rt.ctx, 20.0)
+        rb.rb_decide(rt.ctx, q, p, B, w, a, None, pq, pl)
+    rt.sync()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(n)]
+    for e0, e1 in ev:
+        if flush_buf is not None:
+            with torch.cuda.stream(rt.stream):
+                flush_buf.sum()
+        e0.record(rt.stream)
+        rb.rb_advance_state(rt.ctx, 20.0)
+        rb.rb_decide(rt.ctx, q, p, B, w, a, None, pq, pl)
+        e1.record(rt.stream)
+    rt.sync()
+    us = np.array([e0.elapsed_time(e1) * 1e3 for e0, e1 in ev])
+    rt.set_stage_timing(1)
+    st = {}
+    for _ in range(10):
+        rb.rb_advance_state(rt.ctx, 20.0)
+        rb.rb_decide(rt.ctx, q, p, B, w, a, None, pq, pl)
+        for k_, v in rt.stage_us().items():
+            st[k_] = st.get(k_, 0.0) + v / 10
+    rt.set_stage_timing(0)
+    out = {"B": B, "decisions": n, "decision_us_p50": round(float(np.median(us)), 1), "decision_us_p99": round(float(np.percentile(us, 99)), 1),
+           "requests_per_s": round(B / (float(np.median(us)) * 1e-6), 1),
+           "kernel_us": {"stage": round(st.get("stage", 0.0), 1), "scan": round(st.get("scan", 0.0), 1),
+                         "finish": round(st.get("aggregate", 0.0), 1), "dispatch": round(st.get("dispatch", 0.0), 1),
+                         "note": "CUDA events between the kernels (stage-timing graph): each interval also holds a launch "
+                                 "latency, their sum exceeds a decision"},
+           "l2": "flushed before every decision" if flush_buf is not None else "not flushed"}
+    if orc_bank is not None:
+        from oracle import orc
+        bank_np, qn, ln = orc_bank
+        nq = min(B, oracle_queries)
+        qh, ph = q.cpu().numpy(), p.cpu().numpy()
+        t0 = time.perf_counter()
+        orc.knn(bank_np, qh[:nq], cfg.k, store_dtype="bf16" if bank_np.dtype == np.uint16 else "f32")
+        t_knn = (time.perf_counter() - t0) / nq
+        inst = orc.Instances(**it)
+        t0 = time.perf_counter()
+        orc.decide_from_predictions(inst, queued.numpy(), running.numpy(), pq.cpu().numpy(), pl.cpu().numpy(), ph, w)
+        t_rest = time.perf_counter() - t0
+        out["oracle_ms_per_decision"] = round((t_knn * B + t_rest) * 1e3, 2)
+        out["oracle_note"] = "brute-force KNN timed on %d of the %d queries and extrapolated (%.1f ms per query on %d " \
+                             "threads) + score/dispatch of the whole batch (%.2f ms)" % (nq, B, t_knn * 1e3, orc.num_threads(), t_rest * 1e3)
+    return out
+
+
+def small_configs(synth, Router, rb, dev):
+    """C1 (BASELINE.json configs[0], fp32 bank and the same bank in bf16 storage) and P0 (the paper's own shape): whole
+    decisions, L2-resident banks, with the oracle's full time (no extrapolation)."""
+    import dataclasses
+    out = {}
+    for name, cfg, store, B in (("C1 Tiny fp32 storage", synth.CONFIGS["C1"], "f32", 16), ("C1 Tiny bf16 storage", synth.CONFIGS["C1"], "bf16", 16),
+                                ("P0 paper shape bf16 storage", synth.CONFIGS["P0"], "bf16", 16)):
+        c = dataclasses.replace(cfg, store=store)
+        bank = synth.make_bank(c, device=dev)
+        it = synth.paper_cluster() if name.startswith("P0") else None
+        rt = Router(bank["emb"], bank["quality"], bank["outlen"], c.k, store=store, max_batch=32, device=dev)
+        orc_bank = (bank_to_numpy(bank["emb"]), bank["quality"].cpu().numpy(), bank["outlen"].cpu().numpy())
+        out[name] = decision_stats(rt, rb, synth, c, B, dev, it=it, orc_bank=orc_bank, oracle_queries=B)
+        rt.close()
+    return out
+
+
 def scan_c4(synth, Router, dev, hbm_peak, B=64):
     """BASELINE.json configs[3]: N=10M x d=384 bf16 bank (7.68 GB >> L2), B=64 (or --c4-batch), k=10: the scan kernel alone."""
     import torch
@@ -468,7 +674,7 @@ def scan_c4(synth, Router, dev, hbm_peak, B=64):
             "device_clock_launch_us": round(float(np.mean(dus)), 1), "traffic": recorded_traffic("c4"), "l2": "bank 7.68 GB >> 126 MB L2"}
 
 
-def sweep_c4(synth, Router, dev, hbm_peak):
+def sweep_c4(synth, Router, dev, hbm_peak, rb=None, with_oracle=False):
     """BASELINE.json configs[3], the whole sweep: N=10M x d=384 bf16 (7.68 GB), B in {1, 8, 64, 512, 4096} x k in {10, 32}:
     the scan kernel alone (CUDA events around it, stage timing mode), as GB/s against the HBM roofline and TFLOP/s
     against the tensor roofline; whichever fraction is larger names the bound of that point."""
@@ -477,7 +683,7 @@ def sweep_c4(synth, Router, dev, hbm_peak):
     burst, sustained, _ = measured_tensor_peaks()
     base = synth.CONFIGS["C4"]
     bank = synth.make_bank(base, device=dev)
-    rows = []
+    rows, decisions = [], {}
     for k, slack in ((10, 6), (32, 8)):
         cfg = dataclasses.replace(base, k=k)
         rt = Router(bank["emb"], bank["quality"], bank["outlen"], k, store="bf16", rerank_slack=slack, max_batch=4096, device=dev)
@@ -502,9 +708,14 @@ def sweep_c4(synth, Router, dev, hbm_peak):
             rows.append({"B": B, "k": k, "scan_us": round(t, 1), "finish_us": round(float(np.mean(fin)), 1),
                          "GB/s": round(gbs, 1), "frac_hbm": round(fh, 4), "TFLOP/s": round(tfs, 1), "frac_tensor": round(ft, 4),
                          "bound": "hbm" if fh >= ft else "tensor", "queries/s": round(B / ((t + float(np.mean(fin))) * 1e-6), 1)})
+        if k == 10 and rb is not None:   # whole decisions at both ends of the sweep (I = 64 instances)
+            orc_bank = (bank_to_numpy(bank["emb"]), bank["quality"].cpu().numpy(), bank["outlen"].cpu().numpy()) if with_oracle else None
+            decisions["B=64 k=10"] = decision_stats(rt, rb, synth, cfg, 64, dev, n=200, orc_bank=orc_bank, oracle_queries=1)
+            decisions["B=4096 k=10"] = decision_stats(rt, rb, synth, cfg, 4096, dev, n=40, orc_bank=orc_bank, oracle_queries=1)
+            del orc_bank
         rt.close()
     return {"workload": "C4 N=10M d=384 bf16 (7.68 GB >> L2), scan kernel alone", "hbm_peak_GB/s": hbm_peak,
-            "tensor_peak_TFLOP/s": burst, "rows": rows}
+            "tensor_peak_TFLOP/s": burst, "rows": rows, "decisions": decisions}
 
 
 def paper_shape_p0(synth, Router, dev):
@@ -557,7 +768,7 @@ def measured_tensor_peaks():
     return 1590.0, 1590.0, "fallback (B200_PROFILING.md)"
 
 
-def scan_c3(synth, Router, dev):
+def scan_c3(synth, Router, dev, rb=None, with_oracle=False):
     """BASELINE.json configs[2]: N=1M x d=1024 bf16 bank (2.05 GB), B=1024, k=10: the CTA-pair scan kernel alone
     against the tensor roofline (2*B*N*d flop per launch, true B)."""
     import torch
@@ -576,6 +787,12 @@ def scan_c3(synth, Router, dev):
         st = rt.stage_us()
         us.append(st["scan"])
         fin.append(st["aggregate"])
+    rt.set_stage_timing(0)
+    decisions = {}
+    if rb is not None:
+        orc_bank = (bank_to_numpy(bank["emb"]), bank["quality"].cpu().numpy(), bank["outlen"].cpu().numpy()) if with_oracle else None
+        decisions["B=1024 I=256"] = decision_stats(rt, rb, synth, cfg, cfg.B, dev, n=200, orc_bank=orc_bank, oracle_queries=2)
+        del orc_bank
     rt.close()
     t = float(np.mean(us))
     flop = 2.0 * cfg.B * cfg.N * cfg.d
@@ -585,10 +802,10 @@ def scan_c3(synth, Router, dev):
             "bound": "tensor", "launch_us": round(t, 1), "flop_per_launch": flop, "achieved": round(ach, 1),
             "unit": "TFLOP/s", "peak": burst, "frac": round(ach / burst, 4), "peak_sustained": sustained,
             "frac_of_sustained": round(ach / sustained, 4), "peak_source": src,
-            "finish_us": round(float(np.mean(fin)), 1), "traffic": recorded_traffic("c3")}
+            "finish_us": round(float(np.mean(fin)), 1), "traffic": recorded_traffic("c3"), "decisions": decisions}
 
 
-def sweep_c5(synth, Router, dev):
+def sweep_c5(synth, Router, dev, rb=None, with_oracle=False):
     """BASELINE.json configs[4]: one KNN + aggregate for B=1024 requests (N=1M x d=768), then all 66 points of
     the 3-simplex at step 0.1 through rb_decide_from_predictions(commit=0) from the same dead-reckoned state:
     score + LPT dispatch timed in isolation (CUDA events on the library's stream, one pair per point)."""
@@ -687,6 +904,11 @@ def sweep_c5(synth, Router, dev):
               "note": "replicas of a tier with equal state tie exactly in scores0, so instance-level changes are mostly "
                       "arbitrary picks among equals; model_changed_frac counts requests whose tier (model) differs",
               "paper_context": "paper's replay: 15.6 % of assignments differ, realised quality -0.002 (P:L80)"}
+    decisions = {}
+    if rb is not None:
+        orc_bank = (bank_to_numpy(bank["emb"]), bank["quality"].cpu().numpy(), bank["outlen"].cpu().numpy()) if with_oracle else None
+        decisions["B=1024 I=256"] = decision_stats(rt, rb, synth, cfg, cfg.B, dev, it=it, n=200, orc_bank=orc_bank, oracle_queries=2)
+        del orc_bank
     rt.close()
     # the same sweep with the gradient-boosted TPOT head (latency_mode 2; synthetic forest: 64 trees of depth 5 per
     # tier, 2 auxiliary telemetry features) -- the paper's head is a per-tier XGBoost booster
@@ -719,7 +941,7 @@ def sweep_c5(synth, Router, dev):
             "boosted_head": {"forest": "64 trees x depth 5 per tier, 4 features, synthetic", "score_dispatch_us_mean":
                              round(float(us2.mean()), 1), "us_per_request_step": round(float(us2.mean()) / cfg.B, 4)},
             "matching_replay": replay,
-            "tier_share_at_corners(qual,lat,cost)": corners,
+            "tier_share_at_corners(qual,lat,cost)": corners, "decisions": decisions,
             "paper_context": "paper scoring loop: 12.8/14.3/22.5 us at |I|=13/100/500 per request on CPU (P:L119)"}
 
 
@@ -773,8 +995,7 @@ def run_reference(args):
     out = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
            "ms_per_step": round(t / K * 1e3, 3), "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
            "dtype": "f64 accumulate / f32", "data": "synthetic",
-           "config": {"workload": "C2 paper-shaped stream (BASELINE.json configs[1])", "N": cfg.N, "d": cfg.d, "M": cfg.M,
-                      "I": cfg.I, "k": cfg.k, "B": "<=%d per step (bounded sample)" % q_per_step},
+           "config": c2_config(cfg, world),
            "cpu_baseline": {"value": v, "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle", "sample": sample},
            "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
            "gpu_launches": 0}

@@ -31,6 +31,11 @@ rb_status rb_last_scan_device_us(rb_ctx* ctx, float* us);
  * IEEE division bit for bit on n_pairs pseudo-random in-window operand pairs.  *mismatches [host] must come back 0. */
 rb_status rb_selftest_division(rb_ctx* ctx, uint64_t n_pairs, uint64_t seed, uint64_t* mismatches);
 
+/* Read-only streaming bandwidth of the device (bench.py's ceiling for read-dominated kernels): a kernel of coalesced
+ * 16-byte loads over a scratch buffer of `bytes` bytes (allocated and freed by the call), timed with CUDA events, best of
+ * `repeats` launches.  *gb_per_s [host].  RB_ENOMEM if the buffer cannot be allocated. */
+rb_status rb_testing_read_bandwidth(rb_ctx* ctx, uint64_t bytes, int32_t repeats, double* gb_per_s);
+
 #ifdef __cplusplus
 }
 #endif

@@ -26,7 +26,7 @@ RB_OK, RB_EINVAL, RB_ECUDA, RB_ENOMEM, RB_ESTATE, RB_EUNSUPPORTED = range(6)
 RB_F32, RB_BF16 = 0, 1
 _STATUS = {0: "RB_OK", 1: "RB_EINVAL", 2: "RB_ECUDA", 3: "RB_ENOMEM", 4: "RB_ESTATE", 5: "RB_EUNSUPPORTED"}
 EXPORTS = ["rb_options_default", "rb_create", "rb_set_instances", "rb_set_tpot_forest", "rb_set_telemetry", "rb_set_state", "rb_get_state", "rb_advance_state",
-           "rb_batch_target", "rb_decide", "rb_decide_budgeted", "rb_decide_from_predictions", "rb_decide_from_predictions_budgeted", "rb_sweep_weights", "rb_estimate", "rb_dispatch_pipeline", "rb_match_replay", "rb_set_stage_timing", "rb_last_stage_us", "rb_last_scan_device_us", "rb_selftest_division",
+           "rb_batch_target", "rb_decide", "rb_decide_budgeted", "rb_decide_from_predictions", "rb_decide_from_predictions_budgeted", "rb_sweep_weights", "rb_estimate", "rb_dispatch_pipeline", "rb_match_replay", "rb_set_stage_timing", "rb_last_stage_us", "rb_last_scan_device_us", "rb_selftest_division", "rb_testing_read_bandwidth",
            "rb_launch_count", "rb_sync", "rb_last_error", "rb_destroy"]
 
 
@@ -77,6 +77,7 @@ _lib.rb_set_stage_timing.argtypes = [_vp, _i32]
 _lib.rb_last_stage_us.argtypes = [_vp, ctypes.POINTER(_f * 6)]
 _lib.rb_last_scan_device_us.argtypes = [_vp, ctypes.POINTER(_f)]
 _lib.rb_selftest_division.argtypes = [_vp, ctypes.c_uint64, ctypes.c_uint64, ctypes.POINTER(ctypes.c_uint64)]
+_lib.rb_testing_read_bandwidth.argtypes = [_vp, ctypes.c_uint64, _i32, ctypes.POINTER(ctypes.c_double)]
 _lib.rb_launch_count.argtypes = [_vp]
 _lib.rb_launch_count.restype = _i64
 _lib.rb_sync.argtypes = [_vp]
@@ -280,6 +281,13 @@ def rb_selftest_division(ctx, n_pairs, seed=0):
     bad = ctypes.c_uint64(0)
     _check(ctx, _lib.rb_selftest_division(ctx, int(n_pairs), int(seed), ctypes.byref(bad)))
     return int(bad.value)
+
+
+def rb_testing_read_bandwidth(ctx, nbytes, repeats=10):
+    """GB/s of a plain streaming-read kernel over nbytes of scratch (routebalance_testing.h)."""
+    out = ctypes.c_double(0.0)
+    _check(ctx, _lib.rb_testing_read_bandwidth(ctx, int(nbytes), int(repeats), ctypes.byref(out)))
+    return float(out.value)
 
 
 def rb_launch_count(ctx):

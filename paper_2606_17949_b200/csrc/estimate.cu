@@ -36,6 +36,24 @@ __global__ void stage_queries_kernel(const __grid_constant__ CallParams cpv, __n
     qs[i] = (r < (size_t)B) ? __float2bfloat16_rn(q[r * d + c]) : __float2bfloat16_rn(0.0f);
   }
 }
+// Plain streaming read (rb_testing_read_bandwidth): every thread sums 16-byte loads, 8 in flight; one word written per block.
+__global__ void __launch_bounds__(256) read_stream_kernel(const uint4* __restrict__ in, size_t nvec, uint32_t* __restrict__ sink) {
+  uint32_t acc = 0u;
+  const size_t stride = (size_t)gridDim.x * blockDim.x;
+  size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  for (; i + 7 * stride < nvec; i += 8 * stride) {
+    uint4 v[8];
+#pragma unroll
+    for (int u = 0; u < 8; ++u) v[u] = __ldcs(in + i + u * stride);
+#pragma unroll
+    for (int u = 0; u < 8; ++u) acc += v[u].x ^ v[u].y ^ v[u].z ^ v[u].w;
+  }
+  for (; i < nvec; i += stride) {
+    const uint4 v = __ldcs(in + i);
+    acc += v.x ^ v.y ^ v.z ^ v.w;
+  }
+  if (acc == 0x9e3779b9u) sink[blockIdx.x] = acc;   // (never true for a zeroed buffer: keeps the loads alive)
+}
 __global__ void convert_bf16_kernel(const float* __restrict__ in, __nv_bfloat16* __restrict__ out, size_t n) {
   for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x)
     out[i] = __float2bfloat16_rn(in[i]);
@@ -143,6 +161,11 @@ cudaError_t launch_convert_bf16(const float* in, __nv_bfloat16* out, size_t n, c
   size_t blocks = (n + 255) / 256;
   if (blocks > 148 * 16) blocks = 148 * 16;
   convert_bf16_kernel<<<(int)blocks, 256, 0, s>>>(in, out, n);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_read_stream(const void* buf, size_t bytes, uint32_t* sink, cudaStream_t s) {
+  read_stream_kernel<<<148 * 8, 256, 0, s>>>(reinterpret_cast<const uint4*>(buf), bytes / 16, sink);
   return cudaGetLastError();
 }
 

@@ -1322,6 +1322,34 @@ rb_status rb_selftest_division(rb_ctx* ctx, uint64_t n_pairs, uint64_t seed, uin
   return RB_OK;
 }
 
+rb_status rb_testing_read_bandwidth(rb_ctx* ctx, uint64_t bytes, int32_t repeats, double* gb_per_s) {
+  if (!ctx || !gb_per_s || bytes < (1u << 20) || repeats < 1) return RB_EINVAL;
+  uint8_t* buf = nullptr;
+  uint32_t* sink = nullptr;
+  if (cudaMalloc((void**)&buf, bytes) != cudaSuccess || cudaMalloc((void**)&sink, 148 * 8 * 4) != cudaSuccess) {
+    cudaGetLastError();
+    cudaFree(buf);
+    return fail(ctx, RB_ENOMEM, "cudaMalloc (read bandwidth scratch)");
+  }
+  cudaStream_t s = ctx->stream;
+  cudaError_t e = cudaMemsetAsync(buf, 0, bytes, s);
+  float best = 1e30f;
+  for (int r = 0; r < repeats + 2 && e == cudaSuccess; ++r) {   // two untimed launches first
+    if ((e = cudaEventRecord(ctx->ev[0], s)) != cudaSuccess) break;
+    if ((e = launch_read_stream(buf, bytes, sink, s)) != cudaSuccess) break;
+    if ((e = cudaEventRecord(ctx->ev[1], s)) != cudaSuccess) break;
+    if ((e = cudaStreamSynchronize(s)) != cudaSuccess) break;
+    float ms = 0.0f;
+    if ((e = cudaEventElapsedTime(&ms, ctx->ev[0], ctx->ev[1])) != cudaSuccess) break;
+    if (r >= 2 && ms < best) best = ms;
+  }
+  cudaFree(buf);
+  cudaFree(sink);
+  if (e != cudaSuccess) return fail(ctx, RB_ECUDA, "rb_testing_read_bandwidth", e);
+  *gb_per_s = (double)bytes / (best * 1e-3) / 1e9;
+  return RB_OK;
+}
+
 int64_t rb_launch_count(const rb_ctx* ctx) { return ctx ? ctx->launches : 0; }
 
 rb_status rb_sync(rb_ctx* ctx) {

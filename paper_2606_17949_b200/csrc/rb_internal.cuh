@@ -213,6 +213,8 @@ cudaError_t launch_chained(void (*kernel)(KArgs...), dim3 grid, dim3 block, size
 #endif
 
 // ---- launchers (each returns the cudaError of its launch) ---------------------------------------------
+// plain streaming read of `bytes` bytes (rb_testing_read_bandwidth); sink: 148 * 8 words
+cudaError_t launch_read_stream(const void* buf, size_t bytes, uint32_t* sink, cudaStream_t s);
 // fp32 -> bf16 (RNE), n elements (bank conversion in rb_create).
 cudaError_t launch_convert_bf16(const float* in, __nv_bfloat16* out, size_t n, cudaStream_t s);
 
