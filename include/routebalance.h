@@ -69,11 +69,15 @@ typedef struct {
   int32_t store_dtype;    /* rb_dtype the bank is stored and searched in.                 default RB_BF16 */
                           /* RB_BF16: bank and queries are rounded to bf16 (RNE) once; similarity is the   */
                           /* dot product of the rounded values (tcgen05 tensor-core scan).                 */
-                          /* RB_F32: fp32 bank, exact fp64-accumulated scan; meant for small banks.        */
+                          /* RB_F32: the similarity is the dot product of the fp32 values.  The bank is also kept  */
+                          /* as a three-plane bf16 split (x = hi + mid + lo) that the same tensor-core scan reads   */
+                          /* (candidates good to ~5e-6); the k + slack candidates are then re-ranked exactly from   */
+                          /* the fp32 rows.  14 bytes per value: meant for small banks.                            */
   int32_t weight_mode;    /* 0: inverse distance 1/(dist+eps) ("distance-weighted"); 1: uniform     */
   float dist_eps;         /* eps above.                                                   default 1e-6    */
-  int32_t rerank_slack;   /* RB_BF16 only: the scan keeps k+slack candidates per query, their similarities */
-                          /* are recomputed exactly (fp64 accumulate) and the best k kept. default 6       */
+  int32_t rerank_slack;   /* the scan keeps k+slack candidates per query, their similarities are recomputed       */
+                          /* exactly (fp64 accumulate) and the best k kept.                default 6       */
+                          /* RB_F32 always re-ranks: 0 is read as min(6, 64 - k).                          */
                           /* 0: no re-rank; similarities are the tensor core's fp32 sums (within 4e-6), and  */
                           /* inverse-distance weights amplify that as a neighbour's similarity nears 1.      */
   int32_t lpt_enabled;    /* 1: dispatch in LPT order; 0: in input order.         default 1       */

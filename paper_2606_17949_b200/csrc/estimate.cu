@@ -23,8 +23,21 @@ __device__ __forceinline__ unsigned long long make_key(float sim, int32_t idx) {
 }
 
 // ---- a0 ---------------------------------------------------------------------------------------------
+// fp32 -> three bf16 planes: hi = bf16(x), mid = bf16(x - hi), lo = bf16(x - hi - mid) (both differences are exact in
+// fp32), so that x = hi + mid + lo up to 2^-27 |x|.
+__device__ __forceinline__ void split3(float x, __nv_bfloat16* hi, __nv_bfloat16* mid, __nv_bfloat16* lo) {
+  *hi = __float2bfloat16_rn(x);
+  const float r1 = __fsub_rn(x, __bfloat162float(*hi));
+  *mid = __float2bfloat16_rn(r1);
+  *lo = __float2bfloat16_rn(__fsub_rn(r1, __bfloat162float(*mid)));
+}
+
+// split = 0: qs[row, c] = bf16(q[r, c]).  split = 1 (fp32 storage): rows of 5 d columns [hi | hi | mid | hi | lo], the
+// query's side of the split scan (bank rows hold [hi | mid | hi | lo | hi]): the scan's dot product is then
+// x_hi e_hi + x_hi e_mid + x_mid e_hi + x_hi e_lo + x_lo e_hi, the fp32 dot product up to 2^-18 sum |x_c e_c|.
 __global__ void stage_queries_kernel(const __grid_constant__ CallParams cpv, __nv_bfloat16* __restrict__ qs, int B, int Bpad,
-                                     int d, int group, uint32_t* __restrict__ gthr, int n_gthr) {
+                                     int d, int group, uint32_t* __restrict__ gthr, int n_gthr, int split,
+                                     float* __restrict__ q32) {
   const CallParams* __restrict__ cp = &cpv;   // the per-call parameters travel as a kernel argument (constant bank)
   launch_dependents();
   for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n_gthr; i += gridDim.x * blockDim.x) gthr[i] = 0u;
@@ -33,7 +46,27 @@ __global__ void stage_queries_kernel(const __grid_constant__ CallParams cpv, __n
   for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
     const size_t row = i / d, c = i - row * d;
     const size_t r = row % group;   // replicas of query r at rows r, group + r, ...
-    qs[i] = (r < (size_t)B) ? __float2bfloat16_rn(q[r * d + c]) : __float2bfloat16_rn(0.0f);
+    const float x = (r < (size_t)B) ? q[r * d + c] : 0.0f;
+    if (!split) {
+      qs[i] = __float2bfloat16_rn(x);
+    } else {
+      __nv_bfloat16 hi, mid, lo;
+      split3(x, &hi, &mid, &lo);
+      __nv_bfloat16* o = qs + row * 5 * (size_t)d + c;
+      o[0] = hi; o[d] = hi; o[2 * (size_t)d] = mid; o[3 * (size_t)d] = hi; o[4 * (size_t)d] = lo;
+      if (row < (size_t)B) q32[i] = x;   // device copy of the fp32 rows for the exact re-rank (the caller's may be host memory)
+    }
+  }
+}
+// fp32 bank [n x d] -> split bank [n x 5 d] bf16: [hi | mid | hi | lo | hi] (rb_create, fp32 storage)
+__global__ void split_bank_kernel(const float* __restrict__ in, __nv_bfloat16* __restrict__ out, size_t rows, int d) {
+  const size_t n = rows * d;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+    const size_t row = i / d, c = i - row * d;
+    __nv_bfloat16 hi, mid, lo;
+    split3(in[i], &hi, &mid, &lo);
+    __nv_bfloat16* o = out + row * 5 * (size_t)d + c;
+    o[0] = hi; o[d] = mid; o[2 * (size_t)d] = hi; o[3 * (size_t)d] = lo; o[4 * (size_t)d] = hi;
   }
 }
 // Plain streaming read (rb_testing_read_bandwidth): every thread sums 16-byte loads, 8 in flight; one word written per block.
@@ -57,92 +90,6 @@ __global__ void __launch_bounds__(256) read_stream_kernel(const uint4* __restric
 __global__ void convert_bf16_kernel(const float* __restrict__ in, __nv_bfloat16* __restrict__ out, size_t n) {
   for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x)
     out[i] = __float2bfloat16_rn(in[i]);
-}
-
-// ---- a1, fp32 storage -----------------------------------------------------------------------------------
-// s[r,n] = fl32( sum_c (double)x[r,c] * (double)e[n,c] ) in index order: the product of two fp32 values is
-// exact in fp64, so one fp64 FMA per term is exactly "multiply, then add with one rounding".
-constexpr int kF32Rows = 128;   // bank rows per block, one per thread
-constexpr int kF32Q = 8;        // queries per register group
-constexpr int kF32Chunk = 64;   // columns staged per step
-__global__ void __launch_bounds__(kF32Rows)
-scan_f32_kernel(const float* __restrict__ bank, const __grid_constant__ CallParams cpv, int r0, int64_t N, int d, int nq,
-                float* __restrict__ sims) {
-  __shared__ float xs[kF32Q][kF32Chunk];
-  const CallParams* __restrict__ cp = &cpv;
-  const float* __restrict__ q = cp->query + (size_t)r0 * d;
-  const int64_t n = (int64_t)blockIdx.x * kF32Rows + threadIdx.x;
-  const float* row = bank + (n < N ? n : N - 1) * (int64_t)d;
-  for (int q0 = 0; q0 < nq; q0 += kF32Q) {
-    double acc[kF32Q];
-#pragma unroll
-    for (int j = 0; j < kF32Q; ++j) acc[j] = 0.0;
-    for (int c0 = 0; c0 < d; c0 += kF32Chunk) {
-      __syncthreads();
-      for (int t = threadIdx.x; t < kF32Q * kF32Chunk; t += kF32Rows) {
-        const int j = t / kF32Chunk, c = t % kF32Chunk;
-        xs[j][c] = (q0 + j < nq && c0 + c < d) ? q[(size_t)(q0 + j) * d + c0 + c] : 0.0f;
-      }
-      __syncthreads();
-      const int cn = min(kF32Chunk, d - c0);
-      for (int c = 0; c < cn; c += 4) {
-        const float4 e = *reinterpret_cast<const float4*>(row + c0 + c);
-#pragma unroll
-        for (int j = 0; j < kF32Q; ++j) {
-          acc[j] = fma((double)xs[j][c + 0], (double)e.x, acc[j]);
-          acc[j] = fma((double)xs[j][c + 1], (double)e.y, acc[j]);
-          acc[j] = fma((double)xs[j][c + 2], (double)e.z, acc[j]);
-          acc[j] = fma((double)xs[j][c + 3], (double)e.w, acc[j]);
-        }
-      }
-    }
-    if (n < N) {
-#pragma unroll
-      for (int j = 0; j < kF32Q; ++j)
-        if (q0 + j < nq) sims[(size_t)(q0 + j) * N + n] = (float)acc[j];
-    }
-  }
-}
-
-// One block per query: kc rounds, each takes the best row strictly after the previous pick in the total order.
-__global__ void __launch_bounds__(256)
-select_f32_kernel(const float* __restrict__ sims, int64_t N, int kc, float* __restrict__ cand_sim, int32_t* __restrict__ cand_idx) {
-  __shared__ unsigned long long wbest[8];
-  __shared__ unsigned long long prev_s;
-  const float* s = sims + (size_t)blockIdx.x * N;
-  unsigned long long prev = ~0ull;
-  for (int j = 0; j < kc; ++j) {
-    unsigned long long best = 0;
-    for (int64_t n = threadIdx.x; n < N; n += blockDim.x) {
-      const float v = s[n];
-      if (v == v) {   // NaN never selected
-        const unsigned long long key = make_key(v, (int32_t)n);
-        if (key < prev && key > best) best = key;
-      }
-    }
-    for (int o = 16; o > 0; o >>= 1) {
-      const unsigned long long other = __shfl_xor_sync(0xffffffffu, best, o);
-      best = other > best ? other : best;
-    }
-    if ((threadIdx.x & 31) == 0) wbest[threadIdx.x >> 5] = best;
-    __syncthreads();
-    if (threadIdx.x == 0) {
-      unsigned long long b = 0;
-      for (int w = 0; w < 8; ++w) b = wbest[w] > b ? wbest[w] : b;
-      prev_s = b;
-      const size_t o = (size_t)blockIdx.x * kc + j;
-      if (b == 0) {
-        cand_sim[o] = -INFINITY;
-        cand_idx[o] = -1;
-      } else {
-        cand_sim[o] = f32_unordered((uint32_t)(b >> 32));
-        cand_idx[o] = (int32_t)(0xffffffffu - (uint32_t)b);
-      }
-    }
-    __syncthreads();
-    prev = prev_s;
-    if (prev == 0) prev = 1;   // exhausted: later rounds find nothing
-  }
 }
 
 // ---- a2 + a3 + a4: one CTA per query (finish_body.cuh) ---------------------------------------------------
@@ -170,32 +117,25 @@ cudaError_t launch_read_stream(const void* buf, size_t bytes, uint32_t* sink, cu
 }
 
 cudaError_t launch_stage_queries(const CallParams& cp, __nv_bfloat16* qs, int B, int Bpad, int d, int rep, uint32_t* gthr,
-                                 int n_gthr, cudaStream_t s) {
+                                 int n_gthr, int split, float* q32, cudaStream_t s) {
   const size_t n = (size_t)Bpad * d;
   int blocks = (int)((n + 255) / 256);
   if (blocks > 148 * 8) blocks = 148 * 8;
-  stage_queries_kernel<<<blocks, 256, 0, s>>>(cp, qs, B, Bpad, d, rep > 1 ? kTileM / rep : Bpad, gthr, n_gthr);
+  stage_queries_kernel<<<blocks, 256, 0, s>>>(cp, qs, B, Bpad, d, rep > 1 ? kTileM / rep : Bpad, gthr, n_gthr, split, q32);
   return cudaGetLastError();
 }
 
-cudaError_t launch_scan_f32(const float* bank, const CallParams& cp, int r0, int64_t N, int d, int nq, float* sims,
-                            cudaStream_t s) {
-  const int blocks = (int)((N + kF32Rows - 1) / kF32Rows);
-  scan_f32_kernel<<<blocks, kF32Rows, 0, s>>>(bank, cp, r0, N, d, nq, sims);
-  return cudaGetLastError();
-}
-
-cudaError_t launch_select_f32(const float* sims, int64_t N, int nq, int kc, float* cand_sim, int32_t* cand_idx,
-                              cudaStream_t s) {
-  select_f32_kernel<<<nq, 256, 0, s>>>(sims, N, kc, cand_sim, cand_idx);
+cudaError_t launch_split_bank(const float* in, __nv_bfloat16* out, size_t rows, int d, cudaStream_t s) {
+  size_t blocks = (rows * d + 255) / 256;
+  if (blocks > 148 * 16) blocks = 148 * 16;
+  split_bank_kernel<<<(int)blocks, 256, 0, s>>>(in, out, rows, d);
   return cudaGetLastError();
 }
 
 // Position and count of the arguments of this file's kernels that carry the per-call parameters (graph replays update
 // that one argument): returns the index of the CallParams argument, or -1 if func is not one of them.
 int estimate_cp_arg(const void* func, int* nargs) {
-  if (func == (const void*)stage_queries_kernel) { *nargs = 8; return 0; }
-  if (func == (const void*)scan_f32_kernel) { *nargs = 7; return 1; }
+  if (func == (const void*)stage_queries_kernel) { *nargs = 10; return 0; }
   if (func == (const void*)finish_kernel) { *nargs = 3; return 2; }
   return -1;
 }

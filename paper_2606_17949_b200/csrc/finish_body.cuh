@@ -90,6 +90,30 @@ __device__ __forceinline__ float exact_sim_bf16(const uint4* __restrict__ qrow, 
   return (float)acc;
 }
 
+// s = fl32( sum_c (double)x[c]*(double)e[c] ) of two fp32 rows of d values (d % 4 == 0), lanes' fp64 partials added by shuffles.
+__device__ __forceinline__ float exact_sim_f32(const float4* __restrict__ qrow, const float4* __restrict__ brow, int nvec4,
+                                               int lane) {
+  double acc = 0.0;
+#pragma unroll 2
+  for (int v = lane; v < nvec4; v += 32) {
+    const float4 x = qrow[v], e = __ldg(brow + v);
+    acc = fma((double)x.x, (double)e.x, acc);
+    acc = fma((double)x.y, (double)e.y, acc);
+    acc = fma((double)x.z, (double)e.z, acc);
+    acc = fma((double)x.w, (double)e.w, acc);
+  }
+  for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+  return (float)acc;
+}
+// Exact similarity of query row r to bank row n in the storage precision (a.rerank: 1 bf16 rows, 2 fp32 rows).
+__device__ __forceinline__ float exact_sim(const FinishArgs& a, const float* __restrict__ q32, int r, int64_t n, int lane) {
+  if (a.rerank == 2)
+    return exact_sim_f32(reinterpret_cast<const float4*>(q32 + (size_t)r * a.d),
+                         reinterpret_cast<const float4*>(a.bank32 + (size_t)n * a.d), a.d / 4, lane);
+  return exact_sim_bf16(reinterpret_cast<const uint4*>(a.qs + (size_t)r * a.d),
+                        reinterpret_cast<const uint4*>(a.bank + (size_t)n * a.d), a.d / 8, lane);
+}
+
 // kc rounds of a block-wide maximum over distinct 64-bit keys: each round takes the largest key below the previous
 // pick (keys [n] in shared memory; 0 = empty).  Result in out[0..kc), descending (0 = exhausted).  All threads of the
 // block must call.  Rare path: kept out of line.
@@ -131,7 +155,7 @@ __device__ __forceinline__ void slab_rows(const FinishArgs& a, int c, int nslabs
 // The slabs whose list may hide members of the kc best (last entry at or above kstar, the kc-th best key found) are
 // searched again with exact similarities; S.cand becomes the kc best of those slabs' rows and of the candidates that
 // came from the other slabs.  s_keys is overwritten ([nwarps][kRescanKeep] + [kc]).  All threads must call; rare path.
-__device__ __noinline__ void rescan_slabs(const FinishArgs a, const uint4* qrow, int nvec, unsigned long long kstar,
+__device__ __noinline__ void rescan_slabs(const FinishArgs a, const float* q32, int r, unsigned long long kstar,
                                           unsigned long long* s_keys, FinScratch& S) {
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, nwarps = blockDim.x >> 5;
   const int kc = a.kc, kcap = a.kcap;
@@ -165,7 +189,7 @@ __device__ __noinline__ void rescan_slabs(const FinishArgs a, const uint4* qrow,
     int64_t row0, row1;
     slab_rows(a, S.flag[f], nslabs, &row0, &row1);
     for (int64_t n = row0 + warp; n < row1; n += nwarps) {
-      const float sx = exact_sim_bf16(qrow, reinterpret_cast<const uint4*>(a.bank + (size_t)n * a.d), nvec, lane);
+      const float sx = exact_sim(a, q32, r, n, lane);
       const unsigned long long x = fin_key(sx, (int32_t)n);
       if (sx == sx && x > thr) {
         const int p = __popc(__ballot_sync(0xffffffffu, la > x)) + __popc(__ballot_sync(0xffffffffu, lb > x));
@@ -217,9 +241,7 @@ __device__ __forceinline__ void finish_query(const FinishArgs& a, const InstTabl
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int nthreads = blockDim.x, nwarps = blockDim.x >> 5;
   const int kc = a.kc, k = a.k, kcap = a.kcap, M = a.M;
-  const int nvec = a.d / 8;   // d % 8 == 0
   const int total = a.nlists * kcap;
-  const uint4* qrow = reinterpret_cast<const uint4*>(a.qs + (size_t)r * a.d);
   // coefficients of the score terms: requested now, consumed at the very end (their latency hides behind the merge)
   float c_pin = 0.0f, c_pout = 0.0f, c_pre = 0.0f, c_ell = 0.0f, c_budget = 0.0f;
   bool has_budget = false;
@@ -344,7 +366,7 @@ __device__ __forceinline__ void finish_query(const FinishArgs& a, const InstTabl
       const unsigned long long last = s_keys[(size_t)l * kcap + kcap - 1];
       flagged |= (last != 0ull && last >= kstar);
     }
-    if (__syncthreads_or(flagged)) rescan_slabs(a, qrow, nvec, kstar, s_keys, S);
+    if (__syncthreads_or(flagged)) rescan_slabs(a, a.q32, r, kstar, s_keys, S);
   }
 
   // ---- exact re-rank: warp c recomputes candidate c, then -- without waiting for the others -- its weight and
@@ -357,7 +379,7 @@ __device__ __forceinline__ void finish_query(const FinishArgs& a, const InstTabl
     float l = 0.0f;   // the labels are requested first: independent of the bank row's loads
     if (id >= 0 && lane < 2 * M)
       l = (lane < M) ? __ldg(a.bank_quality + (size_t)id * M + lane) : __ldg(a.bank_outlen + (size_t)id * M + lane - M);
-    if (id >= 0 && a.rerank) sx = exact_sim_bf16(qrow, reinterpret_cast<const uint4*>(a.bank + (size_t)id * a.d), nvec, lane);
+    if (id >= 0 && a.rerank) sx = exact_sim(a, a.q32, r, id, lane);
     float w = 1.0f;
     if (id < 0) {
       w = 0.0f;   // fewer than kc rows reachable; sorts last and adds +0 if it is ever summed

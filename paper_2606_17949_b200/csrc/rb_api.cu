@@ -28,7 +28,9 @@ struct rb_ctx {
   bool own_stream = false;
   int num_sms = 148;
   // bank
-  void* bank = nullptr;          // bf16 [N x d] or fp32 [N x d]
+  void* bank = nullptr;          // what the tensor-core scan reads: bf16 [N x d], or (fp32 storage) the split bank bf16 [N x 5 d]
+  float* bank32 = nullptr;       // fp32 storage: the fp32 bank [N x d] the exact re-rank reads
+  int d_scan = 0;                // columns of a scanned row: d, or 5 d (fp32 storage: three-plane bf16 split)
   float* bank_quality = nullptr; // [N x M]
   float* bank_outlen = nullptr;
   // instances
@@ -40,14 +42,14 @@ struct rb_ctx {
   int32_t* bq = nullptr;
   // per-call staging + scratch (sized by max_batch)
   int Bpad_max = 0;
-  float* q32 = nullptr;             // [max_batch x d]
+  float* q32 = nullptr;             // [max_batch x d] fp32 storage: device copy of the queries for the exact re-rank
+  float* q32_in = nullptr;          // [max_batch x d] staging of host queries that do not fit the pinned block
   __nv_bfloat16* qs = nullptr;      // [Bpad_max x d]
   int32_t* plen = nullptr;          // [max_batch]
   CallParams cp_cur{};              // per-call parameters of the call being enqueued (passed to the kernels by value)
   uint32_t* gthr = nullptr;         // [Bpad_max] cross-slab admission thresholds of the scan (cleared per decision)
   float* part_sim = nullptr;        // [num_sms][kcap][Bpad_max]
   int32_t* part_idx = nullptr;
-  float* sims = nullptr;            // fp32 storage only: [kF32Group x N]
   float* cand_sim = nullptr;        // [max_batch x kc]
   int32_t* cand_idx = nullptr;
   int32_t* scratch_nn_idx = nullptr;   // [max_batch x k] staging for host callers
@@ -124,7 +126,6 @@ struct rb_ctx {
 
 namespace {
 
-constexpr int kF32Group = 64;   // queries per pass of the fp32-storage scan
 
 rb_status fail(rb_ctx* c, rb_status st, const char* what, cudaError_t e = cudaSuccess) {
   if (c) {
@@ -258,7 +259,8 @@ rb_status enqueue_estimate(rb_ctx* ctx, int B, bool with_terms, Timer& tm, int s
   fa.weight_mode = ctx->opt.weight_mode; fa.eps = ctx->opt.dist_eps; fa.with_terms = with_terms ? 1 : 0;
   fa.pred_q = S.pred_q; fa.pred_l = S.pred_l; fa.termA = S.termA; fa.termP = S.termP; fa.key = S.key;
   const bool front = part != kBack, back = part != kFront;
-  if (ctx->opt.store_dtype == RB_BF16) {
+  const int split = ctx->opt.store_dtype == RB_F32 ? 1 : 0;   // fp32 storage: the scan runs over the three-plane bf16 split
+  {
     if (ctx->stage_timing && front) {   // before the first mark: nothing but the kernels between the stage events
       CK(cudaMemcpyAsync(ctx->dev_clock, ctx->dev_clock_init, 16, cudaMemcpyDeviceToDevice, s));
     }
@@ -272,10 +274,10 @@ rb_status enqueue_estimate(rb_ctx* ctx, int B, bool with_terms, Timer& tm, int s
       // popped completely is searched again by the finishing kernel, as for the single-CTA scan
       const int kcap2 = std::min(ctx->kcap, 16);
       if (front) {
-        CK(launch_stage_queries(ctx->cp_cur, S.qs, B, Bpad2, ctx->d, 1, ctx->gthr, Bpad2 * (1 + ncl), s));
+        CK(launch_stage_queries(ctx->cp_cur, S.qs, B, Bpad2, ctx->d, 1, ctx->gthr, Bpad2 * (1 + ncl), split, ctx->q32, s));
         tm.mark();
         int ncl_used = 0;
-        CK(launch_scan_tc2(&S.tm_q, &ctx->tm_bank, ctx->N, ctx->d, B, Bpad2, kcap2, ctx->kc, ctx->num_sms, S.part_sim,
+        CK(launch_scan_tc2(&S.tm_q, &ctx->tm_bank, ctx->N, ctx->d_scan, B, Bpad2, kcap2, ctx->kc, ctx->num_sms, S.part_sim,
                            S.part_idx, ctx->gthr, &ncl_used, s));
         tm.mark();
         ctx->launches += 2;
@@ -287,10 +289,10 @@ rb_status enqueue_estimate(rb_ctx* ctx, int B, bool with_terms, Timer& tm, int s
       const int64_t units = (ctx->N + kBoxN - 1) / kBoxN;
       const int grid = (int)(units < ctx->num_sms ? units : ctx->num_sms);   // what launch_scan_tc uses
       if (front) {
-        CK(launch_stage_queries(ctx->cp_cur, S.qs, B, Bpad, ctx->d, rep, ctx->gthr, 0, s));
+        CK(launch_stage_queries(ctx->cp_cur, S.qs, B, Bpad, ctx->d, rep, ctx->gthr, 0, split, ctx->q32, s));
         tm.mark();
         int grid_used = 0;
-        CK(launch_scan_tc(&S.tm_q, &ctx->tm_bank, ctx->N, ctx->d, B, Bpad, ctx->ks, ctx->num_sms, S.part_sim, S.part_idx,
+        CK(launch_scan_tc(&S.tm_q, &ctx->tm_bank, ctx->N, ctx->d_scan, B, Bpad, ctx->ks, ctx->num_sms, S.part_sim, S.part_idx,
                           &grid_used, ctx->stage_timing ? ctx->dev_clock : nullptr, s));
         tm.mark();
         ctx->launches += 2;
@@ -300,24 +302,11 @@ rb_status enqueue_estimate(rb_ctx* ctx, int B, bool with_terms, Timer& tm, int s
       fa.Bpad = Bpad; fa.slab_unit = kBoxN;
       fa.rescan = ctx->ks < ctx->kc ? 1 : 0;
     }
-    fa.bank = (const __nv_bfloat16*)ctx->bank; fa.qs = S.qs; fa.rerank = ctx->opt.rerank_slack > 0 ? 1 : 0;
-  } else {
-    if (front) {
-      tm.mark();
-      tm.mark();
-      for (int r0 = 0; r0 < B; r0 += kF32Group) {
-        const int nq = (B - r0 < kF32Group) ? (B - r0) : kF32Group;
-        CK(launch_scan_f32((const float*)ctx->bank, ctx->cp_cur, r0, ctx->N, ctx->d, nq, ctx->sims, s));
-        CK(launch_select_f32(ctx->sims, ctx->N, nq, ctx->kc, ctx->cand_sim + (size_t)r0 * ctx->kc,
-                             ctx->cand_idx + (size_t)r0 * ctx->kc, s));
-        ctx->launches += 2;
-      }
-      tm.mark();
+    if (split) {   // exact similarities from the fp32 rows (the definition of fp32 storage), always
+      fa.bank = nullptr; fa.qs = nullptr; fa.bank32 = ctx->bank32; fa.q32 = ctx->q32; fa.rerank = 2;
+    } else {
+      fa.bank = (const __nv_bfloat16*)ctx->bank; fa.qs = S.qs; fa.rerank = ctx->opt.rerank_slack > 0 ? 1 : 0;
     }
-    // the selected candidates are one already-merged list per query: [1][B][kc]
-    fa.part_sim = ctx->cand_sim; fa.part_idx = ctx->cand_idx; fa.nlists = 1; fa.lists_per_cta = 1; fa.kcap = ctx->kc; fa.Bpad = B;
-    fa.slab_unit = kBoxN;
-    fa.bank = nullptr; fa.qs = nullptr; fa.rerank = 0;
   }
   if (back) {
     CK(launch_finish(fa, table_of(ctx), ctx->cp_cur, B, s));
@@ -619,7 +608,10 @@ rb_status rb_create(rb_ctx** out, const void* bank_emb, const float* bank_qualit
   if (opt.bank_dtype != RB_F32 && opt.bank_dtype != RB_BF16) return RB_EINVAL;
   if (opt.store_dtype != RB_F32 && opt.store_dtype != RB_BF16) return RB_EINVAL;
   if (opt.store_dtype == RB_F32 && opt.bank_dtype != RB_F32) return RB_EINVAL;
-  if (opt.store_dtype == RB_F32 || opt.rerank_slack < 0) opt.rerank_slack = 0;
+  if (opt.rerank_slack < 0) opt.rerank_slack = 0;
+  // fp32 storage always re-ranks (exact fp32-row similarities are its definition): the candidates come from a scan of
+  // the three-plane bf16 split, good to ~5e-6, so a few spare candidates are kept
+  if (opt.store_dtype == RB_F32 && opt.rerank_slack == 0) opt.rerank_slack = std::min(6, kMaxK - k);
   if (k + opt.rerank_slack > kMaxK) return RB_EINVAL;
   if (opt.max_batch < 1 || opt.max_batch > 4096) return RB_EINVAL;
   if (!(opt.dist_eps >= 0.0f) || !std::isfinite(opt.dist_eps)) return RB_EINVAL;
@@ -644,6 +636,7 @@ rb_status rb_create(rb_ctx** out, const void* bank_emb, const float* bank_qualit
   rb_ctx* ctx = new (std::nothrow) rb_ctx();
   if (!ctx) return RB_ENOMEM;
   ctx->N = N; ctx->d = d; ctx->M = M; ctx->k = k; ctx->opt = opt;
+  ctx->d_scan = opt.store_dtype == RB_F32 ? 5 * d : d;
   ctx->kc = k + opt.rerank_slack;
   ctx->kcap = ctx->kc <= 16 ? 16 : (ctx->kc <= 32 ? 32 : 64);
   ctx->num_sms = prop.multiProcessorCount;
@@ -723,11 +716,13 @@ rb_status rb_create(rb_ctx** out, const void* bank_emb, const float* bank_qualit
       cudaFree(tmp);
     }
   } else {
-    float* b32 = nullptr;
-    ALLOC(b32, nd);
-    ctx->bank = b32;
-    CK(cudaMemcpyAsync(b32, bank_emb, nd * 4, cudaMemcpyDefault, s));
-    ALLOC(ctx->sims, (size_t)kF32Group * N);
+    // fp32 storage: the fp32 rows (exact re-rank) and their three-plane bf16 split (what the tensor cores scan)
+    ALLOC(ctx->bank32, nd);
+    CK(cudaMemcpyAsync(ctx->bank32, bank_emb, nd * 4, cudaMemcpyDefault, s));
+    __nv_bfloat16* bs = nullptr;
+    ALLOC(bs, 5 * nd);
+    ctx->bank = bs;
+    CK(launch_split_bank(ctx->bank32, bs, (size_t)N, d, s));
   }
   ALLOC(ctx->bank_quality, (size_t)N * M);
   ALLOC(ctx->bank_outlen, (size_t)N * M);
@@ -736,6 +731,7 @@ rb_status rb_create(rb_ctx** out, const void* bank_emb, const float* bank_qualit
 
   const size_t mb = opt.max_batch;
   ALLOC(ctx->q32, mb * d);
+  ALLOC(ctx->q32_in, mb * d);
   // Everything a decision's latency-bound kernels touch (per-call parameters, instance table, state, per-request
   // terms and outputs) lives in ONE allocation, packed: a cold kernel then pays for one or two TLB misses instead
   // of one per buffer.
@@ -776,17 +772,18 @@ rb_status rb_create(rb_ctx** out, const void* bank_emb, const float* bank_qualit
     }
     CK(cudaMemsetAsync(ctx->arena, 0, off, s));
   }
-  if (opt.store_dtype == RB_BF16) {
-    ALLOC(ctx->qs, (size_t)ctx->Bpad_max * d);
+  {
+    const int ds = ctx->d_scan;
+    ALLOC(ctx->qs, (size_t)ctx->Bpad_max * ds);
     ALLOC(ctx->gthr, (size_t)ctx->Bpad_max * (2 + ctx->num_sms / 2));
     // [grid * rep][Bpad][ks]: rep = 4 replicas only when Bpad = 128
     const size_t part_n = (size_t)ctx->num_sms * ctx->kcap * std::max<size_t>(ctx->Bpad_max, 4 * kTileM);
     ALLOC(ctx->part_sim, 2 * part_n);          // one allocation: [similarities | indices], or 32-byte records over all of it
     ctx->part_idx = reinterpret_cast<int32_t*>(ctx->part_sim + part_n);
-    CK(cudaMemsetAsync(ctx->qs, 0, (size_t)ctx->Bpad_max * d * 2, s));
-    rb_status st = encode_map(ctx, &ctx->tm_bank, ctx->bank, (uint64_t)N, (uint64_t)d, kBoxN);
+    CK(cudaMemsetAsync(ctx->qs, 0, (size_t)ctx->Bpad_max * ds * 2, s));
+    rb_status st = encode_map(ctx, &ctx->tm_bank, ctx->bank, (uint64_t)N, (uint64_t)ds, kBoxN);
     if (st != RB_OK) return st;
-    st = encode_map(ctx, &ctx->tm_q, ctx->qs, (uint64_t)ctx->Bpad_max, (uint64_t)d, kTileM);
+    st = encode_map(ctx, &ctx->tm_q, ctx->qs, (uint64_t)ctx->Bpad_max, (uint64_t)ds, kTileM);
     if (st != RB_OK) return st;
     if (opt.pipeline) {
       // second buffer set, for batches of at most 128 requests (larger ones are not pipelined)
@@ -1051,8 +1048,8 @@ rb_status rb_decide_budgeted(rb_ctx* ctx, const float* query_emb, const int32_t*
   CallParams cp{};
   cp.w_qual = w[0]; cp.w_lat = w[1]; cp.w_cost = w[2]; cp.commit = 1;
   bool adv_folded = false;
-  if (ctx->opt.store_dtype == RB_BF16 && ctx->opt.latency_mode != 2) {
-    cp.n_adv = ctx->n_pending;   // applied by the staging kernel, ahead of everything that reads the state
+  if (ctx->opt.latency_mode != 2) {
+    cp.n_adv = ctx->n_pending;   // applied by the dispatch kernel when it loads the state
     for (int a = 0; a < ctx->n_pending; ++a) cp.adv_ms[a] = ctx->pending_adv[a];
     adv_folded = true;           // (n_pending is cleared only once the decision has been enqueued: a failed call changes nothing)
   } else {
@@ -1060,7 +1057,9 @@ rb_status rb_decide_budgeted(rb_ctx* ctx, const float* query_emb, const int32_t*
     if (st != RB_OK) return st;
   }
   // (the fp32-storage scan reads every query from every block: it wants them in device memory)
-  cp.query = sg.in_zc(query_emb, 0, ctx->opt.store_dtype == RB_BF16 ? ctx->zc_query_cap : 0, ctx->q32, (size_t)B * ctx->d * 4);
+  // (host queries: read in place from the pinned block by the staging kernel, which -- under fp32 storage -- also leaves
+  // the device copy the re-rank reads; the copy-engine fallback stages them in a separate buffer)
+  cp.query = sg.in_zc(query_emb, 0, ctx->zc_query_cap, ctx->q32_in, (size_t)B * ctx->d * 4);
   cp.plen = sg.in_zc(prompt_len, ctx->zc_off_plen, (size_t)B * 4, ctx->plen, (size_t)B * 4);
   cp.q_src = ctx->pred_q;
   cp.l_src = ctx->pred_l;
@@ -1106,7 +1105,7 @@ rb_status rb_estimate(rb_ctx* ctx, const float* query_emb, int32_t B, float* pre
   const size_t bm = (size_t)B * ctx->M * 4, bk = (size_t)B * ctx->k * 4;
   Stager sg{ctx};
   CallParams cp{};
-  cp.query = sg.in(query_emb, ctx->q32, (size_t)B * ctx->d * 4);
+  cp.query = sg.in(query_emb, ctx->q32_in, (size_t)B * ctx->d * 4);
   cp.pred_q = sg.out_internal(pred_quality, ctx->pred_q, bm);
   cp.pred_l = sg.out_internal(pred_outlen, ctx->pred_l, bm);
   cp.nn_idx = sg.out(nn_idx, ctx->scratch_nn_idx, bk);
@@ -1365,8 +1364,8 @@ void rb_destroy(rb_ctx* ctx) {
   if (ctx->front) cudaStreamSynchronize(ctx->front);
   if (ctx->stream) cudaStreamSynchronize(ctx->stream);
   drop_graphs(ctx);
-  void* ptrs[] = {ctx->bank, ctx->bank_quality, ctx->bank_outlen, ctx->arena, ctx->q32, ctx->qs, ctx->part_sim,
-                  ctx->gthr, ctx->sims, ctx->scratch_nn_idx, ctx->scratch_nn_sim, ctx->scores, ctx->scores0, ctx->f_nodes,
+  void* ptrs[] = {ctx->bank, ctx->bank_quality, ctx->bank_outlen, ctx->arena, ctx->q32, ctx->q32_in, ctx->qs, ctx->part_sim,
+                  ctx->gthr, ctx->bank32, ctx->scratch_nn_idx, ctx->scratch_nn_sim, ctx->scores, ctx->scores0, ctx->f_nodes,
                   ctx->f_root, ctx->f_begin, ctx->f_base, ctx->dev_clock, ctx->sweep_buf};
   for (void* p : ptrs) cudaFree(p);
   cudaFree(ctx->slot[1].qs);

@@ -220,8 +220,11 @@ cudaError_t launch_convert_bf16(const float* in, __nv_bfloat16* out, size_t n, c
 
 // a0: cp->query (fp32) -> bf16 staging [Bpad x d]; rep copies of the B queries at rows j*(128/rep) + r (rep > 1 only
 // when Bpad = 128), all other rows zero.  Also clears gthr [n_gthr] (the scan's cross-slab thresholds).
+// split = 1 (fp32 storage): rows of 5 d columns [hi | hi | mid | hi | lo] of the three-plane bf16 split of every value.
 cudaError_t launch_stage_queries(const CallParams& cp, __nv_bfloat16* qs, int B, int Bpad, int d, int rep, uint32_t* gthr,
-                                 int n_gthr, cudaStream_t s);
+                                 int n_gthr, int split, float* q32 /* split: device copy of the B fp32 rows */, cudaStream_t s);
+// fp32 bank rows -> [hi | mid | hi | lo | hi] bf16 rows of 5 d columns (fp32 storage: the bank the tensor-core scan reads)
+cudaError_t launch_split_bank(const float* in, __nv_bfloat16* out, size_t rows, int d, cudaStream_t s);
 // query replicas over the TMEM lane quarters: 4 (B <= 32), 2 (B <= 64), 1; halved while the finishing kernel could not
 // hold max_grid * replicas lists of kcap entries in shared memory (long lists: k = 32)
 int scan_tc_replicas(int B, int kcap, int max_grid);
@@ -248,13 +251,6 @@ cudaError_t launch_scan_tc2(const CUtensorMap* tm_q, const CUtensorMap* tm_bank,
 int scan_tc2_clusters(int64_t N, int max_grid);
 cudaError_t scan_tc2_prepare();
 
-// a1 (fp32 storage): exact fp64-accumulated similarities of nq queries (q: [nq x d]) to sims [nq x N],
-// then per-query selection of the kc best (sim desc, idx asc) into cand_* [nq x kc].
-cudaError_t launch_scan_f32(const float* bank, const CallParams& cp, int r0, int64_t N, int d, int nq, float* sims,
-                            cudaStream_t s);
-cudaError_t launch_select_f32(const float* sims, int64_t N, int nq, int kc, float* cand_sim, int32_t* cand_idx,
-                              cudaStream_t s);
-
 // a2 + a3 (+ a4 when with_terms): one CTA per query merges the nlists sorted partial lists
 // (part_* [nlists][Bpad][kcap]) into the kc best, re-ranks them exactly (bf16 storage, rerank != 0), keeps k,
 // aggregates the labels with distance weights and, when with_terms, derives the per-(request, tier) terms
@@ -270,7 +266,9 @@ struct FinishArgs {
   int64_t N;
   const __nv_bfloat16* bank;
   const __nv_bfloat16* qs;
-  int d, rerank;
+  const float* bank32;      // fp32 storage: the fp32 bank rows the exact re-rank reads (rerank = 2) ...
+  const float* q32;         // ... and the fp32 query rows (device copy made by the staging kernel)
+  int d, rerank;            // rerank: 0 none, 1 exact from the bf16 rows (bf16 storage), 2 exact from the fp32 rows
   int rescan;               // 1: lists are shorter than kc -> slabs whose list was popped completely are searched again
   const float* bank_quality;
   const float* bank_outlen;
