@@ -273,14 +273,14 @@ def run_ours(args):
             flush_buf.sum()          # read-only sweep of 3x L2: evicts the bank without leaving dirty lines
 
     # the steps' device buffers are views prepared beforehand: slicing torch tensors is Python overhead, not the library's
-    qv = [allq[offs[j]:offs[j + 1]] for j in range(W + K)]
-    pv = [allp[offs[j]:offs[j + 1]] for j in range(W + K)]
-    av = [assign_all[offs[j]:offs[j + 1]] for j in range(W + K)]
+    dev_q = [allq[offs[j]:offs[j + 1]] for j in range(W + K)]
+    dev_p = [allp[offs[j]:offs[j + 1]] for j in range(W + K)]
+    dev_a = [assign_all[offs[j]:offs[j + 1]] for j in range(W + K)]
 
     def step_device(j, r=None, out=None):
         r = rt if r is None else r
         rb.rb_advance_state(r.ctx, elapsed[j])
-        rb.rb_decide(r.ctx, qv[j], pv[j], sizes[j], weights[j], assign_dev[:sizes[j]] if out is None else av[j])
+        rb.rb_decide(r.ctx, dev_q[j], dev_p[j], sizes[j], weights[j], assign_dev[:sizes[j]] if out is None else dev_a[j])
 
     def barrier():
         torch.cuda.synchronize()
