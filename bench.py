@@ -369,6 +369,24 @@ def run_ours(args):
         rb.rb_decide(rt.ctx, qv, pv, B, weights[W + j], av)
         e2e_s += time.perf_counter() - t0
     barrier()
+    e2e_sync_max, _ = reduce_over_ranks(dist, dev, e2e_s, timed_req)
+    # the serving loop with two decisions in flight: submit(j + 1), collect(j) -- same host buffers, same bytes across the bus
+    rtp.set_state(queued, running)
+    for j in range(4):
+        rb.rb_decide_submit(rtp.ctx, views[j][0], views[j][1], sizes[W + j], weights[W + j])
+        rb.rb_decide_collect(rtp.ctx, views[j][2], sizes[W + j])
+    rtp.set_state(queued, running)
+    barrier()
+    t0 = time.perf_counter()
+    for j in range(K):
+        qv, pv, av = views[j]
+        rb.rb_advance_state(rtp.ctx, elapsed[W + j])
+        rb.rb_decide_submit(rtp.ctx, qv, pv, sizes[W + j], weights[W + j])
+        if j >= 1:
+            rb.rb_decide_collect(rtp.ctx, views[j - 1][2], sizes[W + j - 1])
+    rb.rb_decide_collect(rtp.ctx, views[K - 1][2], sizes[W + K - 1])
+    e2e_s = time.perf_counter() - t0
+    barrier()
     e2e_max, _ = reduce_over_ranks(dist, dev, e2e_s, timed_req)
     # (inputs cross the bus inside the timed call: host memcpy into the library's pinned block, read from there by the
     # staging kernel; the assignment is written to pinned host memory by the dispatch kernel)
@@ -423,7 +441,14 @@ def run_ours(args):
                            "mode": "one decision at a time, unpipelined context, L2 flushed before each",
                            "unpipelined_flushed_requests_per_s": round(lat_req_per_s, 1)},
            "e2e": {"value": round(units / e2e_max, 1), "unit": UNIT, "h2d_bytes_per_step": round(h2d, 1),
-                   "d2h_bytes_per_step": round(d2h, 1), "us_per_decision": round(e2e_max / K * 1e6, 2)},
+                   "d2h_bytes_per_step": round(d2h, 1), "us_per_decision": round(e2e_max / K * 1e6, 2),
+                   "mode": "rb_decide_submit / rb_decide_collect from pinned host buffers, two decisions in flight (wall clock "
+                           "over the K steps; each step's inputs are copied into the library's pinned block and read over the "
+                           "bus by its kernels, the assignment is written to pinned host memory by the dispatch kernel)",
+                   "synchronous_call": {"us_per_decision": round(e2e_sync_max / K * 1e6, 2),
+                                        "requests_per_s": round(units / e2e_sync_max, 1),
+                                        "note": "one rb_decide at a time from the same host buffers, L2 flushed before each: "
+                                                "the latency a single caller sees"}},
            "gpu_launches": int(launches), "clocks": sampler.summary(), "roofline": roofline,
            "paper_context": "paper: ~32 ms per decision at 12 req/s on its 96-core CPU host, encoder included (P:L7)"}
 

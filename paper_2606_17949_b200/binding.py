@@ -26,7 +26,7 @@ RB_OK, RB_EINVAL, RB_ECUDA, RB_ENOMEM, RB_ESTATE, RB_EUNSUPPORTED = range(6)
 RB_F32, RB_BF16 = 0, 1
 _STATUS = {0: "RB_OK", 1: "RB_EINVAL", 2: "RB_ECUDA", 3: "RB_ENOMEM", 4: "RB_ESTATE", 5: "RB_EUNSUPPORTED"}
 EXPORTS = ["rb_options_default", "rb_create", "rb_set_instances", "rb_set_tpot_forest", "rb_set_telemetry", "rb_set_state", "rb_get_state", "rb_advance_state",
-           "rb_batch_target", "rb_decide", "rb_decide_budgeted", "rb_decide_from_predictions", "rb_decide_from_predictions_budgeted", "rb_sweep_weights", "rb_estimate", "rb_dispatch_pipeline", "rb_match_replay", "rb_set_stage_timing", "rb_last_stage_us", "rb_last_scan_device_us", "rb_selftest_division", "rb_testing_read_bandwidth",
+           "rb_batch_target", "rb_decide", "rb_decide_submit", "rb_decide_collect", "rb_decide_budgeted", "rb_decide_from_predictions", "rb_decide_from_predictions_budgeted", "rb_sweep_weights", "rb_estimate", "rb_dispatch_pipeline", "rb_match_replay", "rb_set_stage_timing", "rb_last_stage_us", "rb_last_scan_device_us", "rb_selftest_division", "rb_testing_read_bandwidth",
            "rb_launch_count", "rb_sync", "rb_last_error", "rb_destroy"]
 
 
@@ -64,6 +64,8 @@ _lib.rb_set_state.argtypes = [_vp, _vp, _vp]
 _lib.rb_get_state.argtypes = [_vp, _vp, _vp]
 _lib.rb_advance_state.argtypes = [_vp, _f]
 _lib.rb_batch_target.argtypes = [_vp, _i32, _i32, _vp, _vp]
+_lib.rb_decide_submit.argtypes = [_vp, _vp, _vp, _i32, ctypes.POINTER(_f * 3)]
+_lib.rb_decide_collect.argtypes = [_vp, _vp, _i32]
 _lib.rb_decide.argtypes = [_vp, _vp, _vp, _i32, ctypes.POINTER(_f * 3), _vp, _vp, _vp, _vp, _vp, _vp]
 _lib.rb_decide_from_predictions.argtypes = [_vp, _vp, _vp, _vp, _i32, ctypes.POINTER(_f * 3), _i32, _vp, _vp, _vp, _vp]
 _lib.rb_decide_budgeted.argtypes = [_vp, _vp, _vp, _vp, _i32, ctypes.POINTER(_f * 3), _vp, _vp, _vp, _vp, _vp, _vp, _vp]
@@ -205,6 +207,18 @@ def rb_decide(ctx, query_emb, prompt_len, B, w, assignment, scores=None, pred_qu
     _check(ctx, _lib.rb_decide(ctx, _ptr(query_emb, f32), _ptr(prompt_len, i32), B, _w3(w), _ptr(assignment, i32),
                                _ptr(scores, f32), _ptr(pred_quality, f32), _ptr(pred_outlen, f32), _ptr(nn_idx, i32),
                                _ptr(nn_sim, f32)))
+
+
+def rb_decide_submit(ctx, query_emb, prompt_len, B, w):
+    """Enqueues a decision from HOST buffers and returns at once (rb_options.pipeline = 1; at most two in flight)."""
+    f32, i32 = (torch.float32, torch.int32) if torch else (np.float32, np.int32)
+    _check(ctx, _lib.rb_decide_submit(ctx, _ptr(query_emb, f32), _ptr(prompt_len, i32), B, _w3(w)))
+
+
+def rb_decide_collect(ctx, assignment, B):
+    """Waits for the oldest submitted decision and copies its assignment into the HOST buffer `assignment`."""
+    i32 = torch.int32 if torch else np.int32
+    _check(ctx, _lib.rb_decide_collect(ctx, _ptr(assignment, i32), B))
 
 
 def rb_decide_from_predictions(ctx, quality, outlen, prompt_len, B, w, commit, assignment, scores=None, scores0=None,

@@ -85,6 +85,17 @@ struct rb_ctx {
   uint8_t* d_zc = nullptr;          // the same block as the device addresses it
   size_t zc_query_cap = 0, zc_off_plen = 0, zc_off_budget = 0, zc_off_assign = 0, zc_off_flag = 0;
   uint32_t done_seq = 0;
+  // rb_decide_submit / rb_decide_collect: one pinned block per buffer set ([query | plen | assignment | completion word],
+  // at most 128 requests) and what is in flight in it
+  struct AsyncSlot {
+    uint8_t *h = nullptr, *d = nullptr;
+    bool busy = false;
+    uint32_t seq = 0;
+    int B = 0;
+  } async[2];
+  size_t az_off_plen = 0, az_off_assign = 0, az_off_flag = 0;
+  uint64_t async_head = 0;            // submissions collected so far (the oldest in flight is async[head & 1])
+  uint64_t async_tail = 0;            // submissions made so far
   // boosted TPOT head (latency_mode 2)
   int4* f_nodes = nullptr;
   int32_t *f_root = nullptr, *f_begin = nullptr;
@@ -684,6 +695,8 @@ rb_status rb_create(rb_ctx** out, const void* bank_emb, const float* bank_qualit
     } else {   // no mapped pinned memory: host callers go through the copy engine
       cudaGetLastError();
       if (ctx->h_zc) cudaFreeHost(ctx->h_zc);
+  for (auto& A : ctx->async)
+    if (A.h) cudaFreeHost(A.h);
       ctx->h_zc = nullptr;
       ctx->d_zc = nullptr;
     }
@@ -807,6 +820,21 @@ rb_status rb_create(rb_ctx** out, const void* bank_emb, const float* bank_qualit
       for (int j = 0; j < 2; ++j) {
         CK(cudaEventCreateWithFlags(&ctx->slot[j].ev_front, cudaEventDisableTiming));
         CK(cudaEventCreateWithFlags(&ctx->slot[j].ev_back, cudaEventDisableTiming));
+      }
+      // pinned blocks of the asynchronous host path
+      ctx->az_off_plen = ((size_t)kTileM * d * 4 + 255) & ~(size_t)255;
+      ctx->az_off_assign = ctx->az_off_plen + 512;
+      ctx->az_off_flag = ctx->az_off_assign + 512;
+      for (int j = 0; j < 2; ++j) {
+        rb_ctx::AsyncSlot& A = ctx->async[j];
+        if (cudaHostAlloc((void**)&A.h, ctx->az_off_flag + 256, cudaHostAllocMapped) != cudaSuccess ||
+            cudaHostGetDevicePointer((void**)&A.d, A.h, 0) != cudaSuccess) {
+          cudaGetLastError();
+          if (A.h) cudaFreeHost(A.h);
+          A.h = A.d = nullptr;   // no mapped pinned memory: rb_decide_submit returns RB_EUNSUPPORTED
+        } else {
+          std::memset(A.h, 0, ctx->az_off_flag + 256);
+        }
       }
     }
     CK(scan_tc_prepare());
@@ -1103,6 +1131,73 @@ rb_status rb_decide_budgeted(rb_ctx* ctx, const float* query_emb, const int32_t*
   return sg.finish();
 }
 
+rb_status rb_decide_submit(rb_ctx* ctx, const float* query_emb, const int32_t* prompt_len, int32_t B, const float w[3]) {
+  if (!ctx) return RB_EINVAL;
+  if (ctx->I == 0) return fail(ctx, RB_ESTATE, "rb_decide_submit before rb_set_instances");
+  if (!ctx->front) return fail(ctx, RB_ESTATE, "rb_decide_submit needs rb_options.pipeline = 1");
+  if (ctx->opt.latency_mode == 2 || !ctx->opt.use_graph || ctx->stage_timing)
+    return fail(ctx, RB_EUNSUPPORTED, "rb_decide_submit: linear or static latency head, graph replay on, stage timing off");
+  if (!query_emb || !prompt_len) return fail(ctx, RB_EINVAL, "NULL argument");
+  if (B < 1 || B > kTileM || B > ctx->opt.max_batch) return fail(ctx, RB_EINVAL, "B out of range [1, min(128, max_batch)]");
+  rb_status st = check_weights(ctx, w);
+  if (st != RB_OK) return st;
+  if (ctx->async_tail - ctx->async_head >= 2) return fail(ctx, RB_ESTATE, "two decisions in flight: rb_decide_collect first");
+  // the buffer set the next pipelined decision uses decides the pinned block
+  rb_ctx::AsyncSlot& A = ctx->async[ctx->pipe_seq & 1];
+  if (!A.h) return fail(ctx, RB_EUNSUPPORTED, "no mapped pinned host memory");
+  if (A.busy) return fail(ctx, RB_ESTATE, "the buffer set of this submission is still in flight: rb_decide_collect first");
+  std::memcpy(A.h, query_emb, (size_t)B * ctx->d * 4);
+  std::memcpy(A.h + ctx->az_off_plen, prompt_len, (size_t)B * 4);
+  CallParams cp{};
+  cp.w_qual = w[0]; cp.w_lat = w[1]; cp.w_cost = w[2]; cp.commit = 1;
+  cp.n_adv = ctx->n_pending;
+  for (int a = 0; a < ctx->n_pending; ++a) cp.adv_ms[a] = ctx->pending_adv[a];
+  cp.query = reinterpret_cast<const float*>(A.d);
+  cp.plen = reinterpret_cast<const int32_t*>(A.d + ctx->az_off_plen);
+  cp.assignment = reinterpret_cast<int32_t*>(A.d + ctx->az_off_assign);
+  cp.done_flag = reinterpret_cast<uint32_t*>(A.d + ctx->az_off_flag);
+  cp.done_seq = ++ctx->done_seq;
+  const rb_ctx::Slot& S = ctx->slot[ctx->pipe_seq & 1];
+  cp.q_src = S.pred_q;
+  cp.l_src = S.pred_l;
+  st = push_params(ctx, cp);
+  if (st != RB_OK) return st;
+  st = run_pipelined(ctx, B);
+  if (st != RB_OK) return st;
+  ctx->n_pending = 0;
+  A.busy = true;
+  A.seq = cp.done_seq;
+  A.B = B;
+  ctx->async_tail += 1;
+  return RB_OK;
+}
+
+rb_status rb_decide_collect(rb_ctx* ctx, int32_t* assignment, int32_t B) {
+  if (!ctx) return RB_EINVAL;
+  if (!assignment) return fail(ctx, RB_EINVAL, "NULL argument");
+  if (ctx->async_tail == ctx->async_head) return fail(ctx, RB_ESTATE, "rb_decide_collect: nothing in flight");
+  // submissions alternate between the two blocks in submission order, unless synchronous pipelined calls came in
+  // between: the oldest one in flight is the busy block with the smaller sequence number
+  rb_ctx::AsyncSlot* A = nullptr;
+  for (auto& c : ctx->async)
+    if (c.busy && (!A || (int32_t)(c.seq - A->seq) < 0)) A = &c;
+  if (!A) return fail(ctx, RB_ESTATE, "rb_decide_collect: nothing in flight");
+  if (B != A->B) return fail(ctx, RB_EINVAL, "rb_decide_collect: B differs from the submitted batch");
+  volatile uint32_t* flag = reinterpret_cast<volatile uint32_t*>(A->h + ctx->az_off_flag);
+  for (uint32_t spins = 1; *flag != A->seq; ++spins) {
+    if ((spins & 0x3fff) == 0) {
+      const cudaError_t q = cudaStreamQuery(ctx->stream);
+      if (q == cudaSuccess) break;
+      if (q != cudaErrorNotReady) return fail(ctx, RB_ECUDA, "cudaStreamQuery", q);
+    }
+  }
+  if (*flag != A->seq) CK(cudaStreamSynchronize(ctx->stream));
+  std::memcpy(assignment, A->h + ctx->az_off_assign, (size_t)B * 4);
+  A->busy = false;
+  ctx->async_head += 1;
+  return RB_OK;
+}
+
 rb_status rb_estimate(rb_ctx* ctx, const float* query_emb, int32_t B, float* pred_quality, float* pred_outlen,
                       int32_t* nn_idx, float* nn_sim) {
   if (!ctx) return RB_EINVAL;
@@ -1384,6 +1479,8 @@ void rb_destroy(rb_ctx* ctx) {
   for (auto& e : ctx->ev)
     if (e) cudaEventDestroy(e);
   if (ctx->h_zc) cudaFreeHost(ctx->h_zc);
+  for (auto& A : ctx->async)
+    if (A.h) cudaFreeHost(A.h);
   if (ctx->own_stream) cudaStreamDestroy(ctx->stream);
   delete ctx;
 }

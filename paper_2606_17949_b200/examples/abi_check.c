@@ -34,6 +34,7 @@ int main(void) {
     if (rb_decide(NULL, dummy, a, 1, w, a, NULL, NULL, NULL, NULL, NULL) != RB_EINVAL) return 9;
     if (rb_advance_state(NULL, 1.0f) != RB_EINVAL) return 10;
     if (rb_batch_target(NULL, 4, 64, a, NULL) != RB_EINVAL) return 14;
+    if (rb_decide_submit(NULL, dummy, a, 1, w) != RB_EINVAL || rb_decide_collect(NULL, a, 1) != RB_EINVAL) return 15;
     if (rb_sweep_weights(NULL, dummy, dummy, a, NULL, 1, w, 1, a) != RB_EINVAL) return 13;
     if (rb_launch_count(NULL) != 0) return 11;
     if (strcmp(rb_last_error(NULL), "null context") != 0) return 12;

@@ -1054,3 +1054,51 @@ def test_pipelined_decisions_equal_unpipelined_ones(orc):
     s = rt.get_state()
     assert np.array_equal(s[0].numpy(), dq) and np.array_equal(s[1].numpy(), bq)
     rt.close()
+
+
+def test_submit_collect_equals_synchronous_decisions(orc):
+    """rb_decide_submit / rb_decide_collect (two decisions in flight from host buffers): the assignments and the final
+    state of 200 decisions with rb_advance_state in between equal those of synchronous rb_decide calls on an unpipelined
+    context; call-order errors are reported (third submission, collect with nothing in flight, wrong batch size)."""
+    from paper_2606_17949_b200 import binding as rb
+    cfg = dataclasses.replace(synth.CONFIGS["C2"], N=30000, d=256, Kc=16, seed=71)
+    bank = synth.make_bank(cfg, device="cuda")
+    it = synth.make_instances(cfg.I, cfg.M, cap=6)
+    queued, running = synth.make_state(cfg.I, it["cap"], cfg.seed)
+    rng = np.random.default_rng(71)
+    sizes = [int(x) for x in rng.integers(1, 65, 200)]
+    offs = np.concatenate([[0], np.cumsum(sizes)])
+    q = synth.make_queries(cfg, B=int(offs[-1]), device="cpu").pin_memory()
+    p = synth.make_prompt_len(cfg, B=int(offs[-1]), device="cpu").pin_memory()
+    torch.cuda.synchronize()
+    presets = list(synth.PRESETS.values())
+    ref_rt = _router(bank, cfg, max_batch=64)
+    ref_rt.set_instances(**it)
+    ref_rt.set_state(queued, running)
+    ref = torch.empty(int(offs[-1]), dtype=torch.int32)
+    for j, B in enumerate(sizes):
+        ref_rt.advance_state(float(2.0 + j % 5))
+        rb.rb_decide(ref_rt.ctx, q[offs[j]:offs[j + 1]], p[offs[j]:offs[j + 1]], B, presets[j % 4], ref[offs[j]:offs[j + 1]])
+    ref_state = ref_rt.get_state()
+    ref_rt.close()
+    rt = _router(bank, cfg, max_batch=64, pipeline=1)
+    rt.set_instances(**it)
+    rt.set_state(queued, running)
+    got = torch.empty(int(offs[-1]), dtype=torch.int32)
+    with pytest.raises(rb.RbError):
+        rb.rb_decide_collect(rt.ctx, got[:1], 1)                       # nothing in flight
+    for j, B in enumerate(sizes):
+        rt.advance_state(float(2.0 + j % 5))
+        rb.rb_decide_submit(rt.ctx, q[offs[j]:offs[j + 1]], p[offs[j]:offs[j + 1]], B, presets[j % 4])
+        if j == 1:
+            with pytest.raises(rb.RbError):                            # two in flight: a third is refused, nothing changes
+                rb.rb_decide_submit(rt.ctx, q[:1], p[:1], 1, presets[0])
+            with pytest.raises(rb.RbError):
+                rb.rb_decide_collect(rt.ctx, got[:sizes[0] + 1], sizes[0] + 1)   # not the submitted batch size
+        if j >= 1:
+            rb.rb_decide_collect(rt.ctx, got[offs[j - 1]:offs[j]], sizes[j - 1])
+    rb.rb_decide_collect(rt.ctx, got[offs[-2]:offs[-1]], sizes[-1])
+    assert torch.equal(got, ref)
+    s = rt.get_state()
+    assert torch.equal(s[0], ref_state[0]) and torch.equal(s[1], ref_state[1])
+    rt.close()
