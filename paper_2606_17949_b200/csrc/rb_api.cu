@@ -11,6 +11,7 @@
 #include <new>
 #include <string>
 #include <unordered_map>
+#include <utility>
 #include <vector>
 
 #include <cudaTypedefs.h>
@@ -98,7 +99,8 @@ struct rb_ctx {
   uint64_t async_tail = 0;            // submissions made so far
   // boosted TPOT head (latency_mode 2)
   int4* f_nodes = nullptr;
-  int32_t *f_root = nullptr, *f_begin = nullptr;
+  int32_t *f_root = nullptr, *f_begin = nullptr, *f_nbegin = nullptr;   // roots, trees per tier, nodes per tier
+  int f_max_tier_nodes = 0;
   float *f_base = nullptr, *f_aux = nullptr, *f_tpot0 = nullptr;
   int f_features = 0;
   bool has_forest = false;
@@ -180,7 +182,7 @@ DispatchModes modes_of(const rb_ctx* c) {
 ForestDev forest_of(const rb_ctx* c) {
   ForestDev f{};
   f.nodes = c->f_nodes; f.tree_root = c->f_root; f.tier_begin = c->f_begin; f.base = c->f_base; f.aux = c->f_aux;
-  f.tpot0 = c->f_tpot0; f.n_features = c->f_features;
+  f.tpot0 = c->f_tpot0; f.n_features = c->f_features; f.tier_node_begin = c->f_nbegin; f.max_tier_nodes = c->f_max_tier_nodes;
   return f;
 }
 
@@ -949,20 +951,53 @@ rb_status rb_set_tpot_forest(rb_ctx* ctx, const rb_tree_node* nodes, int32_t n_n
     if (nodes[n].left <= n || nodes[n].left >= n_nodes || nodes[n].right <= n || nodes[n].right >= n_nodes)
       return fail(ctx, RB_EINVAL, "node children must lie after their parent and inside the node array");
   }
+  // The nodes are stored tier by tier (each tree copied out in pre-order, child links re-pointed): the dispatch kernel
+  // keeps the nodes of the tier it is evaluating in shared memory (a walk is then a chain of shared-memory reads, not of
+  // L2 round trips).  Pure re-arrangement of the caller's forest: every walk visits the same tests and the same leaf.
+  std::vector<rb_tree_node> pk;
+  std::vector<int32_t> root2((size_t)n_trees), nbegin((size_t)M + 1, 0);
+  pk.reserve((size_t)n_nodes);
+  int max_tier_nodes = 0;
+  for (int m = 0; m < M; ++m) {
+    nbegin[m] = (int32_t)pk.size();
+    for (int tr = tier_tree_begin[m]; tr < tier_tree_begin[m + 1]; ++tr) {
+      std::vector<std::pair<int32_t, int32_t>> todo;   // (old node, slot of the link to patch; -1: the root)
+      todo.push_back({tree_root[tr], -1});
+      while (!todo.empty()) {
+        const auto [old, link] = todo.back();
+        todo.pop_back();
+        const int32_t id = (int32_t)pk.size();
+        if (pk.size() >= ((size_t)1 << 23)) return fail(ctx, RB_EINVAL, "forest too large once its trees are unshared");
+        pk.push_back(nodes[old]);
+        if (link < 0) root2[tr] = id;
+        else if (link & 1) pk[link >> 1].right = id;
+        else pk[link >> 1].left = id;
+        if (nodes[old].feature >= 0) {
+          todo.push_back({nodes[old].right, 2 * id + 1});
+          todo.push_back({nodes[old].left, 2 * id});
+        }
+      }
+    }
+    max_tier_nodes = std::max(max_tier_nodes, (int)pk.size() - nbegin[m]);
+  }
+  nbegin[M] = (int32_t)pk.size();
   cudaStream_t s = ctx->stream;
   CK(cudaStreamSynchronize(s));
-  cudaFree(ctx->f_nodes); cudaFree(ctx->f_root); cudaFree(ctx->f_begin); cudaFree(ctx->f_base);
-  ctx->f_nodes = nullptr; ctx->f_root = ctx->f_begin = nullptr; ctx->f_base = nullptr;
+  cudaFree(ctx->f_nodes); cudaFree(ctx->f_root); cudaFree(ctx->f_begin); cudaFree(ctx->f_base); cudaFree(ctx->f_nbegin);
+  ctx->f_nodes = nullptr; ctx->f_root = ctx->f_begin = ctx->f_nbegin = nullptr; ctx->f_base = nullptr;
+  ctx->f_max_tier_nodes = max_tier_nodes;
   ctx->has_forest = false;
   static_assert(sizeof(rb_tree_node) == sizeof(int4), "rb_tree_node is read as int4");
-  if (dev_alloc(&ctx->f_nodes, (size_t)n_nodes) != cudaSuccess || dev_alloc(&ctx->f_root, (size_t)n_trees) != cudaSuccess ||
-      dev_alloc(&ctx->f_begin, (size_t)M + 1) != cudaSuccess || dev_alloc(&ctx->f_base, (size_t)M) != cudaSuccess) {
+  if (dev_alloc(&ctx->f_nodes, pk.size()) != cudaSuccess || dev_alloc(&ctx->f_root, (size_t)n_trees) != cudaSuccess ||
+      dev_alloc(&ctx->f_begin, (size_t)M + 1) != cudaSuccess || dev_alloc(&ctx->f_base, (size_t)M) != cudaSuccess ||
+      dev_alloc(&ctx->f_nbegin, (size_t)M + 1) != cudaSuccess) {
     cudaGetLastError();
     return fail(ctx, RB_ENOMEM, "cudaMalloc forest");
   }
-  CK(cudaMemcpyAsync(ctx->f_nodes, nodes, (size_t)n_nodes * sizeof(rb_tree_node), cudaMemcpyHostToDevice, s));
-  CK(cudaMemcpyAsync(ctx->f_root, tree_root, (size_t)n_trees * 4, cudaMemcpyHostToDevice, s));
+  CK(cudaMemcpyAsync(ctx->f_nodes, pk.data(), pk.size() * sizeof(rb_tree_node), cudaMemcpyHostToDevice, s));
+  CK(cudaMemcpyAsync(ctx->f_root, root2.data(), (size_t)n_trees * 4, cudaMemcpyHostToDevice, s));
   CK(cudaMemcpyAsync(ctx->f_begin, tier_tree_begin, (size_t)(M + 1) * 4, cudaMemcpyHostToDevice, s));
+  CK(cudaMemcpyAsync(ctx->f_nbegin, nbegin.data(), (size_t)(M + 1) * 4, cudaMemcpyHostToDevice, s));
   CK(cudaMemcpyAsync(ctx->f_base, base, (size_t)M * 4, cudaMemcpyHostToDevice, s));
   CK(cudaStreamSynchronize(s));
   if (n_features != ctx->f_features) CK(cudaMemsetAsync(ctx->f_aux, 0, (size_t)kMaxI * kMaxFeatures * 4, s));
@@ -1467,7 +1502,7 @@ void rb_destroy(rb_ctx* ctx) {
   drop_graphs(ctx);
   void* ptrs[] = {ctx->bank, ctx->bank_quality, ctx->bank_outlen, ctx->arena, ctx->q32, ctx->q32_in, ctx->qs, ctx->part_sim,
                   ctx->gthr, ctx->bank32, ctx->scratch_nn_idx, ctx->scratch_nn_sim, ctx->scores, ctx->scores0, ctx->f_nodes,
-                  ctx->f_root, ctx->f_begin, ctx->f_base, ctx->dev_clock, ctx->sweep_buf};
+                  ctx->f_root, ctx->f_begin, ctx->f_nbegin, ctx->f_base, ctx->dev_clock, ctx->sweep_buf};
   for (void* p : ptrs) cudaFree(p);
   cudaFree(ctx->slot[1].qs);
   cudaFree(ctx->slot[1].part_sim);

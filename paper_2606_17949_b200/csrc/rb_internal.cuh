@@ -35,7 +35,9 @@ struct InstTable {
 constexpr int kMaxTreesPerTier = 256;
 constexpr int kMaxFeatures = 8;
 struct ForestDev {
-  const int4* nodes;           // (feature, value bits, left, right); feature < 0: leaf
+  const int4* nodes;           // (feature, value bits, left, right); feature < 0: leaf.  Stored tier by tier:
+  const int32_t* tier_node_begin;   // [M+1] tier t's nodes are nodes[tier_node_begin[t] .. tier_node_begin[t+1])
+  int32_t max_tier_nodes;      // the largest tier's node count (shared-memory cache sizing)
   const int32_t* tree_root;    // [n_trees]
   const int32_t* tier_begin;   // [M+1]
   const float* base;           // [M]
