@@ -68,6 +68,7 @@ def parse_args(argv=None):
     ap.add_argument("--no-scan-c4", action="store_true", help="skip the C4 (10M x 384) bank-scan roofline leg")
     ap.add_argument("--only-scan-c4", action="store_true", help="run only the C4 bank-scan leg (profiling runs)")
     ap.add_argument("--c4-batch", type=int, default=64, help="B of the --only-scan-c4 leg (1..4096)")
+    ap.add_argument("--c4-k", type=int, default=10, help="k of the --only-scan-c4 leg (10 or 32; slack 6 / 8)")
     ap.add_argument("--only-scan-c3", action="store_true", help="run only the C3 tensor-bound scan leg (profiling runs)")
     ap.add_argument("--only-sweep-c5", action="store_true", help="run only the C5 weight-sweep leg (profiling runs)")
     ap.add_argument("--no-large", action="store_true", help="skip the C3 (tensor-bound scan) and C5 (weight sweep) legs")
@@ -236,7 +237,7 @@ def run_ours(args):
     torch.cuda.set_device(dev)
 
     if args.only_scan_c4:
-        out = scan_c4(synth, Router, dev, measured_peaks()[0], B=args.c4_batch)
+        out = scan_c4(synth, Router, dev, measured_peaks()[0], B=args.c4_batch, k=args.c4_k)
         print(json.dumps(out))
         return out
     if args.only_scan_c3:
@@ -671,14 +672,15 @@ def small_configs(synth, Router, rb, dev):
     return out
 
 
-def scan_c4(synth, Router, dev, hbm_peak, B=64):
+def scan_c4(synth, Router, dev, hbm_peak, B=64, k=10):
     """BASELINE.json configs[3]: N=10M x d=384 bf16 bank (7.68 GB >> L2), B=64 (or --c4-batch), k=10: the scan kernel alone."""
     import torch
     cfg = synth.CONFIGS["C4"]
     bank = synth.make_bank(cfg, device=dev)
     q = synth.make_queries(cfg, B=B, device=dev)
     torch.cuda.synchronize()
-    rt = Router(bank["emb"], bank["quality"], bank["outlen"], cfg.k, store="bf16", max_batch=max(B, 64), device=dev)
+    rt = Router(bank["emb"], bank["quality"], bank["outlen"], k, store="bf16", max_batch=max(B, 64), device=dev,
+                rerank_slack=6 if k <= 16 else 8)
     for _ in range(3):
         rt.estimate(q)
     rt.sync()
@@ -692,7 +694,7 @@ def scan_c4(synth, Router, dev, hbm_peak, B=64):
     t = float(np.mean(us))
     nbytes = cfg.N * cfg.d * 2 + B * cfg.d * 2
     ach = nbytes / (t * 1e-6) / 1e9
-    return {"workload": "C4 N=10M d=384 bf16 B=%d k=10" % B, "kernel": "scan_tc_kernel" if B <= 128 else "scan_tc2_kernel",
+    return {"workload": "C4 N=10M d=384 bf16 B=%d k=%d" % (B, k), "kernel": "scan_tc_kernel" if B <= 128 else "scan_tc2_kernel",
             "tflops": round(2.0 * B * cfg.N * cfg.d / (t * 1e-6) / 1e12, 1), "launch_us": round(t, 1),
             "bytes_per_launch": int(nbytes), "achieved": round(ach, 1), "unit": "GB/s", "peak": hbm_peak,
             "frac": round(ach / hbm_peak, 4), "frac_of_nominal_8TBs": round(ach / 8000.0, 4),
