@@ -261,7 +261,7 @@ __device__ __forceinline__ void finish_query(const FinishArgs& a, const InstTabl
   // ---- load: lists -> keys in shared memory; every thread remembers the best similarity it has seen ----
   uint32_t tmax = 0u;
   const bool quads = a.records != 0;   // query-major records of 4 ready-made keys (scan_tc.cu): one item = one quad
-  const int step = quads ? 4 : 1, nitems = total / step;
+  const int step = quads ? 4 : 1, nitems = quads ? total >> 2 : total;
   if (quads) {
     const uint4* rec = reinterpret_cast<const uint4*>(a.part_sim) + (size_t)r * nitems * 2;
     uint4* dst = reinterpret_cast<uint4*>(s_keys);
@@ -283,17 +283,18 @@ __device__ __forceinline__ void finish_query(const FinishArgs& a, const InstTabl
       tmax = max(tmax, (uint32_t)(key >> 32));
     }
   }
-  // ---- bound: the threads that hold entries form groups of 8 lanes (fewer lanes while that leaves under 2 kc
-  // groups); the kc-th largest group maximum is reached by kc distinct entries, so every member of the kc best
-  // reaches it too.  With ~32 entries per group about kc + 4 entries survive.  The groups are ranked by counting: the
+  // ---- bound: the threads that hold entries form groups of adjacent lanes, as coarse as still leaves 2 kc groups;
+  // the kc-th largest group maximum is reached by kc distinct entries, so every member of the kc best reaches it
+  // too.  About kc + 6 entries survive.  The groups are ranked by counting: the
   // lanes of a group share its G comparisons and add their counts up by shuffles. ----
   const int nact = min(nthreads, nitems);   // threads that loaded something
-  int glanes = 8;
-  while (glanes > 1 && (nact + glanes - 1) / glanes < 2 * kc) glanes >>= 1;
+  int gshift = 5;   // groups of 2^gshift lanes: the coarsest that still leaves 2 kc groups
+  while (gshift > 0 && ((nact + (1 << gshift) - 1) >> gshift) < 2 * kc) --gshift;
+  const int glanes = 1 << gshift;
   for (int o = 1; o < glanes; o <<= 1) tmax = max(tmax, __shfl_xor_sync(0xffffffffu, tmax, o));
-  const int ngroups = (nact + glanes - 1) / glanes;   // <= kFinThreadsMax
+  const int ngroups = (nact + glanes - 1) >> gshift;   // <= kFinThreadsMax
   const bool bounded = ngroups >= kc && total > kSurvMax;   // (a small input is ranked whole)
-  const int g = tid / glanes;
+  const int g = tid >> gshift;
   if ((tid & (glanes - 1)) == 0 && g < ngroups) S.gmax[g] = tmax;
   __syncthreads();
   if (bounded) {
@@ -343,9 +344,10 @@ __device__ __forceinline__ void finish_query(const FinishArgs& a, const InstTabl
   const int nsurv = S.nsurv;
   if (nsurv <= kSurvMax) {
     // rank by counting (keys are distinct): `sl` adjacent lanes share the comparisons of one survivor
-    int sl = 32;
-    while (sl > 1 && nsurv * sl > nthreads) sl >>= 1;
-    const int c = tid / sl, s = tid & (sl - 1);
+    int sshift = 5;
+    while (sshift > 0 && (nsurv << sshift) > nthreads) --sshift;
+    const int sl = 1 << sshift;
+    const int c = tid >> sshift, s = tid & (sl - 1);
     const unsigned long long mine = c < nsurv ? S.surv[c] : 0ull;
     int ahead = 0;
     if (c < nsurv) {
