@@ -282,10 +282,11 @@ rb_status enqueue_estimate(rb_ctx* ctx, int B, bool with_terms, Timer& tm, int s
       // tensor-bound regime: CTA pairs, 256-query m-tiles
       const int Bpad2 = (B + 2 * kTileM - 1) / (2 * kTileM) * (2 * kTileM);
       const int ncl = scan_tc2_clusters(ctx->N, ctx->num_sms);
-      // lists of at most 16 entries per (cluster, query): longer ones put the sorted insertions (in global memory) on the
-      // tensor pipe's time line (k = 32: 0.54 of the tensor roofline with 64-entry lists); a cluster whose list is
-      // popped completely is searched again by the finishing kernel, as for the single-CTA scan
-      const int kcap2 = std::min(ctx->kcap, 16);
+      // lists of at most 32 entries per (cluster, query): 64-entry lists put the sorted insertions (in global memory) on
+      // the tensor pipe's time line (k = 32: 0.54 of the tensor roofline), 16-entry ones under k + slack = 40 weaken the
+      // pooled admission bound (0.69 against 0.74 with 32, C4 at B = 512 and 4096); a cluster whose list is popped
+      // completely is searched again by the finishing kernel, as for the single-CTA scan
+      const int kcap2 = std::min(ctx->kcap, 32);
       if (front) {
         CK(launch_stage_queries(ctx->cp_cur, S.qs, B, Bpad2, ctx->d, 1, ctx->gthr, Bpad2 * (1 + ncl), split, ctx->q32, s));
         tm.mark();

@@ -109,7 +109,7 @@ def test_bf16_pair_scan_large_batches(orc, N, d, B, k, slack):
 def test_bf16_pair_scan_long_slabs_all_queries(orc, k, slack, sort_bank):
     """The CTA-pair scan in its long-slab regime, every query checked: N = 256 * 74 * 41 + 77 rows (41-42 tiles of 256
     rows per cluster), B = 700 (three 256-query m-pairs, the last one ragged), k = 32 with slack 8 (candidate lists of
-    40 against the scan's 16-entry global lists: pooled cross-slab admission bounds, list caps and the finishing
+    40 against the scan's 32-entry global lists: pooled cross-slab admission bounds, list caps and the finishing
     kernel's re-search of a popped-out slab all take part) and k = 10; on the bank as drawn and on the bank sorted by
     mixture component (all of a query's neighbours in one or two clusters' slabs -- the re-search is certain)."""
     cfg = dataclasses.replace(synth.CONFIGS["C2"], N=256 * 74 * 41 + 77, d=64, B=700, k=k, Kc=24, seed=41)
