@@ -123,7 +123,7 @@ def read_only_peak_gbs(rt, rb):
     return rb.rb_testing_read_bandwidth(rt.ctx, 2 << 30, 10)
 
 
-def c_harness_e2e(N, d, B, I, steps=300):
+def c_harness_e2e(N, d, B, I, steps=300, pipeline=0):
     """examples/e2e_bench.c: rb_advance_state + rb_decide from host buffers through the C ABI, no Python on the path."""
     import subprocess
     import tempfile
@@ -132,7 +132,7 @@ def c_harness_e2e(N, d, B, I, steps=300):
     try:
         subprocess.run(["gcc", "-std=c99", "-O2", "-I", os.path.join(ROOT, "include"), os.path.join(pkg, "examples", "e2e_bench.c"),
                         "-o", exe, "-L", pkg, "-lrouteb", "-lm", "-Wl,-rpath," + pkg], check=True, capture_output=True)
-        r = subprocess.run([exe, str(N), str(d), str(B), str(I), str(steps)], capture_output=True, text=True, timeout=300)
+        r = subprocess.run([exe, str(N), str(d), str(B), str(I), str(steps), str(pipeline)], capture_output=True, text=True, timeout=300)
         return json.loads(r.stdout.strip().splitlines()[-1])
     except Exception as e:   # reported, never fatal for the bench line
         return {"error": repr(e)[:200]}
@@ -470,7 +470,8 @@ def run_ours(args):
         rt.close()
         del bank, rt, flush_buf
         torch.cuda.empty_cache()
-        out["e2e"]["c_harness"] = c_harness_e2e(cfg.N, cfg.d, 12, cfg.I)
+        out["e2e"]["c_harness"] = {"synchronous": c_harness_e2e(cfg.N, cfg.d, 12, cfg.I),
+                                   "two_in_flight": c_harness_e2e(cfg.N, cfg.d, 12, cfg.I, pipeline=1)}
         torch.cuda.empty_cache()
         if not args.skip_cpu:
             per_config.update(small_configs(synth, Router, rb, dev))
