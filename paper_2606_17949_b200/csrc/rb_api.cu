@@ -108,7 +108,7 @@ struct rb_ctx {
   float pending_adv[kMaxPendingAdvance]{};
   int n_pending = 0;
   float *scores = nullptr, *scores0 = nullptr;  // [max_batch x I], allocated by rb_set_instances
-  CUtensorMap tm_q{}, tm_bank{};
+  CUtensorMap tm_q{}, tm_bank{}, tm_bank16{};   // bank: 64-row boxes; the same with 16-row boxes
   // graphs: key = B * 8 + kind (0 decide, 1 estimate, 2 from_predictions) + 4 if stage timing is on
   // One captured graph per decision shape.  The per-call parameters are an argument of the kernels that need them; a
   // replay rewrites that one argument of those kernel nodes (cudaGraphExecKernelNodeSetParams) -- no transfer of any
@@ -312,14 +312,14 @@ rb_status enqueue_estimate(rb_ctx* ctx, int B, bool with_terms, Timer& tm, int s
         CK(launch_stage_queries(ctx->cp_cur, S.qs, B, Bpad, ctx->d, rep, ctx->gthr, 0, split, ctx->q32, s));
         tm.mark();
         int grid_used = 0;
-        CK(launch_scan_tc(&S.tm_q, &ctx->tm_bank, ctx->N, ctx->d_scan, B, Bpad, ctx->ks, sms, S.part_sim, S.part_idx,
+        CK(launch_scan_tc(&S.tm_q, &ctx->tm_bank, &ctx->tm_bank16, ctx->N, ctx->d_scan, B, Bpad, ctx->ks, sms, S.part_sim, S.part_idx,
                           &grid_used, ctx->stage_timing ? ctx->dev_clock : nullptr, s));
         tm.mark();
         ctx->launches += 2;
       }
       fa.part_sim = S.part_sim; fa.part_idx = S.part_idx; fa.nlists = grid * rep; fa.lists_per_cta = rep; fa.kcap = ctx->ks;
       fa.records = 1;
-      fa.Bpad = Bpad; fa.slab_unit = kBoxN;
+      fa.Bpad = Bpad; fa.slab_unit = kRowUnit;
       fa.rescan = ctx->ks < ctx->kc ? 1 : 0;
     }
     if (split) {   // exact similarities from the fp32 rows (the definition of fp32 storage), always
@@ -804,6 +804,8 @@ rb_status rb_create(rb_ctx** out, const void* bank_emb, const float* bank_qualit
     ctx->part_idx = reinterpret_cast<int32_t*>(ctx->part_sim + part_n);
     CK(cudaMemsetAsync(ctx->qs, 0, (size_t)ctx->Bpad_max * ds * 2, s));
     rb_status st = encode_map(ctx, &ctx->tm_bank, ctx->bank, (uint64_t)N, (uint64_t)ds, kBoxN);
+    if (st != RB_OK) return st;
+    st = encode_map(ctx, &ctx->tm_bank16, ctx->bank, (uint64_t)N, (uint64_t)ds, kRowUnit);
     if (st != RB_OK) return st;
     st = encode_map(ctx, &ctx->tm_q, ctx->qs, (uint64_t)ctx->Bpad_max, (uint64_t)ds, kTileM);
     if (st != RB_OK) return st;

@@ -12,7 +12,8 @@ constexpr int kMaxM = 16;          // model tiers
 constexpr int kMaxI = 1024;        // instances
 constexpr int kTileM = 128;        // queries per MMA tile (TMEM lanes)
 constexpr int kTileN = 256;        // bank rows per MMA tile (TMEM columns of one accumulator)
-constexpr int kBoxN = 64;          // bank rows per TMA box; slabs are multiples of this
+constexpr int kBoxN = 64;          // bank rows per TMA box
+constexpr int kRowUnit = 16;       // the single-CTA scan splits the bank over its CTAs in groups of this many rows
 constexpr int kTileK = 64;         // bf16 per K chunk = one 128-byte swizzle row
 constexpr int kMaxPendingAdvance = 4;   // rb_advance_state calls a decision can absorb (CallParams::adv_ms)
 
@@ -234,8 +235,9 @@ int scan_tc_replicas(int B, int kcap, int max_grid);
 // a1 (bf16): tcgen05 scan.  The lists (sim fp32 / idx int32, idx -1 = empty, each sorted by (sim desc, idx asc)) are
 // written through part_sim as QUERY-MAJOR 32-byte records: record ((r * nlists + list) * KCAP/4 + quad) =
 // [4 similarities | 4 indices], nlists = grid * rep; part_sim must have room for nlists * Bpad * KCAP * 8 bytes.  Returns the grid size used through *grid_out.  kcap in {4,8,16,32,64}; bank
-// rows are split over the CTAs in units of kBoxN rows: CTA c owns units [units*c/grid, units*(c+1)/grid).
-cudaError_t launch_scan_tc(const CUtensorMap* tm_q, const CUtensorMap* tm_bank, int64_t N, int d, int B, int Bpad,
+// rows are split over the CTAs in units of kRowUnit rows: CTA c owns units [units*c/grid, units*(c+1)/grid);
+// tm_bank16: the bank again with 16-row boxes (the remainder of a CTA's last tile).
+cudaError_t launch_scan_tc(const CUtensorMap* tm_q, const CUtensorMap* tm_bank, const CUtensorMap* tm_bank16, int64_t N, int d, int B, int Bpad,
                            int kcap, int max_grid, float* part_sim, int32_t* part_idx, int* grid_out,
                            unsigned long long* dev_clock /* NULL, or [2] = {~0, 0}: earliest CTA start / latest CTA end (globaltimer ns) */,
                            cudaStream_t s);

@@ -36,8 +36,8 @@ constexpr int kSmemBytes = kStages * kStageBytes + kCandSlots * kTileM * 8 + 256
 
 template <int KCAP>
 __global__ void __launch_bounds__(kThreads, 1)
-scan_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_bank, int64_t N, int d,
-               int B, int Bpad, int rep, float* __restrict__ part_sim, int32_t* __restrict__ part_idx,
+scan_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_bank,
+               const __grid_constant__ CUtensorMap tm_bank16, int64_t N, int d, int B, int Bpad, int rep, float* __restrict__ part_sim, int32_t* __restrict__ part_idx,
                unsigned long long* __restrict__ dev_clock) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);   // 128B swizzle wants 1024 B alignment
@@ -52,12 +52,15 @@ scan_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int n_mt = Bpad / kTileM;
   const int nk = (d + kTileK - 1) / kTileK;
-  const int64_t units = (N + kBoxN - 1) / kBoxN;
+  // This CTA's rows: the bank is split in groups of kRowUnit = 16 rows (what the MMA's N and the 16-row boxes of tm_bank16
+  // resolve), so the CTAs' shares differ by at most 16 rows -- with 64-row units C2 gave 83 CTAs 11 units and 65 CTAs 10,
+  // and the last 10 % of the stream ran on 56 % of the SMs (CTA ends spread over 3.7 us of 24).
+  const int64_t units = (N + kRowUnit - 1) / kRowUnit;
   const int64_t u0 = units * blockIdx.x / gridDim.x;
   const int64_t u1 = units * (blockIdx.x + 1) / gridDim.x;
-  const int nunits = (int)(u1 - u0);
-  const int64_t row0 = u0 * kBoxN;
-  const int ntiles = (nunits + 3) / 4;
+  const int nrows = (int)(u1 - u0) * kRowUnit;
+  const int64_t row0 = u0 * kRowUnit;
+  const int ntiles = (nrows + kTileN - 1) / kTileN;
 
   launch_dependents();
   if (dev_clock != nullptr && threadIdx.x == 0) {   // stage-timing mode: earliest CTA start on the device's own clock
@@ -68,6 +71,7 @@ scan_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__
   if (warp == 0 && lane == 0) {
     asm volatile("prefetch.tensormap [%0];" ::"l"(&tm_q) : "memory");
     asm volatile("prefetch.tensormap [%0];" ::"l"(&tm_bank) : "memory");
+    asm volatile("prefetch.tensormap [%0];" ::"l"(&tm_bank16) : "memory");
     for (int s = 0; s < kStages; ++s) {
       mbar_init(&full[s], 1);
       mbar_init(&empty[s], 1);
@@ -97,7 +101,8 @@ scan_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__
       uint32_t kit = 0;
       for (int tile = 0; tile < ntiles; ++tile) {
         const int n0 = (int)(row0 + (int64_t)tile * kTileN);
-        const int nun = min(4, nunits - tile * 4);
+        const int trows = min(kTileN, nrows - tile * kTileN);   // a multiple of 16
+        const int nun = trows / kBoxN, n16 = (trows % kBoxN) / kRowUnit;
         for (int mt = 0; mt < n_mt; ++mt) {
           for (int kc = 0; kc < nk; ++kc, ++kit) {
             const int s = kit % kStages;
@@ -105,9 +110,12 @@ scan_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__
             mbar_wait(&empty[s], ph ^ 1);
             uint8_t* sa = smem + s * kStageBytes;
             uint8_t* sb = sa + kABytes;
-            mbar_arrive_expect_tx(&full[s], kABytes + nun * kBoxBytes);
+            mbar_arrive_expect_tx(&full[s], kABytes + trows * kTileK * 2);
             tma_load_2d(sa, &tm_q, kc * kTileK, mt * kTileM, &full[s]);
             for (int u = 0; u < nun; ++u) tma_load_2d(sb + u * kBoxBytes, &tm_bank, kc * kTileK, n0 + u * kBoxN, &full[s]);
+            // (the rest of a last tile: 16-row boxes, laid out like a quarter of a 64-row box -- the swizzle repeats every 8 rows)
+            for (int u = 0; u < n16; ++u)
+              tma_load_2d(sb + nun * kBoxBytes + u * (kBoxBytes / 4), &tm_bank16, kc * kTileK, n0 + nun * kBoxN + u * kRowUnit, &full[s]);
           }
         }
       }
@@ -118,8 +126,8 @@ scan_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__
     if (lane == 0) {
       uint32_t kit = 0, it = 0;
       for (int tile = 0; tile < ntiles; ++tile) {
-        const int nun = min(4, nunits - tile * 4);
-        const uint32_t idesc = make_idesc(kTileM, nun * kBoxN);
+        const int trows = min(kTileN, nrows - tile * kTileN);
+        const uint32_t idesc = make_idesc(kTileM, trows);
         for (int mt = 0; mt < n_mt; ++mt, ++it) {
           const uint32_t acc = it & 1, aph = (it >> 1) & 1;
           mbar_wait(&tempty[acc], aph ^ 1);
@@ -154,17 +162,17 @@ scan_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__
     const int tl = quarter * 32 + lane;        // TMEM lane inside the m-tile
     const int group = kTileM / rep;            // lanes per replica
     const int replica = tl / group;
-    const int col_lo = replica * (kTileN / rep);
-    const int col_hi = col_lo + kTileN / rep;
     float v[KCAP];
     int32_t ix[KCAP];
     uint32_t it = 0;
     for (int tile = 0; tile < ntiles; ++tile) {
       const int n0 = (int)(row0 + (int64_t)tile * kTileN);
-      const int nun = min(4, nunits - tile * 4);
-      const int ncols = nun * kBoxN;
+      const int ncols = min(kTileN, nrows - tile * kTileN);
       const int nvalid = (int)min((int64_t)ncols, N - (int64_t)n0);   // rows >= N are TMA zero fill
-      const int c_end = min(col_hi, nvalid);
+      // the replicas share the tile's columns in runs of 32 (one TMEM load): a short last tile is spread over all of them
+      const int cpr = ((ncols + rep - 1) / rep + 31) & ~31;
+      const int col_lo = replica * cpr;
+      const int c_end = min(col_lo + cpr, nvalid);
       for (int mt = 0; mt < n_mt; ++mt, ++it) {
         const uint32_t acc = it & 1, aph = (it >> 1) & 1;
         const int r = mt * kTileM + (tl - replica * group);
@@ -278,7 +286,7 @@ int scan_tc_replicas(int B, int kcap, int max_grid) {
   return rep;
 }
 
-cudaError_t launch_scan_tc(const CUtensorMap* tm_q, const CUtensorMap* tm_bank, int64_t N, int d, int B, int Bpad,
+cudaError_t launch_scan_tc(const CUtensorMap* tm_q, const CUtensorMap* tm_bank, const CUtensorMap* tm_bank16, int64_t N, int d, int B, int Bpad,
                            int kcap, int max_grid, float* part_sim, int32_t* part_idx, int* grid_out,
                            unsigned long long* dev_clock, cudaStream_t s) {
   const int64_t units = (N + kBoxN - 1) / kBoxN;
@@ -287,7 +295,7 @@ cudaError_t launch_scan_tc(const CUtensorMap* tm_q, const CUtensorMap* tm_bank, 
   if (grid_out) *grid_out = grid;
   cudaError_t e = cudaSuccess;
 #define RB_SCAN_LAUNCH(KC)                                                                                          \
-  e = launch_chained(scan_tc_kernel<KC>, dim3(grid), dim3(kThreads), kSmemBytes, s, *tm_q, *tm_bank, N, d, B, Bpad, rep, \
+  e = launch_chained(scan_tc_kernel<KC>, dim3(grid), dim3(kThreads), kSmemBytes, s, *tm_q, *tm_bank, *tm_bank16, N, d, B, Bpad, rep, \
                      part_sim, part_idx, dev_clock)
   switch (kcap) {
     case 4: RB_SCAN_LAUNCH(4); break;
