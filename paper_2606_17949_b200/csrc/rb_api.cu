@@ -101,6 +101,7 @@ struct rb_ctx {
   int4* f_nodes = nullptr;
   int32_t *f_root = nullptr, *f_begin = nullptr, *f_nbegin = nullptr;   // roots, trees per tier, nodes per tier
   int f_max_tier_nodes = 0;
+  float f_tpot_hi = 0.0f;             // bound of the head's output over all states (see ForestDev)
   float *f_base = nullptr, *f_aux = nullptr, *f_tpot0 = nullptr;
   int f_features = 0;
   bool has_forest = false;
@@ -182,7 +183,7 @@ DispatchModes modes_of(const rb_ctx* c) {
 ForestDev forest_of(const rb_ctx* c) {
   ForestDev f{};
   f.nodes = c->f_nodes; f.tree_root = c->f_root; f.tier_begin = c->f_begin; f.base = c->f_base; f.aux = c->f_aux;
-  f.tpot0 = c->f_tpot0; f.n_features = c->f_features; f.tier_node_begin = c->f_nbegin; f.max_tier_nodes = c->f_max_tier_nodes;
+  f.tpot0 = c->f_tpot0; f.n_features = c->f_features; f.tier_node_begin = c->f_nbegin; f.max_tier_nodes = c->f_max_tier_nodes; f.tpot_hi = c->f_tpot_hi;
   return f;
 }
 
@@ -961,9 +962,12 @@ rb_status rb_set_tpot_forest(rb_ctx* ctx, const rb_tree_node* nodes, int32_t n_n
   std::vector<int32_t> root2((size_t)n_trees), nbegin((size_t)M + 1, 0);
   pk.reserve((size_t)n_nodes);
   int max_tier_nodes = 0;
+  double tpot_hi = 1e-6;   // |base| + sum over the tier's trees of the largest |leaf|: no evaluation exceeds it
   for (int m = 0; m < M; ++m) {
     nbegin[m] = (int32_t)pk.size();
+    double tier_hi = std::fabs((double)base[m]);
     for (int tr = tier_tree_begin[m]; tr < tier_tree_begin[m + 1]; ++tr) {
+      double leaf_hi = 0.0;
       std::vector<std::pair<int32_t, int32_t>> todo;   // (old node, slot of the link to patch; -1: the root)
       todo.push_back({tree_root[tr], -1});
       while (!todo.empty()) {
@@ -978,9 +982,13 @@ rb_status rb_set_tpot_forest(rb_ctx* ctx, const rb_tree_node* nodes, int32_t n_n
         if (nodes[old].feature >= 0) {
           todo.push_back({nodes[old].right, 2 * id + 1});
           todo.push_back({nodes[old].left, 2 * id});
+        } else {
+          leaf_hi = std::max(leaf_hi, std::fabs((double)nodes[old].value));
         }
       }
+      tier_hi += leaf_hi;
     }
+    tpot_hi = std::max(tpot_hi, tier_hi);
     max_tier_nodes = std::max(max_tier_nodes, (int)pk.size() - nbegin[m]);
   }
   nbegin[M] = (int32_t)pk.size();
@@ -989,6 +997,7 @@ rb_status rb_set_tpot_forest(rb_ctx* ctx, const rb_tree_node* nodes, int32_t n_n
   cudaFree(ctx->f_nodes); cudaFree(ctx->f_root); cudaFree(ctx->f_begin); cudaFree(ctx->f_base); cudaFree(ctx->f_nbegin);
   ctx->f_nodes = nullptr; ctx->f_root = ctx->f_begin = ctx->f_nbegin = nullptr; ctx->f_base = nullptr;
   ctx->f_max_tier_nodes = max_tier_nodes;
+  ctx->f_tpot_hi = (float)std::min(2.0 * tpot_hi, 3.0e38);   // (doubled: the fp32 sum rounds)
   ctx->has_forest = false;
   static_assert(sizeof(rb_tree_node) == sizeof(int4), "rb_tree_node is read as int4");
   if (dev_alloc(&ctx->f_nodes, pk.size()) != cudaSuccess || dev_alloc(&ctx->f_root, (size_t)n_trees) != cudaSuccess ||

@@ -45,6 +45,7 @@ struct ForestDev {
   const float* aux;            // [I x (F-2)] auxiliary telemetry features
   const float* tpot0;          // [I] head evaluated on the batch-start state (tpot_kernel)
   int32_t n_features;
+  float tpot_hi;               // no evaluation of the head exceeds this (|base| + sum of the trees' largest |leaf|, doubled)
 };
 
 // Per-call parameters live in device memory so that a captured graph can be replayed with new weights and new
