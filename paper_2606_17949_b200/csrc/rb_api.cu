@@ -59,18 +59,21 @@ struct rb_ctx {
   float *stage_q = nullptr, *stage_l = nullptr; // [max_batch x M] staging of caller-supplied predictions (host)
   float *termA = nullptr, *termP = nullptr, *key = nullptr;
   // Pipelined decisions (rb_options.pipeline): a second set of everything a decision's estimate hands to its dispatch
-  // side (staged queries + their tensor map, partial lists, predictions, terms, keys), an internal stream for the front
-  // half (staging + scan) and the events that order the two halves and the reuse of a set.
+  // side (staged queries + their tensor map, partial lists, predictions, terms, keys), internal streams for the staging
+  // and for the scan, and the events that order the three parts of a decision and the reuse of a set.
   struct Slot {
     __nv_bfloat16* qs = nullptr;
     CUtensorMap tm_q{};
     float* part_sim = nullptr;
     int32_t* part_idx = nullptr;
     float *pred_q = nullptr, *pred_l = nullptr, *termA = nullptr, *termP = nullptr, *key = nullptr;
-    cudaEvent_t ev_front = nullptr;   // front half (staging + scan) done, recorded on the front stream
+    float* q32 = nullptr;             // fp32 storage: this set's copy of the queries for the exact re-rank
+    cudaEvent_t ev_stage = nullptr;   // staging done, recorded on the staging stream
+    cudaEvent_t ev_front = nullptr;   // bank scan done, recorded on the front stream
     cudaEvent_t ev_back = nullptr;    // back half (finish + dispatch) done, recorded on the context's stream
   } slot[2];
-  cudaStream_t front = nullptr;       // low-priority internal stream of the front halves
+  cudaStream_t front = nullptr;       // low-priority internal stream of the bank scans
+  cudaStream_t sstage = nullptr;      // internal stream of the staging kernels (they run beside the scan before them)
   uint64_t pipe_seq = 0;              // pipelined decisions issued so far (slot = seq & 1)
   bool front_busy = false;            // a front half may still be running on the internal stream
   int32_t *order = nullptr, *assignment = nullptr, *max_tokens = nullptr;
@@ -110,7 +113,8 @@ struct rb_ctx {
   int n_pending = 0;
   float *scores = nullptr, *scores0 = nullptr;  // [max_batch x I], allocated by rb_set_instances
   CUtensorMap tm_q{}, tm_bank{}, tm_bank16{};   // bank: 64-row boxes; the same with 16-row boxes
-  // graphs: key = B * 8 + kind (0 decide, 1 estimate, 2 from_predictions) + 4 if stage timing is on
+  // graphs: key from (B, kind, buffer set, stage timing); kinds: 0 decide, 1 estimate, 2 from_predictions; throughput mode:
+  // 5 staging, 3 scan, 4 finish + dispatch
   // One captured graph per decision shape.  The per-call parameters are an argument of the kernels that need them; a
   // replay rewrites that one argument of those kernel nodes (cudaGraphExecKernelNodeSetParams) -- no transfer of any
   // kind sits between the host and the decision's first kernel.
@@ -260,8 +264,9 @@ struct Timer {
 };
 
 // with_terms: the finishing kernel also derives the score terms (rb_decide); otherwise estimate only.
-// sl: buffer set.  part: kAll = staging + scan + finish on stream s; kFront = staging + scan; kBack = finish.
-enum EstimatePart { kAll = 0, kFront = 1, kBack = 2 };
+// sl: buffer set.  part: kAll = staging + scan + finish on stream s; kStage / kScan / kBack = one of the three
+// (throughput mode: each on its own stream).
+enum EstimatePart { kAll = 0, kStage = 1, kScan = 2, kBack = 3 };
 rb_status enqueue_estimate(rb_ctx* ctx, int B, bool with_terms, Timer& tm, int sl = 0, EstimatePart part = kAll,
                            cudaStream_t s = nullptr) {
   if (!s) s = ctx->stream;
@@ -272,7 +277,8 @@ rb_status enqueue_estimate(rb_ctx* ctx, int B, bool with_terms, Timer& tm, int s
   fa.bank_quality = ctx->bank_quality; fa.bank_outlen = ctx->bank_outlen; fa.M = ctx->M;
   fa.weight_mode = ctx->opt.weight_mode; fa.eps = ctx->opt.dist_eps; fa.with_terms = with_terms ? 1 : 0;
   fa.pred_q = S.pred_q; fa.pred_l = S.pred_l; fa.termA = S.termA; fa.termP = S.termP; fa.key = S.key;
-  const bool front = part != kBack, back = part != kFront;
+  const bool do_stage = part == kAll || part == kStage, do_scan = part == kAll || part == kScan, back = part == kAll || part == kBack;
+  const bool front = do_stage || do_scan;
   const int split = ctx->opt.store_dtype == RB_F32 ? 1 : 0;   // fp32 storage: the scan runs over the three-plane bf16 split
   {
     if (ctx->stage_timing && front) {   // before the first mark: nothing but the kernels between the stage events
@@ -288,8 +294,8 @@ rb_status enqueue_estimate(rb_ctx* ctx, int B, bool with_terms, Timer& tm, int s
       // pooled admission bound (0.69 against 0.74 with 32, C4 at B = 512 and 4096); a cluster whose list is popped
       // completely is searched again by the finishing kernel, as for the single-CTA scan
       const int kcap2 = std::min(ctx->kcap, 32);
-      if (front) {
-        CK(launch_stage_queries(ctx->cp_cur, S.qs, B, Bpad2, ctx->d, 1, ctx->gthr, Bpad2 * (1 + ncl), split, ctx->q32, s));
+      if (front) {   // (never split over streams: batches above 128 are not pipelined)
+        CK(launch_stage_queries(ctx->cp_cur, S.qs, B, Bpad2, ctx->d, 1, ctx->gthr, Bpad2 * (1 + ncl), split, S.q32, s));
         tm.mark();
         int ncl_used = 0;
         CK(launch_scan_tc2(&S.tm_q, &ctx->tm_bank, ctx->N, ctx->d_scan, B, Bpad2, kcap2, ctx->kc, ctx->num_sms, S.part_sim,
@@ -309,14 +315,17 @@ rb_status enqueue_estimate(rb_ctx* ctx, int B, bool with_terms, Timer& tm, int s
       int sms = ctx->num_sms;
       if (part != kAll && ctx->num_sms >= 64) sms -= B <= 32 ? (B + 3) / 4 * 4 : 16;
       const int grid = (int)(units < sms ? units : sms);   // what launch_scan_tc uses
-      if (front) {
-        CK(launch_stage_queries(ctx->cp_cur, S.qs, B, Bpad, ctx->d, rep, ctx->gthr, 0, split, ctx->q32, s));
+      if (do_stage) {
+        CK(launch_stage_queries(ctx->cp_cur, S.qs, B, Bpad, ctx->d, rep, ctx->gthr, 0, split, S.q32, s));
         tm.mark();
+        ctx->launches += 1;
+      }
+      if (do_scan) {
         int grid_used = 0;
         CK(launch_scan_tc(&S.tm_q, &ctx->tm_bank, &ctx->tm_bank16, ctx->N, ctx->d_scan, B, Bpad, ctx->ks, sms, S.part_sim, S.part_idx,
                           &grid_used, ctx->stage_timing ? ctx->dev_clock : nullptr, s));
         tm.mark();
-        ctx->launches += 2;
+        ctx->launches += 1;
       }
       fa.part_sim = S.part_sim; fa.part_idx = S.part_idx; fa.nlists = grid * rep; fa.lists_per_cta = rep; fa.kcap = ctx->ks;
       fa.records = 1;
@@ -324,7 +333,7 @@ rb_status enqueue_estimate(rb_ctx* ctx, int B, bool with_terms, Timer& tm, int s
       fa.rescan = ctx->ks < ctx->kc ? 1 : 0;
     }
     if (split) {   // exact similarities from the fp32 rows (the definition of fp32 storage), always
-      fa.bank = nullptr; fa.qs = nullptr; fa.bank32 = ctx->bank32; fa.q32 = ctx->q32; fa.rerank = 2;
+      fa.bank = nullptr; fa.qs = nullptr; fa.bank32 = ctx->bank32; fa.q32 = S.q32; fa.rerank = 2;
     } else {
       fa.bank = (const __nv_bfloat16*)ctx->bank; fa.qs = S.qs; fa.rerank = ctx->opt.rerank_slack > 0 ? 1 : 0;
     }
@@ -447,16 +456,29 @@ rb_status run_path(rb_ctx* ctx, int B, int kind) {
   return st;
 }
 
-// rb_decide in throughput mode (rb_options.pipeline): the front half of the decision (staging + bank scan) goes to the
-// internal low-priority stream, the back half (finishing + dispatch) to the context's stream, joined by events; the two
-// buffer sets alternate, so the front half of this call overlaps the back half of the call before it.
+// rb_decide in throughput mode (rb_options.pipeline): the bank scan goes to the internal low-priority stream, where the
+// scans of consecutive decisions follow one another; the query staging in front of it to a second internal stream, so
+// that it runs beside the scan of the decision before (C2, B = 11: 33.1 -> 31.0 us per decision); the back half
+// (finishing + dispatch) to the context's stream.  Events join the three; the two buffer sets alternate.
 rb_status run_pipelined(rb_ctx* ctx, int B) {
   const int sl = (int)(ctx->pipe_seq & 1);
   rb_ctx::Slot& S = ctx->slot[sl];
   Timer tm(ctx);
-  CK(cudaStreamWaitEvent(ctx->front, S.ev_back, 0));   // the back half that last read this buffer set is done
-  rb_status st = graph_run(ctx, graph_key(ctx, B, 3, sl), ctx->front,
-                           [&]() -> rb_status { return enqueue_estimate(ctx, B, true, tm, sl, kFront, ctx->front); });
+  // staging: beside the scan of the decision before (on the SMs that scan leaves free), once the back half that last
+  // read this buffer set is done
+  // (B > 32: the back half is the longer one and the next scan waits for it through this buffer set; staging then
+  // goes in front of its scan on the same stream -- across streams the hand-over costs more than the overlap saves:
+  // B = 64 46.5 against 39.9 us per decision, B = 11 31.0 against 35.0, B = 32 33.4 against 38.4)
+  cudaStream_t sstage = B > 32 ? ctx->front : ctx->sstage;
+  CK(cudaStreamWaitEvent(sstage, S.ev_back, 0));
+  rb_status st = graph_run(ctx, graph_key(ctx, B, 5, sl), sstage,
+                           [&]() -> rb_status { return enqueue_estimate(ctx, B, true, tm, sl, kStage, sstage); });
+  if (st != RB_OK) return st;
+  CK(cudaEventRecord(S.ev_stage, sstage));
+  // scan: behind the scan before it on the front stream
+  CK(cudaStreamWaitEvent(ctx->front, S.ev_stage, 0));
+  st = graph_run(ctx, graph_key(ctx, B, 3, sl), ctx->front,
+                 [&]() -> rb_status { return enqueue_estimate(ctx, B, true, tm, sl, kScan, ctx->front); });
   if (st != RB_OK) return st;
   CK(cudaEventRecord(S.ev_front, ctx->front));
   CK(cudaStreamWaitEvent(ctx->stream, S.ev_front, 0));
@@ -823,7 +845,10 @@ rb_status rb_create(rb_ctx** out, const void* bank_emb, const float* bank_qualit
       int lo = 0, hi = 0;
       CK(cudaDeviceGetStreamPriorityRange(&lo, &hi));   // lo = least priority
       CK(cudaStreamCreateWithPriority(&ctx->front, cudaStreamNonBlocking, lo));
+      CK(cudaStreamCreateWithPriority(&ctx->sstage, cudaStreamNonBlocking, hi));
+      ALLOC(S1.q32, (size_t)kTileM * d);
       for (int j = 0; j < 2; ++j) {
+        CK(cudaEventCreateWithFlags(&ctx->slot[j].ev_stage, cudaEventDisableTiming));
         CK(cudaEventCreateWithFlags(&ctx->slot[j].ev_front, cudaEventDisableTiming));
         CK(cudaEventCreateWithFlags(&ctx->slot[j].ev_back, cudaEventDisableTiming));
       }
@@ -848,7 +873,7 @@ rb_status rb_create(rb_ctx** out, const void* bank_emb, const float* bank_qualit
   }
   {
     rb_ctx::Slot& S0 = ctx->slot[0];   // the primary buffer set
-    S0.qs = ctx->qs; S0.tm_q = ctx->tm_q; S0.part_sim = ctx->part_sim; S0.part_idx = ctx->part_idx;
+    S0.qs = ctx->qs; S0.tm_q = ctx->tm_q; S0.part_sim = ctx->part_sim; S0.part_idx = ctx->part_idx; S0.q32 = ctx->q32;
     S0.pred_q = ctx->pred_q; S0.pred_l = ctx->pred_l; S0.termA = ctx->termA; S0.termP = ctx->termP; S0.key = ctx->key;
   }
   {
@@ -1509,6 +1534,7 @@ const char* rb_last_error(const rb_ctx* ctx) { return ctx ? ctx->err.c_str() : "
 
 void rb_destroy(rb_ctx* ctx) {
   if (!ctx) return;
+  if (ctx->sstage) cudaStreamSynchronize(ctx->sstage);
   if (ctx->front) cudaStreamSynchronize(ctx->front);
   if (ctx->stream) cudaStreamSynchronize(ctx->stream);
   drop_graphs(ctx);
@@ -1518,11 +1544,14 @@ void rb_destroy(rb_ctx* ctx) {
   for (void* p : ptrs) cudaFree(p);
   cudaFree(ctx->slot[1].qs);
   cudaFree(ctx->slot[1].part_sim);
+  cudaFree(ctx->slot[1].q32);
   for (auto& sl : ctx->slot) {
+    if (sl.ev_stage) cudaEventDestroy(sl.ev_stage);
     if (sl.ev_front) cudaEventDestroy(sl.ev_front);
     if (sl.ev_back) cudaEventDestroy(sl.ev_back);
   }
   if (ctx->front) cudaStreamDestroy(ctx->front);
+  if (ctx->sstage) cudaStreamDestroy(ctx->sstage);
   for (auto& e : ctx->ev)
     if (e) cudaEventDestroy(e);
   if (ctx->h_zc) cudaFreeHost(ctx->h_zc);
