@@ -203,15 +203,16 @@ rb_status rb_decide(rb_ctx* ctx, const float* query_emb, const int32_t* prompt_l
                     const float w[3], int32_t* assignment, float* scores, float* pred_quality,
                     float* pred_outlen, int32_t* nn_idx, float* nn_sim);
 
-/* rb_decide for a serving loop that keeps two decisions in flight (needs rb_options.pipeline = 1): rb_decide_submit copies
+/* rb_decide for a serving loop that keeps up to three decisions in flight (needs rb_options.pipeline = 1): rb_decide_submit copies
  * the batch into pinned memory the kernels read in place, enqueues the decision and returns at once; rb_decide_collect
  * waits for the OLDEST submitted decision and copies its assignment out (the dispatch kernel writes it, then a completion
- * word, into pinned host memory).  The usual loop is submit(j + 1); collect(j): the host side of one decision and the bank
- * scan of the next overlap the finishing and dispatch stages of the one before.  rb_advance_state calls made before a
+ * word, into pinned host memory).  The usual loop is submit(j + 2); collect(j): the host side of one decision and the bank
+ * scan of the next overlap the finishing and dispatch stages of the one before (with only submit(j + 1); collect(j) the
+ * rate is half a decision's latency, not the scan's duration).  rb_advance_state calls made before a
  * submission are applied by that decision, in order, exactly as with rb_decide; results equal rb_decide's bit for bit.
  *   query_emb   [host] B x d fp32;   prompt_len [host] B int32;   1 <= B <= min(128, max_batch)
  *   assignment  [host] B int32 (rb_decide_collect; B must be the submitted batch's)
- * RB_ESTATE: a third submission with two in flight, a collect with none, pipeline = 0.  RB_EUNSUPPORTED: boosted latency
+ * RB_ESTATE: a fourth submission with three in flight, a collect with none, pipeline = 0.  RB_EUNSUPPORTED: boosted latency
  * head, graph replay off, no mapped pinned memory. */
 rb_status rb_decide_submit(rb_ctx* ctx, const float* query_emb, const int32_t* prompt_len, int32_t B, const float w[3]);
 rb_status rb_decide_collect(rb_ctx* ctx, int32_t* assignment, int32_t B);

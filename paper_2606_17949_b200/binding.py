@@ -210,7 +210,7 @@ def rb_decide(ctx, query_emb, prompt_len, B, w, assignment, scores=None, pred_qu
 
 
 def rb_decide_submit(ctx, query_emb, prompt_len, B, w):
-    """Enqueues a decision from HOST buffers and returns at once (rb_options.pipeline = 1; at most two in flight)."""
+    """Enqueues a decision from HOST buffers and returns at once (rb_options.pipeline = 1; at most three in flight)."""
     f32, i32 = (torch.float32, torch.int32) if torch else (np.float32, np.int32)
     _check(ctx, _lib.rb_decide_submit(ctx, _ptr(query_emb, f32), _ptr(prompt_len, i32), B, _w3(w)))
 

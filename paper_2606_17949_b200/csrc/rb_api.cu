@@ -71,10 +71,10 @@ struct rb_ctx {
     cudaEvent_t ev_stage = nullptr;   // staging done, recorded on the staging stream
     cudaEvent_t ev_front = nullptr;   // bank scan done, recorded on the front stream
     cudaEvent_t ev_back = nullptr;    // back half (finish + dispatch) done, recorded on the context's stream
-  } slot[2];
+  } slot[kSlots];
   cudaStream_t front = nullptr;       // low-priority internal stream of the bank scans
   cudaStream_t sstage = nullptr;      // internal stream of the staging kernels (they run beside the scan before them)
-  uint64_t pipe_seq = 0;              // pipelined decisions issued so far (slot = seq & 1)
+  uint64_t pipe_seq = 0;              // pipelined decisions issued so far (slot = seq % kSlots)
   bool front_busy = false;            // a front half may still be running on the internal stream
   int32_t *order = nullptr, *assignment = nullptr, *max_tokens = nullptr;
   float* budget = nullptr;          // [max_batch] staging of host budgets
@@ -96,9 +96,9 @@ struct rb_ctx {
     bool busy = false;
     uint32_t seq = 0;
     int B = 0;
-  } async[2];
+  } async[kSlots];
   size_t az_off_plen = 0, az_off_assign = 0, az_off_flag = 0;
-  uint64_t async_head = 0;            // submissions collected so far (the oldest in flight is async[head & 1])
+  uint64_t async_head = 0;            // submissions collected so far (the oldest in flight: the busy block with the smallest sequence number)
   uint64_t async_tail = 0;            // submissions made so far
   // boosted TPOT head (latency_mode 2)
   int4* f_nodes = nullptr;
@@ -429,7 +429,7 @@ rb_status graph_run(rb_ctx* ctx, int64_t gkey, cudaStream_t s, F&& enqueue) {
 }
 
 int64_t graph_key(const rb_ctx* ctx, int B, int kind, int sl) {
-  return (((int64_t)B * 8 + kind) * 2 + sl) * 2 + (ctx->stage_timing ? 1 : 0);
+  return (((int64_t)B * 8 + kind) * kSlots + sl) * 2 + (ctx->stage_timing ? 1 : 0);
 }
 
 // kind: 0 = estimate + dispatch, 1 = estimate, 2 = dispatch (+scores0)
@@ -459,9 +459,11 @@ rb_status run_path(rb_ctx* ctx, int B, int kind) {
 // rb_decide in throughput mode (rb_options.pipeline): the bank scan goes to the internal low-priority stream, where the
 // scans of consecutive decisions follow one another; the query staging in front of it to a second internal stream, so
 // that it runs beside the scan of the decision before (C2, B = 11: 33.1 -> 31.0 us per decision); the back half
-// (finishing + dispatch) to the context's stream.  Events join the three; the two buffer sets alternate.
-rb_status run_pipelined(rb_ctx* ctx, int B) {
-  const int sl = (int)(ctx->pipe_seq & 1);
+// (finishing + dispatch) to the context's stream.  Events join the three; kSlots buffer sets rotate
+// (three: with two, the scan of decision j + 2 waits for the back half of decision j, and a host loop of submissions is
+// limited to two in flight, i.e. to half a decision's latency per decision).
+rb_status run_pipelined(rb_ctx* ctx, int B, bool paced) {
+  const int sl = (int)(ctx->pipe_seq % kSlots);
   rb_ctx::Slot& S = ctx->slot[sl];
   Timer tm(ctx);
   // staging: beside the scan of the decision before (on the SMs that scan leaves free), once the back half that last
@@ -471,6 +473,13 @@ rb_status run_pipelined(rb_ctx* ctx, int B) {
   // B = 64 46.5 against 39.9 us per decision, B = 11 31.0 against 35.0, B = 32 33.4 against 38.4)
   cudaStream_t sstage = B > 32 ? ctx->front : ctx->sstage;
   CK(cudaStreamWaitEvent(sstage, S.ev_back, 0));
+  // Calls that run ahead of the device (rb_decide with device buffers returns at once, so the queue is deep): the staging
+  // kernel also waits for the back half of the decision two before it, and so runs in the middle of the scan before its
+  // own.  Free to start at once it is launched just when the front stream launches that scan, and the scan starts later
+  // (32.4 against 30.9 us per decision, B = 11).  Submissions paced by rb_decide_collect arrive mid-scan by themselves,
+  // and there the extra wait costs the third decision in flight (36.5 against 33.6 us per decision).
+  if (!paced && B <= 32 && ctx->pipe_seq >= 2)
+    CK(cudaStreamWaitEvent(sstage, ctx->slot[(ctx->pipe_seq + 1) % kSlots].ev_back, 0));
   rb_status st = graph_run(ctx, graph_key(ctx, B, 5, sl), sstage,
                            [&]() -> rb_status { return enqueue_estimate(ctx, B, true, tm, sl, kStage, sstage); });
   if (st != RB_OK) return st;
@@ -794,8 +803,11 @@ rb_status rb_create(rb_ctx** out, const void* bank_emb, const float* bank_qualit
                  o_tst = take((kMaxM + 1) * 4), o_cur = take(kMaxM * 4), o_cnt = take(8);
     // second set of what an estimate hands to its dispatch side (pipelined decisions of at most 128 requests)
     const size_t m1 = opt.pipeline ? (size_t)kTileM : 0;
-    const size_t o_pq1 = take(m1 * M * 4), o_pl1 = take(m1 * M * 4), o_ta1 = take(m1 * M * 4), o_tp1 = take(m1 * M * 4),
-                 o_key1 = take(m1 * 4);
+    size_t o_pq1[kSlots], o_pl1[kSlots], o_ta1[kSlots], o_tp1[kSlots], o_key1[kSlots];
+    for (int j = 1; j < kSlots; ++j) {
+      o_pq1[j] = take(m1 * M * 4); o_pl1[j] = take(m1 * M * 4); o_ta1[j] = take(m1 * M * 4); o_tp1[j] = take(m1 * M * 4);
+      o_key1[j] = take(m1 * 4);
+    }
     ALLOC(ctx->arena, off);
     uint8_t* a = ctx->arena;
     ctx->plen = (int32_t*)(a + o_plen); ctx->cand_sim = (float*)(a + o_csim);
@@ -810,10 +822,10 @@ rb_status rb_create(rb_ctx** out, const void* bank_emb, const float* bank_qualit
     ctx->f_aux = (float*)(a + o_aux); ctx->f_tpot0 = (float*)(a + o_tpot0);
     ctx->members = (int32_t*)(a + o_mem); ctx->tstart = (int32_t*)(a + o_tst); ctx->pipe_cursor = (int32_t*)(a + o_cur);
     ctx->pipe_counter = (unsigned long long*)(a + o_cnt);
-    {
-      rb_ctx::Slot& S1 = ctx->slot[1];
-      S1.pred_q = (float*)(a + o_pq1); S1.pred_l = (float*)(a + o_pl1); S1.termA = (float*)(a + o_ta1);
-      S1.termP = (float*)(a + o_tp1); S1.key = (float*)(a + o_key1);
+    for (int j = 1; j < kSlots; ++j) {
+      rb_ctx::Slot& S1 = ctx->slot[j];
+      S1.pred_q = (float*)(a + o_pq1[j]); S1.pred_l = (float*)(a + o_pl1[j]); S1.termA = (float*)(a + o_ta1[j]);
+      S1.termP = (float*)(a + o_tp1[j]); S1.key = (float*)(a + o_key1[j]);
     }
     CK(cudaMemsetAsync(ctx->arena, 0, off, s));
   }
@@ -833,21 +845,23 @@ rb_status rb_create(rb_ctx** out, const void* bank_emb, const float* bank_qualit
     st = encode_map(ctx, &ctx->tm_q, ctx->qs, (uint64_t)ctx->Bpad_max, (uint64_t)ds, kTileM);
     if (st != RB_OK) return st;
     if (opt.pipeline) {
-      // second buffer set, for batches of at most 128 requests (larger ones are not pipelined)
-      rb_ctx::Slot& S1 = ctx->slot[1];
-      ALLOC(S1.qs, (size_t)kTileM * d);
-      const size_t part_n1 = (size_t)ctx->num_sms * ctx->kcap * 4 * kTileM;
-      ALLOC(S1.part_sim, 2 * part_n1);
-      S1.part_idx = reinterpret_cast<int32_t*>(S1.part_sim + part_n1);
-      CK(cudaMemsetAsync(S1.qs, 0, (size_t)kTileM * d * 2, s));
-      st = encode_map(ctx, &S1.tm_q, S1.qs, (uint64_t)kTileM, (uint64_t)d, kTileM);
-      if (st != RB_OK) return st;
+      // further buffer sets, for batches of at most 128 requests (larger ones are not pipelined)
+      for (int j = 1; j < kSlots; ++j) {
+        rb_ctx::Slot& S1 = ctx->slot[j];
+        ALLOC(S1.qs, (size_t)kTileM * d);
+        const size_t part_n1 = (size_t)ctx->num_sms * ctx->kcap * 4 * kTileM;
+        ALLOC(S1.part_sim, 2 * part_n1);
+        S1.part_idx = reinterpret_cast<int32_t*>(S1.part_sim + part_n1);
+        CK(cudaMemsetAsync(S1.qs, 0, (size_t)kTileM * d * 2, s));
+        st = encode_map(ctx, &S1.tm_q, S1.qs, (uint64_t)kTileM, (uint64_t)d, kTileM);
+        if (st != RB_OK) return st;
+        ALLOC(S1.q32, (size_t)kTileM * d);
+      }
       int lo = 0, hi = 0;
       CK(cudaDeviceGetStreamPriorityRange(&lo, &hi));   // lo = least priority
       CK(cudaStreamCreateWithPriority(&ctx->front, cudaStreamNonBlocking, lo));
       CK(cudaStreamCreateWithPriority(&ctx->sstage, cudaStreamNonBlocking, hi));
-      ALLOC(S1.q32, (size_t)kTileM * d);
-      for (int j = 0; j < 2; ++j) {
+      for (int j = 0; j < kSlots; ++j) {
         CK(cudaEventCreateWithFlags(&ctx->slot[j].ev_stage, cudaEventDisableTiming));
         CK(cudaEventCreateWithFlags(&ctx->slot[j].ev_front, cudaEventDisableTiming));
         CK(cudaEventCreateWithFlags(&ctx->slot[j].ev_back, cudaEventDisableTiming));
@@ -856,7 +870,7 @@ rb_status rb_create(rb_ctx** out, const void* bank_emb, const float* bank_qualit
       ctx->az_off_plen = ((size_t)kTileM * d * 4 + 255) & ~(size_t)255;
       ctx->az_off_assign = ctx->az_off_plen + 512;
       ctx->az_off_flag = ctx->az_off_assign + 512;
-      for (int j = 0; j < 2; ++j) {
+      for (int j = 0; j < kSlots; ++j) {
         rb_ctx::AsyncSlot& A = ctx->async[j];
         if (cudaHostAlloc((void**)&A.h, ctx->az_off_flag + 256, cudaHostAllocMapped) != cudaSuccess ||
             cudaHostGetDevicePointer((void**)&A.d, A.h, 0) != cudaSuccess) {
@@ -1190,13 +1204,13 @@ rb_status rb_decide_budgeted(rb_ctx* ctx, const float* query_emb, const int32_t*
   const bool pipelined = ctx->front != nullptr && !sg.any_host && B <= kTileM && adv_folded && !ctx->stage_timing &&
                          ctx->opt.use_graph != 0;
   if (pipelined) {
-    const rb_ctx::Slot& S = ctx->slot[ctx->pipe_seq & 1];
+    const rb_ctx::Slot& S = ctx->slot[ctx->pipe_seq % kSlots];
     cp.q_src = S.pred_q;
     cp.l_src = S.pred_l;
   }
   st = push_params(ctx, cp);
   if (st != RB_OK) return st;
-  st = pipelined ? run_pipelined(ctx, B) : run_path(ctx, B, 0);
+  st = pipelined ? run_pipelined(ctx, B, false) : run_path(ctx, B, 0);
   if (st != RB_OK) return st;
   if (adv_folded) ctx->n_pending = 0;
   collect_stage_times(ctx, 0);
@@ -1213,9 +1227,10 @@ rb_status rb_decide_submit(rb_ctx* ctx, const float* query_emb, const int32_t* p
   if (B < 1 || B > kTileM || B > ctx->opt.max_batch) return fail(ctx, RB_EINVAL, "B out of range [1, min(128, max_batch)]");
   rb_status st = check_weights(ctx, w);
   if (st != RB_OK) return st;
-  if (ctx->async_tail - ctx->async_head >= 2) return fail(ctx, RB_ESTATE, "two decisions in flight: rb_decide_collect first");
+  if (ctx->async_tail - ctx->async_head >= (uint64_t)kSlots)
+    return fail(ctx, RB_ESTATE, "three decisions in flight: rb_decide_collect first");
   // the buffer set the next pipelined decision uses decides the pinned block
-  rb_ctx::AsyncSlot& A = ctx->async[ctx->pipe_seq & 1];
+  rb_ctx::AsyncSlot& A = ctx->async[ctx->pipe_seq % kSlots];
   if (!A.h) return fail(ctx, RB_EUNSUPPORTED, "no mapped pinned host memory");
   if (A.busy) return fail(ctx, RB_ESTATE, "the buffer set of this submission is still in flight: rb_decide_collect first");
   std::memcpy(A.h, query_emb, (size_t)B * ctx->d * 4);
@@ -1229,12 +1244,12 @@ rb_status rb_decide_submit(rb_ctx* ctx, const float* query_emb, const int32_t* p
   cp.assignment = reinterpret_cast<int32_t*>(A.d + ctx->az_off_assign);
   cp.done_flag = reinterpret_cast<uint32_t*>(A.d + ctx->az_off_flag);
   cp.done_seq = ++ctx->done_seq;
-  const rb_ctx::Slot& S = ctx->slot[ctx->pipe_seq & 1];
+  const rb_ctx::Slot& S = ctx->slot[ctx->pipe_seq % kSlots];
   cp.q_src = S.pred_q;
   cp.l_src = S.pred_l;
   st = push_params(ctx, cp);
   if (st != RB_OK) return st;
-  st = run_pipelined(ctx, B);
+  st = run_pipelined(ctx, B, true);
   if (st != RB_OK) return st;
   ctx->n_pending = 0;
   A.busy = true;
@@ -1248,7 +1263,7 @@ rb_status rb_decide_collect(rb_ctx* ctx, int32_t* assignment, int32_t B) {
   if (!ctx) return RB_EINVAL;
   if (!assignment) return fail(ctx, RB_EINVAL, "NULL argument");
   if (ctx->async_tail == ctx->async_head) return fail(ctx, RB_ESTATE, "rb_decide_collect: nothing in flight");
-  // submissions alternate between the two blocks in submission order, unless synchronous pipelined calls came in
+  // submissions rotate through the blocks in submission order, unless synchronous pipelined calls came in
   // between: the oldest one in flight is the busy block with the smaller sequence number
   rb_ctx::AsyncSlot* A = nullptr;
   for (auto& c : ctx->async)
@@ -1542,9 +1557,11 @@ void rb_destroy(rb_ctx* ctx) {
                   ctx->gthr, ctx->bank32, ctx->scratch_nn_idx, ctx->scratch_nn_sim, ctx->scores, ctx->scores0, ctx->f_nodes,
                   ctx->f_root, ctx->f_begin, ctx->f_nbegin, ctx->f_base, ctx->dev_clock, ctx->sweep_buf};
   for (void* p : ptrs) cudaFree(p);
-  cudaFree(ctx->slot[1].qs);
-  cudaFree(ctx->slot[1].part_sim);
-  cudaFree(ctx->slot[1].q32);
+  for (int j = 1; j < kSlots; ++j) {
+    cudaFree(ctx->slot[j].qs);
+    cudaFree(ctx->slot[j].part_sim);
+    cudaFree(ctx->slot[j].q32);
+  }
   for (auto& sl : ctx->slot) {
     if (sl.ev_stage) cudaEventDestroy(sl.ev_stage);
     if (sl.ev_front) cudaEventDestroy(sl.ev_front);

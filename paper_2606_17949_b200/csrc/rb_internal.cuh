@@ -13,6 +13,7 @@ constexpr int kMaxI = 1024;        // instances
 constexpr int kTileM = 128;        // queries per MMA tile (TMEM lanes)
 constexpr int kTileN = 256;        // bank rows per MMA tile (TMEM columns of one accumulator)
 constexpr int kBoxN = 64;          // bank rows per TMA box
+constexpr int kSlots = 3;          // buffer sets of the throughput mode = decisions that can be in flight
 constexpr int kRowUnit = 16;       // the single-CTA scan splits the bank over its CTAs in groups of this many rows
 constexpr int kTileK = 64;         // bf16 per K chunk = one 128-byte swizzle row
 constexpr int kMaxPendingAdvance = 4;   // rb_advance_state calls a decision can absorb (CallParams::adv_ms)

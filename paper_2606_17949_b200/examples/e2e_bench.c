@@ -1,6 +1,6 @@
 /* e2e_bench.c -- end-to-end latency of one decision through the C ABI alone (no Python, no torch): host buffers in,
  * assignment out, rb_advance_state + rb_decide per step.  Prints one JSON line.  Built and run by bench.py
- * (gcc ... -lrouteb); usage: e2e_bench N d B I steps [pipeline]   (pipeline = 1: rb_decide_submit / rb_decide_collect, two
+ * (gcc ... -lrouteb); usage: e2e_bench N d B I steps [pipeline]   (pipeline = 1: rb_decide_submit / rb_decide_collect, three
  * decisions in flight)
  * The bank is synthetic (unit-norm rows around a few centres, a multiplicative congruential generator): this program
  * measures the library's host path, not parity. */
@@ -93,7 +93,7 @@ int main(int argc, char** argv) {
       if (s >= 0) { t[s] = now_us() - t0; total_us += t[s]; }
     }
   } else {
-    /* submit(j + 1), collect(j): the inputs of every step are generated before the timed loop */
+    /* submit(j + 2), collect(j): the inputs of every step are generated before the timed loop */
     const int n = steps + 20;
     float* allq = malloc((size_t)n * B * d * 4);
     int32_t* allp = malloc((size_t)n * B * 4);
@@ -108,13 +108,13 @@ int main(int argc, char** argv) {
       const double t0 = now_us();
       if (rb_advance_state(ctx, 40.0f) != RB_OK ||
           rb_decide_submit(ctx, allq + (size_t)s * B * d, allp + (size_t)s * B, B, w) != RB_OK ||
-          (s >= 1 && rb_decide_collect(ctx, assignment, B) != RB_OK)) {
+          (s >= 2 && rb_decide_collect(ctx, assignment, B) != RB_OK)) {
         printf("{\"error\": \"%s\"}\n", rb_last_error(ctx));
         return 1;
       }
       if (s >= 20) t[s - 20] = now_us() - t0;
     }
-    if (rb_decide_collect(ctx, assignment, B) != RB_OK) return 1;
+    if (rb_decide_collect(ctx, assignment, B) != RB_OK || rb_decide_collect(ctx, assignment, B) != RB_OK) return 1;
     total_us = now_us() - t_start;
   }
   const double sum = total_us;
@@ -122,7 +122,7 @@ int main(int argc, char** argv) {
   printf("{\"N\": %ld, \"d\": %d, \"B\": %d, \"I\": %d, \"steps\": %d, \"us_mean\": %.2f, \"us_p50\": %.2f, \"us_p99\": %.2f, "
          "\"mode\": \"%s\", \"buffers\": \"pageable host memory in, host memory out\", \"l2\": \"not flushed (bank %.1f MB)\"}\n",
          N, d, B, I, steps, sum / steps, t[steps / 2], t[(int)(steps * 0.99)],
-         pipeline ? "rb_decide_submit / rb_decide_collect, two in flight (us_mean = wall clock over all steps / steps)" : "rb_decide, one at a time",
+         pipeline ? "rb_decide_submit / rb_decide_collect, three in flight (us_mean = wall clock over all steps / steps)" : "rb_decide, one at a time",
          (double)N * d * 2 / 1e6);
   rb_destroy(ctx);
   return 0;

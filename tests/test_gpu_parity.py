@@ -1057,9 +1057,9 @@ def test_pipelined_decisions_equal_unpipelined_ones(orc):
 
 
 def test_submit_collect_equals_synchronous_decisions(orc):
-    """rb_decide_submit / rb_decide_collect (two decisions in flight from host buffers): the assignments and the final
+    """rb_decide_submit / rb_decide_collect (up to three decisions in flight from host buffers): the assignments and the final
     state of 200 decisions with rb_advance_state in between equal those of synchronous rb_decide calls on an unpipelined
-    context; call-order errors are reported (third submission, collect with nothing in flight, wrong batch size)."""
+    context; call-order errors are reported (fourth submission, collect with nothing in flight, wrong batch size)."""
     from paper_2606_17949_b200 import binding as rb
     cfg = dataclasses.replace(synth.CONFIGS["C2"], N=30000, d=256, Kc=16, seed=71)
     bank = synth.make_bank(cfg, device="cuda")
@@ -1087,17 +1087,22 @@ def test_submit_collect_equals_synchronous_decisions(orc):
     got = torch.empty(int(offs[-1]), dtype=torch.int32)
     with pytest.raises(rb.RbError):
         rb.rb_decide_collect(rt.ctx, got[:1], 1)                       # nothing in flight
+    pending = []
     for j, B in enumerate(sizes):
         rt.advance_state(float(2.0 + j % 5))
         rb.rb_decide_submit(rt.ctx, q[offs[j]:offs[j + 1]], p[offs[j]:offs[j + 1]], B, presets[j % 4])
-        if j == 1:
-            with pytest.raises(rb.RbError):                            # two in flight: a third is refused, nothing changes
+        pending.append(j)
+        if j == 2:
+            with pytest.raises(rb.RbError):                            # three in flight: a fourth is refused, nothing changes
                 rb.rb_decide_submit(rt.ctx, q[:1], p[:1], 1, presets[0])
             with pytest.raises(rb.RbError):
                 rb.rb_decide_collect(rt.ctx, got[:sizes[0] + 1], sizes[0] + 1)   # not the submitted batch size
-        if j >= 1:
-            rb.rb_decide_collect(rt.ctx, got[offs[j - 1]:offs[j]], sizes[j - 1])
-    rb.rb_decide_collect(rt.ctx, got[offs[-2]:offs[-1]], sizes[-1])
+        depth = 3 if (j // 10) % 3 == 0 else (2 if (j // 10) % 3 == 1 else 1)    # every depth of the loop
+        while len(pending) >= depth:
+            c = pending.pop(0)
+            rb.rb_decide_collect(rt.ctx, got[offs[c]:offs[c + 1]], sizes[c])
+    for c in pending:
+        rb.rb_decide_collect(rt.ctx, got[offs[c]:offs[c + 1]], sizes[c])
     assert torch.equal(got, ref)
     s = rt.get_state()
     assert torch.equal(s[0], ref_state[0]) and torch.equal(s[1], ref_state[1])
