@@ -249,13 +249,15 @@ scan_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__
     }
   }
 
-  tc_fence_before();
-  __syncthreads();
-  if (dev_clock != nullptr && threadIdx.x == 0) {   // ... and latest CTA end
+  if (dev_clock != nullptr && warp >= 2 && lane == 0) {   // ... and latest CTA end: an epilogue warp, behind its last store
+    // (a stamp taken by another warp behind the closing barrier reads the timer when the BAR.SYNC.DEFER_BLOCKING is
+    // issued, not when it completes: it came out 2 us before the epilogue's own end)
     unsigned long long t1;
-    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t1));
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t1)::"memory");
     atomicMax(dev_clock + 1, t1);
   }
+  tc_fence_before();
+  __syncthreads();
   if (warp == 1) {
     tc_fence_after();
     asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(512) : "memory");
