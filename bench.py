@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py -- RouteBalance per-batch scheduling decision on B200: requests routed per second.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--l2 flush|warm] [--no-scan-c4]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--no-scan-c4]
 
 A *step* is one pass of the whole hot path over one batch of waiting requests: rb_advance_state(elapsed) +
 rb_decide(query_emb, prompt_len, w) = staging, tcgen05 bank scan with fused top-k, merge, re-rank + aggregate,
@@ -63,8 +63,6 @@ def parse_args(argv=None):
     ap.add_argument("--steps", type=int, default=1000)
     ap.add_argument("--warmup", type=int, default=20)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--l2", default="flush", choices=["flush", "warm"],
-                    help="flush: read a 3x-L2 buffer before every timed step; warm: back-to-back steps")
     ap.add_argument("--no-scan-c4", action="store_true", help="skip the C4 (10M x 384) bank-scan roofline leg")
     ap.add_argument("--only-scan-c4", action="store_true", help="run only the C4 bank-scan leg (profiling runs)")
     ap.add_argument("--c4-batch", type=int, default=64, help="B of the --only-scan-c4 leg (1..4096)")

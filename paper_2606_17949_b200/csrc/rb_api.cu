@@ -51,8 +51,6 @@ struct rb_ctx {
   uint32_t* gthr = nullptr;         // [Bpad_max] cross-slab admission thresholds of the scan (cleared per decision)
   float* part_sim = nullptr;        // [num_sms][kcap][Bpad_max]
   int32_t* part_idx = nullptr;
-  float* cand_sim = nullptr;        // [max_batch x kc]
-  int32_t* cand_idx = nullptr;
   int32_t* scratch_nn_idx = nullptr;   // [max_batch x k] staging for host callers
   float* scratch_nn_sim = nullptr;
   float *pred_q = nullptr, *pred_l = nullptr;   // [max_batch x M] the estimate, consumed by score/dispatch
@@ -792,8 +790,7 @@ rb_status rb_create(rb_ctx** out, const void* bank_emb, const float* bank_qualit
   {
     size_t off = 0;
     auto take = [&](size_t bytes) { const size_t o = off; off = (off + bytes + 255) & ~(size_t)255; return o; };
-    const size_t o_plen = take(mb * 4), o_csim = take(mb * ctx->kc * 4),
-                 o_cidx = take(mb * ctx->kc * 4), o_pq = take(mb * M * 4), o_pl = take(mb * M * 4), o_sq = take(mb * M * 4),
+    const size_t o_plen = take(mb * 4), o_pq = take(mb * M * 4), o_pl = take(mb * M * 4), o_sq = take(mb * M * 4),
                  o_sl = take(mb * M * 4), o_ta = take(mb * M * 4), o_tp = take(mb * M * 4), o_key = take(mb * 4),
                  o_ord = take(mb * 4), o_asg = take(mb * 4), o_mt = take(mb * 4), o_bud = take(mb * 4),
                  o_tier = take(kMaxI * 4), o_cap = take(kMaxI * 4), o_dq = take(kMaxI * 4), o_bq = take(kMaxI * 4),
@@ -810,8 +807,7 @@ rb_status rb_create(rb_ctx** out, const void* bank_emb, const float* bank_qualit
     }
     ALLOC(ctx->arena, off);
     uint8_t* a = ctx->arena;
-    ctx->plen = (int32_t*)(a + o_plen); ctx->cand_sim = (float*)(a + o_csim);
-    ctx->cand_idx = (int32_t*)(a + o_cidx); ctx->pred_q = (float*)(a + o_pq); ctx->pred_l = (float*)(a + o_pl);
+    ctx->plen = (int32_t*)(a + o_plen); ctx->pred_q = (float*)(a + o_pq); ctx->pred_l = (float*)(a + o_pl);
     ctx->stage_q = (float*)(a + o_sq); ctx->stage_l = (float*)(a + o_sl); ctx->termA = (float*)(a + o_ta);
     ctx->termP = (float*)(a + o_tp); ctx->key = (float*)(a + o_key); ctx->order = (int32_t*)(a + o_ord);
     ctx->assignment = (int32_t*)(a + o_asg); ctx->max_tokens = (int32_t*)(a + o_mt); ctx->budget = (float*)(a + o_bud);

@@ -15,10 +15,13 @@
 //   warps 2-5  epilogue: thread t owns TMEM lane t = query t of the m-tile; tcgen05.ld 32 columns at a time,
 //            compare against the thread's current KCAP-th best similarity, append the rare survivors to a
 //            shared-memory buffer, then insert them into a sorted register list in warp lock-step.
-// Bank rows are split over CTAs in units of 64 rows; a CTA walks its slab in tiles of 256 rows and, for
+// Bank rows are split over CTAs in groups of 16 rows (the remainder of a slab's last tile is loaded through a second
+// tensor map with 16-row boxes); a CTA walks its slab in tiles of 256 rows and, for
 // B > 128, revisits each tile once per 128-query m-tile (bank tile then comes from L2), carrying the lists
 // through global memory between visits.  For B <= 64 the queries are replicated over the lane quarters so that
 // all four epilogue warps share the columns of a tile (the epilogue of a short slab is latency-bound).
+// A CTA's lists leave as 32-byte records of the finishing kernel's 64-bit keys (order-preserving image of the similarity,
+// ~index), query-major: the finishing CTA of a query reads them as one contiguous stream.
 #include "rb_internal.cuh"
 #include "tc_scan.cuh"
 

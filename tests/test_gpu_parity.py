@@ -570,6 +570,47 @@ def test_dispatch_fast_division_is_ieee_exact():
     rt.close()
 
 
+@pytest.mark.parametrize("I,M,B", [(13, 4, 24), (200, 5, 150)])
+@pytest.mark.parametrize("case", ["tiny_lengths", "huge_queue", "denormal_length", "huge_lengths", "in_window"])
+def test_dispatch_operand_ranges_pick_the_division(orc, I, M, B, case):
+    """The greedy loop runs without any division fallback when the batch's operand ranges (binary exponents of the
+    lengths, prefill terms, queues, decode constants, batch slopes) keep every quotient inside the exact window of the
+    reciprocal-refinement sequence, and with the IEEE division otherwise.  Batches on both sides of the test, single- and
+    multi-warp kernels: assignment, scores and the committed state equal the oracle's bit for bit."""
+    from paper_2606_17949_b200.router import Router
+    rng = np.random.default_rng(7000 + I + len(case))
+    it = synth.make_instances(I, M, cap=3)
+    rt = Router(torch.randn(64, 16).cuda(), torch.rand(64, M).cuda(), torch.rand(64, M).cuda() + 1, 4, store="f32", max_batch=B)
+    rt.set_instances(**it)
+    queued = rng.integers(0, 20001, I).astype(np.float32)
+    running = np.minimum(rng.integers(0, 6, I), it["cap"]).astype(np.int32)
+    L = rng.lognormal(5.5, 0.7, (B, M)).astype(np.float32)
+    if case == "tiny_lengths":
+        L *= np.float32(1e-30)                 # T^ far below 2^-34
+        queued[:] = 0
+    elif case == "huge_queue":
+        queued *= np.float32(1e22)             # d / b and T^ above 2^62
+    elif case == "denormal_length":
+        L[3, 1] = np.float32(1e-41)
+    elif case == "huge_lengths":
+        L *= np.float32(1e16)
+    Q = rng.uniform(0, 1, (B, M)).astype(np.float32)
+    plen = rng.integers(1, 4000, B).astype(np.int32)
+    inst = orc.Instances(**it)
+    rt.set_state(torch.from_numpy(queued), torch.from_numpy(running))
+    dq, bq = queued, running
+    for w in [(0.2, 0.5, 0.3), (0.0, 1.0, 0.0)]:
+        g = _np(rt.decide_from_predictions(torch.from_numpy(Q).cuda(), torch.from_numpy(L).cuda(), torch.from_numpy(plen).cuda(),
+                                           w, commit=1))
+        ref = orc.dispatch(inst, dq, bq, Q, L, plen, np.asarray(w, dtype=np.float32))
+        for key in ("assignment", "order", "scores"):
+            assert np.array_equal(g[key], ref[key], equal_nan=True), (case, key, w)
+        dq, bq = ref["queued"], ref["running"]
+        s = rt.get_state()
+        assert np.array_equal(s[0].numpy(), dq) and np.array_equal(s[1].numpy(), bq), (case, "state", w)
+    rt.close()
+
+
 def test_deferred_advance_is_applied_in_call_order(orc):
     """rb_advance_state is deferred into the next rb_decide's first kernel; every other reader or writer of the state
     must see it applied (or, for an overwrite, dropped): sequences of advances, reads, overwrites and both decision
