@@ -246,6 +246,23 @@ rb_status rb_decide_from_predictions_budgeted(rb_ctx* ctx, const float* quality,
                                               int32_t commit, int32_t* assignment, int32_t* max_tokens, float* scores,
                                               float* scores0, int32_t* order);
 
+/* rb_decide_from_predictions for callers that may not allocate (code inside a CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): the same score + dispatch stages (Eq. 1), launched
+ * directly on the context's stream, with the kernels' scratch -- the per-(request, tier) terms and the LPT keys -- in a
+ * fixed __device__ array of the library (69,632 bytes per GPU that loads the library, held until the process exits)
+ * instead of allocated buffers.  The call allocates nothing: no cudaMalloc / cudaFree, no graph capture or instantiation,
+ * no staging copies, no stream synchronisation.
+ *   quality, outlen  [device] B x M fp32;   prompt_len [device] B int32;   assignment [device] B int32 (-1 as rb_decide)
+ *   w, commit        as rb_decide_from_predictions; pending rb_advance_state calls are applied first, as there
+ * Limit: 1 <= B <= 1024 and B * M <= 8192; beyond it RB_EINVAL (rb_last_error names the limit), nothing launched.
+ * RB_EINVAL also for a host pointer.  The array is ONE per GPU, shared by every context and every call, and keeps the last
+ * call's contents (nothing in it has to start at zero: every word a call reads it has written first): calls that overlap
+ * on the GPU -- two contexts on different streams, or threads -- race on it; calls on one stream do not.
+ * Results equal rb_decide_from_predictions' bit for bit. */
+rb_status rb_decide_from_predictions_static(rb_ctx* ctx, const float* quality, const float* outlen,
+                                            const int32_t* prompt_len, int32_t B, const float w[3],
+                                            int32_t commit, int32_t* assignment);
+
 /* Weight sweep ("RouteBalance sweeps 16 weight tuples on the simplex"; "turning only the weight vector,
  * RouteBalance traces a monotone frontier"): P independent score + dispatch passes over the same predictions from the
  * same dead-reckoned state, one per weight vector, none committed.  Point p's result equals that of

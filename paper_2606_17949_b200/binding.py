@@ -26,7 +26,7 @@ RB_OK, RB_EINVAL, RB_ECUDA, RB_ENOMEM, RB_ESTATE, RB_EUNSUPPORTED = range(6)
 RB_F32, RB_BF16 = 0, 1
 _STATUS = {0: "RB_OK", 1: "RB_EINVAL", 2: "RB_ECUDA", 3: "RB_ENOMEM", 4: "RB_ESTATE", 5: "RB_EUNSUPPORTED"}
 EXPORTS = ["rb_options_default", "rb_create", "rb_set_instances", "rb_set_tpot_forest", "rb_set_telemetry", "rb_set_state", "rb_get_state", "rb_advance_state",
-           "rb_batch_target", "rb_decide", "rb_decide_submit", "rb_decide_collect", "rb_decide_budgeted", "rb_decide_from_predictions", "rb_decide_from_predictions_budgeted", "rb_sweep_weights", "rb_estimate", "rb_dispatch_pipeline", "rb_match_replay", "rb_set_stage_timing", "rb_last_stage_us", "rb_last_scan_device_us", "rb_selftest_division", "rb_testing_read_bandwidth",
+           "rb_batch_target", "rb_decide", "rb_decide_submit", "rb_decide_collect", "rb_decide_budgeted", "rb_decide_from_predictions", "rb_decide_from_predictions_budgeted", "rb_decide_from_predictions_static", "rb_sweep_weights", "rb_estimate", "rb_dispatch_pipeline", "rb_match_replay", "rb_set_stage_timing", "rb_last_stage_us", "rb_last_scan_device_us", "rb_selftest_division", "rb_testing_read_bandwidth",
            "rb_launch_count", "rb_sync", "rb_last_error", "rb_destroy"]
 
 
@@ -69,6 +69,7 @@ _lib.rb_decide_collect.argtypes = [_vp, _vp, _i32]
 _lib.rb_decide.argtypes = [_vp, _vp, _vp, _i32, ctypes.POINTER(_f * 3), _vp, _vp, _vp, _vp, _vp, _vp]
 _lib.rb_decide_from_predictions.argtypes = [_vp, _vp, _vp, _vp, _i32, ctypes.POINTER(_f * 3), _i32, _vp, _vp, _vp, _vp]
 _lib.rb_decide_budgeted.argtypes = [_vp, _vp, _vp, _vp, _i32, ctypes.POINTER(_f * 3), _vp, _vp, _vp, _vp, _vp, _vp, _vp]
+_lib.rb_decide_from_predictions_static.argtypes = [_vp, _vp, _vp, _vp, _i32, ctypes.POINTER(_f * 3), _i32, _vp]
 _lib.rb_decide_from_predictions_budgeted.argtypes = [_vp, _vp, _vp, _vp, _vp, _i32, ctypes.POINTER(_f * 3), _i32, _vp, _vp,
                                                      _vp, _vp, _vp]
 _lib.rb_sweep_weights.argtypes = [_vp, _vp, _vp, _vp, _vp, _i32, _vp, _i32, _vp]
@@ -227,6 +228,13 @@ def rb_decide_from_predictions(ctx, quality, outlen, prompt_len, B, w, commit, a
     _check(ctx, _lib.rb_decide_from_predictions(ctx, _ptr(quality, f32), _ptr(outlen, f32), _ptr(prompt_len, i32), B,
                                                 _w3(w), int(commit), _ptr(assignment, i32), _ptr(scores, f32),
                                                 _ptr(scores0, f32), _ptr(order, i32)))
+
+
+def rb_decide_from_predictions_static(ctx, quality, outlen, prompt_len, B, w, commit, assignment):
+    """rb_decide_from_predictions without any allocation (device buffers only; B <= 1024, B * M <= 8192)."""
+    f32, i32 = (torch.float32, torch.int32) if torch else (np.float32, np.int32)
+    _check(ctx, _lib.rb_decide_from_predictions_static(ctx, _ptr(quality, f32), _ptr(outlen, f32), _ptr(prompt_len, i32), B,
+                                                       _w3(w), int(commit), _ptr(assignment, i32)))
 
 
 def rb_decide_budgeted(ctx, query_emb, prompt_len, budget, B, w, assignment, max_tokens=None, scores=None,

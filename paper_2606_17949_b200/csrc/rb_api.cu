@@ -1345,6 +1345,42 @@ rb_status rb_decide_from_predictions_budgeted(rb_ctx* ctx, const float* quality,
   return sg.finish();
 }
 
+rb_status rb_decide_from_predictions_static(rb_ctx* ctx, const float* quality, const float* outlen,
+                                            const int32_t* prompt_len, int32_t B, const float w[3], int32_t commit,
+                                            int32_t* assignment) {
+  if (!ctx) return RB_EINVAL;
+  if (ctx->I == 0) return fail(ctx, RB_ESTATE, "rb_decide_from_predictions_static before rb_set_instances");
+  if (ctx->opt.latency_mode == 2 && !ctx->has_forest) return fail(ctx, RB_ESTATE, "latency_mode 2 needs rb_set_tpot_forest first");
+  if (!quality || !outlen || !prompt_len || !assignment) return fail(ctx, RB_EINVAL, "NULL argument");
+  if (B < 1 || B > static_scratch_max_b() || (long long)B * ctx->M > static_scratch_max_bm()) {
+    char buf[160];
+    snprintf(buf, sizeof buf, "rb_decide_from_predictions_static: B = %d with M = %d exceeds the static scratch (1 <= B <= %d and B * M <= %d)",
+             (int)B, ctx->M, static_scratch_max_b(), static_scratch_max_bm());
+    return fail(ctx, RB_EINVAL, buf);
+  }
+  // (host buffers would need staging copies through allocated memory and a stream synchronisation: not this entry point)
+  if (is_host_ptr(quality) || is_host_ptr(outlen) || is_host_ptr(prompt_len) || is_host_ptr(assignment))
+    return fail(ctx, RB_EINVAL, "rb_decide_from_predictions_static: quality, outlen, prompt_len and assignment must be device memory");
+  rb_status st = check_weights(ctx, w);
+  if (st != RB_OK) return st;
+  st = flush_pending(ctx);   // the score kernel's CTAs all read the state: it must be current before they start
+  if (st != RB_OK) return st;
+  CallParams cp{};
+  cp.w_qual = w[0]; cp.w_lat = w[1]; cp.w_cost = w[2]; cp.commit = commit ? 1 : 0;
+  cp.q_src = quality;
+  cp.l_src = outlen;
+  cp.plen = prompt_len;
+  cp.assignment = assignment;
+  InstTable t = table_of(ctx);
+  if (ctx->opt.latency_mode == 2) {   // the head over the batch-start state
+    CK(launch_tpot_forest(t, forest_of(ctx), ctx->dq, ctx->bq, ctx->f_tpot0, -1.0f, ctx->stream));
+    ctx->launches += 1;
+  }
+  CK(launch_score_dispatch_static(t, ctx->dq, ctx->bq, cp, B, modes_of(ctx), forest_of(ctx), ctx->stream));
+  ctx->launches += 2;
+  return RB_OK;
+}
+
 rb_status rb_sweep_weights(rb_ctx* ctx, const float* quality, const float* outlen, const int32_t* prompt_len,
                            const float* budget, int32_t B, const float* w, int32_t P, int32_t* assignment) {
   if (!ctx) return RB_EINVAL;

@@ -305,6 +305,14 @@ cudaError_t launch_lpt_dispatch(InstTable t, float* dq, int32_t* bq, const float
 
 cudaError_t lpt_dispatch_prepare();  // opt in to the dynamic shared memory size; call once
 
+// a4..a7 from caller-supplied predictions (cp->q_src, cp->l_src) with the terms and keys in a file-scope __device__ array
+// of score_dispatch.cu instead of allocated buffers (rb_decide_from_predictions_static): B <= static_scratch_max_b() and
+// B * M <= static_scratch_max_bm(), else cudaErrorInvalidValue.  Allocates nothing.
+int static_scratch_max_b();
+int static_scratch_max_bm();
+cudaError_t launch_score_dispatch_static(InstTable t, float* dq, int32_t* bq, const CallParams& cp, int B, DispatchModes modes,
+                                         ForestDev forest, cudaStream_t s);
+
 // Boosted head over the current state: tpot_out[i] = max(base + sum of leaves (fp32, tree order), 1e-6) for every
 // instance (one CTA per instance, one thread per tree, sequential sum by thread 0).  elapsed_ms >= 0: also applies
 // the a8 drain rule with that tpot (rb_advance_state under latency_mode 2).

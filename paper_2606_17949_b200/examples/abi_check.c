@@ -36,6 +36,7 @@ int main(void) {
     if (rb_batch_target(NULL, 4, 64, a, NULL) != RB_EINVAL) return 14;
     if (rb_decide_submit(NULL, dummy, a, 1, w) != RB_EINVAL || rb_decide_collect(NULL, a, 1) != RB_EINVAL) return 15;
     if (rb_sweep_weights(NULL, dummy, dummy, a, NULL, 1, w, 1, a) != RB_EINVAL) return 13;
+    if (rb_decide_from_predictions_static(NULL, dummy, dummy, a, 1, w, 0, a) != RB_EINVAL) return 16;
     if (rb_launch_count(NULL) != 0) return 11;
     if (strcmp(rb_last_error(NULL), "null context") != 0) return 12;
     rb_destroy(NULL);

@@ -159,6 +159,16 @@ class Router:
                                           out["scores"], out["scores0"], out["order"])
         return out
 
+    def decide_from_predictions_static(self, quality, outlen, prompt_len, w, commit=0, assignment=None):
+        """The allocation-free entry point (rb_decide_from_predictions_static): device tensors only; `assignment` may be a
+        caller-owned int32 device tensor (then nothing is allocated on the Python side either).  Returns the assignment."""
+        B = quality.shape[0]
+        if assignment is None:
+            assignment = self._buf((B,), torch.int32, quality.device)
+        with self._ordered(quality, outlen, prompt_len, assignment):
+            rb.rb_decide_from_predictions_static(self.ctx, quality, outlen, prompt_len, B, w, commit, assignment)
+        return assignment
+
     def sweep_weights(self, quality, outlen, prompt_len, weights, budget=None, out_device=None):
         """P weight vectors over the same predictions and state, none committed: assignment [P, B]."""
         B = quality.shape[0]
