@@ -7,6 +7,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -71,6 +72,7 @@ struct rb_ctx {
     cudaEvent_t ev_back = nullptr;    // back half (finish + dispatch) done, recorded on the context's stream
   } slot[kSlots];
   cudaStream_t front = nullptr;       // low-priority internal stream of the bank scans
+  cudaStream_t front2 = nullptr;      // second stream of the bank scans (see run_pipelined)
   cudaStream_t sstage = nullptr;      // internal stream of the staging kernels (they run beside the scan before them)
   uint64_t pipe_seq = 0;              // pipelined decisions issued so far (slot = seq % kSlots)
   bool front_busy = false;            // a front half may still be running on the internal stream
@@ -454,40 +456,36 @@ rb_status run_path(rb_ctx* ctx, int B, int kind) {
   return st;
 }
 
-// rb_decide in throughput mode (rb_options.pipeline): the bank scan goes to the internal low-priority stream, where the
-// scans of consecutive decisions follow one another; the query staging in front of it to a second internal stream, so
+// rb_decide in throughput mode (rb_options.pipeline): the bank scan goes to one of two internal low-priority streams
+// (consecutive decisions alternate); the query staging in front of it to a second internal stream, so
 // that it runs beside the scan of the decision before (C2, B = 11: 33.1 -> 31.0 us per decision); the back half
 // (finishing + dispatch) to the context's stream.  Events join the three; kSlots buffer sets rotate
 // (three: with two, the scan of decision j + 2 waits for the back half of decision j, and a host loop of submissions is
 // limited to two in flight, i.e. to half a decision's latency per decision).
-rb_status run_pipelined(rb_ctx* ctx, int B, bool paced) {
+rb_status run_pipelined(rb_ctx* ctx, int B) {
   const int sl = (int)(ctx->pipe_seq % kSlots);
   rb_ctx::Slot& S = ctx->slot[sl];
   Timer tm(ctx);
-  // staging: beside the scan of the decision before (on the SMs that scan leaves free), once the back half that last
-  // read this buffer set is done
-  // (B > 32: the back half is the longer one and the next scan waits for it through this buffer set; staging then
-  // goes in front of its scan on the same stream -- across streams the hand-over costs more than the overlap saves:
-  // B = 64 46.5 against 39.9 us per decision, B = 11 31.0 against 35.0, B = 32 33.4 against 38.4)
-  cudaStream_t sstage = B > 32 ? ctx->front : ctx->sstage;
+  // The scans of consecutive decisions alternate between two streams: the CTAs of scan j + 1 start on the SMs that the
+  // CTAs of scan j leave (its slabs end up to 3.7 us apart), instead of behind a kernel boundary and a launch gap -- C2,
+  // decisions back to back, B = 11: 30.9 -> 23.8 us per decision, B = 64: 42 -> 34.  (Two scans under way read the same
+  // bank a few MB apart, so part of the later one's lines come from L2: 23.8 us is less than one scan alone takes.)
+  // Staging: beside the scan of the decision before (on the SMs that scan leaves free), once the back half that last
+  // read this buffer set is done.  B > 32: the back half is the longer one and the next scan waits for it through this
+  // buffer set; staging then goes in front of its scan on the same stream -- across streams the hand-over costs more
+  // than the overlap saves.
+  cudaStream_t fr = (ctx->pipe_seq & 1) ? ctx->front2 : ctx->front;
+  cudaStream_t sstage = B > 32 ? fr : ctx->sstage;
   CK(cudaStreamWaitEvent(sstage, S.ev_back, 0));
-  // Calls that run ahead of the device (rb_decide with device buffers returns at once, so the queue is deep): the staging
-  // kernel also waits for the back half of the decision two before it, and so runs in the middle of the scan before its
-  // own.  Free to start at once it is launched just when the front stream launches that scan, and the scan starts later
-  // (32.4 against 30.9 us per decision, B = 11).  Submissions paced by rb_decide_collect arrive mid-scan by themselves,
-  // and there the extra wait costs the third decision in flight (36.5 against 33.6 us per decision).
-  if (!paced && B <= 32 && ctx->pipe_seq >= 2)
-    CK(cudaStreamWaitEvent(sstage, ctx->slot[(ctx->pipe_seq + 1) % kSlots].ev_back, 0));
   rb_status st = graph_run(ctx, graph_key(ctx, B, 5, sl), sstage,
                            [&]() -> rb_status { return enqueue_estimate(ctx, B, true, tm, sl, kStage, sstage); });
   if (st != RB_OK) return st;
   CK(cudaEventRecord(S.ev_stage, sstage));
-  // scan: behind the scan before it on the front stream
-  CK(cudaStreamWaitEvent(ctx->front, S.ev_stage, 0));
-  st = graph_run(ctx, graph_key(ctx, B, 3, sl), ctx->front,
-                 [&]() -> rb_status { return enqueue_estimate(ctx, B, true, tm, sl, kScan, ctx->front); });
+  CK(cudaStreamWaitEvent(fr, S.ev_stage, 0));
+  st = graph_run(ctx, graph_key(ctx, B, 3, sl), fr,
+                 [&]() -> rb_status { return enqueue_estimate(ctx, B, true, tm, sl, kScan, fr); });
   if (st != RB_OK) return st;
-  CK(cudaEventRecord(S.ev_front, ctx->front));
+  CK(cudaEventRecord(S.ev_front, fr));
   CK(cudaStreamWaitEvent(ctx->stream, S.ev_front, 0));
   st = graph_run(ctx, graph_key(ctx, B, 4, sl), ctx->stream, [&]() -> rb_status {
     rb_status s1 = enqueue_estimate(ctx, B, true, tm, sl, kBack, ctx->stream);
@@ -856,6 +854,7 @@ rb_status rb_create(rb_ctx** out, const void* bank_emb, const float* bank_qualit
       int lo = 0, hi = 0;
       CK(cudaDeviceGetStreamPriorityRange(&lo, &hi));   // lo = least priority
       CK(cudaStreamCreateWithPriority(&ctx->front, cudaStreamNonBlocking, lo));
+      CK(cudaStreamCreateWithPriority(&ctx->front2, cudaStreamNonBlocking, lo));
       CK(cudaStreamCreateWithPriority(&ctx->sstage, cudaStreamNonBlocking, hi));
       for (int j = 0; j < kSlots; ++j) {
         CK(cudaEventCreateWithFlags(&ctx->slot[j].ev_stage, cudaEventDisableTiming));
@@ -1206,7 +1205,7 @@ rb_status rb_decide_budgeted(rb_ctx* ctx, const float* query_emb, const int32_t*
   }
   st = push_params(ctx, cp);
   if (st != RB_OK) return st;
-  st = pipelined ? run_pipelined(ctx, B, false) : run_path(ctx, B, 0);
+  st = pipelined ? run_pipelined(ctx, B) : run_path(ctx, B, 0);
   if (st != RB_OK) return st;
   if (adv_folded) ctx->n_pending = 0;
   collect_stage_times(ctx, 0);
@@ -1245,7 +1244,7 @@ rb_status rb_decide_submit(rb_ctx* ctx, const float* query_emb, const int32_t* p
   cp.l_src = S.pred_l;
   st = push_params(ctx, cp);
   if (st != RB_OK) return st;
-  st = run_pipelined(ctx, B, true);
+  st = run_pipelined(ctx, B);
   if (st != RB_OK) return st;
   ctx->n_pending = 0;
   A.busy = true;
@@ -1583,6 +1582,7 @@ void rb_destroy(rb_ctx* ctx) {
   if (!ctx) return;
   if (ctx->sstage) cudaStreamSynchronize(ctx->sstage);
   if (ctx->front) cudaStreamSynchronize(ctx->front);
+  if (ctx->front2) cudaStreamSynchronize(ctx->front2);
   if (ctx->stream) cudaStreamSynchronize(ctx->stream);
   drop_graphs(ctx);
   void* ptrs[] = {ctx->bank, ctx->bank_quality, ctx->bank_outlen, ctx->arena, ctx->q32, ctx->q32_in, ctx->qs, ctx->part_sim,
@@ -1600,6 +1600,7 @@ void rb_destroy(rb_ctx* ctx) {
     if (sl.ev_back) cudaEventDestroy(sl.ev_back);
   }
   if (ctx->front) cudaStreamDestroy(ctx->front);
+  if (ctx->front2) cudaStreamDestroy(ctx->front2);
   if (ctx->sstage) cudaStreamDestroy(ctx->sstage);
   for (auto& e : ctx->ev)
     if (e) cudaEventDestroy(e);
