@@ -103,6 +103,9 @@ struct rb_ctx {
   // boosted TPOT head (latency_mode 2)
   int4* f_nodes = nullptr;
   int32_t *f_root = nullptr, *f_begin = nullptr, *f_nbegin = nullptr;   // roots, trees per tier, nodes per tier
+  uint32_t* f_cwords = nullptr;       // the packed forest (ForestDev::cwords) ...
+  int32_t* f_cbegin = nullptr;        // ... and its per-tier blocks
+  int f_total_cwords = 0, f_max_tier_cwords = 0;
   int f_max_tier_nodes = 0;
   float f_tpot_hi = 0.0f;             // bound of the head's output over all states (see ForestDev)
   float *f_base = nullptr, *f_aux = nullptr, *f_tpot0 = nullptr;
@@ -188,6 +191,7 @@ ForestDev forest_of(const rb_ctx* c) {
   ForestDev f{};
   f.nodes = c->f_nodes; f.tree_root = c->f_root; f.tier_begin = c->f_begin; f.base = c->f_base; f.aux = c->f_aux;
   f.tpot0 = c->f_tpot0; f.n_features = c->f_features; f.tier_node_begin = c->f_nbegin; f.max_tier_nodes = c->f_max_tier_nodes; f.tpot_hi = c->f_tpot_hi;
+  f.cwords = c->f_cwords; f.tier_cbegin = c->f_cbegin; f.total_cwords = c->f_total_cwords; f.max_tier_cwords = c->f_max_tier_cwords;
   return f;
 }
 
@@ -1026,17 +1030,56 @@ rb_status rb_set_tpot_forest(rb_ctx* ctx, const rb_tree_node* nodes, int32_t n_n
     max_tier_nodes = std::max(max_tier_nodes, (int)pk.size() - nbegin[m]);
   }
   nbegin[M] = (int32_t)pk.size();
+  // The packed copy for the dispatch loop's shared-memory cache (ForestDev::cwords): 8 bytes per inner node, 4 per leaf,
+  // so that a whole forest of the paper's size class stays resident (64 trees of depth 5 per tier, 8 tiers: 190 KB
+  // against 516 KB of 16-byte nodes).  Same tests, same leaves: a re-encoding.
+  std::vector<uint32_t> cw;
+  std::vector<int32_t> cbegin((size_t)M + 1, 0);
+  int max_tier_cwords = 0;
+  {
+    auto bits = [](float f) { uint32_t u; std::memcpy(&u, &f, 4); return u; };
+    std::vector<uint32_t> off(pk.size(), 0);
+    for (int m = 0; m < M; ++m) {
+      cbegin[m] = (int32_t)cw.size();
+      const int t0 = tier_tree_begin[m], t1 = tier_tree_begin[m + 1];
+      uint32_t o = (uint32_t)(t1 - t0);   // the roots come first
+      for (int n = nbegin[m]; n < nbegin[m + 1]; ++n) {   // pre-order: offsets in node order
+        off[n] = o;
+        o += pk[n].feature >= 0 ? 2u : 1u;
+      }
+      if (o >= (1u << 27)) return fail(ctx, RB_EINVAL, "forest too large for the packed encoding");
+      cw.resize((size_t)cbegin[m] + o, 0u);
+      uint32_t* blk = cw.data() + cbegin[m];
+      for (int tr = t0; tr < t1; ++tr) blk[tr - t0] = (off[root2[tr]] << 1) | (pk[root2[tr]].feature < 0 ? 1u : 0u);
+      for (int n = nbegin[m]; n < nbegin[m + 1]; ++n) {
+        if (pk[n].feature < 0) {
+          blk[off[n]] = bits(pk[n].value);
+        } else {
+          const int l = pk[n].left, r = pk[n].right;   // l == n + 1 (pre-order)
+          blk[off[n]] = bits(pk[n].value);
+          blk[off[n] + 1] = (uint32_t)pk[n].feature | (pk[l].feature < 0 ? 8u : 0u) | (pk[r].feature < 0 ? 16u : 0u) |
+                            ((off[r] - off[n]) << 5);
+        }
+      }
+      max_tier_cwords = std::max(max_tier_cwords, (int)o);
+    }
+    cbegin[M] = (int32_t)cw.size();
+  }
   cudaStream_t s = ctx->stream;
   CK(cudaStreamSynchronize(s));
   cudaFree(ctx->f_nodes); cudaFree(ctx->f_root); cudaFree(ctx->f_begin); cudaFree(ctx->f_base); cudaFree(ctx->f_nbegin);
+  cudaFree(ctx->f_cwords); cudaFree(ctx->f_cbegin);
   ctx->f_nodes = nullptr; ctx->f_root = ctx->f_begin = ctx->f_nbegin = nullptr; ctx->f_base = nullptr;
+  ctx->f_cwords = nullptr; ctx->f_cbegin = nullptr;
+  ctx->f_total_cwords = (int)cw.size(); ctx->f_max_tier_cwords = max_tier_cwords;
   ctx->f_max_tier_nodes = max_tier_nodes;
   ctx->f_tpot_hi = (float)std::min(2.0 * tpot_hi, 3.0e38);   // (doubled: the fp32 sum rounds)
   ctx->has_forest = false;
   static_assert(sizeof(rb_tree_node) == sizeof(int4), "rb_tree_node is read as int4");
   if (dev_alloc(&ctx->f_nodes, pk.size()) != cudaSuccess || dev_alloc(&ctx->f_root, (size_t)n_trees) != cudaSuccess ||
       dev_alloc(&ctx->f_begin, (size_t)M + 1) != cudaSuccess || dev_alloc(&ctx->f_base, (size_t)M) != cudaSuccess ||
-      dev_alloc(&ctx->f_nbegin, (size_t)M + 1) != cudaSuccess) {
+      dev_alloc(&ctx->f_nbegin, (size_t)M + 1) != cudaSuccess || dev_alloc(&ctx->f_cwords, cw.size()) != cudaSuccess ||
+      dev_alloc(&ctx->f_cbegin, (size_t)M + 1) != cudaSuccess) {
     cudaGetLastError();
     return fail(ctx, RB_ENOMEM, "cudaMalloc forest");
   }
@@ -1045,6 +1088,8 @@ rb_status rb_set_tpot_forest(rb_ctx* ctx, const rb_tree_node* nodes, int32_t n_n
   CK(cudaMemcpyAsync(ctx->f_begin, tier_tree_begin, (size_t)(M + 1) * 4, cudaMemcpyHostToDevice, s));
   CK(cudaMemcpyAsync(ctx->f_nbegin, nbegin.data(), (size_t)(M + 1) * 4, cudaMemcpyHostToDevice, s));
   CK(cudaMemcpyAsync(ctx->f_base, base, (size_t)M * 4, cudaMemcpyHostToDevice, s));
+  CK(cudaMemcpyAsync(ctx->f_cwords, cw.data(), cw.size() * 4, cudaMemcpyHostToDevice, s));
+  CK(cudaMemcpyAsync(ctx->f_cbegin, cbegin.data(), (size_t)(M + 1) * 4, cudaMemcpyHostToDevice, s));
   CK(cudaStreamSynchronize(s));
   if (n_features != ctx->f_features) CK(cudaMemsetAsync(ctx->f_aux, 0, (size_t)kMaxI * kMaxFeatures * 4, s));
   ctx->f_features = n_features;
@@ -1587,7 +1632,7 @@ void rb_destroy(rb_ctx* ctx) {
   drop_graphs(ctx);
   void* ptrs[] = {ctx->bank, ctx->bank_quality, ctx->bank_outlen, ctx->arena, ctx->q32, ctx->q32_in, ctx->qs, ctx->part_sim,
                   ctx->gthr, ctx->bank32, ctx->scratch_nn_idx, ctx->scratch_nn_sim, ctx->scores, ctx->scores0, ctx->f_nodes,
-                  ctx->f_root, ctx->f_begin, ctx->f_nbegin, ctx->f_base, ctx->dev_clock, ctx->sweep_buf};
+                  ctx->f_root, ctx->f_begin, ctx->f_nbegin, ctx->f_base, ctx->dev_clock, ctx->sweep_buf, ctx->f_cwords, ctx->f_cbegin};
   for (void* p : ptrs) cudaFree(p);
   for (int j = 1; j < kSlots; ++j) {
     cudaFree(ctx->slot[j].qs);

@@ -46,6 +46,13 @@ struct ForestDev {
   const float* aux;            // [I x (F-2)] auxiliary telemetry features
   const float* tpot0;          // [I] head evaluated on the batch-start state (tpot_kernel)
   int32_t n_features;
+  // the forest again, packed for the dispatch loop's shared-memory cache: tier t's block = cwords[tier_cbegin[t] ..
+  // tier_cbegin[t+1]) = [one root word per tree | nodes in pre-order]; an inner node is two words (threshold bits;
+  // feature | left-is-leaf << 3 | right-is-leaf << 4 | (right child's offset - own offset) << 5), its left child follows
+  // it; a leaf is one word (value bits); a root word = (offset in the block) << 1 | is-leaf
+  const uint32_t* cwords;
+  const int32_t* tier_cbegin;  // [M+1]
+  int32_t total_cwords, max_tier_cwords;
   float tpot_hi;               // no evaluation of the head exceeds this (|base| + sum of the trees' largest |leaf|, doubled)
 };
 
