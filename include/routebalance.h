@@ -70,9 +70,9 @@ typedef struct {
                           /* RB_BF16: bank and queries are rounded to bf16 (RNE) once; similarity is the   */
                           /* dot product of the rounded values (tcgen05 tensor-core scan).                 */
                           /* RB_F32: the similarity is the dot product of the fp32 values.  The bank is also kept  */
-                          /* as a three-plane bf16 split (x = hi + mid + lo) that the same tensor-core scan reads   */
-                          /* (candidates good to ~5e-6); the k + slack candidates are then re-ranked exactly from   */
-                          /* the fp32 rows.  14 bytes per value: meant for small banks.                            */
+                          /* as a two-plane bf16 split (x ~ hi + mid, three column blocks) that the same tensor-core  */
+                          /* scan reads (candidates good to ~1e-5); the k + slack candidates are then re-ranked       */
+                          /* exactly from the fp32 rows.  10 bytes per value: meant for small banks.                  */
   int32_t weight_mode;    /* 0: inverse distance 1/(dist+eps) ("distance-weighted"); 1: uniform     */
   float dist_eps;         /* eps above.                                                   default 1e-6    */
   int32_t rerank_slack;   /* the scan keeps k+slack candidates per query, their similarities are recomputed       */

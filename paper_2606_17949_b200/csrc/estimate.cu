@@ -23,18 +23,18 @@ __device__ __forceinline__ unsigned long long make_key(float sim, int32_t idx) {
 }
 
 // ---- a0 ---------------------------------------------------------------------------------------------
-// fp32 -> three bf16 planes: hi = bf16(x), mid = bf16(x - hi), lo = bf16(x - hi - mid) (both differences are exact in
-// fp32), so that x = hi + mid + lo up to 2^-27 |x|.
-__device__ __forceinline__ void split3(float x, __nv_bfloat16* hi, __nv_bfloat16* mid, __nv_bfloat16* lo) {
+// fp32 -> two bf16 planes: hi = bf16(x), mid = bf16(x - hi) (the difference is exact in fp32), so that x = hi + mid up to
+// 2^-18 |x|.
+__device__ __forceinline__ void split2(float x, __nv_bfloat16* hi, __nv_bfloat16* mid) {
   *hi = __float2bfloat16_rn(x);
-  const float r1 = __fsub_rn(x, __bfloat162float(*hi));
-  *mid = __float2bfloat16_rn(r1);
-  *lo = __float2bfloat16_rn(__fsub_rn(r1, __bfloat162float(*mid)));
+  *mid = __float2bfloat16_rn(__fsub_rn(x, __bfloat162float(*hi)));
 }
 
-// split = 0: qs[row, c] = bf16(q[r, c]).  split = 1 (fp32 storage): rows of 5 d columns [hi | hi | mid | hi | lo], the
-// query's side of the split scan (bank rows hold [hi | mid | hi | lo | hi]): the scan's dot product is then
-// x_hi e_hi + x_hi e_mid + x_mid e_hi + x_hi e_lo + x_lo e_hi, the fp32 dot product up to 2^-18 sum |x_c e_c|.
+// split = 0: qs[row, c] = bf16(q[r, c]).  split = 1 (fp32 storage): rows of kSplitPlanes d columns [hi | hi | mid], the
+// query's side of the split scan (bank rows hold [hi | mid | hi]): the scan's dot product is then
+// x_hi e_hi + x_hi e_mid + x_mid e_hi, the fp32 dot product up to 3 * 2^-18 sum |x_c e_c| (the mid-mid and the two
+// third-plane terms) -- 1.1e-5 at most for unit vectors; it picks the k + slack candidates, whose similarities are then
+// recomputed from the fp32 rows.  (Five planes, [hi | mid | hi | lo | hi], were 5e-6 for 5/3 of the bytes and flops.)
 __global__ void stage_queries_kernel(const __grid_constant__ CallParams cpv, __nv_bfloat16* __restrict__ qs, int B, int Bpad,
                                      int d, int group, uint32_t* __restrict__ gthr, int n_gthr, int split,
                                      float* __restrict__ q32) {
@@ -50,23 +50,23 @@ __global__ void stage_queries_kernel(const __grid_constant__ CallParams cpv, __n
     if (!split) {
       qs[i] = __float2bfloat16_rn(x);
     } else {
-      __nv_bfloat16 hi, mid, lo;
-      split3(x, &hi, &mid, &lo);
-      __nv_bfloat16* o = qs + row * 5 * (size_t)d + c;
-      o[0] = hi; o[d] = hi; o[2 * (size_t)d] = mid; o[3 * (size_t)d] = hi; o[4 * (size_t)d] = lo;
+      __nv_bfloat16 hi, mid;
+      split2(x, &hi, &mid);
+      __nv_bfloat16* o = qs + row * kSplitPlanes * (size_t)d + c;
+      o[0] = hi; o[d] = hi; o[2 * (size_t)d] = mid;
       if (row < (size_t)B) q32[i] = x;   // device copy of the fp32 rows for the exact re-rank (the caller's may be host memory)
     }
   }
 }
-// fp32 bank [n x d] -> split bank [n x 5 d] bf16: [hi | mid | hi | lo | hi] (rb_create, fp32 storage)
+// fp32 bank [n x d] -> split bank [n x kSplitPlanes d] bf16: [hi | mid | hi] (rb_create, fp32 storage)
 __global__ void split_bank_kernel(const float* __restrict__ in, __nv_bfloat16* __restrict__ out, size_t rows, int d) {
   const size_t n = rows * d;
   for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
     const size_t row = i / d, c = i - row * d;
-    __nv_bfloat16 hi, mid, lo;
-    split3(in[i], &hi, &mid, &lo);
-    __nv_bfloat16* o = out + row * 5 * (size_t)d + c;
-    o[0] = hi; o[d] = mid; o[2 * (size_t)d] = hi; o[3 * (size_t)d] = lo; o[4 * (size_t)d] = hi;
+    __nv_bfloat16 hi, mid;
+    split2(in[i], &hi, &mid);
+    __nv_bfloat16* o = out + row * kSplitPlanes * (size_t)d + c;
+    o[0] = hi; o[d] = mid; o[2 * (size_t)d] = hi;
   }
 }
 // Plain streaming read (rb_testing_read_bandwidth): every thread sums 16-byte loads, 8 in flight; one word written per block.

@@ -30,9 +30,9 @@ struct rb_ctx {
   bool own_stream = false;
   int num_sms = 148;
   // bank
-  void* bank = nullptr;          // what the tensor-core scan reads: bf16 [N x d], or (fp32 storage) the split bank bf16 [N x 5 d]
+  void* bank = nullptr;          // what the tensor-core scan reads: bf16 [N x d], or (fp32 storage) the split bank bf16 [N x 3 d]
   float* bank32 = nullptr;       // fp32 storage: the fp32 bank [N x d] the exact re-rank reads
-  int d_scan = 0;                // columns of a scanned row: d, or 5 d (fp32 storage: three-plane bf16 split)
+  int d_scan = 0;                // columns of a scanned row: d, or kSplitPlanes d (fp32 storage: two-plane bf16 split)
   float* bank_quality = nullptr; // [N x M]
   float* bank_outlen = nullptr;
   // instances
@@ -688,7 +688,7 @@ rb_status rb_create(rb_ctx** out, const void* bank_emb, const float* bank_qualit
   rb_ctx* ctx = new (std::nothrow) rb_ctx();
   if (!ctx) return RB_ENOMEM;
   ctx->N = N; ctx->d = d; ctx->M = M; ctx->k = k; ctx->opt = opt;
-  ctx->d_scan = opt.store_dtype == RB_F32 ? 5 * d : d;
+  ctx->d_scan = opt.store_dtype == RB_F32 ? kSplitPlanes * d : d;
   ctx->kc = k + opt.rerank_slack;
   ctx->kcap = ctx->kc <= 16 ? 16 : (ctx->kc <= 32 ? 32 : 64);
   ctx->num_sms = prop.multiProcessorCount;
@@ -770,11 +770,11 @@ rb_status rb_create(rb_ctx** out, const void* bank_emb, const float* bank_qualit
       cudaFree(tmp);
     }
   } else {
-    // fp32 storage: the fp32 rows (exact re-rank) and their three-plane bf16 split (what the tensor cores scan)
+    // fp32 storage: the fp32 rows (exact re-rank) and their two-plane bf16 split in three column blocks (what the tensor cores scan)
     ALLOC(ctx->bank32, nd);
     CK(cudaMemcpyAsync(ctx->bank32, bank_emb, nd * 4, cudaMemcpyDefault, s));
     __nv_bfloat16* bs = nullptr;
-    ALLOC(bs, 5 * nd);
+    ALLOC(bs, kSplitPlanes * nd);
     ctx->bank = bs;
     CK(launch_split_bank(ctx->bank32, bs, (size_t)N, d, s));
   }

@@ -14,6 +14,7 @@ constexpr int kTileM = 128;        // queries per MMA tile (TMEM lanes)
 constexpr int kTileN = 256;        // bank rows per MMA tile (TMEM columns of one accumulator)
 constexpr int kBoxN = 64;          // bank rows per TMA box
 constexpr int kSlots = 3;          // buffer sets of the throughput mode = decisions that can be in flight
+constexpr int kSplitPlanes = 3;     // fp32 storage: bf16 columns per fp32 column in the scanned rows ([hi | mid | hi] x [hi | hi | mid])
 constexpr int kRowUnit = 16;       // the single-CTA scan splits the bank over its CTAs in groups of this many rows
 constexpr int kTileK = 64;         // bf16 per K chunk = one 128-byte swizzle row
 constexpr int kMaxPendingAdvance = 4;   // rb_advance_state calls a decision can absorb (CallParams::adv_ms)
@@ -232,10 +233,10 @@ cudaError_t launch_convert_bf16(const float* in, __nv_bfloat16* out, size_t n, c
 
 // a0: cp->query (fp32) -> bf16 staging [Bpad x d]; rep copies of the B queries at rows j*(128/rep) + r (rep > 1 only
 // when Bpad = 128), all other rows zero.  Also clears gthr [n_gthr] (the scan's cross-slab thresholds).
-// split = 1 (fp32 storage): rows of 5 d columns [hi | hi | mid | hi | lo] of the three-plane bf16 split of every value.
+// split = 1 (fp32 storage): rows of kSplitPlanes d columns [hi | hi | mid] of the two-plane bf16 split of every value.
 cudaError_t launch_stage_queries(const CallParams& cp, __nv_bfloat16* qs, int B, int Bpad, int d, int rep, uint32_t* gthr,
                                  int n_gthr, int split, float* q32 /* split: device copy of the B fp32 rows */, cudaStream_t s);
-// fp32 bank rows -> [hi | mid | hi | lo | hi] bf16 rows of 5 d columns (fp32 storage: the bank the tensor-core scan reads)
+// fp32 bank rows -> [hi | mid | hi] bf16 rows of kSplitPlanes d columns (fp32 storage: the bank the tensor-core scan reads)
 cudaError_t launch_split_bank(const float* in, __nv_bfloat16* out, size_t rows, int d, cudaStream_t s);
 // query replicas over the TMEM lane quarters: 4 (B <= 32), 2 (B <= 64), 1; halved while the finishing kernel could not
 // hold max_grid * replicas lists of kcap entries in shared memory (long lists: k = 32)
