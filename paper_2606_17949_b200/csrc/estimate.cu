@@ -42,19 +42,24 @@ __global__ void stage_queries_kernel(const __grid_constant__ CallParams cpv, __n
   launch_dependents();
   for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n_gthr; i += gridDim.x * blockDim.x) gthr[i] = 0u;
   const float* __restrict__ q = cp->query;
-  const size_t n = (size_t)Bpad * d;
+  // every query value is read once and written to all of its replica rows (rows r, group + r, ...): the queries may sit in
+  // pinned host memory (rb_decide_submit), where a read crosses the bus
+  const int nrep = Bpad / group;
+  const size_t n = (size_t)group * d;
   for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
-    const size_t row = i / d, c = i - row * d;
-    const size_t r = row % group;   // replicas of query r at rows r, group + r, ...
-    const float x = (r < (size_t)B) ? q[r * d + c] : 0.0f;
+    const size_t r = i / d, c = i - r * d;
+    const float x = (r < (size_t)B) ? q[i] : 0.0f;
     if (!split) {
-      qs[i] = __float2bfloat16_rn(x);
+      const __nv_bfloat16 v = __float2bfloat16_rn(x);
+      for (int j = 0; j < nrep; ++j) qs[((size_t)j * group + r) * d + c] = v;
     } else {
       __nv_bfloat16 hi, mid;
       split2(x, &hi, &mid);
-      __nv_bfloat16* o = qs + row * kSplitPlanes * (size_t)d + c;
-      o[0] = hi; o[d] = hi; o[2 * (size_t)d] = mid;
-      if (row < (size_t)B) q32[i] = x;   // device copy of the fp32 rows for the exact re-rank (the caller's may be host memory)
+      for (int j = 0; j < nrep; ++j) {
+        __nv_bfloat16* o = qs + ((size_t)j * group + r) * kSplitPlanes * (size_t)d + c;
+        o[0] = hi; o[d] = hi; o[2 * (size_t)d] = mid;
+      }
+      if (r < (size_t)B) q32[i] = x;   // device copy of the fp32 rows for the exact re-rank (the caller's may be host memory)
     }
   }
 }
@@ -118,10 +123,12 @@ cudaError_t launch_read_stream(const void* buf, size_t bytes, uint32_t* sink, cu
 
 cudaError_t launch_stage_queries(const CallParams& cp, __nv_bfloat16* qs, int B, int Bpad, int d, int rep, uint32_t* gthr,
                                  int n_gthr, int split, float* q32, cudaStream_t s) {
-  const size_t n = (size_t)Bpad * d;
-  int blocks = (int)((n + 255) / 256);
+  const int group = rep > 1 ? kTileM / rep : Bpad;
+  const size_t n = (size_t)group * d;
+  int blocks = (int)((n + 127) / 128);
   if (blocks > 148 * 8) blocks = 148 * 8;
-  stage_queries_kernel<<<blocks, 256, 0, s>>>(cp, qs, B, Bpad, d, rep > 1 ? kTileM / rep : Bpad, gthr, n_gthr, split, q32);
+  if (blocks < 1) blocks = 1;
+  stage_queries_kernel<<<blocks, 128, 0, s>>>(cp, qs, B, Bpad, d, group, gthr, n_gthr, split, q32);
   return cudaGetLastError();
 }
 
