@@ -475,11 +475,9 @@ rb_status run_pipelined(rb_ctx* ctx, int B) {
   // decisions back to back, B = 11: 30.9 -> 23.8 us per decision, B = 64: 42 -> 34.  (Two scans under way read the same
   // bank a few MB apart, so part of the later one's lines come from L2: 23.8 us is less than one scan alone takes.)
   // Staging: beside the scan of the decision before (on the SMs that scan leaves free), once the back half that last
-  // read this buffer set is done.  B > 32: the back half is the longer one and the next scan waits for it through this
-  // buffer set; staging then goes in front of its scan on the same stream -- across streams the hand-over costs more
-  // than the overlap saves.
+  // read this buffer set is done.
   cudaStream_t fr = (ctx->pipe_seq & 1) ? ctx->front2 : ctx->front;
-  cudaStream_t sstage = B > 32 ? fr : ctx->sstage;
+  cudaStream_t sstage = ctx->sstage;
   CK(cudaStreamWaitEvent(sstage, S.ev_back, 0));
   rb_status st = graph_run(ctx, graph_key(ctx, B, 5, sl), sstage,
                            [&]() -> rb_status { return enqueue_estimate(ctx, B, true, tm, sl, kStage, sstage); });
