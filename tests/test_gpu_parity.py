@@ -1028,7 +1028,7 @@ def test_adaptive_batch_rule_and_stream_driver_lockstep(orc):
 
 def test_pipelined_decisions_equal_unpipelined_ones(orc):
     """rb_options.pipeline (throughput mode: the bank scan of a decision overlaps the finishing and dispatch stages of the
-    one before it, two buffer sets alternating): a stream of 300 decisions of varying size with rb_advance_state between
+    one before it, three buffer sets rotating, consecutive scans on two streams): a stream of 300 decisions of varying size with rb_advance_state between
     them, estimate-only calls, state reads and a budgeted call mixed in, gives bit for bit the outputs and the final state
     of the same calls on an unpipelined context; and the first 40 decisions are checked against the oracle in lock-step."""
     cfg = dataclasses.replace(synth.CONFIGS["C2"], N=30000, d=256, Kc=16, seed=61)
