@@ -95,7 +95,7 @@ typedef struct {
                           /* 2: live gradient-boosted TPOT head (rb_set_tpot_forest) in place of the linear one;   */
                           /* 1: static per-tier prior T^ = decode_ms_per_tok * L^ ("nominal TPOT x predicted       */
                           /* length; zero telemetry", P:L227 arm 4): no wait, batch-slope or prefill term          */
-  int32_t pipeline;       /* 1 (RB_BF16 storage only): consecutive rb_decide calls with DEVICE buffers and at most 128     */
+  int32_t pipeline;       /* 1: consecutive rb_decide calls with DEVICE buffers and at most 128                            */
                           /* requests overlap -- the bank scan of a call runs on an internal stream (its query staging on */
                           /* another, beside the scan before it) while the finishing and dispatch stages of the call     */
                           /* before it run on the context's stream.  Device inputs of                                    */

@@ -670,7 +670,7 @@ rb_status rb_create(rb_ctx** out, const void* bank_emb, const float* bank_qualit
   if (opt.tiebreak_mode != 0 && opt.tiebreak_mode != 1) return RB_EINVAL;
   if (opt.latency_mode < 0 || opt.latency_mode > 2) return RB_EINVAL;
   opt.lpt_enabled = opt.lpt_enabled ? 1 : 0;
-  opt.pipeline = (opt.pipeline && opt.store_dtype == RB_BF16) ? 1 : 0;
+  opt.pipeline = opt.pipeline ? 1 : 0;
   if (opt.scan_list != 0 && opt.scan_list != 4 && opt.scan_list != 8 && opt.scan_list != 16 && opt.scan_list != 32 &&
       opt.scan_list != 64)
     return RB_EINVAL;
@@ -844,12 +844,12 @@ rb_status rb_create(rb_ctx** out, const void* bank_emb, const float* bank_qualit
       // further buffer sets, for batches of at most 128 requests (larger ones are not pipelined)
       for (int j = 1; j < kSlots; ++j) {
         rb_ctx::Slot& S1 = ctx->slot[j];
-        ALLOC(S1.qs, (size_t)kTileM * d);
+        ALLOC(S1.qs, (size_t)kTileM * ds);
         const size_t part_n1 = (size_t)ctx->num_sms * ctx->kcap * 4 * kTileM;
         ALLOC(S1.part_sim, 2 * part_n1);
         S1.part_idx = reinterpret_cast<int32_t*>(S1.part_sim + part_n1);
-        CK(cudaMemsetAsync(S1.qs, 0, (size_t)kTileM * d * 2, s));
-        st = encode_map(ctx, &S1.tm_q, S1.qs, (uint64_t)kTileM, (uint64_t)d, kTileM);
+        CK(cudaMemsetAsync(S1.qs, 0, (size_t)kTileM * ds * 2, s));
+        st = encode_map(ctx, &S1.tm_q, S1.qs, (uint64_t)kTileM, (uint64_t)ds, kTileM);
         if (st != RB_OK) return st;
         ALLOC(S1.q32, (size_t)kTileM * d);
       }

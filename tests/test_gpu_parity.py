@@ -1026,6 +1026,52 @@ def test_adaptive_batch_rule_and_stream_driver_lockstep(orc):
     rt.close()
 
 
+def test_pipelined_decisions_under_fp32_storage():
+    """Throughput mode under fp32 storage (the staging kernel leaves the fp32 query rows of every buffer set for the exact
+    re-rank): 90 decisions of varying size through rb_decide with device buffers and through rb_decide_submit /
+    rb_decide_collect give the assignments and the final state of an unpipelined context, bit for bit."""
+    from paper_2606_17949_b200 import binding as rb
+    cfg = dataclasses.replace(synth.CONFIGS["C1"], N=9000, d=192, Kc=16, seed=63)
+    assert cfg.store == "f32"
+    bank = synth.make_bank(cfg, device="cuda")
+    it = synth.make_instances(cfg.I, cfg.M, cap=5)
+    queued, running = synth.make_state(cfg.I, it["cap"], cfg.seed)
+    rng = np.random.default_rng(63)
+    sizes = [int(x) for x in rng.integers(1, 97, 90)]
+    offs = np.concatenate([[0], np.cumsum(sizes)])
+    q = synth.make_queries(cfg, B=int(offs[-1]), device="cuda")
+    p = synth.make_prompt_len(cfg, B=int(offs[-1]), device="cuda")
+    qh, ph = q.cpu().pin_memory(), p.cpu().pin_memory()
+    torch.cuda.synchronize()
+    presets = list(synth.PRESETS.values())
+    res = []
+    for mode in ("plain", "device", "host"):
+        rt = _router(bank, cfg, max_batch=128, pipeline=0 if mode == "plain" else 1)
+        rt.set_instances(**it)
+        rt.set_state(queued, running)
+        got = torch.empty(int(offs[-1]), dtype=torch.int32, device="cpu" if mode == "host" else "cuda")
+        pending = []
+        for j, B in enumerate(sizes):
+            rt.advance_state(float(2.0 + j % 5))
+            sl = slice(int(offs[j]), int(offs[j + 1]))
+            if mode == "host":
+                rb.rb_decide_submit(rt.ctx, qh[sl], ph[sl], B, presets[j % 4])
+                pending.append(j)
+                while len(pending) >= 3:
+                    c = pending.pop(0)
+                    rb.rb_decide_collect(rt.ctx, got[int(offs[c]):int(offs[c + 1])], sizes[c])
+            else:
+                rb.rb_decide(rt.ctx, q[sl], p[sl], B, presets[j % 4], got[sl])
+        for c in pending:
+            rb.rb_decide_collect(rt.ctx, got[int(offs[c]):int(offs[c + 1])], sizes[c])
+        rt.sync()
+        s = rt.get_state()
+        res.append((got.cpu().clone(), s[0].clone(), s[1].clone()))
+        rt.close()
+    for got, dq, bq in res[1:]:
+        assert torch.equal(got, res[0][0]) and torch.equal(dq, res[0][1]) and torch.equal(bq, res[0][2])
+
+
 def test_pipelined_decisions_equal_unpipelined_ones(orc):
     """rb_options.pipeline (throughput mode: the bank scan of a decision overlaps the finishing and dispatch stages of the
     one before it, three buffer sets rotating, consecutive scans on two streams): a stream of 300 decisions of varying size with rb_advance_state between
