@@ -1110,6 +1110,12 @@ def test_pipelined_decisions_equal_unpipelined_ones(orc):
             if j % 41 == 40:
                 s = rt.get_state()
                 rec.append({"dq": s[0].clone(), "bq": s[1].clone()})
+            if j % 29 == 28:                               # other readers and writers of the state between pipelined calls
+                tgt, busy = rt.batch_target(4, 64)
+                rec.append({"target": torch.tensor([int(tgt), int(busy)])})
+            if j % 31 == 30:                               # the allocation-free score + dispatch entry point, committing
+                a2 = rt.decide_from_predictions_static(o["pred_quality"], o["pred_outlen"], pp, presets[(j + 1) % 4], commit=1)
+                rec.append({"static": a2.clone()})
             off += B
         rt.sync()
         s = rt.get_state()
