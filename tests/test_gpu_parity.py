@@ -501,7 +501,9 @@ def _forest_pair(orc, it, I, M, n_trees, depth, Fa, seed):
                                                     (33, 3, 50, 256, 2, 6), (5, 2, 9, 1, 0, 1),
                                                     # the packed forest does not fit shared memory as a whole (one tier at a
                                                     # time: 4 x ~80 KB) / not even one tier does (walk in global memory)
-                                                    (64, 4, 200, 256, 5, 3), (40, 2, 30, 200, 9, 2)])
+                                                    (64, 4, 200, 256, 5, 3), (40, 2, 30, 200, 9, 2),
+                                                    # ... and fits with ~200 KB of dynamic shared memory
+                                                    (90, 6, 50, 256, 4, 2)])
 @pytest.mark.parametrize("upd,tb", [(1, 0), (2, 1)])
 def test_boosted_tpot_head_bit_exact(orc, I, M, B, n_trees, depth, Fa, upd, tb):
     """latency_mode 2 -- per-tier gradient-boosted TPOT head over (running, queued, aux telemetry),
