@@ -95,13 +95,13 @@ typedef struct {
                           /* 2: live gradient-boosted TPOT head (rb_set_tpot_forest) in place of the linear one;   */
                           /* 1: static per-tier prior T^ = decode_ms_per_tok * L^ ("nominal TPOT x predicted       */
                           /* length; zero telemetry", P:L227 arm 4): no wait, batch-slope or prefill term          */
-  int32_t pipeline;       /* 1: consecutive rb_decide calls with DEVICE buffers and at most 128                            */
-                          /* requests overlap -- the bank scan of a call runs on an internal stream (its query staging on */
-                          /* another, beside the scan before it) while the finishing and dispatch stages of the call     */
-                          /* before it run on the context's stream.  Device inputs of                                    */
+  int32_t pipeline;       /* 1: consecutive rb_decide calls with DEVICE buffers overlap -- the bank scan of a call runs on  */
+                          /* an internal stream (its query staging on another, beside the scan before it) while the      */
+                          /* finishing and dispatch stages of the call before it run on the context's stream (above 128  */
+                          /* requests: the dispatch stage only).  Device inputs of                                       */
                           /* rb_decide must then be COMPLETE when the call is made (they are not ordered after earlier   */
                           /* work on the context's stream); outputs stay in stream order.  Results are those of the      */
-                          /* unpipelined calls, bit for bit.                              default 0                      */
+                          /* unpipelined calls, bit for bit.  Three sets of per-decision buffers are kept.  default 0    */
   void* stream;           /* cudaStream_t all work is ordered on; NULL = legacy default stream            */
 } rb_options;
 

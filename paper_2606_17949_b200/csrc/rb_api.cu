@@ -67,13 +67,16 @@ struct rb_ctx {
     int32_t* part_idx = nullptr;
     float *pred_q = nullptr, *pred_l = nullptr, *termA = nullptr, *termP = nullptr, *key = nullptr;
     float* q32 = nullptr;             // fp32 storage: this set's copy of the queries for the exact re-rank
+    uint32_t* gthr = nullptr;         // the pair scan's cross-slab admission thresholds (cleared by the staging kernel)
     cudaEvent_t ev_stage = nullptr;   // staging done, recorded on the staging stream
     cudaEvent_t ev_front = nullptr;   // bank scan done, recorded on the front stream
     cudaEvent_t ev_back = nullptr;    // back half (finish + dispatch) done, recorded on the context's stream
   } slot[kSlots];
   cudaStream_t front = nullptr;       // low-priority internal stream of the bank scans
   cudaStream_t front2 = nullptr;      // second stream of the bank scans (see run_pipelined)
-  cudaStream_t sstage = nullptr;      // internal stream of the staging kernels (they run beside the scan before them)
+  cudaStream_t sstage = nullptr;      // internal stream of the staging kernels
+  cudaEvent_t ev_bigfin = nullptr;    // finishing kernel of the last pipelined decision of more than 128 requests done
+  bool bigfin_pending = false;        // ... and the next scan has not waited for it yet (they run beside the scan before them)
   uint64_t pipe_seq = 0;              // pipelined decisions issued so far (slot = seq % kSlots)
   bool front_busy = false;            // a front half may still be running on the internal stream
   int32_t *order = nullptr, *assignment = nullptr, *max_tokens = nullptr;
@@ -292,20 +295,25 @@ rb_status enqueue_estimate(rb_ctx* ctx, int B, bool with_terms, Timer& tm, int s
     if (B > kTileM && ctx->num_sms >= 2) {
       // tensor-bound regime: CTA pairs, 256-query m-tiles
       const int Bpad2 = (B + 2 * kTileM - 1) / (2 * kTileM) * (2 * kTileM);
-      const int ncl = scan_tc2_clusters(ctx->N, ctx->num_sms);
+      // throughput mode: one cluster's two SMs are left to the dispatch CTA of the decision before
+      const int sms2 = (part != kAll && ctx->num_sms >= 64) ? ctx->num_sms - 2 : ctx->num_sms;
+      const int ncl = scan_tc2_clusters(ctx->N, sms2);
       // lists of at most 32 entries per (cluster, query): 64-entry lists put the sorted insertions (in global memory) on
       // the tensor pipe's time line (k = 32: 0.54 of the tensor roofline), 16-entry ones under k + slack = 40 weaken the
       // pooled admission bound (0.69 against 0.74 with 32, C4 at B = 512 and 4096); a cluster whose list is popped
       // completely is searched again by the finishing kernel, as for the single-CTA scan
       const int kcap2 = std::min(ctx->kcap, 32);
-      if (front) {   // (never split over streams: batches above 128 are not pipelined)
-        CK(launch_stage_queries(ctx->cp_cur, S.qs, B, Bpad2, ctx->d, 1, ctx->gthr, Bpad2 * (1 + ncl), split, S.q32, s));
+      if (do_stage) {
+        CK(launch_stage_queries(ctx->cp_cur, S.qs, B, Bpad2, ctx->d, 1, S.gthr, Bpad2 * (1 + ncl), split, S.q32, s));
         tm.mark();
+        ctx->launches += 1;
+      }
+      if (do_scan) {
         int ncl_used = 0;
-        CK(launch_scan_tc2(&S.tm_q, &ctx->tm_bank, ctx->N, ctx->d_scan, B, Bpad2, kcap2, ctx->kc, ctx->num_sms, S.part_sim,
-                           S.part_idx, ctx->gthr, &ncl_used, s));
+        CK(launch_scan_tc2(&S.tm_q, &ctx->tm_bank, ctx->N, ctx->d_scan, B, Bpad2, kcap2, ctx->kc, sms2, S.part_sim, S.part_idx,
+                           S.gthr, &ncl_used, s));
         tm.mark();
-        ctx->launches += 2;
+        ctx->launches += 1;
       }
       fa.part_sim = S.part_sim; fa.part_idx = S.part_idx; fa.nlists = ncl; fa.lists_per_cta = 1; fa.kcap = kcap2;
       fa.Bpad = Bpad2; fa.slab_unit = kTileN; fa.rescan = kcap2 < ctx->kc ? 1 : 0;
@@ -484,15 +492,31 @@ rb_status run_pipelined(rb_ctx* ctx, int B) {
   if (st != RB_OK) return st;
   CK(cudaEventRecord(S.ev_stage, sstage));
   CK(cudaStreamWaitEvent(fr, S.ev_stage, 0));
+  if (ctx->bigfin_pending) {
+    // the decision before has more than 128 requests: its finishing kernel (one CTA per request) wants the whole GPU, so
+    // this scan starts behind it -- and then runs beside that decision's dispatch CTA
+    CK(cudaStreamWaitEvent(fr, ctx->ev_bigfin, 0));
+    ctx->bigfin_pending = false;
+  }
   st = graph_run(ctx, graph_key(ctx, B, 3, sl), fr,
                  [&]() -> rb_status { return enqueue_estimate(ctx, B, true, tm, sl, kScan, fr); });
   if (st != RB_OK) return st;
   CK(cudaEventRecord(S.ev_front, fr));
   CK(cudaStreamWaitEvent(ctx->stream, S.ev_front, 0));
-  st = graph_run(ctx, graph_key(ctx, B, 4, sl), ctx->stream, [&]() -> rb_status {
-    rb_status s1 = enqueue_estimate(ctx, B, true, tm, sl, kBack, ctx->stream);
-    return s1 != RB_OK ? s1 : enqueue_dispatch(ctx, B, false, tm, sl);
-  });
+  if (B > kTileM) {
+    st = graph_run(ctx, graph_key(ctx, B, 4, sl), ctx->stream,
+                   [&]() -> rb_status { return enqueue_estimate(ctx, B, true, tm, sl, kBack, ctx->stream); });
+    if (st != RB_OK) return st;
+    CK(cudaEventRecord(ctx->ev_bigfin, ctx->stream));
+    ctx->bigfin_pending = true;
+    st = graph_run(ctx, graph_key(ctx, B, 6, sl), ctx->stream,
+                   [&]() -> rb_status { return enqueue_dispatch(ctx, B, false, tm, sl); });
+  } else {
+    st = graph_run(ctx, graph_key(ctx, B, 4, sl), ctx->stream, [&]() -> rb_status {
+      rb_status s1 = enqueue_estimate(ctx, B, true, tm, sl, kBack, ctx->stream);
+      return s1 != RB_OK ? s1 : enqueue_dispatch(ctx, B, false, tm, sl);
+    });
+  }
   if (st != RB_OK) return st;
   CK(cudaEventRecord(S.ev_back, ctx->stream));
   ctx->pipe_seq += 1;
@@ -798,8 +822,8 @@ rb_status rb_create(rb_ctx** out, const void* bank_emb, const float* bank_qualit
                  o_dec = take(kMaxM * 4), o_slope = take(kMaxM * 4), o_deci = take(kMaxI * 4), o_slopei = take(kMaxI * 4),
                  o_aux = take((size_t)kMaxI * kMaxFeatures * 4), o_tpot0 = take(kMaxI * 4), o_mem = take(kMaxI * 4),
                  o_tst = take((kMaxM + 1) * 4), o_cur = take(kMaxM * 4), o_cnt = take(8);
-    // second set of what an estimate hands to its dispatch side (pipelined decisions of at most 128 requests)
-    const size_t m1 = opt.pipeline ? (size_t)kTileM : 0;
+    // further sets of what an estimate hands to its dispatch side (pipelined decisions)
+    const size_t m1 = opt.pipeline ? mb : 0;
     size_t o_pq1[kSlots], o_pl1[kSlots], o_ta1[kSlots], o_tp1[kSlots], o_key1[kSlots];
     for (int j = 1; j < kSlots; ++j) {
       o_pq1[j] = take(m1 * M * 4); o_pl1[j] = take(m1 * M * 4); o_ta1[j] = take(m1 * M * 4); o_tp1[j] = take(m1 * M * 4);
@@ -841,23 +865,24 @@ rb_status rb_create(rb_ctx** out, const void* bank_emb, const float* bank_qualit
     st = encode_map(ctx, &ctx->tm_q, ctx->qs, (uint64_t)ctx->Bpad_max, (uint64_t)ds, kTileM);
     if (st != RB_OK) return st;
     if (opt.pipeline) {
-      // further buffer sets, for batches of at most 128 requests (larger ones are not pipelined)
+      // further buffer sets, sized like the first
       for (int j = 1; j < kSlots; ++j) {
         rb_ctx::Slot& S1 = ctx->slot[j];
-        ALLOC(S1.qs, (size_t)kTileM * ds);
-        const size_t part_n1 = (size_t)ctx->num_sms * ctx->kcap * 4 * kTileM;
-        ALLOC(S1.part_sim, 2 * part_n1);
-        S1.part_idx = reinterpret_cast<int32_t*>(S1.part_sim + part_n1);
-        CK(cudaMemsetAsync(S1.qs, 0, (size_t)kTileM * ds * 2, s));
-        st = encode_map(ctx, &S1.tm_q, S1.qs, (uint64_t)kTileM, (uint64_t)ds, kTileM);
+        ALLOC(S1.qs, (size_t)ctx->Bpad_max * ds);
+        ALLOC(S1.part_sim, 2 * part_n);
+        S1.part_idx = reinterpret_cast<int32_t*>(S1.part_sim + part_n);
+        ALLOC(S1.gthr, (size_t)ctx->Bpad_max * (2 + ctx->num_sms / 2));
+        CK(cudaMemsetAsync(S1.qs, 0, (size_t)ctx->Bpad_max * ds * 2, s));
+        st = encode_map(ctx, &S1.tm_q, S1.qs, (uint64_t)ctx->Bpad_max, (uint64_t)ds, kTileM);
         if (st != RB_OK) return st;
-        ALLOC(S1.q32, (size_t)kTileM * d);
+        ALLOC(S1.q32, mb * d);
       }
       int lo = 0, hi = 0;
       CK(cudaDeviceGetStreamPriorityRange(&lo, &hi));   // lo = least priority
       CK(cudaStreamCreateWithPriority(&ctx->front, cudaStreamNonBlocking, lo));
       CK(cudaStreamCreateWithPriority(&ctx->front2, cudaStreamNonBlocking, lo));
       CK(cudaStreamCreateWithPriority(&ctx->sstage, cudaStreamNonBlocking, hi));
+      CK(cudaEventCreateWithFlags(&ctx->ev_bigfin, cudaEventDisableTiming));
       for (int j = 0; j < kSlots; ++j) {
         CK(cudaEventCreateWithFlags(&ctx->slot[j].ev_stage, cudaEventDisableTiming));
         CK(cudaEventCreateWithFlags(&ctx->slot[j].ev_front, cudaEventDisableTiming));
@@ -885,6 +910,7 @@ rb_status rb_create(rb_ctx** out, const void* bank_emb, const float* bank_qualit
   {
     rb_ctx::Slot& S0 = ctx->slot[0];   // the primary buffer set
     S0.qs = ctx->qs; S0.tm_q = ctx->tm_q; S0.part_sim = ctx->part_sim; S0.part_idx = ctx->part_idx; S0.q32 = ctx->q32;
+    S0.gthr = ctx->gthr;
     S0.pred_q = ctx->pred_q; S0.pred_l = ctx->pred_l; S0.termA = ctx->termA; S0.termP = ctx->termP; S0.key = ctx->key;
   }
   {
@@ -1238,8 +1264,8 @@ rb_status rb_decide_budgeted(rb_ctx* ctx, const float* query_emb, const int32_t*
   } else {
     sg.needs_sync = sg.any_host;
   }
-  // throughput mode: device buffers only (host buffers make the call synchronous anyway), at most one 128-query tile
-  const bool pipelined = ctx->front != nullptr && !sg.any_host && B <= kTileM && adv_folded && !ctx->stage_timing &&
+  // throughput mode: device buffers only (host buffers make the call synchronous anyway)
+  const bool pipelined = ctx->front != nullptr && !sg.any_host && adv_folded && !ctx->stage_timing &&
                          ctx->opt.use_graph != 0;
   if (pipelined) {
     const rb_ctx::Slot& S = ctx->slot[ctx->pipe_seq % kSlots];
@@ -1636,6 +1662,7 @@ void rb_destroy(rb_ctx* ctx) {
     cudaFree(ctx->slot[j].qs);
     cudaFree(ctx->slot[j].part_sim);
     cudaFree(ctx->slot[j].q32);
+    cudaFree(ctx->slot[j].gthr);
   }
   for (auto& sl : ctx->slot) {
     if (sl.ev_stage) cudaEventDestroy(sl.ev_stage);
@@ -1645,6 +1672,7 @@ void rb_destroy(rb_ctx* ctx) {
   if (ctx->front) cudaStreamDestroy(ctx->front);
   if (ctx->front2) cudaStreamDestroy(ctx->front2);
   if (ctx->sstage) cudaStreamDestroy(ctx->sstage);
+  if (ctx->ev_bigfin) cudaEventDestroy(ctx->ev_bigfin);
   for (auto& e : ctx->ev)
     if (e) cudaEventDestroy(e);
   if (ctx->h_zc) cudaFreeHost(ctx->h_zc);

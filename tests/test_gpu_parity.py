@@ -1028,6 +1028,41 @@ def test_adaptive_batch_rule_and_stream_driver_lockstep(orc):
     rt.close()
 
 
+def test_pipelined_decisions_above_128_requests():
+    """Throughput mode with batches on both sides of 128 requests (CTA-pair scan above: its finishing kernel gets the GPU
+    before the next scan starts, the dispatch CTA runs beside that scan): 50 decisions of 60..400 requests give the outputs
+    and the final state of an unpipelined context, bit for bit."""
+    cfg = dataclasses.replace(synth.CONFIGS["C2"], N=40000, d=256, Kc=16, seed=67)
+    bank = synth.make_bank(cfg, device="cuda")
+    it = synth.make_instances(40, cfg.M, cap=6)
+    queued, running = synth.make_state(40, it["cap"], cfg.seed)
+    rng = np.random.default_rng(67)
+    sizes = [int(x) for x in rng.integers(60, 401, 50)]
+    q = synth.make_queries(cfg, B=sum(sizes), device="cuda")
+    p = synth.make_prompt_len(cfg, B=sum(sizes), device="cuda")
+    torch.cuda.synchronize()
+    presets = list(synth.PRESETS.values())
+    outs = []
+    for pipeline in (0, 1):
+        rt = _router(bank, cfg, max_batch=512, pipeline=pipeline)
+        rt.set_instances(**it)
+        rt.set_state(queued, running)
+        rec, off = [], 0
+        for j, B in enumerate(sizes):
+            rt.advance_state(float(3.0 + (j % 7)))
+            o = rt.decide(q[off:off + B], p[off:off + B], presets[j % 4])
+            rec.append({k_: v.clone() for k_, v in o.items()})
+            off += B
+        rt.sync()
+        s = rt.get_state()
+        rec.append({"dq": s[0].clone(), "bq": s[1].clone()})
+        outs.append(rec)
+        rt.close()
+    for a, b in zip(*outs):
+        for key in a:
+            assert torch.equal(a[key].cpu(), b[key].cpu()), key
+
+
 def test_pipelined_decisions_under_fp32_storage():
     """Throughput mode under fp32 storage (the staging kernel leaves the fp32 query rows of every buffer set for the exact
     re-rank): 90 decisions of varying size through rb_decide with device buffers and through rb_decide_submit /
